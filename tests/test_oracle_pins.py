@@ -1,0 +1,501 @@
+"""Pins of the CPU oracle against what the mathematics fixes (no GPU, no CUDA library).
+
+The paper (arxiv 1405.2915) prints no worked example for any skeleton (it names them only,
+PAPER.md L75/L83), so the pins are the ones BASELINE.json L5 names (dot(x_i=i, ones) = n(n-1)/2,
+scan(ones) = indices, stencil(const) = const * sum w) plus: impulse / one-hot shifts (orientation,
+indexing, edge policy), invariants (split, permutation, separable identity, transpose symmetry),
+library special cases (numpy cumsum / correlate, math.fsum) and pure-Python brute force on tiny
+inputs. The golden closed-form values live in tests/golden/closed_forms.txt.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1405_2915_b200 import inputs as I
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")
+BOUNDARY_N = [1, 2, 3, 4, 5, 7, 8, 31, 32, 33, 127, 128, 129, 1023, 1024, 1025]
+
+
+def wrap32(v: int) -> int:
+    v &= 0xFFFFFFFF
+    return v - (1 << 32) if v >= (1 << 31) else v
+
+
+def golden():
+    out = {}
+    with open(GOLD) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                k, v = line.split()
+                out[k] = int(v)
+    return out
+
+
+# ------------------------------------------------------------------ generators (host logic)
+def test_generator_is_stateless_and_in_range():
+    a = I.uniform_pm1_f32(7, 1000)
+    b = I.uniform_pm1_f32(7, 2000)[:1000]
+    assert np.array_equal(a, b)
+    assert a.min() >= -1.0 and a.max() < 1.0 and abs(a.mean()) < 0.1
+    assert not np.array_equal(a, I.uniform_pm1_f32(8, 1000))
+    # streams of neighbouring seeds are not shifted copies of each other
+    c = I.uniform_pm1_f32(8, 1001)
+    assert not np.array_equal(a[1:], c[:999]) and not np.array_equal(a[:999], c[1:1000])
+    v = I.uniform_int_i32(9, 100000, 15)
+    assert v.min() == 0 and v.max() == 15 and abs(v.mean() - 7.5) < 0.1
+    w = I.positive_weights_f32(3, 33)
+    assert (w > 0).all() and abs(w.astype(np.float64).sum() - 1.0) < 33 * 2.0 ** -24
+    p = I.permutation(4, 1000)
+    assert np.array_equal(np.sort(p), np.arange(1000))
+
+
+def test_generator_crosses_chunk_boundary_consistently():
+    n = (1 << 24) + 5
+    a = I.raw_u64(11, n)
+    assert np.array_equal(a[-10:], I.raw_u64(11, 10, start=n - 10))
+
+
+# ------------------------------------------------------------------ Map
+def test_map_saxpy_closed_form_exact():
+    # x_i = i, y = 1, c = 2.5 -> 2.5 i + 1, exactly representable for i < 2^22 (SURVEY (c).1 pins)
+    n = 1 << 16
+    x = np.arange(n, dtype=np.float32)
+    y = np.ones(n, np.float32)
+    out = O.map_f32(O.FN_SAXPY, 2.5, x, y)
+    assert np.array_equal(out, 2.5 * np.arange(n, dtype=np.float64) + 1.0)
+
+
+def test_map_identities_and_constant_rounding():
+    x = I.uniform_pm1_f32(21, 1025)
+    assert np.array_equal(O.map_f32(O.FN_MULT, 1.0, x), x.astype(np.float64))
+    assert np.array_equal(O.map_f32(O.FN_ADD, 0.0, x), x.astype(np.float64))
+    # the constant is rounded to fp32 first (reading (c).1 iii): x * (double)(float)1.0001
+    c32 = float(np.float32(1.0001))
+    assert c32 != 1.0001
+    assert np.array_equal(O.map_f32(O.FN_MULT, 1.0001, x), x.astype(np.float64) * c32)
+
+
+@pytest.mark.parametrize("fn", [O.FN_ADD, O.FN_MULT, O.FN_MAX, O.FN_SAXPY])
+def test_map_brute_force(fn):
+    for n in [0] + BOUNDARY_N[:9]:
+        a = I.uniform_pm1_f32(30 + n, n)
+        b = I.uniform_pm1_f32(31 + n, n)
+        c = float(np.float32(0.3))
+        exp = []
+        for i in range(n):
+            ai, bi = float(a[i]), float(b[i])
+            exp.append({O.FN_ADD: ai + bi, O.FN_MULT: ai * bi, O.FN_MAX: max(ai, bi), O.FN_SAXPY: c * ai + bi}[fn])
+        assert np.array_equal(O.map_f32(fn, 0.3, a, b), np.array(exp, np.float64))
+
+
+def test_map_i32_wraps():
+    a = np.array([2 ** 31 - 1, -2 ** 31, 70000, -5], np.int32)
+    b = np.array([1, -1, 70000, 3], np.int32)
+    assert O.map_i32(O.FN_ADD, 0, a, b).tolist() == [wrap32(int(x) + int(y)) for x, y in zip(a, b)]
+    assert O.map_i32(O.FN_MULT, 0, a, b).tolist() == [wrap32(int(x) * int(y)) for x, y in zip(a, b)]
+    assert O.map_i32(O.FN_MAX, 0, a, b).tolist() == [max(int(x), int(y)) for x, y in zip(a, b)]
+    assert O.map_i32(O.FN_SAXPY, 3, a, b).tolist() == [wrap32(3 * int(x) + int(y)) for x, y in zip(a, b)]
+    assert O.map_i32(O.FN_ADD, 7, a).tolist() == [wrap32(int(x) + 7) for x in a]
+
+
+# ------------------------------------------------------------------ Reduce
+def test_reduce_closed_forms():
+    g = golden()
+    for n in BOUNDARY_N + [1 << 20]:
+        ones = np.ones(n, np.float32)
+        assert O.reduce_f32(O.FN_ADD, ones)[0] == n
+        idx = np.arange(n, dtype=np.int32)
+        r, exact = O.reduce_i32(O.FN_ADD, idx)
+        assert exact == n * (n - 1) // 2 and r == wrap32(n * (n - 1) // 2)
+    n = 1 << 20
+    assert O.reduce_i32(O.FN_ADD, np.arange(n, dtype=np.int32))[1] == g["sum_i_lt_2p20"]
+    # wraps: sum of 2^17 copies of 2^20 = 2^37 = 0 mod 2^32
+    assert O.reduce_i32(O.FN_ADD, np.full(1 << 17, 1 << 20, np.int32)) == (0, 1 << 37)
+    assert g["sum_i_lt_2p17_mod32"] == wrap32((1 << 17) * ((1 << 17) - 1) // 2)
+    assert O.reduce_i32(O.FN_ADD, np.arange(1 << 17, dtype=np.int32))[0] == g["sum_i_lt_2p17_mod32"]
+
+
+def test_reduce_max_of_permutation_wherever_it_sits():
+    n = 4099
+    base = I.permutation(5, n).astype(np.int32)
+    for pos in [0, 1, n // 2, 1023, 1024, n - 2, n - 1]:
+        p = base.copy()
+        j = int(np.argmax(p))
+        p[j], p[pos] = p[pos], p[j]
+        assert O.reduce_i32(O.FN_MAX, p)[0] == n - 1
+        assert O.reduce_f32(O.FN_MAX, p.astype(np.float32))[0] == n - 1
+
+
+def test_reduce_split_and_permutation_invariants():
+    n = 5003
+    v = I.full_range_i32(6, n)
+    total = O.reduce_i32(O.FN_ADD, v)[0]
+    for k in [1, 17, 2500, n - 1]:
+        a = O.reduce_i32(O.FN_ADD, v[:k])[0]
+        b = O.reduce_i32(O.FN_ADD, v[k:])[0]
+        assert wrap32(a + b) == total
+    assert O.reduce_i32(O.FN_ADD, v[I.permutation(7, n)])[0] == total
+    small = (v % 7).astype(np.int32)
+    prod = O.reduce_i32(O.FN_MULT, small)[0]
+    assert O.reduce_i32(O.FN_MULT, small[I.permutation(8, n)])[0] == prod
+    x = I.uniform_pm1_f32(9, n)
+    s, a = O.reduce_f32(O.FN_ADD, x)
+    s1 = O.reduce_f32(O.FN_ADD, x[:1234])[0] + O.reduce_f32(O.FN_ADD, x[1234:])[0]
+    assert abs(s - s1) <= 1e-14 * a
+    assert abs(O.reduce_f32(O.FN_ADD, x[I.permutation(10, n)])[0] - s) <= 1e-14 * a
+
+
+def test_reduce_matches_fsum_and_python_loops():
+    for n in BOUNDARY_N:
+        x = I.uniform_pm1_f32(40 + n, n)
+        s, a = O.reduce_f32(O.FN_ADD, x)
+        exact = math.fsum(float(t) for t in x)
+        assert abs(s - exact) <= 4e-16 * max(a, 1e-300)
+        assert a == pytest.approx(math.fsum(abs(float(t)) for t in x), rel=1e-15)
+        assert O.reduce_f32(O.FN_MAX, x)[0] == max(float(t) for t in x)
+        v = I.full_range_i32(41 + n, n)
+        acc = int(v[0])
+        for t in v[1:]:
+            acc = wrap32(acc + int(t))
+        assert O.reduce_i32(O.FN_ADD, v)[0] == acc
+    with pytest.raises(ValueError):
+        O.reduce_f32(O.FN_ADD, np.zeros(0, np.float32))
+    with pytest.raises(ValueError):
+        O.reduce_i32(O.FN_ADD, np.zeros(0, np.int32))
+
+
+def test_reduce_config2_semantics_overflow_is_wrap():
+    # BJ:L8 inputs uniform{0..1000}: at n = 2^26 the sum exceeds 2^32; check the wrap on a
+    # scaled-down instance whose exact sum is known from the int64 path
+    v = I.uniform_int_i32(I.config_seed(2, 2), 1 << 18, 1000) * 20000
+    r, exact = O.reduce_i32(O.FN_ADD, v)
+    assert exact == int(v.astype(np.int64).sum()) and exact > 2 ** 32 and r == wrap32(exact)
+
+
+# ------------------------------------------------------------------ MapReduce
+def test_dot_closed_form_and_unit_vectors():
+    g = golden()
+    for n in BOUNDARY_N + [1 << 20]:
+        x = np.arange(n, dtype=np.float32)  # exact for n <= 2^24
+        ones = np.ones(n, np.float32)
+        r, a = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, ones)
+        assert r == n * (n - 1) // 2 and a == r
+    assert O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, np.arange(1 << 20, dtype=np.float32), np.ones(1 << 20, np.float32))[0] == g["sum_i_lt_2p20"]
+    x = I.uniform_pm1_f32(50, 777)
+    for j in [0, 5, 776]:
+        e = np.zeros(777, np.float32)
+        e[j] = 1.0
+        assert O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, e)[0] == float(x[j])
+    r, a = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, x)
+    assert r >= 0 and r == pytest.approx(a, rel=1e-15)
+
+
+def test_mapreduce_fusion_invariant_and_brute_force():
+    for n in BOUNDARY_N:
+        x = I.uniform_pm1_f32(60 + n, n)
+        y = I.uniform_pm1_f32(61 + n, n)
+        r, a = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, y)
+        exact = math.fsum(float(p) * float(q) for p, q in zip(x, y))  # products exact in fp64
+        assert abs(r - exact) <= 4e-16 * max(a, 1e-300)
+        # max of sums
+        r2, _ = O.mapreduce_f32(O.FN_ADD, O.FN_MAX, 0.0, x, y)
+        assert r2 == max(float(p) + float(q) for p, q in zip(x, y))
+        # saxpy then add: c*sum x + sum y
+        r3, _ = O.mapreduce_f32(O.FN_SAXPY, O.FN_ADD, 2.5, x, y)
+        assert r3 == pytest.approx(math.fsum(2.5 * float(p) + float(q) for p, q in zip(x, y)), abs=1e-12)
+        a_i = I.full_range_i32(62 + n, n)
+        b_i = I.full_range_i32(63 + n, n)
+        fused = O.mapreduce_i32(O.FN_MULT, O.FN_ADD, 0, a_i, b_i)
+        assert fused == O.reduce_i32(O.FN_ADD, O.map_i32(O.FN_MULT, 0, a_i, b_i))[0]
+        assert fused == wrap32(sum(int(p) * int(q) for p, q in zip(a_i, b_i)))
+
+
+# ------------------------------------------------------------------ Scan
+def test_scan_closed_forms():
+    for n in [0] + BOUNDARY_N + [4096, 4097, 1 << 18]:
+        ones = np.ones(n, np.int32)
+        assert np.array_equal(O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, ones), np.arange(1, n + 1, dtype=np.int32))
+        assert np.array_equal(O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 0, ones), np.arange(0, n, dtype=np.int32))
+    n = 1 << 17  # i(i+1)/2 exceeds 2^32 -> wraps
+    i = np.arange(n, dtype=np.int64)
+    exp = ((i * (i + 1) // 2) & 0xFFFFFFFF).astype(np.uint32).view(np.int32)
+    assert np.array_equal(O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, np.arange(n, dtype=np.int32)), exp)
+
+
+def test_scan_matches_cumsum_and_invariants():
+    for n in BOUNDARY_N + [5000]:
+        x = I.full_range_i32(70 + n, n)
+        inc = O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, x)
+        exc = O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 5, x)
+        lib = np.cumsum(x.astype(np.int64)).astype(np.uint64).astype(np.uint32).view(np.int32)
+        assert np.array_equal(inc, lib)
+        assert exc[0] == 5
+        assert np.array_equal(exc[1:], (inc[:-1].astype(np.int64) + 5).astype(np.uint64).astype(np.uint32).view(np.int32))
+        assert inc[-1] == O.reduce_i32(O.FN_ADD, x)[0]
+        mx = O.scan_i32(O.FN_MAX, O.SCAN_INCLUSIVE, 0, x)
+        assert np.array_equal(mx, np.maximum.accumulate(x))
+        mxe = O.scan_i32(O.FN_MAX, O.SCAN_EXCLUSIVE, -7, x)
+        assert mxe[0] == -7 and np.array_equal(mxe[1:], np.maximum(np.maximum.accumulate(x)[:-1], -7))
+
+
+def test_scan_brute_force_every_small_n():
+    for n in range(0, 70):
+        x = I.uniform_int_i32(80 + n, n, 15)
+        acc, inc, exc = 0, [], []
+        e = 3
+        for t in x:
+            exc.append(e)
+            e = wrap32(e + int(t))
+            acc = wrap32(acc + int(t))
+            inc.append(acc)
+        assert O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, x).tolist() == inc
+        assert O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 3, x).tolist() == exc
+
+
+def test_scan_f32_against_cumsum():
+    x = I.uniform_pm1_f32(90, 3000)
+    out, ab = O.scan_f32(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, x)
+    assert np.allclose(out, np.cumsum(x.astype(np.float64)), rtol=0, atol=1e-12)
+    assert np.allclose(ab, np.cumsum(np.abs(x.astype(np.float64))), rtol=1e-14)
+    oute, _ = O.scan_f32(O.FN_ADD, O.SCAN_EXCLUSIVE, 1.5, x)
+    assert oute[0] == 1.5 and np.allclose(oute[1:], 1.5 + out[:-1], atol=1e-12)
+
+
+# ------------------------------------------------------------------ MapOverlap 1D
+EDGES = [O.EDGE_CONSTANT, O.EDGE_DUPLICATE]
+
+
+@pytest.mark.parametrize("r", [0, 1, 4, 16])
+def test_overlap1d_constant_input_closed_form(r):
+    n, K = 100, 3.0
+    w = I.positive_weights_f32(100 + r, 2 * r + 1)
+    wd = w.astype(np.float64)
+    x = np.full(n, K, np.float32)
+    out, ab = O.mapoverlap_1d(w, r, O.EDGE_DUPLICATE, 0.0, x)
+    seq = 0.0
+    for k in range(2 * r + 1):
+        seq += wd[k] * K
+    assert np.all(out == seq) and abs(seq - K) < 1e-5 and np.array_equal(out, ab)
+    out0, _ = O.mapoverlap_1d(w, r, O.EDGE_CONSTANT, 0.0, x)
+    for i in range(n):
+        exp = K * math.fsum(wd[k + r] for k in range(-r, r + 1) if 0 <= i + k < n)
+        assert out0[i] == pytest.approx(exp, rel=1e-14)
+    # non-zero pad: border cells see the pad value
+    outp, _ = O.mapoverlap_1d(w, r, O.EDGE_CONSTANT, 7.0, x)
+    for i in [0, n - 1]:
+        exp = math.fsum(wd[k + r] * (K if 0 <= i + k < n else 7.0) for k in range(-r, r + 1))
+        assert outp[i] == pytest.approx(exp, rel=1e-14)
+
+
+@pytest.mark.parametrize("edge", EDGES)
+def test_overlap1d_impulse_pins_orientation(edge):
+    # x = e_j -> out[i] = w[(j - i) + r] for |i-j| <= r else 0: correlation, not convolution
+    r, n = 4, 41
+    w = I.signed_weights_f32(110, 2 * r + 1)
+    for j in [0, 1, 3, 20, n - 2, n - 1]:
+        x = np.zeros(n, np.float32)
+        x[j] = 1.0
+        out, _ = O.mapoverlap_1d(w, r, edge, 0.0, x)
+        for i in range(n):
+            exp = float(w[(j - i) + r]) if abs(i - j) <= r else 0.0
+            if edge == O.EDGE_DUPLICATE and j in (0, n - 1):
+                # the impulse sits on the border and is replicated outwards
+                exp = math.fsum(float(w[k + r]) for k in range(-r, r + 1) if min(max(i + k, 0), n - 1) == j)
+            assert out[i] == pytest.approx(exp, abs=1e-15)
+
+
+@pytest.mark.parametrize("edge", EDGES)
+@pytest.mark.parametrize("r", [1, 3, 16])
+def test_overlap1d_one_hot_weights_are_a_shift_bit_exact(edge, r):
+    for n in [1, 2, r, r + 1, 2 * r + 1, 50]:
+        x = I.uniform_pm1_f32(120 + n, n)
+        for m in range(2 * r + 1):
+            w = np.zeros(2 * r + 1, np.float32)
+            w[m] = 1.0
+            out, _ = O.mapoverlap_1d(w, r, edge, 0.25, x)
+            for i in range(n):
+                j = i + m - r
+                if 0 <= j < n:
+                    exp = float(x[j])
+                elif edge == O.EDGE_CONSTANT:
+                    exp = 0.25
+                else:
+                    exp = float(x[min(max(j, 0), n - 1)])
+                assert out[i] == exp
+
+
+def test_overlap1d_identity_linearity_convexity_and_numpy_correlate():
+    x = I.uniform01_f32(130, 500)
+    y = I.uniform01_f32(131, 500)
+    out, _ = O.mapoverlap_1d(np.ones(1, np.float32), 0, O.EDGE_DUPLICATE, 0.0, x)
+    assert np.array_equal(out, x.astype(np.float64))
+    r = 4
+    w = I.positive_weights_f32(132, 2 * r + 1)
+    a, b = 2.0, -0.5  # exactly representable scalings keep the fp32 combination exact
+    ox, _ = O.mapoverlap_1d(w, r, O.EDGE_DUPLICATE, 0.0, x)
+    oy, _ = O.mapoverlap_1d(w, r, O.EDGE_DUPLICATE, 0.0, y)
+    z = (a * x.astype(np.float64) + b * y.astype(np.float64))
+    z32 = z.astype(np.float32)
+    oz, _ = O.mapoverlap_1d(w, r, O.EDGE_DUPLICATE, 0.0, z32)
+    assert np.allclose(oz, a * ox + b * oy, atol=1e-6)
+    assert ox.min() >= x.min() - 1e-6 and ox.max() <= x.max() + 1e-6
+    # library special case: constant-0 edges == numpy.correlate(..., 'same') on zero-padded input
+    lib = np.correlate(x.astype(np.float64), w.astype(np.float64), mode="same")
+    o0, _ = O.mapoverlap_1d(w, r, O.EDGE_CONSTANT, 0.0, x)
+    assert np.allclose(o0, lib, rtol=0, atol=1e-14)
+    # duplicate edges == correlate 'valid' on an edge-padded copy
+    xp = np.pad(x.astype(np.float64), r, mode="edge")
+    assert np.allclose(ox, np.correlate(xp, w.astype(np.float64), mode="valid"), rtol=0, atol=1e-14)
+
+
+@pytest.mark.parametrize("edge", EDGES)
+def test_overlap1d_brute_force_small(edge):
+    for r in [0, 1, 2, 5, 16]:
+        w = I.signed_weights_f32(140 + r, 2 * r + 1)
+        for n in [1, 2, 3, r, r + 1, 2 * r, 2 * r + 1, 2 * r + 2, 70]:
+            if n == 0:
+                continue
+            x = I.uniform_pm1_f32(141 + n, n)
+            out, ab = O.mapoverlap_1d(w, r, edge, -0.5, x)
+            for i in range(n):
+                acc = 0.0
+                aacc = 0.0
+                for k in range(-r, r + 1):
+                    j = i + k
+                    if 0 <= j < n:
+                        v = float(x[j])
+                    elif edge == O.EDGE_CONSTANT:
+                        v = -0.5
+                    else:
+                        v = float(x[min(max(j, 0), n - 1)])
+                    acc += float(w[k + r]) * v
+                    aacc += abs(float(w[k + r]) * v)
+                assert out[i] == acc and ab[i] == aacc
+            # range form agrees with the full call
+            if n > 3:
+                part, _ = O.mapoverlap_1d(w, r, edge, -0.5, x, 1, n - 1)
+                assert np.array_equal(part, out[1:n - 1])
+
+
+@pytest.mark.parametrize("edge", EDGES)
+def test_overlap1d_matrix_axes(edge):
+    rows, cols, r = 13, 17, 3
+    w = I.signed_weights_f32(150, 2 * r + 1)
+    X = I.uniform_pm1_f32(151, rows * cols).reshape(rows, cols)
+    rw, _ = O.mapoverlap_1d_matrix(w, r, edge, 0.5, O.AXIS_ROW, X)
+    for i in range(rows):
+        assert np.array_equal(rw[i], O.mapoverlap_1d(w, r, edge, 0.5, X[i])[0])
+    cw, _ = O.mapoverlap_1d_matrix(w, r, edge, 0.5, O.AXIS_COL, X)
+    # col-wise on X == transpose(row-wise on X^T)
+    assert np.array_equal(cw, O.mapoverlap_1d_matrix(w, r, edge, 0.5, O.AXIS_ROW, np.ascontiguousarray(X.T))[0].T)
+    # 1 x n matrix row-wise == vector call; fp64-input entry == fp32 entry on widened data
+    v = X.reshape(1, -1)
+    assert np.array_equal(O.mapoverlap_1d_matrix(w, r, edge, 0.5, O.AXIS_ROW, v)[0][0], O.mapoverlap_1d(w, r, edge, 0.5, v[0])[0])
+    assert np.array_equal(O.mapoverlap_1d_matrix(w, r, edge, 0.5, O.AXIS_COL, X.astype(np.float64))[0], cw)
+
+
+# ------------------------------------------------------------------ MapOverlap 2D
+@pytest.mark.parametrize("edge", EDGES)
+def test_overlap2d_brute_force_small(edge):
+    for (ry, rx) in [(0, 0), (1, 0), (0, 2), (1, 1), (2, 2), (4, 4), (3, 1)]:
+        W = I.signed_weights_f32(160 + ry * 5 + rx, (2 * ry + 1) * (2 * rx + 1)).reshape(2 * ry + 1, 2 * rx + 1)
+        for (rows, cols) in [(1, 1), (2, 3), (5, 4), (9, 11), (20, 23)]:
+            X = I.uniform_pm1_f32(161 + rows, rows * cols).reshape(rows, cols)
+            out, ab = O.mapoverlap_2d(W, ry, rx, edge, 0.75, X)
+            for i in range(rows):
+                for j in range(cols):
+                    acc = 0.0
+                    for a in range(-ry, ry + 1):
+                        for b in range(-rx, rx + 1):
+                            p, q = i + a, j + b
+                            if 0 <= p < rows and 0 <= q < cols:
+                                v = float(X[p, q])
+                            elif edge == O.EDGE_CONSTANT:
+                                v = 0.75
+                            else:
+                                v = float(X[min(max(p, 0), rows - 1), min(max(q, 0), cols - 1)])
+                            acc += float(W[a + ry, b + rx]) * v
+                    assert out[i, j] == acc
+            if rows > 2:
+                part, _ = O.mapoverlap_2d(W, ry, rx, edge, 0.75, X, 1, rows - 1)
+                assert np.array_equal(part, out[1:rows - 1])
+
+
+def test_overlap2d_constant_impulse_onehot():
+    ry, rx = 2, 2
+    W = I.positive_weights_f32(170, 25).reshape(5, 5)
+    X = np.full((12, 9), 2.0, np.float32)
+    out, _ = O.mapoverlap_2d(W, ry, rx, O.EDGE_DUPLICATE, 0.0, X)
+    assert np.allclose(out, 2.0 * W.astype(np.float64).sum(), rtol=1e-15)
+    Wsg = I.signed_weights_f32(171, 25).reshape(5, 5)
+    X = np.zeros((12, 9), np.float32)
+    X[6, 4] = 1.0
+    out, _ = O.mapoverlap_2d(Wsg, ry, rx, O.EDGE_CONSTANT, 0.0, X)
+    for i in range(12):
+        for j in range(9):
+            exp = float(Wsg[6 - i + ry, 4 - j + rx]) if abs(i - 6) <= ry and abs(j - 4) <= rx else 0.0
+            assert out[i, j] == pytest.approx(exp, abs=1e-15)
+    X = I.uniform_pm1_f32(172, 7 * 6).reshape(7, 6)
+    for edge in EDGES:
+        for a in range(5):
+            for b in range(5):
+                W1 = np.zeros((5, 5), np.float32)
+                W1[a, b] = 1.0
+                out, _ = O.mapoverlap_2d(W1, ry, rx, edge, 0.125, X)
+                for i in range(7):
+                    for j in range(6):
+                        p, q = i + a - ry, j + b - rx
+                        if 0 <= p < 7 and 0 <= q < 6:
+                            exp = float(X[p, q])
+                        elif edge == O.EDGE_CONSTANT:
+                            exp = 0.125
+                        else:
+                            exp = float(X[min(max(p, 0), 6), min(max(q, 0), 5)])
+                        assert out[i, j] == exp
+
+
+@pytest.mark.parametrize("edge", EDGES)
+def test_overlap2d_degenerate_axes_separable_identity_transpose(edge):
+    rows, cols = 19, 21
+    X = I.uniform01_f32(180, rows * cols).reshape(rows, cols)
+    wr = I.positive_weights_f32(181, 7)
+    wc = I.positive_weights_f32(182, 5)
+    # ry = 0 == row-wise 1D; rx = 0 == col-wise 1D
+    assert np.array_equal(O.mapoverlap_2d(wr.reshape(1, 7), 0, 3, edge, 0.0, X)[0], O.mapoverlap_1d_matrix(wr, 3, edge, 0.0, O.AXIS_ROW, X)[0])
+    assert np.array_equal(O.mapoverlap_2d(wc.reshape(5, 1), 2, 0, edge, 0.0, X)[0], O.mapoverlap_1d_matrix(wc, 2, edge, 0.0, O.AXIS_COL, X)[0])
+    # separable identity: row pass then column pass (fp64 intermediate) == dense outer-product
+    # filter; holds for duplicate edges and for constant-0 edges (SURVEY (c).6 pins). The outer
+    # product is rounded to fp32 for the dense call, hence the 1e-6 slack.
+    T, _ = O.mapoverlap_1d_matrix(wr, 3, edge, 0.0, O.AXIS_ROW, X)
+    S, _ = O.mapoverlap_1d_matrix(wc, 2, edge, 0.0, O.AXIS_COL, T)
+    Wd = np.outer(wc.astype(np.float64), wr.astype(np.float64))
+    D, _ = O.mapoverlap_2d(Wd.astype(np.float32), 2, 3, edge, 0.0, X)
+    assert np.allclose(S, D, rtol=0, atol=1e-6)
+    # transpose symmetry
+    W = I.signed_weights_f32(183, 15).reshape(3, 5)
+    A, _ = O.mapoverlap_2d(W, 1, 2, edge, 0.5, X)
+    B, _ = O.mapoverlap_2d(np.ascontiguousarray(W.T), 2, 1, edge, 0.5, np.ascontiguousarray(X.T))
+    assert np.allclose(A, B.T, rtol=0, atol=1e-14)
+
+
+def test_openmp_build_matches_single_thread():
+    x = I.uniform01_f32(190, 10007)
+    w = I.positive_weights_f32(191, 9)
+    X = x[:10000].reshape(100, 100)
+    W = I.positive_weights_f32(192, 25)
+    O.use_openmp(False)
+    a = O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, x)[0]
+    b = O.mapoverlap_2d(W, 2, 2, O.EDGE_DUPLICATE, 0.0, X)[0]
+    c = O.map_f32(O.FN_SAXPY, 2.5, x, x)
+    try:
+        O.use_openmp(True)
+        assert np.array_equal(a, O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, x)[0])
+        assert np.array_equal(b, O.mapoverlap_2d(W, 2, 2, O.EDGE_DUPLICATE, 0.0, X)[0])
+        assert np.array_equal(c, O.map_f32(O.FN_SAXPY, 2.5, x, x))
+    finally:
+        O.use_openmp(False)
