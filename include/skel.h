@@ -1,0 +1,244 @@
+/* skel.h — C ABI of the B200-native data-parallel skeleton library.
+ *
+ * What it is. arxiv 1405.2915 (Kessler, Dastgeer, Li) reviews SkePU, a library of "pre-defined
+ * generic software components derived from higher-order functions such as map, farm, scan and
+ * reduce, which can be parameterized in problem-specific user code" (§III); its
+ * data-parallel skeletons are "map, mapoverlap, scan, reduce, ..." and "all
+ * non-scalar operands of SkePU skeleton calls are passed in smart containers" (§IV,
+ * PAPER.md L111-L123). A *skeleton instance* is "a combination of a skeleton and parameterizing
+ * user function(s)". This header is that model as a C ABI: every skeleton call takes
+ * an enum-selected user function and smart_vector / smart_matrix handles. The paper prints no
+ * formulas; the exact semantics are the readings of DESIGN.md.
+ *
+ * Conventions.
+ *  - Every function returns skel_status (0 = SKEL_OK). Results come back through out-pointers.
+ *  - Handles are opaque, owned by the library, released by the matching *_destroy.
+ *    NULL handles -> SKEL_ERR_INVALID_ARG.
+ *  - skel_last_error(ctx) returns a string owned by the context, valid until the next call on it.
+ *  - A context is used from one host thread at a time.
+ *  - All skeleton calls are ASYNCHRONOUS on the context's CUDA stream (containers
+ *    track dependences so that calls can be asynchronous) and execute in call order. Only the
+ *    forms that return a scalar to a HOST pointer (skel_reduce, skel_mapreduce) and host access
+ *    to a container (*_host_acquire) block.
+ *  - A CUDA failure is sticky: it is returned as SKEL_ERR_CUDA by that call or the next one.
+ *  - There is no CPU fallback: every skeleton runs as hand-written CUDA for sm_100a.
+ *  - "host pointer" / "device pointer" is stated for every plain-pointer argument.
+ */
+#ifndef SKEL_H_
+#define SKEL_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SKEL_ABI_VERSION 1
+
+/* ---- enums (values are ABI) ------------------------------------------------------------- */
+typedef enum {
+  SKEL_OK = 0,
+  SKEL_ERR_INVALID_ARG = 1,   /* NULL handle/pointer, bad enum value, handle of another context */
+  SKEL_ERR_SIZE_MISMATCH = 2, /* operand sizes/shapes differ */
+  SKEL_ERR_DTYPE = 3,         /* operand element types differ, or fn not defined for the dtype */
+  SKEL_ERR_UNSUPPORTED = 4,   /* radius out of range, fn not valid in this position, ... */
+  SKEL_ERR_EMPTY = 5,         /* Reduce / MapReduce of n == 0 (no identity is passed) */
+  SKEL_ERR_ALIAS = 6,         /* out aliases in where that is not allowed (MapOverlap) */
+  SKEL_ERR_UNINIT = 7,        /* reading a container that was never written */
+  SKEL_ERR_OOM = 8,
+  SKEL_ERR_CUDA = 9,
+  SKEL_ERR_BUSY = 10,         /* ctx destroyed with live containers; host access still held */
+  SKEL_ERR_IO = 11            /* plan file could not be read / written / parsed */
+} skel_status;
+
+typedef enum { SKEL_F32 = 0, SKEL_I32 = 1 } skel_dtype;
+
+/* user functions (BASELINE.json L5: "add, mult, max, saxpy, weighted stencil").
+ * Map:      ADD a+b, MULT a*b, MAX max(a,b), SAXPY c*a+b (one fused multiply-add for f32).
+ * Reduce / Scan operator, MapReduce reduce operator: ADD, MULT, MAX only.
+ * WSTENCIL is the user function of MapOverlap (weights passed with the call); it is accepted
+ * nowhere else. */
+typedef enum { SKEL_FN_ADD = 0, SKEL_FN_MULT = 1, SKEL_FN_MAX = 2, SKEL_FN_SAXPY = 3, SKEL_FN_WSTENCIL = 4 } skel_fn;
+
+/* edge policy of MapOverlap: out-of-range neighbours read `pad` (CONSTANT) or the nearest
+ * in-range element, each index clamped independently (DUPLICATE). */
+typedef enum { SKEL_EDGE_CONSTANT = 0, SKEL_EDGE_DUPLICATE = 1 } skel_edge;
+typedef enum { SKEL_SCAN_INCLUSIVE = 0, SKEL_SCAN_EXCLUSIVE = 1 } skel_scan_mode;
+typedef enum { SKEL_AXIS_ROW = 0, SKEL_AXIS_COL = 1 } skel_axis;
+typedef enum { SKEL_READ = 0, SKEL_WRITE = 1, SKEL_READWRITE = 2 } skel_access;
+/* LAZY: the coherence protocol of PAPER.md L121-L123 (valid copies are reused, transfers happen
+ * only when the accessing side has no valid copy). EAGER: the "no smart containers" baseline:
+ * every skeleton call uploads each input that has a valid host copy and downloads each output. */
+typedef enum { SKEL_LAZY = 0, SKEL_EAGER = 1 } skel_coherence;
+
+/* skeleton ids (selector keys, skel_force_variant, skel_last_variant) */
+typedef enum {
+  SKEL_SK_MAP = 0, SKEL_SK_REDUCE = 1, SKEL_SK_MAPREDUCE = 2, SKEL_SK_SCAN = 3,
+  SKEL_SK_OVERLAP1D = 4,      /* vector, and row-wise on a matrix */
+  SKEL_SK_OVERLAP1D_COL = 5,  /* column-wise on a matrix */
+  SKEL_SK_OVERLAP2D = 6,
+  SKEL_SK_COUNT = 7
+} skel_skeleton;
+
+typedef struct skel_ctx skel_ctx;
+typedef struct skel_vector skel_vector;
+typedef struct skel_matrix skel_matrix;
+
+/* ---- context ---------------------------------------------------------------------------- */
+/* Device-memory callbacks (e.g. PyTorch's caching allocator). alloc returns a device pointer
+ * (NULL on failure) usable on `stream`; free releases it. Both NULL -> cudaMalloc / cudaFree. */
+typedef void* (*skel_alloc_fn)(size_t bytes, void* stream, void* user);
+typedef void (*skel_free_fn)(void* dptr, void* user);
+
+/* cuda_stream: a cudaStream_t (NULL = the legacy default stream) owned by the caller; all device
+ * work of the context is enqueued on it. The library owns plans, scratch and statistics. */
+skel_status skel_ctx_create(void* cuda_stream, skel_alloc_fn alloc, skel_free_fn free_, void* user, skel_ctx** out);
+/* Synchronises the stream and frees scratch. Live containers -> SKEL_ERR_BUSY (nothing freed). */
+skel_status skel_ctx_destroy(skel_ctx* ctx);
+skel_status skel_ctx_sync(skel_ctx* ctx);
+skel_status skel_ctx_set_coherence(skel_ctx* ctx, skel_coherence mode);
+const char* skel_last_error(skel_ctx* ctx);
+int skel_abi_version(void);
+
+/* ---- smart containers ------------------------------------------ */
+/* A container owns a pinned host buffer (allocated on first host use) and a device buffer
+ * (allocated on first device use) and tracks which of the two copies is valid.
+ *   create:       contents undefined, state UNINIT.
+ *   create_from:  copies n elements from caller HOST memory `src` at call time; state HOST.
+ *   adopt_device: wraps a caller-owned DEVICE buffer of n elements as the device copy; state
+ *                 DEVICE. The caller keeps it alive and does not touch it while calls are in
+ *                 flight; the library never frees it.
+ * n == 0 is legal. */
+skel_status skel_vector_create(skel_ctx* ctx, skel_dtype dt, size_t n, skel_vector** out);
+skel_status skel_vector_create_from(skel_ctx* ctx, skel_dtype dt, size_t n, const void* src, skel_vector** out);
+skel_status skel_vector_adopt_device(skel_ctx* ctx, skel_dtype dt, size_t n, void* dptr, skel_vector** out);
+skel_status skel_vector_destroy(skel_vector* v);
+skel_status skel_vector_size(const skel_vector* v, size_t* n);
+/* Host access (replaces SkePU's operator-overloaded element access). Blocks until
+ * the device work that the access depends on has finished; READ / READWRITE download the data
+ * if only the device copy is valid. *host_ptr (HOST memory, n elements, library-owned pinned
+ * buffer) stays valid until host_release. WRITE means the caller overwrites ALL elements.
+ * Skeleton calls on a container whose host access is held -> SKEL_ERR_BUSY. */
+skel_status skel_vector_host_acquire(skel_vector* v, skel_access mode, void** host_ptr);
+skel_status skel_vector_host_release(skel_vector* v);
+/* Device pointer of the current device copy for inspection/interop (NULL if none); *valid = 1
+ * if the device copy is valid. No transfer, no state change. */
+skel_status skel_vector_device_ptr(const skel_vector* v, void** dptr, int* valid);
+/* 0 UNINIT, 1 HOST, 2 DEVICE, 3 SHARED (bit 0 = host valid, bit 1 = device valid) */
+skel_status skel_vector_state(const skel_vector* v, int* state);
+
+/* matrices: row-major rows x cols, contiguous (pitch = cols) */
+skel_status skel_matrix_create(skel_ctx* ctx, skel_dtype dt, size_t rows, size_t cols, skel_matrix** out);
+skel_status skel_matrix_create_from(skel_ctx* ctx, skel_dtype dt, size_t rows, size_t cols, const void* src, skel_matrix** out);
+skel_status skel_matrix_adopt_device(skel_ctx* ctx, skel_dtype dt, size_t rows, size_t cols, void* dptr, skel_matrix** out);
+skel_status skel_matrix_destroy(skel_matrix* m);
+skel_status skel_matrix_shape(const skel_matrix* m, size_t* rows, size_t* cols);
+skel_status skel_matrix_host_acquire(skel_matrix* m, skel_access mode, void** host_ptr);
+skel_status skel_matrix_host_release(skel_matrix* m);
+/* A flattened alias (rows*cols elements) sharing storage and coherence state with the matrix;
+ * destroy it like any vector (the storage lives until the last handle is destroyed). */
+skel_status skel_matrix_as_vector(skel_matrix* m, skel_vector** view);
+
+/* ---- skeletons ---------------------------------------------------------------------------- */
+/* `c` is the scalar constant of the user function, converted to the element type on entry
+ * (round-to-nearest to f32; for i32 it must be an integer in int32 range, else INVALID_ARG). */
+
+/* Map: out[i] = f(in0[i], b_i), b_i = in1[i], or the constant c when in1 == NULL.
+ * SAXPY: out[i] = c*in0[i] + in1[i] (in1 required). out may alias in0 and/or in1 (in place). */
+skel_status skel_map(skel_ctx* ctx, skel_fn f, double c, const skel_vector* in0, const skel_vector* in1, skel_vector* out);
+
+/* Reduce: in[0] (+) ... (+) in[n-1], (+) in {ADD, MULT, MAX}; i32 ADD/MULT wrap mod 2^32.
+ * skel_reduce writes one element of the element type to HOST memory `host_result` and blocks.
+ * skel_reduce_to writes it to out[out_index] on the device and does not block. */
+skel_status skel_reduce(skel_ctx* ctx, skel_fn op, const skel_vector* in, void* host_result);
+skel_status skel_reduce_to(skel_ctx* ctx, skel_fn op, const skel_vector* in, skel_vector* out, size_t out_index);
+
+/* MapReduce: (+)_i map_f(in0[i], b_i), fused: the mapped vector is never materialised. */
+skel_status skel_mapreduce(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double c, const skel_vector* in0,
+                           const skel_vector* in1, void* host_result);
+skel_status skel_mapreduce_to(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double c, const skel_vector* in0,
+                              const skel_vector* in1, skel_vector* out, size_t out_index);
+
+/* MapOverlap 1D (f32 only): out[i] = sum_{k=-r..r} w[k+r] * x~[i+k] (correlation: w[0]
+ * multiplies the left-most neighbour). w: HOST pointer to 2r+1 floats, copied at call time.
+ * 0 <= r <= SKEL_MAX_RADIUS_1D. out must not alias in. `pad` is used by SKEL_EDGE_CONSTANT. */
+#define SKEL_MAX_RADIUS_1D 64
+#define SKEL_MAX_RADIUS_2D 8
+skel_status skel_mapoverlap_1d(skel_ctx* ctx, const float* w, int r, skel_edge edge, double pad,
+                               const skel_vector* in, skel_vector* out);
+/* the same along every row (SKEL_AXIS_ROW) or every column (SKEL_AXIS_COL) of a matrix */
+skel_status skel_mapoverlap_1d_matrix(skel_ctx* ctx, const float* w, int r, skel_edge edge, double pad,
+                                      skel_axis axis, const skel_matrix* in, skel_matrix* out);
+/* MapOverlap 2D (f32 only): out[i][j] = sum_a sum_b W[a+ry][b+rx] * X~[i+a][j+b].
+ * W: HOST pointer, (2ry+1)*(2rx+1) floats row-major. 0 <= ry, rx <= SKEL_MAX_RADIUS_2D. */
+skel_status skel_mapoverlap_2d(skel_ctx* ctx, const float* W, int ry, int rx, skel_edge edge, double pad,
+                               const skel_matrix* in, skel_matrix* out);
+
+/* Scan: inclusive out[i] = x[0] (+)...(+) x[i]; exclusive out[0] = init, out[i] = init (+) x[0]
+ * (+)...(+) x[i-1]. (+) in {ADD, MULT, MAX}. `init` is ignored for inclusive. out may alias in. */
+skel_status skel_scan(skel_ctx* ctx, skel_fn op, skel_scan_mode mode, double init, const skel_vector* in, skel_vector* out);
+
+/* ---- variant selector ("execution plan"; L53 off-line tuned dispatch) --------- */
+/* A skeleton instance: the key an execution plan is attached to. Unused fields are 0. */
+typedef struct {
+  int32_t skeleton; /* skel_skeleton */
+  int32_t fn;       /* Map/MapReduce: map function; Reduce/Scan: operator; MapOverlap: WSTENCIL */
+  int32_t fn2;      /* MapReduce: reduce operator */
+  int32_t dtype;    /* skel_dtype */
+  int32_t r0;       /* MapOverlap 1D: r; 2D: ry */
+  int32_t r1;       /* 2D: rx */
+  int32_t edge;     /* skel_edge */
+  int32_t mode;     /* Scan: skel_scan_mode; Map/MapReduce: 1 if in1 is a vector, 0 if it is the constant */
+} skel_instance;
+
+/* Number of kernel variants of a skeleton and the name of one (static string). */
+int skel_variant_count(int skeleton);
+const char* skel_variant_name(int skeleton, int variant);
+/* Measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), median
+ * of `reps` launches timed with CUDA events on the context stream, and store size breakpoints
+ * in the context's plan. For matrix skeletons `cols` gives the row length (rows = n/cols);
+ * pass 0 for vectors. Blocks. */
+skel_status skel_tune_instance(skel_ctx* ctx, const skel_instance* inst, int log2_lo, int log2_hi, size_t cols, int reps);
+skel_status skel_plan_save(skel_ctx* ctx, const char* path);
+skel_status skel_plan_load(skel_ctx* ctx, const char* path);
+skel_status skel_plan_clear(skel_ctx* ctx);
+/* Pure host lookup (no GPU needed): which variant would the plan run for `inst` at n elements?
+ * Alignment- or radius-driven fallbacks are applied at launch time and reported by
+ * skel_last_variant. */
+skel_status skel_plan_lookup(skel_ctx* ctx, const skel_instance* inst, size_t n, int* variant);
+/* Insert one breakpoint by hand: variant `variant` from n >= n_min (until the next breakpoint). */
+skel_status skel_plan_set(skel_ctx* ctx, const skel_instance* inst, size_t n_min, int variant);
+/* Timing table of the last skel_tune_instance: times_us[(k-log2_lo)*nvariants + v], NaN where a
+ * variant is not applicable. Copies at most `capacity` floats; *count = number available. */
+skel_status skel_tune_table(skel_ctx* ctx, float* times_us, size_t capacity, size_t* count);
+/* Force a variant for a skeleton (variant -1 = back to the plan). A forced variant that is not
+ * applicable to a call (dtype, radius, alignment) makes the call fail with UNSUPPORTED. */
+skel_status skel_force_variant(skel_ctx* ctx, int skeleton, int variant);
+skel_status skel_last_variant(skel_ctx* ctx, int* skeleton, int* variant);
+
+/* ---- observability -------------------------------------------------------------------------- */
+typedef struct {
+  uint64_t h2d_bytes, h2d_count;     /* container uploads */
+  uint64_t d2h_bytes, d2h_count;     /* container downloads */
+  uint64_t h2d_elided;               /* device reads served by an already valid device copy */
+  uint64_t d2h_elided;               /* outputs left on the device (EAGER would download them) */
+  uint64_t scalar_d2h_count;         /* Reduce / MapReduce scalars returned to the host */
+  uint64_t launches;                 /* kernels launched by the library */
+} skel_stats;
+skel_status skel_get_stats(skel_ctx* ctx, skel_stats* out);
+skel_status skel_reset_stats(skel_ctx* ctx);
+
+/* The coherence protocol as a pure function (used by the library itself
+ * and exposed so that it can be tested without a GPU).
+ * state: bit 0 host valid, bit 1 device valid. actor: 0 = device (skeleton operand), 1 = host.
+ * mode: LAZY or EAGER. Outputs: *new_state (once the access / the kernel is done); *transfer: bit
+ * mask, 1 = H2D before the kernel, 2 = D2H (host actor: before the access; device actor, EAGER
+ * only: after the kernel). Returns SKEL_ERR_UNINIT when the access would read a container with no
+ * valid copy. */
+skel_status skel_coherence_step(int state, int actor, skel_access access, skel_coherence mode, int* new_state, int* transfer);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SKEL_H_ */

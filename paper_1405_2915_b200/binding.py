@@ -1,0 +1,389 @@
+"""Thin ctypes binding of libskel.so (include/skel.h). Argument marshalling only: every step of
+the skeleton path runs in the library's CUDA kernels. There is no CPU fallback; importing this
+module fails loudly when the library has not been built (``python -m paper_1405_2915_b200.build`` or
+``__graft_entry__.build()``).
+
+The module-level ``skel_*`` functions are the C entry points with their argtypes set. The small
+classes below (Context, Vector, Matrix) only own handles and convert numpy arrays / torch
+tensors to pointers. PyTorch supplies the CUDA stream and the caching allocator, nothing else.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libskel.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: the CUDA library has not been built. Run __graft_entry__.build() "
+        "(nvcc, sm_100a). There is no CPU fallback.")
+lib = C.CDLL(LIB_PATH)
+
+# ---- enums (include/skel.h) --------------------------------------------------------------------
+OK, ERR_INVALID_ARG, ERR_SIZE_MISMATCH, ERR_DTYPE, ERR_UNSUPPORTED, ERR_EMPTY, ERR_ALIAS, ERR_UNINIT, \
+    ERR_OOM, ERR_CUDA, ERR_BUSY, ERR_IO = range(12)
+STATUS_NAMES = ["OK", "INVALID_ARG", "SIZE_MISMATCH", "DTYPE", "UNSUPPORTED", "EMPTY", "ALIAS", "UNINIT", "OOM",
+                "CUDA", "BUSY", "IO"]
+F32, I32 = 0, 1
+FN_ADD, FN_MULT, FN_MAX, FN_SAXPY, FN_WSTENCIL = 0, 1, 2, 3, 4
+EDGE_CONSTANT, EDGE_DUPLICATE = 0, 1
+SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
+AXIS_ROW, AXIS_COL = 0, 1
+READ, WRITE, READWRITE = 0, 1, 2
+LAZY, EAGER = 0, 1
+SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_COUNT = range(8)
+ST_UNINIT, ST_HOST, ST_DEVICE, ST_SHARED = 0, 1, 2, 3
+
+_NP = {F32: np.float32, I32: np.int32}
+
+
+class SkelInstance(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("skeleton", "fn", "fn2", "dtype", "r0", "r1", "edge", "mode")]
+
+
+class SkelStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("h2d_bytes", "h2d_count", "d2h_bytes", "d2h_count", "h2d_elided",
+                                           "d2h_elided", "scalar_d2h_count", "launches")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+_vp, _sz, _i, _d = C.c_void_p, C.c_size_t, C.c_int, C.c_double
+_pp = C.POINTER(C.c_void_p)
+_SIGS = {
+    "skel_abi_version": ([], _i),
+    "skel_ctx_create": ([_vp, ALLOC_FN, FREE_FN, _vp, _pp], _i),
+    "skel_ctx_destroy": ([_vp], _i),
+    "skel_ctx_sync": ([_vp], _i),
+    "skel_ctx_set_coherence": ([_vp, _i], _i),
+    "skel_last_error": ([_vp], C.c_char_p),
+    "skel_vector_create": ([_vp, _i, _sz, _pp], _i),
+    "skel_vector_create_from": ([_vp, _i, _sz, _vp, _pp], _i),
+    "skel_vector_adopt_device": ([_vp, _i, _sz, _vp, _pp], _i),
+    "skel_vector_destroy": ([_vp], _i),
+    "skel_vector_size": ([_vp, C.POINTER(_sz)], _i),
+    "skel_vector_host_acquire": ([_vp, _i, _pp], _i),
+    "skel_vector_host_release": ([_vp], _i),
+    "skel_vector_device_ptr": ([_vp, _pp, C.POINTER(_i)], _i),
+    "skel_vector_state": ([_vp, C.POINTER(_i)], _i),
+    "skel_matrix_create": ([_vp, _i, _sz, _sz, _pp], _i),
+    "skel_matrix_create_from": ([_vp, _i, _sz, _sz, _vp, _pp], _i),
+    "skel_matrix_adopt_device": ([_vp, _i, _sz, _sz, _vp, _pp], _i),
+    "skel_matrix_destroy": ([_vp], _i),
+    "skel_matrix_shape": ([_vp, C.POINTER(_sz), C.POINTER(_sz)], _i),
+    "skel_matrix_host_acquire": ([_vp, _i, _pp], _i),
+    "skel_matrix_host_release": ([_vp], _i),
+    "skel_matrix_as_vector": ([_vp, _pp], _i),
+    "skel_map": ([_vp, _i, _d, _vp, _vp, _vp], _i),
+    "skel_reduce": ([_vp, _i, _vp, _vp], _i),
+    "skel_reduce_to": ([_vp, _i, _vp, _vp, _sz], _i),
+    "skel_mapreduce": ([_vp, _i, _i, _d, _vp, _vp, _vp], _i),
+    "skel_mapreduce_to": ([_vp, _i, _i, _d, _vp, _vp, _vp, _sz], _i),
+    "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
+    "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
+    "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
+    "skel_scan": ([_vp, _i, _i, _d, _vp, _vp], _i),
+    "skel_variant_count": ([_i], _i),
+    "skel_variant_name": ([_i, _i], C.c_char_p),
+    "skel_tune_instance": ([_vp, C.POINTER(SkelInstance), _i, _i, _sz, _i], _i),
+    "skel_plan_save": ([_vp, C.c_char_p], _i),
+    "skel_plan_load": ([_vp, C.c_char_p], _i),
+    "skel_plan_clear": ([_vp], _i),
+    "skel_plan_lookup": ([_vp, C.POINTER(SkelInstance), _sz, C.POINTER(_i)], _i),
+    "skel_plan_set": ([_vp, C.POINTER(SkelInstance), _sz, _i], _i),
+    "skel_tune_table": ([_vp, C.POINTER(C.c_float), _sz, C.POINTER(_sz)], _i),
+    "skel_force_variant": ([_vp, _i, _i], _i),
+    "skel_last_variant": ([_vp, C.POINTER(_i), C.POINTER(_i)], _i),
+    "skel_get_stats": ([_vp, C.POINTER(SkelStats)], _i),
+    "skel_reset_stats": ([_vp], _i),
+    "skel_coherence_step": ([_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)], _i),
+}
+EXPORTS = sorted(_SIGS)
+for _name, (_args, _res) in _SIGS.items():
+    _f = getattr(lib, _name)  # AttributeError here = the library does not export a declared symbol
+    _f.argtypes = _args
+    _f.restype = _res
+    globals()[_name] = _f
+
+
+class SkelError(RuntimeError):
+    def __init__(self, status: int, msg: str = ""):
+        self.status = status
+        name = STATUS_NAMES[status] if 0 <= status < len(STATUS_NAMES) else str(status)
+        super().__init__(f"SKEL_ERR_{name}: {msg}")
+
+
+def coherence_step(state: int, actor: int, access: int, mode: int = LAZY):
+    """Pure protocol function. -> (status, new_state, transfer_mask)."""
+    ns, tr = C.c_int(), C.c_int()
+    st = lib.skel_coherence_step(state, actor, access, mode, C.byref(ns), C.byref(tr))
+    return st, ns.value, tr.value
+
+
+def variant_names(skeleton: int) -> list[str]:
+    return [lib.skel_variant_name(skeleton, v).decode() for v in range(lib.skel_variant_count(skeleton))]
+
+
+class Context:
+    """Owns a skel_ctx. `stream`: an int cudaStream_t (default: torch's current stream).
+    `torch_allocator`: route container device memory through torch's caching allocator."""
+
+    def __init__(self, stream: int | None = None, torch_allocator: bool = True, lazy_cuda: bool = False):
+        self._alloc_cb = ALLOC_FN()
+        self._free_cb = FREE_FN()
+        if stream is None and not lazy_cuda:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        if torch_allocator and not lazy_cuda:
+            import torch
+            dev = torch.cuda.current_device()
+
+            def _alloc(nbytes, strm, _user):
+                try:
+                    return torch.cuda.caching_allocator_alloc(nbytes, dev, strm or 0)
+                except Exception:  # OOM -> NULL, reported as SKEL_ERR_OOM
+                    return None
+
+            def _free(ptr, _user):
+                torch.cuda.caching_allocator_delete(ptr)
+
+            self._alloc_cb = ALLOC_FN(_alloc)
+            self._free_cb = FREE_FN(_free)
+        h = C.c_void_p()
+        st = lib.skel_ctx_create(C.c_void_p(stream or 0), self._alloc_cb, self._free_cb, None, C.byref(h))
+        if st != OK:
+            raise SkelError(st, "skel_ctx_create")
+        self.h = h
+        self.stream = stream or 0
+
+    def check(self, st: int):
+        if st != OK:
+            raise SkelError(st, lib.skel_last_error(self.h).decode())
+
+    def close(self):
+        if self.h:
+            self.check(lib.skel_ctx_destroy(self.h))
+            self.h = None
+
+    def sync(self):
+        self.check(lib.skel_ctx_sync(self.h))
+
+    def set_coherence(self, mode: int):
+        self.check(lib.skel_ctx_set_coherence(self.h, mode))
+
+    def stats(self) -> dict:
+        s = SkelStats()
+        self.check(lib.skel_get_stats(self.h, C.byref(s)))
+        return s.as_dict()
+
+    def reset_stats(self):
+        self.check(lib.skel_reset_stats(self.h))
+
+    def force_variant(self, skeleton: int, variant: int):
+        self.check(lib.skel_force_variant(self.h, skeleton, variant))
+
+    def last_variant(self):
+        a, b = C.c_int(), C.c_int()
+        self.check(lib.skel_last_variant(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    # ---- containers
+    def vector(self, n: int, dtype: int = F32) -> "Vector":
+        h = C.c_void_p()
+        self.check(lib.skel_vector_create(self.h, dtype, n, C.byref(h)))
+        return Vector(self, h, dtype, n)
+
+    def vector_from(self, arr: np.ndarray) -> "Vector":
+        arr = np.ascontiguousarray(arr)
+        dtype = F32 if arr.dtype == np.float32 else I32
+        assert arr.dtype in (np.float32, np.int32)
+        h = C.c_void_p()
+        self.check(lib.skel_vector_create_from(self.h, dtype, arr.size, arr.ctypes.data_as(C.c_void_p), C.byref(h)))
+        return Vector(self, h, dtype, arr.size)
+
+    def vector_adopt(self, tensor) -> "Vector":
+        """Wrap a contiguous 1-D torch CUDA tensor (float32 / int32); keeps a reference to it."""
+        import torch
+        assert tensor.is_cuda and tensor.is_contiguous()
+        dtype = F32 if tensor.dtype == torch.float32 else I32
+        assert tensor.dtype in (torch.float32, torch.int32)
+        h = C.c_void_p()
+        self.check(lib.skel_vector_adopt_device(self.h, dtype, tensor.numel(), C.c_void_p(tensor.data_ptr()), C.byref(h)))
+        v = Vector(self, h, dtype, tensor.numel())
+        v._keep = tensor
+        return v
+
+    def matrix(self, rows: int, cols: int, dtype: int = F32) -> "Matrix":
+        h = C.c_void_p()
+        self.check(lib.skel_matrix_create(self.h, dtype, rows, cols, C.byref(h)))
+        return Matrix(self, h, dtype, rows, cols)
+
+    def matrix_from(self, arr: np.ndarray) -> "Matrix":
+        arr = np.ascontiguousarray(arr)
+        assert arr.ndim == 2 and arr.dtype in (np.float32, np.int32)
+        dtype = F32 if arr.dtype == np.float32 else I32
+        h = C.c_void_p()
+        self.check(lib.skel_matrix_create_from(self.h, dtype, arr.shape[0], arr.shape[1], arr.ctypes.data_as(C.c_void_p), C.byref(h)))
+        return Matrix(self, h, dtype, arr.shape[0], arr.shape[1])
+
+    def matrix_adopt(self, tensor) -> "Matrix":
+        import torch
+        assert tensor.is_cuda and tensor.is_contiguous() and tensor.dim() == 2
+        dtype = F32 if tensor.dtype == torch.float32 else I32
+        h = C.c_void_p()
+        self.check(lib.skel_matrix_adopt_device(self.h, dtype, tensor.shape[0], tensor.shape[1], C.c_void_p(tensor.data_ptr()), C.byref(h)))
+        m = Matrix(self, h, dtype, tensor.shape[0], tensor.shape[1])
+        m._keep = tensor
+        return m
+
+    # ---- skeletons (same names and argument order as the C entry points)
+    def map(self, f: int, c: float, in0: "Vector", in1: "Vector | None", out: "Vector"):
+        self.check(lib.skel_map(self.h, f, c, in0.h, in1.h if in1 is not None else None, out.h))
+
+    def reduce(self, op: int, x: "Vector"):
+        res = (C.c_float if x.dtype == F32 else C.c_int32)()
+        self.check(lib.skel_reduce(self.h, op, x.h, C.byref(res)))
+        return res.value
+
+    def reduce_to(self, op: int, x: "Vector", out: "Vector", out_index: int = 0):
+        self.check(lib.skel_reduce_to(self.h, op, x.h, out.h, out_index))
+
+    def mapreduce(self, map_f: int, red_op: int, c: float, in0: "Vector", in1: "Vector | None"):
+        res = (C.c_float if in0.dtype == F32 else C.c_int32)()
+        self.check(lib.skel_mapreduce(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, C.byref(res)))
+        return res.value
+
+    def mapreduce_to(self, map_f: int, red_op: int, c: float, in0, in1, out: "Vector", out_index: int = 0):
+        self.check(lib.skel_mapreduce_to(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, out.h, out_index))
+
+    def mapoverlap_1d(self, w, r: int, edge: int, pad: float, x: "Vector", out: "Vector"):
+        w = np.ascontiguousarray(w, np.float32)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, x.h, out.h))
+
+    def mapoverlap_1d_matrix(self, w, r: int, edge: int, pad: float, axis: int, x: "Matrix", out: "Matrix"):
+        w = np.ascontiguousarray(w, np.float32)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d_matrix(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, axis, x.h, out.h))
+
+    def mapoverlap_2d(self, W, ry: int, rx: int, edge: int, pad: float, x: "Matrix", out: "Matrix"):
+        W = np.ascontiguousarray(W, np.float32)
+        assert W.size == (2 * ry + 1) * (2 * rx + 1)
+        self.check(lib.skel_mapoverlap_2d(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
+
+    def scan(self, op: int, mode: int, init: float, x: "Vector", out: "Vector"):
+        self.check(lib.skel_scan(self.h, op, mode, init, x.h, out.h))
+
+    # ---- selector
+    def tune(self, inst: SkelInstance, log2_lo: int, log2_hi: int, cols: int = 0, reps: int = 5) -> np.ndarray:
+        """-> timing table [log2 size, variant] in microseconds (NaN = not applicable)."""
+        self.check(lib.skel_tune_instance(self.h, C.byref(inst), log2_lo, log2_hi, cols, reps))
+        cnt = C.c_size_t()
+        self.check(lib.skel_tune_table(self.h, None, 0, C.byref(cnt)))
+        buf = (C.c_float * cnt.value)()
+        self.check(lib.skel_tune_table(self.h, buf, cnt.value, C.byref(cnt)))
+        nv = lib.skel_variant_count(inst.skeleton)
+        return np.array(buf, np.float32).reshape(-1, nv)
+
+    def plan_lookup(self, inst: SkelInstance, n: int) -> int:
+        v = C.c_int()
+        self.check(lib.skel_plan_lookup(self.h, C.byref(inst), n, C.byref(v)))
+        return v.value
+
+    def plan_set(self, inst: SkelInstance, n_min: int, variant: int):
+        self.check(lib.skel_plan_set(self.h, C.byref(inst), n_min, variant))
+
+    def plan_save(self, path: str):
+        self.check(lib.skel_plan_save(self.h, path.encode()))
+
+    def plan_load(self, path: str):
+        self.check(lib.skel_plan_load(self.h, path.encode()))
+
+    def plan_clear(self):
+        self.check(lib.skel_plan_clear(self.h))
+
+
+class _Container:
+    _acquire = _release = _destroy = None
+
+    def __init__(self, ctx: Context, h, dtype: int, shape):
+        self.ctx, self.h, self.dtype, self.shape = ctx, h, dtype, shape
+        self._keep = None
+
+    @property
+    def size(self) -> int:
+        return int(np.prod(self.shape))
+
+    def host_view(self, mode: int) -> np.ndarray:
+        """Acquire host access; returns a numpy view of the library's pinned buffer. Call release()."""
+        p = C.c_void_p()
+        self.ctx.check(self._acquire(self.h, mode, C.byref(p)))
+        if self.size == 0:
+            return np.empty(self.shape, _NP[self.dtype])
+        buf = (C.c_byte * (self.size * 4)).from_address(p.value)
+        return np.frombuffer(buf, dtype=_NP[self.dtype]).reshape(self.shape)
+
+    def release(self):
+        self.ctx.check(self._release(self.h))
+
+    def numpy(self) -> np.ndarray:
+        """Copy of the contents (downloads if only the device copy is valid)."""
+        v = self.host_view(READ)
+        try:
+            return v.copy()
+        finally:
+            self.release()
+
+    def write(self, arr: np.ndarray):
+        v = self.host_view(WRITE)
+        try:
+            v[...] = np.asarray(arr, _NP[self.dtype]).reshape(self.shape)
+        finally:
+            self.release()
+
+    def destroy(self):
+        if self.h:
+            self.ctx.check(self._destroy(self.h))
+            self.h = None
+            self._keep = None
+
+
+class Vector(_Container):
+    _acquire = staticmethod(lib.skel_vector_host_acquire)
+    _release = staticmethod(lib.skel_vector_host_release)
+    _destroy = staticmethod(lib.skel_vector_destroy)
+
+    def __init__(self, ctx, h, dtype, n):
+        super().__init__(ctx, h, dtype, (n,))
+
+    def state(self) -> int:
+        s = C.c_int()
+        self.ctx.check(lib.skel_vector_state(self.h, C.byref(s)))
+        return s.value
+
+    def device_ptr(self):
+        p, valid = C.c_void_p(), C.c_int()
+        self.ctx.check(lib.skel_vector_device_ptr(self.h, C.byref(p), C.byref(valid)))
+        return p.value, bool(valid.value)
+
+
+class Matrix(_Container):
+    _acquire = staticmethod(lib.skel_matrix_host_acquire)
+    _release = staticmethod(lib.skel_matrix_host_release)
+    _destroy = staticmethod(lib.skel_matrix_destroy)
+
+    def __init__(self, ctx, h, dtype, rows, cols):
+        super().__init__(ctx, h, dtype, (rows, cols))
+
+    def as_vector(self) -> Vector:
+        h = C.c_void_p()
+        self.ctx.check(lib.skel_matrix_as_vector(self.h, C.byref(h)))
+        return Vector(self.ctx, h, self.dtype, self.size)

@@ -1,0 +1,1114 @@
+// C ABI of libskel.so (include/skel.h): contexts, smart containers with the coherence protocol,
+// skeleton entry points, variant selection and tuning. Host code only; kernels live in the other
+// translation units (kernels.hpp).
+#include "../../include/skel.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "coherence.hpp"
+#include "kernels.hpp"
+#include "plan.hpp"
+
+using namespace skel;
+
+namespace {
+
+constexpr uint32_t MAGIC_CTX = 0x534b4358, MAGIC_VEC = 0x534b5645, MAGIC_MAT = 0x534b4d41;
+constexpr int FN_IDENT_ = 100;  // same value as skel::FN_IDENT in common.cuh (identity map of plain Reduce)
+
+struct Storage {
+  skel_ctx* ctx;
+  int dtype;
+  size_t n;
+  void* host = nullptr;  // pinned, library owned, allocated on first host use
+  void* dev = nullptr;
+  bool dev_owned = true;
+  int state = ST_UNINIT;
+  bool host_held = false;
+  int refs = 1;
+  uint64_t last_seq = 0;  // ctx->seq of the last enqueued device operation that touched it
+};
+
+struct Handle {
+  uint32_t magic;
+  Storage* st;
+  size_t rows, cols;  // vectors: rows = 1, cols = n
+};
+
+}  // namespace
+
+struct skel_vector : Handle {};
+struct skel_matrix : Handle {};
+
+struct skel_ctx {
+  uint32_t magic = MAGIC_CTX;
+  cudaStream_t stream = nullptr;
+  skel_alloc_fn alloc = nullptr;
+  skel_free_fn free_ = nullptr;
+  void* user = nullptr;
+  int mode = MODE_LAZY;
+  skel_stats stats{};
+  std::string err;
+  int live = 0;
+  bool dev_ready = false;
+  int sms = 148;
+  Scratch scratch{};
+  void* d_result = nullptr;  // device slot for scalars returned to the host
+  void* h_result = nullptr;  // pinned host slot
+  uint64_t seq = 0, synced_seq = 0;
+  bool sticky = false;
+  Plan plan;
+  int forced[SKEL_SK_COUNT];
+  int last_sk = -1, last_var = -1;
+  int launches = 0;
+  std::vector<float> tune_table;
+};
+
+namespace {
+
+skel_status fail(skel_ctx* c, skel_status s, const char* msg) {
+  if (c) c->err = msg;
+  return s;
+}
+
+skel_status cuda_fail(skel_ctx* c, cudaError_t e, const char* where) {
+  c->sticky = true;
+  c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return SKEL_ERR_CUDA;
+}
+
+#define CU(ctx, call)                                      \
+  do {                                                     \
+    cudaError_t e_ = (call);                               \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+bool ctx_ok(const skel_ctx* c) { return c && c->magic == MAGIC_CTX; }
+bool vec_ok(const skel_vector* v) { return v && v->magic == MAGIC_VEC && v->st; }
+bool mat_ok(const skel_matrix* m) { return m && m->magic == MAGIC_MAT && m->st; }
+
+size_t esize(int) { return 4; }
+
+skel_status ensure_device(skel_ctx* c) {
+  if (c->sticky) return SKEL_ERR_CUDA;
+  if (c->dev_ready) return SKEL_OK;
+  int dev = 0;
+  CU(c, cudaGetDevice(&dev));
+  CU(c, cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
+  char* base = nullptr;
+  const size_t partial_bytes = size_t(MAX_PARTIALS) * 8;
+  CU(c, cudaMalloc(reinterpret_cast<void**>(&base), partial_bytes + 256));
+  CU(c, cudaMemsetAsync(base, 0, partial_bytes + 256, c->stream));
+  c->scratch.partials = base;
+  c->scratch.ticket = reinterpret_cast<unsigned*>(base + partial_bytes);
+  c->scratch.scan_ticket = reinterpret_cast<unsigned*>(base + partial_bytes + 64);
+  c->d_result = base + partial_bytes + 128;
+  c->scratch.scan_state = nullptr;
+  c->scratch.scan_state_tiles = 0;
+  c->scratch.scan_epoch = 0;
+  CU(c, cudaHostAlloc(&c->h_result, 64, cudaHostAllocDefault));
+  c->dev_ready = true;
+  return SKEL_OK;
+}
+
+skel_status ensure_scan_state(skel_ctx* c, size_t n) {
+  const size_t need = scan_tiles_needed(n);
+  if (need <= c->scratch.scan_state_tiles) return SKEL_OK;
+  if (c->scratch.scan_state) {
+    CU(c, cudaStreamSynchronize(c->stream));
+    CU(c, cudaFree(c->scratch.scan_state));
+    c->scratch.scan_state = nullptr;
+    c->scratch.scan_state_tiles = 0;
+  }
+  size_t cap = 1024;
+  while (cap < need) cap *= 2;
+  CU(c, cudaMalloc(reinterpret_cast<void**>(&c->scratch.scan_state), cap * 8));
+  CU(c, cudaMemsetAsync(c->scratch.scan_state, 0, cap * 8, c->stream));
+  c->scratch.scan_state_tiles = cap;
+  c->scratch.scan_epoch = 0;
+  return SKEL_OK;
+}
+
+skel_status dev_alloc(skel_ctx* c, size_t bytes, void** out) {
+  *out = nullptr;
+  if (bytes == 0) return SKEL_OK;
+  if (c->alloc) {
+    *out = c->alloc(bytes, c->stream, c->user);
+    if (!*out) return fail(c, SKEL_ERR_OOM, "device allocator callback returned NULL");
+    return SKEL_OK;
+  }
+  cudaError_t e = cudaMalloc(out, bytes);
+  if (e == cudaErrorMemoryAllocation) {
+    cudaGetLastError();
+    return fail(c, SKEL_ERR_OOM, "cudaMalloc: out of memory");
+  }
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaMalloc");
+  return SKEL_OK;
+}
+
+void dev_free(skel_ctx* c, void* p) {
+  if (!p) return;
+  if (c->alloc) {
+    if (c->free_) c->free_(p, c->user);
+  } else {
+    cudaFree(p);
+  }
+}
+
+skel_status ensure_host(skel_ctx* c, Storage* s) {
+  if (s->host || s->n == 0) return SKEL_OK;
+  cudaError_t e = cudaHostAlloc(&s->host, s->n * esize(s->dtype), cudaHostAllocDefault);
+  if (e == cudaErrorMemoryAllocation) {
+    cudaGetLastError();
+    return fail(c, SKEL_ERR_OOM, "cudaHostAlloc: out of memory");
+  }
+  if (e != cudaSuccess) return cuda_fail(c, e, "cudaHostAlloc");
+  return SKEL_OK;
+}
+
+// wait until every enqueued device operation that touched `s` has finished
+skel_status wait_for(skel_ctx* c, Storage* s) {
+  if (s->last_seq > c->synced_seq) {
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->synced_seq = c->seq;
+  }
+  return SKEL_OK;
+}
+
+// ---- containers --------------------------------------------------------------------------------
+template <typename H>
+skel_status make_handle(skel_ctx* c, uint32_t magic, int dt, size_t rows, size_t cols, H** out) {
+  if (!ctx_ok(c) || !out) return fail(ctx_ok(c) ? c : nullptr, SKEL_ERR_INVALID_ARG, "NULL context or out pointer");
+  *out = nullptr;
+  if (dt != SKEL_F32 && dt != SKEL_I32) return fail(c, SKEL_ERR_INVALID_ARG, "unknown dtype");
+  if (cols != 0 && rows > std::numeric_limits<size_t>::max() / 8 / cols)
+    return fail(c, SKEL_ERR_INVALID_ARG, "size overflow");
+  Storage* s = new (std::nothrow) Storage;
+  H* h = new (std::nothrow) H;
+  if (!s || !h) {
+    delete s;
+    delete h;
+    return fail(c, SKEL_ERR_OOM, "host allocation failed");
+  }
+  s->ctx = c;
+  s->dtype = dt;
+  s->n = rows * cols;
+  h->magic = magic;
+  h->st = s;
+  h->rows = rows;
+  h->cols = cols;
+  ++c->live;
+  *out = h;
+  return SKEL_OK;
+}
+
+skel_status release_handle(Handle* h) {
+  Storage* s = h->st;
+  skel_ctx* c = s->ctx;
+  if (s->host_held && s->refs == 1) return fail(c, SKEL_ERR_BUSY, "host access is still held");
+  if (--s->refs == 0) {
+    if (s->last_seq > c->synced_seq && !c->sticky) {
+      cudaStreamSynchronize(c->stream);
+      c->synced_seq = c->seq;
+    }
+    if (s->dev_owned) dev_free(c, s->dev);
+    if (s->host) cudaFreeHost(s->host);
+    delete s;
+  }
+  h->magic = 0;
+  h->st = nullptr;
+  --c->live;
+  return SKEL_OK;
+}
+
+skel_status fill_from(skel_ctx* c, Storage* s, const void* src) {
+  if (s->n == 0) {
+    s->state = ST_HOST;
+    return SKEL_OK;
+  }
+  if (!src) return fail(c, SKEL_ERR_INVALID_ARG, "src is NULL");
+  skel_status st = ensure_device(c);  // pinned allocations need the CUDA context
+  if (st != SKEL_OK) return st;
+  st = ensure_host(c, s);
+  if (st != SKEL_OK) return st;
+  memcpy(s->host, src, s->n * esize(s->dtype));
+  s->state = ST_HOST;
+  return SKEL_OK;
+}
+
+skel_status host_acquire(Handle* h, skel_access mode, void** host_ptr) {
+  Storage* s = h->st;
+  skel_ctx* c = s->ctx;
+  if (!host_ptr) return fail(c, SKEL_ERR_INVALID_ARG, "host_ptr is NULL");
+  if (mode != SKEL_READ && mode != SKEL_WRITE && mode != SKEL_READWRITE)
+    return fail(c, SKEL_ERR_INVALID_ARG, "bad access mode");
+  if (s->host_held) return fail(c, SKEL_ERR_BUSY, "host access already held");
+  const CoherenceStep step = coherence_step(s->state, ACTOR_HOST, mode, c->mode);
+  if (!step.ok) return fail(c, SKEL_ERR_UNINIT, "host read of a container that was never written");
+  skel_status st = SKEL_OK;
+  if (s->n > 0) {
+    st = ensure_device(c);
+    if (st != SKEL_OK) return st;
+    st = ensure_host(c, s);
+    if (st != SKEL_OK) return st;
+    if (step.transfer & XFER_D2H) {
+      CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->stream));
+      c->stats.d2h_bytes += s->n * esize(s->dtype);
+      c->stats.d2h_count += 1;
+      s->last_seq = ++c->seq;
+    }
+    st = wait_for(c, s);
+    if (st != SKEL_OK) return st;
+  }
+  s->state = step.new_state;
+  s->host_held = true;
+  *host_ptr = s->host;
+  return SKEL_OK;
+}
+
+skel_status host_release(Handle* h) {
+  Storage* s = h->st;
+  if (!s->host_held) return fail(s->ctx, SKEL_ERR_INVALID_ARG, "host access is not held");
+  s->host_held = false;
+  return SKEL_OK;
+}
+
+// ---- operand acquisition for a skeleton call -----------------------------------------------------
+struct Operand {
+  Storage* st;
+  int access;
+  CoherenceStep step;
+};
+
+struct OperandSet {
+  Operand ops[4];
+  int count = 0;
+  void add(Storage* s, int access) {
+    for (int i = 0; i < count; ++i)
+      if (ops[i].st == s) {
+        if (ops[i].access != access) ops[i].access = ACC_READWRITE;
+        return;
+      }
+    ops[count++] = Operand{s, access, {}};
+  }
+};
+
+skel_status acquire_all(skel_ctx* c, OperandSet& set) {
+  skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  for (int i = 0; i < set.count; ++i) {  // validate everything before any side effect
+    Operand& o = set.ops[i];
+    if (o.st->ctx != c) return fail(c, SKEL_ERR_INVALID_ARG, "container belongs to another context");
+    if (o.st->host_held) return fail(c, SKEL_ERR_BUSY, "container is held by the host");
+    o.step = coherence_step(o.st->state, ACTOR_DEVICE, o.access, c->mode);
+    if (!o.step.ok) return fail(c, SKEL_ERR_UNINIT, "skeleton input was never written");
+  }
+  for (int i = 0; i < set.count; ++i) {
+    Operand& o = set.ops[i];
+    Storage* s = o.st;
+    if (!s->dev && s->n > 0) {
+      st = dev_alloc(c, s->n * esize(s->dtype), &s->dev);
+      if (st != SKEL_OK) return st;
+    }
+    if ((o.step.transfer & XFER_H2D) && s->n > 0) {
+      CU(c, cudaMemcpyAsync(s->dev, s->host, s->n * esize(s->dtype), cudaMemcpyHostToDevice, c->stream));
+      c->stats.h2d_bytes += s->n * esize(s->dtype);
+      c->stats.h2d_count += 1;
+    } else if (o.access != ACC_WRITE && !(o.step.transfer & XFER_H2D)) {
+      c->stats.h2d_elided += 1;
+    }
+  }
+  return SKEL_OK;
+}
+
+skel_status publish_all(skel_ctx* c, OperandSet& set) {
+  const uint64_t seq = ++c->seq;
+  for (int i = 0; i < set.count; ++i) {
+    Operand& o = set.ops[i];
+    Storage* s = o.st;
+    if (o.step.transfer & XFER_D2H) {  // EAGER: download the output right after the kernel
+      if (s->n > 0) {
+        skel_status st = ensure_host(c, s);
+        if (st != SKEL_OK) return st;
+        CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->stream));
+        c->stats.d2h_bytes += s->n * esize(s->dtype);
+        c->stats.d2h_count += 1;
+      }
+    } else if (o.access != ACC_READ) {
+      c->stats.d2h_elided += 1;
+    }
+    s->state = o.step.new_state;
+    s->last_seq = seq;
+  }
+  c->stats.launches += c->launches;
+  c->launches = 0;
+  return SKEL_OK;
+}
+
+// ---- calls, variants ---------------------------------------------------------------------------
+struct Call {
+  skel_instance inst{};
+  const void* in0 = nullptr;
+  const void* in1 = nullptr;
+  void* out = nullptr;
+  size_t n = 0, rows = 1, cols = 0;
+  uint32_t cbits = 0;  // constant c / scan init, as the element type's bits
+  float pad = 0.f;
+  Weights1D w1;
+  Weights2D w2;
+};
+
+InstanceKey key_of(const skel_instance& i) {
+  InstanceKey k;
+  k.f = {i.skeleton, i.fn, i.fn2, i.dtype, i.r0, i.r1, i.edge, i.mode};
+  return k;
+}
+
+int variant_count(int sk) {
+  switch (sk) {
+    case SKEL_SK_MAP: return map_variant_count();
+    case SKEL_SK_REDUCE:
+    case SKEL_SK_MAPREDUCE: return reduce_variant_count();
+    case SKEL_SK_SCAN: return scan_variant_count();
+    case SKEL_SK_OVERLAP1D: return overlap1d_variant_count();
+    case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_count();
+    case SKEL_SK_OVERLAP2D: return overlap2d_variant_count();
+  }
+  return 0;
+}
+
+const char* variant_name(int sk, int v) {
+  switch (sk) {
+    case SKEL_SK_MAP: return map_variant_name(v);
+    case SKEL_SK_REDUCE:
+    case SKEL_SK_MAPREDUCE: return reduce_variant_name(v);
+    case SKEL_SK_SCAN: return scan_variant_name(v);
+    case SKEL_SK_OVERLAP1D: return overlap1d_variant_name(v);
+    case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_name(v);
+    case SKEL_SK_OVERLAP2D: return overlap2d_variant_name(v);
+  }
+  return nullptr;
+}
+
+bool variant_ok(const Call& k, int v) {
+  switch (k.inst.skeleton) {
+    case SKEL_SK_MAP: return map_variant_ok(v, k.in0, k.in1, k.out, k.n);
+    case SKEL_SK_REDUCE:
+    case SKEL_SK_MAPREDUCE: return reduce_variant_ok(v, k.in0, k.in1, k.n);
+    case SKEL_SK_SCAN: return scan_variant_ok(v, k.inst.dtype, k.in0, k.out, k.n);
+    case SKEL_SK_OVERLAP1D: return overlap1d_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_OVERLAP2D: return overlap2d_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
+  }
+  return false;
+}
+
+// Untuned defaults: preference order per skeleton; the last entry runs every call.
+const int* preference(int sk, int dtype, int* count) {
+  static const int map_p[] = {2, 1, 0};
+  static const int red_p[] = {1, 0};
+  static const int scan_i[] = {0, 4, 5};
+  static const int scan_f[] = {4, 5};
+  static const int o1_p[] = {2, 1, 0};
+  static const int col_p[] = {2, 0};
+  static const int o2_p[] = {1, 0};
+  switch (sk) {
+    case SKEL_SK_MAP: *count = 3; return map_p;
+    case SKEL_SK_REDUCE:
+    case SKEL_SK_MAPREDUCE: *count = 2; return red_p;
+    case SKEL_SK_SCAN:
+      if (dtype == SKEL_I32) { *count = 3; return scan_i; }
+      *count = 2; return scan_f;
+    case SKEL_SK_OVERLAP1D: *count = 3; return o1_p;
+    case SKEL_SK_OVERLAP1D_COL: *count = 2; return col_p;
+    case SKEL_SK_OVERLAP2D: *count = 2; return o2_p;
+  }
+  *count = 0;
+  return nullptr;
+}
+
+skel_status choose_variant(skel_ctx* c, const Call& k, int* chosen) {
+  const int sk = k.inst.skeleton;
+  const int forced = c->forced[sk];
+  if (forced >= 0) {
+    if (forced >= variant_count(sk) || !variant_ok(k, forced))
+      return fail(c, SKEL_ERR_UNSUPPORTED, "forced variant is not applicable to this call");
+    *chosen = forced;
+    return SKEL_OK;
+  }
+  int v = c->plan.lookup(key_of(k.inst), k.n);
+  if (v >= 0 && v < variant_count(sk) && variant_ok(k, v)) {
+    *chosen = v;
+    return SKEL_OK;
+  }
+  int cnt = 0;
+  const int* pref = preference(sk, k.inst.dtype, &cnt);
+  for (int i = 0; i < cnt; ++i)
+    if (variant_ok(k, pref[i])) {
+      *chosen = pref[i];
+      return SKEL_OK;
+    }
+  return fail(c, SKEL_ERR_UNSUPPORTED, "no applicable kernel variant");
+}
+
+cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
+  Launch L{c->stream, c->sms, &c->launches};
+  const skel_instance& i = k.inst;
+  switch (i.skeleton) {
+    case SKEL_SK_MAP:
+      return launch_map(L, v, i.dtype, i.fn, i.mode != 0, k.cbits, k.in0, k.in1, k.out, k.n);
+    case SKEL_SK_REDUCE:
+      return launch_mapreduce(L, c->scratch, v, i.dtype, FN_IDENT_, false, i.fn, 0, k.in0, nullptr, k.n, k.out);
+    case SKEL_SK_MAPREDUCE:
+      return launch_mapreduce(L, c->scratch, v, i.dtype, i.fn, i.mode != 0, i.fn2, k.cbits, k.in0, k.in1, k.n, k.out);
+    case SKEL_SK_SCAN:
+      return launch_scan(L, c->scratch, v, i.dtype, i.fn, i.mode == SKEL_SCAN_EXCLUSIVE, k.cbits, k.in0, k.out, k.n);
+    case SKEL_SK_OVERLAP1D:
+      return launch_overlap1d_rows(L, v, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
+                                   static_cast<float*>(k.out), k.rows, k.cols);
+    case SKEL_SK_OVERLAP1D_COL:
+      return launch_overlap1d_cols(L, v, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
+                                   static_cast<float*>(k.out), k.rows, k.cols);
+    case SKEL_SK_OVERLAP2D:
+      return launch_overlap2d(L, v, k.w2, i.r0, i.r1, i.edge, k.pad, static_cast<const float*>(k.in0),
+                              static_cast<float*>(k.out), k.rows, k.cols);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// choose + launch + bookkeeping
+skel_status run_call(skel_ctx* c, const Call& k) {
+  int v = -1;
+  skel_status st = choose_variant(c, k, &v);
+  if (st != SKEL_OK) return st;
+  if (k.inst.skeleton == SKEL_SK_SCAN) {
+    st = ensure_scan_state(c, k.n);
+    if (st != SKEL_OK) return st;
+  }
+  cudaError_t e = launch_call(c, k, v);
+  if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+  c->last_sk = k.inst.skeleton;
+  c->last_var = v;
+  return SKEL_OK;
+}
+
+bool red_op_ok(int op) { return op == SKEL_FN_ADD || op == SKEL_FN_MULT || op == SKEL_FN_MAX; }
+bool map_fn_ok(int f) { return f == SKEL_FN_ADD || f == SKEL_FN_MULT || f == SKEL_FN_MAX || f == SKEL_FN_SAXPY; }
+
+// convert the scalar constant to the element type's bits
+skel_status const_bits(skel_ctx* c, int dtype, double v, uint32_t* bits) {
+  if (dtype == SKEL_F32) {
+    const float f = static_cast<float>(v);
+    memcpy(bits, &f, 4);
+    return SKEL_OK;
+  }
+  if (!(v >= -2147483648.0 && v <= 2147483647.0) || v != floor(v))
+    return fail(c, SKEL_ERR_INVALID_ARG, "constant is not an int32 value");
+  const int32_t i = static_cast<int32_t>(v);
+  memcpy(bits, &i, 4);
+  return SKEL_OK;
+}
+
+skel_status scalar_to_host(skel_ctx* c, int dtype, void* host_result) {
+  CU(c, cudaMemcpyAsync(c->h_result, c->d_result, esize(dtype), cudaMemcpyDeviceToHost, c->stream));
+  CU(c, cudaStreamSynchronize(c->stream));
+  c->synced_seq = c->seq;
+  memcpy(host_result, c->h_result, esize(dtype));
+  c->stats.scalar_d2h_count += 1;
+  return SKEL_OK;
+}
+
+skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op, double cval, const skel_vector* in0,
+                           const skel_vector* in1, void* host_result, skel_vector* out, size_t out_index) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in0) || (in1 && !vec_ok(in1))) return fail(c, SKEL_ERR_INVALID_ARG, "bad input handle");
+  if (!host_result && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "no result destination");
+  if (!red_op_ok(red_op)) return fail(c, SKEL_ERR_UNSUPPORTED, "reduce operator must be ADD, MULT or MAX");
+  if (!plain_reduce && !map_fn_ok(map_f)) return fail(c, SKEL_ERR_UNSUPPORTED, "map function must be ADD, MULT, MAX or SAXPY");
+  if (!plain_reduce && map_f == SKEL_FN_SAXPY && !in1) return fail(c, SKEL_ERR_INVALID_ARG, "SAXPY needs in1");
+  Storage* a = in0->st;
+  Storage* b = in1 ? in1->st : nullptr;
+  if (b && b->dtype != a->dtype) return fail(c, SKEL_ERR_DTYPE, "operand element types differ");
+  if (b && b->n != a->n) return fail(c, SKEL_ERR_SIZE_MISMATCH, "operand sizes differ");
+  if (out) {
+    if (out->st->dtype != a->dtype) return fail(c, SKEL_ERR_DTYPE, "result element type differs");
+    if (out_index >= out->st->n) return fail(c, SKEL_ERR_INVALID_ARG, "out_index out of range");
+    if (out->st == a || out->st == b) return fail(c, SKEL_ERR_ALIAS, "result vector aliases an input");
+  }
+  if (a->n == 0) return fail(c, SKEL_ERR_EMPTY, "reduce of an empty vector");
+  Call k;
+  k.inst.skeleton = plain_reduce ? SKEL_SK_REDUCE : SKEL_SK_MAPREDUCE;
+  k.inst.fn = plain_reduce ? red_op : map_f;
+  k.inst.fn2 = plain_reduce ? 0 : red_op;
+  k.inst.dtype = a->dtype;
+  k.inst.mode = b ? 1 : 0;
+  skel_status st = SKEL_OK;
+  if (!plain_reduce) {
+    st = const_bits(c, a->dtype, cval, &k.cbits);
+    if (st != SKEL_OK) return st;
+  }
+  OperandSet set;
+  set.add(a, ACC_READ);
+  if (b) set.add(b, ACC_READ);
+  if (out) set.add(out->st, (out->st->n == 1 || out->st->state == ST_UNINIT) ? ACC_WRITE : ACC_READWRITE);
+  st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = a->dev;
+  k.in1 = b ? b->dev : nullptr;
+  k.n = a->n;
+  k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->d_result;
+  st = run_call(c, k);
+  if (st != SKEL_OK) return st;
+  st = publish_all(c, set);
+  if (st != SKEL_OK) return st;
+  if (host_result) return scalar_to_host(c, a->dtype, host_result);
+  return SKEL_OK;
+}
+
+skel_status overlap_check(skel_ctx* c, const Handle* in, const Handle* out, int edge) {
+  if (in->st->dtype != SKEL_F32 || out->st->dtype != SKEL_F32) return fail(c, SKEL_ERR_DTYPE, "MapOverlap is defined for f32 only");
+  if (in->rows != out->rows || in->cols != out->cols) return fail(c, SKEL_ERR_SIZE_MISMATCH, "input and output shapes differ");
+  if (in->st == out->st) return fail(c, SKEL_ERR_ALIAS, "MapOverlap output must not alias its input");
+  if (edge != SKEL_EDGE_CONSTANT && edge != SKEL_EDGE_DUPLICATE) return fail(c, SKEL_ERR_INVALID_ARG, "bad edge policy");
+  return SKEL_OK;
+}
+
+skel_status overlap_run(skel_ctx* c, Call& k, const Handle* in, Handle* out) {
+  OperandSet set;
+  set.add(in->st, ACC_READ);
+  set.add(out->st, ACC_WRITE);
+  skel_status st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = in->st->dev;
+  k.out = out->st->dev;
+  k.n = in->st->n;
+  st = run_call(c, k);
+  if (st != SKEL_OK) return st;
+  return publish_all(c, set);
+}
+
+}  // namespace
+
+// =================================================================================================
+#pragma GCC visibility push(default)
+extern "C" {
+
+int skel_abi_version(void) { return SKEL_ABI_VERSION; }
+
+skel_status skel_ctx_create(void* cuda_stream, skel_alloc_fn alloc, skel_free_fn free_, void* user, skel_ctx** out) {
+  if (!out) return SKEL_ERR_INVALID_ARG;
+  *out = nullptr;
+  if ((alloc == nullptr) != (free_ == nullptr)) return SKEL_ERR_INVALID_ARG;
+  skel_ctx* c = new (std::nothrow) skel_ctx;
+  if (!c) return SKEL_ERR_OOM;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  c->alloc = alloc;
+  c->free_ = free_;
+  c->user = user;
+  for (int i = 0; i < SKEL_SK_COUNT; ++i) c->forced[i] = -1;
+  const char* env = getenv("SKEL_COHERENCE");
+  if (env && strcmp(env, "eager") == 0) c->mode = MODE_EAGER;
+  const char* plan = getenv("SKEL_PLAN_FILE");
+  if (plan && *plan) c->plan.load(plan);
+  *out = c;
+  return SKEL_OK;
+}
+
+skel_status skel_ctx_destroy(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (c->live > 0) return fail(c, SKEL_ERR_BUSY, "containers of this context are still alive");
+  if (c->dev_ready) {
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->scratch.partials);
+    if (c->scratch.scan_state) cudaFree(c->scratch.scan_state);
+    cudaFreeHost(c->h_result);
+  }
+  c->magic = 0;
+  delete c;
+  return SKEL_OK;
+}
+
+skel_status skel_ctx_sync(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (c->sticky) return SKEL_ERR_CUDA;
+  if (!c->dev_ready) return SKEL_OK;
+  CU(c, cudaStreamSynchronize(c->stream));
+  c->synced_seq = c->seq;
+  return SKEL_OK;
+}
+
+skel_status skel_ctx_set_coherence(skel_ctx* c, skel_coherence mode) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (mode != SKEL_LAZY && mode != SKEL_EAGER) return fail(c, SKEL_ERR_INVALID_ARG, "bad coherence mode");
+  c->mode = mode;
+  return SKEL_OK;
+}
+
+const char* skel_last_error(skel_ctx* c) { return ctx_ok(c) ? c->err.c_str() : "invalid context"; }
+
+// ---- vectors ------------------------------------------------------------------------------------
+skel_status skel_vector_create(skel_ctx* c, skel_dtype dt, size_t n, skel_vector** out) {
+  return make_handle<skel_vector>(c, MAGIC_VEC, dt, 1, n, out);
+}
+
+skel_status skel_vector_create_from(skel_ctx* c, skel_dtype dt, size_t n, const void* src, skel_vector** out) {
+  skel_status st = make_handle<skel_vector>(c, MAGIC_VEC, dt, 1, n, out);
+  if (st != SKEL_OK) return st;
+  st = fill_from(c, (*out)->st, src);
+  if (st != SKEL_OK) {
+    release_handle(*out);
+    delete *out;
+    *out = nullptr;
+  }
+  return st;
+}
+
+skel_status skel_vector_adopt_device(skel_ctx* c, skel_dtype dt, size_t n, void* dptr, skel_vector** out) {
+  if (ctx_ok(c) && n > 0 && !dptr) return fail(c, SKEL_ERR_INVALID_ARG, "dptr is NULL");
+  skel_status st = make_handle<skel_vector>(c, MAGIC_VEC, dt, 1, n, out);
+  if (st != SKEL_OK) return st;
+  (*out)->st->dev = dptr;
+  (*out)->st->dev_owned = false;
+  (*out)->st->state = ST_DEVICE;
+  return SKEL_OK;
+}
+
+skel_status skel_vector_destroy(skel_vector* v) {
+  if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
+  skel_status st = release_handle(v);
+  if (st == SKEL_OK) delete v;
+  return st;
+}
+
+skel_status skel_vector_size(const skel_vector* v, size_t* n) {
+  if (!vec_ok(v) || !n) return SKEL_ERR_INVALID_ARG;
+  *n = v->st->n;
+  return SKEL_OK;
+}
+
+skel_status skel_vector_host_acquire(skel_vector* v, skel_access mode, void** host_ptr) {
+  if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
+  return host_acquire(v, mode, host_ptr);
+}
+
+skel_status skel_vector_host_release(skel_vector* v) {
+  if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
+  return host_release(v);
+}
+
+skel_status skel_vector_device_ptr(const skel_vector* v, void** dptr, int* valid) {
+  if (!vec_ok(v) || !dptr) return SKEL_ERR_INVALID_ARG;
+  *dptr = v->st->dev;
+  if (valid) *valid = (v->st->state & 2) ? 1 : 0;
+  return SKEL_OK;
+}
+
+skel_status skel_vector_state(const skel_vector* v, int* state) {
+  if (!vec_ok(v) || !state) return SKEL_ERR_INVALID_ARG;
+  *state = v->st->state;
+  return SKEL_OK;
+}
+
+// ---- matrices -----------------------------------------------------------------------------------
+skel_status skel_matrix_create(skel_ctx* c, skel_dtype dt, size_t rows, size_t cols, skel_matrix** out) {
+  return make_handle<skel_matrix>(c, MAGIC_MAT, dt, rows, cols, out);
+}
+
+skel_status skel_matrix_create_from(skel_ctx* c, skel_dtype dt, size_t rows, size_t cols, const void* src, skel_matrix** out) {
+  skel_status st = make_handle<skel_matrix>(c, MAGIC_MAT, dt, rows, cols, out);
+  if (st != SKEL_OK) return st;
+  st = fill_from(c, (*out)->st, src);
+  if (st != SKEL_OK) {
+    release_handle(*out);
+    delete *out;
+    *out = nullptr;
+  }
+  return st;
+}
+
+skel_status skel_matrix_adopt_device(skel_ctx* c, skel_dtype dt, size_t rows, size_t cols, void* dptr, skel_matrix** out) {
+  if (ctx_ok(c) && rows * cols > 0 && !dptr) return fail(c, SKEL_ERR_INVALID_ARG, "dptr is NULL");
+  skel_status st = make_handle<skel_matrix>(c, MAGIC_MAT, dt, rows, cols, out);
+  if (st != SKEL_OK) return st;
+  (*out)->st->dev = dptr;
+  (*out)->st->dev_owned = false;
+  (*out)->st->state = ST_DEVICE;
+  return SKEL_OK;
+}
+
+skel_status skel_matrix_destroy(skel_matrix* m) {
+  if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
+  skel_status st = release_handle(m);
+  if (st == SKEL_OK) delete m;
+  return st;
+}
+
+skel_status skel_matrix_shape(const skel_matrix* m, size_t* rows, size_t* cols) {
+  if (!mat_ok(m) || !rows || !cols) return SKEL_ERR_INVALID_ARG;
+  *rows = m->rows;
+  *cols = m->cols;
+  return SKEL_OK;
+}
+
+skel_status skel_matrix_host_acquire(skel_matrix* m, skel_access mode, void** host_ptr) {
+  if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
+  return host_acquire(m, mode, host_ptr);
+}
+
+skel_status skel_matrix_host_release(skel_matrix* m) {
+  if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
+  return host_release(m);
+}
+
+skel_status skel_matrix_as_vector(skel_matrix* m, skel_vector** view) {
+  if (!mat_ok(m) || !view) return SKEL_ERR_INVALID_ARG;
+  skel_vector* v = new (std::nothrow) skel_vector;
+  if (!v) return fail(m->st->ctx, SKEL_ERR_OOM, "host allocation failed");
+  v->magic = MAGIC_VEC;
+  v->st = m->st;
+  v->rows = 1;
+  v->cols = m->st->n;
+  ++m->st->refs;
+  ++m->st->ctx->live;
+  *view = v;
+  return SKEL_OK;
+}
+
+// ---- Map ------------------------------------------------------------------------------------------
+skel_status skel_map(skel_ctx* c, skel_fn f, double cval, const skel_vector* in0, const skel_vector* in1, skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in0) || (in1 && !vec_ok(in1)) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad vector handle");
+  if (!map_fn_ok(f)) return fail(c, SKEL_ERR_UNSUPPORTED, "map function must be ADD, MULT, MAX or SAXPY");
+  if (f == SKEL_FN_SAXPY && !in1) return fail(c, SKEL_ERR_INVALID_ARG, "SAXPY needs in1");
+  Storage* a = in0->st;
+  Storage* b = in1 ? in1->st : nullptr;
+  Storage* o = out->st;
+  if ((b && b->dtype != a->dtype) || o->dtype != a->dtype) return fail(c, SKEL_ERR_DTYPE, "operand element types differ");
+  if ((b && b->n != a->n) || o->n != a->n) return fail(c, SKEL_ERR_SIZE_MISMATCH, "operand sizes differ");
+  Call k;
+  k.inst.skeleton = SKEL_SK_MAP;
+  k.inst.fn = f;
+  k.inst.dtype = a->dtype;
+  k.inst.mode = b ? 1 : 0;
+  skel_status st = const_bits(c, a->dtype, cval, &k.cbits);
+  if (st != SKEL_OK) return st;
+  OperandSet set;
+  set.add(a, ACC_READ);
+  if (b) set.add(b, ACC_READ);
+  set.add(o, ACC_WRITE);
+  st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = a->dev;
+  k.in1 = b ? b->dev : nullptr;
+  k.out = o->dev;
+  k.n = a->n;
+  if (k.n > 0) {
+    st = run_call(c, k);
+    if (st != SKEL_OK) return st;
+  }
+  return publish_all(c, set);
+}
+
+// ---- Reduce / MapReduce ---------------------------------------------------------------------------
+skel_status skel_reduce(skel_ctx* c, skel_fn op, const skel_vector* in, void* host_result) {
+  if (ctx_ok(c) && !host_result) return fail(c, SKEL_ERR_INVALID_ARG, "host_result is NULL");
+  return mapreduce_impl(c, true, 0, op, 0.0, in, nullptr, host_result, nullptr, 0);
+}
+
+skel_status skel_reduce_to(skel_ctx* c, skel_fn op, const skel_vector* in, skel_vector* out, size_t out_index) {
+  if (ctx_ok(c) && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad result vector");
+  return mapreduce_impl(c, true, 0, op, 0.0, in, nullptr, nullptr, out, out_index);
+}
+
+skel_status skel_mapreduce(skel_ctx* c, skel_fn map_f, skel_fn red_op, double cval, const skel_vector* in0,
+                           const skel_vector* in1, void* host_result) {
+  if (ctx_ok(c) && !host_result) return fail(c, SKEL_ERR_INVALID_ARG, "host_result is NULL");
+  return mapreduce_impl(c, false, map_f, red_op, cval, in0, in1, host_result, nullptr, 0);
+}
+
+skel_status skel_mapreduce_to(skel_ctx* c, skel_fn map_f, skel_fn red_op, double cval, const skel_vector* in0,
+                              const skel_vector* in1, skel_vector* out, size_t out_index) {
+  if (ctx_ok(c) && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad result vector");
+  return mapreduce_impl(c, false, map_f, red_op, cval, in0, in1, nullptr, out, out_index);
+}
+
+// ---- MapOverlap -----------------------------------------------------------------------------------
+skel_status skel_mapoverlap_1d(skel_ctx* c, const float* w, int r, skel_edge edge, double pad, const skel_vector* in,
+                               skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in) || !vec_ok(out) || !w) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
+  if (r < 0 || r > SKEL_MAX_RADIUS_1D) return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = SKEL_SK_OVERLAP1D;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = SKEL_F32;
+  k.inst.r0 = r;
+  k.inst.edge = edge;
+  k.pad = static_cast<float>(pad);
+  memcpy(k.w1.w, w, sizeof(float) * (2 * r + 1));
+  k.rows = 1;
+  k.cols = in->st->n;
+  return overlap_run(c, k, in, out);
+}
+
+skel_status skel_mapoverlap_1d_matrix(skel_ctx* c, const float* w, int r, skel_edge edge, double pad, skel_axis axis,
+                                      const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out) || !w) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
+  if (axis != SKEL_AXIS_ROW && axis != SKEL_AXIS_COL) return fail(c, SKEL_ERR_INVALID_ARG, "bad axis");
+  if (r < 0 || r > SKEL_MAX_RADIUS_1D) return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = axis == SKEL_AXIS_ROW ? SKEL_SK_OVERLAP1D : SKEL_SK_OVERLAP1D_COL;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = SKEL_F32;
+  k.inst.r0 = r;
+  k.inst.edge = edge;
+  k.pad = static_cast<float>(pad);
+  memcpy(k.w1.w, w, sizeof(float) * (2 * r + 1));
+  k.rows = in->rows;
+  k.cols = in->cols;
+  return overlap_run(c, k, in, out);
+}
+
+skel_status skel_mapoverlap_2d(skel_ctx* c, const float* W, int ry, int rx, skel_edge edge, double pad,
+                               const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out) || !W) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
+  if (ry < 0 || rx < 0 || ry > SKEL_MAX_RADIUS_2D || rx > SKEL_MAX_RADIUS_2D)
+    return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = SKEL_SK_OVERLAP2D;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = SKEL_F32;
+  k.inst.r0 = ry;
+  k.inst.r1 = rx;
+  k.inst.edge = edge;
+  k.pad = static_cast<float>(pad);
+  memcpy(k.w2.w, W, sizeof(float) * (2 * ry + 1) * (2 * rx + 1));
+  k.rows = in->rows;
+  k.cols = in->cols;
+  return overlap_run(c, k, in, out);
+}
+
+// ---- Scan -------------------------------------------------------------------------------------------
+skel_status skel_scan(skel_ctx* c, skel_fn op, skel_scan_mode mode, double init, const skel_vector* in, skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad vector handle");
+  if (!red_op_ok(op)) return fail(c, SKEL_ERR_UNSUPPORTED, "scan operator must be ADD, MULT or MAX");
+  if (mode != SKEL_SCAN_INCLUSIVE && mode != SKEL_SCAN_EXCLUSIVE) return fail(c, SKEL_ERR_INVALID_ARG, "bad scan mode");
+  Storage* a = in->st;
+  Storage* o = out->st;
+  if (a->dtype != o->dtype) return fail(c, SKEL_ERR_DTYPE, "operand element types differ");
+  if (a->n != o->n) return fail(c, SKEL_ERR_SIZE_MISMATCH, "operand sizes differ");
+  Call k;
+  k.inst.skeleton = SKEL_SK_SCAN;
+  k.inst.fn = op;
+  k.inst.dtype = a->dtype;
+  k.inst.mode = mode;
+  skel_status st = const_bits(c, a->dtype, mode == SKEL_SCAN_EXCLUSIVE ? init : 0.0, &k.cbits);
+  if (st != SKEL_OK) return st;
+  OperandSet set;
+  set.add(a, ACC_READ);
+  set.add(o, ACC_WRITE);
+  st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = a->dev;
+  k.out = o->dev;
+  k.n = a->n;
+  if (k.n > 0) {
+    st = run_call(c, k);
+    if (st != SKEL_OK) return st;
+  }
+  return publish_all(c, set);
+}
+
+// ---- selector ---------------------------------------------------------------------------------------
+int skel_variant_count(int skeleton) { return variant_count(skeleton); }
+const char* skel_variant_name(int skeleton, int variant) { return variant_name(skeleton, variant); }
+
+skel_status skel_plan_save(skel_ctx* c, const char* path) {
+  if (!ctx_ok(c) || !path) return SKEL_ERR_INVALID_ARG;
+  return c->plan.save(path) ? SKEL_OK : fail(c, SKEL_ERR_IO, "cannot write plan file");
+}
+
+skel_status skel_plan_load(skel_ctx* c, const char* path) {
+  if (!ctx_ok(c) || !path) return SKEL_ERR_INVALID_ARG;
+  return c->plan.load(path) ? SKEL_OK : fail(c, SKEL_ERR_IO, "cannot read or parse plan file");
+}
+
+skel_status skel_plan_clear(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  c->plan.clear();
+  return SKEL_OK;
+}
+
+skel_status skel_plan_lookup(skel_ctx* c, const skel_instance* inst, size_t n, int* variant) {
+  if (!ctx_ok(c) || !inst || !variant) return SKEL_ERR_INVALID_ARG;
+  if (inst->skeleton < 0 || inst->skeleton >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
+  int v = c->forced[inst->skeleton];
+  if (v < 0) v = c->plan.lookup(key_of(*inst), n);
+  if (v < 0 || v >= variant_count(inst->skeleton)) {
+    int cnt = 0;
+    const int* pref = preference(inst->skeleton, inst->dtype, &cnt);
+    v = cnt > 0 ? pref[0] : -1;
+  }
+  *variant = v;
+  return SKEL_OK;
+}
+
+skel_status skel_plan_set(skel_ctx* c, const skel_instance* inst, size_t n_min, int variant) {
+  if (!ctx_ok(c) || !inst) return SKEL_ERR_INVALID_ARG;
+  if (inst->skeleton < 0 || inst->skeleton >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
+  if (variant < 0 || variant >= variant_count(inst->skeleton)) return fail(c, SKEL_ERR_INVALID_ARG, "bad variant id");
+  c->plan.set(key_of(*inst), n_min, variant);
+  return SKEL_OK;
+}
+
+skel_status skel_force_variant(skel_ctx* c, int skeleton, int variant) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (skeleton < 0 || skeleton >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
+  if (variant < -1 || variant >= variant_count(skeleton)) return fail(c, SKEL_ERR_INVALID_ARG, "bad variant id");
+  c->forced[skeleton] = variant;
+  return SKEL_OK;
+}
+
+skel_status skel_last_variant(skel_ctx* c, int* skeleton, int* variant) {
+  if (!ctx_ok(c) || !skeleton || !variant) return SKEL_ERR_INVALID_ARG;
+  *skeleton = c->last_sk;
+  *variant = c->last_var;
+  return SKEL_OK;
+}
+
+skel_status skel_tune_table(skel_ctx* c, float* times_us, size_t capacity, size_t* count) {
+  if (!ctx_ok(c) || !count) return SKEL_ERR_INVALID_ARG;
+  *count = c->tune_table.size();
+  if (times_us) memcpy(times_us, c->tune_table.data(), sizeof(float) * std::min(capacity, c->tune_table.size()));
+  return SKEL_OK;
+}
+
+skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_lo, int log2_hi, size_t cols, int reps) {
+  if (!ctx_ok(c) || !inst) return SKEL_ERR_INVALID_ARG;
+  const int sk = inst->skeleton;
+  if (sk < 0 || sk >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
+  if (log2_lo < 0 || log2_hi > 32 || log2_lo > log2_hi || reps < 1) return fail(c, SKEL_ERR_INVALID_ARG, "bad tuning range");
+  const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || (sk == SKEL_SK_OVERLAP1D && cols > 0);
+  if (matrix && cols == 0) return fail(c, SKEL_ERR_INVALID_ARG, "matrix skeletons need cols");
+  skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  const size_t nmax = size_t(1) << log2_hi;
+  st = ensure_scan_state(c, nmax);
+  if (st != SKEL_OK) return st;
+  void *b0 = nullptr, *b1 = nullptr, *b2 = nullptr;
+  CU(c, cudaMalloc(&b0, nmax * 4));
+  CU(c, cudaMalloc(&b1, nmax * 4));
+  CU(c, cudaMalloc(&b2, nmax * 4));
+  CU(c, cudaMemsetAsync(b0, 0, nmax * 4, c->stream));
+  CU(c, cudaMemsetAsync(b1, 0, nmax * 4, c->stream));
+  CU(c, cudaMemsetAsync(b2, 0, nmax * 4, c->stream));
+  cudaEvent_t e0, e1;
+  CU(c, cudaEventCreate(&e0));
+  CU(c, cudaEventCreate(&e1));
+  const int nv = variant_count(sk);
+  c->tune_table.assign(size_t(log2_hi - log2_lo + 1) * nv, std::numeric_limits<float>::quiet_NaN());
+  const InstanceKey key = key_of(*inst);
+  c->plan.erase(key);
+  int prev_best = -1;
+  skel_status result = SKEL_OK;
+  std::vector<float> samples(reps);
+  for (int lg = log2_lo; lg <= log2_hi && result == SKEL_OK; ++lg) {
+    Call k;
+    k.inst = *inst;
+    k.n = size_t(1) << lg;
+    k.rows = 1;
+    k.cols = k.n;
+    if (matrix) {
+      if (k.n < cols) continue;
+      k.cols = cols;
+      k.rows = k.n / cols;
+    }
+    k.in0 = b0;
+    k.in1 = (sk == SKEL_SK_MAP || sk == SKEL_SK_MAPREDUCE) && inst->mode ? b1 : nullptr;
+    k.out = (sk == SKEL_SK_REDUCE || sk == SKEL_SK_MAPREDUCE) ? c->d_result : b2;
+    for (int i = 0; i < 129; ++i) k.w1.w[i] = 1.0f / 129.0f;
+    for (int i = 0; i < 17 * 17; ++i) k.w2.w[i] = 1.0f / 289.0f;
+    float best_t = 0.f;
+    int best = -1;
+    for (int v = 0; v < nv; ++v) {
+      if (!variant_ok(k, v)) continue;
+      bool bad = false;
+      for (int rep = -1; rep < reps && !bad; ++rep) {  // rep -1 is the warm-up
+        cudaEventRecord(e0, c->stream);
+        bad = launch_call(c, k, v) != cudaSuccess;
+        cudaEventRecord(e1, c->stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess) bad = true;
+        float ms = 0.f;
+        if (!bad) cudaEventElapsedTime(&ms, e0, e1);
+        if (rep >= 0) samples[rep] = ms * 1000.f;
+      }
+      if (bad) {
+        result = cuda_fail(c, cudaGetLastError(), "tuning launch");
+        break;
+      }
+      std::sort(samples.begin(), samples.end());
+      const float med = samples[reps / 2];
+      c->tune_table[size_t(lg - log2_lo) * nv + v] = med;
+      if (best < 0 || med < best_t) {  // ties -> lower variant id
+        best = v;
+        best_t = med;
+      }
+    }
+    c->stats.launches += c->launches;
+    c->launches = 0;
+    if (best >= 0 && best != prev_best) {
+      c->plan.set(key, prev_best < 0 ? 0 : k.n, best);
+      prev_best = best;
+    }
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(b0);
+  cudaFree(b1);
+  cudaFree(b2);
+  return result;
+}
+
+// ---- observability ------------------------------------------------------------------------------------
+skel_status skel_get_stats(skel_ctx* c, skel_stats* out) {
+  if (!ctx_ok(c) || !out) return SKEL_ERR_INVALID_ARG;
+  *out = c->stats;
+  return SKEL_OK;
+}
+
+skel_status skel_reset_stats(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  c->stats = skel_stats{};
+  return SKEL_OK;
+}
+
+skel_status skel_coherence_step(int state, int actor, skel_access access, skel_coherence mode, int* new_state, int* transfer) {
+  if (state < 0 || state > 3 || (actor != 0 && actor != 1) || access < 0 || access > 2 || (mode != SKEL_LAZY && mode != SKEL_EAGER) ||
+      !new_state || !transfer)
+    return SKEL_ERR_INVALID_ARG;
+  const CoherenceStep s = coherence_step(state, actor, access, mode);
+  *new_state = s.new_state;
+  *transfer = s.transfer;
+  return s.ok ? SKEL_OK : SKEL_ERR_UNINIT;
+}
+
+}  // extern "C"
+#pragma GCC visibility pop

@@ -1,0 +1,124 @@
+// Device-side helpers shared by the skeleton kernels (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <type_traits>
+
+namespace skel {
+
+// user-function ids: same values as skel_fn in include/skel.h
+enum : int { FN_ADD = 0, FN_MULT = 1, FN_MAX = 2, FN_SAXPY = 3, FN_IDENT = 100 };
+
+// ---- streaming 32/128/256-bit global accesses ------------------------------------------------
+// NC = true uses the non-coherent path (only legal when the kernel never writes the buffer, i.e.
+// not for in-place calls). L1::no_allocate: every skeleton input is touched once per call.
+template <int V, bool NC>
+__device__ __forceinline__ void ld_stream(uint32_t (&r)[V], const void* p) {
+  static_assert(V == 1 || V == 2 || V == 4 || V == 8, "vector width");
+  if constexpr (V == 8) {
+    if constexpr (NC)
+      asm volatile("ld.global.nc.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                   : "l"(p));
+    else
+      asm volatile("ld.global.L1::no_allocate.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                   : "l"(p)
+                   : "memory");
+  } else if constexpr (V == 4) {
+    if constexpr (NC)
+      asm volatile("ld.global.nc.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                   : "l"(p));
+    else
+      asm volatile("ld.global.L1::no_allocate.v4.b32 {%0,%1,%2,%3}, [%4];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                   : "l"(p)
+                   : "memory");
+  } else if constexpr (V == 2) {
+    if constexpr (NC)
+      asm volatile("ld.global.nc.L1::no_allocate.v2.b32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "l"(p));
+    else
+      asm volatile("ld.global.L1::no_allocate.v2.b32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "l"(p) : "memory");
+  } else {
+    if constexpr (NC)
+      asm volatile("ld.global.nc.L1::no_allocate.b32 %0, [%1];" : "=r"(r[0]) : "l"(p));
+    else
+      asm volatile("ld.global.L1::no_allocate.b32 %0, [%1];" : "=r"(r[0]) : "l"(p) : "memory");
+  }
+}
+
+template <int V>
+__device__ __forceinline__ void st_stream(void* p, const uint32_t (&r)[V]) {
+  static_assert(V == 1 || V == 2 || V == 4 || V == 8, "vector width");
+  if constexpr (V == 8)
+    asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "r"(r[0]), "r"(r[1]),
+                 "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                 : "memory");
+  else if constexpr (V == 4)
+    asm volatile("st.global.L1::no_allocate.v4.b32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(r[0]), "r"(r[1]), "r"(r[2]),
+                 "r"(r[3])
+                 : "memory");
+  else if constexpr (V == 2)
+    asm volatile("st.global.L1::no_allocate.v2.b32 [%0], {%1,%2};" ::"l"(p), "r"(r[0]), "r"(r[1]) : "memory");
+  else
+    asm volatile("st.global.L1::no_allocate.b32 [%0], %1;" ::"l"(p), "r"(r[0]) : "memory");
+}
+
+// ---- bit casts between the 32-bit register image and the element type ---------------------------
+template <typename T> __device__ __forceinline__ T from_bits(uint32_t b);
+template <> __device__ __forceinline__ float from_bits<float>(uint32_t b) { return __uint_as_float(b); }
+template <> __device__ __forceinline__ int32_t from_bits<int32_t>(uint32_t b) { return static_cast<int32_t>(b); }
+__device__ __forceinline__ uint32_t to_bits(float v) { return __float_as_uint(v); }
+__device__ __forceinline__ uint32_t to_bits(int32_t v) { return static_cast<uint32_t>(v); }
+
+// ---- user functions --------------------------------------------------------------------------
+// f32: add/mult are correctly rounded; saxpy is ONE fused multiply-add (reading 4);
+// i32: two's-complement wrap-around (computed on uint32_t, reading 7).
+template <int FN> __device__ __forceinline__ float apply_fn(float c, float a, float b) {
+  if constexpr (FN == FN_ADD) return __fadd_rn(a, b);
+  else if constexpr (FN == FN_MULT) return __fmul_rn(a, b);
+  else if constexpr (FN == FN_MAX) return a < b ? b : a;
+  else if constexpr (FN == FN_SAXPY) return __fmaf_rn(c, a, b);
+  else return a;  // FN_IDENT
+}
+template <int FN> __device__ __forceinline__ int32_t apply_fn(int32_t c, int32_t a, int32_t b) {
+  if constexpr (FN == FN_ADD) return static_cast<int32_t>(static_cast<uint32_t>(a) + static_cast<uint32_t>(b));
+  else if constexpr (FN == FN_MULT) return static_cast<int32_t>(static_cast<uint32_t>(a) * static_cast<uint32_t>(b));
+  else if constexpr (FN == FN_MAX) return a < b ? b : a;
+  else if constexpr (FN == FN_SAXPY)
+    return static_cast<int32_t>(static_cast<uint32_t>(c) * static_cast<uint32_t>(a) + static_cast<uint32_t>(b));
+  else return a;
+}
+
+// identity element of a reduction operator
+template <typename T, int OP> __device__ __forceinline__ T identity() {
+  if constexpr (OP == FN_ADD) return T(0);
+  else if constexpr (OP == FN_MULT) return T(1);
+  else {
+    if constexpr (std::is_floating_point<T>::value) return T(-INFINITY);
+    else return T(INT32_MIN);
+  }
+}
+
+template <typename T, int OP> __device__ __forceinline__ T warp_reduce(T v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = apply_fn<OP>(T(0), v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// Block-wide reduction; result valid in thread 0. `smem` holds >= 32 elements of T.
+// The combination order is fixed by (blockDim, lane, warp): deterministic run to run.
+template <typename T, int OP> __device__ __forceinline__ T block_reduce(T v, T* smem) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (blockDim.x + 31) >> 5;
+  v = warp_reduce<T, OP>(v);
+  if (lane == 0) smem[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    v = lane < nwarps ? smem[lane] : identity<T, OP>();
+    v = warp_reduce<T, OP>(v);
+  }
+  return v;
+}
+
+}  // namespace skel

@@ -1,0 +1,74 @@
+// Host-side launch interface of the skeleton kernels (internal to libskel.so).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace skel {
+
+enum : int { DT_F32 = 0, DT_I32 = 1 };
+
+struct Launch {
+  cudaStream_t stream;
+  int sms;            // SM count of the device (148 on B200)
+  int* launches;      // incremented once per kernel launch
+};
+
+struct Scratch {       // device scratch owned by the context (see api.cu)
+  void* partials;      // >= MAX_PARTIALS 8-byte slots (reduce partials, scan block sums)
+  unsigned* ticket;    // reduce: atomicInc ticket (self-resetting)
+  unsigned* scan_ticket;        // scan: dynamic tile id counter (reset by the last tile)
+  unsigned long long* scan_state;  // scan: per-tile (epoch|status|value) words, zero-initialised
+  size_t scan_state_tiles;      // capacity of scan_state in tiles
+  uint32_t scan_epoch;          // incremented per look-back launch (host side)
+};
+constexpr int MAX_PARTIALS = 8192;
+
+// ---- Map -------------------------------------------------------------------------------------
+int map_variant_count();
+const char* map_variant_name(int v);
+// whether variant v can run this call (alignment / size constraints)
+bool map_variant_ok(int v, const void* in0, const void* in1, const void* out, size_t n);
+cudaError_t launch_map(const Launch& L, int v, int dtype, int fn, bool has_in1, uint32_t cbits,
+                       const void* in0, const void* in1, void* out, size_t n);
+
+// ---- Reduce / MapReduce (map_fn = FN_IDENT for plain Reduce) --------------------------------------
+int reduce_variant_count();
+const char* reduce_variant_name(int v);
+bool reduce_variant_ok(int v, const void* in0, const void* in1, size_t n);
+cudaError_t launch_mapreduce(const Launch& L, const Scratch& S, int v, int dtype, int map_fn, bool has_in1,
+                             int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n,
+                             void* result /* device, one element */);
+
+// ---- Scan ------------------------------------------------------------------------------------
+int scan_variant_count();
+const char* scan_variant_name(int v);
+bool scan_variant_ok(int v, int dtype, const void* in, const void* out, size_t n);
+cudaError_t launch_scan(const Launch& L, Scratch& S, int v, int dtype, int op, bool exclusive, uint32_t init_bits,
+                        const void* in, void* out, size_t n);
+size_t scan_tiles_needed(size_t n);
+
+// ---- MapOverlap ---------------------------------------------------------------------------------
+struct Weights1D { float w[129]; };   // 2r+1 <= 129 taps, passed by value (constant bank)
+struct Weights2D { float w[17 * 17]; };
+
+int overlap1d_variant_count();
+const char* overlap1d_variant_name(int v);
+bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols);
+// vector: rows = 1. Row-wise on a matrix: every row independently.
+cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+                                  const float* in, float* out, size_t rows, size_t cols);
+
+int overlap1d_col_variant_count();
+const char* overlap1d_col_variant_name(int v);
+bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols);
+cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+                                  const float* in, float* out, size_t rows, size_t cols);
+
+int overlap2d_variant_count();
+const char* overlap2d_variant_name(int v);
+bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols);
+cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
+                             const float* in, float* out, size_t rows, size_t cols);
+
+}  // namespace skel

@@ -1,0 +1,224 @@
+// MapOverlap 1D skeleton on a vector or along the rows of a matrix (PAPER.md L83 names
+// "mapoverlap"; definition: DESIGN.md reading 5):
+//   out[i] = sum_{k=-r..r} w[k+r] * x~[i+k]      (correlation; edge policy constant(pad) | duplicate)
+// Every row of a rows x cols matrix is an independent vector (a plain vector is rows = 1).
+//
+// Variants:
+//  * "direct": any r <= 64, any alignment. One output per thread, coalesced; the 2r+1 neighbour
+//    loads of a warp overlap and are served by L1.
+//  * "tiled_o{4,8,16}": the tile plus a halo is staged once in shared memory with 128-bit loads;
+//    every thread then produces O consecutive outputs from a register window that slides over
+//    128-bit shared-memory reads ((O + 2*ceil4(r))/4 reads per O outputs), weights come from the
+//    constant bank, taps are fully unrolled (r is a template parameter: 1,2,3,4,8,16).
+//    The tile is padded by 4 floats every O floats so that the 128-bit reads of a quarter warp
+//    fall into distinct banks.
+#include "common.cuh"
+#include "kernels.hpp"
+
+namespace skel {
+namespace {
+
+enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1 };
+
+// x~ of one row (reading 5): c may be out of [0, cols)
+__device__ __forceinline__ float ext_row(const float* row, long long cols, long long c, int edge, float pad) {
+  if (c >= 0 && c < cols) return __ldg(row + c);
+  if (edge == EDGE_CONSTANT) return pad;
+  return __ldg(row + (c < 0 ? 0 : cols - 1));
+}
+
+// ---- direct --------------------------------------------------------------------------------
+// Sums are chained in groups of 16 taps so that the rounding-error bound stays below
+// (16 + #groups) * 2^-24 of sum|w x| for every r.
+__global__ void __launch_bounds__(256)
+overlap1d_direct_kernel(const __grid_constant__ Weights1D W, int r, int edge, float pad, const float* in, float* out,
+                        size_t rows, size_t cols) {
+  const size_t total = rows * cols;
+  for (size_t idx = blockIdx.x * size_t(blockDim.x) + threadIdx.x; idx < total; idx += size_t(gridDim.x) * blockDim.x) {
+    const size_t row = idx / cols;
+    const long long j = static_cast<long long>(idx - row * cols);
+    const float* x = in + row * cols;
+    float total_acc = 0.f;
+    const bool interior = (j - r >= 0) && (j + r < static_cast<long long>(cols));
+    for (int k0 = 0; k0 <= 2 * r; k0 += 16) {
+      const int k1 = min(k0 + 16, 2 * r + 1);
+      float acc = 0.f;
+      if (interior) {
+        for (int k = k0; k < k1; ++k) acc = fmaf(W.w[k], __ldg(x + j + k - r), acc);
+      } else {
+        for (int k = k0; k < k1; ++k) acc = fmaf(W.w[k], ext_row(x, (long long)cols, j + k - r, edge, pad), acc);
+      }
+      total_acc = k0 == 0 ? acc : total_acc + acc;
+    }
+    out[idx] = total_acc;
+  }
+}
+
+// ---- shared-memory tiled ---------------------------------------------------------------------
+constexpr int T1_THREADS = 256;
+
+template <int O> __device__ __forceinline__ int phys(int sc) {  // padded smem index of tile coordinate sc
+  if constexpr (O == 4) return sc;
+  else return sc + 4 * (sc / O);
+}
+
+template <int R, int O>
+__global__ void __launch_bounds__(T1_THREADS)
+overlap1d_tiled_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
+                       size_t rows, size_t cols) {
+  constexpr int HP = (R + 3) / 4 * 4;            // halo rounded up to whole 128-bit groups
+  constexpr int TILE = T1_THREADS * O;           // outputs per tile
+  constexpr int SPAN = TILE + 2 * HP;            // staged elements per tile
+  constexpr int NG = (O + 2 * HP) / 4;           // 128-bit groups a thread reads
+  extern __shared__ __align__(16) float sm[];
+
+  const size_t tiles_per_row = (cols + TILE - 1) / TILE;
+  const size_t ntiles = rows * tiles_per_row;
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t row = tile / tiles_per_row;
+    const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE);  // first output column
+    const float* x = in + row * cols;
+    // stage x~[c0 - HP, c0 + TILE + HP) at tile coordinates sc = 0 .. SPAN-1
+    for (int g = threadIdx.x; g < SPAN / 4; g += T1_THREADS) {
+      const long long c = c0 - HP + 4 * g;
+      float4 v;
+      if (c >= 0 && c + 3 < static_cast<long long>(cols)) {
+        uint32_t raw[4];
+        ld_stream<4, true>(raw, x + c);
+        v = make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
+      } else {
+        v.x = ext_row(x, (long long)cols, c, edge, pad);
+        v.y = ext_row(x, (long long)cols, c + 1, edge, pad);
+        v.z = ext_row(x, (long long)cols, c + 2, edge, pad);
+        v.w = ext_row(x, (long long)cols, c + 3, edge, pad);
+      }
+      *reinterpret_cast<float4*>(sm + phys<O>(4 * g)) = v;
+    }
+    __syncthreads();
+
+    // thread t produces outputs c0 + t*O .. + O-1 from tile coordinates t*O .. t*O + O + 2HP - 1
+    float acc[O];
+#pragma unroll
+    for (int o = 0; o < O; ++o) acc[o] = 0.f;
+    const int sc0 = threadIdx.x * O;
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+      const float4 v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
+      const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
+        // tap k = p - HP - o + R, 0 <= k <= 2R
+#pragma unroll
+        for (int o = 0; o < O; ++o) {
+          const int k = 4 * g + e - HP - o + R;
+          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+        }
+      }
+    }
+    const long long cbase = c0 + sc0;
+    if (cbase + O <= static_cast<long long>(cols)) {
+      float* dst = out + row * cols + cbase;
+      if constexpr (O % 8 == 0) {
+#pragma unroll
+        for (int q = 0; q < O / 8; ++q) {
+          uint32_t raw[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) raw[e] = __float_as_uint(acc[8 * q + e]);
+          st_stream<8>(dst + 8 * q, raw);
+        }
+      } else {
+#pragma unroll
+        for (int q = 0; q < O / 4; ++q) {
+          uint32_t raw[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) raw[e] = __float_as_uint(acc[4 * q + e]);
+          st_stream<4>(dst + 4 * q, raw);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int o = 0; o < O; ++o)
+        if (cbase + o < static_cast<long long>(cols)) out[row * cols + cbase + o] = acc[o];
+    }
+    __syncthreads();  // the tile buffer is reused
+  }
+}
+
+template <int O> constexpr size_t tiled_smem_bytes(int R) {
+  const int HP = (R + 3) / 4 * 4;
+  const int span = T1_THREADS * O + 2 * HP;
+  return size_t(O == 4 ? span : span + 4 * (span / O) + 4) * sizeof(float);
+}
+
+struct O1Variant { const char* name; int o; };  // o == 0: direct
+const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}};
+constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
+
+inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
+
+template <int R, int O>
+cudaError_t launch_tiled(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
+                         size_t rows, size_t cols) {
+  constexpr int TILE = T1_THREADS * O;
+  const size_t smem = tiled_smem_bytes<O>(R);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(overlap1d_tiled_kernel<R, O>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_done = true;
+  }
+  const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
+  size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
+  overlap1d_tiled_kernel<R, O><<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <int O>
+cudaError_t launch_tiled_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in,
+                           float* out, size_t rows, size_t cols) {
+  switch (r) {
+    case 1: return launch_tiled<1, O>(L, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_tiled<2, O>(L, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_tiled<3, O>(L, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_tiled<4, O>(L, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_tiled<8, O>(L, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_tiled<16, O>(L, w, edge, pad, in, out, rows, cols);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+int overlap1d_variant_count() { return kNumVariants; }
+const char* overlap1d_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kVariants[v].name : nullptr; }
+
+bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
+  if (v < 0 || v >= kNumVariants) return false;
+  if (kVariants[v].o == 0) return true;
+  if (!templated_radius(r)) return false;
+  const bool al = reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
+  return al && (rows == 1 || cols % 8 == 0);
+}
+
+cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+                                  const float* in, float* out, size_t rows, size_t cols) {
+  if (rows * cols == 0) return cudaSuccess;
+  switch (kVariants[v].o) {
+    case 0: {
+      const size_t total = rows * cols;
+      size_t grid = (total + 255) / 256;
+      const size_t cap = size_t(L.sms) * 64;
+      if (grid > cap) grid = cap;
+      overlap1d_direct_kernel<<<(unsigned)grid, 256, 0, L.stream>>>(w, r, edge, pad, in, out, rows, cols);
+      ++*L.launches;
+      return cudaGetLastError();
+    }
+    case 4: return launch_tiled_r<4>(L, w, r, edge, pad, in, out, rows, cols);
+    case 8: return launch_tiled_r<8>(L, w, r, edge, pad, in, out, rows, cols);
+    case 16: return launch_tiled_r<16>(L, w, r, edge, pad, in, out, rows, cols);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace skel

@@ -1,0 +1,271 @@
+// MapOverlap 2D skeleton and the column-wise 1D form on a matrix (readings 5 and 6):
+//   out[i][j] = sum_{a=-ry..ry} sum_{b=-rx..rx} W[a+ry][b+rx] * X~[i+a][j+b]
+// X~ = pad (CONSTANT) or X[clamp i][clamp j] (DUPLICATE, every index clamped on its own).
+// Column-wise 1D is the rx = 0 case (a (2r+1) x 1 filter).
+//
+// Variants:
+//  * "direct": any radii, any alignment; one output per thread, neighbours served by L1/L2.
+//  * "tiled_oy{4,8}": a (8*OY + 2ry) x (128 + 2*ceil4(rx)) tile is staged in shared memory with
+//    128-bit loads; a thread produces a 4 (x) by OY (y) block of outputs. Each staged row it reads
+//    (one or a few 128-bit shared loads) is reused for up to 2ry+1 output rows from registers;
+//    weights come from the constant bank; all taps are unrolled (radii are template parameters).
+// Summation order: a outer, b inner, like the definition. When a filter has more than 33 taps,
+// each filter row is summed on its own and the row sums are then added (rounding-error bound
+// (2rx+1 + 2ry) * 2^-24 of sum|W x| instead of (2ry+1)(2rx+1) * 2^-24).
+#include "common.cuh"
+#include "kernels.hpp"
+
+namespace skel {
+namespace {
+
+enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1 };
+
+__device__ __forceinline__ float ext2(const float* X, long long rows, long long cols, long long p, long long q,
+                                      int edge, float pad) {
+  if (p >= 0 && p < rows && q >= 0 && q < cols) return __ldg(X + p * cols + q);
+  if (edge == EDGE_CONSTANT) return pad;
+  p = p < 0 ? 0 : (p >= rows ? rows - 1 : p);
+  q = q < 0 ? 0 : (q >= cols ? cols - 1 : q);
+  return __ldg(X + p * cols + q);
+}
+
+// ---- direct --------------------------------------------------------------------------------
+// Filter rows are summed separately in chains of at most 17 taps, then added.
+template <typename WT>
+__global__ void __launch_bounds__(256)
+overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, float pad, const float* in, float* out,
+                        size_t rows, size_t cols) {
+  const size_t total = rows * cols;
+  const int fw = 2 * rx + 1;
+  for (size_t idx = blockIdx.x * size_t(blockDim.x) + threadIdx.x; idx < total; idx += size_t(gridDim.x) * blockDim.x) {
+    const long long i = static_cast<long long>(idx / cols);
+    const long long j = static_cast<long long>(idx - size_t(i) * cols);
+    const bool interior = i - ry >= 0 && i + ry < (long long)rows && j - rx >= 0 && j + rx < (long long)cols;
+    float acc = 0.f;
+    if (rx == 0) {  // column-wise 1D: chains of 16 taps
+      for (int a0 = 0; a0 <= 2 * ry; a0 += 16) {
+        const int a1 = min(a0 + 16, 2 * ry + 1);
+        float p = 0.f;
+        for (int a = a0; a < a1; ++a) {
+          const float v = interior ? __ldg(in + (i + a - ry) * (long long)cols + j)
+                                   : ext2(in, rows, cols, i + a - ry, j, edge, pad);
+          p = fmaf(W.w[a], v, p);
+        }
+        acc = a0 == 0 ? p : acc + p;
+      }
+    } else {
+      for (int a = 0; a <= 2 * ry; ++a) {
+        float p = 0.f;
+        for (int b = 0; b <= 2 * rx; ++b) {
+          const float v = interior ? __ldg(in + (i + a - ry) * (long long)cols + (j + b - rx))
+                                   : ext2(in, rows, cols, i + a - ry, j + b - rx, edge, pad);
+          p = fmaf(W.w[a * fw + b], v, p);
+        }
+        acc = a == 0 ? p : acc + p;
+      }
+    }
+    out[idx] = acc;
+  }
+}
+
+// ---- shared-memory tiled, register blocked -------------------------------------------------
+constexpr int T2_THREADS = 256;  // 32 (x) by 8 (y)
+constexpr int T2_TW = 128;       // tile width in outputs: 32 threads x 4
+
+template <int RY, int RX, int OY, typename WT>
+__global__ void __launch_bounds__(T2_THREADS)
+overlap2d_tiled_kernel(const __grid_constant__ WT W, int edge, float pad, const float* in, float* out, size_t rows,
+                       size_t cols) {
+  constexpr int RXP = (RX + 3) / 4 * 4;
+  constexpr int TH = 8 * OY;
+  constexpr int SW = T2_TW + 2 * RXP;  // staged row length (floats)
+  constexpr int SH = TH + 2 * RY;      // staged rows
+  constexpr int NGX = (4 + 2 * RXP) / 4;
+  constexpr int FW = 2 * RX + 1;
+  constexpr bool PER_ROW = (2 * RY + 1) * (2 * RX + 1) > 33;
+  extern __shared__ __align__(16) float sm[];
+
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const size_t tiles_x = (cols + T2_TW - 1) / T2_TW, tiles_y = (rows + TH - 1) / TH;
+  const size_t ntiles = tiles_x * tiles_y;
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t tyi = tile / tiles_x;
+    const long long r0 = static_cast<long long>(tyi * TH);
+    const long long c0 = static_cast<long long>((tile - tyi * tiles_x) * T2_TW);
+    // stage X~[r0-RY .. r0+TH+RY) x [c0-RXP .. c0+TW+RXP)
+#pragma unroll 4
+    for (int g = threadIdx.x; g < SH * (SW / 4); g += T2_THREADS) {
+      const int gy = g / (SW / 4), gx = g - gy * (SW / 4);
+      const long long p = r0 - RY + gy, q = c0 - RXP + 4 * gx;
+      float4 v;
+      if (p >= 0 && p < (long long)rows && q >= 0 && q + 3 < (long long)cols) {
+        uint32_t raw[4];
+        ld_stream<4, true>(raw, in + p * (long long)cols + q);
+        v = make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
+      } else {
+        v.x = ext2(in, rows, cols, p, q, edge, pad);
+        v.y = ext2(in, rows, cols, p, q + 1, edge, pad);
+        v.z = ext2(in, rows, cols, p, q + 2, edge, pad);
+        v.w = ext2(in, rows, cols, p, q + 3, edge, pad);
+      }
+      *reinterpret_cast<float4*>(sm + gy * SW + 4 * gx) = v;
+    }
+    __syncthreads();
+
+    float acc[OY][4];
+#pragma unroll
+    for (int o = 0; o < OY; ++o)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) acc[o][e] = 0.f;
+
+#pragma unroll
+    for (int ir = 0; ir < OY + 2 * RY; ++ir) {
+      const float* srow = sm + (ty * OY + ir) * SW + tx * 4;
+      float v[4 * NGX];
+#pragma unroll
+      for (int g = 0; g < NGX; ++g) {
+        const float4 t = *reinterpret_cast<const float4*>(srow + 4 * g);
+        v[4 * g] = t.x; v[4 * g + 1] = t.y; v[4 * g + 2] = t.z; v[4 * g + 3] = t.w;
+      }
+#pragma unroll
+      for (int o = 0; o < OY; ++o) {
+        const int a = ir - o;  // filter row that this staged row feeds for output row o
+        if (a >= 0 && a <= 2 * RY) {
+          if constexpr (PER_ROW) {
+            float p[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int b = 0; b < FW; ++b)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) acc[o][e] = a == 0 ? p[e] : acc[o][e] + p[e];
+          } else {
+#pragma unroll
+            for (int b = 0; b < FW; ++b)
+#pragma unroll
+              for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
+          }
+        }
+      }
+    }
+    const long long oc = c0 + tx * 4;
+#pragma unroll
+    for (int o = 0; o < OY; ++o) {
+      const long long orow = r0 + ty * OY + o;
+      if (orow < (long long)rows) {
+        float* dst = out + orow * (long long)cols + oc;
+        if (oc + 3 < (long long)cols) {
+          uint32_t raw[4] = {__float_as_uint(acc[o][0]), __float_as_uint(acc[o][1]), __float_as_uint(acc[o][2]),
+                             __float_as_uint(acc[o][3])};
+          st_stream<4>(dst, raw);
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            if (oc + e < (long long)cols) dst[e] = acc[o][e];
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+template <int RY, int RX, int OY> constexpr size_t tiled2_smem() {
+  return size_t(8 * OY + 2 * RY) * (T2_TW + 2 * ((RX + 3) / 4 * 4)) * sizeof(float);
+}
+
+template <int RY, int RX, int OY, typename WT>
+cudaError_t launch_tiled2(const Launch& L, const WT& w, int edge, float pad, const float* in, float* out, size_t rows,
+                          size_t cols) {
+  constexpr size_t smem = tiled2_smem<RY, RX, OY>();
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(overlap2d_tiled_kernel<RY, RX, OY, WT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_done = true;
+  }
+  const size_t ntiles = ((cols + T2_TW - 1) / T2_TW) * ((rows + 8 * OY - 1) / (8 * OY));
+  const size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
+  overlap2d_tiled_kernel<RY, RX, OY, WT><<<(unsigned)grid, T2_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename WT>
+cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edge, float pad, const float* in,
+                           float* out, size_t rows, size_t cols) {
+  const size_t total = rows * cols;
+  size_t grid = (total + 255) / 256;
+  const size_t cap = size_t(L.sms) * 64;
+  if (grid > cap) grid = cap;
+  overlap2d_direct_kernel<WT><<<(unsigned)grid, 256, 0, L.stream>>>(w, ry, rx, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8"};
+constexpr int kNumVariants = 3;
+
+inline bool tiled_alignment_ok(const void* in, const void* out, size_t cols) {
+  return reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 && cols % 4 == 0;
+}
+
+}  // namespace
+
+// ---- column-wise 1D ----------------------------------------------------------------------------
+int overlap1d_col_variant_count() { return kNumVariants; }
+const char* overlap1d_col_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kNames[v] : nullptr; }
+bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t, size_t cols) {
+  if (v < 0 || v >= kNumVariants) return false;
+  if (v == 0) return true;
+  const bool templated = r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16;
+  return templated && tiled_alignment_ok(in, out, cols);
+}
+
+cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+                                  const float* in, float* out, size_t rows, size_t cols) {
+  if (rows * cols == 0) return cudaSuccess;
+  if (v == 0) return launch_direct2<Weights1D>(L, w, r, 0, edge, pad, in, out, rows, cols);
+#define SKEL_COL_CASE(R)                                                                                      \
+  case R:                                                                                                     \
+    return v == 1 ? launch_tiled2<R, 0, 4, Weights1D>(L, w, edge, pad, in, out, rows, cols)                   \
+                  : launch_tiled2<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);
+  switch (r) {
+    SKEL_COL_CASE(1)
+    SKEL_COL_CASE(2)
+    SKEL_COL_CASE(3)
+    SKEL_COL_CASE(4)
+    SKEL_COL_CASE(8)
+    SKEL_COL_CASE(16)
+  }
+#undef SKEL_COL_CASE
+  return cudaErrorInvalidValue;
+}
+
+// ---- 2D ----------------------------------------------------------------------------------------
+int overlap2d_variant_count() { return kNumVariants; }
+const char* overlap2d_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kNames[v] : nullptr; }
+bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out, size_t, size_t cols) {
+  if (v < 0 || v >= kNumVariants) return false;
+  if (v == 0) return true;
+  const bool templated = ry == rx && ry >= 1 && ry <= 4;
+  return templated && tiled_alignment_ok(in, out, cols);
+}
+
+cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
+                             const float* in, float* out, size_t rows, size_t cols) {
+  if (rows * cols == 0) return cudaSuccess;
+  if (v == 0) return launch_direct2<Weights2D>(L, w, ry, rx, edge, pad, in, out, rows, cols);
+#define SKEL_2D_CASE(R)                                                                                       \
+  case R:                                                                                                     \
+    return v == 1 ? launch_tiled2<R, R, 4, Weights2D>(L, w, edge, pad, in, out, rows, cols)                   \
+                  : launch_tiled2<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);
+  switch (ry) {
+    SKEL_2D_CASE(1)
+    SKEL_2D_CASE(2)
+    SKEL_2D_CASE(3)
+    SKEL_2D_CASE(4)
+  }
+#undef SKEL_2D_CASE
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace skel

@@ -1,0 +1,196 @@
+// Reduce and fused MapReduce skeletons (readings 2 and 3):
+//   result = (+)_i f(in0[i], b_i)      f = identity for plain Reduce; the mapped value is never stored.
+// One kernel: every thread folds its elements into V independent accumulators (128/256-bit
+// streaming loads, U vectors per operand in flight), warp-shuffle + shared-memory block tree,
+// one partial per block; the block that draws the last ticket folds the partials in a fixed order
+// (bitwise deterministic for a given n and variant; no floating-point atomics). The ticket is an
+// atomicInc that wraps to 0, so no memset is needed between calls. The "two_pass" variants write
+// the partials and fold them in a second tiny kernel instead.
+#include "common.cuh"
+#include "kernels.hpp"
+#include <string.h>
+
+namespace skel {
+namespace {
+
+constexpr int RED_THREADS = 256;
+
+template <typename T, int OP>
+__device__ __forceinline__ void fold_partials(const T* partials, unsigned count, T* result, T* smem) {
+  T acc = identity<T, OP>();
+  for (unsigned i = threadIdx.x; i < count; i += blockDim.x) acc = apply_fn<OP>(T(0), acc, partials[i]);
+  __syncthreads();  // smem reuse
+  acc = block_reduce<T, OP>(acc, smem);
+  if (threadIdx.x == 0) *result = acc;
+}
+
+template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U, bool SINGLE_PASS>
+__global__ void __launch_bounds__(RED_THREADS)
+mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigned* ticket, T* result) {
+  __shared__ T smem[32];
+  __shared__ bool is_last;
+  constexpr size_t TILE = size_t(RED_THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  T acc[V];
+#pragma unroll
+  for (int j = 0; j < V; ++j) acc[j] = identity<T, OP>();
+
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t base = tile * TILE + size_t(threadIdx.x) * V;
+    if (base + (U - 1) * size_t(RED_THREADS) * V + V <= n) {
+      uint32_t a[U][V], b[U][V];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        ld_stream<V, true>(a[u], in0 + base + size_t(u) * RED_THREADS * V);
+        if constexpr (HAS_IN1) ld_stream<V, true>(b[u], in1 + base + size_t(u) * RED_THREADS * V);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          T bv = HAS_IN1 ? from_bits<T>(b[u][j]) : c;
+          acc[j] = apply_fn<OP>(T(0), acc[j], apply_fn<MAPF>(c, from_bits<T>(a[u][j]), bv));
+        }
+    } else {
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          const size_t i = base + size_t(u) * RED_THREADS * V + j;
+          if (i < n) {
+            T bv = HAS_IN1 ? in1[i] : c;
+            acc[j] = apply_fn<OP>(T(0), acc[j], apply_fn<MAPF>(c, in0[i], bv));
+          }
+        }
+    }
+  }
+  T v = acc[0];
+#pragma unroll
+  for (int j = 1; j < V; ++j) v = apply_fn<OP>(T(0), v, acc[j]);
+  v = block_reduce<T, OP>(v, smem);
+
+  if constexpr (SINGLE_PASS) {
+    if (gridDim.x == 1) {
+      if (threadIdx.x == 0) *result = v;
+      return;
+    }
+    if (threadIdx.x == 0) {
+      partials[blockIdx.x] = v;
+      __threadfence();
+      const unsigned t = atomicInc(ticket, gridDim.x - 1);  // wraps back to 0 on the last arrival
+      is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+      __threadfence();
+      fold_partials<T, OP>(partials, gridDim.x, result, smem);
+    }
+  } else {
+    if (threadIdx.x == 0) partials[blockIdx.x] = v;
+  }
+}
+
+template <typename T, int OP>
+__global__ void __launch_bounds__(RED_THREADS) fold_kernel(const T* partials, unsigned count, T* result) {
+  __shared__ T smem[32];
+  fold_partials<T, OP>(partials, count, result, smem);
+}
+
+struct RedVariant { const char* name; int v, u; bool single; int blocks_per_sm; };
+const RedVariant kRedVariants[] = {
+    {"scalar_single_pass", 1, 4, true, 8},
+    {"v4_u4_single_pass", 4, 4, true, 8},
+    {"v8_u2_single_pass", 8, 2, true, 8},
+    {"v4_u4_two_pass", 4, 4, false, 8},
+    {"v8_u2_two_pass", 8, 2, false, 8},
+    {"v4_u4_single_pass_4bps", 4, 4, true, 4},
+};
+constexpr int kNumRedVariants = sizeof(kRedVariants) / sizeof(kRedVariants[0]);
+
+inline bool aligned_to(const void* p, size_t a) { return p == nullptr || (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U>
+cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, const T* in0, const T* in1, T c,
+                       size_t n, T* result) {
+  constexpr size_t TILE = size_t(RED_THREADS) * V * U;
+  size_t ntiles = (n + TILE - 1) / TILE;
+  size_t grid = size_t(L.sms) * rv.blocks_per_sm;
+  if (grid > ntiles) grid = ntiles;
+  if (grid > MAX_PARTIALS) grid = MAX_PARTIALS;
+  T* partials = static_cast<T*>(S.partials);
+  if (rv.single) {
+    mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, true>
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result);
+    ++*L.launches;
+  } else {
+    mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, false>
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result);
+    fold_kernel<T, OP><<<1, RED_THREADS, 0, L.stream>>>(partials, (unsigned)grid, result);
+    *L.launches += 2;
+  }
+  return cudaGetLastError();
+}
+
+template <typename T, int MAPF, bool HAS_IN1, int OP>
+cudaError_t launch_vu(const Launch& L, const Scratch& S, const RedVariant& rv, const T* in0, const T* in1, T c,
+                      size_t n, T* result) {
+  if (rv.v == 1) return launch_one<T, MAPF, HAS_IN1, OP, 1, 4>(L, S, rv, in0, in1, c, n, result);
+  if (rv.v == 4) return launch_one<T, MAPF, HAS_IN1, OP, 4, 4>(L, S, rv, in0, in1, c, n, result);
+  return launch_one<T, MAPF, HAS_IN1, OP, 8, 2>(L, S, rv, in0, in1, c, n, result);
+}
+
+template <typename T, int MAPF, bool HAS_IN1>
+cudaError_t launch_op(const Launch& L, const Scratch& S, const RedVariant& rv, int op, const T* in0, const T* in1,
+                      T c, size_t n, T* result) {
+  switch (op) {
+    case FN_ADD: return launch_vu<T, MAPF, HAS_IN1, FN_ADD>(L, S, rv, in0, in1, c, n, result);
+    case FN_MULT: return launch_vu<T, MAPF, HAS_IN1, FN_MULT>(L, S, rv, in0, in1, c, n, result);
+    case FN_MAX: return launch_vu<T, MAPF, HAS_IN1, FN_MAX>(L, S, rv, in0, in1, c, n, result);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <typename T>
+cudaError_t launch_t(const Launch& L, const Scratch& S, const RedVariant& rv, int map_fn, bool has_in1, int op,
+                     T c, const T* in0, const T* in1, size_t n, T* result) {
+#define SKEL_MR_CASE(F)                                                                   \
+  case F:                                                                                 \
+    return has_in1 ? launch_op<T, F, true>(L, S, rv, op, in0, in1, c, n, result)          \
+                   : launch_op<T, F, false>(L, S, rv, op, in0, in1, c, n, result);
+  switch (map_fn) {
+    case FN_IDENT: return launch_op<T, FN_IDENT, false>(L, S, rv, op, in0, in1, c, n, result);
+    SKEL_MR_CASE(FN_ADD)
+    SKEL_MR_CASE(FN_MULT)
+    SKEL_MR_CASE(FN_MAX)
+    case FN_SAXPY: return launch_op<T, FN_SAXPY, true>(L, S, rv, op, in0, in1, c, n, result);
+  }
+#undef SKEL_MR_CASE
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+int reduce_variant_count() { return kNumRedVariants; }
+const char* reduce_variant_name(int v) { return (v >= 0 && v < kNumRedVariants) ? kRedVariants[v].name : nullptr; }
+
+bool reduce_variant_ok(int v, const void* in0, const void* in1, size_t) {
+  if (v < 0 || v >= kNumRedVariants) return false;
+  const size_t a = size_t(kRedVariants[v].v) * 4;
+  return aligned_to(in0, a) && aligned_to(in1, a);
+}
+
+cudaError_t launch_mapreduce(const Launch& L, const Scratch& S, int v, int dtype, int map_fn, bool has_in1,
+                             int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n, void* result) {
+  const RedVariant& rv = kRedVariants[v];
+  if (dtype == DT_F32) {
+    float c;
+    memcpy(&c, &cbits, 4);
+    return launch_t<float>(L, S, rv, map_fn, has_in1, red_op, c, static_cast<const float*>(in0),
+                           static_cast<const float*>(in1), n, static_cast<float*>(result));
+  }
+  return launch_t<int32_t>(L, S, rv, map_fn, has_in1, red_op, static_cast<int32_t>(cbits),
+                           static_cast<const int32_t*>(in0), static_cast<const int32_t*>(in1), n,
+                           static_cast<int32_t*>(result));
+}
+
+}  // namespace skel

