@@ -1,0 +1,528 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs. Sizes span several tiles and ragged tails; every kernel variant is forced
+through the same checks. Tolerances: BASELINE.json L5 (integers bit-exact; Map <= 1 ulp; fp32
+Reduce/MapReduce <= 1e-5 * sum|terms|; MapOverlap <= 2e-6 * sum|w x|)."""
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import SIZES, SIZES_SHORT, assert_map_f32, assert_overlap, assert_reduce_f32
+from paper_1405_2915_b200 import inputs as I
+from paper_1405_2915_b200 import skel as S
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import torch
+    assert torch.cuda.is_available()
+    c = S.Context()
+    yield c
+    c.close()
+
+
+def variants(sk):
+    return list(range(S.lib.skel_variant_count(sk)))
+
+
+class forced:
+    def __init__(self, ctx, sk, v):
+        self.ctx, self.sk, self.v = ctx, sk, v
+
+    def __enter__(self):
+        self.ctx.force_variant(self.sk, self.v)
+
+    def __exit__(self, *a):
+        self.ctx.force_variant(self.sk, -1)
+
+
+# ------------------------------------------------------------------ Map
+@pytest.mark.parametrize("v", variants(S.SK_MAP))
+def test_map_f32_all_functions(ctx, v):
+    with forced(ctx, S.SK_MAP, v):
+        for n in SIZES:
+            x, y = I.uniform_pm1_f32(100 + n, n), I.uniform_pm1_f32(101 + n, n)
+            vx, vy, vo = ctx.vector_from(x), ctx.vector_from(y), ctx.vector(n)
+            for fn in (S.FN_ADD, S.FN_MULT, S.FN_MAX, S.FN_SAXPY):
+                ctx.map(fn, 2.5, vx, vy, vo)
+                assert ctx.last_variant() == (S.SK_MAP, v)
+                assert_map_f32(vo.numpy(), O.map_f32(fn, 2.5, x, y))
+            for fn in (S.FN_ADD, S.FN_MULT, S.FN_MAX):
+                ctx.map(fn, 1.0001, vx, None, vo)
+                assert_map_f32(vo.numpy(), O.map_f32(fn, 1.0001, x))
+            for c in (vx, vy, vo):
+                c.destroy()
+
+
+def test_map_saxpy_cancellation_needs_fma(ctx):
+    # c*x ~ -y: a separate multiply and add would be hundreds of ulps off (reading (c).1 ii)
+    n = 50000
+    x = I.uniform_pm1_f32(110, n)
+    c32 = np.float32(2.5000001)
+    y = (-(c32 * x)).astype(np.float32)
+    vx, vy, vo = ctx.vector_from(x), ctx.vector_from(y), ctx.vector(n)
+    ctx.map(S.FN_SAXPY, float(c32), vx, vy, vo)
+    assert_map_f32(vo.numpy(), O.map_f32(O.FN_SAXPY, float(c32), x, y))
+    for c in (vx, vy, vo):
+        c.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_MAP))
+def test_map_i32_and_in_place(ctx, v):
+    with forced(ctx, S.SK_MAP, v):
+        for n in SIZES_SHORT:
+            a, b = I.full_range_i32(120 + n, n), I.full_range_i32(121 + n, n)
+            va, vb, vo = ctx.vector_from(a), ctx.vector_from(b), ctx.vector(n, S.I32)
+            for fn in (S.FN_ADD, S.FN_MULT, S.FN_MAX, S.FN_SAXPY):
+                ctx.map(fn, -7, va, vb, vo)
+                assert np.array_equal(vo.numpy(), O.map_i32(fn, -7, a, b))
+            ctx.map(S.FN_ADD, 12345, va, None, vo)
+            assert np.array_equal(vo.numpy(), O.map_i32(O.FN_ADD, 12345, a))
+            # in place: out aliases in0, then in1, then both
+            ctx.map(S.FN_MULT, 0, va, vb, va)
+            a1 = O.map_i32(O.FN_MULT, 0, a, b)
+            assert np.array_equal(va.numpy(), a1)
+            ctx.map(S.FN_ADD, 0, va, vb, vb)
+            b1 = O.map_i32(O.FN_ADD, 0, a1, b)
+            assert np.array_equal(vb.numpy(), b1)
+            ctx.map(S.FN_ADD, 0, vb, vb, vb)
+            assert np.array_equal(vb.numpy(), O.map_i32(O.FN_ADD, 0, b1, b1))
+            for c in (va, vb, vo):
+                c.destroy()
+
+
+def test_map_closed_form_and_empty(ctx):
+    n = 1 << 20
+    x = np.arange(n, dtype=np.float32)
+    vx, vy, vo = ctx.vector_from(x), ctx.vector_from(np.ones(n, np.float32)), ctx.vector(n)
+    ctx.map(S.FN_SAXPY, 2.5, vx, vy, vo)
+    assert np.array_equal(vo.numpy(), (2.5 * np.arange(n, dtype=np.float64) + 1).astype(np.float32))
+    ctx.map(S.FN_MULT, 1.0, vx, None, vo)
+    assert np.array_equal(vo.numpy(), x)
+    e0, e1 = ctx.vector_from(np.zeros(0, np.float32)), ctx.vector(0)
+    ctx.map(S.FN_ADD, 1.0, e0, None, e1)
+    assert e1.numpy().size == 0
+    for c in (vx, vy, vo, e0, e1):
+        c.destroy()
+
+
+def test_map_misaligned_adopted_pointer_falls_back(ctx):
+    import torch
+    n = 10001
+    x = I.uniform_pm1_f32(130, n + 3)
+    t = torch.from_numpy(x).cuda()
+    to = torch.empty(n + 3, dtype=torch.float32, device="cuda")
+    vx, vo = ctx.vector_adopt(t[1:n + 1]), ctx.vector_adopt(to[3:n + 3])
+    ctx.map(S.FN_MULT, 3.0, vx, None, vo)
+    assert ctx.last_variant() == (S.SK_MAP, 0)  # the any-alignment variant
+    ctx.sync()
+    assert_map_f32(to[3:n + 3].cpu().numpy(), O.map_f32(O.FN_MULT, 3.0, x[1:n + 1]))
+    with forced(ctx, S.SK_MAP, 2):
+        with pytest.raises(S.SkelError) as ei:
+            ctx.map(S.FN_MULT, 3.0, vx, None, vo)
+        assert ei.value.status == S.ERR_UNSUPPORTED
+    vx.destroy()
+    vo.destroy()
+
+
+# ------------------------------------------------------------------ Reduce / MapReduce
+@pytest.mark.parametrize("v", variants(S.SK_REDUCE))
+def test_reduce_i32_bit_exact(ctx, v):
+    with forced(ctx, S.SK_REDUCE, v):
+        for n in SIZES:
+            a = I.full_range_i32(200 + n, n)
+            va = ctx.vector_from(a)
+            assert ctx.reduce(S.FN_ADD, va) == O.reduce_i32(O.FN_ADD, a)[0]
+            assert ctx.reduce(S.FN_MAX, va) == O.reduce_i32(O.FN_MAX, a)[0]
+            small = (a % 5 + 1).astype(np.int32)
+            va.write(small)
+            assert ctx.reduce(S.FN_MULT, va) == O.reduce_i32(O.FN_MULT, small)[0]
+            va.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_REDUCE))
+def test_reduce_f32_tolerance_and_determinism(ctx, v):
+    with forced(ctx, S.SK_REDUCE, v):
+        for n in SIZES_SHORT + [(1 << 22) + 7]:
+            x = I.uniform_pm1_f32(210 + n, n)
+            vx = ctx.vector_from(x)
+            got = ctx.reduce(S.FN_ADD, vx)
+            ref, ab = O.reduce_f32(O.FN_ADD, x)
+            assert_reduce_f32(got, ref, ab)
+            assert all(ctx.reduce(S.FN_ADD, vx) == got for _ in range(3))  # bitwise run-to-run
+            assert ctx.reduce(S.FN_MAX, vx) == O.reduce_f32(O.FN_MAX, x)[0]
+            y = (1.0 + x * 2.0 ** -12).astype(np.float32)[: min(n, 5000)]
+            vy = ctx.vector_from(y)
+            refm, _ = O.reduce_f32(O.FN_MULT, y)
+            assert abs(ctx.reduce(S.FN_MULT, vy) - refm) <= 1e-4 * abs(refm)
+            vx.destroy()
+            vy.destroy()
+
+
+def test_reduce_closed_forms_and_max_position(ctx):
+    for n in [1, 1000, 4096, (1 << 20) + 3]:
+        v = ctx.vector_from(np.ones(n, np.float32))
+        assert ctx.reduce(S.FN_ADD, v) == n
+        v.destroy()
+        idx = np.arange(n, dtype=np.int32)
+        vi = ctx.vector_from(idx)
+        exp = (n * (n - 1) // 2) & 0xFFFFFFFF
+        assert ctx.reduce(S.FN_ADD, vi) & 0xFFFFFFFF == exp
+        vi.destroy()
+    n = 70001
+    base = I.permutation(220, n).astype(np.int32)
+    for pos in [0, 1, 255, 256, 4095, 4096, n // 2, n - 1]:
+        p = base.copy()
+        j = int(np.argmax(p))
+        p[j], p[pos] = p[pos], p[j]
+        vp = ctx.vector_from(p)
+        assert ctx.reduce(S.FN_MAX, vp) == n - 1
+        vp.destroy()
+
+
+def test_reduce_to_device_slot_and_errors(ctx):
+    x = I.uniform_int_i32(230, 5000, 1000)
+    vx = ctx.vector_from(x)
+    res = ctx.vector(4, S.I32)
+    ctx.reduce_to(S.FN_ADD, vx, res, 2)
+    ctx.reduce_to(S.FN_MAX, vx, res, 0)
+    got = res.numpy()
+    assert got[2] == O.reduce_i32(O.FN_ADD, x)[0] and got[0] == O.reduce_i32(O.FN_MAX, x)[0]
+    with pytest.raises(S.SkelError) as ei:
+        ctx.reduce_to(S.FN_ADD, vx, res, 4)
+    assert ei.value.status == S.ERR_INVALID_ARG
+    un = ctx.vector(10, S.I32)
+    with pytest.raises(S.SkelError) as ei:
+        ctx.reduce(S.FN_ADD, un)
+    assert ei.value.status == S.ERR_UNINIT
+    for c in (vx, res, un):
+        c.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_MAPREDUCE))
+def test_mapreduce_dot_and_friends(ctx, v):
+    with forced(ctx, S.SK_MAPREDUCE, v):
+        for n in SIZES_SHORT + [1 << 20]:
+            x, y = I.uniform_pm1_f32(300 + n, n), I.uniform_pm1_f32(301 + n, n)
+            vx, vy = ctx.vector_from(x), ctx.vector_from(y)
+            got = ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, vx, vy)
+            ref, ab = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, y)
+            assert_reduce_f32(got, ref, ab)
+            assert ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, vx, vy) == got
+            got = ctx.mapreduce(S.FN_ADD, S.FN_MAX, 0.0, vx, vy)
+            assert got == np.float32(O.mapreduce_f32(O.FN_ADD, O.FN_MAX, 0.0, x, y)[0])
+            got = ctx.mapreduce(S.FN_SAXPY, S.FN_ADD, 2.5, vx, vy)
+            ref, ab = O.mapreduce_f32(O.FN_SAXPY, O.FN_ADD, 2.5, x, y)
+            assert_reduce_f32(got, ref, ab)
+            got = ctx.mapreduce(S.FN_MULT, S.FN_ADD, 3.0, vx, None)  # sum of 3*x
+            ref, ab = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 3.0, x, None)
+            assert_reduce_f32(got, ref, ab)
+            a, b = I.full_range_i32(302 + n, n), I.full_range_i32(303 + n, n)
+            va, vb = ctx.vector_from(a), ctx.vector_from(b)
+            assert ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0, va, vb) == O.mapreduce_i32(O.FN_MULT, O.FN_ADD, 0, a, b)
+            assert ctx.mapreduce(S.FN_ADD, S.FN_MAX, 0, va, vb) == O.mapreduce_i32(O.FN_ADD, O.FN_MAX, 0, a, b)
+            for c in (vx, vy, va, vb):
+                c.destroy()
+
+
+def test_dot_closed_form_and_fusion_invariant(ctx):
+    n = 1 << 20
+    vx, vy = ctx.vector_from(np.arange(n, dtype=np.float32)), ctx.vector_from(np.ones(n, np.float32))
+    exact = n * (n - 1) // 2
+    assert abs(ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, vx, vy) - exact) <= 1e-5 * exact
+    a, b = I.full_range_i32(310, 99999), I.full_range_i32(311, 99999)
+    va, vb, vt = ctx.vector_from(a), ctx.vector_from(b), ctx.vector(99999, S.I32)
+    ctx.map(S.FN_MULT, 0, va, vb, vt)
+    assert ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0, va, vb) == ctx.reduce(S.FN_ADD, vt)
+    for c in (vx, vy, va, vb, vt):
+        c.destroy()
+
+
+# ------------------------------------------------------------------ Scan
+SCAN_SIZES = SIZES + [(1 << 21) + 13]
+
+
+@pytest.mark.parametrize("v", variants(S.SK_SCAN))
+def test_scan_i32_bit_exact(ctx, v):
+    with forced(ctx, S.SK_SCAN, v):
+        for n in SCAN_SIZES:
+            x = I.full_range_i32(400 + n, n)
+            vx, vo = ctx.vector_from(x), ctx.vector(n, S.I32)
+            ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, vx, vo)
+            assert ctx.last_variant() == (S.SK_SCAN, v)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, x))
+            ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, -12345, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, -12345, x))
+            ctx.scan(S.FN_MAX, S.SCAN_INCLUSIVE, 0, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_MAX, O.SCAN_INCLUSIVE, 0, x))
+            ctx.scan(S.FN_MAX, S.SCAN_EXCLUSIVE, 77, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_MAX, O.SCAN_EXCLUSIVE, 77, x))
+            ctx.scan(S.FN_MULT, S.SCAN_INCLUSIVE, 0, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_MULT, O.SCAN_INCLUSIVE, 0, x))
+            # in place
+            ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 5, vx, vx)
+            assert np.array_equal(vx.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 5, x))
+            vx.destroy()
+            vo.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_SCAN))
+def test_scan_every_small_n_and_tile_boundaries(ctx, v):
+    with forced(ctx, S.SK_SCAN, v):
+        sizes = list(range(0, 70)) + [4096 * k + d for k in (1, 2, 3) for d in (-1, 0, 1)] + [8192 * 3 + 1, 16384 + 1]
+        for n in sizes:
+            x = I.uniform_int_i32(410 + n, n, 15)
+            vx, vo = ctx.vector_from(x), ctx.vector(n, S.I32)
+            ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, x))
+            ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 3, vx, vo)
+            assert np.array_equal(vo.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 3, x))
+            vx.destroy()
+            vo.destroy()
+
+
+def test_scan_closed_forms_many_repeats(ctx):
+    # ones -> indices; repeated launches exercise the epoch-tagged tile states and the ticket reset
+    n = (1 << 22) + 5
+    vx, vo = ctx.vector_from(np.ones(n, np.int32)), ctx.vector(n, S.I32)
+    for v in variants(S.SK_SCAN):
+        with forced(ctx, S.SK_SCAN, v):
+            for rep in range(6):
+                ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, vx, vo)
+            assert np.array_equal(vo.numpy(), np.arange(1, n + 1, dtype=np.int32))
+            ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 0, vx, vo)
+            assert np.array_equal(vo.numpy(), np.arange(0, n, dtype=np.int32))
+    vx.destroy()
+    vo.destroy()
+
+
+def test_scan_f32_three_kernel(ctx):
+    for n in SIZES_SHORT:
+        x = I.uniform_pm1_f32(420 + n, n)
+        vx, vo = ctx.vector_from(x), ctx.vector(n)
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        assert S.variant_names(S.SK_SCAN)[ctx.last_variant()[1]].startswith("three_kernel")
+        ref, ab = O.scan_f32(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, x)
+        got = vo.numpy()
+        assert np.all(np.abs(got - ref) <= 1e-5 * ab)
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        assert np.array_equal(vo.numpy(), got)  # deterministic
+        ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 1.5, vx, vo)
+        ref, ab = O.scan_f32(O.FN_ADD, O.SCAN_EXCLUSIVE, 1.5, x)
+        assert np.all(np.abs(vo.numpy() - ref) <= 1e-5 * ab)
+        ctx.scan(S.FN_MAX, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        assert np.array_equal(vo.numpy(), O.scan_f32(O.FN_MAX, O.SCAN_INCLUSIVE, 0.0, x)[0].astype(np.float32))
+        vx.destroy()
+        vo.destroy()
+    with forced(ctx, S.SK_SCAN, 0):  # look-back variants are int32 only
+        vx, vo = ctx.vector_from(np.ones(10, np.float32)), ctx.vector(10)
+        with pytest.raises(S.SkelError) as ei:
+            ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        assert ei.value.status == S.ERR_UNSUPPORTED
+        vx.destroy()
+        vo.destroy()
+
+
+# ------------------------------------------------------------------ MapOverlap 1D
+EDGE_CASES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICATE, 0.0)]
+O1_SIZES = [1, 2, 3, 5, 16, 17, 33, 100, 1023, 4096, 4097, 8200, 16385, 65537, 300001]
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
+@pytest.mark.parametrize("r", [0, 1, 2, 3, 4, 5, 8, 16, 17, 64])
+def test_overlap1d_vector(ctx, v, r):
+    tiled = v != 0
+    if tiled and r not in (1, 2, 3, 4, 8, 16):
+        pytest.skip("tiled variants are instantiated for r in {1,2,3,4,8,16}")
+    w = I.positive_weights_f32(500 + r, 2 * r + 1)
+    ws = I.signed_weights_f32(501 + r, 2 * r + 1)
+    with forced(ctx, S.SK_OVERLAP1D, v):
+        for n in O1_SIZES:
+            x = I.uniform01_f32(502 + n, n)
+            vx, vo = ctx.vector_from(x), ctx.vector(n)
+            for edge, pad in EDGE_CASES:
+                ctx.mapoverlap_1d(w, r, edge, pad, vx, vo)
+                assert ctx.last_variant() == (S.SK_OVERLAP1D, v)
+                ref, ab = O.mapoverlap_1d(w, r, edge, pad, x)
+                assert_overlap(vo.numpy(), ref, ab)
+            ctx.mapoverlap_1d(ws, r, S.EDGE_DUPLICATE, 0.0, vx, vo)
+            ref, ab = O.mapoverlap_1d(ws, r, S.EDGE_DUPLICATE, 0.0, x)
+            assert_overlap(vo.numpy(), ref, ab)
+            vx.destroy()
+            vo.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
+def test_overlap1d_one_hot_weights_shift_bit_exact(ctx, v):
+    with forced(ctx, S.SK_OVERLAP1D, v):
+        for r in (1, 4, 16):
+            for n in (3, 50, 4099, 8193):
+                x = I.uniform_pm1_f32(510 + n, n)
+                vx, vo = ctx.vector_from(x), ctx.vector(n)
+                for m in range(2 * r + 1):
+                    w = np.zeros(2 * r + 1, np.float32)
+                    w[m] = 1.0
+                    for edge, pad in ((S.EDGE_CONSTANT, 0.25), (S.EDGE_DUPLICATE, 0.0)):
+                        ctx.mapoverlap_1d(w, r, edge, pad, vx, vo)
+                        j = np.arange(n) + m - r
+                        if edge == S.EDGE_CONSTANT:
+                            exp = np.where((j >= 0) & (j < n), x[np.clip(j, 0, n - 1)], np.float32(pad))
+                        else:
+                            exp = x[np.clip(j, 0, n - 1)]
+                        assert np.array_equal(vo.numpy(), exp.astype(np.float32))
+                vx.destroy()
+                vo.destroy()
+
+
+def test_overlap1d_constant_input_and_impulse(ctx):
+    for v in variants(S.SK_OVERLAP1D):
+        with forced(ctx, S.SK_OVERLAP1D, v):
+            for r in (1, 4, 16):
+                n = 20000
+                w = I.positive_weights_f32(520 + r, 2 * r + 1)
+                vx, vo = ctx.vector_from(np.full(n, 3.0, np.float32)), ctx.vector(n)
+                ctx.mapoverlap_1d(w, r, S.EDGE_DUPLICATE, 0.0, vx, vo)
+                got = vo.numpy()
+                assert np.all(np.abs(got - 3.0 * w.astype(np.float64).sum()) <= 2e-6 * 3.0)
+                assert np.all(got == got[0])
+                x = np.zeros(n, np.float32)
+                j = 8192
+                x[j] = 1.0
+                vx.write(x)
+                ctx.mapoverlap_1d(w, r, S.EDGE_CONSTANT, 0.0, vx, vo)
+                got = vo.numpy()
+                exp = np.zeros(n, np.float32)
+                for i in range(j - r, j + r + 1):
+                    exp[i] = w[(j - i) + r]
+                assert np.array_equal(got, exp)
+                vx.destroy()
+                vo.destroy()
+
+
+MAT_SHAPES = [(1, 1), (3, 5), (37, 129), (64, 128), (65, 136), (200, 520), (130, 1032), (1030, 264)]
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
+@pytest.mark.parametrize("r", [1, 4, 8, 16, 5])
+def test_overlap1d_matrix_rows(ctx, v, r):
+    w = I.positive_weights_f32(530 + r, 2 * r + 1)
+    for rows, cols in MAT_SHAPES:
+        X = I.uniform01_f32(531 + rows, rows * cols).reshape(rows, cols)
+        mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
+        tiled_ok = r in (1, 2, 3, 4, 8, 16) and (rows == 1 or cols % 8 == 0)
+        with forced(ctx, S.SK_OVERLAP1D, v):
+            for edge, pad in EDGE_CASES:
+                if v != 0 and not tiled_ok:
+                    with pytest.raises(S.SkelError):
+                        ctx.mapoverlap_1d_matrix(w, r, edge, pad, S.AXIS_ROW, mx, mo)
+                    continue
+                ctx.mapoverlap_1d_matrix(w, r, edge, pad, S.AXIS_ROW, mx, mo)
+                ref, ab = O.mapoverlap_1d_matrix(w, r, edge, pad, O.AXIS_ROW, X)
+                assert_overlap(mo.numpy(), ref, ab)
+        mx.destroy()
+        mo.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D_COL))
+@pytest.mark.parametrize("r", [0, 1, 2, 3, 4, 8, 16, 5, 40])
+def test_overlap1d_matrix_cols(ctx, v, r):
+    w = I.positive_weights_f32(540 + r, 2 * r + 1)
+    for rows, cols in MAT_SHAPES:
+        X = I.uniform01_f32(541 + rows, rows * cols).reshape(rows, cols)
+        mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
+        tiled_ok = r in (1, 2, 3, 4, 8, 16) and cols % 4 == 0
+        with forced(ctx, S.SK_OVERLAP1D_COL, v):
+            for edge, pad in EDGE_CASES:
+                if v != 0 and not tiled_ok:
+                    with pytest.raises(S.SkelError):
+                        ctx.mapoverlap_1d_matrix(w, r, edge, pad, S.AXIS_COL, mx, mo)
+                    continue
+                ctx.mapoverlap_1d_matrix(w, r, edge, pad, S.AXIS_COL, mx, mo)
+                assert ctx.last_variant() == (S.SK_OVERLAP1D_COL, v)
+                ref, ab = O.mapoverlap_1d_matrix(w, r, edge, pad, O.AXIS_COL, X)
+                assert_overlap(mo.numpy(), ref, ab)
+        mx.destroy()
+        mo.destroy()
+
+
+# ------------------------------------------------------------------ MapOverlap 2D
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP2D))
+@pytest.mark.parametrize("radii", [(0, 0), (1, 1), (2, 2), (3, 3), (4, 4), (2, 4), (1, 0), (0, 3), (8, 8)])
+def test_overlap2d(ctx, v, radii):
+    ry, rx = radii
+    W = I.positive_weights_f32(600 + ry * 9 + rx, (2 * ry + 1) * (2 * rx + 1))
+    Ws = I.signed_weights_f32(601 + ry * 9 + rx, (2 * ry + 1) * (2 * rx + 1))
+    for rows, cols in MAT_SHAPES:
+        X = I.uniform01_f32(602 + rows, rows * cols).reshape(rows, cols)
+        mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
+        tiled_ok = ry == rx and 1 <= ry <= 4 and cols % 4 == 0
+        with forced(ctx, S.SK_OVERLAP2D, v):
+            for edge, pad in EDGE_CASES:
+                if v != 0 and not tiled_ok:
+                    with pytest.raises(S.SkelError):
+                        ctx.mapoverlap_2d(W, ry, rx, edge, pad, mx, mo)
+                    continue
+                ctx.mapoverlap_2d(W, ry, rx, edge, pad, mx, mo)
+                assert ctx.last_variant() == (S.SK_OVERLAP2D, v)
+                ref, ab = O.mapoverlap_2d(W, ry, rx, edge, pad, X)
+                assert_overlap(mo.numpy(), ref, ab)
+            if v == 0 or tiled_ok:
+                ctx.mapoverlap_2d(Ws, ry, rx, S.EDGE_DUPLICATE, 0.0, mx, mo)
+                ref, ab = O.mapoverlap_2d(Ws, ry, rx, O.EDGE_DUPLICATE, 0.0, X)
+                assert_overlap(mo.numpy(), ref, ab)
+        mx.destroy()
+        mo.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP2D))
+def test_overlap2d_one_hot_shift_bit_exact_and_separable_identity(ctx, v):
+    rows, cols = 70, 136
+    X = I.uniform_pm1_f32(610, rows * cols).reshape(rows, cols)
+    mx, mo, mt = ctx.matrix_from(X), ctx.matrix(rows, cols), ctx.matrix(rows, cols)
+    with forced(ctx, S.SK_OVERLAP2D, v):
+        for a in range(5):
+            for b in range(5):
+                W = np.zeros((5, 5), np.float32)
+                W[a, b] = 1.0
+                for edge, pad in ((S.EDGE_CONSTANT, 0.125), (S.EDGE_DUPLICATE, 0.0)):
+                    ctx.mapoverlap_2d(W, 2, 2, edge, pad, mx, mo)
+                    p = np.arange(rows)[:, None] + a - 2
+                    q = np.arange(cols)[None, :] + b - 2
+                    inside = (p >= 0) & (p < rows) & (q >= 0) & (q < cols)
+                    val = X[np.clip(p, 0, rows - 1), np.clip(q, 0, cols - 1)]
+                    exp = val if edge == S.EDGE_DUPLICATE else np.where(inside, val, np.float32(pad))
+                    assert np.array_equal(mo.numpy(), exp.astype(np.float32))
+        # row pass then column pass == dense outer-product filter (within tolerance)
+        X01 = np.abs(X)
+        mx.write(X01)
+        wr, wc = I.positive_weights_f32(611, 9), I.positive_weights_f32(612, 9)
+        ctx.mapoverlap_1d_matrix(wr, 4, S.EDGE_DUPLICATE, 0.0, S.AXIS_ROW, mx, mt)
+        ctx.mapoverlap_1d_matrix(wc, 4, S.EDGE_DUPLICATE, 0.0, S.AXIS_COL, mt, mo)
+        sep = mo.numpy()
+        Wd = np.outer(wc.astype(np.float64), wr.astype(np.float64)).astype(np.float32)
+        ctx.mapoverlap_2d(Wd, 4, 4, S.EDGE_DUPLICATE, 0.0, mx, mo)
+        assert np.allclose(sep, mo.numpy(), rtol=0, atol=4e-6)
+    for c in (mx, mo, mt):
+        c.destroy()
+
+
+def test_separable_pair_lock_step(ctx):
+    # BJ:L10 "separable row-then-column 1D passes of radius 8": two calls, fp32 intermediate;
+    # each pass is checked against the oracle fed with that pass's actual input (reading (c).6 iii)
+    rows, cols, r = 300, 520, 8
+    X = I.uniform01_f32(620, rows * cols).reshape(rows, cols)
+    wr, wc = I.positive_weights_f32(621, 17), I.positive_weights_f32(622, 17)
+    mx, mt, mo = ctx.matrix_from(X), ctx.matrix(rows, cols), ctx.matrix(rows, cols)
+    ctx.mapoverlap_1d_matrix(wr, r, S.EDGE_DUPLICATE, 0.0, S.AXIS_ROW, mx, mt)
+    ctx.mapoverlap_1d_matrix(wc, r, S.EDGE_DUPLICATE, 0.0, S.AXIS_COL, mt, mo)
+    T = mt.numpy()
+    ref, ab = O.mapoverlap_1d_matrix(wr, r, O.EDGE_DUPLICATE, 0.0, O.AXIS_ROW, X)
+    assert_overlap(T, ref, ab)
+    ref2, ab2 = O.mapoverlap_1d_matrix(wc, r, O.EDGE_DUPLICATE, 0.0, O.AXIS_COL, T)
+    assert_overlap(mo.numpy(), ref2, ab2)
+    # against the oracle's fp64 chain: the fp32 rounding of the intermediate stays inside 2e-6
+    ref3, ab3 = O.mapoverlap_1d_matrix(wc, r, O.EDGE_DUPLICATE, 0.0, O.AXIS_COL, ref)
+    assert_overlap(mo.numpy(), ref3, ab3)
+    for c in (mx, mt, mo):
+        c.destroy()
