@@ -1,0 +1,415 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the skeleton hot path on B200 (contract: see DESIGN.md "Measurement").
+
+One *step* = one pass of the whole hot path over one batch of synthetic input: every skeleton of
+SURVEY.md §8(a) at the largest size BASELINE.json's configs give it (Map saxpy 2^26, int32 Reduce
+sum+max 2^26, MapReduce dot 2^26, MapOverlap 1D r in {1,4,16} x {constant-0, duplicate} 2^26,
+MapOverlap 2D 5x5 / 9x9 and the separable r=8 row+column pair on 8192^2, int32 Scan inclusive +
+exclusive 2^28). `value` = algorithmic bytes of the step / device time of the step (GB/s), inputs
+resident in HBM. `e2e` = the same through host buffers (uploads and downloads inside the timed
+region). Every working set is > L2 (126 MB), so no flush is needed between iterations.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--scale S] [--impl reference]
+
+N > 1 (under torchrun): independent replicas, one per GPU ("replicas only": the path does not
+shard, BASELINE.json L5). --impl reference times the CPU oracle (the only reference this tier has).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "skeleton throughput (algorithmic GB/s over one pass of all skeletons at their largest config)"
+UNIT = "GB/s"
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f).get("hbm_gbs", 6650.0), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------------
+def sizes(scale: float):
+    lg = lambda full: max(12, int(round(full + np.log2(scale))))  # noqa: E731
+    side = 1 << max(6, int(round(13 + np.log2(scale) / 2)))
+    return {"n26": 1 << lg(26), "n28": 1 << lg(28), "side": side}
+
+
+def gen_inputs(sz):
+    from paper_1405_2915_b200 import inputs as I
+    t = time.time()
+    d = {
+        "x": I.uniform_pm1_f32(I.config_seed(2, 0), sz["n26"]),
+        "y": I.uniform_pm1_f32(I.config_seed(2, 1), sz["n26"]),
+        "vi": I.uniform_int_i32(I.config_seed(2, 2), sz["n26"], 1000),
+        "s": I.uniform01_f32(I.config_seed(3, 0), sz["n26"]),
+        "X": I.uniform01_f32(I.config_seed(4, 0), sz["side"] * sz["side"]).reshape(sz["side"], sz["side"]),
+        "scan": I.uniform_int_i32(I.config_seed(5, 0), sz["n28"], 15),
+        "w": {r: I.positive_weights_f32(I.config_seed(3, 10 + r), 2 * r + 1) for r in (1, 4, 8, 16)},
+        "W5": I.positive_weights_f32(I.config_seed(4, 1), 25),
+        "W9": I.positive_weights_f32(I.config_seed(4, 2), 81),
+        "wr8": I.positive_weights_f32(I.config_seed(4, 3), 17),
+        "wc8": I.positive_weights_f32(I.config_seed(4, 4), 17),
+    }
+    log(f"[bench] inputs generated in {time.time() - t:.1f} s")
+    return d
+
+
+class Workload:
+    """Containers + the ordered list of skeleton calls of one step."""
+
+    def __init__(self, S, ctx, d, sz):
+        self.S, self.ctx, self.sz = S, ctx, sz
+        n26, n28, side = sz["n26"], sz["n28"], sz["side"]
+        self.vx, self.vy = ctx.vector_from(d["x"]), ctx.vector_from(d["y"])
+        self.vr = ctx.vector(n26)
+        self.vi = ctx.vector_from(d["vi"])
+        self.vs, self.vso = ctx.vector_from(d["s"]), ctx.vector(n26)
+        self.mX, self.mT, self.mO = ctx.matrix_from(d["X"]), ctx.matrix(side, side), ctx.matrix(side, side)
+        self.vscan, self.vscan_o = ctx.vector_from(d["scan"]), ctx.vector(n28, S.I32)
+        self.res = ctx.vector(8, S.I32)
+        self.resf = ctx.vector(8, S.F32)
+        self.inputs = [self.vx, self.vy, self.vi, self.vs, self.mX, self.vscan]
+        self.outputs = [self.vr, self.vso, self.mO, self.vscan_o, self.res, self.resf]
+        m = side * side
+        ops = []
+        add = lambda name, fam, fn, nbytes, elems: ops.append((name, fam, fn, nbytes, elems))  # noqa: E731
+        add("map_saxpy_f32", "map", lambda: ctx.map(S.FN_SAXPY, 2.5, self.vx, self.vy, self.vr), 12 * n26, n26)
+        add("reduce_sum_i32", "reduce", lambda: ctx.reduce_to(S.FN_ADD, self.vi, self.res, 0), 4 * n26, n26)
+        add("reduce_max_i32", "reduce", lambda: ctx.reduce_to(S.FN_MAX, self.vi, self.res, 1), 4 * n26, n26)
+        add("mapreduce_dot_f32", "mapreduce",
+            lambda: ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, self.vx, self.vy, self.resf, 0), 8 * n26, n26)
+        for r in (1, 4, 16):
+            for edge, en in ((S.EDGE_CONSTANT, "const0"), (S.EDGE_DUPLICATE, "dup")):
+                add(f"overlap1d_r{r}_{en}", "overlap1d",
+                    (lambda r=r, edge=edge: ctx.mapoverlap_1d(d["w"][r], r, edge, 0.0, self.vs, self.vso)), 8 * n26, n26)
+        add("overlap2d_5x5_dup", "overlap2d", lambda: ctx.mapoverlap_2d(d["W5"], 2, 2, S.EDGE_DUPLICATE, 0.0, self.mX, self.mO), 8 * m, m)
+        add("overlap2d_9x9_dup", "overlap2d", lambda: ctx.mapoverlap_2d(d["W9"], 4, 4, S.EDGE_DUPLICATE, 0.0, self.mX, self.mO), 8 * m, m)
+        add("overlap1d_rows_r8_dup", "overlap1d",
+            lambda: ctx.mapoverlap_1d_matrix(d["wr8"], 8, S.EDGE_DUPLICATE, 0.0, S.AXIS_ROW, self.mX, self.mT), 8 * m, m)
+        add("overlap1d_cols_r8_dup", "overlap1d_col",
+            lambda: ctx.mapoverlap_1d_matrix(d["wc8"], 8, S.EDGE_DUPLICATE, 0.0, S.AXIS_COL, self.mT, self.mO), 8 * m, m)
+        add("scan_inclusive_i32", "scan", lambda: ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, self.vscan, self.vscan_o), 8 * n28, n28)
+        add("scan_exclusive_i32", "scan", lambda: ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 0, self.vscan, self.vscan_o), 8 * n28, n28)
+        self.ops = ops
+        self.bytes_per_step = sum(o[3] for o in ops)
+        self.elems_per_step = sum(o[4] for o in ops)
+
+    def step(self, events=None):
+        import torch
+        for i, (_, _, fn, _, _) in enumerate(self.ops):
+            if events is not None:
+                events[i][0].record()
+            fn()
+            if events is not None:
+                events[i][1].record()
+
+    def e2e_step(self):
+        """Host produces new inputs (pinned buffers), all skeletons run, host reads every output."""
+        S = self.S
+        for c in self.inputs:  # host write access: the device copy becomes stale -> next use uploads
+            c.host_view(S.WRITE)
+            c.release()
+        self.step()
+        tot = 0.0
+        for c in self.outputs:  # host read access: downloads
+            v = c.host_view(S.READ)
+            tot += float(v.reshape(-1)[0])
+            c.release()
+        return tot
+
+    def verify(self, d):
+        """Cheap O(n) property checks on the step's outputs (full parity lives in tests/)."""
+        S = self.S
+        res = self.res.numpy()
+        assert int(res[0]) & 0xFFFFFFFF == int(d["vi"].astype(np.int64).sum()) & 0xFFFFFFFF, "reduce sum mismatch"
+        assert int(res[1]) == int(d["vi"].max()), "reduce max mismatch"
+        dot = float(self.resf.numpy()[0])
+        ref = float(np.dot(d["x"].astype(np.float64), d["y"].astype(np.float64)))
+        assert abs(dot - ref) <= 1e-5 * float(np.abs(d["x"].astype(np.float64) * d["y"]).sum()), "dot mismatch"
+        sc = self.vscan_o.numpy()  # last call of the step was the exclusive scan
+        x = d["scan"]
+        assert sc[0] == 0 and np.array_equal(sc[1:] - sc[:-1], x[:-1]), "scan mismatch"
+        r = self.vr.numpy()
+        assert np.array_equal(r[:4096], (np.float32(2.5) * d["x"][:4096].astype(np.float64) + d["y"][:4096]).astype(np.float32)) or \
+            np.max(np.abs(r[:4096] - (2.5 * d["x"][:4096].astype(np.float64) + d["y"][:4096]))) < 1e-6, "map mismatch"
+
+    def destroy(self):
+        for c in self.inputs + self.outputs + [self.mT]:
+            c.destroy()
+
+
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+# --------------------------------------------------------------------------------------------------
+def cpu_oracle_pass(scale_div: int = 4, quiet=False):
+    """One pass of the same hot path by the CPU oracle on a bounded sample (every size / scale_div).
+    Returns (algorithmic bytes, seconds, threads, description)."""
+    import oracle as O
+    from paper_1405_2915_b200 import inputs as I
+    O.use_openmp(False)
+    n = (1 << 26) // scale_div
+    n28 = (1 << 28) // scale_div
+    side = int(8192 / np.sqrt(scale_div))
+    x, y = I.uniform_pm1_f32(1, n), I.uniform_pm1_f32(2, n)
+    vi = I.uniform_int_i32(3, n, 1000)
+    s = I.uniform01_f32(4, n)
+    X = I.uniform01_f32(5, side * side).reshape(side, side)
+    sc = I.uniform_int_i32(6, n28, 15)
+    w = {r: I.positive_weights_f32(10 + r, 2 * r + 1) for r in (1, 4, 8, 16)}
+    W5, W9 = I.positive_weights_f32(20, 25), I.positive_weights_f32(21, 81)
+    t0 = time.perf_counter()
+    nbytes = 0
+    O.map_f32(O.FN_SAXPY, 2.5, x, y); nbytes += 12 * n
+    O.reduce_i32(O.FN_ADD, vi); O.reduce_i32(O.FN_MAX, vi); nbytes += 8 * n
+    O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, y); nbytes += 8 * n
+    for r in (1, 4, 16):
+        for edge in (O.EDGE_CONSTANT, O.EDGE_DUPLICATE):
+            O.mapoverlap_1d(w[r], r, edge, 0.0, s); nbytes += 8 * n
+    O.mapoverlap_2d(W5, 2, 2, O.EDGE_DUPLICATE, 0.0, X); nbytes += 8 * side * side
+    O.mapoverlap_2d(W9, 4, 4, O.EDGE_DUPLICATE, 0.0, X); nbytes += 8 * side * side
+    T, _ = O.mapoverlap_1d_matrix(w[8], 8, O.EDGE_DUPLICATE, 0.0, O.AXIS_ROW, X); nbytes += 8 * side * side
+    O.mapoverlap_1d_matrix(w[8], 8, O.EDGE_DUPLICATE, 0.0, O.AXIS_COL, T); nbytes += 8 * side * side
+    O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, sc); O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 0, sc); nbytes += 16 * n28
+    dt = time.perf_counter() - t0
+    desc = (f"one pass of all skeletons, each at 1/{scale_div} of its bench size (vectors 2^26/{scale_div}, scan "
+            f"2^28/{scale_div}, matrix {side}^2), single-thread build of oracle/oracle.cpp as it stands")
+    return nbytes, dt, 1, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    O.build()
+    times = []
+    nbytes = desc = None
+    for i in range(args.warmup + args.steps):
+        nbytes, dt, threads, desc = cpu_oracle_pass(args.ref_div)
+        if i >= args.warmup:
+            times.append(dt)
+    t = float(np.mean(times))
+    v = nbytes / t / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, BASELINE.json configs)",
+            "config": {"workload": "all skeletons at BASELINE.json configs[1..4] sizes, bounded sample for the CPU oracle"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink every size (testing only; <1 invalidates the number)")
+    ap.add_argument("--ref-div", type=int, default=8)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--plan", default=os.path.join(ROOT, "paper_1405_2915_b200", "plans", "b200.plan"))
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_1405_2915_b200 import skel as S  # fails loudly if libskel.so is missing
+
+    sz = sizes(args.scale)
+    d = gen_inputs(sz)
+    ctx = S.Context()
+    if args.plan and os.path.exists(args.plan):
+        ctx.plan_load(args.plan)
+    wl = Workload(S, ctx, d, sz)
+    nops = len(wl.ops)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        wl.step()
+    barrier()
+    ev = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nops)]
+          for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    sampler.start()
+    ctx.reset_stats()
+    barrier()
+    e0.record()
+    for k in range(args.steps):
+        wl.step(ev[k])
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = ctx.stats()["launches"]
+    total_ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * wl.bytes_per_step / (ms_per_step * 1e-3) / 1e9
+    wl.verify(d)
+
+    # per-call breakdown (median over steps)
+    peak, peak_src = measured_peaks()
+    per = {}
+    fam_time = {}
+    for i, (name, fam, _, nbytes, elems) in enumerate(wl.ops):
+        ts = sorted(ev[k][i][0].elapsed_time(ev[k][i][1]) for k in range(args.steps))
+        med = ts[len(ts) // 2]
+        mean = float(np.mean(ts))
+        per[name] = {"us": round(med * 1e3, 2), "GB/s": round(nbytes / (med * 1e-3) / 1e9, 1),
+                     "Gelem/s": round(elems / (med * 1e-3) / 1e9, 1), "frac_measured_hbm": round(nbytes / (med * 1e-3) / 1e9 / peak, 4),
+                     "frac_8TBs": round(nbytes / (med * 1e-3) / 1e9 / 8000.0, 4), "variant": None}
+        fam_time.setdefault(fam, [0.0, 0, 0, 0])
+        fam_time[fam][0] += mean
+        fam_time[fam][1] += nbytes
+        fam_time[fam][2] += 1
+    # variant names actually chosen
+    for i, (name, fam, fn, _, _) in enumerate(wl.ops):
+        fn()
+        sk, v = ctx.last_variant()
+        per[name]["variant"] = S.variant_names(sk)[v]
+    ctx.sync()
+    dom = max(fam_time, key=lambda f: fam_time[f][0])
+    dt_ms, dbytes, dcount, _ = fam_time[dom]
+    achieved = dbytes / (dt_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": None, "peak_source": peak_src,
+                "launches_per_step": dcount, "avg_launch_us": round(dt_ms * 1e3 / dcount, 2),
+                "share_of_step": round(dt_ms / ms_per_step, 4)}
+
+    # ---- small-n latency (config 0: dot n = 2^20, L2 resident) — reported, not part of `value`
+    from paper_1405_2915_b200 import inputs as I
+    n20 = 1 << 20
+    a20, b20 = ctx.vector_from(I.uniform_pm1_f32(I.config_seed(1, 0), n20)), ctx.vector_from(I.uniform_pm1_f32(I.config_seed(1, 1), n20))
+    for _ in range(5):
+        ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, a20, b20, wl.resf, 1)
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s0.record()
+    for _ in range(50):
+        ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, a20, b20, wl.resf, 1)
+    s1.record()
+    torch.cuda.synchronize()
+    dot20_us = s0.elapsed_time(s1) * 1e3 / 50
+    a20.destroy()
+    b20.destroy()
+
+    # ---- end to end through host buffers
+    e2e = None
+    if not args.no_e2e:
+        wl.e2e_step()
+        barrier()
+        ctx.reset_stats()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            wl.e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        st = ctx.stats()
+        e2e = {"value": round(world * wl.bytes_per_step * args.steps / dt / 1e9, 2), "unit": UNIT,
+               "h2d_bytes_per_step": st["h2d_bytes"] // args.steps, "d2h_bytes_per_step": st["d2h_bytes"] // args.steps,
+               "ms_per_step": round(dt / args.steps * 1e3, 2)}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        nb, dt, threads, desc = cpu_oracle_pass(2)
+        cpu = {"value": round(nb / dt / 1e9, 3), "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+               "seconds": round(dt, 2), "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": round(ms_per_step, 4), "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32+i32", "data": "synthetic (seeded counter-based generator, BASELINE.json configs)",
+                "config": {"workload": "all skeletons at their largest BASELINE.json config (configs[1..4]): Map saxpy 2^26, "
+                                       "Reduce sum+max i32 2^26, MapReduce dot 2^26, MapOverlap1D r{1,4,16}x{const0,dup} 2^26, "
+                                       "MapOverlap2D 5x5/9x9 + separable r8 on 8192^2, Scan incl+excl i32 2^28",
+                           "scale": args.scale, "l2": "every working set > 126 MB L2; no flush", "calls_per_step": nops,
+                           "bytes_per_step": wl.bytes_per_step, "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
+                "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "per_skeleton": per}
+        print(json.dumps(line), flush=True)
+    wl.destroy()
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

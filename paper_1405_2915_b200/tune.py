@@ -1,0 +1,72 @@
+"""Off-line tuning of the execution plan for this machine (plans are "recomputed
+for each new target system"; L53: dispatch structures precomputed from sample executions).
+
+  python -m paper_1405_2915_b200.tune [--out plans/b200.plan] [--reps 7]
+
+Times every applicable kernel variant of the skeleton instances the bench configs use at
+n = 2^k, stores the per-size winners as breakpoints, prints the timing tables (microseconds) and
+writes the plan file that bench.py and users load with skel_plan_load.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def instances(S):
+    I = S.SkelInstance
+    out = []
+    out.append(("map_saxpy_f32", I(skeleton=S.SK_MAP, fn=S.FN_SAXPY, dtype=S.F32, mode=1), 12, 26, 0))
+    out.append(("map_mult_const_f32", I(skeleton=S.SK_MAP, fn=S.FN_MULT, dtype=S.F32, mode=0), 12, 26, 0))
+    out.append(("reduce_add_i32", I(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.I32), 12, 26, 0))
+    out.append(("reduce_max_i32", I(skeleton=S.SK_REDUCE, fn=S.FN_MAX, dtype=S.I32), 12, 26, 0))
+    out.append(("reduce_add_f32", I(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.F32), 12, 26, 0))
+    out.append(("dot_f32", I(skeleton=S.SK_MAPREDUCE, fn=S.FN_MULT, fn2=S.FN_ADD, dtype=S.F32, mode=1), 12, 26, 0))
+    for mode, mn in ((S.SCAN_INCLUSIVE, "incl"), (S.SCAN_EXCLUSIVE, "excl")):
+        out.append((f"scan_add_i32_{mn}", I(skeleton=S.SK_SCAN, fn=S.FN_ADD, dtype=S.I32, mode=mode), 12, 28, 0))
+    for r in (1, 4, 16):
+        for edge in (S.EDGE_CONSTANT, S.EDGE_DUPLICATE):
+            out.append((f"overlap1d_r{r}_e{edge}", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, edge=edge), 12, 26, 0))
+    out.append(("overlap1d_rows_r8", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    out.append(("overlap1d_cols_r8", I(skeleton=S.SK_OVERLAP1D_COL, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    for r in (2, 4):
+        out.append((f"overlap2d_{2*r+1}x{2*r+1}", I(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, r1=r, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--out", default=os.path.join(HERE, "plans", "b200.plan"))
+    ap.add_argument("--reps", type=int, default=7)
+    ap.add_argument("--tables", default=None, help="write the timing tables as JSON here")
+    args = ap.parse_args()
+    sys.path.insert(0, os.path.dirname(HERE))
+    from paper_1405_2915_b200 import skel as S
+
+    ctx = S.Context()
+    tables = {}
+    for name, inst, lo, hi, cols in instances(S):
+        t = ctx.tune(inst, lo, hi, cols, args.reps)
+        names = S.variant_names(inst.skeleton)
+        tables[name] = {"variants": names, "log2_lo": lo, "us": [[None if x != x else round(float(x), 2) for x in row] for row in t]}
+        print(f"== {name}: " + ", ".join(f"{i}:{n}" for i, n in enumerate(names)))
+        for k, row in enumerate(t):
+            if all(x != x for x in row):
+                continue
+            best = min((x, i) for i, x in enumerate(row) if x == x)[1]
+            print(f"  2^{lo + k:2d}  " + " ".join(f"{x:9.1f}" for x in row) + f"   -> {best}")
+    os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
+    ctx.plan_save(args.out)
+    if args.tables:
+        with open(args.tables, "w") as f:
+            json.dump(tables, f)
+    ctx.close()
+    print("plan written to", args.out)
+
+
+if __name__ == "__main__":
+    main()
