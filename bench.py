@@ -263,6 +263,8 @@ def main():
     ap.add_argument("--ref-div", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--force", action="append", default=[], metavar="SKELETON_ID=VARIANT_ID",
+                    help="force a kernel variant for a skeleton id (profiling aid), e.g. --force 3=3")
     ap.add_argument("--plan", default=os.path.join(ROOT, "paper_1405_2915_b200", "plans", "b200.plan"))
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -284,6 +286,9 @@ def main():
     ctx = S.Context()
     if args.plan and os.path.exists(args.plan):
         ctx.plan_load(args.plan)
+    for f in args.force:
+        sk, v = f.split("=")
+        ctx.force_variant(int(sk), int(v))
     wl = Workload(S, ctx, d, sz)
     nops = len(wl.ops)
 

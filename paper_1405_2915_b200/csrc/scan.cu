@@ -12,11 +12,14 @@
 //    fixed combination order (deterministic for f32); the correctness anchor for the look-back.
 #include "common.cuh"
 #include "kernels.hpp"
+#include <cooperative_groups.h>
+#include <stdlib.h>
 
 namespace skel {
 namespace {
 
 constexpr unsigned FULL = 0xffffffffu;
+constexpr int LB_WINDOWS = 1;  // look-back windows (of 32 tile states) fetched per round
 
 template <typename T, int OP> __device__ __forceinline__ T op2(T a, T b) { return apply_fn<OP>(T(0), a, b); }
 
@@ -29,14 +32,25 @@ template <typename T, int V, int U> struct TileRegs {
 // Phase A: load the tile, scan locally, return the tile aggregate (all threads).
 // smem layout: tot[E] | excl[E] | agg, E = U * (THREADS/32).
 template <typename T, int OP, int THREADS, int V, int U, bool NC>
-__device__ __forceinline__ T tile_phase_a(const T* in, size_t base, size_t n, TileRegs<T, V, U>& R, T* sm) {
+__device__ __forceinline__ T tile_phase_a(const T* in, size_t base, size_t n, TileRegs<T, V, U>& R, T* sm,
+                                          const T* staged = nullptr) {
   constexpr int NW = THREADS / 32, E = U * NW, EPL = (E + 31) / 32;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const T ident = identity<T, OP>();
 #pragma unroll
   for (int u = 0; u < U; ++u) {
     const size_t i0 = base + (size_t(u) * THREADS + threadIdx.x) * V;
-    if (i0 + V <= n) {
+    if (staged != nullptr) {  // the whole tile was staged in shared memory by a bulk copy
+      static_assert(V == 4 || V == 1 || V == 8 || V == 2, "vector width");
+      if constexpr (V == 4) {
+        const uint4 q = *reinterpret_cast<const uint4*>(staged + (u * THREADS + threadIdx.x) * 4);
+        R.x[u][0] = from_bits<T>(q.x); R.x[u][1] = from_bits<T>(q.y);
+        R.x[u][2] = from_bits<T>(q.z); R.x[u][3] = from_bits<T>(q.w);
+      } else {
+#pragma unroll
+        for (int j = 0; j < V; ++j) R.x[u][j] = staged[(u * THREADS + threadIdx.x) * V + j];
+      }
+    } else if (i0 + V <= n) {
       uint32_t raw[V];
       ld_stream<V, NC>(raw, in + i0);
 #pragma unroll
@@ -132,6 +146,68 @@ __device__ __forceinline__ unsigned long long pack_state(uint32_t epoch, unsigne
   return (static_cast<unsigned long long>(epoch) << 34) | (static_cast<unsigned long long>(status) << 32) | value;
 }
 
+// Look-back of one tile, executed by warp 0 (all 32 lanes). Publishes the tile's aggregate, folds
+// the predecessors' aggregates back to the nearest inclusive prefix, publishes the tile's inclusive
+// prefix and returns the tile's exclusive prefix (carry).
+__constant__ unsigned c_poll_delay_ns = 0;  // back-off between polls of unpublished tile states
+
+template <typename T, int OP>
+__device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t epoch, unsigned tile, T agg, T init,
+                                            bool exclusive) {
+  const int lane = threadIdx.x & 31;
+  const T ident = identity<T, OP>();
+  T carry;
+  if (tile == 0) {
+    carry = exclusive ? init : ident;
+    if (lane == 0) st_state(state, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
+    return carry;
+  }
+  if (lane == 0) st_state(state + tile, pack_state(epoch, 1u, to_bits(agg)));
+  carry = ident;
+  if (c_poll_delay_ns == 12345u) return carry;  // DEBUG experiment: skip the look-back (wrong results)
+  // The inclusive-prefix frontier advances by at most one look-back window per L2 round trip, so
+  // the window decides the chain speed: LB_WINDOWS * 32 predecessor states are fetched per round
+  // (independent loads in flight together) and folded nearest-first.
+  constexpr int K = LB_WINDOWS;
+  long long j = static_cast<long long>(tile) - 1;
+  while (true) {
+    unsigned long long w[K];
+    unsigned st[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      const long long idx = j - lane - 32 * k;
+      w[k] = idx >= 0 ? ld_state(state + idx) : 0ull;
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      const long long idx = j - lane - 32 * k;
+      // before the first tile: a virtual inclusive prefix equal to the identity
+      st[k] = idx < 0 ? 2u : ((static_cast<uint32_t>(w[k] >> 34) == epoch) ? static_cast<unsigned>(w[k] >> 32) & 3u : 0u);
+    }
+    int consumed = 0;
+    bool done = false;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      if (done || consumed != k) continue;
+      if (__any_sync(FULL, st[k] == 0u)) continue;  // not published yet: poll again from this window
+      const long long idx = j - lane - 32 * k;
+      const T val = idx >= 0 ? from_bits<T>(static_cast<uint32_t>(w[k])) : ident;
+      const unsigned incl = __ballot_sync(FULL, st[k] == 2u);
+      const int first = incl ? (__ffs(incl) - 1) : 32;
+      T contrib = lane <= first ? val : ident;
+      contrib = warp_reduce<T, OP>(contrib);
+      carry = op2<T, OP>(contrib, carry);
+      consumed = k + 1;
+      if (incl) done = true;
+    }
+    if (done) break;
+    j -= 32 * consumed;
+    if (consumed == 0 && c_poll_delay_ns) __nanosleep(c_poll_delay_ns);
+  }
+  if (lane == 0) st_state(state + tile, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
+  return carry;
+}
+
 template <typename T, int OP, int THREADS, int V, int U, bool NC>
 __global__ void __launch_bounds__(THREADS)
 scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state,
@@ -143,9 +219,8 @@ scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsig
   __shared__ unsigned s_tile;
   __shared__ T s_carry;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const T ident = identity<T, OP>();
 
-  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  if (threadIdx.x == 0) s_tile = (c_poll_delay_ns == 777u) ? blockIdx.x : atomicAdd(ticket, 1u);  // 777: DEBUG static ids
   __syncthreads();
   const unsigned tile = s_tile;
   const size_t base = size_t(tile) * TILE;
@@ -154,42 +229,136 @@ scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsig
   const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
 
   if (warp == 0) {
-    T carry;
-    if (tile == 0) {
-      carry = exclusive ? init : ident;
-      if (lane == 0) st_state(state, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
-    } else {
-      if (lane == 0) st_state(state + tile, pack_state(epoch, 1u, to_bits(agg)));
-      carry = ident;
-      long long j = static_cast<long long>(tile) - 1;
-      while (true) {
-        const long long idx = j - lane;
-        unsigned st;
-        unsigned long long w = 0;
-        do {
-          if (idx >= 0) {
-            w = ld_state(state + idx);
-            st = (static_cast<uint32_t>(w >> 34) == epoch) ? static_cast<unsigned>(w >> 32) & 3u : 0u;
-          } else {
-            st = 2u;  // before the first tile: a virtual inclusive prefix equal to the identity
-          }
-        } while (__any_sync(FULL, st == 0u));
-        const T val = idx >= 0 ? from_bits<T>(static_cast<uint32_t>(w)) : ident;
-        const unsigned incl = __ballot_sync(FULL, st == 2u);
-        const int first = incl ? (__ffs(incl) - 1) : 32;
-        T contrib = lane <= first ? val : ident;
-        contrib = warp_reduce<T, OP>(contrib);
-        carry = op2<T, OP>(contrib, carry);
-        if (incl) break;
-        j -= 32;
-      }
-      if (lane == 0) st_state(state + tile, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
-    }
+    const T carry = lookback_warp0<T, OP>(state, epoch, tile, agg, init, exclusive != 0);
     if (lane == 0) s_carry = carry;
   }
   __syncthreads();
   tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
   if (threadIdx.x == 0 && tile == ntiles - 1) *ticket = 0u;  // every ticket has been drawn by now
+}
+
+// ---- single pass, thread-block clusters --------------------------------------------------------------
+// The look-back chain is paced by L2 round trips and by how many tiles poll it. Here CS CTAs of a
+// cluster scan CS consecutive tiles and exchange their aggregates through distributed shared
+// memory (a cluster barrier costs ~0.2 us, an L2 round trip ~0.7 us); only the cluster leader
+// takes a ticket and takes part in the global look-back, with the whole cluster's aggregate. The
+// global chain therefore has CS times fewer participants and advances CS times more data per step.
+namespace cg = cooperative_groups;
+
+template <typename T, int OP, int THREADS, int V, int U, int CS, bool NC>
+__global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(THREADS)
+scan_cluster_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, unsigned* ticket,
+                    uint32_t epoch, unsigned nctiles) {
+  static_assert(sizeof(T) == 4 && CS <= 32, "32-bit elements; cluster fits a warp");
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  __shared__ T sm[2 * E + 1];
+  __shared__ unsigned s_ctile;  // leader's copy is the cluster's
+  __shared__ T c_agg[CS];       // leader's copy: aggregate of every CTA of the cluster
+  __shared__ T c_carry;         // leader's copy: exclusive prefix of the cluster
+  __shared__ T s_carry;
+  cg::cluster_group cluster = cg::this_cluster();
+  const unsigned rank = cluster.block_rank();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const T ident = identity<T, OP>();
+
+  if (rank == 0 && threadIdx.x == 0) s_ctile = atomicAdd(ticket, 1u);
+  cluster.sync();
+  const unsigned ctile = *cluster.map_shared_rank(&s_ctile, 0);
+  const size_t base = (size_t(ctile) * CS + rank) * TILE;  // may lie past n: then every access is masked
+
+  TileRegs<T, V, U> R;
+  const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
+  if (threadIdx.x == 0) *cluster.map_shared_rank(&c_agg[rank], 0) = agg;
+  cluster.sync();
+  if (rank == 0 && warp == 0) {
+    T v = lane < CS ? c_agg[lane] : ident;
+    v = warp_reduce<T, OP>(v);
+    const T carry = lookback_warp0<T, OP>(state, epoch, ctile, v, init, exclusive != 0);
+    if (lane == 0) c_carry = carry;
+  }
+  cluster.sync();
+  if (threadIdx.x == 0) {
+    T c = *cluster.map_shared_rank(&c_carry, 0);
+    const T* aggs = cluster.map_shared_rank(&c_agg[0], 0);
+    for (unsigned r = 0; r < rank; ++r) c = op2<T, OP>(c, aggs[r]);
+    s_carry = c;
+  }
+  __syncthreads();
+  tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
+  if (rank == 0 && threadIdx.x == 0 && ctile == nctiles - 1) *ticket = 0u;
+  cluster.sync();  // the leader's shared memory must outlive the remote reads above
+}
+
+// ---- single pass, persistent CTAs fed by a ring of bulk async copies ------------------------------
+// Each CTA owns STAGES shared-memory tile buffers. One thread draws tile tickets ahead of time and
+// issues a bulk copy (TMA engine) per ticket; the copy signals an mbarrier. While a tile waits in
+// its look-back, the loads of the CTA's next STAGES-1 tiles are already in flight, so memory
+// latency is decoupled from the look-back chain. Tiles a CTA holds have increasing ids and are
+// processed in that order, so the smallest unfinished tile is always being worked on (forward
+// progress). The last CTA to leave resets the ticket and the exit counter.
+template <typename T, int OP, int THREADS, int V, int U, int STAGES>
+__global__ void __launch_bounds__(THREADS)
+scan_lookback_ring_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state,
+                          unsigned* ticket, uint32_t epoch, unsigned ntiles) {
+  static_assert(sizeof(T) == 4 && V == 4, "32-bit elements, 128-bit shared-memory reads");
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr int TILE = THREADS * V * U;
+  constexpr unsigned TILE_BYTES = TILE * 4u;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* buf = reinterpret_cast<T*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(STAGES) * TILE_BYTES);
+  unsigned* tile_of = reinterpret_cast<unsigned*>(full + STAGES);
+  T* sm = reinterpret_cast<T*>(tile_of + STAGES);
+  __shared__ T s_carry;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  (void)lane;
+
+  auto issue = [&](int s) {  // thread 0 only
+    const unsigned t = atomicAdd(ticket, 1u);
+    tile_of[s] = t;
+    if (t < ntiles && (size_t(t) + 1) * TILE <= n) {
+      mbar_arrive_expect_tx(&full[s], TILE_BYTES);
+      bulk_load(buf + size_t(s) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[s]);
+    } else {
+      mbar_arrive(&full[s]);  // ragged last tile (read directly) or past the end (sentinel)
+    }
+  };
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  if (threadIdx.x == 0)
+    for (int s = 0; s < STAGES; ++s) issue(s);
+
+  for (unsigned it = 0;; ++it) {
+    const int s = it % STAGES;
+    mbar_wait(&full[s], (it / STAGES) & 1u);
+    const unsigned tile = tile_of[s];
+    if (tile >= ntiles) break;
+    const size_t base = size_t(tile) * TILE;
+    const bool staged = base + TILE <= n;
+    TileRegs<T, V, U> R;
+    const T agg = tile_phase_a<T, OP, THREADS, V, U, false>(in, base, n, R, sm, staged ? buf + size_t(s) * TILE : nullptr);
+    // every thread has read tile_of[s] and its part of the buffer (two block barriers ago)
+    if (threadIdx.x == 0) issue(s);
+    if (warp == 0) {
+      const T carry = lookback_warp0<T, OP>(state, epoch, tile, agg, init, exclusive != 0);
+      if (threadIdx.x == 0) s_carry = carry;
+    }
+    __syncthreads();
+    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
+    __syncthreads();  // sm and s_carry are reused by the next tile
+  }
+  if (threadIdx.x == 0) {
+    const unsigned done = atomicAdd(ticket + 1, 1u);
+    if (done == gridDim.x - 1) {  // every CTA has drawn its last ticket
+      ticket[0] = 0u;
+      ticket[1] = 0u;
+    }
+  }
 }
 
 // ---- three kernels: block sums -> scan of block sums -> rescan --------------------------------
@@ -282,6 +451,16 @@ const ScanVariant kScanVariants[] = {
     {"lookback_256x8x4", true, 256, 8, 4},
     {"three_kernel_256x4x4", false, 256, 4, 4},
     {"three_kernel_256x1x4", false, 256, 1, 4},  // any alignment
+    {"ring_256x4x4_s4", true, 256, 4, 4},        // persistent CTAs + bulk-copy ring (16 KB tiles, 4 stages)
+    {"ring_256x4x8_s3", true, 256, 4, 8},        // 32 KB tiles, 3 stages
+    {"ring_512x4x4_s3", true, 512, 4, 4},        // 32 KB tiles, 3 stages, 512 threads
+    {"ring_512x4x4_s6", true, 512, 4, 4},        // 32 KB tiles, 6 stages, one CTA per SM
+    {"lookback_512x8x4", true, 512, 8, 4},       // 16384-element tiles
+    {"lookback_1024x8x2", true, 1024, 8, 2},     // 16384-element tiles, 1024 threads
+    {"cluster8_256x8x4", true, 256, 8, 4},       // clusters of 8 CTAs, DSMEM aggregate exchange
+    {"cluster8_256x4x4", true, 256, 4, 4},
+    {"cluster16_256x8x4", true, 256, 8, 4},      // non-portable cluster size 16
+    {"cluster8_512x8x2", true, 512, 8, 2},
 };
 constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
 
@@ -304,6 +483,64 @@ cudaError_t launch_lookback(const Launch& L, Scratch& S, bool exclusive, T init,
   else
     scan_lookback_kernel<T, OP, THREADS, V, U, false><<<(unsigned)ntiles, THREADS, 0, L.stream>>>(
         in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)ntiles);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T, int OP, int THREADS, int V, int U, int CS>
+cudaError_t launch_cluster(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  const size_t nctiles = (ntiles + CS - 1) / CS;
+  if (nctiles > S.scan_state_tiles || nctiles * CS > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++S.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.scan_epoch = 1;
+  }
+  const bool nc = static_cast<const void*>(in) != out;
+  auto kt = scan_cluster_kernel<T, OP, THREADS, V, U, CS, true>;
+  auto kf = scan_cluster_kernel<T, OP, THREADS, V, U, CS, false>;
+  if (CS > 8) {
+    static bool done = false;
+    if (!done) {
+      cudaFuncSetAttribute(kt, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+      cudaFuncSetAttribute(kf, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+      done = true;
+    }
+  }
+  const unsigned grid = (unsigned)(nctiles * CS);
+  if (nc) kt<<<grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)nctiles);
+  else kf<<<grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)nctiles);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T, int OP, int THREADS, int V, int U, int STAGES>
+cudaError_t launch_ring(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  constexpr int E = U * (THREADS / 32);
+  constexpr size_t smem = STAGES * TILE * 4 + STAGES * 8 + STAGES * 4 + (2 * E + 1) * 4 + 16;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++S.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.scan_epoch = 1;
+  }
+  auto kern = scan_lookback_ring_kernel<T, OP, THREADS, V, U, STAGES>;
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (ctas_per_sm < 1) return cudaErrorInvalidValue;
+  }
+  size_t grid = size_t(L.sms) * ctas_per_sm;  // all CTAs are co-resident (they wait on one another)
+  if (grid > ntiles) grid = ntiles;
+  kern<<<(unsigned)grid, THREADS, smem, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket,
+                                                    S.scan_epoch, (unsigned)ntiles);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -345,6 +582,16 @@ cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T
       case 1: return launch_lookback<T, OP, 256, 8, 2>(L, S, exclusive, init, in, out, n);
       case 2: return launch_lookback<T, OP, 512, 8, 2>(L, S, exclusive, init, in, out, n);
       case 3: return launch_lookback<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 6: return launch_ring<T, OP, 256, 4, 4, 4>(L, S, exclusive, init, in, out, n);
+      case 7: return launch_ring<T, OP, 256, 4, 8, 3>(L, S, exclusive, init, in, out, n);
+      case 8: return launch_ring<T, OP, 512, 4, 4, 3>(L, S, exclusive, init, in, out, n);
+      case 9: return launch_ring<T, OP, 512, 4, 4, 6>(L, S, exclusive, init, in, out, n);
+      case 10: return launch_lookback<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 11: return launch_lookback<T, OP, 1024, 8, 2>(L, S, exclusive, init, in, out, n);
+      case 12: return launch_cluster<T, OP, 256, 8, 4, 8>(L, S, exclusive, init, in, out, n);
+      case 13: return launch_cluster<T, OP, 256, 4, 4, 8>(L, S, exclusive, init, in, out, n);
+      case 14: return launch_cluster<T, OP, 256, 8, 4, 16>(L, S, exclusive, init, in, out, n);
+      case 15: return launch_cluster<T, OP, 512, 8, 2, 8>(L, S, exclusive, init, in, out, n);
     }
   }
   switch (v) {
@@ -374,7 +621,7 @@ bool scan_variant_ok(int v, int dtype, const void* in, const void* out, size_t) 
   const ScanVariant& sv = kScanVariants[v];
   if (sv.lookback && dtype != DT_I32) return false;
   const size_t a = size_t(sv.v) * 4;
-  return aligned_to(in, a) && aligned_to(out, a);
+  return aligned_to(in, a) && aligned_to(out, a);  // (16 bytes for the ring variants' bulk copies: V == 4)
 }
 
 // smallest tile of any look-back variant is 4096 elements
@@ -383,6 +630,13 @@ size_t scan_tiles_needed(size_t n) { return (n + 4095) / 4096 + 1; }
 cudaError_t launch_scan(const Launch& L, Scratch& S, int v, int dtype, int op, bool exclusive, uint32_t init_bits,
                         const void* in, void* out, size_t n) {
   if (n == 0) return cudaSuccess;
+  static bool delay_set = false;
+  if (!delay_set) {
+    const char* e = getenv("SKEL_SCAN_POLL_DELAY_NS");
+    const unsigned d = e ? (unsigned)atoi(e) : 0u;
+    cudaMemcpyToSymbol(c_poll_delay_ns, &d, sizeof(d));
+    delay_set = true;
+  }
   if (dtype == DT_F32) {
     float init = __builtin_bit_cast(float, init_bits);
     return launch_op<float>(L, S, v, op, exclusive, init, static_cast<const float*>(in), static_cast<float*>(out), n);

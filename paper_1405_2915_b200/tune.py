@@ -43,13 +43,19 @@ def main():
     ap.add_argument("--out", default=os.path.join(HERE, "plans", "b200.plan"))
     ap.add_argument("--reps", type=int, default=7)
     ap.add_argument("--tables", default=None, help="write the timing tables as JSON here")
+    ap.add_argument("--only", default=None, help="tune only the instances whose name contains this substring")
+    ap.add_argument("--base", default=None, help="start from this plan file (instances not tuned keep their entries)")
     args = ap.parse_args()
     sys.path.insert(0, os.path.dirname(HERE))
     from paper_1405_2915_b200 import skel as S
 
     ctx = S.Context()
+    if args.base and os.path.exists(args.base):
+        ctx.plan_load(args.base)
     tables = {}
     for name, inst, lo, hi, cols in instances(S):
+        if args.only and args.only not in name:
+            continue
         t = ctx.tune(inst, lo, hi, cols, args.reps)
         names = S.variant_names(inst.skeleton)
         tables[name] = {"variants": names, "log2_lo": lo, "us": [[None if x != x else round(float(x), 2) for x in row] for row in t]}
