@@ -145,6 +145,85 @@ overlap1d_tiled_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
   }
 }
 
+// ---- register window + warp shuffles (no shared memory, no block barrier) ---------------------
+// A thread owns 16 consecutive outputs: it fetches its own 16 inputs with two 256-bit loads (one
+// full 32-byte sector each, all issued before the first use, like the Map kernel) and gets the r
+// halo values on each side from the neighbouring lanes by shuffles; only lanes 0 and 31 read
+// their outer halo from memory (those lines are being fetched by the neighbouring warp anyway).
+template <int R>
+__global__ void __launch_bounds__(T1_THREADS)
+overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
+                      size_t rows, size_t cols) {
+  constexpr int O = 16;
+  constexpr int TILE = T1_THREADS * O;
+  static_assert(R >= 1 && R <= O, "halo comes from the direct neighbours only");
+  const int lane = threadIdx.x & 31;
+  const size_t tiles_per_row = (cols + TILE - 1) / TILE;
+  const size_t ntiles = rows * tiles_per_row;
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t row = tile / tiles_per_row;
+    const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE) + threadIdx.x * O;
+    const float* x = in + row * cols;
+    const long long lc = static_cast<long long>(cols);
+    float win[O + 2 * R];
+    if (c0 + O <= lc) {
+      uint32_t a[8], b[8];
+      ld_stream<8, true>(a, x + c0);
+      ld_stream<8, true>(b, x + c0 + 8);
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { win[R + j] = __uint_as_float(a[j]); win[R + 8 + j] = __uint_as_float(b[j]); }
+    } else {
+#pragma unroll
+      for (int j = 0; j < O; ++j) win[R + j] = ext_row(x, lc, c0 + j, edge, pad);
+    }
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+      const float l = __shfl_up_sync(0xffffffffu, win[R + O - R + j], 1);
+      const float r = __shfl_down_sync(0xffffffffu, win[R + j], 1);
+      win[j] = l;
+      win[R + O + j] = r;
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) win[j] = ext_row(x, lc, c0 - R + j, edge, pad);
+    }
+    if (lane == 31) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) win[R + O + j] = ext_row(x, lc, c0 + O + j, edge, pad);
+    }
+    float acc[O];
+#pragma unroll
+    for (int o = 0; o < O; ++o) acc[o] = 0.f;
+#pragma unroll
+    for (int k = 0; k <= 2 * R; ++k)
+#pragma unroll
+      for (int o = 0; o < O; ++o) acc[o] = fmaf(W.w[k], win[o + k], acc[o]);
+    if (c0 + O <= lc) {
+      float* dst = out + row * cols + c0;
+      uint32_t r0[8], r1[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { r0[e] = __float_as_uint(acc[e]); r1[e] = __float_as_uint(acc[8 + e]); }
+      st_stream<8>(dst, r0);
+      st_stream<8>(dst + 8, r1);
+    } else {
+#pragma unroll
+      for (int o = 0; o < O; ++o)
+        if (c0 + o < lc) out[row * cols + c0 + o] = acc[o];
+    }
+  }
+}
+
+template <int R>
+cudaError_t launch_shfl(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
+                        size_t rows, size_t cols) {
+  constexpr int TILE = T1_THREADS * 16;
+  const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
+  const size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
+  overlap1d_shfl_kernel<R><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
 template <int O> constexpr size_t tiled_smem_bytes(int R) {
   const int HP = (R + 3) / 4 * 4;
   const int span = T1_THREADS * O + 2 * HP;
@@ -152,7 +231,7 @@ template <int O> constexpr size_t tiled_smem_bytes(int R) {
 }
 
 struct O1Variant { const char* name; int o; };  // o == 0: direct
-const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}};
+const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16}};
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
@@ -197,7 +276,7 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
   if (v < 0 || v >= kNumVariants) return false;
   if (kVariants[v].o == 0) return true;
   if (!templated_radius(r)) return false;
-  const bool al = reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
+  const bool al = reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
   return al && (rows == 1 || cols % 8 == 0);
 }
 
@@ -217,6 +296,16 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 4: return launch_tiled_r<4>(L, w, r, edge, pad, in, out, rows, cols);
     case 8: return launch_tiled_r<8>(L, w, r, edge, pad, in, out, rows, cols);
     case 16: return launch_tiled_r<16>(L, w, r, edge, pad, in, out, rows, cols);
+    case -16:
+      switch (r) {
+        case 1: return launch_shfl<1>(L, w, edge, pad, in, out, rows, cols);
+        case 2: return launch_shfl<2>(L, w, edge, pad, in, out, rows, cols);
+        case 3: return launch_shfl<3>(L, w, edge, pad, in, out, rows, cols);
+        case 4: return launch_shfl<4>(L, w, edge, pad, in, out, rows, cols);
+        case 8: return launch_shfl<8>(L, w, edge, pad, in, out, rows, cols);
+        case 16: return launch_shfl<16>(L, w, edge, pad, in, out, rows, cols);
+      }
+      return cudaErrorInvalidValue;
   }
   return cudaErrorInvalidValue;
 }

@@ -149,7 +149,6 @@ __device__ __forceinline__ unsigned long long pack_state(uint32_t epoch, unsigne
 // Look-back of one tile, executed by warp 0 (all 32 lanes). Publishes the tile's aggregate, folds
 // the predecessors' aggregates back to the nearest inclusive prefix, publishes the tile's inclusive
 // prefix and returns the tile's exclusive prefix (carry).
-__constant__ unsigned c_poll_delay_ns = 0;  // back-off between polls of unpublished tile states
 
 template <typename T, int OP>
 __device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t epoch, unsigned tile, T agg, T init,
@@ -164,7 +163,6 @@ __device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t 
   }
   if (lane == 0) st_state(state + tile, pack_state(epoch, 1u, to_bits(agg)));
   carry = ident;
-  if (c_poll_delay_ns == 12345u) return carry;  // DEBUG experiment: skip the look-back (wrong results)
   // The inclusive-prefix frontier advances by at most one look-back window per L2 round trip, so
   // the window decides the chain speed: LB_WINDOWS * 32 predecessor states are fetched per round
   // (independent loads in flight together) and folded nearest-first.
@@ -202,7 +200,6 @@ __device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t 
     }
     if (done) break;
     j -= 32 * consumed;
-    if (consumed == 0 && c_poll_delay_ns) __nanosleep(c_poll_delay_ns);
   }
   if (lane == 0) st_state(state + tile, pack_state(epoch, 2u, to_bits(op2<T, OP>(carry, agg))));
   return carry;
@@ -220,7 +217,7 @@ scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsig
   __shared__ T s_carry;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-  if (threadIdx.x == 0) s_tile = (c_poll_delay_ns == 777u) ? blockIdx.x : atomicAdd(ticket, 1u);  // 777: DEBUG static ids
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
   __syncthreads();
   const unsigned tile = s_tile;
   const size_t base = size_t(tile) * TILE;
@@ -235,6 +232,31 @@ scan_lookback_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsig
   __syncthreads();
   tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
   if (threadIdx.x == 0 && tile == ntiles - 1) *ticket = 0u;  // every ticket has been drawn by now
+}
+
+// Persistent form: a grid of co-resident blocks, block b scans tiles b, b+G, b+2G, ... in that
+// order (ids grow inside a block, so the smallest unfinished tile is always being worked on).
+template <typename T, int OP, int THREADS, int V, int U, bool NC>
+__global__ void __launch_bounds__(THREADS)
+scan_lookback_persist_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state,
+                             uint32_t epoch, unsigned ntiles) {
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  __shared__ T sm[2 * E + 1];
+  __shared__ T s_carry;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (unsigned tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t base = size_t(tile) * TILE;
+    TileRegs<T, V, U> R;
+    const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
+    if (warp == 0) {
+      const T carry = lookback_warp0<T, OP>(state, epoch, tile, agg, init, exclusive != 0);
+      if (lane == 0) s_carry = carry;
+    }
+    __syncthreads();
+    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
+    __syncthreads();
+  }
 }
 
 // ---- single pass, thread-block clusters --------------------------------------------------------------
@@ -461,6 +483,9 @@ const ScanVariant kScanVariants[] = {
     {"cluster8_256x4x4", true, 256, 4, 4},
     {"cluster16_256x8x4", true, 256, 8, 4},      // non-portable cluster size 16
     {"cluster8_512x8x2", true, 512, 8, 2},
+    {"persist_256x8x4", true, 256, 8, 4},        // persistent blocks, strided tiles, no ticket
+    {"persist_256x4x4", true, 256, 4, 4},
+    {"persist_512x8x4", true, 512, 8, 4},
 };
 constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
 
@@ -483,6 +508,32 @@ cudaError_t launch_lookback(const Launch& L, Scratch& S, bool exclusive, T init,
   else
     scan_lookback_kernel<T, OP, THREADS, V, U, false><<<(unsigned)ntiles, THREADS, 0, L.stream>>>(
         in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)ntiles);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T, int OP, int THREADS, int V, int U>
+cudaError_t launch_persist(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++S.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.scan_epoch = 1;
+  }
+  auto kt = scan_lookback_persist_kernel<T, OP, THREADS, V, U, true>;
+  auto kf = scan_lookback_persist_kernel<T, OP, THREADS, V, U, false>;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kf, THREADS, 0);
+    if (e != cudaSuccess || per_sm < 1) return cudaErrorInvalidValue;
+  }
+  size_t grid = size_t(L.sms) * per_sm;
+  if (grid > ntiles) grid = ntiles;
+  const bool nc = static_cast<const void*>(in) != out;
+  if (nc) kt<<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_epoch, (unsigned)ntiles);
+  else kf<<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_epoch, (unsigned)ntiles);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -592,6 +643,9 @@ cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T
       case 13: return launch_cluster<T, OP, 256, 4, 4, 8>(L, S, exclusive, init, in, out, n);
       case 14: return launch_cluster<T, OP, 256, 8, 4, 16>(L, S, exclusive, init, in, out, n);
       case 15: return launch_cluster<T, OP, 512, 8, 2, 8>(L, S, exclusive, init, in, out, n);
+      case 16: return launch_persist<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 17: return launch_persist<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
+      case 18: return launch_persist<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
     }
   }
   switch (v) {
@@ -630,13 +684,6 @@ size_t scan_tiles_needed(size_t n) { return (n + 4095) / 4096 + 1; }
 cudaError_t launch_scan(const Launch& L, Scratch& S, int v, int dtype, int op, bool exclusive, uint32_t init_bits,
                         const void* in, void* out, size_t n) {
   if (n == 0) return cudaSuccess;
-  static bool delay_set = false;
-  if (!delay_set) {
-    const char* e = getenv("SKEL_SCAN_POLL_DELAY_NS");
-    const unsigned d = e ? (unsigned)atoi(e) : 0u;
-    cudaMemcpyToSymbol(c_poll_delay_ns, &d, sizeof(d));
-    delay_set = true;
-  }
   if (dtype == DT_F32) {
     float init = __builtin_bit_cast(float, init_bits);
     return launch_op<float>(L, S, v, op, exclusive, init, static_cast<const float*>(in), static_cast<float*>(out), n);
