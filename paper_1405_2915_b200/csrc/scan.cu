@@ -150,7 +150,7 @@ __device__ __forceinline__ unsigned long long pack_state(uint32_t epoch, unsigne
 // the predecessors' aggregates back to the nearest inclusive prefix, publishes the tile's inclusive
 // prefix and returns the tile's exclusive prefix (carry).
 
-template <typename T, int OP>
+template <typename T, int OP, int K = LB_WINDOWS>
 __device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t epoch, unsigned tile, T agg, T init,
                                             bool exclusive) {
   const int lane = threadIdx.x & 31;
@@ -166,7 +166,6 @@ __device__ __forceinline__ T lookback_warp0(unsigned long long* state, uint32_t 
   // The inclusive-prefix frontier advances by at most one look-back window per L2 round trip, so
   // the window decides the chain speed: LB_WINDOWS * 32 predecessor states are fetched per round
   // (independent loads in flight together) and folded nearest-first.
-  constexpr int K = LB_WINDOWS;
   long long j = static_cast<long long>(tile) - 1;
   while (true) {
     unsigned long long w[K];
@@ -383,6 +382,219 @@ scan_lookback_ring_kernel(const T* in, T* out, size_t n, T init, int exclusive, 
   }
 }
 
+// ---- single pass, persistent CTAs, STATIC strided tiles fed by a ring of bulk async copies ----------
+// CTA b scans tiles b, b+G, b+2G, ... (G = gridDim.x, all CTAs co-resident). Because the tiles of
+// a CTA are known in advance, one thread keeps STAGES bulk copies (TMA engine) in flight per CTA:
+// the load stream never stops while a tile sits in its look-back, which is what bounds the plain
+// one-tile-per-block kernel (loads are only in flight during ~1/3 of a block's life time).
+// Unlike the ticket ring above, tile t-1 is processed by CTA b-1 in the SAME iteration, so its
+// aggregate never queues behind another tile's look-back: the dependence depth is the iteration
+// count, as in the non-ring kernels. Forward progress: tile t waits only on tiles < t, which are
+// held by co-resident CTAs at the same or an earlier iteration (induction on t); the launch is a
+// cooperative one, so co-residency is guaranteed by the driver, not assumed.
+template <typename T, int OP, int THREADS, int V, int U, int STAGES>
+__global__ void __launch_bounds__(THREADS)
+scan_sring_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, uint32_t epoch,
+                  unsigned ntiles) {
+  static_assert(sizeof(T) == 4 && V == 4, "32-bit elements, 128-bit shared-memory reads");
+  constexpr int NW = THREADS / 32, E = U * NW;
+  constexpr int TILE = THREADS * V * U;
+  constexpr unsigned TILE_BYTES = TILE * 4u;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* buf = reinterpret_cast<T*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(STAGES) * TILE_BYTES);
+  T* sm = reinterpret_cast<T*>(full + STAGES);
+  __shared__ T s_carry;
+  const int warp = threadIdx.x >> 5;
+  const unsigned G = gridDim.x;
+
+  auto issue = [&](int s, unsigned long long t) {  // thread 0 only
+    if (t >= ntiles) return;                        // never waited for
+    if ((t + 1) * TILE <= n) {
+      mbar_arrive_expect_tx(&full[s], TILE_BYTES);
+      bulk_load(buf + size_t(s) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[s]);
+    } else {
+      mbar_arrive(&full[s]);  // ragged last tile: read directly with guarded loads
+    }
+  };
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+    mbar_fence_init();
+    for (int s = 0; s < STAGES; ++s) issue(s, blockIdx.x + (unsigned long long)s * G);
+  }
+  __syncthreads();
+
+  unsigned it = 0;
+  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+    const int s = it % STAGES;
+    mbar_wait(&full[s], (it / STAGES) & 1u);
+    const size_t base = size_t(tile) * TILE;
+    const bool staged = base + TILE <= n;
+    TileRegs<T, V, U> R;
+    const T agg = tile_phase_a<T, OP, THREADS, V, U, false>(in, base, n, R, sm, staged ? buf + size_t(s) * TILE : nullptr);
+    // every thread has copied its part of buffer s into registers (two block barriers ago)
+    if (threadIdx.x == 0) issue(s, tile + (unsigned long long)STAGES * G);
+    if (warp == 0) {
+      const T carry = lookback_warp0<T, OP>(state, epoch, (unsigned)tile, agg, init, exclusive != 0);
+      if (threadIdx.x == 0) s_carry = carry;
+    }
+    __syncthreads();
+    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
+    __syncthreads();  // sm and s_carry are reused by the next tile
+  }
+}
+
+// ---- single pass, warp-specialised persistent CTAs ("ws") ------------------------------------------
+// Measured on B200 (profiles/r01_scan_probe.txt): in the one-tile-per-block kernel a tile spends
+// ~2/3 of its life spinning in the look-back, not because the chain is long but because the load
+// latency under a saturated HBM has a heavy tail (p50 2.5 us, p99 7 us) and a tile's aggregate is
+// only published once ITS loads have landed; every later tile waits for the slowest earlier one,
+// and while it waits its registers hold no loads in flight. The same kernel without the look-back
+// runs at copy speed. This kernel takes the look-back off the data path:
+//  * CTA b owns tiles b, b+G, b+2G, ... (static; cooperative launch => all CTAs co-resident).
+//  * A ring of S shared-memory stages per CTA is filled by bulk async copies (TMA engine), so up to
+//    S tiles per SM are in flight or waiting no matter what the look-back does.
+//  * Stage s has its own PREFIX WARP: as soon as the tile lands it sums the NSW sub-tiles, publishes
+//    the tile aggregate (so successors never wait for more than the landing itself), runs the
+//    look-back, publishes the inclusive prefix and hands carry + sub-tile prefixes to the scanners
+//    through shared memory. The S prefix warps run concurrently, so one slow look-back delays
+//    neither the aggregates nor the look-backs of the CTA's other staged tiles.
+//  * NSW SCANNER WARPS take the stages in order; warp w scans sub-tile w (32*4*U elements) from
+//    shared memory with no block-level barrier, adds carry + sub-tile prefix, and streams the
+//    result to global memory with 128-bit stores; then the stage is handed back for the next copy.
+// Forward progress: tile t depends only on tiles < t, which belong to co-resident CTAs at the same
+// or an earlier ring position; aggregates depend on nothing but the copy.
+template <typename T, int OP, int NSW, int U, int S, int K>
+__global__ void __launch_bounds__((NSW + S) * 32, 1)
+scan_ws_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, uint32_t epoch,
+               unsigned ntiles) {
+  static_assert(sizeof(T) == 4 && NSW <= 32, "32-bit elements");
+  constexpr int SUB = 32 * 4 * U;       // elements per scanner warp and tile
+  constexpr int TILE = NSW * SUB;
+  constexpr unsigned TILE_BYTES = TILE * 4u;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* buf = reinterpret_cast<T*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(S) * TILE_BYTES);  // copy landed
+  uint64_t* ready = full + S;                                                       // prefixes written
+  uint64_t* empty = ready + S;                                                      // scanners done reading
+  T* pre = reinterpret_cast<T*>(empty + S);                                         // [S][NSW] carry (+) sub-tile prefix
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned G = gridDim.x;
+  const T ident = identity<T, OP>();
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < S; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&ready[s], 1);
+      mbar_init(&empty[s], NSW);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (warp >= NSW) {
+    // ---------------- prefix warp of stage s ----------------
+    const int s = warp - NSW;
+    T* stage = buf + size_t(s) * TILE;
+    unsigned use = 0;
+    for (unsigned long long tile = blockIdx.x + (unsigned long long)s * G; tile < ntiles; tile += (unsigned long long)S * G, ++use) {
+      const size_t base = size_t(tile) * TILE;
+      const bool whole = base + TILE <= n;
+      if (use > 0) mbar_wait(&empty[s], (use - 1) & 1u);
+      if (whole) {
+        if (lane == 0) {
+          mbar_arrive_expect_tx(&full[s], TILE_BYTES);
+          bulk_load(stage, in + base, TILE_BYTES, &full[s]);
+        }
+      } else {  // ragged last tile: guarded copy, identity padding
+        for (int i = lane; i < TILE; i += 32) stage[i] = (base + i < n) ? in[base + i] : ident;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[s]);
+      }
+      mbar_wait(&full[s], use & 1u);
+      // sub-tile sums (same striped layout as the scanners: conflict-free 128-bit reads)
+      T sub = ident;  // lane w < NSW ends up holding the sum of sub-tile w
+#pragma unroll
+      for (int w = 0; w < NSW; ++w) {
+        T a = ident;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+          const uint4 q = *reinterpret_cast<const uint4*>(stage + w * SUB + (u * 32 + lane) * 4);
+          a = op2<T, OP>(a, op2<T, OP>(op2<T, OP>(from_bits<T>(q.x), from_bits<T>(q.y)),
+                                       op2<T, OP>(from_bits<T>(q.z), from_bits<T>(q.w))));
+        }
+        a = warp_reduce<T, OP>(a);
+        if (lane == w) sub = a;
+      }
+      // exclusive prefix of the sub-tile sums over lanes 0..NSW-1, and the tile aggregate
+      T inc = sub;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        T y = __shfl_up_sync(FULL, inc, o);
+        if (lane >= o) inc = op2<T, OP>(y, inc);
+      }
+      T exc = __shfl_up_sync(FULL, inc, 1);
+      if (lane == 0) exc = ident;
+      const T agg = __shfl_sync(FULL, inc, NSW - 1);
+      const T carry = lookback_warp0<T, OP, K>(state, epoch, (unsigned)tile, agg, init, exclusive != 0);
+      if (lane < NSW) pre[s * NSW + lane] = op2<T, OP>(carry, exc);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&ready[s]);
+    }
+  } else {
+    // ---------------- scanner warp `warp`: sub-tile `warp` of every tile of this CTA ----------------
+    unsigned it = 0;
+    for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+      const int s = it % S;
+      const unsigned use = it / S;
+      const T* stage = buf + size_t(s) * TILE + warp * SUB;
+      mbar_wait(&ready[s], use & 1u);
+      const T p0 = pre[s * NSW + warp];
+      T x[U][4];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const uint4 q = *reinterpret_cast<const uint4*>(stage + (u * 32 + lane) * 4);
+        x[u][0] = from_bits<T>(q.x); x[u][1] = from_bits<T>(q.y); x[u][2] = from_bits<T>(q.z); x[u][3] = from_bits<T>(q.w);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);  // the stage may be refilled
+      const size_t base = size_t(tile) * TILE + size_t(warp) * SUB;
+      T run = p0;  // exclusive prefix of vector-row u of this sub-tile
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+#pragma unroll
+        for (int j = 1; j < 4; ++j) x[u][j] = op2<T, OP>(x[u][j - 1], x[u][j]);
+        T ws = x[u][3];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          T y = __shfl_up_sync(FULL, ws, o);
+          if (lane >= o) ws = op2<T, OP>(y, ws);
+        }
+        T ex = __shfl_up_sync(FULL, ws, 1);
+        const T p = lane == 0 ? run : op2<T, OP>(run, ex);
+        run = op2<T, OP>(run, __shfl_sync(FULL, ws, 31));
+        T o4[4];
+        if (exclusive) {
+          o4[0] = p; o4[1] = op2<T, OP>(p, x[u][0]); o4[2] = op2<T, OP>(p, x[u][1]); o4[3] = op2<T, OP>(p, x[u][2]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) o4[j] = op2<T, OP>(p, x[u][j]);
+        }
+        const size_t i0 = base + (size_t(u) * 32 + lane) * 4;
+        if (i0 + 4 <= n) {
+          uint32_t raw[4] = {to_bits(o4[0]), to_bits(o4[1]), to_bits(o4[2]), to_bits(o4[3])};
+          st_stream<4>(out + i0, raw);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            if (i0 + j < n) out[i0 + j] = o4[j];
+        }
+      }
+    }
+  }
+}
+
 // ---- three kernels: block sums -> scan of block sums -> rescan --------------------------------
 template <typename T, int OP, int THREADS, int V, int U>
 __global__ void __launch_bounds__(THREADS)
@@ -486,6 +698,20 @@ const ScanVariant kScanVariants[] = {
     {"persist_256x8x4", true, 256, 8, 4},        // persistent blocks, strided tiles, no ticket
     {"persist_256x4x4", true, 256, 4, 4},
     {"persist_512x8x4", true, 512, 8, 4},
+    {"sring_256x4x4_s3", true, 256, 4, 4},       // static strided tiles + bulk-copy ring: 16 KB tiles, 3 stages
+    {"sring_256x4x8_s2", true, 256, 4, 8},       // 32 KB tiles, 2 stages
+    {"sring_512x4x4_s2", true, 512, 4, 4},       // 32 KB tiles, 2 stages, 512 threads
+    {"sring_256x4x4_s2", true, 256, 4, 4},       // 16 KB tiles, 2 stages
+    {"sring_512x4x4_s3", true, 512, 4, 4},       // 32 KB tiles, 3 stages
+    {"sring_128x4x8_s3", true, 128, 4, 8},       // 16 KB tiles, 128 threads, 3 stages
+    {"ws_8w_u8_s6_k2", true, 256, 4, 8},         // warp-specialised: 32 KB tiles, 6 stages, 1 CTA/SM
+    {"ws_8w_u8_s3_k2", true, 256, 4, 8},         // 32 KB tiles, 3 stages, 2 CTAs/SM
+    {"ws_8w_u4_s6_k2", true, 256, 4, 4},         // 16 KB tiles, 6 stages, 2 CTAs/SM
+    {"ws_8w_u8_s6_k1", true, 256, 4, 8},
+    {"ws_8w_u8_s6_k4", true, 256, 4, 8},
+    {"ws_8w_u12_s4_k2", true, 256, 4, 12},       // 48 KB tiles, 4 stages
+    {"ws_16w_u4_s6_k2", true, 512, 4, 4},        // 32 KB tiles, 16 scanner warps
+    {"ws_4w_u8_s6_k2", true, 128, 4, 8},         // 16 KB tiles, 4 scanner warps, 2 CTAs/SM
 };
 constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
 
@@ -596,6 +822,75 @@ cudaError_t launch_ring(const Launch& L, Scratch& S, bool exclusive, T init, con
   return cudaGetLastError();
 }
 
+template <typename T, int OP, int THREADS, int V, int U, int STAGES>
+cudaError_t launch_sring(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(THREADS) * V * U;
+  constexpr int E = U * (THREADS / 32);
+  constexpr size_t smem = STAGES * TILE * 4 + STAGES * 8 + (2 * E + 1) * 4 + 16;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++S.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.scan_epoch = 1;
+  }
+  auto kern = scan_sring_kernel<T, OP, THREADS, V, U, STAGES>;
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per < 1) return cudaErrorInvalidValue;
+    ctas_per_sm = per;
+  }
+  size_t grid = size_t(L.sms) * ctas_per_sm;
+  if (grid > ntiles) grid = ntiles;
+  int excl = exclusive ? 1 : 0;
+  uint32_t epoch = S.scan_epoch;
+  unsigned nt = (unsigned)ntiles;
+  void* args[] = {&in, &out, &n, &init, &excl, &S.scan_state, &epoch, &nt};
+  // cooperative launch: the driver guarantees that all CTAs are co-resident (they wait on one another)
+  cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3((unsigned)grid), dim3(THREADS), args, smem, L.stream);
+  ++*L.launches;
+  return e;
+}
+
+template <typename T, int OP, int NSW, int U, int S, int K>
+cudaError_t launch_ws(const Launch& L, Scratch& Sc, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(NSW) * 32 * 4 * U;
+  constexpr int THREADS = (NSW + S) * 32;
+  constexpr size_t smem = S * TILE * 4 + 3 * S * 8 + S * NSW * 4 + 16;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > Sc.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++Sc.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(Sc.scan_state, 0, Sc.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    Sc.scan_epoch = 1;
+  }
+  auto kern = scan_ws_kernel<T, OP, NSW, U, S, K>;
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per < 1) return cudaErrorInvalidValue;
+    ctas_per_sm = per;
+  }
+  size_t grid = size_t(L.sms) * ctas_per_sm;
+  if (grid > ntiles) grid = ntiles;
+  int excl = exclusive ? 1 : 0;
+  uint32_t epoch = Sc.scan_epoch;
+  unsigned nt = (unsigned)ntiles;
+  void* args[] = {&in, &out, &n, &init, &excl, &Sc.scan_state, &epoch, &nt};
+  cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3((unsigned)grid), dim3(THREADS), args, smem, L.stream);
+  ++*L.launches;
+  return e;
+}
+
 template <typename T, int OP, int THREADS, int V, int U>
 cudaError_t launch_three(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
   constexpr size_t TILE = size_t(THREADS) * V * U;
@@ -646,6 +941,20 @@ cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T
       case 16: return launch_persist<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
       case 17: return launch_persist<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
       case 18: return launch_persist<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 19: return launch_sring<T, OP, 256, 4, 4, 3>(L, S, exclusive, init, in, out, n);
+      case 20: return launch_sring<T, OP, 256, 4, 8, 2>(L, S, exclusive, init, in, out, n);
+      case 21: return launch_sring<T, OP, 512, 4, 4, 2>(L, S, exclusive, init, in, out, n);
+      case 22: return launch_sring<T, OP, 256, 4, 4, 2>(L, S, exclusive, init, in, out, n);
+      case 23: return launch_sring<T, OP, 512, 4, 4, 3>(L, S, exclusive, init, in, out, n);
+      case 24: return launch_sring<T, OP, 128, 4, 8, 3>(L, S, exclusive, init, in, out, n);
+      case 25: return launch_ws<T, OP, 8, 8, 6, 2>(L, S, exclusive, init, in, out, n);
+      case 26: return launch_ws<T, OP, 8, 8, 3, 2>(L, S, exclusive, init, in, out, n);
+      case 27: return launch_ws<T, OP, 8, 4, 6, 2>(L, S, exclusive, init, in, out, n);
+      case 28: return launch_ws<T, OP, 8, 8, 6, 1>(L, S, exclusive, init, in, out, n);
+      case 29: return launch_ws<T, OP, 8, 8, 6, 4>(L, S, exclusive, init, in, out, n);
+      case 30: return launch_ws<T, OP, 8, 12, 4, 2>(L, S, exclusive, init, in, out, n);
+      case 31: return launch_ws<T, OP, 16, 4, 6, 2>(L, S, exclusive, init, in, out, n);
+      case 32: return launch_ws<T, OP, 4, 8, 6, 2>(L, S, exclusive, init, in, out, n);
     }
   }
   switch (v) {
