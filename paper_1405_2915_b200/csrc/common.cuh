@@ -65,6 +65,30 @@ __device__ __forceinline__ void st_stream(void* p, const uint32_t (&r)[V]) {
     asm volatile("st.global.L1::no_allocate.b32 [%0], %1;" ::"l"(p), "r"(r[0]) : "memory");
 }
 
+// ---- 128-bit global accesses with an L2 eviction-priority policy ---------------------------------
+// evict_last: "I will read this line again soon" (kept in L2); evict_first: touch-once streaming.
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+  uint64_t p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void ld_hint4(uint32_t (&r)[4], const void* p, uint64_t policy) {
+  asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.b32 {%0,%1,%2,%3}, [%4], %5;"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "l"(p), "l"(policy)
+               : "memory");
+}
+__device__ __forceinline__ void st_hint4(void* p, const uint32_t (&r)[4], uint64_t policy) {
+  asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.b32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "r"(r[0]), "r"(r[1]),
+               "r"(r[2]), "r"(r[3]), "l"(policy)
+               : "memory");
+}
+
 // ---- mbarrier + bulk async copy (TMA engine, 1-D form; SASS: UBLKCP / SYNCS) ---------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
@@ -97,6 +121,15 @@ __device__ __forceinline__ void bulk_load(void* smem_dst, const void* gsrc, unsi
                    smem_u32(smem_dst)),
                "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
+}
+
+// the same with an L2 eviction-priority policy (createpolicy)
+__device__ __forceinline__ void bulk_load_hint(void* smem_dst, const void* gsrc, unsigned bytes, uint64_t* bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
 }
 
 // ---- bit casts between the 32-bit register image and the element type ---------------------------

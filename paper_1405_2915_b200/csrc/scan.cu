@@ -595,6 +595,241 @@ scan_ws_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned lo
   }
 }
 
+// ---- single pass over HBM, two passes over L2 ("l2ahead") --------------------------------------------
+// What bounds every chained single-pass kernel above on B200 is not the chain arithmetic but the
+// load-latency tail of a saturated HBM (profiles/r01_scan_probe.txt: p50 2.5 us, p99 7 us, max ~10
+// us): tile t cannot be finished before every earlier tile has LANDED, so each slot of on-chip
+// buffering is held for the tail latency, not the mean, and 192 KB of shared memory per SM is not
+// enough buffer. Here the buffer is the 126 MB L2 and there is no chain at all:
+//  * CTA b owns tiles b, b+G, b+2G, ... (static; cooperative launch => all CTAs co-resident).
+//  * REDUCE phase (worker warps): tile k+D is streamed once from HBM (loads tagged L2::evict_last),
+//    summed, and its aggregate published. Order-free, never waits.
+//  * PREFIX warp (one per CTA, runs ahead of the scan phase): the exclusive prefix of the CTA's
+//    next tile is the prefix of its previous tile (+) the G consecutive aggregates in between - a
+//    windowed sum over already-published aggregates (all loads of a window in flight together), no
+//    look-back chain, no inclusive prefixes to publish. It hands the carry to the workers through a
+//    small shared-memory queue.
+//  * SCAN phase (worker warps): tile k is read a second time - now from L2 (evict_first, like the
+//    output stores) - scanned locally, offset by the carry and streamed out.
+// HBM traffic stays 8 B/elem; L2 carries 12 B/elem (+ G*8 B of aggregate reads per tile), which it
+// sustains (profiles/r01_l2_probe.txt). Run-ahead = D*G tiles. Forward progress: the reduce phase
+// waits for nothing; a prefix waits only for aggregates, i.e. for reduce phases.
+template <int N> __device__ __forceinline__ void bar_workers() { asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ unsigned ld_acquire_shared(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_shared(unsigned* p, unsigned v) {
+  asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+
+template <typename T, int OP, int NW, int U, int D, int KW, int S, int MINB>
+__global__ void __launch_bounds__((NW + 1) * 32, MINB)
+scan_l2_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, uint32_t epoch,
+               unsigned ntiles) {
+  static_assert(sizeof(T) == 4, "32-bit elements");
+  constexpr int V = 4, WT = NW * 32, E = U * NW, Q = D + 2;
+  constexpr size_t TILE = size_t(WT) * V * U;
+  __shared__ T sm[2 * E + 1];
+  __shared__ T red[2][NW];
+  __shared__ T cq[Q];
+  __shared__ unsigned cq_head, cq_tail;  // carries produced / consumed
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned long long G = gridDim.x;
+  const T ident = identity<T, OP>();
+  if (threadIdx.x == 0) {
+    cq_head = 0;
+    cq_tail = 0;
+  }
+  __syncthreads();
+
+  if (warp == NW) {
+    // ---------------- prefix warp ----------------
+    T carry = exclusive ? init : ident;
+    unsigned long long lo = 0;
+    unsigned j = 0;
+    for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++j) {
+      // carry(tile) = carry(previous own tile) (+) aggregates of tiles [lo, tile)
+      T acc = ident;
+      for (unsigned long long c0 = lo; c0 < tile; c0 += 32ull * KW) {
+        bool pending = true;
+        unsigned long long w[KW];
+        while (pending) {
+          pending = false;
+#pragma unroll
+          for (int k = 0; k < KW; ++k) {
+            const unsigned long long idx = c0 + 32ull * k + lane;
+            w[k] = idx < tile ? ld_state(state + idx) : pack_state(epoch, 1u, to_bits(ident));
+          }
+#pragma unroll
+          for (int k = 0; k < KW; ++k) pending |= static_cast<uint32_t>(w[k] >> 34) != epoch;
+          pending = __any_sync(FULL, pending);
+        }
+#pragma unroll
+        for (int k = 0; k < KW; ++k) acc = op2<T, OP>(acc, from_bits<T>(static_cast<uint32_t>(w[k])));
+      }
+      carry = op2<T, OP>(carry, warp_reduce<T, OP>(acc));
+      lo = tile;
+      while (j - ld_acquire_shared(&cq_tail) >= unsigned(Q)) {}  // queue full: wait for the workers
+      if (lane == 0) {
+        cq[j % Q] = carry;
+        st_release_shared(&cq_head, j + 1);
+      }
+      __syncwarp();
+    }
+    return;
+  }
+
+  // ---------------- worker warps ----------------
+  // The reduce pass is fed by a ring of S bulk async copies (TMA engine, L2::evict_last), so the HBM
+  // stream runs S tiles ahead of the reduce, which runs D tiles ahead of the scan.
+  constexpr unsigned TILE_BYTES = unsigned(TILE) * 4u;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  T* ring = reinterpret_cast<T*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(S) * TILE_BYTES);
+  const uint64_t keep = l2_policy_evict_last(), stream = l2_policy_evict_first();
+  auto red_tile = [&](unsigned j) { return blockIdx.x + (unsigned long long)j * G; };
+  auto issue = [&](unsigned j) {  // thread 0: arm stage j % S with reduce-tile j (whole tiles only)
+    const unsigned long long t = red_tile(j);
+    if (t < ntiles && (t + 1) * TILE <= n) {
+      mbar_arrive_expect_tx(&full[j % S], TILE_BYTES);
+      bulk_load_hint(ring + size_t(j % S) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[j % S], keep);
+    }
+  };
+  if (threadIdx.x == 0) {
+    for (int st = 0; st < S; ++st) mbar_init(&full[st], 1);
+    mbar_fence_init();
+    for (unsigned j = 0; j < unsigned(S); ++j) issue(j);
+  }
+  bar_workers<WT>();
+  unsigned par = 0;
+  auto reduce_tile = [&](unsigned j) {  // sum reduce-tile j, publish its aggregate, refill its stage
+    const unsigned long long tile = red_tile(j);
+    const size_t base = size_t(tile) * TILE;
+    T a = ident;
+    if (base + TILE <= n) {
+      mbar_wait(&full[j % S], (j / S) & 1u);
+      const T* stage = ring + size_t(j % S) * TILE;
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const uint4 q = *reinterpret_cast<const uint4*>(stage + (u * WT + threadIdx.x) * 4);
+        a = op2<T, OP>(a, op2<T, OP>(op2<T, OP>(from_bits<T>(q.x), from_bits<T>(q.y)),
+                                     op2<T, OP>(from_bits<T>(q.z), from_bits<T>(q.w))));
+      }
+    } else {  // ragged last tile: guarded loads
+      for (size_t i = base + threadIdx.x; i < n; i += WT) a = op2<T, OP>(a, in[i]);
+    }
+    a = warp_reduce<T, OP>(a);
+    if (lane == 0) red[par][warp] = a;
+    bar_workers<WT>();  // every worker has read the stage
+    if (warp == 0) {
+      T v = lane < NW ? red[par][lane] : ident;
+      v = warp_reduce<T, OP>(v);
+      if (lane == 0) {
+        st_state(state + tile, pack_state(epoch, 1u, to_bits(v)));
+        issue(j + S);
+      }
+    }
+    par ^= 1u;  // red[par] is rewritten two reduces later, with worker barriers in between
+  };
+  auto load_tile = [&](unsigned long long tile, uint32_t (&raw)[U][V], uint64_t policy) {
+    const size_t base = size_t(tile) * TILE;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * V;
+      if (i0 + V <= n) {
+        ld_hint4(raw[u], in + i0, policy);
+      } else {
+#pragma unroll
+        for (int j = 0; j < V; ++j) raw[u][j] = to_bits((i0 + j < n) ? in[i0 + j] : ident);
+      }
+    }
+  };
+
+  for (unsigned j = 0; j < unsigned(D); ++j) {  // prologue: run D tiles ahead
+    if (red_tile(j) >= ntiles) break;
+    reduce_tile(j);
+  }
+  unsigned it = 0;
+  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+    uint32_t rb[U][V];
+    load_tile(tile, rb, stream);
+    if (red_tile(it + D) < ntiles) reduce_tile(it + D);
+    // local scan of the tile (registers)
+    T x[U][V], lane_excl[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+#pragma unroll
+      for (int j = 0; j < V; ++j) x[u][j] = from_bits<T>(rb[u][j]);
+#pragma unroll
+      for (int j = 1; j < V; ++j) x[u][j] = op2<T, OP>(x[u][j - 1], x[u][j]);
+      T ws = x[u][V - 1];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        T y = __shfl_up_sync(FULL, ws, o);
+        if (lane >= o) ws = op2<T, OP>(y, ws);
+      }
+      T ex = __shfl_up_sync(FULL, ws, 1);
+      lane_excl[u] = lane == 0 ? ident : ex;
+      if (lane == 31) sm[u * NW + warp] = ws;
+    }
+    bar_workers<WT>();
+    if (warp == 0) {
+      constexpr int EPL = (E + 31) / 32;
+      T v[EPL];
+      T run = ident;
+#pragma unroll
+      for (int k = 0; k < EPL; ++k) {
+        const int e = lane * EPL + k;
+        v[k] = e < E ? sm[e] : ident;
+        run = op2<T, OP>(run, v[k]);
+      }
+      T ws = run;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        T y = __shfl_up_sync(FULL, ws, o);
+        if (lane >= o) ws = op2<T, OP>(y, ws);
+      }
+      T ex = __shfl_up_sync(FULL, ws, 1);
+      ex = lane == 0 ? ident : ex;
+#pragma unroll
+      for (int k = 0; k < EPL; ++k) {
+        const int e = lane * EPL + k;
+        if (e < E) sm[E + e] = ex;
+        ex = op2<T, OP>(ex, v[k]);
+      }
+    }
+    while (ld_acquire_shared(&cq_head) <= it) {}  // carry of this tile (normally long there)
+    const T carry = cq[it % Q];
+    bar_workers<WT>();
+    const size_t base = size_t(tile) * TILE;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const T p = op2<T, OP>(op2<T, OP>(carry, sm[E + u * NW + warp]), lane_excl[u]);
+      T o[V];
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        if (exclusive) o[j] = j == 0 ? p : op2<T, OP>(p, x[u][j - 1]);
+        else o[j] = op2<T, OP>(p, x[u][j]);
+      }
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * V;
+      if (i0 + V <= n) {
+        uint32_t raw[V];
+#pragma unroll
+        for (int j = 0; j < V; ++j) raw[j] = to_bits(o[j]);
+        st_hint4(out + i0, raw, stream);
+      } else {
+#pragma unroll
+        for (int j = 0; j < V; ++j)
+          if (i0 + j < n) out[i0 + j] = o[j];
+      }
+    }
+    bar_workers<WT>();  // sm is reused; every worker has read its carry
+    if (threadIdx.x == 0) st_release_shared(&cq_tail, it + 1);
+  }
+}
+
 // ---- three kernels: block sums -> scan of block sums -> rescan --------------------------------
 template <typename T, int OP, int THREADS, int V, int U>
 __global__ void __launch_bounds__(THREADS)
@@ -712,6 +947,14 @@ const ScanVariant kScanVariants[] = {
     {"ws_8w_u12_s4_k2", true, 256, 4, 12},       // 48 KB tiles, 4 stages
     {"ws_16w_u4_s6_k2", true, 512, 4, 4},        // 32 KB tiles, 16 scanner warps
     {"ws_4w_u8_s6_k2", true, 128, 4, 8},         // 16 KB tiles, 4 scanner warps, 2 CTAs/SM
+    {"l2ahead_8w_u4_d2_s2", true, 256, 4, 4},    // TMA ring (S stages) -> reduce D tiles ahead -> scan re-reads from L2
+    {"l2ahead_8w_u4_d2_s2_b3", true, 256, 4, 4}, // register cap for 3 CTAs/SM
+    {"l2ahead_8w_u4_d3_s2_b3", true, 256, 4, 4},
+    {"l2ahead_8w_u4_d2_s3_b3", true, 256, 4, 4},
+    {"l2ahead_8w_u4_d4_s2_b3", true, 256, 4, 4},
+    {"l2ahead_8w_u4_d3_s2_b4", true, 256, 4, 4},
+    {"l2ahead_8w_u8_d2_s2_b2", true, 256, 4, 8},
+    {"l2ahead_8w_u4_d3_s3_b3", true, 256, 4, 4},
 };
 constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
 
@@ -891,6 +1134,40 @@ cudaError_t launch_ws(const Launch& L, Scratch& Sc, bool exclusive, T init, cons
   return e;
 }
 
+template <typename T, int OP, int NW, int U, int D, int KW, int S, int MINB>
+cudaError_t launch_l2(const Launch& L, Scratch& Sc, bool exclusive, T init, const T* in, T* out, size_t n) {
+  constexpr size_t TILE = size_t(NW) * 32 * 4 * U;
+  constexpr int THREADS = (NW + 1) * 32;
+  constexpr size_t smem = S * TILE * 4 + S * 8 + 16;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  if (ntiles > Sc.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  if (++Sc.scan_epoch >= (1u << 30)) {
+    cudaError_t e = cudaMemsetAsync(Sc.scan_state, 0, Sc.scan_state_tiles * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    Sc.scan_epoch = 1;
+  }
+  auto kern = scan_l2_kernel<T, OP, NW, U, D, KW, S, MINB>;
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per < 1) return cudaErrorInvalidValue;
+    ctas_per_sm = per;
+  }
+  size_t grid = size_t(L.sms) * ctas_per_sm;
+  if (grid > ntiles) grid = ntiles;
+  int excl = exclusive ? 1 : 0;
+  uint32_t epoch = Sc.scan_epoch;
+  unsigned nt = (unsigned)ntiles;
+  void* args[] = {&in, &out, &n, &init, &excl, &Sc.scan_state, &epoch, &nt};
+  cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3((unsigned)grid), dim3(THREADS), args, smem, L.stream);
+  ++*L.launches;
+  return e;
+}
+
 template <typename T, int OP, int THREADS, int V, int U>
 cudaError_t launch_three(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
   constexpr size_t TILE = size_t(THREADS) * V * U;
@@ -955,6 +1232,14 @@ cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T
       case 30: return launch_ws<T, OP, 8, 12, 4, 2>(L, S, exclusive, init, in, out, n);
       case 31: return launch_ws<T, OP, 16, 4, 6, 2>(L, S, exclusive, init, in, out, n);
       case 32: return launch_ws<T, OP, 4, 8, 6, 2>(L, S, exclusive, init, in, out, n);
+      case 33: return launch_l2<T, OP, 8, 4, 2, 8, 2, 1>(L, S, exclusive, init, in, out, n);
+      case 34: return launch_l2<T, OP, 8, 4, 2, 8, 2, 3>(L, S, exclusive, init, in, out, n);
+      case 35: return launch_l2<T, OP, 8, 4, 3, 8, 2, 3>(L, S, exclusive, init, in, out, n);
+      case 36: return launch_l2<T, OP, 8, 4, 2, 8, 3, 3>(L, S, exclusive, init, in, out, n);
+      case 37: return launch_l2<T, OP, 8, 4, 4, 8, 2, 3>(L, S, exclusive, init, in, out, n);
+      case 38: return launch_l2<T, OP, 8, 4, 3, 8, 2, 4>(L, S, exclusive, init, in, out, n);
+      case 39: return launch_l2<T, OP, 8, 8, 2, 8, 2, 2>(L, S, exclusive, init, in, out, n);
+      case 40: return launch_l2<T, OP, 8, 4, 3, 8, 3, 3>(L, S, exclusive, init, in, out, n);
     }
   }
   switch (v) {
