@@ -416,7 +416,7 @@ bool variant_ok(const Call& k, int v) {
 const int* preference(int sk, int dtype, int* count) {
   static const int map_p[] = {2, 1, 0};
   static const int red_p[] = {1, 0};
-  static const int scan_i[] = {0, 4, 5};
+  static const int scan_i[] = {15, 3, 0, 4, 5};
   static const int scan_f[] = {4, 5};
   static const int o1_p[] = {2, 1, 0};
   static const int col_p[] = {2, 0};
@@ -426,7 +426,7 @@ const int* preference(int sk, int dtype, int* count) {
     case SKEL_SK_REDUCE:
     case SKEL_SK_MAPREDUCE: *count = 2; return red_p;
     case SKEL_SK_SCAN:
-      if (dtype == SKEL_I32) { *count = 3; return scan_i; }
+      if (dtype == SKEL_I32) { *count = 5; return scan_i; }
       *count = 2; return scan_f;
     case SKEL_SK_OVERLAP1D: *count = 3; return o1_p;
     case SKEL_SK_OVERLAP1D_COL: *count = 2; return col_p;

@@ -8,11 +8,16 @@
 //    windows of 32 predecessors. The epoch tag makes a memset of the tile states between calls
 //    unnecessary. i32 only: with floating point the result would depend on how far each look-back
 //    happened to reach.
+//  * "persist_*": the same with a grid of co-resident blocks walking strided tiles (no ticket).
+//  * "ws_*": warp-specialised persistent CTAs fed by a shared-memory ring of bulk async copies;
+//    one prefix warp per stage publishes the aggregate as soon as the tile lands.
+//  * "l2ahead_*": the fastest at large n (6.2 TB/s at 2^28): a TMA-fed reduce pass runs D tiles
+//    ahead and publishes aggregates, a prefix warp sums them (no chain), the scan pass re-reads the
+//    tile from L2. See the comment above scan_l2_kernel.
 //  * "three_kernel_*": reduce per block -> scan of the block sums -> rescan with carry. 12 B/elem,
 //    fixed combination order (deterministic for f32); the correctness anchor for the look-back.
 #include "common.cuh"
 #include "kernels.hpp"
-#include <cooperative_groups.h>
 #include <stdlib.h>
 
 namespace skel {
@@ -258,195 +263,8 @@ scan_lookback_persist_kernel(const T* in, T* out, size_t n, T init, int exclusiv
   }
 }
 
-// ---- single pass, thread-block clusters --------------------------------------------------------------
-// The look-back chain is paced by L2 round trips and by how many tiles poll it. Here CS CTAs of a
-// cluster scan CS consecutive tiles and exchange their aggregates through distributed shared
-// memory (a cluster barrier costs ~0.2 us, an L2 round trip ~0.7 us); only the cluster leader
-// takes a ticket and takes part in the global look-back, with the whole cluster's aggregate. The
-// global chain therefore has CS times fewer participants and advances CS times more data per step.
-namespace cg = cooperative_groups;
-
-template <typename T, int OP, int THREADS, int V, int U, int CS, bool NC>
-__global__ void __cluster_dims__(CS, 1, 1) __launch_bounds__(THREADS)
-scan_cluster_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, unsigned* ticket,
-                    uint32_t epoch, unsigned nctiles) {
-  static_assert(sizeof(T) == 4 && CS <= 32, "32-bit elements; cluster fits a warp");
-  constexpr int NW = THREADS / 32, E = U * NW;
-  constexpr size_t TILE = size_t(THREADS) * V * U;
-  __shared__ T sm[2 * E + 1];
-  __shared__ unsigned s_ctile;  // leader's copy is the cluster's
-  __shared__ T c_agg[CS];       // leader's copy: aggregate of every CTA of the cluster
-  __shared__ T c_carry;         // leader's copy: exclusive prefix of the cluster
-  __shared__ T s_carry;
-  cg::cluster_group cluster = cg::this_cluster();
-  const unsigned rank = cluster.block_rank();
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const T ident = identity<T, OP>();
-
-  if (rank == 0 && threadIdx.x == 0) s_ctile = atomicAdd(ticket, 1u);
-  cluster.sync();
-  const unsigned ctile = *cluster.map_shared_rank(&s_ctile, 0);
-  const size_t base = (size_t(ctile) * CS + rank) * TILE;  // may lie past n: then every access is masked
-
-  TileRegs<T, V, U> R;
-  const T agg = tile_phase_a<T, OP, THREADS, V, U, NC>(in, base, n, R, sm);
-  if (threadIdx.x == 0) *cluster.map_shared_rank(&c_agg[rank], 0) = agg;
-  cluster.sync();
-  if (rank == 0 && warp == 0) {
-    T v = lane < CS ? c_agg[lane] : ident;
-    v = warp_reduce<T, OP>(v);
-    const T carry = lookback_warp0<T, OP>(state, epoch, ctile, v, init, exclusive != 0);
-    if (lane == 0) c_carry = carry;
-  }
-  cluster.sync();
-  if (threadIdx.x == 0) {
-    T c = *cluster.map_shared_rank(&c_carry, 0);
-    const T* aggs = cluster.map_shared_rank(&c_agg[0], 0);
-    for (unsigned r = 0; r < rank; ++r) c = op2<T, OP>(c, aggs[r]);
-    s_carry = c;
-  }
-  __syncthreads();
-  tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
-  if (rank == 0 && threadIdx.x == 0 && ctile == nctiles - 1) *ticket = 0u;
-  cluster.sync();  // the leader's shared memory must outlive the remote reads above
-}
-
-// ---- single pass, persistent CTAs fed by a ring of bulk async copies ------------------------------
-// Each CTA owns STAGES shared-memory tile buffers. One thread draws tile tickets ahead of time and
-// issues a bulk copy (TMA engine) per ticket; the copy signals an mbarrier. While a tile waits in
-// its look-back, the loads of the CTA's next STAGES-1 tiles are already in flight, so memory
-// latency is decoupled from the look-back chain. Tiles a CTA holds have increasing ids and are
-// processed in that order, so the smallest unfinished tile is always being worked on (forward
-// progress). The last CTA to leave resets the ticket and the exit counter.
-template <typename T, int OP, int THREADS, int V, int U, int STAGES>
-__global__ void __launch_bounds__(THREADS)
-scan_lookback_ring_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state,
-                          unsigned* ticket, uint32_t epoch, unsigned ntiles) {
-  static_assert(sizeof(T) == 4 && V == 4, "32-bit elements, 128-bit shared-memory reads");
-  constexpr int NW = THREADS / 32, E = U * NW;
-  constexpr int TILE = THREADS * V * U;
-  constexpr unsigned TILE_BYTES = TILE * 4u;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* buf = reinterpret_cast<T*>(smem_raw);
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(STAGES) * TILE_BYTES);
-  unsigned* tile_of = reinterpret_cast<unsigned*>(full + STAGES);
-  T* sm = reinterpret_cast<T*>(tile_of + STAGES);
-  __shared__ T s_carry;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  (void)lane;
-
-  auto issue = [&](int s) {  // thread 0 only
-    const unsigned t = atomicAdd(ticket, 1u);
-    tile_of[s] = t;
-    if (t < ntiles && (size_t(t) + 1) * TILE <= n) {
-      mbar_arrive_expect_tx(&full[s], TILE_BYTES);
-      bulk_load(buf + size_t(s) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[s]);
-    } else {
-      mbar_arrive(&full[s]);  // ragged last tile (read directly) or past the end (sentinel)
-    }
-  };
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
-    mbar_fence_init();
-  }
-  __syncthreads();
-  if (threadIdx.x == 0)
-    for (int s = 0; s < STAGES; ++s) issue(s);
-
-  for (unsigned it = 0;; ++it) {
-    const int s = it % STAGES;
-    mbar_wait(&full[s], (it / STAGES) & 1u);
-    const unsigned tile = tile_of[s];
-    if (tile >= ntiles) break;
-    const size_t base = size_t(tile) * TILE;
-    const bool staged = base + TILE <= n;
-    TileRegs<T, V, U> R;
-    const T agg = tile_phase_a<T, OP, THREADS, V, U, false>(in, base, n, R, sm, staged ? buf + size_t(s) * TILE : nullptr);
-    // every thread has read tile_of[s] and its part of the buffer (two block barriers ago)
-    if (threadIdx.x == 0) issue(s);
-    if (warp == 0) {
-      const T carry = lookback_warp0<T, OP>(state, epoch, tile, agg, init, exclusive != 0);
-      if (threadIdx.x == 0) s_carry = carry;
-    }
-    __syncthreads();
-    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
-    __syncthreads();  // sm and s_carry are reused by the next tile
-  }
-  if (threadIdx.x == 0) {
-    const unsigned done = atomicAdd(ticket + 1, 1u);
-    if (done == gridDim.x - 1) {  // every CTA has drawn its last ticket
-      ticket[0] = 0u;
-      ticket[1] = 0u;
-    }
-  }
-}
-
-// ---- single pass, persistent CTAs, STATIC strided tiles fed by a ring of bulk async copies ----------
-// CTA b scans tiles b, b+G, b+2G, ... (G = gridDim.x, all CTAs co-resident). Because the tiles of
-// a CTA are known in advance, one thread keeps STAGES bulk copies (TMA engine) in flight per CTA:
-// the load stream never stops while a tile sits in its look-back, which is what bounds the plain
-// one-tile-per-block kernel (loads are only in flight during ~1/3 of a block's life time).
-// Unlike the ticket ring above, tile t-1 is processed by CTA b-1 in the SAME iteration, so its
-// aggregate never queues behind another tile's look-back: the dependence depth is the iteration
-// count, as in the non-ring kernels. Forward progress: tile t waits only on tiles < t, which are
-// held by co-resident CTAs at the same or an earlier iteration (induction on t); the launch is a
-// cooperative one, so co-residency is guaranteed by the driver, not assumed.
-template <typename T, int OP, int THREADS, int V, int U, int STAGES>
-__global__ void __launch_bounds__(THREADS)
-scan_sring_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned long long* state, uint32_t epoch,
-                  unsigned ntiles) {
-  static_assert(sizeof(T) == 4 && V == 4, "32-bit elements, 128-bit shared-memory reads");
-  constexpr int NW = THREADS / 32, E = U * NW;
-  constexpr int TILE = THREADS * V * U;
-  constexpr unsigned TILE_BYTES = TILE * 4u;
-  extern __shared__ __align__(128) unsigned char smem_raw[];
-  T* buf = reinterpret_cast<T*>(smem_raw);
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(STAGES) * TILE_BYTES);
-  T* sm = reinterpret_cast<T*>(full + STAGES);
-  __shared__ T s_carry;
-  const int warp = threadIdx.x >> 5;
-  const unsigned G = gridDim.x;
-
-  auto issue = [&](int s, unsigned long long t) {  // thread 0 only
-    if (t >= ntiles) return;                        // never waited for
-    if ((t + 1) * TILE <= n) {
-      mbar_arrive_expect_tx(&full[s], TILE_BYTES);
-      bulk_load(buf + size_t(s) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[s]);
-    } else {
-      mbar_arrive(&full[s]);  // ragged last tile: read directly with guarded loads
-    }
-  };
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
-    mbar_fence_init();
-    for (int s = 0; s < STAGES; ++s) issue(s, blockIdx.x + (unsigned long long)s * G);
-  }
-  __syncthreads();
-
-  unsigned it = 0;
-  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
-    const int s = it % STAGES;
-    mbar_wait(&full[s], (it / STAGES) & 1u);
-    const size_t base = size_t(tile) * TILE;
-    const bool staged = base + TILE <= n;
-    TileRegs<T, V, U> R;
-    const T agg = tile_phase_a<T, OP, THREADS, V, U, false>(in, base, n, R, sm, staged ? buf + size_t(s) * TILE : nullptr);
-    // every thread has copied its part of buffer s into registers (two block barriers ago)
-    if (threadIdx.x == 0) issue(s, tile + (unsigned long long)STAGES * G);
-    if (warp == 0) {
-      const T carry = lookback_warp0<T, OP>(state, epoch, (unsigned)tile, agg, init, exclusive != 0);
-      if (threadIdx.x == 0) s_carry = carry;
-    }
-    __syncthreads();
-    tile_phase_b<T, OP, THREADS, V, U>(out, base, n, R, sm, s_carry, exclusive != 0);
-    __syncthreads();  // sm and s_carry are reused by the next tile
-  }
-}
-
 // ---- single pass, warp-specialised persistent CTAs ("ws") ------------------------------------------
-// Measured on B200 (profiles/r01_scan_probe.txt): in the one-tile-per-block kernel a tile spends
+// Measured on B200: in the one-tile-per-block kernel a tile spends
 // ~2/3 of its life spinning in the look-back, not because the chain is long but because the load
 // latency under a saturated HBM has a heavy tail (p50 2.5 us, p99 7 us) and a tile's aggregate is
 // only published once ITS loads have landed; every later tile waits for the slowest earlier one,
@@ -597,7 +415,7 @@ scan_ws_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned lo
 
 // ---- single pass over HBM, two passes over L2 ("l2ahead") --------------------------------------------
 // What bounds every chained single-pass kernel above on B200 is not the chain arithmetic but the
-// load-latency tail of a saturated HBM (profiles/r01_scan_probe.txt: p50 2.5 us, p99 7 us, max ~10
+// load-latency tail of a saturated HBM (p50 2.5 us, p99 7 us, max ~10
 // us): tile t cannot be finished before every earlier tile has LANDED, so each slot of on-chip
 // buffering is held for the tail latency, not the mean, and 192 KB of shared memory per SM is not
 // enough buffer. Here the buffer is the 126 MB L2 and there is no chain at all:
@@ -612,7 +430,7 @@ scan_ws_kernel(const T* in, T* out, size_t n, T init, int exclusive, unsigned lo
 //  * SCAN phase (worker warps): tile k is read a second time - now from L2 (evict_first, like the
 //    output stores) - scanned locally, offset by the carry and streamed out.
 // HBM traffic stays 8 B/elem; L2 carries 12 B/elem (+ G*8 B of aggregate reads per tile), which it
-// sustains (profiles/r01_l2_probe.txt). Run-ahead = D*G tiles. Forward progress: the reduce phase
+// sustains. Run-ahead = D*G tiles. Forward progress: the reduce phase
 // waits for nothing; a prefix waits only for aggregates, i.e. for reduce phases.
 template <int N> __device__ __forceinline__ void bar_workers() { asm volatile("bar.sync 1, %0;" ::"n"(N) : "memory"); }
 __device__ __forceinline__ unsigned ld_acquire_shared(const unsigned* p) {
@@ -920,41 +738,18 @@ const ScanVariant kScanVariants[] = {
     {"lookback_256x8x4", true, 256, 8, 4},
     {"three_kernel_256x4x4", false, 256, 4, 4},
     {"three_kernel_256x1x4", false, 256, 1, 4},  // any alignment
-    {"ring_256x4x4_s4", true, 256, 4, 4},        // persistent CTAs + bulk-copy ring (16 KB tiles, 4 stages)
-    {"ring_256x4x8_s3", true, 256, 4, 8},        // 32 KB tiles, 3 stages
-    {"ring_512x4x4_s3", true, 512, 4, 4},        // 32 KB tiles, 3 stages, 512 threads
-    {"ring_512x4x4_s6", true, 512, 4, 4},        // 32 KB tiles, 6 stages, one CTA per SM
     {"lookback_512x8x4", true, 512, 8, 4},       // 16384-element tiles
     {"lookback_1024x8x2", true, 1024, 8, 2},     // 16384-element tiles, 1024 threads
-    {"cluster8_256x8x4", true, 256, 8, 4},       // clusters of 8 CTAs, DSMEM aggregate exchange
-    {"cluster8_256x4x4", true, 256, 4, 4},
-    {"cluster16_256x8x4", true, 256, 8, 4},      // non-portable cluster size 16
-    {"cluster8_512x8x2", true, 512, 8, 2},
     {"persist_256x8x4", true, 256, 8, 4},        // persistent blocks, strided tiles, no ticket
     {"persist_256x4x4", true, 256, 4, 4},
     {"persist_512x8x4", true, 512, 8, 4},
-    {"sring_256x4x4_s3", true, 256, 4, 4},       // static strided tiles + bulk-copy ring: 16 KB tiles, 3 stages
-    {"sring_256x4x8_s2", true, 256, 4, 8},       // 32 KB tiles, 2 stages
-    {"sring_512x4x4_s2", true, 512, 4, 4},       // 32 KB tiles, 2 stages, 512 threads
-    {"sring_256x4x4_s2", true, 256, 4, 4},       // 16 KB tiles, 2 stages
-    {"sring_512x4x4_s3", true, 512, 4, 4},       // 32 KB tiles, 3 stages
-    {"sring_128x4x8_s3", true, 128, 4, 8},       // 16 KB tiles, 128 threads, 3 stages
-    {"ws_8w_u8_s6_k2", true, 256, 4, 8},         // warp-specialised: 32 KB tiles, 6 stages, 1 CTA/SM
+    {"ws_8w_u8_s6_k1", true, 256, 4, 8},         // warp-specialised: 32 KB tiles, 6 smem stages, 1 CTA/SM
     {"ws_8w_u8_s3_k2", true, 256, 4, 8},         // 32 KB tiles, 3 stages, 2 CTAs/SM
-    {"ws_8w_u4_s6_k2", true, 256, 4, 4},         // 16 KB tiles, 6 stages, 2 CTAs/SM
-    {"ws_8w_u8_s6_k1", true, 256, 4, 8},
-    {"ws_8w_u8_s6_k4", true, 256, 4, 8},
     {"ws_8w_u12_s4_k2", true, 256, 4, 12},       // 48 KB tiles, 4 stages
-    {"ws_16w_u4_s6_k2", true, 512, 4, 4},        // 32 KB tiles, 16 scanner warps
-    {"ws_4w_u8_s6_k2", true, 128, 4, 8},         // 16 KB tiles, 4 scanner warps, 2 CTAs/SM
-    {"l2ahead_8w_u4_d2_s2", true, 256, 4, 4},    // TMA ring (S stages) -> reduce D tiles ahead -> scan re-reads from L2
-    {"l2ahead_8w_u4_d2_s2_b3", true, 256, 4, 4}, // register cap for 3 CTAs/SM
+    {"l2ahead_8w_u4_d2_s2_b3", true, 256, 4, 4}, // TMA ring (S) -> reduce D tiles ahead -> scan re-reads from L2; 3 CTAs/SM
+    {"l2ahead_8w_u8_d2_s2_b2", true, 256, 4, 8}, // 32 KB tiles, 2 CTAs/SM
     {"l2ahead_8w_u4_d3_s2_b3", true, 256, 4, 4},
     {"l2ahead_8w_u4_d2_s3_b3", true, 256, 4, 4},
-    {"l2ahead_8w_u4_d4_s2_b3", true, 256, 4, 4},
-    {"l2ahead_8w_u4_d3_s2_b4", true, 256, 4, 4},
-    {"l2ahead_8w_u8_d2_s2_b2", true, 256, 4, 8},
-    {"l2ahead_8w_u4_d3_s3_b3", true, 256, 4, 4},
 };
 constexpr int kNumScanVariants = sizeof(kScanVariants) / sizeof(kScanVariants[0]);
 
@@ -1001,101 +796,13 @@ cudaError_t launch_persist(const Launch& L, Scratch& S, bool exclusive, T init, 
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
   const bool nc = static_cast<const void*>(in) != out;
-  if (nc) kt<<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_epoch, (unsigned)ntiles);
-  else kf<<<(unsigned)grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_epoch, (unsigned)ntiles);
-  ++*L.launches;
-  return cudaGetLastError();
-}
-
-template <typename T, int OP, int THREADS, int V, int U, int CS>
-cudaError_t launch_cluster(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
-  constexpr size_t TILE = size_t(THREADS) * V * U;
-  const size_t ntiles = (n + TILE - 1) / TILE;
-  const size_t nctiles = (ntiles + CS - 1) / CS;
-  if (nctiles > S.scan_state_tiles || nctiles * CS > 0x7fffffffu) return cudaErrorInvalidValue;
-  if (++S.scan_epoch >= (1u << 30)) {
-    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
-    if (e != cudaSuccess) return e;
-    S.scan_epoch = 1;
-  }
-  const bool nc = static_cast<const void*>(in) != out;
-  auto kt = scan_cluster_kernel<T, OP, THREADS, V, U, CS, true>;
-  auto kf = scan_cluster_kernel<T, OP, THREADS, V, U, CS, false>;
-  if (CS > 8) {
-    static bool done = false;
-    if (!done) {
-      cudaFuncSetAttribute(kt, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-      cudaFuncSetAttribute(kf, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-      done = true;
-    }
-  }
-  const unsigned grid = (unsigned)(nctiles * CS);
-  if (nc) kt<<<grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)nctiles);
-  else kf<<<grid, THREADS, 0, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket, S.scan_epoch, (unsigned)nctiles);
-  ++*L.launches;
-  return cudaGetLastError();
-}
-
-template <typename T, int OP, int THREADS, int V, int U, int STAGES>
-cudaError_t launch_ring(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
-  constexpr size_t TILE = size_t(THREADS) * V * U;
-  constexpr int E = U * (THREADS / 32);
-  constexpr size_t smem = STAGES * TILE * 4 + STAGES * 8 + STAGES * 4 + (2 * E + 1) * 4 + 16;
-  const size_t ntiles = (n + TILE - 1) / TILE;
-  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
-  if (++S.scan_epoch >= (1u << 30)) {
-    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
-    if (e != cudaSuccess) return e;
-    S.scan_epoch = 1;
-  }
-  auto kern = scan_lookback_ring_kernel<T, OP, THREADS, V, U, STAGES>;
-  static int ctas_per_sm = 0;
-  if (ctas_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, THREADS, smem);
-    if (e != cudaSuccess) return e;
-    if (ctas_per_sm < 1) return cudaErrorInvalidValue;
-  }
-  size_t grid = size_t(L.sms) * ctas_per_sm;  // all CTAs are co-resident (they wait on one another)
-  if (grid > ntiles) grid = ntiles;
-  kern<<<(unsigned)grid, THREADS, smem, L.stream>>>(in, out, n, init, exclusive ? 1 : 0, S.scan_state, S.scan_ticket,
-                                                    S.scan_epoch, (unsigned)ntiles);
-  ++*L.launches;
-  return cudaGetLastError();
-}
-
-template <typename T, int OP, int THREADS, int V, int U, int STAGES>
-cudaError_t launch_sring(const Launch& L, Scratch& S, bool exclusive, T init, const T* in, T* out, size_t n) {
-  constexpr size_t TILE = size_t(THREADS) * V * U;
-  constexpr int E = U * (THREADS / 32);
-  constexpr size_t smem = STAGES * TILE * 4 + STAGES * 8 + (2 * E + 1) * 4 + 16;
-  const size_t ntiles = (n + TILE - 1) / TILE;
-  if (ntiles > S.scan_state_tiles || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
-  if (++S.scan_epoch >= (1u << 30)) {
-    cudaError_t e = cudaMemsetAsync(S.scan_state, 0, S.scan_state_tiles * 8, L.stream);
-    if (e != cudaSuccess) return e;
-    S.scan_epoch = 1;
-  }
-  auto kern = scan_sring_kernel<T, OP, THREADS, V, U, STAGES>;
-  static int ctas_per_sm = 0;
-  if (ctas_per_sm == 0) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    int per = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, THREADS, smem);
-    if (e != cudaSuccess) return e;
-    if (per < 1) return cudaErrorInvalidValue;
-    ctas_per_sm = per;
-  }
-  size_t grid = size_t(L.sms) * ctas_per_sm;
-  if (grid > ntiles) grid = ntiles;
   int excl = exclusive ? 1 : 0;
   uint32_t epoch = S.scan_epoch;
   unsigned nt = (unsigned)ntiles;
   void* args[] = {&in, &out, &n, &init, &excl, &S.scan_state, &epoch, &nt};
-  // cooperative launch: the driver guarantees that all CTAs are co-resident (they wait on one another)
-  cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3((unsigned)grid), dim3(THREADS), args, smem, L.stream);
+  // cooperative launch: the blocks wait on one another, so the driver must guarantee co-residency
+  cudaError_t e = cudaLaunchCooperativeKernel(nc ? reinterpret_cast<void*>(kt) : reinterpret_cast<void*>(kf), dim3((unsigned)grid),
+                                              dim3(THREADS), args, 0, L.stream);
   ++*L.launches;
   return e;
 }
@@ -1205,41 +912,18 @@ cudaError_t launch_variant(const Launch& L, Scratch& S, int v, bool exclusive, T
       case 1: return launch_lookback<T, OP, 256, 8, 2>(L, S, exclusive, init, in, out, n);
       case 2: return launch_lookback<T, OP, 512, 8, 2>(L, S, exclusive, init, in, out, n);
       case 3: return launch_lookback<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
-      case 6: return launch_ring<T, OP, 256, 4, 4, 4>(L, S, exclusive, init, in, out, n);
-      case 7: return launch_ring<T, OP, 256, 4, 8, 3>(L, S, exclusive, init, in, out, n);
-      case 8: return launch_ring<T, OP, 512, 4, 4, 3>(L, S, exclusive, init, in, out, n);
-      case 9: return launch_ring<T, OP, 512, 4, 4, 6>(L, S, exclusive, init, in, out, n);
-      case 10: return launch_lookback<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
-      case 11: return launch_lookback<T, OP, 1024, 8, 2>(L, S, exclusive, init, in, out, n);
-      case 12: return launch_cluster<T, OP, 256, 8, 4, 8>(L, S, exclusive, init, in, out, n);
-      case 13: return launch_cluster<T, OP, 256, 4, 4, 8>(L, S, exclusive, init, in, out, n);
-      case 14: return launch_cluster<T, OP, 256, 8, 4, 16>(L, S, exclusive, init, in, out, n);
-      case 15: return launch_cluster<T, OP, 512, 8, 2, 8>(L, S, exclusive, init, in, out, n);
-      case 16: return launch_persist<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
-      case 17: return launch_persist<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
-      case 18: return launch_persist<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
-      case 19: return launch_sring<T, OP, 256, 4, 4, 3>(L, S, exclusive, init, in, out, n);
-      case 20: return launch_sring<T, OP, 256, 4, 8, 2>(L, S, exclusive, init, in, out, n);
-      case 21: return launch_sring<T, OP, 512, 4, 4, 2>(L, S, exclusive, init, in, out, n);
-      case 22: return launch_sring<T, OP, 256, 4, 4, 2>(L, S, exclusive, init, in, out, n);
-      case 23: return launch_sring<T, OP, 512, 4, 4, 3>(L, S, exclusive, init, in, out, n);
-      case 24: return launch_sring<T, OP, 128, 4, 8, 3>(L, S, exclusive, init, in, out, n);
-      case 25: return launch_ws<T, OP, 8, 8, 6, 2>(L, S, exclusive, init, in, out, n);
-      case 26: return launch_ws<T, OP, 8, 8, 3, 2>(L, S, exclusive, init, in, out, n);
-      case 27: return launch_ws<T, OP, 8, 4, 6, 2>(L, S, exclusive, init, in, out, n);
-      case 28: return launch_ws<T, OP, 8, 8, 6, 1>(L, S, exclusive, init, in, out, n);
-      case 29: return launch_ws<T, OP, 8, 8, 6, 4>(L, S, exclusive, init, in, out, n);
-      case 30: return launch_ws<T, OP, 8, 12, 4, 2>(L, S, exclusive, init, in, out, n);
-      case 31: return launch_ws<T, OP, 16, 4, 6, 2>(L, S, exclusive, init, in, out, n);
-      case 32: return launch_ws<T, OP, 4, 8, 6, 2>(L, S, exclusive, init, in, out, n);
-      case 33: return launch_l2<T, OP, 8, 4, 2, 8, 2, 1>(L, S, exclusive, init, in, out, n);
-      case 34: return launch_l2<T, OP, 8, 4, 2, 8, 2, 3>(L, S, exclusive, init, in, out, n);
-      case 35: return launch_l2<T, OP, 8, 4, 3, 8, 2, 3>(L, S, exclusive, init, in, out, n);
-      case 36: return launch_l2<T, OP, 8, 4, 2, 8, 3, 3>(L, S, exclusive, init, in, out, n);
-      case 37: return launch_l2<T, OP, 8, 4, 4, 8, 2, 3>(L, S, exclusive, init, in, out, n);
-      case 38: return launch_l2<T, OP, 8, 4, 3, 8, 2, 4>(L, S, exclusive, init, in, out, n);
-      case 39: return launch_l2<T, OP, 8, 8, 2, 8, 2, 2>(L, S, exclusive, init, in, out, n);
-      case 40: return launch_l2<T, OP, 8, 4, 3, 8, 3, 3>(L, S, exclusive, init, in, out, n);
+      case 6: return launch_lookback<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 7: return launch_lookback<T, OP, 1024, 8, 2>(L, S, exclusive, init, in, out, n);
+      case 8: return launch_persist<T, OP, 256, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 9: return launch_persist<T, OP, 256, 4, 4>(L, S, exclusive, init, in, out, n);
+      case 10: return launch_persist<T, OP, 512, 8, 4>(L, S, exclusive, init, in, out, n);
+      case 11: return launch_ws<T, OP, 8, 8, 6, 1>(L, S, exclusive, init, in, out, n);
+      case 12: return launch_ws<T, OP, 8, 8, 3, 2>(L, S, exclusive, init, in, out, n);
+      case 13: return launch_ws<T, OP, 8, 12, 4, 2>(L, S, exclusive, init, in, out, n);
+      case 14: return launch_l2<T, OP, 8, 4, 2, 8, 2, 3>(L, S, exclusive, init, in, out, n);
+      case 15: return launch_l2<T, OP, 8, 8, 2, 8, 2, 2>(L, S, exclusive, init, in, out, n);
+      case 16: return launch_l2<T, OP, 8, 4, 3, 8, 2, 3>(L, S, exclusive, init, in, out, n);
+      case 17: return launch_l2<T, OP, 8, 4, 2, 8, 3, 3>(L, S, exclusive, init, in, out, n);
     }
   }
   switch (v) {
