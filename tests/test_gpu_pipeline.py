@@ -1,0 +1,184 @@
+"""Smart-container coherence on the GPU and the chained pipeline of
+BASELINE.json configs[4] (readings 14 and 15): transfer counts against the protocol's
+closed forms, lock-step parity of every call against the CPU oracle, run-to-run determinism, and a
+model-based random walk (library vs shadow arrays + the protocol table)."""
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import assert_map_f32, assert_overlap, assert_reduce_f32
+from paper_1405_2915_b200 import inputs as I
+from paper_1405_2915_b200 import skel as S
+
+pytestmark = pytest.mark.gpu
+
+C32 = float(np.float32(1.0001))
+
+
+@pytest.fixture()
+def ctx():
+    import torch
+    assert torch.cuda.is_available()
+    c = S.Context()
+    yield c
+    c.close()
+
+
+def run_pipeline(ctx, x0, w, iters, verify_at=()):
+    """Map(x*1.0001) in place -> MapOverlap1D(r=4, duplicate) -> Reduce(sum); A and B swap roles."""
+    n = x0.size
+    a, b = ctx.vector_from(x0), ctx.vector(n)
+    ctx.reset_stats()
+    scalars = []
+    for k in range(1, iters + 1):
+        check = k in verify_at
+        if check:
+            a_in = a.numpy().copy()  # the GPU's actual input of this call (a host read: counted below)
+        ctx.map(S.FN_MULT, 1.0001, a, None, a)
+        if check:
+            a_mid = a.numpy().copy()
+            assert_map_f32(a_mid, O.map_f32(O.FN_MULT, 1.0001, a_in))
+        ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
+        s = ctx.reduce(S.FN_ADD, b)
+        if check:
+            b_out = b.numpy().copy()
+            ref, ab = O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, a_mid)
+            assert_overlap(b_out, ref, ab)
+            r, absum = O.reduce_f32(O.FN_ADD, b_out)
+            assert_reduce_f32(s, r, absum)
+        scalars.append(s)
+        a, b = b, a
+    st = ctx.stats()
+    final = a.numpy().copy()
+    a.destroy()
+    b.destroy()
+    return scalars, st, final
+
+
+def test_pipeline_lazy_transfer_counts_lockstep_and_determinism(ctx):
+    n, iters = (1 << 20) + 37, 12
+    x0 = I.uniform01_f32(I.config_seed(5, 1), n)
+    w = I.positive_weights_f32(I.config_seed(3, 14), 9)
+    # measurement run: only the scalars are read
+    scal, st, final = run_pipeline(ctx, x0, w, iters)
+    assert st["h2d_count"] == 1 and st["h2d_bytes"] == 4 * n          # the one upload of A
+    assert st["d2h_count"] == 0 and st["d2h_bytes"] == 0              # nothing comes back during the loop
+    assert st["scalar_d2h_count"] == iters
+    assert st["h2d_elided"] == 3 * iters - 1                           # every other device read reused a valid copy
+    assert st["launches"] >= 3 * iters
+    # verification run: every call checked in lock-step at iterations 1, 2 and the last
+    scal2, st2, final2 = run_pipeline(ctx, x0, w, iters, verify_at=(1, 2, iters))
+    assert scal2 == scal, "pipeline scalars are not bit-identical run to run"
+    assert np.array_equal(final, final2)
+    assert st2["h2d_count"] == 1                                       # host reads never invalidate the device copy
+    # three host reads per verified iteration, minus the two that find a valid host copy: A at iteration 1
+    # (created from host data) and A at iteration 2 (it is iteration 1's B, already downloaded)
+    assert st2["d2h_count"] == 3 * 3 - 2
+    # free-running fp64 chain (reported bound, reading 15): drift stays tiny over 12 iterations
+    x = x0.astype(np.float64)
+    for k in range(iters):
+        x = x * C32
+        x, _ = O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, x.astype(np.float32))  # oracle takes fp32 inputs
+    assert abs(scal[-1] - x.sum()) <= 1e-4 * np.abs(x).sum()
+
+
+def test_pipeline_constant_vector_closed_form(ctx):
+    # duplicate edges + weights summing to 1 keep a constant vector constant: s_k = n * K * c32^k
+    n, iters, K = 300007, 10, 0.75
+    w = I.positive_weights_f32(77, 9)
+    wsum = float(w.astype(np.float64).sum())
+    scal, _, _ = run_pipeline(ctx, np.full(n, K, np.float32), w, iters)
+    for k, s in enumerate(scal, start=1):
+        expect = n * K * (C32 * wsum) ** k
+        assert abs(s - expect) <= 1e-5 * abs(expect), (k, s, expect)
+
+
+def test_pipeline_eager_moves_five_containers_per_iteration(ctx):
+    n, iters = 100003, 4
+    x0 = I.uniform01_f32(9001, n)
+    w = I.positive_weights_f32(9002, 9)
+    lazy, _, lazy_final = run_pipeline(ctx, x0, w, iters)
+    ctx.set_coherence(S.EAGER)
+    try:
+        eager, st, eager_final = run_pipeline(ctx, x0, w, iters)
+    finally:
+        ctx.set_coherence(S.LAZY)
+    assert eager == lazy and np.array_equal(lazy_final, eager_final)   # same kernels, same data
+    assert st["h2d_count"] == 3 * iters and st["h2d_bytes"] == 3 * iters * 4 * n
+    assert st["d2h_count"] == 2 * iters and st["d2h_bytes"] == 2 * iters * 4 * n
+    assert st["h2d_elided"] == 0 and st["d2h_elided"] == 0
+
+
+def test_coherence_model_based_random_walk(ctx):
+    """Random sequences of host writes / host reads / skeleton calls on three containers, applied to
+    the library and to shadow host arrays through the oracle + the protocol table."""
+    rng = np.random.default_rng(20140529)
+    n = 5003
+    w = I.positive_weights_f32(31, 5)
+    vecs = [ctx.vector(n) for _ in range(3)]
+    shadow = [None, None, None]          # fp32 arrays as the GPU holds them (downloaded after each call)
+    state = [0, 0, 0]                    # bit 0 host valid, bit 1 device valid
+    h2d = d2h = 0
+    ctx.reset_stats()
+
+    def dev_access(i, access):
+        nonlocal h2d
+        _, new, xfer = S.coherence_step(state[i], 0, access, S.LAZY)
+        h2d += 1 if xfer & 1 else 0
+        state[i] = new
+
+    def host_access(i, access):
+        nonlocal d2h
+        _, new, xfer = S.coherence_step(state[i], 1, access, S.LAZY)
+        d2h += 1 if xfer & 2 else 0
+        state[i] = new
+
+    for step in range(120):
+        op = rng.integers(0, 5)
+        i, j = rng.choice(3, size=2, replace=False)
+        if op == 0 or shadow[i] is None:       # host write (whole container)
+            data = I.uniform01_f32(1000 + step, n)
+            host_access(i, S.WRITE)
+            vecs[i].write(data)
+            shadow[i] = data.copy()
+        elif op == 1:                           # host read
+            host_access(i, S.READ)
+            got = vecs[i].numpy()
+            assert np.array_equal(got, shadow[i]), f"step {step}: stale or wrong data on host read"
+        elif op == 2:                           # Map in place
+            dev_access(i, S.READWRITE)
+            ctx.map(S.FN_MULT, 1.0001, vecs[i], None, vecs[i])
+            ref = O.map_f32(O.FN_MULT, 1.0001, shadow[i])
+            shadow[i] = ref.astype(np.float32)  # mult of two fp32 values is correctly rounded: 0 ulp
+        elif op == 3:                           # MapOverlap i -> j
+            dev_access(i, S.READ)
+            dev_access(j, S.WRITE)
+            ctx.mapoverlap_1d(w, 2, S.EDGE_CONSTANT, 0.0, vecs[i], vecs[j])
+            ref, ab = O.mapoverlap_1d(w, 2, O.EDGE_CONSTANT, 0.0, shadow[i])
+            host_access(j, S.READ)              # download to resynchronise the shadow with the GPU's fp32 result
+            got = vecs[j].numpy()
+            assert_overlap(got, ref, ab)
+            shadow[j] = got.copy()
+        else:                                   # Reduce
+            dev_access(i, S.READ)
+            s = ctx.reduce(S.FN_ADD, vecs[i])
+            r, ab = O.reduce_f32(O.FN_ADD, shadow[i])
+            assert_reduce_f32(s, r, ab)
+        for k in range(3):
+            assert vecs[k].state() == state[k], f"step {step}: container {k} state {vecs[k].state()} != model {state[k]}"
+    st = ctx.stats()
+    assert st["h2d_count"] == h2d and st["d2h_count"] == d2h, (st, h2d, d2h)
+    assert st["h2d_bytes"] == 4 * n * h2d and st["d2h_bytes"] == 4 * n * d2h
+    for v in vecs:
+        v.destroy()
+
+
+def test_uninitialised_read_and_alias_errors(ctx):
+    a, b = ctx.vector(100), ctx.vector(100)
+    with pytest.raises(S.SkelError):
+        ctx.map(S.FN_ADD, 1.0, a, None, b)       # a was never written
+    a.write(np.ones(100, np.float32))
+    with pytest.raises(S.SkelError):
+        ctx.mapoverlap_1d(np.ones(3, np.float32), 1, S.EDGE_DUPLICATE, 0.0, a, a)  # output aliases input
+    a.destroy()
+    b.destroy()
