@@ -29,6 +29,10 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels at full size, from the
+# `ncu --set full` captures summarised in profiles/r01_ncu_scan.md (bytes)
+NCU_DRAM_BYTES_PER_LAUNCH = {"scan": 2152857000}
+
 METRIC = "skeleton throughput (algorithmic GB/s over one pass of all skeletons at their largest config)"
 UNIT = "GB/s"
 
@@ -228,6 +232,61 @@ def cpu_oracle_pass(scale_div: int = 4, quiet=False):
     return nbytes, dt, 1, desc
 
 
+def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
+    """BASELINE.json configs[4], second half: 100 chained calls Map(x*1.0001) -> MapOverlap1D(r=4) ->
+    Reduce(sum) on one fp32 smart_vector of n elements (reading 15). Reports what the
+    smart containers save: transfers and wall time with the coherence protocol (LAZY) against the
+    "no smart containers" baseline (EAGER, run for fewer iterations; per-iteration figures)."""
+    import torch
+    from paper_1405_2915_b200 import inputs as I
+    x0 = I.uniform01_f32(I.config_seed(5, 1), n)
+    w = I.positive_weights_f32(I.config_seed(3, 14), 9)
+
+    def run(k):
+        a, b = ctx.vector_from(x0), ctx.vector(n)
+        ctx.reset_stats()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0.record()
+        s = 0.0
+        for _ in range(k):
+            ctx.map(S.FN_MULT, 1.0001, a, None, a)
+            ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
+            s = ctx.reduce(S.FN_ADD, b)
+            a, b = b, a
+        e1.record()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        st = ctx.stats()
+        a.destroy()
+        b.destroy()
+        return wall, e0.elapsed_time(e1), st, s
+
+    run(3)  # warm-up (allocations, first-use kernel loads)
+    wall_l, dev_l, st_l, s_l = run(iters)
+    ctx.set_coherence(S.EAGER)
+    try:
+        wall_e, _, st_e, _ = run(eager_iters)
+    finally:
+        ctx.set_coherence(S.LAZY)
+    per_iter_bytes = 20 * n  # Map 8 + MapOverlap 8 + Reduce 4 bytes per element
+    return {
+        "n": n, "iterations": iters,
+        "lazy": {"wall_ms_per_iter": round(wall_l / iters * 1e3, 4), "device_ms_per_iter": round(dev_l / iters, 4),
+                 "GB/s_device": round(per_iter_bytes / (dev_l / iters * 1e-3) / 1e9, 1),
+                 "h2d_bytes_total": st_l["h2d_bytes"], "d2h_bytes_total": st_l["d2h_bytes"],
+                 "h2d_count": st_l["h2d_count"], "d2h_count": st_l["d2h_count"],
+                 "scalar_readbacks": st_l["scalar_d2h_count"], "h2d_elided": st_l["h2d_elided"]},
+        "eager": {"iterations_run": eager_iters, "wall_ms_per_iter": round(wall_e / eager_iters * 1e3, 3),
+                  "h2d_bytes_per_iter": st_e["h2d_bytes"] // eager_iters, "d2h_bytes_per_iter": st_e["d2h_bytes"] // eager_iters,
+                  "transfers_per_iter": (st_e["h2d_count"] + st_e["d2h_count"]) // eager_iters},
+        "speedup_lazy_over_eager": round((wall_e / eager_iters) / (wall_l / iters), 1),
+        "closed_form": {"lazy_h2d_bytes": 4 * n, "lazy_d2h_bytes": 0, "eager_bytes_per_iter": 5 * 4 * n},
+        "last_scalar": s_l,
+    }
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -263,6 +322,7 @@ def main():
     ap.add_argument("--ref-div", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-pipeline", action="store_true")
     ap.add_argument("--force", action="append", default=[], metavar="SKELETON_ID=VARIANT_ID",
                     help="force a kernel variant for a skeleton id (profiling aid), e.g. --force 3=3")
     ap.add_argument("--plan", default=os.path.join(ROOT, "paper_1405_2915_b200", "plans", "b200.plan"))
@@ -327,7 +387,14 @@ def main():
     # per-call breakdown (median over steps)
     peak, peak_src = measured_peaks()
     per = {}
-    fam_time = {}
+    kern_time = {}  # kernel (one template instantiation; edge policy / scan mode are run-time arguments) -> totals
+
+    def kernel_key(name):
+        for suffix in ("_const0", "_dup", "_inclusive_i32", "_exclusive_i32"):
+            if name.endswith(suffix):
+                return name[: -len(suffix)]
+        return name
+
     for i, (name, fam, _, nbytes, elems) in enumerate(wl.ops):
         ts = sorted(ev[k][i][0].elapsed_time(ev[k][i][1]) for k in range(args.steps))
         med = ts[len(ts) // 2]
@@ -335,22 +402,23 @@ def main():
         per[name] = {"us": round(med * 1e3, 2), "GB/s": round(nbytes / (med * 1e-3) / 1e9, 1),
                      "Gelem/s": round(elems / (med * 1e-3) / 1e9, 1), "frac_measured_hbm": round(nbytes / (med * 1e-3) / 1e9 / peak, 4),
                      "frac_8TBs": round(nbytes / (med * 1e-3) / 1e9 / 8000.0, 4), "variant": None}
-        fam_time.setdefault(fam, [0.0, 0, 0, 0])
-        fam_time[fam][0] += mean
-        fam_time[fam][1] += nbytes
-        fam_time[fam][2] += 1
+        kt = kern_time.setdefault(kernel_key(name), [0.0, 0, 0])
+        kt[0] += mean
+        kt[1] += nbytes
+        kt[2] += 1
     # variant names actually chosen
     for i, (name, fam, fn, _, _) in enumerate(wl.ops):
         fn()
         sk, v = ctx.last_variant()
         per[name]["variant"] = S.variant_names(sk)[v]
     ctx.sync()
-    dom = max(fam_time, key=lambda f: fam_time[f][0])
-    dt_ms, dbytes, dcount, _ = fam_time[dom]
+    dom = max(kern_time, key=lambda f: kern_time[f][0])
+    dt_ms, dbytes, dcount = kern_time[dom]
     achieved = dbytes / (dt_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                "frac": round(achieved / peak, 4), "traffic": None, "peak_source": peak_src,
-                "launches_per_step": dcount, "avg_launch_us": round(dt_ms * 1e3 / dcount, 2),
+                "frac": round(achieved / peak, 4), "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if args.scale == 1.0 else None,
+                "algorithmic_bytes_per_launch": dbytes // dcount,
+                "peak_source": peak_src, "launches_per_step": dcount, "avg_launch_us": round(dt_ms * 1e3 / dcount, 2),
                 "share_of_step": round(dt_ms / ms_per_step, 4)}
 
     # ---- small-n latency (config 0: dot n = 2^20, L2 resident) — reported, not part of `value`
@@ -369,6 +437,11 @@ def main():
     dot20_us = s0.elapsed_time(s1) * 1e3 / 50
     a20.destroy()
     b20.destroy()
+
+    # ---- chained pipeline / transfer elision (reported, not part of `value`)
+    pipeline = None
+    if rank == 0 and not args.no_pipeline:
+        pipeline = pipeline_experiment(S, ctx, sz["n26"])
 
     # ---- end to end through host buffers
     e2e = None
@@ -408,7 +481,7 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "per_skeleton": per}
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "per_skeleton": per}
         print(json.dumps(line), flush=True)
     wl.destroy()
     ctx.close()
