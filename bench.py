@@ -332,13 +332,10 @@ def main():
         return run_reference(args)
 
     import torch
-    import torch.distributed as dist
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_1405_2915_b200.replicas import Replicas, env_world
+    world, rank, local = env_world()
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rep = Replicas("nccl", torch.device("cuda", local))  # replicas only: barrier + max-over-ranks timing
     from paper_1405_2915_b200 import skel as S  # fails loudly if libskel.so is missing
 
     sz = sizes(args.scale)
@@ -353,8 +350,8 @@ def main():
     nops = len(wl.ops)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        torch.cuda.synchronize()
+        rep.barrier()
         torch.cuda.synchronize()
 
     # ---- device-resident timing
@@ -375,13 +372,8 @@ def main():
     barrier()
     clocks = sampler.stop()
     launches = ctx.stats()["launches"]
-    total_ms = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
-    value = world * wl.bytes_per_step / (ms_per_step * 1e-3) / 1e9
+    value, ms_per_step = rep.aggregate_throughput(wl.bytes_per_step, e0.elapsed_time(e1) / args.steps)
+    value /= 1e9
     wl.verify(d)
 
     # per-call breakdown (median over steps)
@@ -454,10 +446,7 @@ def main():
             wl.e2e_step()
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = rep.max_over_ranks(dt)
         st = ctx.stats()
         e2e = {"value": round(world * wl.bytes_per_step * args.steps / dt / 1e9, 2), "unit": UNIT,
                "h2d_bytes_per_step": st["h2d_bytes"] // args.steps, "d2h_bytes_per_step": st["d2h_bytes"] // args.steps,
@@ -485,8 +474,7 @@ def main():
         print(json.dumps(line), flush=True)
     wl.destroy()
     ctx.close()
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 if __name__ == "__main__":
