@@ -72,100 +72,160 @@ overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, 
 constexpr int T2_THREADS = 256;  // 32 (x) by 8 (y)
 constexpr int T2_TW = 128;       // tile width in outputs: 32 threads x 4
 
+// stage X~[r0-RY .. r0+TH+RY) x [c0-RXP .. c0+TW+RXP) into `sm` (SH rows of SW floats).
+// ASYNC: groups that lie inside the matrix go through cp.async (LDGSTS, no registers, completion
+// via cp.async.wait_group); groups touching an edge are computed with the edge policy and stored.
+template <int RY, int RX, int OY, bool ASYNC>
+__device__ __forceinline__ void stage_tile2(float* sm, const float* in, long long rows, long long cols, long long r0,
+                                            long long c0, int edge, float pad) {
+  constexpr int RXP = (RX + 3) / 4 * 4;
+  constexpr int TH = 8 * OY, SW = T2_TW + 2 * RXP, SH = TH + 2 * RY;
+#pragma unroll 4
+  for (int g = threadIdx.x; g < SH * (SW / 4); g += T2_THREADS) {
+    const int gy = g / (SW / 4), gx = g - gy * (SW / 4);
+    const long long p = r0 - RY + gy, q = c0 - RXP + 4 * gx;
+    float* dst = sm + gy * SW + 4 * gx;
+    if (p >= 0 && p < rows && q >= 0 && q + 3 < cols) {
+      if constexpr (ASYNC) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(in + p * cols + q) : "memory");
+      } else {
+        uint32_t raw[4];
+        ld_stream<4, true>(raw, in + p * cols + q);
+        *reinterpret_cast<float4*>(dst) =
+            make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
+      }
+    } else {
+      float4 v;
+      v.x = ext2(in, rows, cols, p, q, edge, pad);
+      v.y = ext2(in, rows, cols, p, q + 1, edge, pad);
+      v.z = ext2(in, rows, cols, p, q + 2, edge, pad);
+      v.w = ext2(in, rows, cols, p, q + 3, edge, pad);
+      *reinterpret_cast<float4*>(dst) = v;
+    }
+  }
+}
+
+// a thread's 4 (x) by OY (y) outputs from the staged tile, written to `out`
+template <int RY, int RX, int OY, typename WT>
+__device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, float* out, long long rows, long long cols,
+                                              long long r0, long long c0) {
+  constexpr int RXP = (RX + 3) / 4 * 4;
+  constexpr int SW = T2_TW + 2 * RXP;
+  constexpr int NGX = (4 + 2 * RXP) / 4;
+  constexpr int FW = 2 * RX + 1;
+  constexpr bool PER_ROW = (2 * RY + 1) * (2 * RX + 1) > 33;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  float acc[OY][4];
+#pragma unroll
+  for (int o = 0; o < OY; ++o)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) acc[o][e] = 0.f;
+
+#pragma unroll
+  for (int ir = 0; ir < OY + 2 * RY; ++ir) {
+    const float* srow = sm + (ty * OY + ir) * SW + tx * 4;
+    float v[4 * NGX];
+#pragma unroll
+    for (int g = 0; g < NGX; ++g) {
+      const float4 t = *reinterpret_cast<const float4*>(srow + 4 * g);
+      v[4 * g] = t.x; v[4 * g + 1] = t.y; v[4 * g + 2] = t.z; v[4 * g + 3] = t.w;
+    }
+#pragma unroll
+    for (int o = 0; o < OY; ++o) {
+      const int a = ir - o;  // filter row that this staged row feeds for output row o
+      if (a >= 0 && a <= 2 * RY) {
+        if constexpr (PER_ROW) {
+          float p[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+          for (int b = 0; b < FW; ++b)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) acc[o][e] = a == 0 ? p[e] : acc[o][e] + p[e];
+        } else {
+#pragma unroll
+          for (int b = 0; b < FW; ++b)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
+        }
+      }
+    }
+  }
+  const long long oc = c0 + tx * 4;
+#pragma unroll
+  for (int o = 0; o < OY; ++o) {
+    const long long orow = r0 + ty * OY + o;
+    if (orow < rows) {
+      float* dst = out + orow * cols + oc;
+      if (oc + 3 < cols) {
+        uint32_t raw[4] = {__float_as_uint(acc[o][0]), __float_as_uint(acc[o][1]), __float_as_uint(acc[o][2]),
+                           __float_as_uint(acc[o][3])};
+        st_stream<4>(dst, raw);
+      } else {
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+          if (oc + e < cols) dst[e] = acc[o][e];
+      }
+    }
+  }
+}
+
 template <int RY, int RX, int OY, typename WT>
 __global__ void __launch_bounds__(T2_THREADS)
 overlap2d_tiled_kernel(const __grid_constant__ WT W, int edge, float pad, const float* in, float* out, size_t rows,
                        size_t cols) {
-  constexpr int RXP = (RX + 3) / 4 * 4;
   constexpr int TH = 8 * OY;
-  constexpr int SW = T2_TW + 2 * RXP;  // staged row length (floats)
-  constexpr int SH = TH + 2 * RY;      // staged rows
-  constexpr int NGX = (4 + 2 * RXP) / 4;
-  constexpr int FW = 2 * RX + 1;
-  constexpr bool PER_ROW = (2 * RY + 1) * (2 * RX + 1) > 33;
   extern __shared__ __align__(16) float sm[];
-
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   const size_t tiles_x = (cols + T2_TW - 1) / T2_TW, tiles_y = (rows + TH - 1) / TH;
   const size_t ntiles = tiles_x * tiles_y;
   for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const size_t tyi = tile / tiles_x;
     const long long r0 = static_cast<long long>(tyi * TH);
     const long long c0 = static_cast<long long>((tile - tyi * tiles_x) * T2_TW);
-    // stage X~[r0-RY .. r0+TH+RY) x [c0-RXP .. c0+TW+RXP)
-#pragma unroll 4
-    for (int g = threadIdx.x; g < SH * (SW / 4); g += T2_THREADS) {
-      const int gy = g / (SW / 4), gx = g - gy * (SW / 4);
-      const long long p = r0 - RY + gy, q = c0 - RXP + 4 * gx;
-      float4 v;
-      if (p >= 0 && p < (long long)rows && q >= 0 && q + 3 < (long long)cols) {
-        uint32_t raw[4];
-        ld_stream<4, true>(raw, in + p * (long long)cols + q);
-        v = make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
-      } else {
-        v.x = ext2(in, rows, cols, p, q, edge, pad);
-        v.y = ext2(in, rows, cols, p, q + 1, edge, pad);
-        v.z = ext2(in, rows, cols, p, q + 2, edge, pad);
-        v.w = ext2(in, rows, cols, p, q + 3, edge, pad);
-      }
-      *reinterpret_cast<float4*>(sm + gy * SW + 4 * gx) = v;
-    }
+    stage_tile2<RY, RX, OY, false>(sm, in, rows, cols, r0, c0, edge, pad);
     __syncthreads();
-
-    float acc[OY][4];
-#pragma unroll
-    for (int o = 0; o < OY; ++o)
-#pragma unroll
-      for (int e = 0; e < 4; ++e) acc[o][e] = 0.f;
-
-#pragma unroll
-    for (int ir = 0; ir < OY + 2 * RY; ++ir) {
-      const float* srow = sm + (ty * OY + ir) * SW + tx * 4;
-      float v[4 * NGX];
-#pragma unroll
-      for (int g = 0; g < NGX; ++g) {
-        const float4 t = *reinterpret_cast<const float4*>(srow + 4 * g);
-        v[4 * g] = t.x; v[4 * g + 1] = t.y; v[4 * g + 2] = t.z; v[4 * g + 3] = t.w;
-      }
-#pragma unroll
-      for (int o = 0; o < OY; ++o) {
-        const int a = ir - o;  // filter row that this staged row feeds for output row o
-        if (a >= 0 && a <= 2 * RY) {
-          if constexpr (PER_ROW) {
-            float p[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int b = 0; b < FW; ++b)
-#pragma unroll
-              for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
-#pragma unroll
-            for (int e = 0; e < 4; ++e) acc[o][e] = a == 0 ? p[e] : acc[o][e] + p[e];
-          } else {
-#pragma unroll
-            for (int b = 0; b < FW; ++b)
-#pragma unroll
-              for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
-          }
-        }
-      }
-    }
-    const long long oc = c0 + tx * 4;
-#pragma unroll
-    for (int o = 0; o < OY; ++o) {
-      const long long orow = r0 + ty * OY + o;
-      if (orow < (long long)rows) {
-        float* dst = out + orow * (long long)cols + oc;
-        if (oc + 3 < (long long)cols) {
-          uint32_t raw[4] = {__float_as_uint(acc[o][0]), __float_as_uint(acc[o][1]), __float_as_uint(acc[o][2]),
-                             __float_as_uint(acc[o][3])};
-          st_stream<4>(dst, raw);
-        } else {
-#pragma unroll
-          for (int e = 0; e < 4; ++e)
-            if (oc + e < (long long)cols) dst[e] = acc[o][e];
-        }
-      }
-    }
+    compute_tile2<RY, RX, OY, WT>(sm, W, out, rows, cols, r0, c0);
     __syncthreads();
+  }
+}
+
+// Double-buffered persistent form ("_db"): a grid of co-resident blocks walks the tiles; while a
+// block computes tile i from one shared-memory buffer, the cp.async copies of tile i+1 fill the
+// other, so the load phase of a block no longer alternates with its compute phase.
+template <int RY, int RX, int OY, typename WT>
+__global__ void __launch_bounds__(T2_THREADS)
+overlap2d_tiled_db_kernel(const __grid_constant__ WT W, int edge, float pad, const float* in, float* out, size_t rows,
+                          size_t cols) {
+  constexpr int RXP = (RX + 3) / 4 * 4;
+  constexpr int TH = 8 * OY, SW = T2_TW + 2 * RXP, SH = TH + 2 * RY;
+  extern __shared__ __align__(16) float sm[];
+  const size_t tiles_x = (cols + T2_TW - 1) / T2_TW, tiles_y = (rows + TH - 1) / TH;
+  const size_t ntiles = tiles_x * tiles_y;
+  auto origin = [&](size_t tile, long long& r0, long long& c0) {
+    const size_t tyi = tile / tiles_x;
+    r0 = static_cast<long long>(tyi * TH);
+    c0 = static_cast<long long>((tile - tyi * tiles_x) * T2_TW);
+  };
+  long long r0, c0;
+  size_t tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  origin(tile, r0, c0);
+  stage_tile2<RY, RX, OY, true>(sm, in, rows, cols, r0, c0, edge, pad);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  int buf = 0;
+  for (; tile < ntiles; tile += gridDim.x, buf ^= 1) {
+    const size_t next = tile + gridDim.x;
+    if (next < ntiles) {
+      long long nr0, nc0;
+      origin(next, nr0, nc0);
+      stage_tile2<RY, RX, OY, true>(sm + (buf ^ 1) * SH * SW, in, rows, cols, nr0, nc0, edge, pad);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 1;" ::: "memory");  // the current tile has landed (this thread's copies)
+    __syncthreads();                                       // ... and everybody else's
+    origin(tile, r0, c0);
+    compute_tile2<RY, RX, OY, WT>(sm + buf * SH * SW, W, out, rows, cols, r0, c0);
+    __syncthreads();  // the buffer is refilled by the next iteration's prefetch
   }
 }
 
@@ -189,6 +249,25 @@ cudaError_t launch_tiled2(const Launch& L, const WT& w, int edge, float pad, con
   return cudaGetLastError();
 }
 
+template <int RY, int RX, int OY, typename WT>
+cudaError_t launch_tiled2_db(const Launch& L, const WT& w, int edge, float pad, const float* in, float* out, size_t rows,
+                             size_t cols) {
+  constexpr size_t smem = 2 * tiled2_smem<RY, RX, OY>();
+  auto kern = overlap2d_tiled_db_kernel<RY, RX, OY, WT>;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T2_THREADS, smem) != cudaSuccess || per_sm < 1)
+      return cudaErrorInvalidValue;
+  }
+  const size_t ntiles = ((cols + T2_TW - 1) / T2_TW) * ((rows + 8 * OY - 1) / (8 * OY));
+  size_t grid = size_t(L.sms) * per_sm;
+  if (grid > ntiles) grid = ntiles;
+  kern<<<(unsigned)grid, T2_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
 template <typename WT>
 cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edge, float pad, const float* in,
                            float* out, size_t rows, size_t cols) {
@@ -201,8 +280,8 @@ cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edg
   return cudaGetLastError();
 }
 
-const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8"};
-constexpr int kNumVariants = 3;
+const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8", "tiled_oy4_db", "tiled_oy8_db"};
+constexpr int kNumVariants = 5;
 
 inline bool tiled_alignment_ok(const void* in, const void* out, size_t cols) {
   return reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 && cols % 4 == 0;
@@ -226,8 +305,13 @@ cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, in
   if (v == 0) return launch_direct2<Weights1D>(L, w, r, 0, edge, pad, in, out, rows, cols);
 #define SKEL_COL_CASE(R)                                                                                      \
   case R:                                                                                                     \
-    return v == 1 ? launch_tiled2<R, 0, 4, Weights1D>(L, w, edge, pad, in, out, rows, cols)                   \
-                  : launch_tiled2<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);
+    switch (v) {                                                                                              \
+      case 1: return launch_tiled2<R, 0, 4, Weights1D>(L, w, edge, pad, in, out, rows, cols);                 \
+      case 2: return launch_tiled2<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);                 \
+      case 3: return launch_tiled2_db<R, 0, 4, Weights1D>(L, w, edge, pad, in, out, rows, cols);              \
+      case 4: return launch_tiled2_db<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);              \
+    }                                                                                                         \
+    break;
   switch (r) {
     SKEL_COL_CASE(1)
     SKEL_COL_CASE(2)
@@ -256,8 +340,13 @@ cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry,
   if (v == 0) return launch_direct2<Weights2D>(L, w, ry, rx, edge, pad, in, out, rows, cols);
 #define SKEL_2D_CASE(R)                                                                                       \
   case R:                                                                                                     \
-    return v == 1 ? launch_tiled2<R, R, 4, Weights2D>(L, w, edge, pad, in, out, rows, cols)                   \
-                  : launch_tiled2<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);
+    switch (v) {                                                                                              \
+      case 1: return launch_tiled2<R, R, 4, Weights2D>(L, w, edge, pad, in, out, rows, cols);                 \
+      case 2: return launch_tiled2<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);                 \
+      case 3: return launch_tiled2_db<R, R, 4, Weights2D>(L, w, edge, pad, in, out, rows, cols);              \
+      case 4: return launch_tiled2_db<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);              \
+    }                                                                                                         \
+    break;
   switch (ry) {
     SKEL_2D_CASE(1)
     SKEL_2D_CASE(2)
