@@ -62,86 +62,133 @@ template <int O> __device__ __forceinline__ int phys(int sc) {  // padded smem i
   else return sc + 4 * (sc / O);
 }
 
+// stage x~[c0 - HP, c0 + TILE + HP) of one row at tile coordinates sc = 0 .. SPAN-1 (padded layout).
+// ASYNC: in-range 128-bit groups go through cp.async (LDGSTS), edge groups are computed and stored.
+template <int R, int O, bool ASYNC>
+__device__ __forceinline__ void stage_tile1(float* sm, const float* x, long long cols, long long c0, int edge, float pad) {
+  constexpr int HP = (R + 3) / 4 * 4;
+  constexpr int SPAN = T1_THREADS * O + 2 * HP;
+  for (int g = threadIdx.x; g < SPAN / 4; g += T1_THREADS) {
+    const long long c = c0 - HP + 4 * g;
+    float* dst = sm + phys<O>(4 * g);
+    if (c >= 0 && c + 3 < cols) {
+      if constexpr (ASYNC) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(x + c) : "memory");
+      } else {
+        uint32_t raw[4];
+        ld_stream<4, true>(raw, x + c);
+        *reinterpret_cast<float4*>(dst) =
+            make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
+      }
+    } else {
+      float4 v;
+      v.x = ext_row(x, cols, c, edge, pad);
+      v.y = ext_row(x, cols, c + 1, edge, pad);
+      v.z = ext_row(x, cols, c + 2, edge, pad);
+      v.w = ext_row(x, cols, c + 3, edge, pad);
+      *reinterpret_cast<float4*>(dst) = v;
+    }
+  }
+}
+
+// thread t produces outputs c0 + t*O .. + O-1 from tile coordinates t*O .. t*O + O + 2HP - 1
+template <int R, int O>
+__device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& W, float* orow, long long cols, long long c0) {
+  constexpr int HP = (R + 3) / 4 * 4;
+  constexpr int NG = (O + 2 * HP) / 4;  // 128-bit groups a thread reads
+  float acc[O];
+#pragma unroll
+  for (int o = 0; o < O; ++o) acc[o] = 0.f;
+  const int sc0 = threadIdx.x * O;
+#pragma unroll
+  for (int g = 0; g < NG; ++g) {
+    const float4 v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
+    const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
+      // tap k = p - HP - o + R, 0 <= k <= 2R
+#pragma unroll
+      for (int o = 0; o < O; ++o) {
+        const int k = 4 * g + e - HP - o + R;
+        if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+      }
+    }
+  }
+  const long long cbase = c0 + sc0;
+  if (cbase + O <= cols) {
+    float* dst = orow + cbase;
+    if constexpr (O % 8 == 0) {
+#pragma unroll
+      for (int q = 0; q < O / 8; ++q) {
+        uint32_t raw[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) raw[e] = __float_as_uint(acc[8 * q + e]);
+        st_stream<8>(dst + 8 * q, raw);
+      }
+    } else {
+#pragma unroll
+      for (int q = 0; q < O / 4; ++q) {
+        uint32_t raw[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) raw[e] = __float_as_uint(acc[4 * q + e]);
+        st_stream<4>(dst + 4 * q, raw);
+      }
+    }
+  } else {
+#pragma unroll
+    for (int o = 0; o < O; ++o)
+      if (cbase + o < cols) orow[cbase + o] = acc[o];
+  }
+}
+
 template <int R, int O>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tiled_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
                        size_t rows, size_t cols) {
-  constexpr int HP = (R + 3) / 4 * 4;            // halo rounded up to whole 128-bit groups
-  constexpr int TILE = T1_THREADS * O;           // outputs per tile
-  constexpr int SPAN = TILE + 2 * HP;            // staged elements per tile
-  constexpr int NG = (O + 2 * HP) / 4;           // 128-bit groups a thread reads
+  constexpr int TILE = T1_THREADS * O;  // outputs per tile
   extern __shared__ __align__(16) float sm[];
-
   const size_t tiles_per_row = (cols + TILE - 1) / TILE;
   const size_t ntiles = rows * tiles_per_row;
   for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const size_t row = tile / tiles_per_row;
     const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE);  // first output column
-    const float* x = in + row * cols;
-    // stage x~[c0 - HP, c0 + TILE + HP) at tile coordinates sc = 0 .. SPAN-1
-    for (int g = threadIdx.x; g < SPAN / 4; g += T1_THREADS) {
-      const long long c = c0 - HP + 4 * g;
-      float4 v;
-      if (c >= 0 && c + 3 < static_cast<long long>(cols)) {
-        uint32_t raw[4];
-        ld_stream<4, true>(raw, x + c);
-        v = make_float4(__uint_as_float(raw[0]), __uint_as_float(raw[1]), __uint_as_float(raw[2]), __uint_as_float(raw[3]));
-      } else {
-        v.x = ext_row(x, (long long)cols, c, edge, pad);
-        v.y = ext_row(x, (long long)cols, c + 1, edge, pad);
-        v.z = ext_row(x, (long long)cols, c + 2, edge, pad);
-        v.w = ext_row(x, (long long)cols, c + 3, edge, pad);
-      }
-      *reinterpret_cast<float4*>(sm + phys<O>(4 * g)) = v;
-    }
+    stage_tile1<R, O, false>(sm, in + row * cols, (long long)cols, c0, edge, pad);
     __syncthreads();
-
-    // thread t produces outputs c0 + t*O .. + O-1 from tile coordinates t*O .. t*O + O + 2HP - 1
-    float acc[O];
-#pragma unroll
-    for (int o = 0; o < O; ++o) acc[o] = 0.f;
-    const int sc0 = threadIdx.x * O;
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
-      const float4 v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
-      const float v[4] = {v4.x, v4.y, v4.z, v4.w};
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
-        // tap k = p - HP - o + R, 0 <= k <= 2R
-#pragma unroll
-        for (int o = 0; o < O; ++o) {
-          const int k = 4 * g + e - HP - o + R;
-          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
-        }
-      }
-    }
-    const long long cbase = c0 + sc0;
-    if (cbase + O <= static_cast<long long>(cols)) {
-      float* dst = out + row * cols + cbase;
-      if constexpr (O % 8 == 0) {
-#pragma unroll
-        for (int q = 0; q < O / 8; ++q) {
-          uint32_t raw[8];
-#pragma unroll
-          for (int e = 0; e < 8; ++e) raw[e] = __float_as_uint(acc[8 * q + e]);
-          st_stream<8>(dst + 8 * q, raw);
-        }
-      } else {
-#pragma unroll
-        for (int q = 0; q < O / 4; ++q) {
-          uint32_t raw[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) raw[e] = __float_as_uint(acc[4 * q + e]);
-          st_stream<4>(dst + 4 * q, raw);
-        }
-      }
-    } else {
-#pragma unroll
-      for (int o = 0; o < O; ++o)
-        if (cbase + o < static_cast<long long>(cols)) out[row * cols + cbase + o] = acc[o];
-    }
+    compute_tile1<R, O>(sm, W, out + row * cols, (long long)cols, c0);
     __syncthreads();  // the tile buffer is reused
+  }
+}
+
+// Double-buffered persistent form ("_db"): while a block computes tile i from one buffer, the
+// cp.async copies of tile i+1 fill the other.
+template <int R, int O>
+__global__ void __launch_bounds__(T1_THREADS)
+overlap1d_tiled_db_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
+                          size_t rows, size_t cols, unsigned buf_floats) {
+  constexpr int TILE = T1_THREADS * O;
+  extern __shared__ __align__(16) float sm[];
+  const size_t tiles_per_row = (cols + TILE - 1) / TILE;
+  const size_t ntiles = rows * tiles_per_row;
+  size_t tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  auto stage = [&](size_t t, int b) {
+    const size_t row = t / tiles_per_row;
+    const long long c0 = static_cast<long long>((t - row * tiles_per_row) * TILE);
+    stage_tile1<R, O, true>(sm + size_t(b) * buf_floats, in + row * cols, (long long)cols, c0, edge, pad);
+  };
+  stage(tile, 0);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  int buf = 0;
+  for (; tile < ntiles; tile += gridDim.x, buf ^= 1) {
+    if (tile + gridDim.x < ntiles) stage(tile + gridDim.x, buf ^ 1);
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 1;" ::: "memory");
+    __syncthreads();
+    const size_t row = tile / tiles_per_row;
+    const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE);
+    compute_tile1<R, O>(sm + size_t(buf) * buf_floats, W, out + row * cols, (long long)cols, c0);
+    __syncthreads();
   }
 }
 
@@ -231,7 +278,8 @@ template <int O> constexpr size_t tiled_smem_bytes(int R) {
 }
 
 struct O1Variant { const char* name; int o; };  // o == 0: direct
-const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16}};
+const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16},
+                               {"tiled_o8_db", 108}, {"tiled_o16_db", 116}};
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
@@ -251,6 +299,41 @@ cudaError_t launch_tiled(const Launch& L, const Weights1D& w, int edge, float pa
   overlap1d_tiled_kernel<R, O><<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols);
   ++*L.launches;
   return cudaGetLastError();
+}
+
+template <int R, int O>
+cudaError_t launch_tiled_db(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
+                            size_t rows, size_t cols) {
+  constexpr int TILE = T1_THREADS * O;
+  const size_t one = (tiled_smem_bytes<O>(R) + 15) / 16 * 16;
+  const size_t smem = 2 * one;
+  auto kern = overlap1d_tiled_db_kernel<R, O>;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T1_THREADS, smem) != cudaSuccess || per_sm < 1)
+      return cudaErrorInvalidValue;
+  }
+  const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
+  size_t grid = size_t(L.sms) * per_sm;
+  if (grid > ntiles) grid = ntiles;
+  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols, (unsigned)(one / 4));
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <int O>
+cudaError_t launch_tiled_db_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in,
+                              float* out, size_t rows, size_t cols) {
+  switch (r) {
+    case 1: return launch_tiled_db<1, O>(L, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_tiled_db<2, O>(L, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_tiled_db<3, O>(L, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_tiled_db<4, O>(L, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_tiled_db<8, O>(L, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_tiled_db<16, O>(L, w, edge, pad, in, out, rows, cols);
+  }
+  return cudaErrorInvalidValue;
 }
 
 template <int O>
@@ -296,6 +379,8 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 4: return launch_tiled_r<4>(L, w, r, edge, pad, in, out, rows, cols);
     case 8: return launch_tiled_r<8>(L, w, r, edge, pad, in, out, rows, cols);
     case 16: return launch_tiled_r<16>(L, w, r, edge, pad, in, out, rows, cols);
+    case 108: return launch_tiled_db_r<8>(L, w, r, edge, pad, in, out, rows, cols);
+    case 116: return launch_tiled_db_r<16>(L, w, r, edge, pad, in, out, rows, cols);
     case -16:
       switch (r) {
         case 1: return launch_shfl<1>(L, w, edge, pad, in, out, rows, cols);
