@@ -105,8 +105,23 @@ __device__ __forceinline__ void stage_tile2(float* sm, const float* in, long lon
   }
 }
 
+// packed fp32 pairs (Blackwell FFMA2): d = a * b + c on both halves of an aligned register pair
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x0, float x1) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pack2(w, w)), "l"(pack2(x0, x1)), "l"(pack2(lo, hi)));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+
 // a thread's 4 (x) by OY (y) outputs from the staged tile, written to `out`
-template <int RY, int RX, int OY, typename WT>
+// PK: taps whose window index is even use one FFMA2 per output pair (the pair (v[i], v[i+1]) of a
+// 128-bit shared load is an aligned register pair); odd taps stay scalar. Each output still sums its
+// taps in the order b = 0 .. 2RX, so the result is bit-identical to the scalar form.
+template <int RY, int RX, int OY, typename WT, bool PK = false>
 __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, float* out, long long rows, long long cols,
                                               long long r0, long long c0) {
   constexpr int RXP = (RX + 3) / 4 * 4;
@@ -137,16 +152,28 @@ __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, floa
         if constexpr (PER_ROW) {
           float p[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-          for (int b = 0; b < FW; ++b)
+          for (int b = 0; b < FW; ++b) {
+            if (PK && (RXP - RX + b) % 2 == 0) {
+              fma2_into(p[0], p[1], W.w[a * FW + b], v[RXP - RX + b], v[RXP - RX + b + 1]);
+              fma2_into(p[2], p[3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
+            } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
+              for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
+            }
+          }
 #pragma unroll
           for (int e = 0; e < 4; ++e) acc[o][e] = a == 0 ? p[e] : acc[o][e] + p[e];
         } else {
 #pragma unroll
-          for (int b = 0; b < FW; ++b)
+          for (int b = 0; b < FW; ++b) {
+            if (PK && (RXP - RX + b) % 2 == 0) {
+              fma2_into(acc[o][0], acc[o][1], W.w[a * FW + b], v[RXP - RX + b], v[RXP - RX + b + 1]);
+              fma2_into(acc[o][2], acc[o][3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
+            } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
+              for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
+            }
+          }
         }
       }
     }
@@ -192,7 +219,7 @@ overlap2d_tiled_kernel(const __grid_constant__ WT W, int edge, float pad, const 
 // Double-buffered persistent form ("_db"): a grid of co-resident blocks walks the tiles; while a
 // block computes tile i from one shared-memory buffer, the cp.async copies of tile i+1 fill the
 // other, so the load phase of a block no longer alternates with its compute phase.
-template <int RY, int RX, int OY, typename WT>
+template <int RY, int RX, int OY, typename WT, bool PK>
 __global__ void __launch_bounds__(T2_THREADS)
 overlap2d_tiled_db_kernel(const __grid_constant__ WT W, int edge, float pad, const float* in, float* out, size_t rows,
                           size_t cols) {
@@ -224,7 +251,7 @@ overlap2d_tiled_db_kernel(const __grid_constant__ WT W, int edge, float pad, con
     asm volatile("cp.async.wait_group 1;" ::: "memory");  // the current tile has landed (this thread's copies)
     __syncthreads();                                       // ... and everybody else's
     origin(tile, r0, c0);
-    compute_tile2<RY, RX, OY, WT>(sm + buf * SH * SW, W, out, rows, cols, r0, c0);
+    compute_tile2<RY, RX, OY, WT, PK>(sm + buf * SH * SW, W, out, rows, cols, r0, c0);
     __syncthreads();  // the buffer is refilled by the next iteration's prefetch
   }
 }
@@ -249,11 +276,11 @@ cudaError_t launch_tiled2(const Launch& L, const WT& w, int edge, float pad, con
   return cudaGetLastError();
 }
 
-template <int RY, int RX, int OY, typename WT>
+template <int RY, int RX, int OY, typename WT, bool PK = false>
 cudaError_t launch_tiled2_db(const Launch& L, const WT& w, int edge, float pad, const float* in, float* out, size_t rows,
                              size_t cols) {
   constexpr size_t smem = 2 * tiled2_smem<RY, RX, OY>();
-  auto kern = overlap2d_tiled_db_kernel<RY, RX, OY, WT>;
+  auto kern = overlap2d_tiled_db_kernel<RY, RX, OY, WT, PK>;
   static int per_sm = 0;
   if (per_sm == 0) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -280,8 +307,9 @@ cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edg
   return cudaGetLastError();
 }
 
-const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8", "tiled_oy4_db", "tiled_oy8_db"};
-constexpr int kNumVariants = 5;
+const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8", "tiled_oy4_db", "tiled_oy8_db", "tiled_oy4_db_ffma2",
+                              "tiled_oy8_db_ffma2"};
+constexpr int kNumVariants = 7;
 
 inline bool tiled_alignment_ok(const void* in, const void* out, size_t cols) {
   return reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 && cols % 4 == 0;
@@ -310,6 +338,8 @@ cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, in
       case 2: return launch_tiled2<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);                 \
       case 3: return launch_tiled2_db<R, 0, 4, Weights1D>(L, w, edge, pad, in, out, rows, cols);              \
       case 4: return launch_tiled2_db<R, 0, 8, Weights1D>(L, w, edge, pad, in, out, rows, cols);              \
+      case 5: return launch_tiled2_db<R, 0, 4, Weights1D, true>(L, w, edge, pad, in, out, rows, cols);        \
+      case 6: return launch_tiled2_db<R, 0, 8, Weights1D, true>(L, w, edge, pad, in, out, rows, cols);        \
     }                                                                                                         \
     break;
   switch (r) {
@@ -345,6 +375,8 @@ cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry,
       case 2: return launch_tiled2<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);                 \
       case 3: return launch_tiled2_db<R, R, 4, Weights2D>(L, w, edge, pad, in, out, rows, cols);              \
       case 4: return launch_tiled2_db<R, R, 8, Weights2D>(L, w, edge, pad, in, out, rows, cols);              \
+      case 5: return launch_tiled2_db<R, R, 4, Weights2D, true>(L, w, edge, pad, in, out, rows, cols);        \
+      case 6: return launch_tiled2_db<R, R, 8, Weights2D, true>(L, w, edge, pad, in, out, rows, cols);        \
     }                                                                                                         \
     break;
   switch (ry) {
