@@ -92,7 +92,21 @@ __device__ __forceinline__ void stage_tile1(float* sm, const float* x, long long
 }
 
 // thread t produces outputs c0 + t*O .. + O-1 from tile coordinates t*O .. t*O + O + 2HP - 1
-template <int R, int O>
+// packed fp32 pair (Blackwell FFMA2): (lo, hi) += w * (x0, x1), one instruction on an aligned register pair
+__device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x0, float x1) {
+  unsigned long long ww, xx, cc, d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ww) : "f"(w), "f"(w));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(xx) : "f"(x0), "f"(x1));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(cc) : "f"(lo), "f"(hi));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(ww), "l"(xx), "l"(cc));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+
+// thread t produces outputs c0 + t*O .. + O-1 from tile coordinates t*O .. t*O + O + 2HP - 1.
+// PK: the FMAs (x[p] -> out o) and (x[p+1] -> out o+1) with p, o even share the tap and are ONE FFMA2
+// on two aligned register pairs; the other half of the FMAs stays scalar. Emission order keeps, for
+// every output, its taps in ascending order, so the result is bit-identical to the scalar form.
+template <int R, int O, bool PK = false>
 __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& W, float* orow, long long cols, long long c0) {
   constexpr int HP = (R + 3) / 4 * 4;
   constexpr int NG = (O + 2 * HP) / 4;  // 128-bit groups a thread reads
@@ -104,14 +118,35 @@ __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& 
   for (int g = 0; g < NG; ++g) {
     const float4 v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
     const float v[4] = {v4.x, v4.y, v4.z, v4.w};
+    // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
+    // tap k = p - HP - o + R, 0 <= k <= 2R
+    if constexpr (PK) {
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
-      // tap k = p - HP - o + R, 0 <= k <= 2R
+      for (int e = 0; e < 4; e += 2) {
 #pragma unroll
-      for (int o = 0; o < O; ++o) {
-        const int k = 4 * g + e - HP - o + R;
-        if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+        for (int o = 1; o < O; o += 2) {  // x[p] -> odd outputs (scalar), before their paired tap p+1
+          const int k = 4 * g + e - HP - o + R;
+          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+        }
+#pragma unroll
+        for (int o = 0; o < O; o += 2) {  // (x[p], x[p+1]) -> (o, o+1): one FFMA2
+          const int k = 4 * g + e - HP - o + R;
+          if (k >= 0 && k <= 2 * R) fma2_into(acc[o], acc[o + 1], W.w[k], v[e], v[e + 1]);
+        }
+#pragma unroll
+        for (int o = 0; o < O; o += 2) {  // x[p+1] -> even outputs (scalar)
+          const int k = 4 * g + e + 1 - HP - o + R;
+          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e + 1], acc[o]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+#pragma unroll
+        for (int o = 0; o < O; ++o) {
+          const int k = 4 * g + e - HP - o + R;
+          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+        }
       }
     }
   }
@@ -162,7 +197,7 @@ overlap1d_tiled_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
 
 // Double-buffered persistent form ("_db"): while a block computes tile i from one buffer, the
 // cp.async copies of tile i+1 fill the other.
-template <int R, int O>
+template <int R, int O, bool PK>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tiled_db_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
                           size_t rows, size_t cols, unsigned buf_floats) {
@@ -187,7 +222,7 @@ overlap1d_tiled_db_kernel(const __grid_constant__ Weights1D W, int edge, float p
     __syncthreads();
     const size_t row = tile / tiles_per_row;
     const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE);
-    compute_tile1<R, O>(sm + size_t(buf) * buf_floats, W, out + row * cols, (long long)cols, c0);
+    compute_tile1<R, O, PK>(sm + size_t(buf) * buf_floats, W, out + row * cols, (long long)cols, c0);
     __syncthreads();
   }
 }
@@ -279,7 +314,7 @@ template <int O> constexpr size_t tiled_smem_bytes(int R) {
 
 struct O1Variant { const char* name; int o; };  // o == 0: direct
 const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16},
-                               {"tiled_o8_db", 108}, {"tiled_o16_db", 116}};
+                               {"tiled_o8_db", 108}, {"tiled_o16_db", 116}, {"tiled_o16_db_ffma2", 216}};
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
@@ -301,13 +336,13 @@ cudaError_t launch_tiled(const Launch& L, const Weights1D& w, int edge, float pa
   return cudaGetLastError();
 }
 
-template <int R, int O>
+template <int R, int O, bool PK>
 cudaError_t launch_tiled_db(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
                             size_t rows, size_t cols) {
   constexpr int TILE = T1_THREADS * O;
   const size_t one = (tiled_smem_bytes<O>(R) + 15) / 16 * 16;
   const size_t smem = 2 * one;
-  auto kern = overlap1d_tiled_db_kernel<R, O>;
+  auto kern = overlap1d_tiled_db_kernel<R, O, PK>;
   static int per_sm = 0;
   if (per_sm == 0) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -322,16 +357,16 @@ cudaError_t launch_tiled_db(const Launch& L, const Weights1D& w, int edge, float
   return cudaGetLastError();
 }
 
-template <int O>
+template <int O, bool PK>
 cudaError_t launch_tiled_db_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in,
                               float* out, size_t rows, size_t cols) {
   switch (r) {
-    case 1: return launch_tiled_db<1, O>(L, w, edge, pad, in, out, rows, cols);
-    case 2: return launch_tiled_db<2, O>(L, w, edge, pad, in, out, rows, cols);
-    case 3: return launch_tiled_db<3, O>(L, w, edge, pad, in, out, rows, cols);
-    case 4: return launch_tiled_db<4, O>(L, w, edge, pad, in, out, rows, cols);
-    case 8: return launch_tiled_db<8, O>(L, w, edge, pad, in, out, rows, cols);
-    case 16: return launch_tiled_db<16, O>(L, w, edge, pad, in, out, rows, cols);
+    case 1: return launch_tiled_db<1, O, PK>(L, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_tiled_db<2, O, PK>(L, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_tiled_db<3, O, PK>(L, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_tiled_db<4, O, PK>(L, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_tiled_db<8, O, PK>(L, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_tiled_db<16, O, PK>(L, w, edge, pad, in, out, rows, cols);
   }
   return cudaErrorInvalidValue;
 }
@@ -379,8 +414,9 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 4: return launch_tiled_r<4>(L, w, r, edge, pad, in, out, rows, cols);
     case 8: return launch_tiled_r<8>(L, w, r, edge, pad, in, out, rows, cols);
     case 16: return launch_tiled_r<16>(L, w, r, edge, pad, in, out, rows, cols);
-    case 108: return launch_tiled_db_r<8>(L, w, r, edge, pad, in, out, rows, cols);
-    case 116: return launch_tiled_db_r<16>(L, w, r, edge, pad, in, out, rows, cols);
+    case 108: return launch_tiled_db_r<8, false>(L, w, r, edge, pad, in, out, rows, cols);
+    case 116: return launch_tiled_db_r<16, false>(L, w, r, edge, pad, in, out, rows, cols);
+    case 216: return launch_tiled_db_r<16, true>(L, w, r, edge, pad, in, out, rows, cols);
     case -16:
       switch (r) {
         case 1: return launch_shfl<1>(L, w, edge, pad, in, out, rows, cols);
