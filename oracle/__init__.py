@@ -21,7 +21,7 @@ _SRC = os.path.join(_HERE, "oracle.cpp")
 _LIBS = {False: os.path.join(_HERE, "liboracle.so"), True: os.path.join(_HERE, "liboracle_omp.so")}
 
 FN_ADD, FN_MULT, FN_MAX, FN_SAXPY = 0, 1, 2, 3
-EDGE_CONSTANT, EDGE_DUPLICATE = 0, 1
+EDGE_CONSTANT, EDGE_DUPLICATE, EDGE_CYCLIC = 0, 1, 2
 SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
 AXIS_ROW, AXIS_COL = 0, 1
 

@@ -17,7 +17,8 @@
 // two's-complement wrap-around (mod 2^32) arithmetic on uint32_t (reading (c).2 ii).
 //
 // Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): closed forms (sum i = n(n-1)/2, scan of
-// ones = indices, stencil of a constant = constant * sum w, constant-0 border closed form),
+// ones = indices, stencil of a constant = constant * sum w, constant-0 border closed form,
+// cyclic stencil == circular correlation computed with numpy roll / FFT-free definition),
 // impulse / one-hot-weight shift tests (orientation, indexing, edge policy, bit-exact), split and
 // permutation invariants, the separable identity (row pass . col pass == dense outer-product
 // filter), transpose symmetry, library special cases (numpy cumsum / correlate / math.fsum), and
@@ -35,7 +36,7 @@ namespace {
 
 // restated ABI values (see header comment): user functions, edge policies, scan modes, axes
 enum { FN_ADD = 0, FN_MULT = 1, FN_MAX = 2, FN_SAXPY = 3 };
-enum { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1 };
+enum { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1, EDGE_CYCLIC = 2 };
 enum { SCAN_INCLUSIVE = 0, SCAN_EXCLUSIVE = 1 };
 enum { AXIS_ROW = 0, AXIS_COL = 1 };
 
@@ -76,6 +77,9 @@ struct NSum {
 };
 
 inline ptrdiff_t clampi(ptrdiff_t j, ptrdiff_t lo, ptrdiff_t hi) { return j < lo ? lo : (j > hi ? hi : j); }
+// CYCLIC (reading 19): the index wraps around, x~[j] = x[j mod n] with the
+// mathematical (non-negative) remainder; in 2D each index wraps on its own.
+inline ptrdiff_t wrapi(ptrdiff_t j, ptrdiff_t n) { ptrdiff_t m = j % n; return m < 0 ? m + n : m; }
 
 // reading (c).5: x~[j] = x[j] inside; CONSTANT -> pad; DUPLICATE -> x[clamp(j,0,n-1)].
 // `stride` lets the same definition walk a matrix column.
@@ -83,6 +87,7 @@ template <typename T>
 inline double ext1(const T* x, ptrdiff_t n, ptrdiff_t stride, ptrdiff_t j, int edge, double pad) {
   if (j >= 0 && j < n) return static_cast<double>(x[j * stride]);
   if (edge == EDGE_CONSTANT) return pad;
+  if (edge == EDGE_CYCLIC) return static_cast<double>(x[wrapi(j, n) * stride]);
   return static_cast<double>(x[clampi(j, 0, n - 1) * stride]);
 }
 
@@ -122,6 +127,7 @@ inline double ext2(const T* X, ptrdiff_t rows, ptrdiff_t cols, ptrdiff_t p, ptrd
                    double pad) {
   if (p >= 0 && p < rows && q >= 0 && q < cols) return static_cast<double>(X[p * cols + q]);
   if (edge == EDGE_CONSTANT) return pad;
+  if (edge == EDGE_CYCLIC) return static_cast<double>(X[wrapi(p, rows) * cols + wrapi(q, cols)]);
   return static_cast<double>(X[clampi(p, 0, rows - 1) * cols + clampi(q, 0, cols - 1)]);
 }
 

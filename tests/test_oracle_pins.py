@@ -499,3 +499,54 @@ def test_openmp_build_matches_single_thread():
         assert np.array_equal(c, O.map_f32(O.FN_SAXPY, 2.5, x, x))
     finally:
         O.use_openmp(False)
+
+
+# ---- CYCLIC edge policy (reading 19) --------------------------------------
+@pytest.mark.parametrize("r", [0, 1, 4, 16])
+def test_overlap1d_cyclic_is_circular_correlation(r):
+    # pin: out = sum_k w[k+r] * roll(x, -k) (numpy roll is the textbook circular shift); the one-hot
+    # weight case is a pure rotation and must be bit-exact
+    n = 257
+    x = I.uniform01_f32(4200 + r, n)
+    w = I.signed_weights_f32(4300 + r, 2 * r + 1)
+    got, ab = O.mapoverlap_1d(w, r, O.EDGE_CYCLIC, 0.0, x)
+    ref = np.zeros(n)
+    for k in range(-r, r + 1):
+        ref += float(w[k + r]) * np.roll(x.astype(np.float64), -k)
+    assert np.allclose(got, ref, rtol=0, atol=1e-13)
+    for m in range(2 * r + 1):
+        e = np.zeros(2 * r + 1, np.float32)
+        e[m] = 1.0
+        got, _ = O.mapoverlap_1d(e, r, O.EDGE_CYCLIC, 0.0, x)
+        assert np.array_equal(got.astype(np.float32), np.roll(x, -(m - r)))
+
+
+def test_overlap1d_cyclic_short_vector_wraps_more_than_once():
+    # n < r: indices wrap several times (mathematical modulo, never negative)
+    x = np.array([1.0, 10.0, 100.0], np.float32)
+    r = 5
+    w = np.arange(1, 2 * r + 2, dtype=np.float32)
+    got, _ = O.mapoverlap_1d(w, r, O.EDGE_CYCLIC, 0.0, x)
+    for i in range(3):
+        brute = sum(float(w[k + r]) * float(x[(i + k) % 3]) for k in range(-r, r + 1))  # Python % is non-negative
+        assert got[i] == brute
+
+
+def test_overlap2d_cyclic_matches_rolls_and_constant_input():
+    rows, cols, ry, rx = 13, 17, 2, 3
+    X = I.uniform01_f32(4400, rows * cols).reshape(rows, cols)
+    W = I.signed_weights_f32(4401, (2 * ry + 1) * (2 * rx + 1)).reshape(2 * ry + 1, 2 * rx + 1)
+    got, _ = O.mapoverlap_2d(W.ravel(), ry, rx, O.EDGE_CYCLIC, 0.0, X)
+    ref = np.zeros((rows, cols))
+    for a in range(-ry, ry + 1):
+        for b in range(-rx, rx + 1):
+            ref += float(W[a + ry, b + rx]) * np.roll(X.astype(np.float64), (-a, -b), axis=(0, 1))
+    assert np.allclose(got, ref, rtol=0, atol=1e-13)
+    # a constant stays constant * sum(W) everywhere (no border at all)
+    got, _ = O.mapoverlap_2d(W.ravel(), ry, rx, O.EDGE_CYCLIC, 0.0, np.full((rows, cols), 2.0, np.float32))
+    assert np.allclose(got, 2.0 * W.astype(np.float64).sum(), rtol=0, atol=1e-13)
+    # column-wise 1D on a matrix == 2D with rx = 0
+    wc = I.signed_weights_f32(4402, 5)
+    a1, _ = O.mapoverlap_1d_matrix(wc, 2, O.EDGE_CYCLIC, 0.0, O.AXIS_COL, X)
+    a2, _ = O.mapoverlap_2d(wc, 2, 0, O.EDGE_CYCLIC, 0.0, X)
+    assert np.array_equal(a1, a2)
