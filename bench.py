@@ -171,7 +171,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -363,6 +363,12 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(local)
     sampler.start()
+    # untimed pre-roll of the same steps while nvidia-smi starts up (its first sample takes ~0.2 s), so that
+    # the clock / throttle samples are taken under the load of the timed region, not on an idle GPU
+    t_pre = time.perf_counter()
+    while time.perf_counter() - t_pre < 0.5:
+        wl.step()
+        torch.cuda.synchronize()
     ctx.reset_stats()
     barrier()
     e0.record()
