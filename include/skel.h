@@ -61,9 +61,10 @@ typedef enum { SKEL_F32 = 0, SKEL_I32 = 1 } skel_dtype;
  * nowhere else. */
 typedef enum { SKEL_FN_ADD = 0, SKEL_FN_MULT = 1, SKEL_FN_MAX = 2, SKEL_FN_SAXPY = 3, SKEL_FN_WSTENCIL = 4 } skel_fn;
 
-/* edge policy of MapOverlap: out-of-range neighbours read `pad` (CONSTANT) or the nearest
- * in-range element, each index clamped independently (DUPLICATE). */
-typedef enum { SKEL_EDGE_CONSTANT = 0, SKEL_EDGE_DUPLICATE = 1 } skel_edge;
+/* edge policy of MapOverlap: out-of-range neighbours read `pad` (CONSTANT), the nearest in-range
+ * element, each index clamped independently (DUPLICATE), or wrap around, each index taken modulo
+ * its extent with the non-negative remainder (CYCLIC; reading 19). */
+typedef enum { SKEL_EDGE_CONSTANT = 0, SKEL_EDGE_DUPLICATE = 1, SKEL_EDGE_CYCLIC = 2 } skel_edge;
 typedef enum { SKEL_SCAN_INCLUSIVE = 0, SKEL_SCAN_EXCLUSIVE = 1 } skel_scan_mode;
 typedef enum { SKEL_AXIS_ROW = 0, SKEL_AXIS_COL = 1 } skel_axis;
 typedef enum { SKEL_READ = 0, SKEL_WRITE = 1, SKEL_READWRITE = 2 } skel_access;

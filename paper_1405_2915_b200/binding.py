@@ -30,7 +30,7 @@ STATUS_NAMES = ["OK", "INVALID_ARG", "SIZE_MISMATCH", "DTYPE", "UNSUPPORTED", "E
                 "CUDA", "BUSY", "IO"]
 F32, I32 = 0, 1
 FN_ADD, FN_MULT, FN_MAX, FN_SAXPY, FN_WSTENCIL = 0, 1, 2, 3, 4
-EDGE_CONSTANT, EDGE_DUPLICATE = 0, 1
+EDGE_CONSTANT, EDGE_DUPLICATE, EDGE_CYCLIC = 0, 1, 2
 SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
 AXIS_ROW, AXIS_COL = 0, 1
 READ, WRITE, READWRITE = 0, 1, 2

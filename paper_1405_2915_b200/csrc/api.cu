@@ -578,7 +578,7 @@ skel_status overlap_check(skel_ctx* c, const Handle* in, const Handle* out, int 
   if (in->st->dtype != SKEL_F32 || out->st->dtype != SKEL_F32) return fail(c, SKEL_ERR_DTYPE, "MapOverlap is defined for f32 only");
   if (in->rows != out->rows || in->cols != out->cols) return fail(c, SKEL_ERR_SIZE_MISMATCH, "input and output shapes differ");
   if (in->st == out->st) return fail(c, SKEL_ERR_ALIAS, "MapOverlap output must not alias its input");
-  if (edge != SKEL_EDGE_CONSTANT && edge != SKEL_EDGE_DUPLICATE) return fail(c, SKEL_ERR_INVALID_ARG, "bad edge policy");
+  if (edge != SKEL_EDGE_CONSTANT && edge != SKEL_EDGE_DUPLICATE && edge != SKEL_EDGE_CYCLIC) return fail(c, SKEL_ERR_INVALID_ARG, "bad edge policy");
   return SKEL_OK;
 }
 

@@ -1,6 +1,6 @@
 // MapOverlap 1D skeleton on a vector or along the rows of a matrix (PAPER.md L83 names
 // "mapoverlap"; definition: DESIGN.md reading 5):
-//   out[i] = sum_{k=-r..r} w[k+r] * x~[i+k]      (correlation; edge policy constant(pad) | duplicate)
+//   out[i] = sum_{k=-r..r} w[k+r] * x~[i+k]      (correlation; edge policy constant(pad) | duplicate | cyclic)
 // Every row of a rows x cols matrix is an independent vector (a plain vector is rows = 1).
 //
 // Variants:
@@ -18,12 +18,16 @@
 namespace skel {
 namespace {
 
-enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1 };
+enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1, EDGE_CYCLIC = 2 };
 
 // x~ of one row (reading 5): c may be out of [0, cols)
 __device__ __forceinline__ float ext_row(const float* row, long long cols, long long c, int edge, float pad) {
   if (c >= 0 && c < cols) return __ldg(row + c);
   if (edge == EDGE_CONSTANT) return pad;
+  if (edge == EDGE_CYCLIC) {  // non-negative remainder: the index wraps around (possibly several times)
+    long long m = c % cols;
+    return __ldg(row + (m < 0 ? m + cols : m));
+  }
   return __ldg(row + (c < 0 ? 0 : cols - 1));
 }
 

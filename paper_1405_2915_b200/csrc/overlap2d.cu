@@ -1,6 +1,7 @@
 // MapOverlap 2D skeleton and the column-wise 1D form on a matrix (readings 5 and 6):
 //   out[i][j] = sum_{a=-ry..ry} sum_{b=-rx..rx} W[a+ry][b+rx] * X~[i+a][j+b]
-// X~ = pad (CONSTANT) or X[clamp i][clamp j] (DUPLICATE, every index clamped on its own).
+// X~ = pad (CONSTANT), X[clamp i][clamp j] (DUPLICATE, every index clamped on its own) or
+// X[i mod rows][j mod cols] (CYCLIC).
 // Column-wise 1D is the rx = 0 case (a (2r+1) x 1 filter).
 //
 // Variants:
@@ -18,14 +19,21 @@
 namespace skel {
 namespace {
 
-enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1 };
+enum : int { EDGE_CONSTANT = 0, EDGE_DUPLICATE = 1, EDGE_CYCLIC = 2 };
 
 __device__ __forceinline__ float ext2(const float* X, long long rows, long long cols, long long p, long long q,
                                       int edge, float pad) {
   if (p >= 0 && p < rows && q >= 0 && q < cols) return __ldg(X + p * cols + q);
   if (edge == EDGE_CONSTANT) return pad;
-  p = p < 0 ? 0 : (p >= rows ? rows - 1 : p);
-  q = q < 0 ? 0 : (q >= cols ? cols - 1 : q);
+  if (edge == EDGE_CYCLIC) {  // each index wraps on its own (non-negative remainder)
+    p %= rows;
+    q %= cols;
+    p = p < 0 ? p + rows : p;
+    q = q < 0 ? q + cols : q;
+  } else {
+    p = p < 0 ? 0 : (p >= rows ? rows - 1 : p);
+    q = q < 0 ? 0 : (q >= cols ? cols - 1 : q);
+  }
   return __ldg(X + p * cols + q);
 }
 

@@ -325,7 +325,7 @@ def test_scan_f32_three_kernel(ctx):
 
 
 # ------------------------------------------------------------------ MapOverlap 1D
-EDGE_CASES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICATE, 0.0)]
+EDGE_CASES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICATE, 0.0), (S.EDGE_CYCLIC, 0.0)]
 O1_SIZES = [1, 2, 3, 5, 16, 17, 33, 100, 1023, 4096, 4097, 8200, 16385, 65537, 300001]
 
 
@@ -526,3 +526,34 @@ def test_separable_pair_lock_step(ctx):
     assert_overlap(mo.numpy(), ref3, ab3)
     for c in (mx, mt, mo):
         c.destroy()
+
+
+# ------------------------------------------------------------------ CYCLIC edge policy
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
+def test_overlap1d_cyclic_one_hot_is_a_rotation_bit_exact(ctx, v):
+    r = 4
+    with forced(ctx, S.SK_OVERLAP1D, v):
+        for n in (3, 9, 4097, 100003):  # n < r: the index wraps more than once
+            x = I.uniform01_f32(7000 + n, n)
+            vx, vo = ctx.vector_from(x), ctx.vector(n)
+            for m in (0, 3, 4, 8):
+                w = np.zeros(2 * r + 1, np.float32)
+                w[m] = 1.0
+                ctx.mapoverlap_1d(w, r, S.EDGE_CYCLIC, 0.0, vx, vo)
+                assert np.array_equal(vo.numpy(), np.roll(x, -(m - r))), (n, m)
+            vx.destroy()
+            vo.destroy()
+
+
+@pytest.mark.parametrize("v", variants(S.SK_OVERLAP2D))
+def test_overlap2d_cyclic_constant_input_has_no_border(ctx, v):
+    rows, cols = 70, 260
+    W = I.positive_weights_f32(7100, 25)
+    with forced(ctx, S.SK_OVERLAP2D, v):
+        mx, mo = ctx.matrix_from(np.full((rows, cols), 0.5, np.float32)), ctx.matrix(rows, cols)
+        ctx.mapoverlap_2d(W, 2, 2, S.EDGE_CYCLIC, 0.0, mx, mo)
+        got = mo.numpy()
+        assert np.all(np.abs(got - 0.5 * W.astype(np.float64).sum()) <= 2e-6 * 0.5)
+        assert np.all(got == got[0, 0])  # every output saw the same 25 values in the same order
+        mx.destroy()
+        mo.destroy()
