@@ -1017,9 +1017,28 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   CU(c, cudaMalloc(&b0, nmax * 4));
   CU(c, cudaMalloc(&b1, nmax * 4));
   CU(c, cudaMalloc(&b2, nmax * 4));
-  CU(c, cudaMemsetAsync(b0, 0, nmax * 4, c->stream));
-  CU(c, cudaMemsetAsync(b1, 0, nmax * 4, c->stream));
-  CU(c, cudaMemsetAsync(b2, 0, nmax * 4, c->stream));
+  {
+    // Pseudo-random operands, not zeros: an all-zero stream draws less HBM power than real data, and a
+    // plan tuned on it picks variants that lose under the power cap of a sustained run. The bit
+    // patterns are floats in [1, 2) (as int32 they are large values that wrap in sums: harmless).
+    const size_t chunk = std::min<size_t>(nmax, size_t(1) << 22);
+    std::vector<uint32_t> host(chunk);
+    uint64_t z = 0x9E3779B97F4A7C15ull;
+    for (size_t i = 0; i < chunk; ++i) {
+      z ^= z << 13;
+      z ^= z >> 7;
+      z ^= z << 17;
+      host[i] = 0x3F800000u | static_cast<uint32_t>(z >> 41);
+    }
+    void* bufs[3] = {b0, b1, b2};
+    for (void* b : bufs) {
+      CU(c, cudaMemcpyAsync(b, host.data(), chunk * 4, cudaMemcpyHostToDevice, c->stream));
+      for (size_t done = chunk; done < nmax; done *= 2)  // double the filled prefix
+        CU(c, cudaMemcpyAsync(static_cast<char*>(b) + done * 4, b, std::min(done, nmax - done) * 4,
+                              cudaMemcpyDeviceToDevice, c->stream));
+    }
+    CU(c, cudaStreamSynchronize(c->stream));
+  }
   cudaEvent_t e0, e1;
   CU(c, cudaEventCreate(&e0));
   CU(c, cudaEventCreate(&e1));
@@ -1071,6 +1090,12 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
         best = v;
         best_t = med;
       }
+    }
+    // hysteresis: keep the previous size's winner unless it is more than 3 % slower than the best here
+    // (timing noise otherwise turns the plan into a list of spurious breakpoints)
+    if (best >= 0 && prev_best >= 0 && prev_best != best) {
+      const float tp = c->tune_table[size_t(lg - log2_lo) * nv + prev_best];
+      if (tp == tp && tp <= 1.03f * best_t) best = prev_best;
     }
     c->stats.launches += c->launches;
     c->launches = 0;

@@ -104,9 +104,6 @@ const RedVariant kRedVariants[] = {
     {"v4_u4_two_pass", 4, 4, false, 8},
     {"v8_u2_two_pass", 8, 2, false, 8},
     {"v4_u4_single_pass_4bps", 4, 4, true, 4},
-    {"v8_u4_single_pass", 8, 4, true, 8},
-    {"v8_u4_single_pass_4bps", 8, 4, true, 4},
-    {"v8_u2_single_pass_4bps", 8, 2, true, 4},
 };
 constexpr int kNumRedVariants = sizeof(kRedVariants) / sizeof(kRedVariants[0]);
 
@@ -139,7 +136,6 @@ cudaError_t launch_vu(const Launch& L, const Scratch& S, const RedVariant& rv, c
                       size_t n, T* result) {
   if (rv.v == 1) return launch_one<T, MAPF, HAS_IN1, OP, 1, 4>(L, S, rv, in0, in1, c, n, result);
   if (rv.v == 4) return launch_one<T, MAPF, HAS_IN1, OP, 4, 4>(L, S, rv, in0, in1, c, n, result);
-  if (rv.u == 4) return launch_one<T, MAPF, HAS_IN1, OP, 8, 4>(L, S, rv, in0, in1, c, n, result);
   return launch_one<T, MAPF, HAS_IN1, OP, 8, 2>(L, S, rv, in0, in1, c, n, result);
 }
 
