@@ -280,10 +280,20 @@ overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, 
     float acc[O];
 #pragma unroll
     for (int o = 0; o < O; ++o) acc[o] = 0.f;
+    // Taps k with k - R even address window pairs (win[o+k], win[o+k+1]), o even, that are aligned
+    // register pairs of the 256-bit loads: one FFMA2 per output pair (only worth it when the kernel
+    // is issue bound, r >= 8). Per output the taps still accumulate in ascending k: bit-identical.
+    constexpr bool PK = R >= 8;
 #pragma unroll
-    for (int k = 0; k <= 2 * R; ++k)
+    for (int k = 0; k <= 2 * R; ++k) {
+      if (PK && (k + R) % 2 == 0) {
 #pragma unroll
-      for (int o = 0; o < O; ++o) acc[o] = fmaf(W.w[k], win[o + k], acc[o]);
+        for (int o = 0; o < O; o += 2) fma2_into(acc[o], acc[o + 1], W.w[k], win[o + k], win[o + k + 1]);
+      } else {
+#pragma unroll
+        for (int o = 0; o < O; ++o) acc[o] = fmaf(W.w[k], win[o + k], acc[o]);
+      }
+    }
     if (c0 + O <= lc) {
       float* dst = out + row * cols + c0;
       uint32_t r0[8], r1[8];
