@@ -10,7 +10,11 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libskel.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["api.cu", "plan.cpp", "map.cu", "reduce.cu", "scan.cu", "overlap1d.cu", "overlap2d.cu"]
+# (source, object stem, extra defines); overlap2d_inst.cu is compiled once per radius (SKEL_INST),
+# the slowest ones first so that the parallel build ends early
+SOURCES = ([("overlap2d_inst.cu", f"overlap2d_inst{k}", [f"-DSKEL_INST={k}"]) for k in (3, 9, 8, 2, 1, 7, 6, 5, 0, 4)] +
+           [(f, os.path.splitext(f)[0], []) for f in
+            ("scan.cu", "overlap1d.cu", "api.cu", "overlap2d.cu", "reduce.cu", "map.cu", "plan.cpp")])
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
@@ -27,14 +31,15 @@ def _deps_mtime() -> float:
     return max(os.path.getmtime(f) for f in files)
 
 
-def _compile(src: str) -> str:
-    obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+def _compile(item) -> str:
+    src, stem, defines = item
+    obj = os.path.join(OBJ, stem + ".o")
     srcp = os.path.join(CSRC, src)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".hpp", ".cuh"))]
     headers.append(os.path.join(INCLUDE, "skel.h"))
     newest = max(os.path.getmtime(f) for f in [srcp, __file__] + headers)
     if not os.path.exists(obj) or os.path.getmtime(obj) < newest:
-        cmd = [_nvcc(), *NVCC_FLAGS, "-x", "cu", "-I", INCLUDE, "-c", srcp, "-o", obj]
+        cmd = [_nvcc(), *NVCC_FLAGS, *defines, "-x", "cu", "-I", INCLUDE, "-c", srcp, "-o", obj]
         subprocess.run(cmd, check=True)
     return obj
 
@@ -47,7 +52,7 @@ def build(force: bool = False) -> str:
             os.remove(os.path.join(OBJ, f))
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _deps_mtime():
         return LIB
-    with ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
+    with ThreadPoolExecutor(max_workers=min(os.cpu_count() or 4, len(SOURCES))) as ex:
         objs = list(ex.map(_compile, SOURCES))
     subprocess.run([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs], check=True)
     return LIB

@@ -71,4 +71,12 @@ bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out
 cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
                              const float* in, float* out, size_t rows, size_t cols);
 
+// tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
+template <int R>
+cudaError_t launch_overlap2d_tiled(const Launch& L, int v, const Weights2D& w, int edge, float pad, const float* in,
+                                   float* out, size_t rows, size_t cols);
+template <int R>
+cudaError_t launch_overlap1d_cols_tiled(const Launch& L, int v, const Weights1D& w, int edge, float pad,
+                                        const float* in, float* out, size_t rows, size_t cols);
+
 }  // namespace skel

@@ -200,34 +200,68 @@ overlap1d_tiled_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
 }
 
 // Double-buffered persistent form ("_db"): while a block computes tile i from one buffer, the
-// cp.async copies of tile i+1 fill the other.
+// cp.async copies of tile i+1 fill the other. The (row, tile-in-row) coordinates advance by
+// (G div tiles_per_row, G mod tiles_per_row) with one carry (no division per tile), and a tile whose
+// halo lies inside its row is staged by a fast path: the addresses of a thread's 128-bit groups
+// differ by compile-time constants, so a group costs one cp.async.
 template <int R, int O, bool PK>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tiled_db_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
-                          size_t rows, size_t cols, unsigned buf_floats) {
+                          size_t rows, size_t cols, unsigned buf_floats, unsigned tiles_per_row, unsigned dq, unsigned dr) {
   constexpr int TILE = T1_THREADS * O;
+  constexpr int HP = (R + 3) / 4 * 4;
+  constexpr int SPAN = TILE + 2 * HP;
+  static_assert(O == 4 || 1024 % O == 0, "the padded layout must be linear in the group index");
   extern __shared__ __align__(16) float sm[];
-  const size_t tiles_per_row = (cols + TILE - 1) / TILE;
   const size_t ntiles = rows * tiles_per_row;
   size_t tile = blockIdx.x;
   if (tile >= ntiles) return;
-  auto stage = [&](size_t t, int b) {
-    const size_t row = t / tiles_per_row;
-    const long long c0 = static_cast<long long>((t - row * tiles_per_row) * TILE);
-    stage_tile1<R, O, true>(sm + size_t(b) * buf_floats, in + row * cols, (long long)cols, c0, edge, pad);
+  size_t row = tile / tiles_per_row;                                  // the only division
+  unsigned tcol = static_cast<unsigned>(tile - row * tiles_per_row);  // tile index inside the row
+  auto advance = [&](size_t& t, size_t& r, unsigned& c) {
+    t += gridDim.x;
+    r += dq;
+    c += dr;
+    if (c >= tiles_per_row) {
+      c -= tiles_per_row;
+      ++r;
+    }
   };
-  stage(tile, 0);
+  const unsigned soff0 = static_cast<unsigned>(phys<O>(4 * threadIdx.x)) * 4u;  // byte offset of group t in a buffer
+  constexpr unsigned SSTEP = (O == 4 ? 1024u : 1024u + 4096u / O) * 4u;          // ... of group t + 256
+  auto stage = [&](size_t r, unsigned c, int b) {
+    const long long c0 = static_cast<long long>(c) * TILE;
+    const float* xrow = in + r * cols;
+    float* dst = sm + size_t(b) * buf_floats;
+    if (c0 - HP >= 0 && c0 + TILE + HP <= static_cast<long long>(cols)) {
+      const float* g = xrow + c0 - HP + 4 * threadIdx.x;
+      const uint32_t d = smem_u32(dst) + soff0;
+#pragma unroll
+      for (int k = 0; k < SPAN / 4 / T1_THREADS; ++k)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + k * SSTEP), "l"(g + k * 1024) : "memory");
+      constexpr int KL = SPAN / 4 / T1_THREADS;  // the last, partial round of groups
+      if (static_cast<int>(threadIdx.x) < SPAN / 4 - KL * T1_THREADS)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + KL * SSTEP), "l"(g + KL * 1024) : "memory");
+    } else {
+      stage_tile1<R, O, true>(dst, xrow, (long long)cols, c0, edge, pad);
+    }
+  };
+  stage(row, tcol, 0);
   asm volatile("cp.async.commit_group;" ::: "memory");
+  size_t ntile = tile, nrow = row;
+  unsigned ntcol = tcol;
+  advance(ntile, nrow, ntcol);
   int buf = 0;
-  for (; tile < ntiles; tile += gridDim.x, buf ^= 1) {
-    if (tile + gridDim.x < ntiles) stage(tile + gridDim.x, buf ^ 1);
+  for (; tile < ntiles; buf ^= 1) {
+    if (ntile < ntiles) stage(nrow, ntcol, buf ^ 1);
     asm volatile("cp.async.commit_group;" ::: "memory");
     asm volatile("cp.async.wait_group 1;" ::: "memory");
     __syncthreads();
-    const size_t row = tile / tiles_per_row;
-    const long long c0 = static_cast<long long>((tile - row * tiles_per_row) * TILE);
-    compute_tile1<R, O, PK>(sm + size_t(buf) * buf_floats, W, out + row * cols, (long long)cols, c0);
+    compute_tile1<R, O, PK>(sm + size_t(buf) * buf_floats, W, out + row * cols, (long long)cols,
+                            static_cast<long long>(tcol) * TILE);
     __syncthreads();
+    tile = ntile; row = nrow; tcol = ntcol;
+    advance(ntile, nrow, ntcol);
   }
 }
 
@@ -366,7 +400,10 @@ cudaError_t launch_tiled_db(const Launch& L, const Weights1D& w, int edge, float
   const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
-  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols, (unsigned)(one / 4));
+  const size_t tpr = (cols + TILE - 1) / TILE;
+  if (tpr >= (size_t(1) << 31)) return cudaErrorInvalidValue;
+  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, edge, pad, in, out, rows, cols, (unsigned)(one / 4), (unsigned)tpr,
+                                                        (unsigned)(grid / tpr), (unsigned)(grid % tpr));
   ++*L.launches;
   return cudaGetLastError();
 }
