@@ -265,6 +265,15 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
 
     run(3)  # warm-up (allocations, first-use kernel loads)
     wall_l, dev_l, st_l, s_l = run(iters)
+    # the same loop with cross-call fusion on (skel_ctx_set_fusion): Map -> MapOverlap1D -> Reduce is ONE
+    # kernel, 12 instead of 20 bytes per element (every reduce() ends with a scalar read-back, which also
+    # flushes: the events above see every launch)
+    ctx.set_fusion(True)
+    try:
+        run(3)
+        wall_f, dev_f, st_f, s_f = run(iters)
+    finally:
+        ctx.set_fusion(False)
     ctx.set_coherence(S.EAGER)
     try:
         wall_e, _, st_e, _ = run(eager_iters)
@@ -278,6 +287,11 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
                  "h2d_bytes_total": st_l["h2d_bytes"], "d2h_bytes_total": st_l["d2h_bytes"],
                  "h2d_count": st_l["h2d_count"], "d2h_count": st_l["d2h_count"],
                  "scalar_readbacks": st_l["scalar_d2h_count"], "h2d_elided": st_l["h2d_elided"]},
+        "fused": {"wall_ms_per_iter": round(wall_f / iters * 1e3, 4), "device_ms_per_iter": round(dev_f / iters, 4),
+                  "bytes_per_elem": 12, "GB/s_device_at_12B": round(12 * n / (dev_f / iters * 1e-3) / 1e9, 1),
+                  "launches_per_iter": st_f["launches"] / iters, "fused_launches": st_f["fused_launches"],
+                  "h2d_count": st_f["h2d_count"], "d2h_count": st_f["d2h_count"],
+                  "speedup_over_unfused_device": round(dev_l / dev_f, 3), "last_scalar": s_f},
         "eager": {"iterations_run": eager_iters, "wall_ms_per_iter": round(wall_e / eager_iters * 1e3, 3),
                   "h2d_bytes_per_iter": st_e["h2d_bytes"] // eager_iters, "d2h_bytes_per_iter": st_e["d2h_bytes"] // eager_iters,
                   "transfers_per_iter": (st_e["h2d_count"] + st_e["d2h_count"]) // eager_iters},

@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define SKEL_ABI_VERSION 1
+#define SKEL_ABI_VERSION 2
 
 /* ---- enums (values are ABI) ------------------------------------------------------------- */
 typedef enum {
@@ -99,6 +99,27 @@ skel_status skel_ctx_create(void* cuda_stream, skel_alloc_fn alloc, skel_free_fn
 skel_status skel_ctx_destroy(skel_ctx* ctx);
 skel_status skel_ctx_sync(skel_ctx* ctx);
 skel_status skel_ctx_set_coherence(skel_ctx* ctx, skel_coherence mode);
+/* Cross-call fusion (the GPU-only analogue of PAPER.md L137/L149: compose over a
+ * chain of dependent calls instead of call by call). Off by default. When enabled, the kernel launch
+ * of a call that can be part of the chain
+ *     skel_map(f in {ADD, MULT, MAX}, constant c, in1 = NULL, f32)  ->  skel_mapoverlap_1d (r in
+ *     {1,2,3,4,8,16}) on the Map's output  ->  skel_reduce / skel_reduce_to (ADD or MAX) on the
+ *     MapOverlap's output
+ * is held back (argument checks, coherence bookkeeping and transfers still happen inside the call).
+ * When the Reduce arrives the chain runs as ONE kernel that reads the input once (12 B/elem instead
+ * of 20); a Map -> MapOverlap1D or MapOverlap1D -> Reduce pair fuses the same way. Anything else
+ * (another call, a host access, a transfer, skel_ctx_sync, skel_ctx_flush, a destroy, a forced
+ * variant) first launches what is held back, call by call, so results never depend on the setting
+ * beyond the rounding differences between kernel variants (same tolerances). Consequences while
+ * fusion is on: (1) a launch error of a held-back call is reported by the call that flushes it;
+ * (2) callers that enqueue their own work on the context's stream (events, kernels) must call
+ * skel_ctx_flush first; (3) a fused IN-PLACE Map writes into a library buffer that is then swapped
+ * with the container's device buffer: a pointer obtained from skel_vector_device_ptr is valid only
+ * until the next skeleton call that writes the container (adopted buffers are never swapped; such a
+ * chain runs call by call); (4) skel_last_variant reports variant -2 for a fused launch. */
+skel_status skel_ctx_set_fusion(skel_ctx* ctx, int enable);
+/* Launch everything that fusion holds back (no synchronisation). */
+skel_status skel_ctx_flush(skel_ctx* ctx);
 const char* skel_last_error(skel_ctx* ctx);
 int skel_abi_version(void);
 
@@ -226,6 +247,8 @@ typedef struct {
   uint64_t d2h_elided;               /* outputs left on the device (EAGER would download them) */
   uint64_t scalar_d2h_count;         /* Reduce / MapReduce scalars returned to the host */
   uint64_t launches;                 /* kernels launched by the library */
+  uint64_t fused_launches;           /* fused-chain kernels (skel_ctx_set_fusion) */
+  uint64_t fused_calls;              /* skeleton calls that ran inside a fused-chain kernel */
 } skel_stats;
 skel_status skel_get_stats(skel_ctx* ctx, skel_stats* out);
 skel_status skel_reset_stats(skel_ctx* ctx);

@@ -47,7 +47,8 @@ class SkelInstance(C.Structure):
 
 class SkelStats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("h2d_bytes", "h2d_count", "d2h_bytes", "d2h_count", "h2d_elided",
-                                           "d2h_elided", "scalar_d2h_count", "launches")]
+                                           "d2h_elided", "scalar_d2h_count", "launches", "fused_launches",
+                                           "fused_calls")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -64,6 +65,8 @@ _SIGS = {
     "skel_ctx_destroy": ([_vp], _i),
     "skel_ctx_sync": ([_vp], _i),
     "skel_ctx_set_coherence": ([_vp, _i], _i),
+    "skel_ctx_set_fusion": ([_vp, _i], _i),
+    "skel_ctx_flush": ([_vp], _i),
     "skel_last_error": ([_vp], C.c_char_p),
     "skel_vector_create": ([_vp, _i, _sz, _pp], _i),
     "skel_vector_create_from": ([_vp, _i, _sz, _vp, _pp], _i),
@@ -178,6 +181,12 @@ class Context:
 
     def set_coherence(self, mode: int):
         self.check(lib.skel_ctx_set_coherence(self.h, mode))
+
+    def set_fusion(self, enable: bool):
+        self.check(lib.skel_ctx_set_fusion(self.h, 1 if enable else 0))
+
+    def flush(self):
+        self.check(lib.skel_ctx_flush(self.h))
 
     def stats(self) -> dict:
         s = SkelStats()

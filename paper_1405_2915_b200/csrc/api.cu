@@ -46,6 +46,7 @@ struct Handle {
 
 }  // namespace
 
+struct PendingCall;
 struct skel_vector : Handle {};
 struct skel_matrix : Handle {};
 
@@ -71,6 +72,11 @@ struct skel_ctx {
   int last_sk = -1, last_var = -1;
   int launches = 0;
   std::vector<float> tune_table;
+  // cross-call fusion (skel_ctx_set_fusion): launches of a fusible chain are held back here
+  bool fusion = false;
+  std::vector<struct PendingCall> pending;
+  void* spare = nullptr;  // buffer an in-place Map of a fused chain writes into (then swapped with the container's)
+  size_t spare_bytes = 0;
 };
 
 namespace {
@@ -211,10 +217,13 @@ skel_status make_handle(skel_ctx* c, uint32_t magic, int dt, size_t rows, size_t
   return SKEL_OK;
 }
 
+skel_status flush_pending(skel_ctx* c);
+
 skel_status release_handle(Handle* h) {
   Storage* s = h->st;
   skel_ctx* c = s->ctx;
   if (s->host_held && s->refs == 1) return fail(c, SKEL_ERR_BUSY, "host access is still held");
+  flush_pending(c);  // a held-back launch may still reference this container
   if (--s->refs == 0) {
     if (s->last_seq > c->synced_seq && !c->sticky) {
       cudaStreamSynchronize(c->stream);
@@ -254,7 +263,8 @@ skel_status host_acquire(Handle* h, skel_access mode, void** host_ptr) {
   if (s->host_held) return fail(c, SKEL_ERR_BUSY, "host access already held");
   const CoherenceStep step = coherence_step(s->state, ACTOR_HOST, mode, c->mode);
   if (!step.ok) return fail(c, SKEL_ERR_UNINIT, "host read of a container that was never written");
-  skel_status st = SKEL_OK;
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
   if (s->n > 0) {
     st = ensure_device(c);
     if (st != SKEL_OK) return st;
@@ -320,6 +330,8 @@ skel_status acquire_all(skel_ctx* c, OperandSet& set) {
       if (st != SKEL_OK) return st;
     }
     if ((o.step.transfer & XFER_H2D) && s->n > 0) {
+      st = flush_pending(c);  // keep the stream order: held-back launches go first
+      if (st != SKEL_OK) return st;
       CU(c, cudaMemcpyAsync(s->dev, s->host, s->n * esize(s->dtype), cudaMemcpyHostToDevice, c->stream));
       c->stats.h2d_bytes += s->n * esize(s->dtype);
       c->stats.h2d_count += 1;
@@ -337,7 +349,9 @@ skel_status publish_all(skel_ctx* c, OperandSet& set) {
     Storage* s = o.st;
     if (o.step.transfer & XFER_D2H) {  // EAGER: download the output right after the kernel
       if (s->n > 0) {
-        skel_status st = ensure_host(c, s);
+        skel_status st = flush_pending(c);
+        if (st != SKEL_OK) return st;
+        st = ensure_host(c, s);
         if (st != SKEL_OK) return st;
         CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->stream));
         c->stats.d2h_bytes += s->n * esize(s->dtype);
@@ -365,7 +379,12 @@ struct Call {
   float pad = 0.f;
   Weights1D w1;
   Weights2D w2;
+  Storage* in_st = nullptr;   // containers behind in0 / out (fusion: buffer swap of an in-place Map)
+  Storage* out_st = nullptr;
 };
+}  // namespace
+struct PendingCall { Call k; };
+namespace {
 
 InstanceKey key_of(const skel_instance& i) {
   InstanceKey k;
@@ -486,7 +505,7 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
 }
 
 // choose + launch + bookkeeping
-skel_status run_call(skel_ctx* c, const Call& k) {
+skel_status launch_now(skel_ctx* c, const Call& k) {
   int v = -1;
   skel_status st = choose_variant(c, k, &v);
   if (st != SKEL_OK) return st;
@@ -499,6 +518,113 @@ skel_status run_call(skel_ctx* c, const Call& k) {
   c->last_sk = k.inst.skeleton;
   c->last_var = v;
   return SKEL_OK;
+}
+
+// ---- cross-call fusion ----------------------------------------------------------
+// With fusion enabled, the LAUNCH of a call that can be part of the chain
+//   Map(f in {ADD, MULT, MAX}, constant c, f32 vector) -> MapOverlap1D(vector) -> Reduce(ADD | MAX)
+// is held back (coherence bookkeeping and transfers happen at call time as always; every launch is
+// on one in-order stream, so delaying a launch behind nothing but bookkeeping changes no result).
+// The chain is launched as ONE kernel (fused.cu) when its Reduce arrives, or call by call when
+// anything else happens first: every entry point that touches the stream flushes.
+int chain_kind(const skel_ctx* c, const Call& k) {
+  const skel_instance& i = k.inst;
+  if (i.skeleton < 0 || i.skeleton >= SKEL_SK_COUNT || c->forced[i.skeleton] >= 0 || k.n == 0) return 0;
+  if (i.skeleton == SKEL_SK_MAP && i.dtype == SKEL_F32 && i.mode == 0 &&
+      (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MULT || i.fn == SKEL_FN_MAX))
+    return 1;
+  if (i.skeleton == SKEL_SK_OVERLAP1D && k.rows == 1 &&
+      (i.r0 == 1 || i.r0 == 2 || i.r0 == 3 || i.r0 == 4 || i.r0 == 8 || i.r0 == 16))
+    return 2;
+  if (i.skeleton == SKEL_SK_REDUCE && i.dtype == SKEL_F32 && (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MAX)) return 3;
+  return 0;
+}
+
+skel_status flush_pending(skel_ctx* c) {
+  if (c->pending.empty()) return SKEL_OK;
+  std::vector<PendingCall> q;
+  q.swap(c->pending);
+  const Call* map = nullptr;
+  const Call* ov = nullptr;
+  const Call* red = nullptr;
+  for (const PendingCall& p : q) {
+    const int kind = chain_kind(c, p.k);
+    if (kind == 1) map = &p.k;
+    if (kind == 2) ov = &p.k;
+    if (kind == 3) red = &p.k;
+  }
+  skel_status st = SKEL_OK;
+  if (ov && (map || red)) {
+    const float* in = static_cast<const float*>(map ? map->in0 : ov->in0);
+    float* map_out = map ? static_cast<float*>(map->out) : nullptr;
+    bool swap = false;
+    if (map && map->out == map->in0) {  // in place: A' goes to the spare buffer, which then becomes A's
+      Storage* a = map->out_st;
+      const size_t bytes = a->n * esize(a->dtype);
+      if (a->dev_owned) {
+        if (c->spare && c->spare_bytes != bytes) {
+          dev_free(c, c->spare);
+          c->spare = nullptr;
+        }
+        if (!c->spare && dev_alloc(c, bytes, &c->spare) == SKEL_OK) c->spare_bytes = bytes;
+        if (c->spare) {
+          map_out = static_cast<float*>(c->spare);
+          swap = true;
+        }
+      }
+    }
+    const int map_fn = map ? map->inst.fn : FN_IDENT_;
+    const int red_op = red ? red->inst.fn : FUSED_NO_REDUCE;
+    if (fused_chain_ok(map_fn, ov->inst.r0, red_op, in, map_out, ov->out, ov->n)) {
+      Launch L{c->stream, c->sms, &c->launches};
+      cudaError_t e = launch_fused_chain(L, c->scratch, map_fn, map ? map->cbits : 0u, ov->w1, ov->inst.r0, ov->inst.edge,
+                                         ov->pad, red_op, in, map_out, static_cast<float*>(ov->out), ov->n,
+                                         red ? static_cast<float*>(red->out) : nullptr);
+      if (e != cudaSuccess) return cuda_fail(c, e, "fused chain launch");
+      if (swap) {
+        Storage* a = map->out_st;
+        void* old = a->dev;
+        a->dev = c->spare;
+        c->spare = old;
+      }
+      c->last_sk = ov->inst.skeleton;
+      c->last_var = -2;  // "fused"
+      c->stats.fused_launches += 1;
+      c->stats.fused_calls += q.size();
+      c->stats.launches += c->launches;
+      c->launches = 0;
+      return SKEL_OK;
+    }
+  }
+  for (const PendingCall& p : q) {
+    st = launch_now(c, p.k);
+    if (st != SKEL_OK) return st;
+  }
+  c->stats.launches += c->launches;
+  c->launches = 0;
+  return SKEL_OK;
+}
+
+skel_status run_call(skel_ctx* c, const Call& k) {
+  if (!c->fusion) return launch_now(c, k);
+  const int kind = chain_kind(c, k);
+  bool extends = false;
+  if (!c->pending.empty()) {
+    const Call& last = c->pending.back().k;
+    const int lk = chain_kind(c, last);
+    extends = (lk == 1 && kind == 2 && k.in0 == last.out && k.n == last.n) ||
+              (lk == 2 && kind == 3 && k.in0 == last.out && k.n == last.n);
+  }
+  if (!extends) {
+    skel_status st = flush_pending(c);
+    if (st != SKEL_OK) return st;
+  }
+  if (kind == 1 || kind == 2 || (kind == 3 && extends)) {
+    c->pending.push_back(PendingCall{k});
+    if (kind == 3) return flush_pending(c);  // the chain is complete
+    return SKEL_OK;
+  }
+  return launch_now(c, k);
 }
 
 bool red_op_ok(int op) { return op == SKEL_FN_ADD || op == SKEL_FN_MULT || op == SKEL_FN_MAX; }
@@ -519,6 +645,8 @@ skel_status const_bits(skel_ctx* c, int dtype, double v, uint32_t* bits) {
 }
 
 skel_status scalar_to_host(skel_ctx* c, int dtype, void* host_result) {
+  skel_status fst = flush_pending(c);
+  if (fst != SKEL_OK) return fst;
   CU(c, cudaMemcpyAsync(c->h_result, c->d_result, esize(dtype), cudaMemcpyDeviceToHost, c->stream));
   CU(c, cudaStreamSynchronize(c->stream));
   c->synced_seq = c->seq;
@@ -566,6 +694,7 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   k.in1 = b ? b->dev : nullptr;
   k.n = a->n;
   k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->d_result;
+  k.in_st = a;
   st = run_call(c, k);
   if (st != SKEL_OK) return st;
   st = publish_all(c, set);
@@ -591,6 +720,8 @@ skel_status overlap_run(skel_ctx* c, Call& k, const Handle* in, Handle* out) {
   k.in0 = in->st->dev;
   k.out = out->st->dev;
   k.n = in->st->n;
+  k.in_st = in->st;
+  k.out_st = out->st;
   st = run_call(c, k);
   if (st != SKEL_OK) return st;
   return publish_all(c, set);
@@ -627,7 +758,9 @@ skel_status skel_ctx_destroy(skel_ctx* c) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
   if (c->live > 0) return fail(c, SKEL_ERR_BUSY, "containers of this context are still alive");
   if (c->dev_ready) {
+    flush_pending(c);
     cudaStreamSynchronize(c->stream);
+    if (c->spare) dev_free(c, c->spare);
     cudaFree(c->scratch.partials);
     if (c->scratch.scan_state) cudaFree(c->scratch.scan_state);
     cudaFreeHost(c->h_result);
@@ -641,14 +774,30 @@ skel_status skel_ctx_sync(skel_ctx* c) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
   if (c->sticky) return SKEL_ERR_CUDA;
   if (!c->dev_ready) return SKEL_OK;
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
   CU(c, cudaStreamSynchronize(c->stream));
   c->synced_seq = c->seq;
   return SKEL_OK;
 }
 
+skel_status skel_ctx_set_fusion(skel_ctx* c, int enable) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  skel_status st = flush_pending(c);
+  c->fusion = enable != 0;
+  return st;
+}
+
+skel_status skel_ctx_flush(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  return flush_pending(c);
+}
+
 skel_status skel_ctx_set_coherence(skel_ctx* c, skel_coherence mode) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
   if (mode != SKEL_LAZY && mode != SKEL_EAGER) return fail(c, SKEL_ERR_INVALID_ARG, "bad coherence mode");
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
   c->mode = mode;
   return SKEL_OK;
 }
@@ -707,6 +856,7 @@ skel_status skel_vector_host_release(skel_vector* v) {
 
 skel_status skel_vector_device_ptr(const skel_vector* v, void** dptr, int* valid) {
   if (!vec_ok(v) || !dptr) return SKEL_ERR_INVALID_ARG;
+  flush_pending(v->st->ctx);  // the caller is about to use the stream / the pointer (a fused in-place Map swaps buffers)
   *dptr = v->st->dev;
   if (valid) *valid = (v->st->state & 2) ? 1 : 0;
   return SKEL_OK;
@@ -811,6 +961,8 @@ skel_status skel_map(skel_ctx* c, skel_fn f, double cval, const skel_vector* in0
   k.in1 = b ? b->dev : nullptr;
   k.out = o->dev;
   k.n = a->n;
+  k.in_st = a;
+  k.out_st = o;
   if (k.n > 0) {
     st = run_call(c, k);
     if (st != SKEL_OK) return st;
@@ -1009,6 +1161,8 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || (sk == SKEL_SK_OVERLAP1D && cols > 0);
   if (matrix && cols == 0) return fail(c, SKEL_ERR_INVALID_ARG, "matrix skeletons need cols");
   skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
   if (st != SKEL_OK) return st;
   const size_t nmax = size_t(1) << log2_hi;
   st = ensure_scan_state(c, nmax);

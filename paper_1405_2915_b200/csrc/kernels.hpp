@@ -71,6 +71,14 @@ bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out
 cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
                              const float* in, float* out, size_t rows, size_t cols);
 
+// ---- fused chain [Map(f, c)] -> MapOverlap1D -> [Reduce(op)] on one f32 vector (fused.cu) -----------
+// map_fn = FN_IDENT (100): no Map in the chain (map_out unused); red_op = FUSED_NO_REDUCE: no Reduce.
+constexpr int FUSED_NO_REDUCE = -1;
+bool fused_chain_ok(int map_fn, int r, int red_op, const void* in, const void* map_out, const void* ov_out, size_t n);
+cudaError_t launch_fused_chain(const Launch& L, const Scratch& S, int map_fn, uint32_t cbits, const Weights1D& w, int r,
+                               int edge, float pad, int red_op, const float* in, float* map_out, float* ov_out, size_t n,
+                               float* result /* device, one element; unused without a Reduce */);
+
 // tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
 template <int R>
 cudaError_t launch_overlap2d_tiled(const Launch& L, int v, const Weights2D& w, int edge, float pad, const float* in,

@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(S.lib, n), f"libskel.so does not export {n}"
     # the binding declares exactly the header's functions
     assert sorted(S.EXPORTS) == names
-    assert S.skel_abi_version() == 1
+    assert S.skel_abi_version() == 2
 
 
 def test_variant_tables():
