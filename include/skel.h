@@ -79,7 +79,8 @@ typedef enum {
   SKEL_SK_OVERLAP1D = 4,      /* vector, and row-wise on a matrix */
   SKEL_SK_OVERLAP1D_COL = 5,  /* column-wise on a matrix */
   SKEL_SK_OVERLAP2D = 6,
-  SKEL_SK_COUNT = 7
+  SKEL_SK_SEPARABLE = 7,      /* skel_mapoverlap_separable (variant 0 = the two 1D passes) */
+  SKEL_SK_COUNT = 8
 } skel_skeleton;
 
 typedef struct skel_ctx skel_ctx;
@@ -196,6 +197,16 @@ skel_status skel_mapoverlap_1d_matrix(skel_ctx* ctx, const float* w, int r, skel
  * W: HOST pointer, (2ry+1)*(2rx+1) floats row-major. 0 <= ry, rx <= SKEL_MAX_RADIUS_2D. */
 skel_status skel_mapoverlap_2d(skel_ctx* ctx, const float* W, int ry, int rx, skel_edge edge, double pad,
                                const skel_matrix* in, skel_matrix* out);
+/* Separable MapOverlap (BASELINE.json configs[3] "separable row-then-column 1D
+ * passes"): out = colpass(w_col, r_col, T), T = RN_f32(rowpass(w_row, r_row, in)), each pass with the
+ * edge policy, i.e. by definition the result of skel_mapoverlap_1d_matrix(ROW) into a temporary
+ * matrix followed by skel_mapoverlap_1d_matrix(COL). When r_row == r_col is one of {1,2,3,4,8} the
+ * two passes run as ONE kernel that keeps T in shared memory (8 instead of 16 bytes per element of
+ * HBM traffic); otherwise (variant 0, "two_pass") the library runs the two 1D kernels through a
+ * temporary device matrix of its own. w_row, w_col: HOST pointers (2r+1 floats each).
+ * out must not alias in. */
+skel_status skel_mapoverlap_separable(skel_ctx* ctx, const float* w_row, int r_row, const float* w_col, int r_col,
+                                      skel_edge edge, double pad, const skel_matrix* in, skel_matrix* out);
 
 /* Scan: inclusive out[i] = x[0] (+)...(+) x[i]; exclusive out[0] = init, out[i] = init (+) x[0]
  * (+)...(+) x[i-1]. (+) in {ADD, MULT, MAX}. `init` is ignored for inclusive. out may alias in. */

@@ -35,7 +35,7 @@ SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
 AXIS_ROW, AXIS_COL = 0, 1
 READ, WRITE, READWRITE = 0, 1, 2
 LAZY, EAGER = 0, 1
-SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_COUNT = range(8)
+SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_SEPARABLE, SK_COUNT = range(9)
 ST_UNINIT, ST_HOST, ST_DEVICE, ST_SHARED = 0, 1, 2, 3
 
 _NP = {F32: np.float32, I32: np.int32}
@@ -93,6 +93,7 @@ _SIGS = {
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
+    "skel_mapoverlap_separable": ([_vp, _vp, _i, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_scan": ([_vp, _i, _i, _d, _vp, _vp], _i),
     "skel_variant_count": ([_i], _i),
     "skel_variant_name": ([_i, _i], C.c_char_p),
@@ -287,6 +288,12 @@ class Context:
         W = np.ascontiguousarray(W, np.float32)
         assert W.size == (2 * ry + 1) * (2 * rx + 1)
         self.check(lib.skel_mapoverlap_2d(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
+
+    def mapoverlap_separable(self, w_row, r_row: int, w_col, r_col: int, edge: int, pad: float, x: "Matrix", out: "Matrix"):
+        wr, wc = np.ascontiguousarray(w_row, np.float32), np.ascontiguousarray(w_col, np.float32)
+        assert wr.size == 2 * r_row + 1 and wc.size == 2 * r_col + 1
+        self.check(lib.skel_mapoverlap_separable(self.h, wr.ctypes.data_as(C.c_void_p), r_row, wc.ctypes.data_as(C.c_void_p),
+                                                 r_col, edge, pad, x.h, out.h))
 
     def scan(self, op: int, mode: int, init: float, x: "Vector", out: "Vector"):
         self.check(lib.skel_scan(self.h, op, mode, init, x.h, out.h))

@@ -75,6 +75,8 @@ struct skel_ctx {
   // cross-call fusion (skel_ctx_set_fusion): launches of a fusible chain are held back here
   bool fusion = false;
   std::vector<struct PendingCall> pending;
+  void* sep_tmp = nullptr;  // intermediate matrix of the two-pass separable MapOverlap
+  size_t sep_tmp_bytes = 0;
   void* spare = nullptr;  // buffer an in-place Map of a fused chain writes into (then swapped with the container's)
   size_t spare_bytes = 0;
 };
@@ -379,6 +381,7 @@ struct Call {
   float pad = 0.f;
   Weights1D w1;
   Weights2D w2;
+  Weights1D w1b;  // separable: the column filter (w1 = the row filter, r0 / r1 = their radii)
   Storage* in_st = nullptr;   // containers behind in0 / out (fusion: buffer swap of an in-place Map)
   Storage* out_st = nullptr;
 };
@@ -401,6 +404,7 @@ int variant_count(int sk) {
     case SKEL_SK_OVERLAP1D: return overlap1d_variant_count();
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_count();
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_count();
+    case SKEL_SK_SEPARABLE: return separable_variant_count();
   }
   return 0;
 }
@@ -414,6 +418,7 @@ const char* variant_name(int sk, int v) {
     case SKEL_SK_OVERLAP1D: return overlap1d_variant_name(v);
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_name(v);
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_name(v);
+    case SKEL_SK_SEPARABLE: return separable_variant_name(v);
   }
   return nullptr;
 }
@@ -427,6 +432,7 @@ bool variant_ok(const Call& k, int v) {
     case SKEL_SK_OVERLAP1D: return overlap1d_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_SEPARABLE: return separable_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
   }
   return false;
 }
@@ -440,6 +446,7 @@ const int* preference(int sk, int dtype, int* count) {
   static const int o1_p[] = {2, 1, 0};
   static const int col_p[] = {2, 0};
   static const int o2_p[] = {1, 0};
+  static const int sep_p[] = {4, 1, 0};
   switch (sk) {
     case SKEL_SK_MAP: *count = 3; return map_p;
     case SKEL_SK_REDUCE:
@@ -450,6 +457,7 @@ const int* preference(int sk, int dtype, int* count) {
     case SKEL_SK_OVERLAP1D: *count = 3; return o1_p;
     case SKEL_SK_OVERLAP1D_COL: *count = 2; return col_p;
     case SKEL_SK_OVERLAP2D: *count = 2; return o2_p;
+    case SKEL_SK_SEPARABLE: *count = 3; return sep_p;
   }
   *count = 0;
   return nullptr;
@@ -479,10 +487,44 @@ skel_status choose_variant(skel_ctx* c, const Call& k, int* chosen) {
   return fail(c, SKEL_ERR_UNSUPPORTED, "no applicable kernel variant");
 }
 
+cudaError_t launch_call(skel_ctx* c, const Call& k, int v);
+
+// the two 1D passes through the context's temporary matrix, each with the variant its own plan picks
+cudaError_t launch_separable_two_pass(skel_ctx* c, const Call& k) {
+  const size_t bytes = k.rows * k.cols * sizeof(float);
+  if (c->sep_tmp_bytes < bytes) {
+    if (c->sep_tmp) dev_free(c, c->sep_tmp);
+    c->sep_tmp = nullptr;
+    c->sep_tmp_bytes = 0;
+    if (dev_alloc(c, bytes, &c->sep_tmp) != SKEL_OK) return cudaErrorMemoryAllocation;
+    c->sep_tmp_bytes = bytes;
+  }
+  Call p = k;
+  p.inst.skeleton = SKEL_SK_OVERLAP1D;
+  p.inst.r1 = 0;
+  p.out = c->sep_tmp;
+  int v = -1;
+  if (choose_variant(c, p, &v) != SKEL_OK) return cudaErrorInvalidValue;
+  cudaError_t e = launch_call(c, p, v);
+  if (e != cudaSuccess) return e;
+  Call q = k;
+  q.inst.skeleton = SKEL_SK_OVERLAP1D_COL;
+  q.inst.r0 = k.inst.r1;
+  q.inst.r1 = 0;
+  q.w1 = k.w1b;
+  q.in0 = c->sep_tmp;
+  if (choose_variant(c, q, &v) != SKEL_OK) return cudaErrorInvalidValue;
+  return launch_call(c, q, v);
+}
+
 cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
   Launch L{c->stream, c->sms, &c->launches};
   const skel_instance& i = k.inst;
   switch (i.skeleton) {
+    case SKEL_SK_SEPARABLE:
+      if (v == 0) return launch_separable_two_pass(c, k);
+      return launch_separable_fused(L, v, k.w1, k.w1b, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
+                                    static_cast<float*>(k.out), k.rows, k.cols);
     case SKEL_SK_MAP:
       return launch_map(L, v, i.dtype, i.fn, i.mode != 0, k.cbits, k.in0, k.in1, k.out, k.n);
     case SKEL_SK_REDUCE:
@@ -761,6 +803,7 @@ skel_status skel_ctx_destroy(skel_ctx* c) {
     flush_pending(c);
     cudaStreamSynchronize(c->stream);
     if (c->spare) dev_free(c, c->spare);
+    if (c->sep_tmp) dev_free(c, c->sep_tmp);
     cudaFree(c->scratch.partials);
     if (c->scratch.scan_state) cudaFree(c->scratch.scan_state);
     cudaFreeHost(c->h_result);
@@ -1057,6 +1100,29 @@ skel_status skel_mapoverlap_2d(skel_ctx* c, const float* W, int ry, int rx, skel
   return overlap_run(c, k, in, out);
 }
 
+skel_status skel_mapoverlap_separable(skel_ctx* c, const float* w_row, int r_row, const float* w_col, int r_col,
+                                      skel_edge edge, double pad, const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out) || !w_row || !w_col) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
+  if (r_row < 0 || r_col < 0 || r_row > SKEL_MAX_RADIUS_1D || r_col > SKEL_MAX_RADIUS_1D)
+    return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = SKEL_SK_SEPARABLE;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = SKEL_F32;
+  k.inst.r0 = r_row;
+  k.inst.r1 = r_col;
+  k.inst.edge = edge;
+  k.pad = static_cast<float>(pad);
+  memcpy(k.w1.w, w_row, sizeof(float) * (2 * r_row + 1));
+  memcpy(k.w1b.w, w_col, sizeof(float) * (2 * r_col + 1));
+  k.rows = in->rows;
+  k.cols = in->cols;
+  return overlap_run(c, k, in, out);
+}
+
 // ---- Scan -------------------------------------------------------------------------------------------
 skel_status skel_scan(skel_ctx* c, skel_fn op, skel_scan_mode mode, double init, const skel_vector* in, skel_vector* out) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
@@ -1158,7 +1224,8 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   const int sk = inst->skeleton;
   if (sk < 0 || sk >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
   if (log2_lo < 0 || log2_hi > 32 || log2_lo > log2_hi || reps < 1) return fail(c, SKEL_ERR_INVALID_ARG, "bad tuning range");
-  const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || (sk == SKEL_SK_OVERLAP1D && cols > 0);
+  const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || sk == SKEL_SK_SEPARABLE ||
+                      (sk == SKEL_SK_OVERLAP1D && cols > 0);
   if (matrix && cols == 0) return fail(c, SKEL_ERR_INVALID_ARG, "matrix skeletons need cols");
   skel_status st = ensure_device(c);
   if (st != SKEL_OK) return st;
@@ -1217,7 +1284,7 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
     k.in0 = b0;
     k.in1 = (sk == SKEL_SK_MAP || sk == SKEL_SK_MAPREDUCE) && inst->mode ? b1 : nullptr;
     k.out = (sk == SKEL_SK_REDUCE || sk == SKEL_SK_MAPREDUCE) ? c->d_result : b2;
-    for (int i = 0; i < 129; ++i) k.w1.w[i] = 1.0f / 129.0f;
+    for (int i = 0; i < 129; ++i) k.w1.w[i] = k.w1b.w[i] = 1.0f / 129.0f;
     for (int i = 0; i < 17 * 17; ++i) k.w2.w[i] = 1.0f / 289.0f;
     float best_t = 0.f;
     int best = -1;

@@ -79,6 +79,13 @@ cudaError_t launch_fused_chain(const Launch& L, const Scratch& S, int map_fn, ui
                                int edge, float pad, int red_op, const float* in, float* map_out, float* ov_out, size_t n,
                                float* result /* device, one element; unused without a Reduce */);
 
+// ---- fused separable MapOverlap on a matrix (separable.cu); variant 0 = two 1D passes (api.cu) -------
+int separable_variant_count();
+const char* separable_variant_name(int v);
+bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const void* out, size_t rows, size_t cols);
+cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r, int edge,
+                                   float pad, const float* in, float* out, size_t rows, size_t cols);
+
 // tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
 template <int R>
 cudaError_t launch_overlap2d_tiled(const Launch& L, int v, const Weights2D& w, int edge, float pad, const float* in,
