@@ -455,6 +455,30 @@ def main():
     if rank == 0 and not args.no_pipeline:
         pipeline = pipeline_experiment(S, ctx, sz["n26"])
 
+    # ---- fused separable MapOverlap (reported, not part of `value`: the step keeps the two 1D calls of
+    # BASELINE.json configs[3]); same matrix, same filters, one call instead of two
+    separable = None
+    if rank == 0 and not args.no_pipeline:
+        import torch
+        m = sz["side"] * sz["side"]
+        call = lambda: ctx.mapoverlap_separable(d["wr8"], 8, d["wc8"], 8, S.EDGE_DUPLICATE, 0.0, wl.mX, wl.mO)  # noqa: E731
+        for _ in range(3):
+            call()
+        ts = []
+        for _ in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            call()
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        us = float(np.median(ts))
+        two = per["overlap1d_rows_r8_dup"]["us"] + per["overlap1d_cols_r8_dup"]["us"]
+        separable = {"us": round(us, 2), "variant": S.variant_names(S.SK_SEPARABLE)[ctx.last_variant()[1]],
+                     "bytes_per_elem": 8, "GB/s_at_8B": round(8 * m / us / 1e3, 1),
+                     "frac_measured_hbm": round(8 * m / us / 1e3 / peak, 4),
+                     "two_calls_us": round(two, 2), "speedup_over_two_calls": round(two / us, 3)}
+
     # ---- end to end through host buffers
     e2e = None
     if not args.no_e2e:
@@ -490,7 +514,8 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "per_skeleton": per}
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable,
+                "per_skeleton": per}
         print(json.dumps(line), flush=True)
     wl.destroy()
     ctx.close()
