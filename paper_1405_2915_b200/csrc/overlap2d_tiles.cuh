@@ -101,9 +101,14 @@ __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, floa
   constexpr int SW = T2_TW + 2 * RXP;
   constexpr int NGX = (4 + 2 * RXP) / 4;
   constexpr int FW = 2 * RX + 1;
-  constexpr bool PER_ROW = (2 * RY + 1) * (2 * RX + 1) > 33;
+  // Filters with more than 33 taps are summed in groups of GR whole filter rows (at most 33 taps per
+  // chain, e.g. 9x9: three chains of 27), and the group sums are added: rounding-error bound
+  // (GR * FW + #groups - 1) * 2^-24 of sum|W x| (9x9: 29 * 2^-24 = 1.73e-6), DESIGN.md "Tolerances".
+  constexpr bool GROUPED = (2 * RY + 1) * FW > 33;
+  constexpr int GR = GROUPED ? (33 / FW > 0 ? 33 / FW : 1) : 2 * RY + 1;
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   float acc[OY][4];
+  float part[GROUPED ? OY : 1][4];  // running sum of the current group of filter rows, per output row
 #pragma unroll
   for (int o = 0; o < OY; ++o)
 #pragma unroll
@@ -122,31 +127,24 @@ __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, floa
     for (int o = 0; o < OY; ++o) {
       const int a = ir - o;  // filter row that this staged row feeds for output row o
       if (a >= 0 && a <= 2 * RY) {
-        if constexpr (PER_ROW) {
-          float p[4] = {0.f, 0.f, 0.f, 0.f};
+        float* dstp = GROUPED ? part[GROUPED ? o : 0] : acc[o];
+        if (GROUPED && a % GR == 0) {
 #pragma unroll
-          for (int b = 0; b < FW; ++b) {
-            if (PK && (RXP - RX + b) % 2 == 0) {
-              fma2_into(p[0], p[1], W.w[a * FW + b], v[RXP - RX + b], v[RXP - RX + b + 1]);
-              fma2_into(p[2], p[3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
-            } else {
+          for (int e = 0; e < 4; ++e) dstp[e] = 0.f;
+        }
 #pragma unroll
-              for (int e = 0; e < 4; ++e) p[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], p[e]);
-            }
+        for (int b = 0; b < FW; ++b) {
+          if (PK && (RXP - RX + b) % 2 == 0) {
+            fma2_into(dstp[0], dstp[1], W.w[a * FW + b], v[RXP - RX + b], v[RXP - RX + b + 1]);
+            fma2_into(dstp[2], dstp[3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
+          } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) dstp[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], dstp[e]);
           }
+        }
+        if (GROUPED && (a % GR == GR - 1 || a == 2 * RY)) {  // the group is complete
 #pragma unroll
-          for (int e = 0; e < 4; ++e) acc[o][e] = a == 0 ? p[e] : acc[o][e] + p[e];
-        } else {
-#pragma unroll
-          for (int b = 0; b < FW; ++b) {
-            if (PK && (RXP - RX + b) % 2 == 0) {
-              fma2_into(acc[o][0], acc[o][1], W.w[a * FW + b], v[RXP - RX + b], v[RXP - RX + b + 1]);
-              fma2_into(acc[o][2], acc[o][3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
-            } else {
-#pragma unroll
-              for (int e = 0; e < 4; ++e) acc[o][e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], acc[o][e]);
-            }
-          }
+          for (int e = 0; e < 4; ++e) acc[o][e] = a < GR ? dstp[e] : acc[o][e] + dstp[e];
         }
       }
     }
