@@ -197,12 +197,13 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------------------
-def cpu_oracle_pass(scale_div: int = 4, quiet=False):
+def cpu_oracle_pass(scale_div: int = 4, quiet=False, openmp=False):
     """One pass of the same hot path by the CPU oracle on a bounded sample (every size / scale_div).
-    Returns (algorithmic bytes, seconds, threads, description)."""
+    Returns (algorithmic bytes, seconds, threads, description). openmp: the OpenMP build of the same
+    loops; Reduce and Scan stay sequential in it (their order is part of the oracle)."""
     import oracle as O
     from paper_1405_2915_b200 import inputs as I
-    O.use_openmp(False)
+    O.use_openmp(openmp)
     n = (1 << 26) // scale_div
     n28 = (1 << 28) // scale_div
     side = int(8192 / np.sqrt(scale_div))
@@ -227,9 +228,12 @@ def cpu_oracle_pass(scale_div: int = 4, quiet=False):
     O.mapoverlap_1d_matrix(w[8], 8, O.EDGE_DUPLICATE, 0.0, O.AXIS_COL, T); nbytes += 8 * side * side
     O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, sc); O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 0, sc); nbytes += 16 * n28
     dt = time.perf_counter() - t0
+    build = "OpenMP build (-fopenmp)" if openmp else "single-thread build"
     desc = (f"one pass of all skeletons, each at 1/{scale_div} of its bench size (vectors 2^26/{scale_div}, scan "
-            f"2^28/{scale_div}, matrix {side}^2), single-thread build of oracle/oracle.cpp as it stands")
-    return nbytes, dt, 1, desc
+            f"2^28/{scale_div}, matrix {side}^2), {build} of oracle/oracle.cpp as it stands")
+    threads = O.threads()
+    O.use_openmp(False)
+    return nbytes, dt, threads, desc
 
 
 def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
@@ -479,6 +483,51 @@ def main():
                      "frac_measured_hbm": round(8 * m / us / 1e3 / peak, 4),
                      "two_calls_us": round(two, 2), "speedup_over_two_calls": round(two / us, 3)}
 
+    # ---- container-layer overhead ("< 1 %") and the dot-product size sweep
+    # (SURVEY.md 8(d) cfg 1): reported, not part of `value`
+    container_layer = dot_sweep = None
+    if rank == 0 and not args.no_pipeline:
+        import torch
+        enq = []
+        for _ in range(10):  # host time to ENQUEUE one step (16 asynchronous calls), device idle at the start
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            wl.step()
+            enq.append(time.perf_counter() - t0)
+            torch.cuda.synchronize()
+        host_ms = float(np.median(enq)) * 1e3
+        container_layer = {"host_us_per_call": round(host_ms * 1e3 / nops, 2), "host_ms_per_step": round(host_ms, 4),
+                           "device_ms_per_step": round(ms_per_step, 4),
+                           "host_fraction_of_device_time": round(host_ms / ms_per_step, 4),
+                           "note": "argument checks + coherence look-up + plan look-up + launch + publish, through ctypes; "
+                                   "calls are asynchronous, so this host time overlaps the device time of earlier calls"}
+        nmax = 1 << 28
+        tx, ty = torch.rand(nmax, device="cuda") * 2 - 1, torch.rand(nmax, device="cuda") * 2 - 1
+        res = ctx.vector(1)
+        dot_sweep = {}
+        for lg in range(20, 29, 2):
+            n = 1 << lg
+            va, vb = ctx.vector_adopt(tx[:n]), ctx.vector_adopt(ty[:n])
+            call = lambda: ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, va, vb, res, 0)  # noqa: E731
+            for _ in range(3):
+                call()
+            ts = []
+            for _ in range(15):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                call()
+                e1.record()
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3)
+            us = float(np.median(ts))
+            dot_sweep[f"2^{lg}"] = {"us": round(us, 2), "GB/s": round(8 * n / us / 1e3, 1),
+                                    "frac_measured_hbm": round(8 * n / us / 1e3 / peak, 4),
+                                    "l2_resident": 8 * n <= 126 * (1 << 20)}
+            va.destroy()
+            vb.destroy()
+        res.destroy()
+        del tx, ty
+
     # ---- end to end through host buffers
     e2e = None
     if not args.no_e2e:
@@ -496,11 +545,14 @@ def main():
                "h2d_bytes_per_step": st["h2d_bytes"] // args.steps, "d2h_bytes_per_step": st["d2h_bytes"] // args.steps,
                "ms_per_step": round(dt / args.steps * 1e3, 2)}
 
-    cpu = None
+    cpu = cpu_omp = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         nb, dt, threads, desc = cpu_oracle_pass(2)
         cpu = {"value": round(nb / dt / 1e9, 3), "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
                "seconds": round(dt, 2), "host_cores_available": os.cpu_count()}
+        nb, dt, threads, desc = cpu_oracle_pass(2, openmp=True)
+        cpu_omp = {"value": round(nb / dt / 1e9, 3), "unit": UNIT, "cores": threads, "kind": "oracle", "sample": desc,
+                   "seconds": round(dt, 2)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -515,6 +567,7 @@ def main():
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                 "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable,
+                "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)
     wl.destroy()
