@@ -596,7 +596,10 @@ skel_status flush_pending(skel_ctx* c) {
     if (kind == 3) red = &p.k;
   }
   skel_status st = SKEL_OK;
-  if (ov && (map || red)) {
+  // a Reduce whose result lands inside a container the chain itself writes keeps the call-by-call order
+  // (the in-place Map's buffer may be swapped under it)
+  const bool result_in_chain = red && red->out_st && ((map && red->out_st == map->out_st) || (ov && red->out_st == ov->out_st));
+  if (ov && (map || red) && !result_in_chain) {
     const float* in = static_cast<const float*>(map ? map->in0 : ov->in0);
     float* map_out = map ? static_cast<float*>(map->out) : nullptr;
     bool swap = false;
@@ -737,6 +740,7 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   k.n = a->n;
   k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->d_result;
   k.in_st = a;
+  k.out_st = out ? out->st : nullptr;
   st = run_call(c, k);
   if (st != SKEL_OK) return st;
   st = publish_all(c, set);

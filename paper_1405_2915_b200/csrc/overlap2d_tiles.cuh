@@ -426,8 +426,8 @@ inline cudaError_t make_tmap_2d(CUtensorMap* out, const float* base, size_t rows
     encode = reinterpret_cast<EncodeFn>(fn);
   }
   struct Key { const float* base; size_t rows, cols; int bw, bh; };
-  static Key last = {nullptr, 0, 0, 0, 0};
-  static CUtensorMap last_map;
+  static thread_local Key last = {nullptr, 0, 0, 0, 0};  // per host thread: contexts may live on different threads
+  static thread_local CUtensorMap last_map;
   if (last.base == base && last.rows == rows && last.cols == cols && last.bw == box_w && last.bh == box_h) {
     *out = last_map;
     return cudaSuccess;

@@ -238,3 +238,34 @@ def test_fused_pipeline_iterations_ping_pong(ctx):
         xa = b64.astype(np.float32)
     final = a.numpy()
     assert np.allclose(final, xa, rtol=iters * 4e-6, atol=0)
+
+
+def test_fusion_with_eager_coherence_and_result_inside_the_chain(ctx):
+    n, r = 20011, 4
+    x = I.uniform01_f32(I.config_seed(5, 8), n)
+    w = I.positive_weights_f32(I.config_seed(3, 14), 9)
+    ref = oracle_chain(x, O.FN_MULT, 1.0001, w, r, O.EDGE_DUPLICATE, 0.0, O.FN_ADD)
+    # EAGER coherence uploads and downloads around every call: every transfer flushes, nothing fuses
+    ctx.set_coherence(S.EAGER)
+    a, b = ctx.vector_from(x), ctx.vector(n)
+    ctx.reset_stats()
+    ctx.map(S.FN_MULT, 1.0001, a, None, a)
+    ctx.mapoverlap_1d(w, r, S.EDGE_DUPLICATE, 0.0, a, b)
+    s = ctx.reduce(S.FN_ADD, b)
+    ctx.set_coherence(S.LAZY)
+    assert ctx.stats()["fused_launches"] == 0
+    check_chain(a.numpy(), b.numpy(), s, ref, O.FN_ADD)
+    # the Reduce writes its result INTO the Map's container: call-by-call order is kept (Map + MapOverlap fuse)
+    a2, b2 = ctx.vector_from(x), ctx.vector(n)
+    ctx.reset_stats()
+    ctx.map(S.FN_MULT, 1.0001, a2, None, a2)
+    ctx.mapoverlap_1d(w, r, S.EDGE_DUPLICATE, 0.0, a2, b2)
+    ctx.reduce_to(S.FN_ADD, b2, a2, 7)
+    st = ctx.stats()
+    assert st["fused_launches"] == 0 and st["launches"] == 3
+    got_a = a2.numpy()
+    exp_a = ref[0].copy()
+    s2 = got_a[7]
+    exp_a[7] = s2
+    assert np.array_equal(got_a, exp_a)
+    check_chain(None, b2.numpy(), s2, ref, O.FN_ADD)
