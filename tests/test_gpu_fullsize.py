@@ -122,3 +122,62 @@ def test_overlap2d_and_separable_8192(ctx):
         assert_overlap(np.ascontiguousarray(out[:, j]), ref, ab)
     for c in (mx, mt, mo):
         c.destroy()
+
+
+def test_fused_separable_8192(ctx):
+    """skel_mapoverlap_separable at the bench size, with the variant the plan picks: whole result bit-identical to
+    the two public 1D calls (same taps, same order, same fp32 intermediate), sampled columns against the oracle's
+    row pass (fp32) fed to its column pass."""
+    X = I.uniform01_f32(I.config_seed(4, 0), SIDE * SIDE).reshape(SIDE, SIDE)
+    wr, wc = I.positive_weights_f32(I.config_seed(4, 3), 17), I.positive_weights_f32(I.config_seed(4, 4), 17)
+    mx, mt, mo, mf = ctx.matrix_from(X), ctx.matrix(SIDE, SIDE), ctx.matrix(SIDE, SIDE), ctx.matrix(SIDE, SIDE)
+    ctx.mapoverlap_separable(wr, 8, wc, 8, S.EDGE_DUPLICATE, 0.0, mx, mf)
+    sk, v = ctx.last_variant()
+    assert sk == S.SK_SEPARABLE and S.variant_names(sk)[v].startswith("fused")
+    ctx.mapoverlap_1d_matrix(wr, 8, S.EDGE_DUPLICATE, 0.0, S.AXIS_ROW, mx, mt)
+    ctx.mapoverlap_1d_matrix(wc, 8, S.EDGE_DUPLICATE, 0.0, S.AXIS_COL, mt, mo)
+    fused = mf.numpy()
+    assert np.array_equal(fused, mo.numpy())
+    for j in (0, 5, 127, 128, 4097, SIDE - 1):
+        # the row pass of column j reads columns j-8 .. j+8 (clamped): cut a block that contains them and whose own
+        # clamping coincides with the matrix's (it starts at column 0 / ends at the last column) or is never reached
+        lo = 0 if j < 16 else j - 8
+        hi = SIDE if j >= SIDE - 16 else j + 9
+        sub = np.ascontiguousarray(X[:, lo:hi])
+        jj = j - lo
+        t64, tabs = O.mapoverlap_1d_matrix(wr, 8, O.EDGE_DUPLICATE, 0.0, O.AXIS_ROW, sub)
+        tcol = np.ascontiguousarray(t64[:, jj]).astype(np.float32)
+        ref, ab = O.mapoverlap_1d(wc, 8, O.EDGE_DUPLICATE, 0.0, tcol)
+        carried, _ = O.mapoverlap_1d(wc, 8, O.EDGE_DUPLICATE, 0.0, np.ascontiguousarray(tabs[:, jj]).astype(np.float32))
+        err = np.abs(np.ascontiguousarray(fused[:, j]).astype(np.float64) - ref)
+        assert np.all(err <= 2e-6 * (ab + 1.000001 * carried)), (j, float((err / (ab + carried)).max()))
+    for c in (mx, mt, mo, mf):
+        c.destroy()
+
+
+def test_fused_chain_2p26(ctx):
+    """The chained pipeline iteration of BASELINE.json configs[4] as ONE kernel (skel_ctx_set_fusion) at the bench
+    size: A' bit-identical to the oracle's Map, B on sampled windows, the sum against the oracle chain."""
+    x = I.uniform01_f32(I.config_seed(5, 1), N26)
+    w = I.positive_weights_f32(I.config_seed(3, 14), 9)
+    a, b = ctx.vector_from(x), ctx.vector(N26)
+    ctx.set_fusion(True)
+    try:
+        ctx.reset_stats()
+        ctx.map(S.FN_MULT, 1.0001, a, None, a)
+        ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
+        s = ctx.reduce(S.FN_ADD, b)
+        st = ctx.stats()
+    finally:
+        ctx.set_fusion(False)
+    assert st["fused_launches"] == 1 and st["launches"] == 1
+    a1 = O.map_f32(O.FN_MULT, 1.0001, x).astype(np.float32)
+    assert np.array_equal(a.numpy(), a1)
+    ref, ab = O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, a1)
+    got = b.numpy()
+    for lo, hi in windows(N26, 50000):
+        assert_overlap(got[lo:hi], ref[lo:hi], ab[lo:hi])
+    r, asum = O.reduce_f32(O.FN_ADD, ref.astype(np.float32))
+    assert abs(s - r) <= 1e-5 * asum + 2e-6 * float(ab.sum()), (s, r)
+    a.destroy()
+    b.destroy()
