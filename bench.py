@@ -437,6 +437,20 @@ def main():
                 "peak_source": peak_src, "launches_per_step": dcount, "avg_launch_us": round(dt_ms * 1e3 / dcount, 2),
                 "share_of_step": round(dt_ms / ms_per_step, 4)}
 
+    # ---- arithmetic roofline of the MapOverlap rows: FMAs per element over the FP32 FMA rate
+    # measured in this run by a register-only FFMA kernel; "bound" = the larger of the two floors
+    fma_peak = ctx.probe_fma_peak(5)  # FMA/s
+    fma_per_elem = {"overlap1d_r1": 3, "overlap1d_r4": 9, "overlap1d_r16": 33, "overlap2d_5x5": 25, "overlap2d_9x9": 81,
+                    "overlap1d_rows_r8": 17, "overlap1d_cols_r8": 17}
+    for name, _, _, nbytes, elems in wl.ops:
+        for key, f in fma_per_elem.items():
+            if name.startswith(key):
+                alu_us = elems * f / fma_peak * 1e6
+                hbm_us = nbytes / (peak * 1e9) * 1e6
+                per[name].update({"fma_per_elem": f, "alu_floor_us": round(alu_us, 1), "hbm_floor_us": round(hbm_us, 1),
+                                  "bound": "alu" if alu_us > hbm_us else "hbm",
+                                  "frac_fma_roofline": round(alu_us / per[name]["us"], 4)})
+
     # ---- small-n latency (config 0: dot n = 2^20, L2 resident) — reported, not part of `value`
     from paper_1405_2915_b200 import inputs as I
     n20 = 1 << 20
@@ -567,7 +581,7 @@ def main():
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                 "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable,
-                "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
+                "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)
     wl.destroy()

@@ -262,6 +262,10 @@ typedef struct {
   uint64_t fused_calls;              /* skeleton calls that ran inside a fused-chain kernel */
 } skel_stats;
 skel_status skel_get_stats(skel_ctx* ctx, skel_stats* out);
+/* Measures the FP32 fused-multiply-add throughput of the device with a register-only FFMA kernel
+ * (median of `reps` launches, CUDA events on the context's stream; synchronises): *fma_per_s = FMAs per
+ * second (x 2 = FLOP/s). The roofline of the arithmetic-bound MapOverlap instances. */
+skel_status skel_probe_fma_peak(skel_ctx* ctx, int reps, double* fma_per_s);
 skel_status skel_reset_stats(skel_ctx* ctx);
 
 /* The coherence protocol as a pure function (used by the library itself

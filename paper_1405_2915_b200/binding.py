@@ -65,6 +65,7 @@ _SIGS = {
     "skel_ctx_destroy": ([_vp], _i),
     "skel_ctx_sync": ([_vp], _i),
     "skel_ctx_set_coherence": ([_vp, _i], _i),
+    "skel_probe_fma_peak": ([_vp, _i, C.POINTER(C.c_double)], _i),
     "skel_ctx_set_fusion": ([_vp, _i], _i),
     "skel_ctx_flush": ([_vp], _i),
     "skel_last_error": ([_vp], C.c_char_p),
@@ -182,6 +183,12 @@ class Context:
 
     def set_coherence(self, mode: int):
         self.check(lib.skel_ctx_set_coherence(self.h, mode))
+
+    def probe_fma_peak(self, reps: int = 5) -> float:
+        """FP32 FMAs per second of the device (register-only FFMA kernel)."""
+        out = C.c_double(0.0)
+        self.check(lib.skel_probe_fma_peak(self.h, reps, C.byref(out)))
+        return out.value
 
     def set_fusion(self, enable: bool):
         self.check(lib.skel_ctx_set_fusion(self.h, 1 if enable else 0))

@@ -1344,6 +1344,40 @@ skel_status skel_get_stats(skel_ctx* c, skel_stats* out) {
   return SKEL_OK;
 }
 
+skel_status skel_probe_fma_peak(skel_ctx* c, int reps, double* fma_per_s) {
+  if (!ctx_ok(c) || !fma_per_s || reps < 1) return SKEL_ERR_INVALID_ARG;
+  skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  cudaEvent_t e0, e1;
+  CU(c, cudaEventCreate(&e0));
+  CU(c, cudaEventCreate(&e1));
+  Launch L{c->stream, c->sms, &c->launches};
+  std::vector<float> ms(reps);
+  double count = 0;
+  for (int r = -1; r < reps; ++r) {  // r = -1 warms up
+    cudaEventRecord(e0, c->stream);
+    cudaError_t e = launch_fma_probe(L, static_cast<float*>(c->d_result), &count);
+    cudaEventRecord(e1, c->stream);
+    if (e != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess) {
+      cudaEventDestroy(e0);
+      cudaEventDestroy(e1);
+      return cuda_fail(c, e != cudaSuccess ? e : cudaGetLastError(), "FMA probe");
+    }
+    float t = 0.f;
+    cudaEventElapsedTime(&t, e0, e1);
+    if (r >= 0) ms[r] = t;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  std::sort(ms.begin(), ms.end());
+  *fma_per_s = count / (double(ms[reps / 2]) * 1e-3);
+  c->stats.launches += c->launches;
+  c->launches = 0;
+  return SKEL_OK;
+}
+
 skel_status skel_reset_stats(skel_ctx* c) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
   c->stats = skel_stats{};

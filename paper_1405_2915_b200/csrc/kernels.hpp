@@ -86,6 +86,9 @@ bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const voi
 cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r, int edge,
                                    float pad, const float* in, float* out, size_t rows, size_t cols);
 
+// ---- FP32 FMA roofline probe (probe.cu) ------------------------------------------------------------
+cudaError_t launch_fma_probe(const Launch& L, float* scratch /* device, >= 1 float */, double* fma_count);
+
 // tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
 template <int R>
 cudaError_t launch_overlap2d_tiled(const Launch& L, int v, const Weights2D& w, int edge, float pad, const float* in,
