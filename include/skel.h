@@ -230,8 +230,10 @@ int skel_variant_count(int skeleton);
 const char* skel_variant_name(int skeleton, int variant);
 /* Measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), median
  * of `reps` launches timed with CUDA events on the context stream, and store size breakpoints
- * in the context's plan. For matrix skeletons `cols` gives the row length (rows = n/cols);
- * pass 0 for vectors. Blocks. */
+ * in the context's plan. Where the winner changes between two sampled sizes the interval is
+ * bisected (only the two contenders are timed) until it is narrower than 2^(1/4), so breakpoints
+ * are not confined to powers of two (adaptive sampling). For matrix skeletons `cols`
+ * gives the row length (rows = n/cols); pass 0 for vectors. Blocks. */
 skel_status skel_tune_instance(skel_ctx* ctx, const skel_instance* inst, int log2_lo, int log2_hi, size_t cols, int reps);
 skel_status skel_plan_save(skel_ctx* ctx, const char* path);
 skel_status skel_plan_load(skel_ctx* ctx, const char* path);

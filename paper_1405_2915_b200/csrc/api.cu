@@ -1272,62 +1272,107 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   const InstanceKey key = key_of(*inst);
   c->plan.erase(key);
   int prev_best = -1;
+  size_t prev_n = 0;
   skel_status result = SKEL_OK;
-  std::vector<float> samples(reps);
-  for (int lg = log2_lo; lg <= log2_hi && result == SKEL_OK; ++lg) {
-    Call k;
+  auto make_call = [&](size_t n, Call& k) -> bool {  // false: size not representable (matrix smaller than a row)
     k.inst = *inst;
-    k.n = size_t(1) << lg;
+    k.n = n;
     k.rows = 1;
-    k.cols = k.n;
+    k.cols = n;
     if (matrix) {
-      if (k.n < cols) continue;
+      if (n < cols) return false;
       k.cols = cols;
-      k.rows = k.n / cols;
+      k.rows = n / cols;
+      k.n = k.rows * cols;
     }
     k.in0 = b0;
     k.in1 = (sk == SKEL_SK_MAP || sk == SKEL_SK_MAPREDUCE) && inst->mode ? b1 : nullptr;
     k.out = (sk == SKEL_SK_REDUCE || sk == SKEL_SK_MAPREDUCE) ? c->d_result : b2;
     for (int i = 0; i < 129; ++i) k.w1.w[i] = k.w1b.w[i] = 1.0f / 129.0f;
     for (int i = 0; i < 17 * 17; ++i) k.w2.w[i] = 1.0f / 289.0f;
+    return true;
+  };
+  // Median of `reps` launches of every variant in `vs`, INTERLEAVED (rep-major): clock and power state drift
+  // during a tuning run (sw_power_cap), and timing one variant after the other mis-ranks near-equal ones.
+  std::vector<std::vector<float>> tsamp;
+  auto time_variants = [&](const Call& k, const std::vector<int>& vs, std::vector<float>& med_us) -> bool {
+    tsamp.assign(vs.size(), std::vector<float>());
+    for (int rep = -1; rep < reps; ++rep) {  // rep -1 is the warm-up
+      for (size_t j = 0; j < vs.size(); ++j) {
+        cudaEventRecord(e0, c->stream);
+        const bool bad = launch_call(c, k, vs[j]) != cudaSuccess;
+        cudaEventRecord(e1, c->stream);
+        if (cudaEventSynchronize(e1) != cudaSuccess || bad) return false;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep >= 0) tsamp[j].push_back(ms * 1000.f);
+      }
+    }
+    med_us.resize(vs.size());
+    for (size_t j = 0; j < vs.size(); ++j) {
+      std::sort(tsamp[j].begin(), tsamp[j].end());
+      med_us[j] = tsamp[j][reps / 2];
+    }
+    return true;
+  };
+  std::vector<int> vs;
+  std::vector<float> meds;
+  for (int lg = log2_lo; lg <= log2_hi && result == SKEL_OK; ++lg) {
+    Call k;
+    if (!make_call(size_t(1) << lg, k)) continue;
     float best_t = 0.f;
     int best = -1;
-    for (int v = 0; v < nv; ++v) {
-      if (!variant_ok(k, v)) continue;
-      bool bad = false;
-      for (int rep = -1; rep < reps && !bad; ++rep) {  // rep -1 is the warm-up
-        cudaEventRecord(e0, c->stream);
-        bad = launch_call(c, k, v) != cudaSuccess;
-        cudaEventRecord(e1, c->stream);
-        if (cudaEventSynchronize(e1) != cudaSuccess) bad = true;
-        float ms = 0.f;
-        if (!bad) cudaEventElapsedTime(&ms, e0, e1);
-        if (rep >= 0) samples[rep] = ms * 1000.f;
-      }
-      if (bad) {
-        result = cuda_fail(c, cudaGetLastError(), "tuning launch");
-        break;
-      }
-      std::sort(samples.begin(), samples.end());
-      const float med = samples[reps / 2];
-      c->tune_table[size_t(lg - log2_lo) * nv + v] = med;
-      if (best < 0 || med < best_t) {  // ties -> lower variant id
-        best = v;
-        best_t = med;
+    vs.clear();
+    for (int v = 0; v < nv; ++v)
+      if (variant_ok(k, v)) vs.push_back(v);
+    if (!time_variants(k, vs, meds)) {
+      result = cuda_fail(c, cudaGetLastError(), "tuning launch");
+      break;
+    }
+    for (size_t j = 0; j < vs.size(); ++j) {
+      c->tune_table[size_t(lg - log2_lo) * nv + vs[j]] = meds[j];
+      if (best < 0 || meds[j] < best_t) {  // ties -> lower variant id
+        best = vs[j];
+        best_t = meds[j];
       }
     }
-    // hysteresis: keep the previous size's winner unless it is more than 3 % slower than the best here
-    // (timing noise otherwise turns the plan into a list of spurious breakpoints)
+    if (result != SKEL_OK) break;
+    // hysteresis: keep the previous size's winner unless it is more than 3 % AND more than 0.5 us slower than
+    // the best here (timing noise otherwise turns the plan into a list of spurious breakpoints, above all at
+    // the launch-latency-bound small sizes where every variant takes the same few microseconds)
     if (best >= 0 && prev_best >= 0 && prev_best != best) {
       const float tp = c->tune_table[size_t(lg - log2_lo) * nv + prev_best];
-      if (tp == tp && tp <= 1.03f * best_t) best = prev_best;
+      if (tp == tp && (tp <= 1.03f * best_t || tp <= best_t + 0.5f)) best = prev_best;
     }
-    c->stats.launches += c->launches;
-    c->launches = 0;
     if (best >= 0 && best != prev_best) {
-      c->plan.set(key, prev_best < 0 ? 0 : k.n, best);
+      size_t n_min = prev_best < 0 ? 0 : k.n;
+      if (prev_best >= 0) {
+        // Adaptive refinement (adaptive sampling of the context space): the winner changes
+        // somewhere in (prev_n, k.n]; bisect that interval (geometric midpoints, rounded to whole rows / 1024
+        // elements), timing only the two contenders, until it is narrower than 2^(1/4).
+        size_t lo = prev_n, hi = k.n;
+        const size_t gran = matrix ? cols : 1024;
+        while (result == SKEL_OK && double(hi) / double(lo) > 1.19) {
+          size_t mid = static_cast<size_t>(std::sqrt(double(lo) * double(hi))) / gran * gran;
+          if (mid <= lo || mid >= hi) break;
+          Call m;
+          if (!make_call(mid, m) || !variant_ok(m, prev_best) || !variant_ok(m, best)) break;
+          if (!time_variants(m, {prev_best, best}, meds)) {
+            result = cuda_fail(c, cudaGetLastError(), "tuning launch");
+            break;
+          }
+          const float t_old = meds[0], t_new = meds[1];
+          if (t_old <= 1.03f * t_new || t_old <= t_new + 0.5f) lo = mid;  // the old winner still holds (same hysteresis)
+          else hi = mid;
+        }
+        n_min = hi;
+      }
+      c->plan.set(key, n_min, best);
       prev_best = best;
     }
+    prev_n = k.n;
+    c->stats.launches += c->launches;
+    c->launches = 0;
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);

@@ -42,7 +42,7 @@ def instances(S):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(HERE, "plans", "b200.plan"))
-    ap.add_argument("--reps", type=int, default=7)
+    ap.add_argument("--reps", type=int, default=11)
     ap.add_argument("--tables", default=None, help="write the timing tables as JSON here")
     ap.add_argument("--only", default=None, help="tune only the instances whose name contains this substring")
     ap.add_argument("--base", default=None, help="start from this plan file (instances not tuned keep their entries)")
