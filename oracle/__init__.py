@@ -65,6 +65,8 @@ def _lib() -> C.CDLL:
         L.oracle_map_i32.argtypes = [i, C.c_int32, _i32p, vp, sz, _i32p]
         L.oracle_reduce_f32.argtypes = [i, _f32p, sz, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_reduce_i32.argtypes = [i, _i32p, sz, C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+        L.oracle_reduce_rows_f32.argtypes = [i, _f32p, sz, sz, _f64p, _f64p]
+        L.oracle_reduce_rows_i32.argtypes = [i, _i32p, sz, sz, _i32p]
         L.oracle_mapreduce_f32.argtypes = [i, i, dbl, _f32p, vp, sz, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_mapreduce_i32.argtypes = [i, i, C.c_int32, _i32p, vp, sz, C.POINTER(C.c_int32)]
         L.oracle_scan_i32.argtypes = [i, i, C.c_int32, _i32p, sz, _i32p]
@@ -73,7 +75,8 @@ def _lib() -> C.CDLL:
         L.oracle_mapoverlap_1d_matrix_f32.argtypes = [_f32p, i, i, dbl, i, _f32p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_1d_matrix_f64.argtypes = [_f32p, i, i, dbl, i, _f64p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_2d_f32.argtypes = [_f32p, i, i, i, dbl, _f32p, sz, sz, sz, sz, _f64p, _f64p]
-        for name in ("oracle_reduce_f32", "oracle_reduce_i32", "oracle_mapreduce_f32", "oracle_mapreduce_i32"):
+        for name in ("oracle_reduce_f32", "oracle_reduce_i32", "oracle_mapreduce_f32", "oracle_mapreduce_i32",
+                     "oracle_reduce_rows_f32", "oracle_reduce_rows_i32"):
             getattr(L, name).restype = i
         _loaded[_omp] = L
     return _loaded[_omp]
@@ -121,6 +124,25 @@ def reduce_i32(op: int, x):
     if _lib().oracle_reduce_i32(op, x, x.size, C.byref(r), C.byref(e)) != 0:
         raise ValueError("reduce of an empty vector")
     return r.value, e.value
+
+
+def reduce_rows_f32(op: int, X):
+    """Row-wise Reduce of a matrix -> (fp64 results[rows], sum |x| per row)."""
+    X = _c(X, np.float32)
+    rows, cols = X.shape
+    r, a = np.empty(rows, np.float64), np.empty(rows, np.float64)
+    if _lib().oracle_reduce_rows_f32(op, X.reshape(-1), rows, cols, r, a) != 0:
+        raise ValueError("reduce of empty rows")
+    return r, a
+
+
+def reduce_rows_i32(op: int, X) -> np.ndarray:
+    X = _c(X, np.int32)
+    rows, cols = X.shape
+    r = np.empty(rows, np.int32)
+    if _lib().oracle_reduce_rows_i32(op, X.reshape(-1), rows, cols, r) != 0:
+        raise ValueError("reduce of empty rows")
+    return r
 
 
 def mapreduce_f32(map_f: int, red_op: int, c: float, in0, in1=None):

@@ -192,6 +192,27 @@ int oracle_reduce_f32(int op, const float* in, size_t n, double* result, double*
   return 0;
 }
 
+// ---- row-wise Reduce on a matrix: out[i] = Reduce(row i), every row on its own,
+// by the vector Reduce above (that IS the definition). cols == 0 -> returns -1.
+int oracle_reduce_rows_f32(int op, const float* in, size_t rows, size_t cols, double* result, double* abs_sum) {
+  if (cols == 0) return -1;
+#pragma omp parallel for schedule(static)
+  for (long long i = 0; i < (long long)rows; ++i)
+    oracle_reduce_f32(op, in + size_t(i) * cols, cols, result + i, abs_sum ? abs_sum + i : nullptr);
+  return 0;
+}
+
+int oracle_reduce_i32(int op, const int32_t* in, size_t n, int32_t* result, int64_t* exact_i64);
+int oracle_reduce_rows_i32(int op, const int32_t* in, size_t rows, size_t cols, int32_t* result) {
+  if (cols == 0) return -1;
+#pragma omp parallel for schedule(static)
+  for (long long i = 0; i < (long long)rows; ++i) {
+    int64_t ex;
+    oracle_reduce_i32(op, in + size_t(i) * cols, cols, result + i, &ex);
+  }
+  return 0;
+}
+
 // exact_i64 receives the un-wrapped int64 sum for op == add (information only).
 int oracle_reduce_i32(int op, const int32_t* in, size_t n, int32_t* result, int64_t* exact_i64) {
   if (n == 0) return -1;

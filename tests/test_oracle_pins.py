@@ -195,6 +195,50 @@ def test_dot_closed_form_and_unit_vectors():
     assert r >= 0 and r == pytest.approx(a, rel=1e-15)
 
 
+def test_reduce_rows_closed_forms_library_and_brute_force():
+    """Row-wise Reduce: closed forms, numpy's axis reductions and math.fsum (independent
+    library routines), Python-int brute force for the int32 wrap, and the transposition / vector-Reduce
+    invariants. A dropped row, a row/column mix-up or a wrong stride fails one of them."""
+    rows, cols = 37, 129
+    # closed forms: X[i][j] = i -> cols * i; X[i][j] = j -> cols (cols - 1) / 2 in every row
+    Xi = np.repeat(np.arange(rows, dtype=np.float32)[:, None], cols, axis=1)
+    r, a = O.reduce_rows_f32(O.FN_ADD, Xi)
+    assert r.tolist() == [float(cols * i) for i in range(rows)] and a.tolist() == r.tolist()
+    Xj = np.repeat(np.arange(cols, dtype=np.int32)[None, :], rows, axis=0)
+    assert O.reduce_rows_i32(O.FN_ADD, Xj).tolist() == [cols * (cols - 1) // 2] * rows
+    assert O.reduce_rows_i32(O.FN_MAX, Xj).tolist() == [cols - 1] * rows
+    # library routines on random data (not symmetric under transposition: a swapped axis is caught)
+    X = I.uniform_pm1_f32(71, rows * cols).reshape(rows, cols)
+    r, a = O.reduce_rows_f32(O.FN_ADD, X)
+    for i in range(rows):
+        assert r[i] == pytest.approx(math.fsum(float(v) for v in X[i]), rel=0, abs=1e-12)
+        assert a[i] == pytest.approx(math.fsum(abs(float(v)) for v in X[i]), rel=1e-15)
+    assert np.array_equal(O.reduce_rows_f32(O.FN_MAX, X)[0], X.max(axis=1).astype(np.float64))
+    P = 1.0 + 0.001 * X[:5, :40]
+    assert np.allclose(O.reduce_rows_f32(O.FN_MULT, P)[0], np.prod(P.astype(np.float64), axis=1), rtol=1e-13)
+    # every row is the vector Reduce of that row; the row-wise Reduce of X^T reduces the columns of X
+    for i in (0, 7, rows - 1):
+        assert O.reduce_f32(O.FN_ADD, X[i])[0] == r[i]
+    rt, _ = O.reduce_rows_f32(O.FN_ADD, np.ascontiguousarray(X.T))
+    assert np.allclose(rt, X.astype(np.float64).sum(axis=0), rtol=0, atol=1e-12)
+    # int32: wraps modulo 2^32 (Python integers are exact)
+    V = (I.raw_u64(72, 6 * 50) % np.uint64(1 << 31)).astype(np.int64).reshape(6, 50)
+    V32 = V.astype(np.int32)
+    assert O.reduce_rows_i32(O.FN_ADD, V32).tolist() == [wrap32(sum(int(v) for v in row)) for row in V32]
+    assert O.reduce_rows_i32(O.FN_MULT, V32[:, :5]).tolist() == [wrap32(math.prod(int(v) for v in row[:5])) for row in V32]
+    # shapes: a single column is the identity, a single row is the vector Reduce; empty rows are an error
+    assert np.array_equal(O.reduce_rows_f32(O.FN_ADD, X[:, :1])[0], X[:, 0].astype(np.float64))
+    assert O.reduce_rows_f32(O.FN_ADD, X[:1])[0][0] == O.reduce_f32(O.FN_ADD, X[0])[0]
+    with pytest.raises(ValueError):
+        O.reduce_rows_f32(O.FN_ADD, np.zeros((3, 0), np.float32))
+    # the OpenMP build computes the same rows
+    O.use_openmp(True)
+    try:
+        assert np.array_equal(O.reduce_rows_f32(O.FN_ADD, X)[0], r)
+    finally:
+        O.use_openmp(False)
+
+
 def test_mapreduce_fusion_invariant_and_brute_force():
     for n in BOUNDARY_N:
         x = I.uniform_pm1_f32(60 + n, n)
