@@ -497,6 +497,31 @@ def main():
                      "frac_measured_hbm": round(8 * m / us / 1e3 / peak, 4),
                      "two_calls_us": round(two, 2), "speedup_over_two_calls": round(two / us, 3)}
 
+    # ---- row-wise Reduce on the 8192^2 matrix (reported, not part of `value`)
+    reduce_rows = None
+    if rank == 0 and not args.no_pipeline:
+        import torch
+        m = sz["side"] * sz["side"]
+        rr = ctx.vector(sz["side"])
+        call = lambda: ctx.reduce_rows(S.FN_ADD, wl.mX, rr)  # noqa: E731
+        for _ in range(3):
+            call()
+        ts = []
+        for _ in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            call()
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        us = float(np.median(ts))
+        got = rr.numpy()
+        ref = d["X"].astype(np.float64).sum(axis=1)
+        assert np.all(np.abs(got - ref) <= 1e-5 * np.abs(d["X"]).astype(np.float64).sum(axis=1)), "reduce_rows mismatch"
+        reduce_rows = {"us": round(us, 2), "variant": S.variant_names(S.SK_REDUCE_ROWS)[ctx.last_variant()[1]],
+                       "bytes_per_elem": 4, "GB/s": round(4 * m / us / 1e3, 1), "frac_measured_hbm": round(4 * m / us / 1e3 / peak, 4)}
+        rr.destroy()
+
     # ---- container-layer overhead ("< 1 %") and the dot-product size sweep
     # (SURVEY.md 8(d) cfg 1): reported, not part of `value`
     container_layer = dot_sweep = None
@@ -580,7 +605,7 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable,
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows,
                 "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)

@@ -80,7 +80,8 @@ typedef enum {
   SKEL_SK_OVERLAP1D_COL = 5,  /* column-wise on a matrix */
   SKEL_SK_OVERLAP2D = 6,
   SKEL_SK_SEPARABLE = 7,      /* skel_mapoverlap_separable (variant 0 = the two 1D passes) */
-  SKEL_SK_COUNT = 8
+  SKEL_SK_REDUCE_ROWS = 8,    /* skel_reduce_rows */
+  SKEL_SK_COUNT = 9
 } skel_skeleton;
 
 typedef struct skel_ctx skel_ctx;
@@ -182,6 +183,12 @@ skel_status skel_mapreduce(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double 
                            const skel_vector* in1, void* host_result);
 skel_status skel_mapreduce_to(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double c, const skel_vector* in0,
                               const skel_vector* in1, skel_vector* out, size_t out_index);
+
+/* Row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] for every row i.
+ * `out` has `rows` elements of the matrix's element type (f32 or i32; i32 add / mult wrap modulo 2^32);
+ * (+) in {ADD, MULT, MAX}. cols == 0 with rows > 0 -> SKEL_ERR_EMPTY. f32: each row within the Reduce tolerance,
+ * deterministic for a given shape and variant. */
+skel_status skel_reduce_rows(skel_ctx* ctx, skel_fn op, const skel_matrix* in, skel_vector* out);
 
 /* MapOverlap 1D (f32 only): out[i] = sum_{k=-r..r} w[k+r] * x~[i+k] (correlation: w[0]
  * multiplies the left-most neighbour). w: HOST pointer to 2r+1 floats, copied at call time.

@@ -35,7 +35,7 @@ SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
 AXIS_ROW, AXIS_COL = 0, 1
 READ, WRITE, READWRITE = 0, 1, 2
 LAZY, EAGER = 0, 1
-SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_SEPARABLE, SK_COUNT = range(9)
+SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_SEPARABLE, SK_REDUCE_ROWS, SK_COUNT = range(10)
 ST_UNINIT, ST_HOST, ST_DEVICE, ST_SHARED = 0, 1, 2, 3
 
 _NP = {F32: np.float32, I32: np.int32}
@@ -91,6 +91,7 @@ _SIGS = {
     "skel_reduce_to": ([_vp, _i, _vp, _vp, _sz], _i),
     "skel_mapreduce": ([_vp, _i, _i, _d, _vp, _vp, _vp], _i),
     "skel_mapreduce_to": ([_vp, _i, _i, _d, _vp, _vp, _vp, _sz], _i),
+    "skel_reduce_rows": ([_vp, _i, _vp, _vp], _i),
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
@@ -280,6 +281,9 @@ class Context:
 
     def mapreduce_to(self, map_f: int, red_op: int, c: float, in0, in1, out: "Vector", out_index: int = 0):
         self.check(lib.skel_mapreduce_to(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, out.h, out_index))
+
+    def reduce_rows(self, op: int, x: "Matrix", out: "Vector"):
+        self.check(lib.skel_reduce_rows(self.h, op, x.h, out.h))
 
     def mapoverlap_1d(self, w, r: int, edge: int, pad: float, x: "Vector", out: "Vector"):
         w = np.ascontiguousarray(w, np.float32)

@@ -405,6 +405,7 @@ int variant_count(int sk) {
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_count();
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_count();
     case SKEL_SK_SEPARABLE: return separable_variant_count();
+    case SKEL_SK_REDUCE_ROWS: return reduce_rows_variant_count();
   }
   return 0;
 }
@@ -419,6 +420,7 @@ const char* variant_name(int sk, int v) {
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_name(v);
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_name(v);
     case SKEL_SK_SEPARABLE: return separable_variant_name(v);
+    case SKEL_SK_REDUCE_ROWS: return reduce_rows_variant_name(v);
   }
   return nullptr;
 }
@@ -433,6 +435,7 @@ bool variant_ok(const Call& k, int v) {
     case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_OVERLAP2D: return overlap2d_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_SEPARABLE: return separable_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_REDUCE_ROWS: return reduce_rows_variant_ok(v, k.in0, k.rows, k.cols);
   }
   return false;
 }
@@ -447,6 +450,7 @@ const int* preference(int sk, int dtype, int* count) {
   static const int col_p[] = {2, 0};
   static const int o2_p[] = {1, 0};
   static const int sep_p[] = {4, 1, 0};
+  static const int rows_p[] = {1, 0};
   switch (sk) {
     case SKEL_SK_MAP: *count = 3; return map_p;
     case SKEL_SK_REDUCE:
@@ -458,6 +462,7 @@ const int* preference(int sk, int dtype, int* count) {
     case SKEL_SK_OVERLAP1D_COL: *count = 2; return col_p;
     case SKEL_SK_OVERLAP2D: *count = 2; return o2_p;
     case SKEL_SK_SEPARABLE: *count = 3; return sep_p;
+    case SKEL_SK_REDUCE_ROWS: *count = 2; return rows_p;
   }
   *count = 0;
   return nullptr;
@@ -521,6 +526,8 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
   Launch L{c->stream, c->sms, &c->launches};
   const skel_instance& i = k.inst;
   switch (i.skeleton) {
+    case SKEL_SK_REDUCE_ROWS:
+      return launch_reduce_rows(L, v, i.dtype, i.fn, k.in0, k.rows, k.cols, k.out);
     case SKEL_SK_SEPARABLE:
       if (v == 0) return launch_separable_two_pass(c, k);
       return launch_separable_fused(L, v, k.w1, k.w1b, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
@@ -1040,6 +1047,37 @@ skel_status skel_mapreduce_to(skel_ctx* c, skel_fn map_f, skel_fn red_op, double
   return mapreduce_impl(c, false, map_f, red_op, cval, in0, in1, nullptr, out, out_index);
 }
 
+skel_status skel_reduce_rows(skel_ctx* c, skel_fn op, const skel_matrix* in, skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  if (!red_op_ok(op)) return fail(c, SKEL_ERR_UNSUPPORTED, "reduce operator must be ADD, MULT or MAX");
+  if (out->st->dtype != in->st->dtype) return fail(c, SKEL_ERR_DTYPE, "result element type differs");
+  if (out->st->n != in->rows) return fail(c, SKEL_ERR_SIZE_MISMATCH, "result vector must have one element per row");
+  if (out->st == in->st) return fail(c, SKEL_ERR_ALIAS, "result vector aliases the input");
+  if (in->rows > 0 && in->cols == 0) return fail(c, SKEL_ERR_EMPTY, "reduce of empty rows");
+  Call k;
+  k.inst.skeleton = SKEL_SK_REDUCE_ROWS;
+  k.inst.fn = op;
+  k.inst.dtype = in->st->dtype;
+  k.rows = in->rows;
+  k.cols = in->cols;
+  OperandSet set;
+  set.add(in->st, ACC_READ);
+  set.add(out->st, ACC_WRITE);
+  skel_status st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = in->st->dev;
+  k.out = out->st->dev;
+  k.n = in->st->n;
+  k.in_st = in->st;
+  k.out_st = out->st;
+  if (in->rows > 0) {
+    st = run_call(c, k);
+    if (st != SKEL_OK) return st;
+  }
+  return publish_all(c, set);
+}
+
 // ---- MapOverlap -----------------------------------------------------------------------------------
 skel_status skel_mapoverlap_1d(skel_ctx* c, const float* w, int r, skel_edge edge, double pad, const skel_vector* in,
                                skel_vector* out) {
@@ -1229,6 +1267,7 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   if (sk < 0 || sk >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
   if (log2_lo < 0 || log2_hi > 32 || log2_lo > log2_hi || reps < 1) return fail(c, SKEL_ERR_INVALID_ARG, "bad tuning range");
   const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || sk == SKEL_SK_SEPARABLE ||
+                      sk == SKEL_SK_REDUCE_ROWS ||
                       (sk == SKEL_SK_OVERLAP1D && cols > 0);
   if (matrix && cols == 0) return fail(c, SKEL_ERR_INVALID_ARG, "matrix skeletons need cols");
   skel_status st = ensure_device(c);

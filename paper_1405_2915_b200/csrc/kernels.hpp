@@ -40,6 +40,13 @@ cudaError_t launch_mapreduce(const Launch& L, const Scratch& S, int v, int dtype
                              int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n,
                              void* result /* device, one element */);
 
+// ---- row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] (reduce.cu) ----------------
+int reduce_rows_variant_count();
+const char* reduce_rows_variant_name(int v);
+bool reduce_rows_variant_ok(int v, const void* in, size_t rows, size_t cols);
+cudaError_t launch_reduce_rows(const Launch& L, int v, int dtype, int op, const void* in, size_t rows, size_t cols,
+                               void* out /* device, rows elements */);
+
 // ---- Scan ------------------------------------------------------------------------------------
 int scan_variant_count();
 const char* scan_variant_name(int v);

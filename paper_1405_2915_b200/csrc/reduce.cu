@@ -168,7 +168,114 @@ cudaError_t launch_t(const Launch& L, const Scratch& S, const RedVariant& rv, in
   return cudaErrorInvalidValue;
 }
 
+// ---- row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] --------
+// "warp_*": one warp per row (8 rows per block): a lane folds its V-wide vectors into 4 x V independent chains
+// (4 vectors in flight), then a fixed shuffle tree; "block_v4": 256 threads per row (long rows, few of them).
+// The combination order depends only on (cols, variant): deterministic run to run.
+template <typename T, int OP, int V>
+__device__ __forceinline__ T fold_row_part(const T* row, size_t cols, int t, int nt) {
+  // thread t of nt cooperating threads folds the vectors t, t + nt, t + 2 nt, ... of the row
+  constexpr int U = 4;
+  T acc[U][V];
+#pragma unroll
+  for (int u = 0; u < U; ++u)
+#pragma unroll
+    for (int j = 0; j < V; ++j) acc[u][j] = identity<T, OP>();
+  const size_t nvec = cols / V;
+  size_t i = t;
+  for (; i + size_t(U - 1) * nt < nvec; i += size_t(U) * nt) {
+    uint32_t raw[U][V];
+#pragma unroll
+    for (int u = 0; u < U; ++u) ld_stream<V, true>(raw[u], row + (i + size_t(u) * nt) * V);
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+#pragma unroll
+      for (int j = 0; j < V; ++j) acc[u][j] = apply_fn<OP>(T(0), acc[u][j], from_bits<T>(raw[u][j]));
+  }
+  for (; i < nvec; i += nt) {
+    uint32_t raw[V];
+    ld_stream<V, true>(raw, row + i * V);
+#pragma unroll
+    for (int j = 0; j < V; ++j) acc[0][j] = apply_fn<OP>(T(0), acc[0][j], from_bits<T>(raw[j]));
+  }
+  for (size_t c = nvec * V + t; c < cols; c += nt) acc[1][0] = apply_fn<OP>(T(0), acc[1][0], row[c]);  // V > 1: ragged tail
+  T v = identity<T, OP>();
+#pragma unroll
+  for (int u = 0; u < U; ++u)
+#pragma unroll
+    for (int j = 0; j < V; ++j) v = apply_fn<OP>(T(0), v, acc[u][j]);
+  return v;
+}
+
+template <typename T, int OP, int V>
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_rows_warp_kernel(const T* in, size_t rows, size_t cols, T* out) {
+  const int lane = threadIdx.x & 31;
+  const size_t warps_per_grid = size_t(gridDim.x) * (RED_THREADS / 32);
+  for (size_t row = size_t(blockIdx.x) * (RED_THREADS / 32) + (threadIdx.x >> 5); row < rows; row += warps_per_grid) {
+    T v = fold_row_part<T, OP, V>(in + row * cols, cols, lane, 32);
+    v = warp_reduce<T, OP>(v);
+    if (lane == 0) out[row] = v;
+  }
+}
+
+template <typename T, int OP, int V>
+__global__ void __launch_bounds__(RED_THREADS)
+reduce_rows_block_kernel(const T* in, size_t rows, size_t cols, T* out) {
+  __shared__ T smem[32];
+  for (size_t row = blockIdx.x; row < rows; row += gridDim.x) {
+    T v = fold_row_part<T, OP, V>(in + row * cols, cols, threadIdx.x, RED_THREADS);
+    v = block_reduce<T, OP>(v, smem);
+    if (threadIdx.x == 0) out[row] = v;
+    __syncthreads();  // smem is reused by the next row
+  }
+}
+
+const char* const kRowNames[] = {"warp_scalar", "warp_v4", "block_v4"};
+constexpr int kNumRowVariants = 3;
+
+template <typename T, int OP>
+cudaError_t launch_rows_op(const Launch& L, int v, const T* in, size_t rows, size_t cols, T* out) {
+  const size_t cap = size_t(L.sms) * 16;
+  if (v == 2) {
+    const unsigned grid = (unsigned)(rows < cap ? rows : cap);
+    reduce_rows_block_kernel<T, OP, 4><<<grid, RED_THREADS, 0, L.stream>>>(in, rows, cols, out);
+  } else {
+    const size_t blocks = (rows + RED_THREADS / 32 - 1) / (RED_THREADS / 32);
+    const unsigned grid = (unsigned)(blocks < cap ? blocks : cap);
+    if (v == 1) reduce_rows_warp_kernel<T, OP, 4><<<grid, RED_THREADS, 0, L.stream>>>(in, rows, cols, out);
+    else reduce_rows_warp_kernel<T, OP, 1><<<grid, RED_THREADS, 0, L.stream>>>(in, rows, cols, out);
+  }
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_rows_t(const Launch& L, int v, int op, const T* in, size_t rows, size_t cols, T* out) {
+  switch (op) {
+    case FN_ADD: return launch_rows_op<T, FN_ADD>(L, v, in, rows, cols, out);
+    case FN_MULT: return launch_rows_op<T, FN_MULT>(L, v, in, rows, cols, out);
+    case FN_MAX: return launch_rows_op<T, FN_MAX>(L, v, in, rows, cols, out);
+  }
+  return cudaErrorInvalidValue;
+}
+
 }  // namespace
+
+int reduce_rows_variant_count() { return kNumRowVariants; }
+const char* reduce_rows_variant_name(int v) { return (v >= 0 && v < kNumRowVariants) ? kRowNames[v] : nullptr; }
+bool reduce_rows_variant_ok(int v, const void* in, size_t, size_t cols) {
+  if (v < 0 || v >= kNumRowVariants) return false;
+  if (v == 0) return true;
+  return aligned_to(in, 16) && cols % 4 == 0;  // every row starts on a 16-byte boundary
+}
+cudaError_t launch_reduce_rows(const Launch& L, int v, int dtype, int op, const void* in, size_t rows, size_t cols,
+                               void* out) {
+  if (rows == 0) return cudaSuccess;
+  if (dtype == DT_F32)
+    return launch_rows_t<float>(L, v, op, static_cast<const float*>(in), rows, cols, static_cast<float*>(out));
+  return launch_rows_t<int32_t>(L, v, op, static_cast<const int32_t*>(in), rows, cols, static_cast<int32_t*>(out));
+}
 
 int reduce_variant_count() { return kNumRedVariants; }
 const char* reduce_variant_name(int v) { return (v >= 0 && v < kNumRedVariants) ? kRedVariants[v].name : nullptr; }
