@@ -63,6 +63,8 @@ def _lib() -> C.CDLL:
         vp, sz, dbl, i = C.c_void_p, C.c_size_t, C.c_double, C.c_int
         L.oracle_map_f32.argtypes = [i, dbl, _f32p, vp, sz, _f64p]
         L.oracle_map_i32.argtypes = [i, C.c_int32, _i32p, vp, sz, _i32p]
+        L.oracle_map3_f32.argtypes = [_f32p, _f32p, _f32p, sz, _f64p]
+        L.oracle_map3_i32.argtypes = [_i32p, _i32p, _i32p, sz, _i32p]
         L.oracle_reduce_f32.argtypes = [i, _f32p, sz, C.POINTER(dbl), C.POINTER(dbl)]
         L.oracle_reduce_i32.argtypes = [i, _i32p, sz, C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
         L.oracle_reduce_rows_f32.argtypes = [i, _f32p, sz, sz, _f64p, _f64p]
@@ -104,6 +106,21 @@ def map_i32(fn: int, c: int, in0, in1=None) -> np.ndarray:
     in1 = None if in1 is None else _c(in1, np.int32)
     out = np.empty(in0.size, np.int32)
     _lib().oracle_map_i32(fn, int(c), in0, _opt(in1), in0.size, out)
+    return out
+
+
+def map3_muladd_f32(in0, in1, in2) -> np.ndarray:
+    """Three-vector Map, MULADD: in0 * in1 + in2 in fp64."""
+    a, b, c = _c(in0, np.float32), _c(in1, np.float32), _c(in2, np.float32)
+    out = np.empty(a.size, np.float64)
+    _lib().oracle_map3_f32(a, b, c, a.size, out)
+    return out
+
+
+def map3_muladd_i32(in0, in1, in2) -> np.ndarray:
+    a, b, c = _c(in0, np.int32), _c(in1, np.int32), _c(in2, np.int32)
+    out = np.empty(a.size, np.int32)
+    _lib().oracle_map3_i32(a, b, c, a.size, out)
     return out
 
 

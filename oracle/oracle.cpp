@@ -170,6 +170,19 @@ void oracle_map_f32(int fn, double c, const float* in0, const float* in1, size_t
   }
 }
 
+// ---- three-vector Map: MULADD out[i] = in0[i] * in1[i] + in2[i]; fp64 (the product of two
+// fp32 values is exact in fp64), int32 wraps.
+void oracle_map3_f32(const float* in0, const float* in1, const float* in2, size_t n, double* out) {
+  const ptrdiff_t N = static_cast<ptrdiff_t>(n);
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < N; ++i)
+    out[i] = static_cast<double>(in0[i]) * static_cast<double>(in1[i]) + static_cast<double>(in2[i]);
+}
+
+void oracle_map3_i32(const int32_t* in0, const int32_t* in1, const int32_t* in2, size_t n, int32_t* out) {
+  for (size_t i = 0; i < n; ++i) out[i] = i32(u32(in0[i]) * u32(in1[i]) + u32(in2[i]));
+}
+
 void oracle_map_i32(int fn, int32_t c, const int32_t* in0, const int32_t* in1, size_t n, int32_t* out) {
   for (size_t i = 0; i < n; ++i) out[i] = i_apply(fn, c, in0[i], in1 ? in1[i] : c);
 }

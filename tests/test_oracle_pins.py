@@ -103,6 +103,30 @@ def test_map_i32_wraps():
     assert O.map_i32(O.FN_ADD, 7, a).tolist() == [wrap32(int(x) + 7) for x in a]
 
 
+def test_map3_muladd_exact_against_rationals_and_python_ints():
+    """Three-vector Map (MULADD): the fp64 result must be the correctly rounded exact value a*b + c (the product of
+    two fp32 numbers is exact in fp64, so one rounding happens), checked with Python's exact rationals; closed
+    forms; exact cancellation; int32 wraps like Python integers modulo 2^32. Swapping operands is caught (b != c)."""
+    from fractions import Fraction
+    n = 300
+    a, b, c = I.uniform_pm1_f32(81, n), I.uniform_pm1_f32(82, n), I.uniform_pm1_f32(83, n)
+    got = O.map3_muladd_f32(a, b, c)
+    for i in range(n):
+        exact = Fraction(float(a[i])) * Fraction(float(b[i])) + Fraction(float(c[i]))
+        assert got[i] == float(exact), i          # float(Fraction) rounds to nearest even
+    i32s = np.arange(1000, dtype=np.float32)
+    assert np.array_equal(O.map3_muladd_f32(i32s, np.full(1000, 2, np.float32), np.ones(1000, np.float32)), 2.0 * np.arange(1000) + 1)
+    p = (a.astype(np.float64) * b.astype(np.float64))
+    exact_prod = p.astype(np.float32).astype(np.float64) == p   # products that happen to be fp32 numbers
+    cc = (-p).astype(np.float32)
+    assert np.all(O.map3_muladd_f32(a, b, cc)[exact_prod] == 0.0)
+    x = (I.raw_u64(84, 64) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+    y = (I.raw_u64(85, 64) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+    z = (I.raw_u64(86, 64) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+    assert O.map3_muladd_i32(x, y, z).tolist() == [wrap32(int(p) * int(q) + int(r)) for p, q, r in zip(x, y, z)]
+    assert O.map3_muladd_f32(a[:0], b[:0], c[:0]).size == 0
+
+
 # ------------------------------------------------------------------ Reduce
 def test_reduce_closed_forms():
     g = golden()
