@@ -498,7 +498,7 @@ def main():
                      "two_calls_us": round(two, 2), "speedup_over_two_calls": round(two / us, 3)}
 
     # ---- row-wise Reduce on the 8192^2 matrix (reported, not part of `value`)
-    reduce_rows = None
+    reduce_rows = map3 = None
     if rank == 0 and not args.no_pipeline:
         import torch
         m = sz["side"] * sz["side"]
@@ -518,6 +518,22 @@ def main():
         got = rr.numpy()
         ref = d["X"].astype(np.float64).sum(axis=1)
         assert np.all(np.abs(got - ref) <= 1e-5 * np.abs(d["X"]).astype(np.float64).sum(axis=1)), "reduce_rows mismatch"
+        # three-vector Map (MULADD) on the step's vectors: 16 B/elem
+        n26 = sz["n26"]
+        call3 = lambda: ctx.map3(S.FN_MULADD, wl.vx, wl.vy, wl.vs, wl.vr)  # noqa: E731
+        for _ in range(3):
+            call3()
+        t3 = []
+        for _ in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            call3()
+            e1.record()
+            e1.synchronize()
+            t3.append(e0.elapsed_time(e1) * 1e3)
+        us3 = float(np.median(t3))
+        map3 = {"us": round(us3, 2), "variant": S.variant_names(S.SK_MAP)[ctx.last_variant()[1]], "bytes_per_elem": 16,
+                "GB/s": round(16 * n26 / us3 / 1e3, 1), "frac_measured_hbm": round(16 * n26 / us3 / 1e3 / peak, 4)}
         reduce_rows = {"us": round(us, 2), "variant": S.variant_names(S.SK_REDUCE_ROWS)[ctx.last_variant()[1]],
                        "bytes_per_elem": 4, "GB/s": round(4 * m / us / 1e3, 1), "frac_measured_hbm": round(4 * m / us / 1e3 / peak, 4)}
         rr.destroy()
@@ -605,7 +621,7 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows,
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3,
                 "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)

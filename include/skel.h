@@ -59,7 +59,10 @@ typedef enum { SKEL_F32 = 0, SKEL_I32 = 1 } skel_dtype;
  * Reduce / Scan operator, MapReduce reduce operator: ADD, MULT, MAX only.
  * WSTENCIL is the user function of MapOverlap (weights passed with the call); it is accepted
  * nowhere else. */
-typedef enum { SKEL_FN_ADD = 0, SKEL_FN_MULT = 1, SKEL_FN_MAX = 2, SKEL_FN_SAXPY = 3, SKEL_FN_WSTENCIL = 4 } skel_fn;
+typedef enum {
+  SKEL_FN_ADD = 0, SKEL_FN_MULT = 1, SKEL_FN_MAX = 2, SKEL_FN_SAXPY = 3, SKEL_FN_WSTENCIL = 4,
+  SKEL_FN_MULADD = 5  /* three-vector Map only (skel_map3): in0 * in1 + in2 */
+} skel_fn;
 
 /* edge policy of MapOverlap: out-of-range neighbours read `pad` (CONSTANT), the nearest in-range
  * element, each index clamped independently (DUPLICATE), or wrap around, each index taken modulo
@@ -171,6 +174,10 @@ skel_status skel_matrix_as_vector(skel_matrix* m, skel_vector** view);
 /* Map: out[i] = f(in0[i], b_i), b_i = in1[i], or the constant c when in1 == NULL.
  * SAXPY: out[i] = c*in0[i] + in1[i] (in1 required). out may alias in0 and/or in1 (in place). */
 skel_status skel_map(skel_ctx* ctx, skel_fn f, double c, const skel_vector* in0, const skel_vector* in1, skel_vector* out);
+/* Three-vector Map. f must be SKEL_FN_MULADD: out[i] = in0[i] * in1[i] + in2[i] (f32: one fused
+ * multiply-add, <= 1 ulp of the fp64 value rounded to f32; i32 wraps modulo 2^32). out may alias any input. */
+skel_status skel_map3(skel_ctx* ctx, skel_fn f, const skel_vector* in0, const skel_vector* in1, const skel_vector* in2,
+                      skel_vector* out);
 
 /* Reduce: in[0] (+) ... (+) in[n-1], (+) in {ADD, MULT, MAX}; i32 ADD/MULT wrap mod 2^32.
  * skel_reduce writes one element of the element type to HOST memory `host_result` and blocks.

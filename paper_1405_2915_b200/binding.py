@@ -29,7 +29,7 @@ OK, ERR_INVALID_ARG, ERR_SIZE_MISMATCH, ERR_DTYPE, ERR_UNSUPPORTED, ERR_EMPTY, E
 STATUS_NAMES = ["OK", "INVALID_ARG", "SIZE_MISMATCH", "DTYPE", "UNSUPPORTED", "EMPTY", "ALIAS", "UNINIT", "OOM",
                 "CUDA", "BUSY", "IO"]
 F32, I32 = 0, 1
-FN_ADD, FN_MULT, FN_MAX, FN_SAXPY, FN_WSTENCIL = 0, 1, 2, 3, 4
+FN_ADD, FN_MULT, FN_MAX, FN_SAXPY, FN_WSTENCIL, FN_MULADD = 0, 1, 2, 3, 4, 5
 EDGE_CONSTANT, EDGE_DUPLICATE, EDGE_CYCLIC = 0, 1, 2
 SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
 AXIS_ROW, AXIS_COL = 0, 1
@@ -91,6 +91,7 @@ _SIGS = {
     "skel_reduce_to": ([_vp, _i, _vp, _vp, _sz], _i),
     "skel_mapreduce": ([_vp, _i, _i, _d, _vp, _vp, _vp], _i),
     "skel_mapreduce_to": ([_vp, _i, _i, _d, _vp, _vp, _vp, _sz], _i),
+    "skel_map3": ([_vp, _i, _vp, _vp, _vp, _vp], _i),
     "skel_reduce_rows": ([_vp, _i, _vp, _vp], _i),
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
@@ -265,6 +266,9 @@ class Context:
     # ---- skeletons (same names and argument order as the C entry points)
     def map(self, f: int, c: float, in0: "Vector", in1: "Vector | None", out: "Vector"):
         self.check(lib.skel_map(self.h, f, c, in0.h, in1.h if in1 is not None else None, out.h))
+
+    def map3(self, f: int, in0: "Vector", in1: "Vector", in2: "Vector", out: "Vector"):
+        self.check(lib.skel_map3(self.h, f, in0.h, in1.h, in2.h, out.h))
 
     def reduce(self, op: int, x: "Vector"):
         res = (C.c_float if x.dtype == F32 else C.c_int32)()

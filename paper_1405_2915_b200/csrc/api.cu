@@ -375,6 +375,7 @@ struct Call {
   skel_instance inst{};
   const void* in0 = nullptr;
   const void* in1 = nullptr;
+  const void* in2 = nullptr;  // three-vector Map
   void* out = nullptr;
   size_t n = 0, rows = 1, cols = 0;
   uint32_t cbits = 0;  // constant c / scan init, as the element type's bits
@@ -427,7 +428,8 @@ const char* variant_name(int sk, int v) {
 
 bool variant_ok(const Call& k, int v) {
   switch (k.inst.skeleton) {
-    case SKEL_SK_MAP: return map_variant_ok(v, k.in0, k.in1, k.out, k.n);
+    case SKEL_SK_MAP:
+      return map_variant_ok(v, k.in0, k.in1, k.out, k.n) && (k.in2 == nullptr || map_variant_ok(v, k.in2, nullptr, k.out, k.n));
     case SKEL_SK_REDUCE:
     case SKEL_SK_MAPREDUCE: return reduce_variant_ok(v, k.in0, k.in1, k.n);
     case SKEL_SK_SCAN: return scan_variant_ok(v, k.inst.dtype, k.in0, k.out, k.n);
@@ -533,6 +535,7 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
       return launch_separable_fused(L, v, k.w1, k.w1b, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
                                     static_cast<float*>(k.out), k.rows, k.cols);
     case SKEL_SK_MAP:
+      if (i.fn == SKEL_FN_MULADD) return launch_map3(L, v, i.dtype, k.in0, k.in1, k.in2, k.out, k.n);
       return launch_map(L, v, i.dtype, i.fn, i.mode != 0, k.cbits, k.in0, k.in1, k.out, k.n);
     case SKEL_SK_REDUCE:
       return launch_mapreduce(L, c->scratch, v, i.dtype, FN_IDENT_, false, i.fn, 0, k.in0, nullptr, k.n, k.out);
@@ -1024,6 +1027,40 @@ skel_status skel_map(skel_ctx* c, skel_fn f, double cval, const skel_vector* in0
   return publish_all(c, set);
 }
 
+skel_status skel_map3(skel_ctx* c, skel_fn f, const skel_vector* in0, const skel_vector* in1, const skel_vector* in2,
+                      skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in0) || !vec_ok(in1) || !vec_ok(in2) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad vector handle");
+  if (f != SKEL_FN_MULADD) return fail(c, SKEL_ERR_UNSUPPORTED, "the three-vector map function must be MULADD");
+  Storage *a = in0->st, *b = in1->st, *d = in2->st, *o = out->st;
+  if (b->dtype != a->dtype || d->dtype != a->dtype || o->dtype != a->dtype) return fail(c, SKEL_ERR_DTYPE, "operand element types differ");
+  if (b->n != a->n || d->n != a->n || o->n != a->n) return fail(c, SKEL_ERR_SIZE_MISMATCH, "operand sizes differ");
+  Call k;
+  k.inst.skeleton = SKEL_SK_MAP;
+  k.inst.fn = f;
+  k.inst.dtype = a->dtype;
+  k.inst.mode = 2;  // three vectors
+  OperandSet set;
+  set.add(a, ACC_READ);
+  set.add(b, ACC_READ);
+  set.add(d, ACC_READ);
+  set.add(o, ACC_WRITE);
+  skel_status st = acquire_all(c, set);
+  if (st != SKEL_OK) return st;
+  k.in0 = a->dev;
+  k.in1 = b->dev;
+  k.in2 = d->dev;
+  k.out = o->dev;
+  k.n = a->n;
+  k.in_st = a;
+  k.out_st = o;
+  if (k.n > 0) {
+    st = run_call(c, k);
+    if (st != SKEL_OK) return st;
+  }
+  return publish_all(c, set);
+}
+
 // ---- Reduce / MapReduce ---------------------------------------------------------------------------
 skel_status skel_reduce(skel_ctx* c, skel_fn op, const skel_vector* in, void* host_result) {
   if (ctx_ok(c) && !host_result) return fail(c, SKEL_ERR_INVALID_ARG, "host_result is NULL");
@@ -1326,6 +1363,7 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
     }
     k.in0 = b0;
     k.in1 = (sk == SKEL_SK_MAP || sk == SKEL_SK_MAPREDUCE) && inst->mode ? b1 : nullptr;
+    k.in2 = (sk == SKEL_SK_MAP && inst->fn == SKEL_FN_MULADD) ? b0 : nullptr;
     k.out = (sk == SKEL_SK_REDUCE || sk == SKEL_SK_MAPREDUCE) ? c->d_result : b2;
     for (int i = 0; i < 129; ++i) k.w1.w[i] = k.w1b.w[i] = 1.0f / 129.0f;
     for (int i = 0; i < 17 * 17; ++i) k.w2.w[i] = 1.0f / 289.0f;

@@ -32,6 +32,10 @@ bool map_variant_ok(int v, const void* in0, const void* in1, const void* out, si
 cudaError_t launch_map(const Launch& L, int v, int dtype, int fn, bool has_in1, uint32_t cbits,
                        const void* in0, const void* in1, void* out, size_t n);
 
+// three-vector Map, MULADD: out[i] = in0[i] * in1[i] + in2[i] (same variant table; alignment of all four pointers)
+cudaError_t launch_map3(const Launch& L, int v, int dtype, const void* in0, const void* in1, const void* in2, void* out,
+                        size_t n);
+
 // ---- Reduce / MapReduce (map_fn = FN_IDENT for plain Reduce) --------------------------------------
 int reduce_variant_count();
 const char* reduce_variant_name(int v);

@@ -54,6 +54,44 @@ map_kernel(const T* in0, const T* in1, T* out, T c, size_t n) {
   }
 }
 
+// Three-vector Map, MULADD: out[i] = in0[i] * in1[i] + in2[i] (f32: ONE fused multiply-add, like
+// saxpy; i32 wraps). 16 B/elem; same tile layout, U2 = 2 vectors per operand in flight (three operands).
+template <typename T, int V, int U, bool NC>
+__global__ void __launch_bounds__(MAP_THREADS)
+map3_kernel(const T* in0, const T* in1, const T* in2, T* out, size_t n) {
+  constexpr size_t TILE = size_t(MAP_THREADS) * V * U;
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t base = tile * TILE + size_t(threadIdx.x) * V;
+    if (base + (U - 1) * size_t(MAP_THREADS) * V + V <= n) {
+      uint32_t a[U][V], b[U][V], c[U][V];
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        ld_stream<V, NC>(a[u], in0 + base + size_t(u) * MAP_THREADS * V);
+        ld_stream<V, NC>(b[u], in1 + base + size_t(u) * MAP_THREADS * V);
+        ld_stream<V, NC>(c[u], in2 + base + size_t(u) * MAP_THREADS * V);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+#pragma unroll
+        for (int j = 0; j < V; ++j)  // saxpy's arithmetic with a per-element factor: c' * a + b with c' = in0, a = in1, b = in2
+          a[u][j] = to_bits(apply_fn<FN_SAXPY>(from_bits<T>(a[u][j]), from_bits<T>(b[u][j]), from_bits<T>(c[u][j])));
+        st_stream<V>(out + base + size_t(u) * MAP_THREADS * V, a[u]);
+      }
+    } else {
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const size_t i0 = base + size_t(u) * MAP_THREADS * V;
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          const size_t i = i0 + j;
+          if (i < n) out[i] = apply_fn<FN_SAXPY>(in0[i], in1[i], in2[i]);
+        }
+      }
+    }
+  }
+}
+
 struct MapVariant { const char* name; int v, u; bool persist; };
 const MapVariant kMapVariants[] = {
     {"scalar_u4_tiles", 1, 4, false},   // any alignment
@@ -107,7 +145,40 @@ cudaError_t launch_t(const Launch& L, const MapVariant& mv, int fn, bool has_in1
   return cudaErrorInvalidValue;
 }
 
+template <typename T, int V, int U>
+cudaError_t launch_map3_one(const Launch& L, bool persist, bool nc, const T* in0, const T* in1, const T* in2, T* out, size_t n) {
+  constexpr size_t TILE = size_t(MAP_THREADS) * V * U;
+  size_t ntiles = (n + TILE - 1) / TILE;
+  size_t grid = persist ? (size_t)L.sms * 8 : ntiles;
+  if (grid > ntiles) grid = ntiles;
+  if (grid > 0x7fffffffu) grid = 0x7fffffffu;
+  if (nc) map3_kernel<T, V, U, true><<<(unsigned)grid, MAP_THREADS, 0, L.stream>>>(in0, in1, in2, out, n);
+  else map3_kernel<T, V, U, false><<<(unsigned)grid, MAP_THREADS, 0, L.stream>>>(in0, in1, in2, out, n);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_map3_t(const Launch& L, const MapVariant& mv, const T* in0, const T* in1, const T* in2, T* out, size_t n) {
+  const void* o = out;
+  const bool nc = in0 != o && in1 != o && in2 != o;
+  if (mv.v == 1) return launch_map3_one<T, 1, 4>(L, mv.persist, nc, in0, in1, in2, out, n);
+  if (mv.v == 4) return launch_map3_one<T, 4, 2>(L, mv.persist, nc, in0, in1, in2, out, n);
+  return launch_map3_one<T, 8, 2>(L, mv.persist, nc, in0, in1, in2, out, n);
+}
+
 }  // namespace
+
+cudaError_t launch_map3(const Launch& L, int v, int dtype, const void* in0, const void* in1, const void* in2, void* out,
+                        size_t n) {
+  if (n == 0) return cudaSuccess;
+  const MapVariant& mv = kMapVariants[v];
+  if (dtype == DT_F32)
+    return launch_map3_t<float>(L, mv, static_cast<const float*>(in0), static_cast<const float*>(in1),
+                                static_cast<const float*>(in2), static_cast<float*>(out), n);
+  return launch_map3_t<int32_t>(L, mv, static_cast<const int32_t*>(in0), static_cast<const int32_t*>(in1),
+                                static_cast<const int32_t*>(in2), static_cast<int32_t*>(out), n);
+}
 
 int map_variant_count() { return kNumMapVariants; }
 const char* map_variant_name(int v) { return (v >= 0 && v < kNumMapVariants) ? kMapVariants[v].name : nullptr; }

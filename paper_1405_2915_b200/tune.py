@@ -22,6 +22,7 @@ def instances(S):
     out = []
     out.append(("map_saxpy_f32", I(skeleton=S.SK_MAP, fn=S.FN_SAXPY, dtype=S.F32, mode=1), 12, 26, 0))
     out.append(("map_mult_const_f32", I(skeleton=S.SK_MAP, fn=S.FN_MULT, dtype=S.F32, mode=0), 12, 26, 0))
+    out.append(("map3_muladd_f32", I(skeleton=S.SK_MAP, fn=S.FN_MULADD, dtype=S.F32, mode=2), 12, 26, 0))
     out.append(("reduce_add_i32", I(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.I32), 12, 26, 0))
     out.append(("reduce_max_i32", I(skeleton=S.SK_REDUCE, fn=S.FN_MAX, dtype=S.I32), 12, 26, 0))
     out.append(("reduce_add_f32", I(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.F32), 12, 26, 0))

@@ -557,3 +557,42 @@ def test_overlap2d_cyclic_constant_input_has_no_border(ctx, v):
         assert np.all(got == got[0, 0])  # every output saw the same 25 values in the same order
         mx.destroy()
         mo.destroy()
+
+
+# ------------------------------------------------------------------ three-vector Map
+@pytest.mark.parametrize("v", variants(S.SK_MAP))
+def test_map3_muladd(ctx, v):
+    with forced(ctx, S.SK_MAP, v):
+        for n in SIZES_SHORT + [4096, 65536 + 3]:
+            a, b, c = I.uniform_pm1_f32(900 + n, n), I.uniform_pm1_f32(901 + n, n), I.uniform_pm1_f32(902 + n, n)
+            va, vb, vc, vo = ctx.vector_from(a), ctx.vector_from(b), ctx.vector_from(c), ctx.vector(n)
+            ctx.map3(S.FN_MULADD, va, vb, vc, vo)
+            assert ctx.last_variant() == (S.SK_MAP, v)
+            assert_map_f32(vo.numpy(), O.map3_muladd_f32(a, b, c))
+            ctx.map3(S.FN_MULADD, va, vb, vc, vc)      # in place on the addend
+            assert_map_f32(vc.numpy(), O.map3_muladd_f32(a, b, c))
+            x = (I.raw_u64(903 + n, n) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+            y = (I.raw_u64(904 + n, n) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+            z = (I.raw_u64(905 + n, n) % np.uint64(1 << 32)).astype(np.uint32).view(np.int32)
+            vx, vy, vz, vi = ctx.vector_from(x), ctx.vector_from(y), ctx.vector_from(z), ctx.vector(n, S.I32)
+            ctx.map3(S.FN_MULADD, vx, vy, vz, vi)
+            assert np.array_equal(vi.numpy(), O.map3_muladd_i32(x, y, z))
+            for h in (va, vb, vc, vo, vx, vy, vz, vi):
+                h.destroy()
+
+
+def test_map3_cancellation_needs_fma_and_errors(ctx):
+    n = 50000
+    a, b = I.uniform_pm1_f32(910, n), I.uniform_pm1_f32(911, n)
+    c = (-(a.astype(np.float64) * b.astype(np.float64))).astype(np.float32)   # a*b + c ~ the product's rounding error
+    va, vb, vc, vo = ctx.vector_from(a), ctx.vector_from(b), ctx.vector_from(c), ctx.vector(n)
+    ctx.map3(S.FN_MULADD, va, vb, vc, vo)
+    assert_map_f32(vo.numpy(), O.map3_muladd_f32(a, b, c))   # a separate multiply and add would return 0 everywhere
+    assert np.count_nonzero(vo.numpy()) > n // 2
+    with pytest.raises(S.SkelError):
+        ctx.map3(S.FN_ADD, va, vb, vc, vo)
+    short = ctx.vector(n - 1)
+    with pytest.raises(S.SkelError):
+        ctx.map3(S.FN_MULADD, va, vb, short, vo)
+    for h in (va, vb, vc, vo, short):
+        h.destroy()
