@@ -129,7 +129,7 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
       advance(ptile, pty, ptx);
     }
     // ---- phase B: column pass from T (a (2R+1) x 1 filter on a tile without x halo) ----
-    compute_tile2<R, 0, OY, Weights1D, false>(T, Wcol, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
+    compute_tile2<R, 0, OY, Weights1D, true>(T, Wcol, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
     __syncthreads();  // T is rewritten by the next tile's phase A
     advance(tile, tyi, txi);
     if constexpr (STAGES == 2) {
