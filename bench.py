@@ -538,6 +538,39 @@ def main():
                        "bytes_per_elem": 4, "GB/s": round(4 * m / us / 1e3, 1), "frac_measured_hbm": round(4 * m / us / 1e3 / peak, 4)}
         rr.destroy()
 
+    # ---- range-granular host access (PAPER.md L123 partial copies): the host updates 1 MiB of a
+    # 256 MiB vector between two Reduce calls; with a range access only that MiB is uploaded, with the whole-container
+    # protocol (READWRITE access to the container) the device copy is invalidated and 256 MiB go up again
+    range_update = None
+    if rank == 0 and not args.no_pipeline:
+        nr = 1 << 18
+        patch = np.full(nr, 0.5, np.float32)
+
+        def upd(ranged):
+            ctx.reset_stats()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for it in range(5):
+                if ranged:
+                    wl.vs.write_range(4096 * (it + 1), patch)
+                else:
+                    hv = wl.vs.host_view(S.READWRITE)
+                    hv[4096 * (it + 1):4096 * (it + 1) + nr] = patch
+                    wl.vs.release()
+                ctx.reduce(S.FN_ADD, wl.vs)
+            dt = (time.perf_counter() - t0) / 5
+            return dt, ctx.stats()
+
+        ctx.reduce(S.FN_ADD, wl.vs)
+        wl.vs.numpy()  # host copy valid too (SHARED): both protocols start from the same state
+        upd(True)
+        t_r, st_r = upd(True)
+        t_w, st_w = upd(False)
+        range_update = {"range_bytes": 4 * nr, "container_bytes": 4 * sz["n26"],
+                        "range_access": {"ms_per_update_and_reduce": round(t_r * 1e3, 3), "h2d_bytes_per_update": st_r["h2d_bytes"] // 5},
+                        "whole_container_access": {"ms_per_update_and_reduce": round(t_w * 1e3, 3), "h2d_bytes_per_update": st_w["h2d_bytes"] // 5},
+                        "speedup": round(t_w / t_r, 1)}
+
     # ---- container-layer overhead ("< 1 %") and the dot-product size sweep
     # (SURVEY.md 8(d) cfg 1): reported, not part of `value`
     container_layer = dot_sweep = None
@@ -621,7 +654,7 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3,
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3, "range_update": range_update,
                 "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)

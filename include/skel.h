@@ -149,6 +149,17 @@ skel_status skel_vector_size(const skel_vector* v, size_t* n);
  * Skeleton calls on a container whose host access is held -> SKEL_ERR_BUSY. */
 skel_status skel_vector_host_acquire(skel_vector* v, skel_access mode, void** host_ptr);
 skel_status skel_vector_host_release(skel_vector* v);
+/* Range-granular host access (single-GPU half; partial copies, "multiple data
+ * transfers ... when accessing a given range of elements"). *host_ptr points at element `offset` of the library's
+ * pinned host copy and is valid for `count` elements until skel_vector_host_release.
+ *   READ:      if the host copy is not valid only this range is downloaded; the container's state does not change
+ *              (a later whole-container host access still downloads everything).
+ *   WRITE / READWRITE: the range becomes newer on the host than on the device. If the device copy is valid it STAYS
+ *              valid: the next skeleton call that reads the container uploads just the written ranges (ranges merge;
+ *              a whole-container device write discards them), instead of the whole container as after
+ *              skel_vector_host_acquire(WRITE).
+ * The container must have been written before (UNINIT -> SKEL_ERR_UNINIT); offset + count <= n; count > 0. */
+skel_status skel_vector_host_acquire_range(skel_vector* v, skel_access mode, size_t offset, size_t count, void** host_ptr);
 /* Device pointer of the current device copy for inspection/interop (NULL if none); *valid = 1
  * if the device copy is valid. No transfer, no state change. */
 skel_status skel_vector_device_ptr(const skel_vector* v, void** dptr, int* valid);
@@ -163,6 +174,8 @@ skel_status skel_matrix_destroy(skel_matrix* m);
 skel_status skel_matrix_shape(const skel_matrix* m, size_t* rows, size_t* cols);
 skel_status skel_matrix_host_acquire(skel_matrix* m, skel_access mode, void** host_ptr);
 skel_status skel_matrix_host_release(skel_matrix* m);
+/* the same for whole rows row0 .. row0 + nrows - 1 of a matrix */
+skel_status skel_matrix_host_acquire_rows(skel_matrix* m, skel_access mode, size_t row0, size_t nrows, void** host_ptr);
 /* A flattened alias (rows*cols elements) sharing storage and coherence state with the matrix;
  * destroy it like any vector (the storage lives until the last handle is destroyed). */
 skel_status skel_matrix_as_vector(skel_matrix* m, skel_vector** view);
@@ -283,6 +296,10 @@ skel_status skel_get_stats(skel_ctx* ctx, skel_stats* out);
  * second (x 2 = FLOP/s). The roofline of the arithmetic-bound MapOverlap instances. */
 skel_status skel_probe_fma_peak(skel_ctx* ctx, int reps, double* fma_per_s);
 skel_status skel_reset_stats(skel_ctx* ctx);
+
+/* The range list of the range-granular host access as a pure function (no GPU needed): merges [begin, end) into
+ * the sorted list of `*count` disjoint ranges stored as pairs ranges[2k], ranges[2k+1] (capacity in pairs). */
+skel_status skel_ranges_add(uint64_t* ranges, size_t* count, size_t capacity, uint64_t begin, uint64_t end);
 
 /* The coherence protocol as a pure function (used by the library itself
  * and exposed so that it can be tested without a GPU).

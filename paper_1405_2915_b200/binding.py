@@ -75,6 +75,9 @@ _SIGS = {
     "skel_vector_destroy": ([_vp], _i),
     "skel_vector_size": ([_vp, C.POINTER(_sz)], _i),
     "skel_vector_host_acquire": ([_vp, _i, _pp], _i),
+    "skel_vector_host_acquire_range": ([_vp, _i, _sz, _sz, _pp], _i),
+    "skel_matrix_host_acquire_rows": ([_vp, _i, _sz, _sz, _pp], _i),
+    "skel_ranges_add": ([C.POINTER(C.c_uint64), C.POINTER(C.c_size_t), _sz, C.c_uint64, C.c_uint64], _i),
     "skel_vector_host_release": ([_vp], _i),
     "skel_vector_device_ptr": ([_vp, _pp, C.POINTER(_i)], _i),
     "skel_vector_state": ([_vp, C.POINTER(_i)], _i),
@@ -365,6 +368,29 @@ class _Container:
     def release(self):
         self.ctx.check(self._release(self.h))
 
+    def _range_view(self, fn, mode: int, a: int, b: int, count: int, shape) -> np.ndarray:
+        p = C.c_void_p()
+        self.ctx.check(fn(self.h, mode, a, b, C.byref(p)))
+        buf = (C.c_byte * (count * 4)).from_address(p.value)
+        return np.frombuffer(buf, dtype=_NP[self.dtype]).reshape(shape)
+
+    def read_range(self, offset: int, count: int) -> np.ndarray:
+        """Copy of elements offset .. offset+count-1 (flattened index); downloads only that range if needed."""
+        v = self.host_view_range(READ, offset, count)
+        try:
+            return v.copy()
+        finally:
+            self.release()
+
+    def write_range(self, offset: int, arr: np.ndarray):
+        """Overwrite elements from `offset` on; a valid device copy stays valid and gets just this range uploaded."""
+        a = np.ascontiguousarray(arr, _NP[self.dtype]).reshape(-1)
+        v = self.host_view_range(WRITE, offset, a.size)
+        try:
+            v[...] = a
+        finally:
+            self.release()
+
     def numpy(self) -> np.ndarray:
         """Copy of the contents (downloads if only the device copy is valid)."""
         v = self.host_view(READ)
@@ -387,6 +413,17 @@ class _Container:
             self._keep = None
 
 
+def ranges_add(ranges: list[tuple[int, int]], begin: int, end: int) -> list[tuple[int, int]]:
+    """The library's range-list merge as a pure function (no GPU)."""
+    cap = len(ranges) + 1
+    buf = (C.c_uint64 * (2 * cap))(*[x for r in ranges for x in r])
+    cnt = C.c_size_t(len(ranges))
+    st = lib.skel_ranges_add(buf, C.byref(cnt), cap, begin, end)
+    if st != OK:
+        raise SkelError(st)
+    return [(int(buf[2 * k]), int(buf[2 * k + 1])) for k in range(cnt.value)]
+
+
 class Vector(_Container):
     _acquire = staticmethod(lib.skel_vector_host_acquire)
     _release = staticmethod(lib.skel_vector_host_release)
@@ -399,6 +436,10 @@ class Vector(_Container):
         s = C.c_int()
         self.ctx.check(lib.skel_vector_state(self.h, C.byref(s)))
         return s.value
+
+    def host_view_range(self, mode: int, offset: int, count: int) -> np.ndarray:
+        """Range-granular host access (skel_vector_host_acquire_range). Call release()."""
+        return self._range_view(lib.skel_vector_host_acquire_range, mode, offset, count, count, (count,))
 
     def device_ptr(self):
         p, valid = C.c_void_p(), C.c_int()
@@ -413,6 +454,13 @@ class Matrix(_Container):
 
     def __init__(self, ctx, h, dtype, rows, cols):
         super().__init__(ctx, h, dtype, (rows, cols))
+
+    def host_view_range(self, mode: int, offset: int, count: int) -> np.ndarray:
+        """Whole rows only: offset and count must be multiples of cols."""
+        cols = self.shape[1]
+        assert offset % cols == 0 and count % cols == 0
+        return self._range_view(lib.skel_matrix_host_acquire_rows, mode, offset // cols, count // cols, count,
+                                (count // cols, cols))
 
     def as_vector(self) -> Vector:
         h = C.c_void_p()

@@ -36,6 +36,9 @@ struct Storage {
   bool host_held = false;
   int refs = 1;
   uint64_t last_seq = 0;  // ctx->seq of the last enqueued device operation that touched it
+  // range-granular coherence: element ranges whose HOST copy is newer than the (otherwise valid) device copy.
+  // Non-empty only while the device-valid bit of `state` is set.
+  std::vector<ElemRange> host_newer;
 };
 
 struct Handle {
@@ -183,6 +186,32 @@ skel_status ensure_host(skel_ctx* c, Storage* s) {
   return SKEL_OK;
 }
 
+skel_status flush_pending(skel_ctx* c);
+
+// upload the ranges the host has written since the device copy was last made current (device copy stays valid)
+skel_status upload_host_newer(skel_ctx* c, Storage* s) {
+  if (s->host_newer.empty()) return SKEL_OK;
+  skel_status st = flush_pending(c);  // keep the stream order
+  if (st != SKEL_OK) return st;
+  const size_t es = esize(s->dtype);
+  for (const ElemRange& r : s->host_newer) {
+    const size_t bytes = size_t(r.end - r.begin) * es;
+    CU(c, cudaMemcpyAsync(static_cast<char*>(s->dev) + r.begin * es, static_cast<char*>(s->host) + r.begin * es, bytes,
+                          cudaMemcpyHostToDevice, c->stream));
+    c->stats.h2d_bytes += bytes;
+    c->stats.h2d_count += 1;
+  }
+  s->host_newer.clear();
+  s->last_seq = ++c->seq;
+  return SKEL_OK;
+}
+
+void add_host_newer(Storage* s, size_t begin, size_t end) {
+  s->host_newer.resize(s->host_newer.size() + 1);
+  const size_t cnt = ranges_add(s->host_newer.data(), s->host_newer.size() - 1, begin, end);
+  s->host_newer.resize(cnt);
+}
+
 // wait until every enqueued device operation that touched `s` has finished
 skel_status wait_for(skel_ctx* c, Storage* s) {
   if (s->last_seq > c->synced_seq) {
@@ -267,6 +296,17 @@ skel_status host_acquire(Handle* h, skel_access mode, void** host_ptr) {
   if (!step.ok) return fail(c, SKEL_ERR_UNINIT, "host read of a container that was never written");
   skel_status st = flush_pending(c);
   if (st != SKEL_OK) return st;
+  if (!s->host_newer.empty()) {
+    // ranges written through a host range access: a whole-container read of a host copy that is otherwise invalid
+    // must not lose them (make the device current first, then download); an access that leaves the host copy the
+    // only valid one makes the list moot; a read of a fully valid host copy keeps it.
+    if (step.transfer & XFER_D2H) {
+      st = upload_host_newer(c, s);
+      if (st != SKEL_OK) return st;
+    } else if (!(step.new_state & 2)) {
+      s->host_newer.clear();
+    }
+  }
   if (s->n > 0) {
     st = ensure_device(c);
     if (st != SKEL_OK) return st;
@@ -291,6 +331,46 @@ skel_status host_release(Handle* h) {
   Storage* s = h->st;
   if (!s->host_held) return fail(s->ctx, SKEL_ERR_INVALID_ARG, "host access is not held");
   s->host_held = false;
+  return SKEL_OK;
+}
+
+// Range-granular host access (include/skel.h skel_vector_host_acquire_range).
+skel_status host_acquire_range(Handle* h, skel_access mode, size_t offset, size_t count, void** host_ptr) {
+  Storage* s = h->st;
+  skel_ctx* c = s->ctx;
+  if (!host_ptr) return fail(c, SKEL_ERR_INVALID_ARG, "host_ptr is NULL");
+  if (mode != SKEL_READ && mode != SKEL_WRITE && mode != SKEL_READWRITE) return fail(c, SKEL_ERR_INVALID_ARG, "bad access mode");
+  if (count == 0 || offset > s->n || count > s->n - offset) return fail(c, SKEL_ERR_INVALID_ARG, "range out of bounds");
+  if (s->host_held) return fail(c, SKEL_ERR_BUSY, "host access already held");
+  if (s->state == ST_UNINIT) return fail(c, SKEL_ERR_UNINIT, "range access to a container that was never written");
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = ensure_host(c, s);
+  if (st != SKEL_OK) return st;
+  const size_t es = esize(s->dtype);
+  const bool host_valid = s->state & 1, dev_valid = s->state & 2;
+  if (!host_valid && mode != SKEL_WRITE) {
+    // only this range comes down; parts of it the host has written since are newer than the device's: make the
+    // device current first if they overlap
+    for (const ElemRange& r : s->host_newer)
+      if (r.begin < offset + count && offset < r.end) {
+        st = upload_host_newer(c, s);
+        if (st != SKEL_OK) return st;
+        break;
+      }
+    CU(c, cudaMemcpyAsync(static_cast<char*>(s->host) + offset * es, static_cast<char*>(s->dev) + offset * es, count * es,
+                          cudaMemcpyDeviceToHost, c->stream));
+    c->stats.d2h_bytes += count * es;
+    c->stats.d2h_count += 1;
+    s->last_seq = ++c->seq;
+  }
+  st = wait_for(c, s);  // also orders a host write after device reads of the host buffer that are still in flight
+  if (st != SKEL_OK) return st;
+  if (mode != SKEL_READ && dev_valid) add_host_newer(s, offset, offset + count);
+  s->host_held = true;
+  *host_ptr = static_cast<char*>(s->host) + offset * es;
   return SKEL_OK;
 }
 
@@ -330,6 +410,13 @@ skel_status acquire_all(skel_ctx* c, OperandSet& set) {
     if (!s->dev && s->n > 0) {
       st = dev_alloc(c, s->n * esize(s->dtype), &s->dev);
       if (st != SKEL_OK) return st;
+    }
+    if (!s->host_newer.empty()) {
+      if (o.access == ACC_WRITE || (o.step.transfer & XFER_H2D)) s->host_newer.clear();  // overwritten / uploaded whole
+      else {
+        st = upload_host_newer(c, s);  // the device copy is valid except for these ranges
+        if (st != SKEL_OK) return st;
+      }
     }
     if ((o.step.transfer & XFER_H2D) && s->n > 0) {
       st = flush_pending(c);  // keep the stream order: held-back launches go first
@@ -906,6 +993,11 @@ skel_status skel_vector_host_acquire(skel_vector* v, skel_access mode, void** ho
   return host_acquire(v, mode, host_ptr);
 }
 
+skel_status skel_vector_host_acquire_range(skel_vector* v, skel_access mode, size_t offset, size_t count, void** host_ptr) {
+  if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
+  return host_acquire_range(v, mode, offset, count, host_ptr);
+}
+
 skel_status skel_vector_host_release(skel_vector* v) {
   if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
   return host_release(v);
@@ -914,6 +1006,7 @@ skel_status skel_vector_host_release(skel_vector* v) {
 skel_status skel_vector_device_ptr(const skel_vector* v, void** dptr, int* valid) {
   if (!vec_ok(v) || !dptr) return SKEL_ERR_INVALID_ARG;
   flush_pending(v->st->ctx);  // the caller is about to use the stream / the pointer (a fused in-place Map swaps buffers)
+  upload_host_newer(v->st->ctx, v->st);
   *dptr = v->st->dev;
   if (valid) *valid = (v->st->state & 2) ? 1 : 0;
   return SKEL_OK;
@@ -969,6 +1062,12 @@ skel_status skel_matrix_shape(const skel_matrix* m, size_t* rows, size_t* cols) 
 skel_status skel_matrix_host_acquire(skel_matrix* m, skel_access mode, void** host_ptr) {
   if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
   return host_acquire(m, mode, host_ptr);
+}
+
+skel_status skel_matrix_host_acquire_rows(skel_matrix* m, skel_access mode, size_t row0, size_t nrows, void** host_ptr) {
+  if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
+  if (row0 > m->rows || nrows > m->rows - row0) return fail(m->st->ctx, SKEL_ERR_INVALID_ARG, "row range out of bounds");
+  return host_acquire_range(m, mode, row0 * m->cols, nrows * m->cols, host_ptr);
 }
 
 skel_status skel_matrix_host_release(skel_matrix* m) {
@@ -1503,6 +1602,13 @@ skel_status skel_probe_fma_peak(skel_ctx* c, int reps, double* fma_per_s) {
 skel_status skel_reset_stats(skel_ctx* c) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
   c->stats = skel_stats{};
+  return SKEL_OK;
+}
+
+skel_status skel_ranges_add(uint64_t* ranges, size_t* count, size_t capacity, uint64_t begin, uint64_t end) {
+  if (!ranges || !count || *count >= capacity) return SKEL_ERR_INVALID_ARG;
+  static_assert(sizeof(ElemRange) == 2 * sizeof(uint64_t), "pairs of 64-bit bounds");
+  *count = ranges_add(reinterpret_cast<ElemRange*>(ranges), *count, begin, end);
   return SKEL_OK;
 }
 

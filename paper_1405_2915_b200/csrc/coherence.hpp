@@ -4,6 +4,7 @@
 // copy; the protocol details are deferred by the paper to a thesis, so the table is DESIGN.md's
 // "Coherence" reading).
 #pragma once
+#include <stddef.h>
 
 namespace skel {
 
@@ -47,6 +48,33 @@ inline CoherenceStep coherence_step(int state, int actor, int access, int mode) 
     ns = ST_HOST;
   }
   return {true, ns, xfer};
+}
+
+// ---- range extension ("partial copies ... when accessing a given range of elements") ----------
+// A sorted list of disjoint, non-adjacent element ranges [begin, end): the parts of a container whose HOST copy is
+// newer than the device copy (written through a host range access while the device copy stayed valid). Pure data
+// structure, no CUDA: tested on the CPU through skel_ranges_add.
+struct ElemRange { unsigned long long begin, end; };
+
+// merge [begin, end) into the sorted disjoint list `r` of `count` ranges (capacity >= count + 1); returns the new count
+inline size_t ranges_add(ElemRange* r, size_t count, unsigned long long begin, unsigned long long end) {
+  if (begin >= end) return count;
+  size_t i = 0;
+  while (i < count && r[i].end < begin) ++i;          // ranges entirely before (not even adjacent)
+  size_t j = i;
+  while (j < count && r[j].begin <= end) {             // ranges that overlap or touch [begin, end)
+    if (r[j].begin < begin) begin = r[j].begin;
+    if (r[j].end > end) end = r[j].end;
+    ++j;
+  }
+  if (j == i) {                                        // nothing to merge: insert at i
+    for (size_t k = count; k > i; --k) r[k] = r[k - 1];
+    r[i] = {begin, end};
+    return count + 1;
+  }
+  r[i] = {begin, end};                                 // replace r[i..j) by the union
+  for (size_t k = j; k < count; ++k) r[i + 1 + (k - j)] = r[k];
+  return count - (j - i) + 1;
 }
 
 }  // namespace skel
