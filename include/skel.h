@@ -149,6 +149,13 @@ skel_status skel_vector_size(const skel_vector* v, size_t* n);
  * Skeleton calls on a container whose host access is held -> SKEL_ERR_BUSY. */
 skel_status skel_vector_host_acquire(skel_vector* v, skel_access mode, void** host_ptr);
 skel_status skel_vector_host_release(skel_vector* v);
+/* Start downloading the container to its host copy NOW, asynchronously, on a copy stream of the context, if only
+ * the device copy is valid (otherwise nothing happens). The download is ordered after everything enqueued so far and
+ * overlaps later skeleton calls and their uploads (PCIe is full duplex); a later host access waits for it instead of
+ * starting its own copy, a later device write to the container waits for it before it overwrites the buffer.
+ * The communication-optimisation service of PAPER.md L117, made explicit: the lazy protocol alone would start the
+ * download only at the host access. */
+skel_status skel_vector_prefetch_host(skel_vector* v);
 /* Range-granular host access (single-GPU half; partial copies, "multiple data
  * transfers ... when accessing a given range of elements"). *host_ptr points at element `offset` of the library's
  * pinned host copy and is valid for `count` elements until skel_vector_host_release.
@@ -174,6 +181,7 @@ skel_status skel_matrix_destroy(skel_matrix* m);
 skel_status skel_matrix_shape(const skel_matrix* m, size_t* rows, size_t* cols);
 skel_status skel_matrix_host_acquire(skel_matrix* m, skel_access mode, void** host_ptr);
 skel_status skel_matrix_host_release(skel_matrix* m);
+skel_status skel_matrix_prefetch_host(skel_matrix* m);
 /* the same for whole rows row0 .. row0 + nrows - 1 of a matrix */
 skel_status skel_matrix_host_acquire_rows(skel_matrix* m, skel_access mode, size_t row0, size_t nrows, void** host_ptr);
 /* A flattened alias (rows*cols elements) sharing storage and coherence state with the matrix;

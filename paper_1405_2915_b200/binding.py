@@ -75,6 +75,8 @@ _SIGS = {
     "skel_vector_destroy": ([_vp], _i),
     "skel_vector_size": ([_vp, C.POINTER(_sz)], _i),
     "skel_vector_host_acquire": ([_vp, _i, _pp], _i),
+    "skel_vector_prefetch_host": ([_vp], _i),
+    "skel_matrix_prefetch_host": ([_vp], _i),
     "skel_vector_host_acquire_range": ([_vp, _i, _sz, _sz, _pp], _i),
     "skel_matrix_host_acquire_rows": ([_vp, _i, _sz, _sz, _pp], _i),
     "skel_ranges_add": ([C.POINTER(C.c_uint64), C.POINTER(C.c_size_t), _sz, C.c_uint64, C.c_uint64], _i),
@@ -346,7 +348,7 @@ class Context:
 
 
 class _Container:
-    _acquire = _release = _destroy = None
+    _acquire = _release = _destroy = _prefetch = None
 
     def __init__(self, ctx: Context, h, dtype: int, shape):
         self.ctx, self.h, self.dtype, self.shape = ctx, h, dtype, shape
@@ -367,6 +369,10 @@ class _Container:
 
     def release(self):
         self.ctx.check(self._release(self.h))
+
+    def prefetch_host(self):
+        """Start an asynchronous download on the context's copy stream (skel_*_prefetch_host)."""
+        self.ctx.check(self._prefetch(self.h))
 
     def _range_view(self, fn, mode: int, a: int, b: int, count: int, shape) -> np.ndarray:
         p = C.c_void_p()
@@ -426,6 +432,7 @@ def ranges_add(ranges: list[tuple[int, int]], begin: int, end: int) -> list[tupl
 
 class Vector(_Container):
     _acquire = staticmethod(lib.skel_vector_host_acquire)
+    _prefetch = staticmethod(lib.skel_vector_prefetch_host)
     _release = staticmethod(lib.skel_vector_host_release)
     _destroy = staticmethod(lib.skel_vector_destroy)
 
@@ -449,6 +456,7 @@ class Vector(_Container):
 
 class Matrix(_Container):
     _acquire = staticmethod(lib.skel_matrix_host_acquire)
+    _prefetch = staticmethod(lib.skel_matrix_prefetch_host)
     _release = staticmethod(lib.skel_matrix_host_release)
     _destroy = staticmethod(lib.skel_matrix_destroy)
 

@@ -39,6 +39,9 @@ struct Storage {
   // range-granular coherence: element ranges whose HOST copy is newer than the (otherwise valid) device copy.
   // Non-empty only while the device-valid bit of `state` is set.
   std::vector<ElemRange> host_newer;
+  // skel_*_prefetch_host: a download in flight on the context's copy stream (nullptr = none). The host copy counts
+  // as valid in `state`; host accesses and device writes wait for this event first.
+  cudaEvent_t d2h_done = nullptr;
 };
 
 struct Handle {
@@ -78,6 +81,7 @@ struct skel_ctx {
   // cross-call fusion (skel_ctx_set_fusion): launches of a fusible chain are held back here
   bool fusion = false;
   std::vector<struct PendingCall> pending;
+  cudaStream_t copy_stream = nullptr;  // skel_*_prefetch_host: downloads that overlap the compute stream's work
   void* sep_tmp = nullptr;  // intermediate matrix of the two-pass separable MapOverlap
   size_t sep_tmp_bytes = 0;
   void* spare = nullptr;  // buffer an in-place Map of a fused chain writes into (then swapped with the container's)
@@ -188,6 +192,23 @@ skel_status ensure_host(skel_ctx* c, Storage* s) {
 
 skel_status flush_pending(skel_ctx* c);
 
+// a prefetch download in flight: block the host until it has landed
+skel_status finish_prefetch(skel_ctx* c, Storage* s) {
+  if (!s->d2h_done) return SKEL_OK;
+  cudaError_t e = cudaEventSynchronize(s->d2h_done);
+  cudaEventDestroy(s->d2h_done);
+  s->d2h_done = nullptr;
+  if (e != cudaSuccess) return cuda_fail(c, e, "prefetch download");
+  return SKEL_OK;
+}
+
+// ... or make the compute stream wait for it (before a kernel overwrites the device buffer it reads from)
+skel_status order_after_prefetch(skel_ctx* c, Storage* s) {
+  if (!s->d2h_done) return SKEL_OK;
+  CU(c, cudaStreamWaitEvent(c->stream, s->d2h_done, 0));
+  return SKEL_OK;
+}
+
 // upload the ranges the host has written since the device copy was last made current (device copy stays valid)
 skel_status upload_host_newer(skel_ctx* c, Storage* s) {
   if (s->host_newer.empty()) return SKEL_OK;
@@ -255,6 +276,7 @@ skel_status release_handle(Handle* h) {
   skel_ctx* c = s->ctx;
   if (s->host_held && s->refs == 1) return fail(c, SKEL_ERR_BUSY, "host access is still held");
   flush_pending(c);  // a held-back launch may still reference this container
+  if (s->refs == 1) finish_prefetch(c, s);
   if (--s->refs == 0) {
     if (s->last_seq > c->synced_seq && !c->sticky) {
       cudaStreamSynchronize(c->stream);
@@ -292,6 +314,10 @@ skel_status host_acquire(Handle* h, skel_access mode, void** host_ptr) {
   if (mode != SKEL_READ && mode != SKEL_WRITE && mode != SKEL_READWRITE)
     return fail(c, SKEL_ERR_INVALID_ARG, "bad access mode");
   if (s->host_held) return fail(c, SKEL_ERR_BUSY, "host access already held");
+  {
+    skel_status pst = finish_prefetch(c, s);
+    if (pst != SKEL_OK) return pst;
+  }
   const CoherenceStep step = coherence_step(s->state, ACTOR_HOST, mode, c->mode);
   if (!step.ok) return fail(c, SKEL_ERR_UNINIT, "host read of a container that was never written");
   skel_status st = flush_pending(c);
@@ -334,6 +360,37 @@ skel_status host_release(Handle* h) {
   return SKEL_OK;
 }
 
+// Asynchronous download on the copy stream (include/skel.h skel_vector_prefetch_host).
+skel_status prefetch_host(Handle* h) {
+  Storage* s = h->st;
+  skel_ctx* c = s->ctx;
+  if (s->host_held) return fail(c, SKEL_ERR_BUSY, "container is held by the host");
+  if (s->state != ST_DEVICE || s->n == 0) return SKEL_OK;  // nothing to do: the host copy is (becoming) valid
+  skel_status st = finish_prefetch(c, s);  // an earlier download whose result a device write has made stale since
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = ensure_host(c, s);
+  if (st != SKEL_OK) return st;
+  st = upload_host_newer(c, s);  // ranges the host wrote must not be overwritten by the download
+  if (st != SKEL_OK) return st;
+  if (!c->copy_stream) CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+  cudaEvent_t produced;
+  CU(c, cudaEventCreateWithFlags(&produced, cudaEventDisableTiming));
+  CU(c, cudaEventRecord(produced, c->stream));            // everything enqueued so far (the producing kernel)
+  CU(c, cudaStreamWaitEvent(c->copy_stream, produced, 0));
+  cudaEventDestroy(produced);                               // released once it has completed
+  CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->copy_stream));
+  CU(c, cudaEventCreateWithFlags(&s->d2h_done, cudaEventDisableTiming));
+  CU(c, cudaEventRecord(s->d2h_done, c->copy_stream));
+  c->stats.d2h_bytes += s->n * esize(s->dtype);
+  c->stats.d2h_count += 1;
+  s->state = ST_SHARED;  // valid once d2h_done has fired: every host access waits for it
+  return SKEL_OK;
+}
+
 // Range-granular host access (include/skel.h skel_vector_host_acquire_range).
 skel_status host_acquire_range(Handle* h, skel_access mode, size_t offset, size_t count, void** host_ptr) {
   Storage* s = h->st;
@@ -343,7 +400,9 @@ skel_status host_acquire_range(Handle* h, skel_access mode, size_t offset, size_
   if (count == 0 || offset > s->n || count > s->n - offset) return fail(c, SKEL_ERR_INVALID_ARG, "range out of bounds");
   if (s->host_held) return fail(c, SKEL_ERR_BUSY, "host access already held");
   if (s->state == ST_UNINIT) return fail(c, SKEL_ERR_UNINIT, "range access to a container that was never written");
-  skel_status st = flush_pending(c);
+  skel_status st = finish_prefetch(c, s);
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
   if (st != SKEL_OK) return st;
   st = ensure_device(c);
   if (st != SKEL_OK) return st;
@@ -409,6 +468,10 @@ skel_status acquire_all(skel_ctx* c, OperandSet& set) {
     Storage* s = o.st;
     if (!s->dev && s->n > 0) {
       st = dev_alloc(c, s->n * esize(s->dtype), &s->dev);
+      if (st != SKEL_OK) return st;
+    }
+    if (s->d2h_done && (o.access != ACC_READ || (o.step.transfer & XFER_H2D))) {
+      st = order_after_prefetch(c, s);  // the download still reads the device buffer this call overwrites
       if (st != SKEL_OK) return st;
     }
     if (!s->host_newer.empty()) {
@@ -903,6 +966,10 @@ skel_status skel_ctx_destroy(skel_ctx* c) {
   if (c->dev_ready) {
     flush_pending(c);
     cudaStreamSynchronize(c->stream);
+    if (c->copy_stream) {
+      cudaStreamSynchronize(c->copy_stream);
+      cudaStreamDestroy(c->copy_stream);
+    }
     if (c->spare) dev_free(c, c->spare);
     if (c->sep_tmp) dev_free(c, c->sep_tmp);
     cudaFree(c->scratch.partials);
@@ -998,6 +1065,11 @@ skel_status skel_vector_host_acquire_range(skel_vector* v, skel_access mode, siz
   return host_acquire_range(v, mode, offset, count, host_ptr);
 }
 
+skel_status skel_vector_prefetch_host(skel_vector* v) {
+  if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
+  return prefetch_host(v);
+}
+
 skel_status skel_vector_host_release(skel_vector* v) {
   if (!vec_ok(v)) return SKEL_ERR_INVALID_ARG;
   return host_release(v);
@@ -1068,6 +1140,11 @@ skel_status skel_matrix_host_acquire_rows(skel_matrix* m, skel_access mode, size
   if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
   if (row0 > m->rows || nrows > m->rows - row0) return fail(m->st->ctx, SKEL_ERR_INVALID_ARG, "row range out of bounds");
   return host_acquire_range(m, mode, row0 * m->cols, nrows * m->cols, host_ptr);
+}
+
+skel_status skel_matrix_prefetch_host(skel_matrix* m) {
+  if (!mat_ok(m)) return SKEL_ERR_INVALID_ARG;
+  return prefetch_host(m);
 }
 
 skel_status skel_matrix_host_release(skel_matrix* m) {

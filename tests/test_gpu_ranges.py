@@ -130,3 +130,38 @@ def test_random_walk_against_shadow_arrays(ctx):
             val = I.uniform_int_i32(100 + step, n, 50); a.write(val); a_sh = val.copy()
     assert np.array_equal(a.numpy(), a_sh) and np.array_equal(b.numpy(), b_sh)
     a.destroy(); b.destroy()
+
+
+def test_prefetch_host_overlaps_and_stays_coherent(ctx):
+    """skel_vector_prefetch_host: the download runs on a copy stream; host accesses wait for it, device writes are
+    ordered after it, a stale prefetch is redone."""
+    n = 1 << 22
+    x = I.uniform_int_i32(11, n, 1000)
+    v, o, p = ctx.vector_from(x), ctx.vector(n, S.I32), ctx.vector(n, S.I32)
+    ctx.map(S.FN_ADD, 1, v, None, o)
+    ctx.reset_stats()
+    o.prefetch_host()                                  # async download of x + 1
+    assert o.state() == 3 and ctx.stats()["d2h_bytes"] == 4 * n
+    ctx.map(S.FN_ADD, 2, o, None, p)                   # reads o while it downloads: no conflict
+    ctx.map(S.FN_ADD, 10, v, None, o)                  # OVERWRITES o: must wait for the download to finish reading it
+    assert o.state() == 2
+    assert np.array_equal(p.numpy(), x + 3)
+    ctx.reset_stats()
+    assert np.array_equal(o.numpy(), x + 10)           # the prefetched copy was stale: downloaded again
+    assert ctx.stats()["d2h_bytes"] == 4 * n
+    # prefetch, then a host read finds the data without a second transfer
+    ctx.map(S.FN_ADD, 20, v, None, o)
+    o.prefetch_host()
+    o.prefetch_host()                                  # idempotent
+    ctx.reset_stats()
+    assert np.array_equal(o.numpy(), x + 20)
+    assert ctx.stats()["d2h_bytes"] == 0
+    # prefetch of a container with host-written ranges keeps them
+    ctx.map(S.FN_ADD, 30, v, None, o)
+    o.write_range(5, np.full(4, -1, np.int32))
+    o.prefetch_host()
+    exp = x + 30
+    exp[5:9] = -1
+    assert np.array_equal(o.numpy(), exp)
+    for h in (v, o, p):
+        h.destroy()
