@@ -988,6 +988,7 @@ skel_status skel_ctx_sync(skel_ctx* c) {
   skel_status st = flush_pending(c);
   if (st != SKEL_OK) return st;
   CU(c, cudaStreamSynchronize(c->stream));
+  if (c->copy_stream) CU(c, cudaStreamSynchronize(c->copy_stream));  // prefetch downloads in flight
   c->synced_seq = c->seq;
   return SKEL_OK;
 }
