@@ -70,7 +70,8 @@ struct skel_ctx {
   int sms = 148;
   Scratch scratch{};
   void* d_result = nullptr;  // device slot for scalars returned to the host
-  void* h_result = nullptr;  // pinned host slot
+  void* h_result = nullptr;      // pinned, mapped host slot for scalars returned to the host ...
+  void* h_result_dev = nullptr;  // ... and its device-side address: the reducing kernel stores the scalar straight into it
   uint64_t seq = 0, synced_seq = 0;
   bool sticky = false;
   Plan plan;
@@ -130,7 +131,8 @@ skel_status ensure_device(skel_ctx* c) {
   c->scratch.scan_state = nullptr;
   c->scratch.scan_state_tiles = 0;
   c->scratch.scan_epoch = 0;
-  CU(c, cudaHostAlloc(&c->h_result, 64, cudaHostAllocDefault));
+  CU(c, cudaHostAlloc(&c->h_result, 64, cudaHostAllocMapped));
+  CU(c, cudaHostGetDevicePointer(&c->h_result_dev, c->h_result, 0));
   c->dev_ready = true;
   return SKEL_OK;
 }
@@ -852,7 +854,8 @@ skel_status const_bits(skel_ctx* c, int dtype, double v, uint32_t* bits) {
 skel_status scalar_to_host(skel_ctx* c, int dtype, void* host_result) {
   skel_status fst = flush_pending(c);
   if (fst != SKEL_OK) return fst;
-  CU(c, cudaMemcpyAsync(c->h_result, c->d_result, esize(dtype), cudaMemcpyDeviceToHost, c->stream));
+  // zero-copy: the kernel's last block wrote the scalar into the mapped host slot (no device-to-host copy to
+  // enqueue and wait for); visible to the host once the stream has drained
   CU(c, cudaStreamSynchronize(c->stream));
   c->synced_seq = c->seq;
   memcpy(host_result, c->h_result, esize(dtype));
@@ -898,7 +901,7 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   k.in0 = a->dev;
   k.in1 = b ? b->dev : nullptr;
   k.n = a->n;
-  k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->d_result;
+  k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->h_result_dev;
   k.in_st = a;
   k.out_st = out ? out->st : nullptr;
   st = run_call(c, k);
