@@ -354,6 +354,111 @@ cudaError_t launch_shfl(const Launch& L, const Weights1D& w, int edge, float pad
   return cudaGetLastError();
 }
 
+// "regshfl_2x8": the same idea with warp-contiguous accesses. A warp owns 512 consecutive elements; lane l owns the
+// two 8-element chunks A = [8l, 8l+8) and B = [256+8l, 256+8l+8) of them, so that each of the warp's two 256-bit
+// loads (and stores) covers 1024 contiguous bytes (whole 128-byte lines, like the Map kernel) instead of every other
+// 32-byte sector of 2048 bytes. Halos by shuffles with wrap-around: the right neighbour of lane 31's chunk A is lane
+// 0's chunk B, the left neighbour of lane 0's chunk B is lane 31's chunk A; only A's left halo at lane 0 and B's right
+// halo at lane 31 come from memory. r <= 8.
+template <int R>
+__global__ void __launch_bounds__(T1_THREADS)
+overlap1d_shfl2_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
+                       size_t rows, size_t cols) {
+  constexpr int C = 8, TILE = T1_THREADS * 2 * C;
+  static_assert(R >= 1 && R <= C, "halo comes from the direct neighbours only");
+  constexpr unsigned FULLM = 0xffffffffu;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const size_t tiles_per_row = (cols + TILE - 1) / TILE;
+  const size_t ntiles = rows * tiles_per_row;
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const size_t row = tile / tiles_per_row;
+    const long long wbase = static_cast<long long>((tile - row * tiles_per_row) * TILE) + warp * (64 * C);
+    const long long cA = wbase + C * lane, cB = cA + 32 * C;
+    const float* x = in + row * cols;
+    const long long lc = static_cast<long long>(cols);
+    const bool full = wbase + 64 * C <= lc;  // warp-uniform
+    float wa[C + 2 * R], wb[C + 2 * R];
+    if (full) {
+      uint32_t a[8], b[8];
+      ld_stream<8, true>(a, x + cA);
+      ld_stream<8, true>(b, x + cB);
+#pragma unroll
+      for (int j = 0; j < C; ++j) { wa[R + j] = __uint_as_float(a[j]); wb[R + j] = __uint_as_float(b[j]); }
+    } else {
+#pragma unroll
+      for (int j = 0; j < C; ++j) {
+        wa[R + j] = ext_row(x, lc, cA + j, edge, pad);
+        wb[R + j] = ext_row(x, lc, cB + j, edge, pad);
+      }
+    }
+    const int prev = (lane + 31) & 31, next = (lane + 1) & 31;
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+      const float tA = __shfl_sync(FULLM, wa[C + j], prev);  // tail of the previous lane's A (lane 0: lane 31's)
+      const float hA = __shfl_sync(FULLM, wa[R + j], next);  // head of the next lane's A
+      const float tB = __shfl_sync(FULLM, wb[C + j], prev);
+      const float hB = __shfl_sync(FULLM, wb[R + j], next);  // head of the next lane's B (lane 31: lane 0's)
+      wa[j] = tA;                                  // lane 0: replaced below
+      wa[R + C + j] = lane == 31 ? hB : hA;
+      wb[j] = lane == 0 ? tA : tB;
+      wb[R + C + j] = hB;                          // lane 31: replaced below
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) wa[j] = ext_row(x, lc, cA - R + j, edge, pad);
+    }
+    if (lane == 31) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) wb[R + C + j] = ext_row(x, lc, cB + C + j, edge, pad);
+    }
+    float accA[C], accB[C];
+#pragma unroll
+    for (int o = 0; o < C; ++o) accA[o] = accB[o] = 0.f;
+    constexpr bool PK = R >= 8;  // as in overlap1d_shfl_kernel: per output the taps accumulate in ascending k
+#pragma unroll
+    for (int k = 0; k <= 2 * R; ++k) {
+      if (PK && (k + R) % 2 == 0) {
+#pragma unroll
+        for (int o = 0; o < C; o += 2) {
+          fma2_into(accA[o], accA[o + 1], W.w[k], wa[o + k], wa[o + k + 1]);
+          fma2_into(accB[o], accB[o + 1], W.w[k], wb[o + k], wb[o + k + 1]);
+        }
+      } else {
+#pragma unroll
+        for (int o = 0; o < C; ++o) {
+          accA[o] = fmaf(W.w[k], wa[o + k], accA[o]);
+          accB[o] = fmaf(W.w[k], wb[o + k], accB[o]);
+        }
+      }
+    }
+    float* orow = out + row * cols;
+    if (full) {
+      uint32_t r0[8], r1[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { r0[e] = __float_as_uint(accA[e]); r1[e] = __float_as_uint(accB[e]); }
+      st_stream<8>(orow + cA, r0);
+      st_stream<8>(orow + cB, r1);
+    } else {
+#pragma unroll
+      for (int o = 0; o < C; ++o) {
+        if (cA + o < lc) orow[cA + o] = accA[o];
+        if (cB + o < lc) orow[cB + o] = accB[o];
+      }
+    }
+  }
+}
+
+template <int R>
+cudaError_t launch_shfl2(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
+                         size_t rows, size_t cols) {
+  constexpr int TILE = T1_THREADS * 16;
+  const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
+  const size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
+  overlap1d_shfl2_kernel<R><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
 template <int O> constexpr size_t tiled_smem_bytes(int R) {
   const int HP = (R + 3) / 4 * 4;
   const int span = T1_THREADS * O + 2 * HP;
@@ -362,7 +467,8 @@ template <int O> constexpr size_t tiled_smem_bytes(int R) {
 
 struct O1Variant { const char* name; int o; };  // o == 0: direct
 const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16},
-                               {"tiled_o8_db", 108}, {"tiled_o16_db", 116}, {"tiled_o16_db_ffma2", 216}};
+                               {"tiled_o8_db", 108}, {"tiled_o16_db", 116}, {"tiled_o16_db_ffma2", 216},
+                               {"regshfl_2x8", -8}};
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
@@ -445,6 +551,7 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
   if (v < 0 || v >= kNumVariants) return false;
   if (kVariants[v].o == 0) return true;
   if (!templated_radius(r)) return false;
+  if (kVariants[v].o == -8 && r > 8) return false;
   const bool al = reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
   return al && (rows == 1 || cols % 8 == 0);
 }
@@ -468,6 +575,15 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 108: return launch_tiled_db_r<8, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 116: return launch_tiled_db_r<16, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 216: return launch_tiled_db_r<16, true>(L, w, r, edge, pad, in, out, rows, cols);
+    case -8:
+      switch (r) {
+        case 1: return launch_shfl2<1>(L, w, edge, pad, in, out, rows, cols);
+        case 2: return launch_shfl2<2>(L, w, edge, pad, in, out, rows, cols);
+        case 3: return launch_shfl2<3>(L, w, edge, pad, in, out, rows, cols);
+        case 4: return launch_shfl2<4>(L, w, edge, pad, in, out, rows, cols);
+        case 8: return launch_shfl2<8>(L, w, edge, pad, in, out, rows, cols);
+      }
+      return cudaErrorInvalidValue;
     case -16:
       switch (r) {
         case 1: return launch_shfl<1>(L, w, edge, pad, in, out, rows, cols);

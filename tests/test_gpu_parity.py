@@ -26,6 +26,15 @@ def variants(sk):
     return list(range(S.lib.skel_variant_count(sk)))
 
 
+def o1_radius_ok(v, r):
+    """Radii a MapOverlap 1D variant is instantiated for (direct: any; regshfl_2x8: r <= 8)."""
+    if v == 0:
+        return True
+    if S.variant_names(S.SK_OVERLAP1D)[v] == "regshfl_2x8":
+        return r in (1, 2, 3, 4, 8)
+    return r in (1, 2, 3, 4, 8, 16)
+
+
 class forced:
     def __init__(self, ctx, sk, v):
         self.ctx, self.sk, self.v = ctx, sk, v
@@ -332,9 +341,8 @@ O1_SIZES = [1, 2, 3, 5, 16, 17, 33, 100, 1023, 4096, 4097, 8200, 16385, 65537, 3
 @pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
 @pytest.mark.parametrize("r", [0, 1, 2, 3, 4, 5, 8, 16, 17, 64])
 def test_overlap1d_vector(ctx, v, r):
-    tiled = v != 0
-    if tiled and r not in (1, 2, 3, 4, 8, 16):
-        pytest.skip("tiled variants are instantiated for r in {1,2,3,4,8,16}")
+    if not o1_radius_ok(v, r):
+        pytest.skip("tiled variants are instantiated for r in {1,2,3,4,8,16} (regshfl_2x8: r <= 8)")
     w = I.positive_weights_f32(500 + r, 2 * r + 1)
     ws = I.signed_weights_f32(501 + r, 2 * r + 1)
     with forced(ctx, S.SK_OVERLAP1D, v):
@@ -357,6 +365,8 @@ def test_overlap1d_vector(ctx, v, r):
 def test_overlap1d_one_hot_weights_shift_bit_exact(ctx, v):
     with forced(ctx, S.SK_OVERLAP1D, v):
         for r in (1, 4, 16):
+            if not o1_radius_ok(v, r):
+                continue
             for n in (3, 50, 4099, 8193):
                 x = I.uniform_pm1_f32(510 + n, n)
                 vx, vo = ctx.vector_from(x), ctx.vector(n)
@@ -379,6 +389,8 @@ def test_overlap1d_constant_input_and_impulse(ctx):
     for v in variants(S.SK_OVERLAP1D):
         with forced(ctx, S.SK_OVERLAP1D, v):
             for r in (1, 4, 16):
+                if not o1_radius_ok(v, r):
+                    continue
                 n = 20000
                 w = I.positive_weights_f32(520 + r, 2 * r + 1)
                 vx, vo = ctx.vector_from(np.full(n, 3.0, np.float32)), ctx.vector(n)
@@ -410,7 +422,7 @@ def test_overlap1d_matrix_rows(ctx, v, r):
     for rows, cols in MAT_SHAPES:
         X = I.uniform01_f32(531 + rows, rows * cols).reshape(rows, cols)
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
-        tiled_ok = r in (1, 2, 3, 4, 8, 16) and (rows == 1 or cols % 8 == 0)
+        tiled_ok = o1_radius_ok(v, r) and (rows == 1 or cols % 8 == 0)
         with forced(ctx, S.SK_OVERLAP1D, v):
             for edge, pad in EDGE_CASES:
                 if v != 0 and not tiled_ok:
