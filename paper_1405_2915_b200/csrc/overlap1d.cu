@@ -12,6 +12,7 @@
 //    constant bank, taps are fully unrolled (r is a template parameter: 1,2,3,4,8,16).
 //    The tile is padded by 4 floats every O floats so that the 128-bit reads of a quarter warp
 //    fall into distinct banks.
+#include <cuda.h>
 #include "common.cuh"
 #include "kernels.hpp"
 
@@ -110,17 +111,35 @@ __device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x
 // PK: the FMAs (x[p] -> out o) and (x[p+1] -> out o+1) with p, o even share the tap and are ONE FFMA2
 // on two aligned register pairs; the other half of the FMAs stays scalar. Emission order keeps, for
 // every output, its taps in ascending order, so the result is bit-identical to the scalar form.
-template <int R, int O, bool PK = false>
+// SWZ >= 0: the tile is a TMA window of 128-byte rows in the 128-byte swizzle (16-byte chunk c of row q sits at
+// chunk c ^ (q & 7)); the thread's first group is chunk threadIdx.x * O / 4 + SWZ of the window. With u = t + a
+// (a = (SWZ + g) / 4, b = (SWZ + g) % 4; O = 16) the group's byte address is ((u >> 1) * 128 | (((u & 1) * 4) ^
+// ((u >> 1) & 7)) * 16) ^ (b * 16): one XOR per group on top of five integer instructions per a.
+template <int R, int O, bool PK = false, int SWZ = -1>
 __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& W, float* orow, long long cols, long long c0) {
   constexpr int HP = (R + 3) / 4 * 4;
   constexpr int NG = (O + 2 * HP) / 4;  // 128-bit groups a thread reads
+  static_assert(SWZ < 0 || O == 16, "the swizzled window form is written for 16 outputs per thread");
   float acc[O];
 #pragma unroll
   for (int o = 0; o < O; ++o) acc[o] = 0.f;
   const int sc0 = threadIdx.x * O;
+  unsigned swz_a[SWZ >= 0 ? (SWZ + NG + 3) / 4 : 1];
+  if constexpr (SWZ >= 0) {
+#pragma unroll
+    for (int a = 0; a < (SWZ + NG + 3) / 4; ++a) {
+      const unsigned u = threadIdx.x + a, q = u >> 1;
+      swz_a[a] = (q << 7) | ((((u & 1u) << 2) ^ (q & 7u)) << 4);
+    }
+  }
 #pragma unroll
   for (int g = 0; g < NG; ++g) {
-    const float4 v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
+    float4 v4;
+    if constexpr (SWZ >= 0)
+      v4 = *reinterpret_cast<const float4*>(reinterpret_cast<const unsigned char*>(sm) +
+                                            (swz_a[(SWZ + g) / 4] ^ (unsigned((SWZ + g) % 4) << 4)));
+    else
+      v4 = *reinterpret_cast<const float4*>(sm + phys<O>(sc0 + 4 * g));
     const float v[4] = {v4.x, v4.y, v4.z, v4.w};
     // tile coordinate (relative to sc0) p = 4g+e holds x~[out0 - HP + p]; output o uses it with
     // tap k = p - HP - o + R, 0 <= k <= 2R
@@ -262,6 +281,100 @@ overlap1d_tiled_db_kernel(const __grid_constant__ Weights1D W, int edge, float p
     __syncthreads();
     tile = ntile; row = nrow; tcol = ntcol;
     advance(ntile, nrow, ntcol);
+  }
+}
+
+// ---- TMA-fed persistent form on a vector ("tma_swz_o16_s*") --------------------------------------
+// The vector is viewed as a matrix of 128-byte rows (32 floats); one cp.async.bulk.tensor.2d per tile
+// copies the TILE/32 + 2 rows around the tile (one whole row of halo on each side) into a stage in the
+// 128-byte swizzle, which makes the 128-bit shared loads of threads 64 bytes apart conflict-free without
+// padding. Completion is a `full` mbarrier per stage, reuse an `empty` one (one arrival per warp): no
+// block barrier on the interior path and no staging instructions in the compute warps. Rows outside
+// the vector arrive as zeros (CONSTANT-0); cells below 0, at or beyond floor(n / 32) * 32 (the ragged
+// last row, which the tensor map cannot describe) or beyond n are patched in shared memory.
+constexpr int T1W_TILE = T1_THREADS * 16;
+constexpr int T1W_ROWS = T1W_TILE / 32 + 2;
+constexpr unsigned T1W_STAGE_BYTES = T1W_ROWS * 128u;
+constexpr unsigned T1W_STAGE_STRIDE = (T1W_STAGE_BYTES + 1023u) / 1024u * 1024u;
+
+__device__ __forceinline__ void tma_load_rows(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar))
+      : "memory");
+}
+
+template <int R, bool PK, int STAGES>
+__global__ void __launch_bounds__(T1_THREADS)
+overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
+                     const float* in, float* out, long long n, long long nfull, int ntiles) {
+  constexpr int HP = (R + 3) / 4 * 4;
+  constexpr int SWZ = (32 - HP) / 4;
+  extern __shared__ unsigned char smraw0[];
+  unsigned char* smraw = smraw0 + ((1024u - (smem_u32(smraw0) & 1023u)) & 1023u);  // the swizzle is a function of address bits 4..9
+  uint64_t* full = reinterpret_cast<uint64_t*>(smraw + STAGES * T1W_STAGE_STRIDE);
+  uint64_t* empty = full + STAGES;
+  auto stage_ptr = [&](int s) { return reinterpret_cast<float*>(smraw + s * T1W_STAGE_STRIDE); };
+  const int lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full + s, 1);
+      mbar_init(empty + s, T1_THREADS / 32);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+  int tile = blockIdx.x;
+  if (tile >= ntiles) return;
+  int ptile = tile;  // producer state (thread 0)
+  auto request = [&](int s) {
+    mbar_arrive_expect_tx(full + s, T1W_STAGE_BYTES);
+    tma_load_rows(stage_ptr(s), &tmap, 0, ptile * (T1W_TILE / 32) - 1, full + s);
+  };
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int d = 0; d < STAGES - 1; ++d) {
+      if (ptile < ntiles) request(d);
+      ptile += gridDim.x;
+    }
+  }
+  const bool zeros_ok = edge == EDGE_CONSTANT && pad == 0.f;  // what the copy delivers outside the vector
+  int s = 0, ph = 0;
+  int tgt = STAGES - 1, tph = 1;
+  for (int it = 0; tile < ntiles; ++it) {
+    if (threadIdx.x == 0) {
+      if (ptile < ntiles) {
+        if (it > 0) mbar_wait(empty + tgt, tph);
+        request(tgt);
+      }
+      ptile += gridDim.x;
+    }
+    tgt = tgt + 1 == STAGES ? 0 : tgt + 1;
+    if (tgt == 0) tph ^= 1;
+    mbar_wait(full + s, ph);
+    const long long c0 = static_cast<long long>(tile) * T1W_TILE;
+    float* sm = stage_ptr(s);
+    const long long w0 = c0 - 32, w1 = c0 + T1W_TILE + 32;  // the window [w0, w1)
+    const bool patch = (w0 < 0 && !zeros_ok) || (w1 > nfull && (nfull != n || !zeros_ok));  // block-uniform
+    if (patch) {
+      for (int idx = threadIdx.x; idx < T1W_ROWS * 32; idx += T1_THREADS) {
+        const long long gi = w0 + idx;
+        if (gi < 0 || gi >= nfull) {
+          const unsigned q = unsigned(idx) >> 5, c = (unsigned(idx) >> 2) & 7u;
+          sm[q * 32 + ((c ^ (q & 7u)) << 2) + (idx & 3)] = ext_row(in, n, gi, edge, pad);
+        }
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next TMA refill
+      __syncthreads();
+    }
+    compute_tile1<R, 16, PK, SWZ>(sm, W, out, n, c0);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty + s);
+    tile += gridDim.x;
+    s = s + 1 == STAGES ? 0 : s + 1;
+    if (s == 0) ph ^= 1;
   }
 }
 
@@ -468,7 +581,7 @@ template <int O> constexpr size_t tiled_smem_bytes(int R) {
 struct O1Variant { const char* name; int o; };  // o == 0: direct
 const O1Variant kVariants[] = {{"direct", 0}, {"tiled_o4", 4}, {"tiled_o8", 8}, {"tiled_o16", 16}, {"regshfl_o16", -16},
                                {"tiled_o8_db", 108}, {"tiled_o16_db", 116}, {"tiled_o16_db_ffma2", 216},
-                               {"regshfl_2x8", -8}};
+                               {"regshfl_2x8", -8}, {"tma_swz_o16_s2", 302}, {"tma_swz_o16_s3", 303}};
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 inline bool templated_radius(int r) { return r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16; }
@@ -514,6 +627,80 @@ cudaError_t launch_tiled_db(const Launch& L, const Weights1D& w, int edge, float
   return cudaGetLastError();
 }
 
+// Tensor map of a vector seen as floor(n / 32) rows of 32 floats, box = 32 x T1W_ROWS, 128-byte swizzle (host side;
+// the driver entry point is looked up through the runtime, libcuda is not linked). The last map is cached.
+inline cudaError_t make_tmap_rows(CUtensorMap* out, const float* base, size_t nrows) {
+  using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static EncodeFn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+    encode = reinterpret_cast<EncodeFn>(fn);
+  }
+  static thread_local const float* last_base = nullptr;
+  static thread_local size_t last_rows = 0;
+  static thread_local CUtensorMap last_map;
+  if (last_base == base && last_rows == nrows) {
+    *out = last_map;
+    return cudaSuccess;
+  }
+  const cuuint64_t dims[2] = {32, nrows};
+  const cuuint64_t strides[1] = {128};
+  const cuuint32_t box[2] = {32, cuuint32_t(T1W_ROWS)};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  last_base = base;
+  last_rows = nrows;
+  last_map = *out;
+  return cudaSuccess;
+}
+
+// vectors shorter than one tile (and anything the tensor map cannot describe) take the cp.async form
+template <int R, int STAGES>
+cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out, size_t n) {
+  if (n < size_t(T1W_TILE) || n / T1W_TILE >= (size_t(1) << 30)) return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, 1, n);
+  constexpr size_t smem = size_t(STAGES) * T1W_STAGE_STRIDE + 2 * STAGES * sizeof(uint64_t) + 1024;
+  auto kern = overlap1d_tma_kernel<R, true, STAGES>;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T1_THREADS, smem) != cudaSuccess || per_sm < 1)
+      return cudaErrorInvalidValue;
+  }
+  CUtensorMap tmap;
+  cudaError_t e = make_tmap_rows(&tmap, in, n / 32);
+  if (e != cudaSuccess) return e;
+  const size_t ntiles = (n + T1W_TILE - 1) / T1W_TILE;
+  size_t grid = size_t(L.sms) * per_sm;
+  if (grid > ntiles) grid = ntiles;
+  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, tmap, edge, pad, in, out, (long long)n, (long long)(n / 32 * 32),
+                                                        (int)ntiles);
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+template <int STAGES>
+cudaError_t launch_tma1_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in, float* out,
+                          size_t n) {
+  switch (r) {
+    case 1: return launch_tma1<1, STAGES>(L, w, edge, pad, in, out, n);
+    case 2: return launch_tma1<2, STAGES>(L, w, edge, pad, in, out, n);
+    case 3: return launch_tma1<3, STAGES>(L, w, edge, pad, in, out, n);
+    case 4: return launch_tma1<4, STAGES>(L, w, edge, pad, in, out, n);
+    case 8: return launch_tma1<8, STAGES>(L, w, edge, pad, in, out, n);
+    case 16: return launch_tma1<16, STAGES>(L, w, edge, pad, in, out, n);
+  }
+  return cudaErrorInvalidValue;
+}
+
 template <int O, bool PK>
 cudaError_t launch_tiled_db_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in,
                               float* out, size_t rows, size_t cols) {
@@ -552,6 +739,7 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
   if (kVariants[v].o == 0) return true;
   if (!templated_radius(r)) return false;
   if (kVariants[v].o == -8 && r > 8) return false;
+  if (kVariants[v].o >= 300 && rows != 1) return false;  // vectors only
   const bool al = reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
   return al && (rows == 1 || cols % 8 == 0);
 }
@@ -575,6 +763,8 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 108: return launch_tiled_db_r<8, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 116: return launch_tiled_db_r<16, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 216: return launch_tiled_db_r<16, true>(L, w, r, edge, pad, in, out, rows, cols);
+    case 302: return launch_tma1_r<2>(L, w, r, edge, pad, in, out, cols);
+    case 303: return launch_tma1_r<3>(L, w, r, edge, pad, in, out, cols);
     case -8:
       switch (r) {
         case 1: return launch_shfl2<1>(L, w, edge, pad, in, out, rows, cols);
