@@ -308,7 +308,8 @@ __device__ __forceinline__ void tma_load_rows(void* smem_dst, const CUtensorMap*
 template <int R, bool PK, int STAGES>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
-                     const float* in, float* out, long long n, long long nfull, int ntiles) {
+                     const float* in, float* out, long long rows, long long cols, unsigned tiles_per_row, int ntiles,
+                     unsigned dq, unsigned dr) {
   constexpr int HP = (R + 3) / 4 * 4;
   constexpr int SWZ = (32 - HP) / 4;
   extern __shared__ unsigned char smraw0[];
@@ -328,19 +329,37 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
   __syncthreads();
   int tile = blockIdx.x;
   if (tile >= ntiles) return;
-  int ptile = tile;  // producer state (thread 0)
+  long long row = tile / tiles_per_row;  // the only division
+  unsigned tcol = static_cast<unsigned>(tile - row * tiles_per_row);
+  auto advance = [&](int& t, long long& r, unsigned& c) {
+    t += gridDim.x;
+    r += dq;
+    c += dr;
+    if (c >= tiles_per_row) {
+      c -= tiles_per_row;
+      ++r;
+    }
+  };
+  int ptile = tile;  // producer state (thread 0): the next tile to request
+  long long prow = row;
+  unsigned ptcol = tcol;
+  const long long rows128 = cols >> 5;  // 128-byte rows per matrix row (rows > 1: cols % 32 == 0)
   auto request = [&](int s) {
     mbar_arrive_expect_tx(full + s, T1W_STAGE_BYTES);
-    tma_load_rows(stage_ptr(s), &tmap, 0, ptile * (T1W_TILE / 32) - 1, full + s);
+    tma_load_rows(stage_ptr(s), &tmap, 0, static_cast<int>(prow * rows128 + ptcol * (T1W_TILE / 32)) - 1, full + s);
   };
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int d = 0; d < STAGES - 1; ++d) {
       if (ptile < ntiles) request(d);
-      ptile += gridDim.x;
+      advance(ptile, prow, ptcol);
     }
   }
-  const bool zeros_ok = edge == EDGE_CONSTANT && pad == 0.f;  // what the copy delivers outside the vector
+  // Outside the vector the copy delivers zeros (what CONSTANT with pad 0 wants); outside a row of a matrix it delivers
+  // the neighbouring rows. pb: the first column the 128-byte-row view does not hold as part of this row.
+  const bool zeros_ok = rows == 1 && edge == EDGE_CONSTANT && pad == 0.f;
+  const long long pb = cols & ~31ll;
+  const bool back_always = !zeros_ok || pb != cols;
   int s = 0, ph = 0;
   int tgt = STAGES - 1, tph = 1;
   for (int it = 0; tile < ntiles; ++it) {
@@ -349,30 +368,42 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
         if (it > 0) mbar_wait(empty + tgt, tph);
         request(tgt);
       }
-      ptile += gridDim.x;
+      advance(ptile, prow, ptcol);
     }
     tgt = tgt + 1 == STAGES ? 0 : tgt + 1;
     if (tgt == 0) tph ^= 1;
     mbar_wait(full + s, ph);
-    const long long c0 = static_cast<long long>(tile) * T1W_TILE;
+    const long long c0 = static_cast<long long>(tcol) * T1W_TILE;
     float* sm = stage_ptr(s);
-    const long long w0 = c0 - 32, w1 = c0 + T1W_TILE + 32;  // the window [w0, w1)
-    const bool patch = (w0 < 0 && !zeros_ok) || (w1 > nfull && (nfull != n || !zeros_ok));  // block-uniform
-    if (patch) {
-      for (int idx = threadIdx.x; idx < T1W_ROWS * 32; idx += T1_THREADS) {
-        const long long gi = w0 + idx;
-        if (gi < 0 || gi >= nfull) {
-          const unsigned q = unsigned(idx) >> 5, c = (unsigned(idx) >> 2) & 7u;
-          sm[q * 32 + ((c ^ (q & 7u)) << 2) + (idx & 3)] = ext_row(in, n, gi, edge, pad);
-        }
-      }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next TMA refill
-      __syncthreads();
+    const float* xrow = in + row * cols;
+    auto put = [&](int idx, long long c) {  // window cell idx holds column c of the row
+      const unsigned q = unsigned(idx) >> 5, ch = (unsigned(idx) >> 2) & 7u;
+      sm[q * 32 + ((ch ^ (q & 7u)) << 2) + (idx & 3)] = ext_row(xrow, cols, c, edge, pad);
+    };
+    // Patches are per warp, not per block: only thread 0 reads the front halo, so warp 0 writes it; the cells from pb on
+    // are written by every warp that gets here (same values), so no warp waits for another one.
+    bool patched = false;
+    if (tcol == 0 && !zeros_ok && threadIdx.x < 32) {
+      put(lane, lane - 32);
+      patched = true;
     }
-    compute_tile1<R, 16, PK, SWZ>(sm, W, out, n, c0);
+    if (back_always && pb < c0 + T1W_TILE + 32) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const long long c = pb + lane + 32 * j;
+        const long long idx = c - c0 + 32;
+        if (idx < T1W_ROWS * 32) put(static_cast<int>(idx), c);
+      }
+      patched = true;
+    }
+    if (patched) {  // warp-uniform
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next TMA refill
+      __syncwarp();
+    }
+    compute_tile1<R, 16, PK, SWZ>(sm, W, out + row * cols, cols, c0);
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
-    tile += gridDim.x;
+    advance(tile, row, tcol);
     s = s + 1 == STAGES ? 0 : s + 1;
     if (s == 0) ph ^= 1;
   }
@@ -665,8 +696,12 @@ inline cudaError_t make_tmap_rows(CUtensorMap* out, const float* base, size_t nr
 
 // vectors shorter than one tile (and anything the tensor map cannot describe) take the cp.async form
 template <int R, int STAGES>
-cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out, size_t n) {
-  if (n < size_t(T1W_TILE) || n / T1W_TILE >= (size_t(1) << 30)) return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, 1, n);
+cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out, size_t rows,
+                        size_t cols) {
+  const size_t tpr = (cols + T1W_TILE - 1) / T1W_TILE;
+  const size_t ntiles = rows * tpr;
+  if ((rows == 1 && cols < size_t(T1W_TILE)) || cols < 32 || rows * cols / 32 >= (size_t(1) << 31) - 1 || ntiles >= (size_t(1) << 30))
+    return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, rows, cols);
   constexpr size_t smem = size_t(STAGES) * T1W_STAGE_STRIDE + 2 * STAGES * sizeof(uint64_t) + 1024;
   auto kern = overlap1d_tma_kernel<R, true, STAGES>;
   static int per_sm = 0;
@@ -676,27 +711,26 @@ cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad
       return cudaErrorInvalidValue;
   }
   CUtensorMap tmap;
-  cudaError_t e = make_tmap_rows(&tmap, in, n / 32);
+  cudaError_t e = make_tmap_rows(&tmap, in, rows * cols / 32);
   if (e != cudaSuccess) return e;
-  const size_t ntiles = (n + T1W_TILE - 1) / T1W_TILE;
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
-  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, tmap, edge, pad, in, out, (long long)n, (long long)(n / 32 * 32),
-                                                        (int)ntiles);
+  kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, tmap, edge, pad, in, out, (long long)rows, (long long)cols,
+                                                        (unsigned)tpr, (int)ntiles, (unsigned)(grid / tpr), (unsigned)(grid % tpr));
   ++*L.launches;
   return cudaGetLastError();
 }
 
 template <int STAGES>
 cudaError_t launch_tma1_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in, float* out,
-                          size_t n) {
+                          size_t rows, size_t cols) {
   switch (r) {
-    case 1: return launch_tma1<1, STAGES>(L, w, edge, pad, in, out, n);
-    case 2: return launch_tma1<2, STAGES>(L, w, edge, pad, in, out, n);
-    case 3: return launch_tma1<3, STAGES>(L, w, edge, pad, in, out, n);
-    case 4: return launch_tma1<4, STAGES>(L, w, edge, pad, in, out, n);
-    case 8: return launch_tma1<8, STAGES>(L, w, edge, pad, in, out, n);
-    case 16: return launch_tma1<16, STAGES>(L, w, edge, pad, in, out, n);
+    case 1: return launch_tma1<1, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_tma1<2, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_tma1<3, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_tma1<4, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_tma1<8, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_tma1<16, STAGES>(L, w, edge, pad, in, out, rows, cols);
   }
   return cudaErrorInvalidValue;
 }
@@ -739,7 +773,7 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
   if (kVariants[v].o == 0) return true;
   if (!templated_radius(r)) return false;
   if (kVariants[v].o == -8 && r > 8) return false;
-  if (kVariants[v].o >= 300 && rows != 1) return false;  // vectors only
+  if (kVariants[v].o >= 300 && rows != 1 && cols % 32 != 0) return false;  // a matrix row must be whole 128-byte rows
   const bool al = reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
   return al && (rows == 1 || cols % 8 == 0);
 }
@@ -763,8 +797,8 @@ cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, in
     case 108: return launch_tiled_db_r<8, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 116: return launch_tiled_db_r<16, false>(L, w, r, edge, pad, in, out, rows, cols);
     case 216: return launch_tiled_db_r<16, true>(L, w, r, edge, pad, in, out, rows, cols);
-    case 302: return launch_tma1_r<2>(L, w, r, edge, pad, in, out, cols);
-    case 303: return launch_tma1_r<3>(L, w, r, edge, pad, in, out, cols);
+    case 302: return launch_tma1_r<2>(L, w, r, edge, pad, in, out, rows, cols);
+    case 303: return launch_tma1_r<3>(L, w, r, edge, pad, in, out, rows, cols);
     case -8:
       switch (r) {
         case 1: return launch_shfl2<1>(L, w, edge, pad, in, out, rows, cols);

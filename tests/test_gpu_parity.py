@@ -412,7 +412,7 @@ def test_overlap1d_constant_input_and_impulse(ctx):
                 vo.destroy()
 
 
-MAT_SHAPES = [(1, 1), (3, 5), (37, 129), (64, 128), (65, 136), (200, 520), (130, 1032), (1030, 264)]
+MAT_SHAPES = [(1, 1), (3, 5), (37, 129), (64, 128), (65, 136), (200, 520), (130, 1032), (1030, 264), (6, 8256)]
 
 
 @pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
@@ -424,7 +424,7 @@ def test_overlap1d_matrix_rows(ctx, v, r):
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
         tiled_ok = o1_radius_ok(v, r) and (rows == 1 or cols % 8 == 0)
         if S.variant_names(S.SK_OVERLAP1D)[v].startswith("tma_swz"):
-            tiled_ok = tiled_ok and rows == 1  # the 128-byte-row view is of a vector
+            tiled_ok = o1_radius_ok(v, r) and (rows == 1 or cols % 32 == 0)  # a matrix row must be whole 128-byte rows
         with forced(ctx, S.SK_OVERLAP1D, v):
             for edge, pad in EDGE_CASES:
                 if v != 0 and not tiled_ok:
