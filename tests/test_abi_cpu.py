@@ -204,3 +204,32 @@ def test_argument_validation_without_cuda():
     for c in (a, b, i, m, e):
         c.destroy()
     ctx.close()
+
+
+def test_shipped_plan_is_consistent_with_the_variant_tables():
+    """plans/b200.plan (the plan bench.py loads): well-formed, loads, every variant id exists for its skeleton,
+    breakpoints ascend, and the look-up returns the stored winner at BASELINE.json's full sizes."""
+    import os
+
+    path = os.path.join(os.path.dirname(os.path.abspath(S.__file__)), "plans", "b200.plan")
+    lines = open(path).read().split("\n")
+    assert lines[0].strip() == "skelplan 1"
+    ctx = S.Context(lazy_cuda=True)
+    ctx.plan_load(path)
+    seen = 0
+    for line in lines[1:]:
+        f = line.split()
+        if not f:
+            continue
+        key, count, rest = [int(v) for v in f[:8]], int(f[8]), [int(v) for v in f[9:]]
+        assert len(rest) == 2 * count and count >= 1
+        nmins, variants = rest[0::2], rest[1::2]
+        assert nmins == sorted(set(nmins))
+        nv = S.lib.skel_variant_count(key[0])
+        assert all(0 <= v < nv for v in variants), (line, nv)
+        inst = S.SkelInstance(skeleton=key[0], fn=key[1], fn2=key[2], dtype=key[3], r0=key[4], r1=key[5], edge=key[6], mode=key[7])
+        for n, v in zip(nmins, variants):
+            assert ctx.plan_lookup(inst, max(n, 1)) == v or n == 0
+        assert ctx.plan_lookup(inst, 1 << 28) == variants[-1]
+        seen += 1
+    assert seen >= 20
