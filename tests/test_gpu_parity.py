@@ -412,6 +412,38 @@ def test_overlap1d_constant_input_and_impulse(ctx):
                 vo.destroy()
 
 
+@pytest.mark.parametrize("name", ["tma_swz_o16_s2", "tma_swz_o16_s3"])
+def test_overlap1d_tma_pipeline_wraps(ctx, name):
+    """Every persistent block of the TMA kernel walks >= 4 tiles (at most 148 x 6 blocks): the stages are refilled, both
+    mbarrier parities are used, and a ragged tail (n % 32 != 0) ends the walk. Element by element against the oracle."""
+    v = S.variant_names(S.SK_OVERLAP1D).index(name)
+    n = 4096 * 3700 + 77
+    x = I.uniform01_f32(7300, n)
+    vx, vo = ctx.vector_from(x), ctx.vector(n)
+    with forced(ctx, S.SK_OVERLAP1D, v):
+        for r, edge, pad in ((16, S.EDGE_CYCLIC, 0.0), (16, S.EDGE_CONSTANT, 0.0), (8, S.EDGE_DUPLICATE, 0.0), (4, S.EDGE_CONSTANT, 1.5)):
+            w = I.signed_weights_f32(7301 + r, 2 * r + 1)
+            ctx.mapoverlap_1d(w, r, edge, pad, vx, vo)
+            assert ctx.last_variant() == (S.SK_OVERLAP1D, v)
+            ref, ab = O.mapoverlap_1d(w, r, edge, pad, x)
+            assert_overlap(vo.numpy(), ref, ab)
+    vx.destroy()
+    vo.destroy()
+    # rows of a matrix: two tiles per row (the second one 32 columns wide), > 4 tiles per block
+    rows, cols = 3800, 4128
+    X = I.uniform01_f32(7310, rows * cols).reshape(rows, cols)
+    mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
+    with forced(ctx, S.SK_OVERLAP1D, v):
+        for r, edge, pad in ((8, S.EDGE_DUPLICATE, 0.0), (16, S.EDGE_CONSTANT, 0.0), (16, S.EDGE_CYCLIC, 0.0)):
+            w = I.positive_weights_f32(7311 + r, 2 * r + 1)
+            ctx.mapoverlap_1d_matrix(w, r, edge, pad, S.AXIS_ROW, mx, mo)
+            assert ctx.last_variant() == (S.SK_OVERLAP1D, v)
+            ref, ab = O.mapoverlap_1d_matrix(w, r, edge, pad, O.AXIS_ROW, X)
+            assert_overlap(mo.numpy(), ref, ab)
+    mx.destroy()
+    mo.destroy()
+
+
 MAT_SHAPES = [(1, 1), (3, 5), (37, 129), (64, 128), (65, 136), (200, 520), (130, 1032), (1030, 264), (6, 8256)]
 
 
