@@ -64,8 +64,8 @@ cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edg
 }
 
 const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8", "tiled_oy4_db", "tiled_oy8_db",
-                              "tma_oy4", "tma_oy8"};
-constexpr int kNumVariants = 7;
+                              "tma_oy4", "tma_oy8", "tma_oy4_s2"};
+constexpr int kNumVariants = 8;
 
 inline bool tiled_alignment_ok(const void* in, const void* out, size_t rows, size_t cols) {
   return reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 && cols % 4 == 0 &&

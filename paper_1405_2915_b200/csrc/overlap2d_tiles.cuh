@@ -483,6 +483,7 @@ cudaError_t launch_tiled_any(const Launch& L, int v, const WT& w, int edge, floa
     case 4: return launch_tiled2_db<RY, RX, 8, WT, PK>(L, w, edge, pad, in, out, rows, cols);
     case 5: return launch_tma2<RY, RX, 4, WT, PK, 3>(L, w, edge, pad, in, out, rows, cols);
     case 6: return launch_tma2<RY, RX, 8, WT, PK, RX == 0 ? 3 : 2>(L, w, edge, pad, in, out, rows, cols);
+    case 7: return launch_tma2<RY, RX, 4, WT, PK, 2>(L, w, edge, pad, in, out, rows, cols);  // 2 stages: 5 resident blocks
   }
   return cudaErrorInvalidValue;
 }
