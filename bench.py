@@ -57,7 +57,7 @@ def sizes(scale: float):
 
 
 def gen_inputs(sz):
-    from paper_1405_2915_b200 import inputs as I
+    import skel_inputs as I
     t = time.time()
     d = {
         "x": I.uniform_pm1_f32(I.config_seed(2, 0), sz["n26"]),
@@ -213,7 +213,7 @@ def cpu_oracle_pass(scale_div: int = 4, quiet=False, openmp=False):
     Returns (algorithmic bytes, seconds, threads, description). openmp: the OpenMP build of the same
     loops; Reduce and Scan stay sequential in it (their order is part of the oracle)."""
     import oracle as O
-    from paper_1405_2915_b200 import inputs as I
+    import skel_inputs as I
     O.use_openmp(openmp)
     n = (1 << 26) // scale_div
     n28 = (1 << 28) // scale_div
@@ -253,7 +253,7 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
     smart containers save: transfers and wall time with the coherence protocol (LAZY) against the
     "no smart containers" baseline (EAGER, run for fewer iterations; per-iteration figures)."""
     import torch
-    from paper_1405_2915_b200 import inputs as I
+    import skel_inputs as I
     x0 = I.uniform01_f32(I.config_seed(5, 1), n)
     w = I.positive_weights_f32(I.config_seed(3, 14), 9)
 
@@ -463,7 +463,7 @@ def main():
                                   "frac_fma_roofline": round(alu_us / per[name]["us"], 4)})
 
     # ---- small-n latency (config 0: dot n = 2^20, L2 resident) — reported, not part of `value`
-    from paper_1405_2915_b200 import inputs as I
+    import skel_inputs as I
     n20 = 1 << 20
     a20, b20 = ctx.vector_from(I.uniform_pm1_f32(I.config_seed(1, 0), n20)), ctx.vector_from(I.uniform_pm1_f32(I.config_seed(1, 1), n20))
     for _ in range(5):

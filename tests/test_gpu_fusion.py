@@ -12,7 +12,7 @@ import pytest
 
 import oracle as O
 from helpers import assert_map_f32, assert_overlap
-from paper_1405_2915_b200 import inputs as I
+import skel_inputs as I
 from paper_1405_2915_b200 import skel as S
 
 pytestmark = pytest.mark.gpu

@@ -5,7 +5,7 @@ calls."""
 import numpy as np
 import pytest
 
-from paper_1405_2915_b200 import inputs as I
+import skel_inputs as I
 from paper_1405_2915_b200 import skel as S
 
 pytestmark = pytest.mark.gpu

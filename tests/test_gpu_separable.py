@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from paper_1405_2915_b200 import inputs as I
+import skel_inputs as I
 from paper_1405_2915_b200 import skel as S
 
 pytestmark = pytest.mark.gpu

@@ -14,7 +14,7 @@ import numpy as np
 import pytest
 
 import oracle as O
-from paper_1405_2915_b200 import inputs as I
+import skel_inputs as I
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")
 BOUNDARY_N = [1, 2, 3, 4, 5, 7, 8, 31, 32, 33, 127, 128, 129, 1023, 1024, 1025]

@@ -2,7 +2,7 @@
 as a pure function, against a brute-force bitmap model. No GPU."""
 import numpy as np
 
-from paper_1405_2915_b200 import inputs as I
+import skel_inputs as I
 from paper_1405_2915_b200 import skel as S
 
 
