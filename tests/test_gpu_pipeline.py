@@ -109,6 +109,22 @@ def test_pipeline_eager_moves_five_containers_per_iteration(ctx):
     assert st["h2d_elided"] == 0 and st["d2h_elided"] == 0
 
 
+# The protocol of SURVEY.md 8(c).7 / DESIGN.md reading 14 written out as a literal table: the model of the random
+# walk below is THIS table, not the library's own skel_coherence_step. States: bit 0 = host copy valid, bit 1 = device
+# copy valid (0 UNINIT, 1 HOST, 2 DEVICE, 3 SHARED). (state, actor, access) -> (new state, transfer).
+_U, _H, _D, _S = 0, 1, 2, 3
+_R, _W, _RW = 0, 1, 2   # skel_access values (include/skel.h), restated
+MODEL = {
+    (_U, "dev", _W): (_D, None), (_U, "host", _W): (_H, None),
+    (_H, "dev", _R): (_S, "h2d"), (_H, "dev", _W): (_D, None), (_H, "dev", _RW): (_D, "h2d"),
+    (_H, "host", _R): (_H, None), (_H, "host", _W): (_H, None), (_H, "host", _RW): (_H, None),
+    (_D, "dev", _R): (_D, None), (_D, "dev", _W): (_D, None), (_D, "dev", _RW): (_D, None),
+    (_D, "host", _R): (_S, "d2h"), (_D, "host", _W): (_H, None), (_D, "host", _RW): (_H, "d2h"),
+    (_S, "dev", _R): (_S, None), (_S, "dev", _W): (_D, None), (_S, "dev", _RW): (_D, None),
+    (_S, "host", _R): (_S, None), (_S, "host", _W): (_H, None), (_S, "host", _RW): (_H, None),
+}
+
+
 def test_coherence_model_based_random_walk(ctx):
     """Random sequences of host writes / host reads / skeleton calls on three containers, applied to
     the library and to shadow host arrays through the oracle + the protocol table."""
@@ -117,20 +133,21 @@ def test_coherence_model_based_random_walk(ctx):
     w = I.positive_weights_f32(31, 5)
     vecs = [ctx.vector(n) for _ in range(3)]
     shadow = [None, None, None]          # fp32 arrays as the GPU holds them (downloaded after each call)
-    state = [0, 0, 0]                    # bit 0 host valid, bit 1 device valid
+    state = [_U, _U, _U]
+    assert (S.READ, S.WRITE, S.READWRITE) == (_R, _W, _RW)
     h2d = d2h = 0
     ctx.reset_stats()
 
     def dev_access(i, access):
         nonlocal h2d
-        _, new, xfer = S.coherence_step(state[i], 0, access, S.LAZY)
-        h2d += 1 if xfer & 1 else 0
+        new, xfer = MODEL[(state[i], "dev", access)]
+        h2d += 1 if xfer == "h2d" else 0
         state[i] = new
 
     def host_access(i, access):
         nonlocal d2h
-        _, new, xfer = S.coherence_step(state[i], 1, access, S.LAZY)
-        d2h += 1 if xfer & 2 else 0
+        new, xfer = MODEL[(state[i], "host", access)]
+        d2h += 1 if xfer == "d2h" else 0
         state[i] = new
 
     for step in range(120):

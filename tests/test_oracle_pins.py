@@ -283,6 +283,58 @@ def test_mapreduce_fusion_invariant_and_brute_force():
         assert fused == wrap32(sum(int(p) * int(q) for p, q in zip(a_i, b_i)))
 
 
+def test_mapreduce_constant_second_operand():
+    """in1 = None: the second operand of the user function is the constant c, rounded to fp32 first
+    (reading (c).1 iii). Pinned against math.fsum / exact Python integers, never against the oracle."""
+    c = 1.0001
+    c32 = float(np.float32(c))
+    assert c32 != c  # the rounding is visible, so using the unrounded constant fails below
+    for n in BOUNDARY_N:
+        x = I.uniform_pm1_f32(64 + n, n)
+        xs = [float(t) for t in x]
+        r, a = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, c, x)          # sum_i c32 * x_i (products exact in fp64)
+        assert abs(r - math.fsum(c32 * t for t in xs)) <= 4e-16 * max(a, 1e-300)
+        assert a == pytest.approx(math.fsum(abs(c32 * t) for t in xs), rel=1e-15)
+        r, _ = O.mapreduce_f32(O.FN_ADD, O.FN_ADD, c, x)           # sum_i (x_i + c32)
+        assert r == pytest.approx(math.fsum(t + c32 for t in xs), abs=1e-12)
+        r, _ = O.mapreduce_f32(O.FN_MAX, O.FN_ADD, 0.25, x)        # sum_i max(x_i, 0.25)
+        assert r == pytest.approx(math.fsum(max(t, 0.25) for t in xs), abs=1e-12)
+        r, _ = O.mapreduce_f32(O.FN_MULT, O.FN_MAX, -2.0, x)       # max_i (-2 x_i) = -2 min x
+        assert r == -2.0 * min(xs)
+        r, _ = O.mapreduce_f32(O.FN_ADD, O.FN_MULT, 1.0, 0.001 * x)  # prod_i (1 + x_i/1000): left to right in fp64
+        acc = None
+        for t in (0.001 * x).astype(np.float32):
+            acc = float(t) + 1.0 if acc is None else acc * (float(t) + 1.0)
+        assert r == acc
+        v = I.full_range_i32(65 + n, n)
+        vi = [int(t) for t in v]
+        assert O.mapreduce_i32(O.FN_MULT, O.FN_ADD, 3, v) == wrap32(sum(3 * t for t in vi))
+        assert O.mapreduce_i32(O.FN_ADD, O.FN_ADD, -7, v) == wrap32(sum(t - 7 for t in vi))
+        assert O.mapreduce_i32(O.FN_MAX, O.FN_MAX, 12345, v) == max(max(vi), 12345)
+        assert O.mapreduce_i32(O.FN_ADD, O.FN_MAX, 1, v) == max(wrap32(t + 1) for t in vi)
+    # closed form: sum_i c * i with c = 2 over i < n -> n (n - 1); the constant really is the SECOND operand
+    n = 1000
+    assert O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 2.0, np.arange(n, dtype=np.float32))[0] == n * (n - 1)
+    assert O.mapreduce_i32(O.FN_MULT, O.FN_ADD, 2, np.arange(n, dtype=np.int32)) == n * (n - 1)
+
+
+def test_reduce_f32_mult_on_a_vector():
+    """Reduce(mult) over a vector: plain left-to-right fp64 product (reading (c).2), against math.prod,
+    numpy.prod and the closed form n!."""
+    for n in BOUNDARY_N:
+        x = (1.0 + 0.001 * I.uniform_pm1_f32(66 + n, n)).astype(np.float32)
+        r, a = O.reduce_f32(O.FN_MULT, x)
+        acc = float(x[0])
+        for t in x[1:]:
+            acc *= float(t)
+        assert r == acc
+        assert r == pytest.approx(float(np.prod(x.astype(np.float64))), rel=1e-12)
+        assert a == pytest.approx(math.fsum(abs(float(t)) for t in x), rel=1e-15)
+    f = np.arange(1, 19, dtype=np.float32)
+    assert O.reduce_f32(O.FN_MULT, f)[0] == float(math.factorial(18))  # 18! < 2^53: exact
+    assert O.reduce_f32(O.FN_MULT, np.array([3.0, -2.0, 0.5], np.float32))[0] == -3.0
+
+
 # ------------------------------------------------------------------ Scan
 def test_scan_closed_forms():
     for n in [0] + BOUNDARY_N + [4096, 4097, 1 << 18]:
@@ -323,6 +375,55 @@ def test_scan_brute_force_every_small_n():
             inc.append(acc)
         assert O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, x).tolist() == inc
         assert O.scan_i32(O.FN_ADD, O.SCAN_EXCLUSIVE, 3, x).tolist() == exc
+
+
+def test_scan_i32_mult_wraps_like_python_ints():
+    """Scan(mult) on int32: running product modulo 2^32 (reading (c).2 ii), against exact Python
+    integers and the closed form i! mod 2^32."""
+    for n in list(range(0, 40)) + [127, 128, 129, 1025]:
+        x = (I.full_range_i32(84 + n, n) | 1)  # odd factors: the product never collapses to 0
+        acc, inc, exc = None, [], []
+        e = 3
+        for t in x:
+            exc.append(wrap32(e))
+            e = wrap32(e * int(t))
+            acc = int(t) if acc is None else wrap32(acc * int(t))
+            inc.append(acc)
+        assert O.scan_i32(O.FN_MULT, O.SCAN_INCLUSIVE, 0, x).tolist() == inc
+        assert O.scan_i32(O.FN_MULT, O.SCAN_EXCLUSIVE, 3, x).tolist() == exc
+    k = np.arange(1, 21, dtype=np.int32)
+    assert O.scan_i32(O.FN_MULT, O.SCAN_INCLUSIVE, 0, k).tolist() == [wrap32(math.factorial(int(j))) for j in k]
+    assert O.scan_i32(O.FN_MULT, O.SCAN_EXCLUSIVE, 1, k).tolist() == [wrap32(math.factorial(int(j) - 1)) for j in k]
+
+
+def test_scan_f32_max_and_mult():
+    """fp32 Scan with max / mult in fp64: numpy's accumulate routines (independent library) and closed forms;
+    the exclusive forms fold the fp32-rounded init into every prefix (reading (c).4 ii)."""
+    x = I.uniform_pm1_f32(91, 2500)
+    x64 = x.astype(np.float64)
+    out, ab = O.scan_f32(O.FN_MAX, O.SCAN_INCLUSIVE, 0.0, x)
+    assert np.array_equal(out, np.maximum.accumulate(x64))
+    assert np.allclose(ab, np.cumsum(np.abs(x64)), rtol=1e-14)
+    init = 0.3
+    i32 = float(np.float32(init))
+    oute, abe = O.scan_f32(O.FN_MAX, O.SCAN_EXCLUSIVE, init, x)
+    assert oute[0] == i32 and np.array_equal(oute[1:], np.maximum(np.maximum.accumulate(x64)[:-1], i32))
+    assert abe[0] == abs(i32) and np.allclose(abe[1:], abs(i32) + np.cumsum(np.abs(x64))[:-1], rtol=1e-14)
+    # a strictly decreasing input: the running max is the first element; increasing: the identity
+    dec = np.arange(100, 0, -1).astype(np.float32)
+    assert np.array_equal(O.scan_f32(O.FN_MAX, O.SCAN_INCLUSIVE, 0.0, dec)[0], np.full(100, 100.0))
+    assert np.array_equal(O.scan_f32(O.FN_MAX, O.SCAN_INCLUSIVE, 0.0, dec[::-1].copy())[0], dec[::-1].astype(np.float64))
+    p = (1.0 + 0.01 * x[:600]).astype(np.float32)
+    out, _ = O.scan_f32(O.FN_MULT, O.SCAN_INCLUSIVE, 0.0, p)
+    assert np.allclose(out, np.cumprod(p.astype(np.float64)), rtol=1e-13, atol=0)
+    acc = None
+    for k, t in enumerate(p[:50]):
+        acc = float(t) if acc is None else acc * float(t)
+        assert out[k] == acc  # left to right, one rounding per step
+    oute, _ = O.scan_f32(O.FN_MULT, O.SCAN_EXCLUSIVE, 2.0, p)
+    assert oute[0] == 2.0 and np.allclose(oute[1:], 2.0 * np.cumprod(p.astype(np.float64))[:-1], rtol=1e-13)
+    two = np.full(40, 2.0, np.float32)  # closed form 2^(i+1), exact
+    assert O.scan_f32(O.FN_MULT, O.SCAN_INCLUSIVE, 0.0, two)[0].tolist() == [2.0 ** (k + 1) for k in range(40)]
 
 
 def test_scan_f32_against_cumsum():
