@@ -69,6 +69,8 @@ struct skel_ctx {
   bool dev_ready = false;
   int sms = 148;
   Scratch scratch{};
+  unsigned* tile_ctr = nullptr;  // device: tile counter of the persistent TMA kernels (kernels.hpp Launch)
+  unsigned tile_next = 0;        // host: its value when the next launch starts
   void* d_result = nullptr;  // device slot for scalars returned to the host
   void* h_result = nullptr;      // pinned, mapped host slot for scalars returned to the host ...
   void* h_result_dev = nullptr;  // ... and its device-side address: the reducing kernel stores the scalar straight into it
@@ -128,6 +130,8 @@ skel_status ensure_device(skel_ctx* c) {
   c->scratch.ticket = reinterpret_cast<unsigned*>(base + partial_bytes);
   c->scratch.scan_ticket = reinterpret_cast<unsigned*>(base + partial_bytes + 64);
   c->d_result = base + partial_bytes + 128;
+  c->tile_ctr = reinterpret_cast<unsigned*>(base + partial_bytes + 192);
+  c->tile_next = 0;
   c->scratch.scan_state = nullptr;
   c->scratch.scan_state_tiles = 0;
   c->scratch.scan_epoch = 0;
@@ -677,7 +681,7 @@ cudaError_t launch_separable_two_pass(skel_ctx* c, const Call& k) {
 }
 
 cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
-  Launch L{c->stream, c->sms, &c->launches};
+  Launch L{c->stream, c->sms, &c->launches, c->tile_ctr, &c->tile_next};
   const skel_instance& i = k.inst;
   switch (i.skeleton) {
     case SKEL_SK_REDUCE_ROWS:
@@ -783,7 +787,7 @@ skel_status flush_pending(skel_ctx* c) {
     const int map_fn = map ? map->inst.fn : FN_IDENT_;
     const int red_op = red ? red->inst.fn : FUSED_NO_REDUCE;
     if (fused_chain_ok(map_fn, ov->inst.r0, red_op, in, map_out, ov->out, ov->n)) {
-      Launch L{c->stream, c->sms, &c->launches};
+      Launch L{c->stream, c->sms, &c->launches, c->tile_ctr, &c->tile_next};
       cudaError_t e = launch_fused_chain(L, c->scratch, map_fn, map ? map->cbits : 0u, ov->w1, ov->inst.r0, ov->inst.edge,
                                          ov->pad, red_op, in, map_out, static_cast<float*>(ov->out), ov->n,
                                          red ? static_cast<float*>(red->out) : nullptr);
@@ -1655,7 +1659,7 @@ skel_status skel_probe_fma_peak(skel_ctx* c, int reps, double* fma_per_s) {
   cudaEvent_t e0, e1;
   CU(c, cudaEventCreate(&e0));
   CU(c, cudaEventCreate(&e1));
-  Launch L{c->stream, c->sms, &c->launches};
+  Launch L{c->stream, c->sms, &c->launches, c->tile_ctr, &c->tile_next};
   std::vector<float> ms(reps);
   double count = 0;
   for (int r = -1; r < reps; ++r) {  // r = -1 warms up

@@ -12,6 +12,10 @@ struct Launch {
   cudaStream_t stream;
   int sms;            // SM count of the device (148 on B200)
   int* launches;      // incremented once per kernel launch
+  // dynamic tile assignment of the persistent TMA kernels: a device counter that is never reset, and the host's copy
+  // of the value it will have when the next launch starts (launches of a context are ordered on one stream)
+  unsigned* tile_ctr;
+  unsigned* tile_next;
 };
 
 struct Scratch {       // device scratch owned by the context (see api.cu)

@@ -33,8 +33,9 @@ __device__ __forceinline__ float ext_row(const float* row, long long cols, long 
 }
 
 // ---- direct --------------------------------------------------------------------------------
-// Sums are chained in groups of 16 taps so that the rounding-error bound stays below
-// (16 + #groups) * 2^-24 of sum|w x| for every r.
+// Up to 33 taps (r <= 16) are ONE chain in ascending tap order, like every tiled variant (so all variants, and the
+// fused separable kernel, give the same bits; bound 33 * 2^-24 = 1.97e-6 of sum|w x|). Longer filters are chained in
+// groups of 16 taps and the group sums added: (16 + #groups - 1) * 2^-24 <= 1.44e-6.
 __global__ void __launch_bounds__(256)
 overlap1d_direct_kernel(const __grid_constant__ Weights1D W, int r, int edge, float pad, const float* in, float* out,
                         size_t rows, size_t cols) {
@@ -45,8 +46,9 @@ overlap1d_direct_kernel(const __grid_constant__ Weights1D W, int r, int edge, fl
     const float* x = in + row * cols;
     float total_acc = 0.f;
     const bool interior = (j - r >= 0) && (j + r < static_cast<long long>(cols));
-    for (int k0 = 0; k0 <= 2 * r; k0 += 16) {
-      const int k1 = min(k0 + 16, 2 * r + 1);
+    const int chain = 2 * r + 1 <= 33 ? 33 : 16;
+    for (int k0 = 0; k0 <= 2 * r; k0 += chain) {
+      const int k1 = min(k0 + chain, 2 * r + 1);
       float acc = 0.f;
       if (interior) {
         for (int k = k0; k < k1; ++k) acc = fmaf(W.w[k], __ldg(x + j + k - r), acc);
@@ -309,13 +311,14 @@ template <int R, bool PK, int STAGES>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
                      const float* in, float* out, long long rows, long long cols, unsigned tiles_per_row, int ntiles,
-                     unsigned dq, unsigned dr) {
+                     unsigned* tile_ctr, unsigned tile_base) {
   constexpr int HP = (R + 3) / 4 * 4;
   constexpr int SWZ = (32 - HP) / 4;
   extern __shared__ unsigned char smraw0[];
   unsigned char* smraw = smraw0 + ((1024u - (smem_u32(smraw0) & 1023u)) & 1023u);  // the swizzle is a function of address bits 4..9
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw + STAGES * T1W_STAGE_STRIDE);
   uint64_t* empty = full + STAGES;
+  int2* coord = reinterpret_cast<int2*>(empty + STAGES);  // (matrix row, tile column) of the tile in each stage; row < 0: end
   auto stage_ptr = [&](int s) { return reinterpret_cast<float*>(smraw + s * T1W_STAGE_STRIDE); };
   const int lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -327,33 +330,28 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
     mbar_fence_init();
   }
   __syncthreads();
-  int tile = blockIdx.x;
-  if (tile >= ntiles) return;
-  long long row = tile / tiles_per_row;  // the only division
-  unsigned tcol = static_cast<unsigned>(tile - row * tiles_per_row);
-  auto advance = [&](int& t, long long& r, unsigned& c) {
-    t += gridDim.x;
-    r += dq;
-    c += dr;
-    if (c >= tiles_per_row) {
-      c -= tiles_per_row;
-      ++r;
-    }
-  };
-  int ptile = tile;  // producer state (thread 0): the next tile to request
-  long long prow = row;
-  unsigned ptcol = tcol;
   const long long rows128 = cols >> 5;  // 128-byte rows per matrix row (rows > 1: cols % 32 == 0)
-  auto request = [&](int s) {
-    mbar_arrive_expect_tx(full + s, T1W_STAGE_BYTES);
-    tma_load_rows(stage_ptr(s), &tmap, 0, static_cast<int>(prow * rows128 + ptcol * (T1W_TILE / 32)) - 1, full + s);
+  // Dynamic tile assignment (see overlap2d_tiles.cuh "tma_*"): the first tile is the block's index, later ids come from
+  // a global counter; the fetch is issued one tile ahead of its use; exactly one failing fetch per block.
+  unsigned t_next = blockIdx.x;
+  bool exhausted = false;
+  auto produce = [&](int s) {  // thread 0
+    const unsigned t = t_next;
+    if (!exhausted) exhausted = t >= unsigned(ntiles);
+    if (!exhausted) t_next = atomicAdd(tile_ctr, 1u) - tile_base + gridDim.x;
+    if (!exhausted) {
+      const unsigned prow = t / tiles_per_row, ptcol = t - prow * tiles_per_row;
+      coord[s] = make_int2(int(prow), int(ptcol));
+      mbar_arrive_expect_tx(full + s, T1W_STAGE_BYTES);
+      tma_load_rows(stage_ptr(s), &tmap, 0, static_cast<int>(prow * rows128 + ptcol * (T1W_TILE / 32)) - 1, full + s);
+    } else {
+      coord[s] = make_int2(-1, 0);
+      mbar_arrive(full + s);
+    }
   };
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int d = 0; d < STAGES - 1; ++d) {
-      if (ptile < ntiles) request(d);
-      advance(ptile, prow, ptcol);
-    }
+    for (int d = 0; d < STAGES - 1; ++d) produce(d);
   }
   // Outside the vector the copy delivers zeros (what CONSTANT with pad 0 wants); outside a row of a matrix it delivers
   // the neighbouring rows. pb: the first column the 128-byte-row view does not hold as part of this row.
@@ -362,17 +360,18 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
   const bool back_always = !zeros_ok || pb != cols;
   int s = 0, ph = 0;
   int tgt = STAGES - 1, tph = 1;
-  for (int it = 0; tile < ntiles; ++it) {
+  for (int it = 0;; ++it) {
     if (threadIdx.x == 0) {
-      if (ptile < ntiles) {
-        if (it > 0) mbar_wait(empty + tgt, tph);
-        request(tgt);
-      }
-      advance(ptile, prow, ptcol);
+      if (it > 0) mbar_wait(empty + tgt, tph);
+      produce(tgt);
     }
     tgt = tgt + 1 == STAGES ? 0 : tgt + 1;
     if (tgt == 0) tph ^= 1;
     mbar_wait(full + s, ph);
+    const int2 rc = coord[s];
+    if (rc.x < 0) break;
+    const long long row = rc.x;
+    const unsigned tcol = unsigned(rc.y);
     const long long c0 = static_cast<long long>(tcol) * T1W_TILE;
     float* sm = stage_ptr(s);
     const float* xrow = in + row * cols;
@@ -403,7 +402,6 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
     compute_tile1<R, 16, PK, SWZ>(sm, W, out + row * cols, cols, c0);
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
-    advance(tile, row, tcol);
     s = s + 1 == STAGES ? 0 : s + 1;
     if (s == 0) ph ^= 1;
   }
@@ -702,7 +700,7 @@ cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad
   const size_t ntiles = rows * tpr;
   if ((rows == 1 && cols < size_t(T1W_TILE)) || cols < 32 || rows * cols / 32 >= (size_t(1) << 31) - 1 || ntiles >= (size_t(1) << 30))
     return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, rows, cols);
-  constexpr size_t smem = size_t(STAGES) * T1W_STAGE_STRIDE + 2 * STAGES * sizeof(uint64_t) + 1024;
+  constexpr size_t smem = size_t(STAGES) * T1W_STAGE_STRIDE + 3 * STAGES * sizeof(uint64_t) + 1024;  // stages, full/empty, coord
   auto kern = overlap1d_tma_kernel<R, true, STAGES>;
   static int per_sm = 0;
   if (per_sm == 0) {
@@ -716,7 +714,8 @@ cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
   kern<<<(unsigned)grid, T1_THREADS, smem, L.stream>>>(w, tmap, edge, pad, in, out, (long long)rows, (long long)cols,
-                                                        (unsigned)tpr, (int)ntiles, (unsigned)(grid / tpr), (unsigned)(grid % tpr));
+                                                        (unsigned)tpr, (int)ntiles, L.tile_ctr, *L.tile_next);
+  *L.tile_next += unsigned(ntiles);  // ntiles - grid ids fetched from the counter + one failing fetch per block
   ++*L.launches;
   return cudaGetLastError();
 }

@@ -25,9 +25,10 @@ overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, 
     const long long j = static_cast<long long>(idx - size_t(i) * cols);
     const bool interior = i - ry >= 0 && i + ry < (long long)rows && j - rx >= 0 && j + rx < (long long)cols;
     float acc = 0.f;
-    if (rx == 0) {  // column-wise 1D: chains of 16 taps
-      for (int a0 = 0; a0 <= 2 * ry; a0 += 16) {
-        const int a1 = min(a0 + 16, 2 * ry + 1);
+    if (rx == 0) {  // column-wise 1D: one chain up to 33 taps (like the tiled variants), else chains of 16 taps
+      const int chain = 2 * ry + 1 <= 33 ? 33 : 16;
+      for (int a0 = 0; a0 <= 2 * ry; a0 += chain) {
+        const int a1 = min(a0 + chain, 2 * ry + 1);
         float p = 0.f;
         for (int a = a0; a < a1; ++a) {
           const float v = interior ? __ldg(in + (i + a - ry) * (long long)cols + j)
@@ -63,9 +64,12 @@ cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edg
   return cudaGetLastError();
 }
 
+// 8..11: the broadcast-FFMA2 forms of the TMA kernel (overlap2d_tiles.cuh "tma_bx*"), dense 2D only
 const char* const kNames[] = {"direct", "tiled_oy4", "tiled_oy8", "tiled_oy4_db", "tiled_oy8_db",
-                              "tma_oy4", "tma_oy8", "tma_oy4_s2"};
-constexpr int kNumVariants = 8;
+                              "tma_oy4", "tma_oy8", "tma_oy4_s2", "tma_bx_oy4", "tma_bx_oy4_s2", "tma_bx2_oy4_s2",
+                              "tma_bx2_oy2"};
+constexpr int kNumVariants = 12;
+constexpr int kNumColVariants = 8;
 
 inline bool tiled_alignment_ok(const void* in, const void* out, size_t rows, size_t cols) {
   return reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 && cols % 4 == 0 &&
@@ -75,10 +79,10 @@ inline bool tiled_alignment_ok(const void* in, const void* out, size_t rows, siz
 }  // namespace
 
 // ---- column-wise 1D ----------------------------------------------------------------------------
-int overlap1d_col_variant_count() { return kNumVariants; }
-const char* overlap1d_col_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kNames[v] : nullptr; }
+int overlap1d_col_variant_count() { return kNumColVariants; }
+const char* overlap1d_col_variant_name(int v) { return (v >= 0 && v < kNumColVariants) ? kNames[v] : nullptr; }
 bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
-  if (v < 0 || v >= kNumVariants) return false;
+  if (v < 0 || v >= kNumColVariants) return false;
   if (v == 0) return true;
   const bool templated = r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16;
   return templated && tiled_alignment_ok(in, out, rows, cols);

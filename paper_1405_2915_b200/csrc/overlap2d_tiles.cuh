@@ -15,6 +15,15 @@
 // FFMA2 (the persistent 2D variants): taps whose window index is even use one fma.rn.f32x2 per output pair (the pair
 // (v[i], v[i+1]) of a 128-bit shared load is an aligned register pair); odd taps stay scalar. Each
 // output still sums its taps in the order b = 0 .. 2RX: bit-identical to the scalar form.
+// "tma_bx*" (broadcast form, RX > 0): EVERY tap is an FFMA2 whatever its alignment. The pair of outputs (2q, 2q+1) of a
+// thread receives window element x[j] with the taps d = j - 2q (output 2q) and d - 1 (output 2q+1): one FFMA2 whose
+// data operand is the single register x[j] broadcast to both halves (SASS: FFMA2 R, R.F32, UR.F32x2, R) and whose
+// weight operand is the pair (w[d], w[d-1]) held in a uniform-register pair (host-built table WPairs2D, constant bank).
+// The first and last tap of a filter row have no partner and stay scalar: 2RX FFMA2 + 2 FFMA per output pair and
+// filter row (9x9: 10 instructions for 18 FMAs instead of 13), no wasted FMA lane. Every output still receives its
+// taps in ascending order, one fused multiply-add each: bit-identical to the scalar form. "bx2": a thread owns two
+// 4-wide strips 128 columns apart (tile 32 x 256, two TMA boxes per stage), so a weight pair loaded into uniform
+// registers feeds twice as many FFMA2.
 // Summation order: a outer, b inner, like the definition. When a filter has more than 33 taps,
 // each filter row is summed on its own and the row sums are then added.
 #pragma once
@@ -89,6 +98,138 @@ __device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x
   unsigned long long d;
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pack2(w, w)), "l"(pack2(x0, x1)), "l"(pack2(lo, hi)));
   asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+
+// geometry of a staged tile (per strip: an SH x SW window, one TMA box)
+template <int RY, int RX, int OY, int XS = 1> struct Tile2Geom {
+  static constexpr int RXP = (RX + 3) / 4 * 4;
+  static constexpr int TH = 8 * OY, SW = T2_TW + 2 * RXP, SH = TH + 2 * RY;
+  static constexpr int TW = T2_TW * XS;                        // tile width in outputs: XS strips of 128 columns
+  static constexpr unsigned BOX_BYTES = unsigned(SH) * SW * 4u;  // one TMA box (one strip's window)
+  static constexpr unsigned BOX_STRIDE = XS == 1 ? BOX_BYTES : (BOX_BYTES + 127u) / 128u * 128u;  // TMA wants 128-byte aligned boxes
+  static constexpr unsigned STAGE_BYTES = BOX_BYTES * XS;      // bytes the TMA copies deliver per stage
+  static constexpr unsigned STAGE_STRIDE = (BOX_STRIDE * XS + 127u) / 128u * 128u;
+};
+
+// weight pairs of the broadcast form: p[a][d] = (w[a][d], w[a][d-1]) for d = 0 .. FW (w[a][-1] = w[a][FW] = 0);
+// rows padded to a multiple of 16 bytes so that one LDCU.128 fetches two pairs
+template <int RY, int RX> struct alignas(16) WPairs2D {
+  static constexpr int FW = 2 * RX + 1, NP = (FW + 2) / 2 * 2;
+  float2 p[2 * RY + 1][NP];
+};
+template <int RY, int RX> inline void make_wpairs(WPairs2D<RY, RX>& P, const float* w /* (2RY+1) x (2RX+1) */) {
+  constexpr int FW = 2 * RX + 1;
+  for (int a = 0; a <= 2 * RY; ++a)
+    for (int d = 0; d < WPairs2D<RY, RX>::NP; ++d) {
+      P.p[a][d].x = d < FW ? w[a * FW + d] : 0.f;
+      P.p[a][d].y = (d >= 1 && d <= FW) ? w[a * FW + d - 1] : 0.f;
+    }
+}
+// (lo, hi) += (wp.x, wp.y) * (x, x): the data register is broadcast, the weight pair comes from uniform registers
+__device__ __forceinline__ void fma2_bcast(float& lo, float& hi, float2 wp, float x) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pack2(x, x)), "l"(pack2(wp.x, wp.y)), "l"(pack2(lo, hi)));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(d));
+}
+
+// Broadcast form of compute_tile2: a thread's XS strips of 4 (x) by OY (y) outputs; strip s is staged in its own
+// SH x SW window at sm + s * SH * SW and covers output columns c0 + 128 s + 4 tx .. + 3.
+template <int RY, int RX, int OY, int XS>
+__device__ __forceinline__ void compute_tile2_bx(const float* sm, const WPairs2D<RY, RX>& P, float* out, long long rows,
+                                                 long long cols, long long r0, long long c0, bool full_tile) {
+  constexpr int RXP = (RX + 3) / 4 * 4;
+  constexpr int SW = T2_TW + 2 * RXP, SH = 8 * OY + 2 * RY;
+  constexpr int NGX = (4 + 2 * RXP) / 4;
+  constexpr int FW = 2 * RX + 1, OFF = RXP - RX;
+  constexpr bool GROUPED = (2 * RY + 1) * FW > 33;
+  constexpr int GR = GROUPED ? (33 / FW > 0 ? 33 / FW : 1) : 2 * RY + 1;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  float acc[XS][OY][4];
+  float part[XS][GROUPED ? OY : 1][4];
+#pragma unroll
+  for (int s = 0; s < XS; ++s)
+#pragma unroll
+    for (int o = 0; o < OY; ++o)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) acc[s][o][e] = 0.f;
+
+#pragma unroll
+  for (int ir = 0; ir < OY + 2 * RY; ++ir) {
+    float v[XS][4 * NGX];
+#pragma unroll
+    for (int s = 0; s < XS; ++s) {
+      const float* srow = sm + s * int(Tile2Geom<RY, RX, OY, XS>::BOX_STRIDE / 4) + (ty * OY + ir) * SW + tx * 4;
+#pragma unroll
+      for (int g = 0; g < NGX; ++g) {
+        const float4 t = *reinterpret_cast<const float4*>(srow + 4 * g);
+        v[s][4 * g] = t.x; v[s][4 * g + 1] = t.y; v[s][4 * g + 2] = t.z; v[s][4 * g + 3] = t.w;
+      }
+    }
+#pragma unroll
+    for (int o = 0; o < OY; ++o) {
+      const int a = ir - o;
+      if (a >= 0 && a <= 2 * RY) {
+        if (GROUPED && a % GR == 0) {
+#pragma unroll
+          for (int s = 0; s < XS; ++s)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) part[s][GROUPED ? o : 0][e] = 0.f;
+        }
+#pragma unroll
+        for (int d = 0; d <= FW; ++d) {
+          const float2 wp = P.p[a][d];
+#pragma unroll
+          for (int s = 0; s < XS; ++s) {
+            float* dstp = GROUPED ? part[s][GROUPED ? o : 0] : acc[s][o];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+              const float x = v[s][OFF + d + 2 * q];
+              if (d == 0) dstp[2 * q] = fmaf(wp.x, x, dstp[2 * q]);
+              else if (d == FW) dstp[2 * q + 1] = fmaf(wp.y, x, dstp[2 * q + 1]);
+              else fma2_bcast(dstp[2 * q], dstp[2 * q + 1], wp, x);
+            }
+          }
+        }
+        if (GROUPED && (a % GR == GR - 1 || a == 2 * RY)) {
+#pragma unroll
+          for (int s = 0; s < XS; ++s)
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              acc[s][o][e] = a < GR ? part[s][GROUPED ? o : 0][e] : acc[s][o][e] + part[s][GROUPED ? o : 0][e];
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int s = 0; s < XS; ++s) {
+    const long long oc = c0 + s * T2_TW + tx * 4;
+    if (full_tile) {
+      float* dst = out + (r0 + ty * OY) * cols + oc;
+#pragma unroll
+      for (int o = 0; o < OY; ++o, dst += cols) {
+        uint32_t raw[4] = {__float_as_uint(acc[s][o][0]), __float_as_uint(acc[s][o][1]), __float_as_uint(acc[s][o][2]),
+                           __float_as_uint(acc[s][o][3])};
+        st_stream<4>(dst, raw);
+      }
+    } else {
+#pragma unroll
+      for (int o = 0; o < OY; ++o) {
+        const long long orow = r0 + ty * OY + o;
+        if (orow < rows) {
+          float* dst = out + orow * cols + oc;
+          if (oc + 3 < cols) {
+            uint32_t raw[4] = {__float_as_uint(acc[s][o][0]), __float_as_uint(acc[s][o][1]), __float_as_uint(acc[s][o][2]),
+                               __float_as_uint(acc[s][o][3])};
+            st_stream<4>(dst, raw);
+          } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              if (oc + e < cols) dst[e] = acc[s][o][e];
+          }
+        }
+      }
+    }
+  }
 }
 
 // a thread's 4 (x) by OY (y) outputs from the staged tile, written to `out`.
@@ -265,13 +406,17 @@ overlap2d_tiled_db_kernel(const __grid_constant__ WT W, int edge, float pad, con
 }
 
 // ---- TMA-fed persistent form ("tma_*") -----------------------------------------------------------
-// Block b walks tiles b, b+G, b+2G, ... (G = gridDim.x co-resident blocks). Thread 0 is the producer:
-// one cp.async.bulk.tensor.2d per tile copies the (SH x SW) window into stage (it + STAGES-1) % STAGES
-// and completes on that stage's `full` mbarrier; cells outside the matrix arrive as zeros. Every
-// thread waits on `full`, computes, and each warp arrives on the stage's `empty` mbarrier when it
-// has finished reading; thread 0 waits on `empty` before it refills the stage. There is no block
-// barrier on the interior path, so the 8 warps of a block drift by up to STAGES-1 tiles.
-// (tx, ty) tile coordinates advance by (G mod tiles_x, G div tiles_x) with one carry: no division.
+// G = 148 x occupancy co-resident blocks take tiles from a global counter (dynamic assignment: with a static
+// b, b+G, ... walk the blocks of an SM drift apart - the warp scheduler favours the oldest warps - and the SM ends the
+// kernel with one or two of its blocks already gone; ncu showed 2.1 of 3 blocks resident on average). Thread 0 is the
+// producer: it fetches the next tile id (atomicAdd; the counter is never reset, the host passes its value at launch as
+// `tile_base` and advances its own copy by ntiles: ntiles - G successful fetches + one failing fetch per block), writes the tile's origin into
+// the stage's `coord` slot and issues one cp.async.bulk.tensor.2d per strip that copies the (SH x SW) window into
+// stage (it + STAGES-1) % STAGES and completes on that stage's `full` mbarrier; cells outside the matrix arrive as
+// zeros. Every thread waits on `full`, reads `coord`, computes, and each warp arrives on the stage's `empty` mbarrier
+// when it has finished reading; thread 0 waits on `empty` before it refills the stage. A stage whose `coord` is
+// negative ends the walk. There is no block barrier on the interior path, so the 8 warps of a block drift by up to
+// STAGES-1 tiles.
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
   asm volatile(
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
@@ -280,22 +425,19 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
       : "memory");
 }
 
-template <int RY, int RX, int OY> struct Tile2Geom {
-  static constexpr int RXP = (RX + 3) / 4 * 4;
-  static constexpr int TH = 8 * OY, SW = T2_TW + 2 * RXP, SH = TH + 2 * RY;
-  static constexpr unsigned STAGE_BYTES = unsigned(SH) * SW * 4u;
-  static constexpr unsigned STAGE_STRIDE = (STAGE_BYTES + 127u) / 128u * 128u;
-};
 
-template <int RY, int RX, int OY, typename WT, bool PK, int STAGES>
-__global__ void __launch_bounds__(T2_THREADS)
+// XS > 1 / BX: the broadcast form (compute_tile2_bx; WT = WPairs2D<RY, RX>), XS TMA boxes per stage.
+template <int RY, int RX, int OY, typename WT, bool PK, int STAGES, int XS = 1, bool BX = false, int MINB = 0>
+__global__ void __launch_bounds__(T2_THREADS, MINB)
 overlap2d_tma_kernel(const __grid_constant__ WT W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
-                     const float* in, float* out, int rows, int cols, int tiles_x, int ntiles, int dq, int dr) {
-  using G = Tile2Geom<RY, RX, OY>;
-  constexpr int RXP = G::RXP, TH = G::TH, SW = G::SW, SH = G::SH;
+                     const float* in, float* out, int rows, int cols, int tiles_x, int ntiles, unsigned* tile_ctr,
+                     unsigned tile_base) {
+  using G = Tile2Geom<RY, RX, OY, XS>;
+  constexpr int RXP = G::RXP, TH = G::TH, SW = G::SW, SH = G::SH, TW = G::TW;
   extern __shared__ __align__(128) unsigned char smraw[];
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw + STAGES * G::STAGE_STRIDE);
   uint64_t* empty = full + STAGES;
+  int2* coord = reinterpret_cast<int2*>(empty + STAGES);  // (r0, c0) of the tile in each stage; r0 < 0: no more tiles
   auto stage_ptr = [&](int s) { return reinterpret_cast<float*>(smraw + s * G::STAGE_STRIDE); };
   const int lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
@@ -307,62 +449,65 @@ overlap2d_tma_kernel(const __grid_constant__ WT W, const __grid_constant__ CUten
     mbar_fence_init();
   }
   __syncthreads();
-  int tile = blockIdx.x;
-  if (tile >= ntiles) return;
-  int tyi = tile / tiles_x, txi = tile - tyi * tiles_x;
-  // producer state (used by thread 0 only): next tile to request and its coordinates
-  int ptile = tile, pty = tyi, ptx = txi;
-  auto advance = [&](int& t, int& y, int& x) {
-    t += gridDim.x;
-    x += dr;
-    y += dq;
-    if (x >= tiles_x) {
-      x -= tiles_x;
-      ++y;
+  // thread 0: the first tile is the block's own index, later ids come from the counter (+ gridDim.x); the fetch of tile
+  // k+1 is issued while tile k is requested and examined one iteration later, so its latency overlaps a tile's compute.
+  // The id that ends the walk is examined before any further fetch: exactly one failing fetch per block.
+  unsigned t_next = blockIdx.x;
+  bool exhausted = false;
+  auto produce = [&](int s) {  // thread 0: next tile into stage s, or mark the stage as the end of the walk
+    const unsigned t = t_next;
+    if (!exhausted) exhausted = t >= unsigned(ntiles);
+    if (!exhausted) t_next = atomicAdd(tile_ctr, 1u) - tile_base + gridDim.x;
+    if (!exhausted) {
+      const int y = int(t) / tiles_x, x = int(t) - y * tiles_x;
+      coord[s] = make_int2(y * TH, x * TW);
+      mbar_arrive_expect_tx(full + s, G::STAGE_BYTES);
+#pragma unroll
+      for (int k = 0; k < XS; ++k)
+        tma_load_2d(reinterpret_cast<unsigned char*>(stage_ptr(s)) + k * G::BOX_STRIDE, &tmap, x * TW + k * T2_TW - RXP,
+                    y * TH - RY, full + s);
+    } else {
+      coord[s] = make_int2(-1, 0);
+      mbar_arrive(full + s);
     }
-  };
-  auto request = [&](int s) {  // thread 0: TMA copy of tile (pty, ptx) into stage s
-    mbar_arrive_expect_tx(full + s, G::STAGE_BYTES);
-    tma_load_2d(stage_ptr(s), &tmap, ptx * T2_TW - RXP, pty * TH - RY, full + s);
   };
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int d = 0; d < STAGES - 1; ++d) {
-      if (ptile < ntiles) request(d);
-      advance(ptile, pty, ptx);
-    }
+    for (int d = 0; d < STAGES - 1; ++d) produce(d);
   }
   // zeros are what CONSTANT with pad = 0 wants; any other policy patches the cells outside the matrix
   const bool patch_needed = !(edge == EDGE_CONSTANT && pad == 0.f);
   int s = 0, ph = 0;           // stage and parity of this iteration's `full` wait
   int tgt = STAGES - 1, tph = 1;  // thread 0: stage to refill and parity of its `empty` wait
-  for (int it = 0; tile < ntiles; ++it) {
+  for (int it = 0;; ++it) {
     if (threadIdx.x == 0) {
-      if (ptile < ntiles) {
-        if (it > 0) mbar_wait(empty + tgt, tph);  // every warp has finished reading tile it-1
-        request(tgt);
-      }
-      advance(ptile, pty, ptx);
+      if (it > 0) mbar_wait(empty + tgt, tph);  // every warp has finished reading tile it-1
+      produce(tgt);
     }
     tgt = tgt + 1 == STAGES ? 0 : tgt + 1;
     if (tgt == 0) tph ^= 1;
     mbar_wait(full + s, ph);
-    const int r0 = tyi * TH, c0 = txi * T2_TW;
+    const int2 rc = coord[s];
+    if (rc.x < 0) break;
+    const int r0 = rc.x, c0 = rc.y;
     float* sm = stage_ptr(s);
-    const bool window_inside = r0 - RY >= 0 && r0 + TH + RY <= rows && c0 - RXP >= 0 && c0 + T2_TW + RXP <= cols;
+    const bool window_inside = r0 - RY >= 0 && r0 + TH + RY <= rows && c0 - RXP >= 0 && c0 + TW + RXP <= cols;
     if (!window_inside && patch_needed) {  // block-uniform branch
-      for (int idx = threadIdx.x; idx < SH * SW; idx += T2_THREADS) {
-        const int gy = idx / SW, gx = idx - gy * SW;
-        const int p = r0 - RY + gy, q = c0 - RXP + gx;
-        if (p < 0 || p >= rows || q < 0 || q >= cols) sm[idx] = ext2(in, rows, cols, p, q, edge, pad);
+      for (int idx = threadIdx.x; idx < XS * SH * SW; idx += T2_THREADS) {
+        const int k = idx / (SH * SW), rem = idx - k * (SH * SW);
+        const int gy = rem / SW, gx = rem - gy * SW;
+        const int p = r0 - RY + gy, q = c0 + k * T2_TW - RXP + gx;
+        if (p < 0 || p >= rows || q < 0 || q >= cols) sm[k * int(G::BOX_STRIDE / 4) + rem] = ext2(in, rows, cols, p, q, edge, pad);
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next TMA refill
       __syncthreads();
     }
-    compute_tile2<RY, RX, OY, WT, PK>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
+    if constexpr (BX)
+      compute_tile2_bx<RY, RX, OY, XS>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + TW <= cols);
+    else
+      compute_tile2<RY, RX, OY, WT, PK>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
-    advance(tile, tyi, txi);
     s = s + 1 == STAGES ? 0 : s + 1;
     if (s == 0) ph ^= 1;
   }
@@ -449,7 +594,7 @@ template <int RY, int RX, int OY, typename WT, bool PK, int STAGES>
 cudaError_t launch_tma2(const Launch& L, const WT& w, int edge, float pad, const float* in, float* out, size_t rows,
                         size_t cols) {
   using G = Tile2Geom<RY, RX, OY>;
-  constexpr size_t smem = size_t(STAGES) * G::STAGE_STRIDE + 2 * STAGES * sizeof(uint64_t);
+  constexpr size_t smem = size_t(STAGES) * G::STAGE_STRIDE + 3 * STAGES * sizeof(uint64_t);  // stages, full/empty, coord
   static_assert(smem <= 227 * 1024, "stages do not fit");
   auto kern = overlap2d_tma_kernel<RY, RX, OY, WT, PK, STAGES>;
   static int per_sm = 0;
@@ -466,7 +611,39 @@ cudaError_t launch_tma2(const Launch& L, const WT& w, int edge, float pad, const
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
   kern<<<(unsigned)grid, T2_THREADS, smem, L.stream>>>(w, tmap, edge, pad, in, out, (int)rows, (int)cols, (int)tiles_x,
-                                                        (int)ntiles, int(grid / tiles_x), int(grid % tiles_x));
+                                                        (int)ntiles, L.tile_ctr, *L.tile_next);
+  *L.tile_next += unsigned(ntiles);  // ntiles - grid tiles are fetched from the counter, every block fetches one id past the end
+  ++*L.launches;
+  return cudaGetLastError();
+}
+
+// broadcast form (RX > 0): the weight-pair table is built here, per call
+template <int RY, int RX, int OY, int XS, int STAGES, int MINB>
+cudaError_t launch_tma2_bx(const Launch& L, const Weights2D& w, int edge, float pad, const float* in, float* out,
+                           size_t rows, size_t cols) {
+  using G = Tile2Geom<RY, RX, OY, XS>;
+  using WP = WPairs2D<RY, RX>;
+  constexpr size_t smem = size_t(STAGES) * G::STAGE_STRIDE + 3 * STAGES * sizeof(uint64_t);  // stages, full/empty, coord
+  static_assert(smem <= 227 * 1024, "stages do not fit");
+  auto kern = overlap2d_tma_kernel<RY, RX, OY, WP, false, STAGES, XS, true, MINB>;
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, T2_THREADS, smem) != cudaSuccess || per_sm < 1)
+      return cudaErrorInvalidValue;
+  }
+  CUtensorMap tmap;
+  cudaError_t e = make_tmap_2d(&tmap, in, rows, cols, G::SW, G::SH);
+  if (e != cudaSuccess) return e;
+  WP P;
+  make_wpairs<RY, RX>(P, w.w);
+  const size_t tiles_x = (cols + G::TW - 1) / G::TW;
+  const size_t ntiles = tiles_x * ((rows + G::TH - 1) / G::TH);
+  size_t grid = size_t(L.sms) * per_sm;
+  if (grid > ntiles) grid = ntiles;
+  kern<<<(unsigned)grid, T2_THREADS, smem, L.stream>>>(P, tmap, edge, pad, in, out, (int)rows, (int)cols, (int)tiles_x,
+                                                        (int)ntiles, L.tile_ctr, *L.tile_next);
+  *L.tile_next += unsigned(ntiles);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -484,6 +661,14 @@ cudaError_t launch_tiled_any(const Launch& L, int v, const WT& w, int edge, floa
     case 5: return launch_tma2<RY, RX, 4, WT, PK, 3>(L, w, edge, pad, in, out, rows, cols);
     case 6: return launch_tma2<RY, RX, 8, WT, PK, RX == 0 ? 3 : 2>(L, w, edge, pad, in, out, rows, cols);
     case 7: return launch_tma2<RY, RX, 4, WT, PK, 2>(L, w, edge, pad, in, out, rows, cols);  // 2 stages: 5 resident blocks
+  }
+  if constexpr (RX > 0) {  // broadcast-FFMA2 forms (dense 2D only)
+    switch (v) {
+      case 8: return launch_tma2_bx<RY, RX, 4, 1, 3, 3>(L, w, edge, pad, in, out, rows, cols);
+      case 9: return launch_tma2_bx<RY, RX, 4, 1, 2, 1>(L, w, edge, pad, in, out, rows, cols);
+      case 10: return launch_tma2_bx<RY, RX, 4, 2, 2, 2>(L, w, edge, pad, in, out, rows, cols);
+      case 11: return launch_tma2_bx<RY, RX, 2, 2, 3, 3>(L, w, edge, pad, in, out, rows, cols);
+    }
   }
   return cudaErrorInvalidValue;
 }

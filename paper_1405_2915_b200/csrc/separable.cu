@@ -21,7 +21,7 @@ template <int R, int OY, int STAGES> struct SepGeom {
   using G = Tile2Geom<R, R, OY>;
   static constexpr int RXP = G::RXP, TH = G::TH, SW = G::SW, SH = G::SH;
   static constexpr unsigned T_BYTES = unsigned(SH) * T2_TW * 4u;
-  static constexpr size_t SMEM = STAGES * size_t(G::STAGE_STRIDE) + T_BYTES + 4 * sizeof(uint64_t);
+  static constexpr size_t SMEM = STAGES * size_t(G::STAGE_STRIDE) + T_BYTES + 6 * sizeof(uint64_t);  // + full/empty, coord
 };
 
 // STAGES = 2: the window of tile i+1 is requested while tile i is in phase A (full/empty mbarriers).
@@ -31,7 +31,7 @@ template <int R, int OY, int STAGES>
 __global__ void __launch_bounds__(T2_THREADS)
 separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_constant__ Weights1D Wcol,
                        const __grid_constant__ CUtensorMap tmap, int edge, float pad, const float* in, float* out,
-                       int rows, int cols, int tiles_x, int ntiles, int dq, int dr) {
+                       int rows, int cols, int tiles_x, int ntiles, unsigned* tile_ctr, unsigned tile_base) {
   using S = SepGeom<R, OY, STAGES>;
   using G = typename S::G;
   constexpr int RXP = S::RXP, TH = S::TH, SW = S::SW, SH = S::SH;
@@ -40,6 +40,7 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
   float* T = reinterpret_cast<float*>(smraw + STAGES * G::STAGE_STRIDE);
   uint64_t* full = reinterpret_cast<uint64_t*>(smraw + STAGES * G::STAGE_STRIDE + S::T_BYTES);
   uint64_t* empty = full + 2;
+  int2* coord = reinterpret_cast<int2*>(empty + 2);  // (r0, c0) of the tile in each stage; r0 < 0: no more tiles
   auto stage_ptr = [&](int s) { return reinterpret_cast<float*>(smraw + s * G::STAGE_STRIDE); };
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   if (threadIdx.x == 0) {
@@ -50,40 +51,37 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
     mbar_fence_init();
   }
   __syncthreads();
-  int tile = blockIdx.x;
-  if (tile >= ntiles) return;
-  int tyi = tile / tiles_x, txi = tile - tyi * tiles_x;
-  int ptile = tile, pty = tyi, ptx = txi;
-  auto advance = [&](int& t, int& y, int& x) {
-    t += gridDim.x;
-    x += dr;
-    y += dq;
-    if (x >= tiles_x) {
-      x -= tiles_x;
-      ++y;
+  // dynamic tile assignment (see overlap2d_tma_kernel): first tile = block index, then a global counter, fetched one
+  // tile ahead of its use; exactly one failing fetch per block
+  unsigned t_next = blockIdx.x;
+  bool exhausted = false;
+  auto produce = [&](int s) {  // thread 0
+    const unsigned t = t_next;
+    if (!exhausted) exhausted = t >= unsigned(ntiles);
+    if (!exhausted) t_next = atomicAdd(tile_ctr, 1u) - tile_base + gridDim.x;
+    if (!exhausted) {
+      const int y = int(t) / tiles_x, x = int(t) - y * tiles_x;
+      coord[s] = make_int2(y * TH, x * T2_TW);
+      mbar_arrive_expect_tx(full + s, G::STAGE_BYTES);
+      tma_load_2d(stage_ptr(s), &tmap, x * T2_TW - RXP, y * TH - R, full + s);
+    } else {
+      coord[s] = make_int2(-1, 0);
+      mbar_arrive(full + s);
     }
   };
-  auto request = [&](int s) {
-    mbar_arrive_expect_tx(full + s, G::STAGE_BYTES);
-    tma_load_2d(stage_ptr(s), &tmap, ptx * T2_TW - RXP, pty * TH - R, full + s);
-  };
-  if (threadIdx.x == 0) {
-    request(0);
-    advance(ptile, pty, ptx);
-  }
+  if (threadIdx.x == 0) produce(0);
   const bool patch_needed = !(edge == EDGE_CONSTANT && pad == 0.f);
   int s = 0, ph = 0, tph = 1;
-  for (int it = 0; tile < ntiles; ++it) {
+  for (int it = 0;; ++it) {
     if (STAGES == 2 && threadIdx.x == 0) {
-      if (ptile < ntiles) {
-        if (it > 0) mbar_wait(empty + (s ^ 1), tph);
-        request(s ^ 1);
-      }
-      advance(ptile, pty, ptx);
+      if (it > 0) mbar_wait(empty + (s ^ 1), tph);
+      produce(s ^ 1);
     }
     if (s == 0) tph ^= 1;  // parity of the next wait on an `empty` barrier (see overlap2d_tma_kernel)
     mbar_wait(full + s, ph);
-    const int r0 = tyi * TH, c0 = txi * T2_TW;
+    const int2 rc = coord[s];
+    if (rc.x < 0) break;
+    const int r0 = rc.x, c0 = rc.y;
     float* sm = stage_ptr(s);
     const bool window_inside = r0 - R >= 0 && r0 + TH + R <= rows && c0 - RXP >= 0 && c0 + T2_TW + RXP <= cols;
     if (!window_inside && patch_needed) {
@@ -124,14 +122,10 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
       if (lane == 0) mbar_arrive(empty + s);  // this warp no longer reads the X stage
     }
     __syncthreads();  // T is complete (and, with one stage, nobody reads the window any more)
-    if (STAGES == 1 && threadIdx.x == 0) {
-      if (ptile < ntiles) request(0);
-      advance(ptile, pty, ptx);
-    }
+    if (STAGES == 1 && threadIdx.x == 0) produce(0);  // everybody has read coord[0] and the window
     // ---- phase B: column pass from T (a (2R+1) x 1 filter on a tile without x halo) ----
     compute_tile2<R, 0, OY, Weights1D, true>(T, Wcol, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
     __syncthreads();  // T is rewritten by the next tile's phase A
-    advance(tile, tyi, txi);
     if constexpr (STAGES == 2) {
       s ^= 1;
       if (s == 0) ph ^= 1;
@@ -161,8 +155,8 @@ cudaError_t launch_sep(const Launch& L, const Weights1D& wrow, const Weights1D& 
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
   kern<<<(unsigned)grid, T2_THREADS, S::SMEM, L.stream>>>(wrow, wcol, tmap, edge, pad, in, out, (int)rows, (int)cols,
-                                                          (int)tiles_x, (int)ntiles, int(grid / tiles_x),
-                                                          int(grid % tiles_x));
+                                                          (int)tiles_x, (int)ntiles, L.tile_ctr, *L.tile_next);
+  *L.tile_next += unsigned(ntiles);  // ntiles - grid ids fetched from the counter + one failing fetch per block
   ++*L.launches;
   return cudaGetLastError();
 }
