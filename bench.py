@@ -257,7 +257,10 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
     x0 = I.uniform01_f32(I.config_seed(5, 1), n)
     w = I.positive_weights_f32(I.config_seed(3, 14), 9)
 
-    def run(k):
+    def run(k, lag=0):
+        """lag = 0: blocking skel_reduce every iteration. lag > 0: skel_reduce_async, the scalar of iteration i is
+        waited for at iteration i + lag (skel_future_wait: an event behind THAT kernel), so `lag` iterations stay in
+        flight and the host never drains the stream."""
         a, b = ctx.vector_from(x0), ctx.vector(n)
         ctx.reset_stats()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -265,11 +268,19 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
         t0 = time.perf_counter()
         e0.record()
         s = 0.0
+        futs = []
         for _ in range(k):
             ctx.map(S.FN_MULT, 1.0001, a, None, a)
             ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
-            s = ctx.reduce(S.FN_ADD, b)
+            if lag:
+                futs.append(ctx.reduce_async(S.FN_ADD, b))
+                if len(futs) > lag:
+                    s = futs.pop(0).result()
+            else:
+                s = ctx.reduce(S.FN_ADD, b)
             a, b = b, a
+        for f in futs:
+            s = f.result()
         e1.record()
         torch.cuda.synchronize()
         wall = time.perf_counter() - t0
@@ -283,10 +294,13 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
     # the same loop with cross-call fusion on (skel_ctx_set_fusion): Map -> MapOverlap1D -> Reduce is ONE
     # kernel, 12 instead of 20 bytes per element (every reduce() ends with a scalar read-back, which also
     # flushes: the events above see every launch)
+    wall_la, dev_la, st_la, s_la = run(iters, lag=2)
     ctx.set_fusion(True)
     try:
         run(3)
         wall_f, dev_f, st_f, s_f = run(iters)
+        run(3, lag=2)
+        wall_fa, dev_fa, st_fa, s_fa = run(iters, lag=2)
     finally:
         ctx.set_fusion(False)
     ctx.set_coherence(S.EAGER)
@@ -302,11 +316,20 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
                  "h2d_bytes_total": st_l["h2d_bytes"], "d2h_bytes_total": st_l["d2h_bytes"],
                  "h2d_count": st_l["h2d_count"], "d2h_count": st_l["d2h_count"],
                  "scalar_readbacks": st_l["scalar_d2h_count"], "h2d_elided": st_l["h2d_elided"]},
+        "lazy_async": {"wall_ms_per_iter": round(wall_la / iters * 1e3, 4), "device_ms_per_iter": round(dev_la / iters, 4),
+                       "iterations_in_flight": 2, "scalar_readbacks": st_la["scalar_d2h_count"],
+                       "same_scalar_as_blocking": bool(s_la == s_l),
+                       "note": "skel_reduce_async + skel_future_wait two iterations late: the host waits on the event "
+                               "behind each reducing kernel, never on the whole stream"},
         "fused": {"wall_ms_per_iter": round(wall_f / iters * 1e3, 4), "device_ms_per_iter": round(dev_f / iters, 4),
                   "bytes_per_elem": 12, "GB/s_device_at_12B": round(12 * n / (dev_f / iters * 1e-3) / 1e9, 1),
                   "launches_per_iter": st_f["launches"] / iters, "fused_launches": st_f["fused_launches"],
                   "h2d_count": st_f["h2d_count"], "d2h_count": st_f["d2h_count"],
                   "speedup_over_unfused_device": round(dev_l / dev_f, 3), "last_scalar": s_f},
+        "fused_async": {"wall_ms_per_iter": round(wall_fa / iters * 1e3, 4), "device_ms_per_iter": round(dev_fa / iters, 4),
+                        "iterations_in_flight": 2, "launches_per_iter": st_fa["launches"] / iters,
+                        "scalar_readbacks": st_fa["scalar_d2h_count"], "same_scalar_as_blocking": bool(s_fa == s_f),
+                        "GB/s_wall_at_12B": round(12 * n / (wall_fa / iters) / 1e9, 1)},
         "eager": {"iterations_run": eager_iters, "wall_ms_per_iter": round(wall_e / eager_iters * 1e3, 3),
                   "h2d_bytes_per_iter": st_e["h2d_bytes"] // eager_iters, "d2h_bytes_per_iter": st_e["d2h_bytes"] // eager_iters,
                   "transfers_per_iter": (st_e["h2d_count"] + st_e["d2h_count"]) // eager_iters},

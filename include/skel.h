@@ -90,6 +90,7 @@ typedef enum {
 typedef struct skel_ctx skel_ctx;
 typedef struct skel_vector skel_vector;
 typedef struct skel_matrix skel_matrix;
+typedef struct skel_future skel_future; /* the scalar result of a skel_*_async call (below) */
 
 /* ---- context ---------------------------------------------------------------------------- */
 /* Device-memory callbacks (e.g. PyTorch's caching allocator). alloc returns a device pointer
@@ -211,6 +212,21 @@ skel_status skel_mapreduce(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double 
                            const skel_vector* in1, void* host_result);
 skel_status skel_mapreduce_to(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double c, const skel_vector* in0,
                               const skel_vector* in1, skel_vector* out, size_t out_index);
+
+/* Asynchronous forms ("asynchronous skeleton calls ... allow the runtime to run ahead", L116 "data
+ * dependence tracking"): the call returns at once with a future; the scalar lands in a pinned host slot the kernel
+ * writes directly (zero-copy). skel_future_wait blocks until THAT reduction has finished - an event recorded right
+ * after its kernel, not the whole stream - and copies one element of the element type to HOST memory `host_result`;
+ * it may be called more than once. skel_future_ready polls (*ready = 1 when the result is there). A loop that calls
+ * Map -> MapOverlap -> skel_reduce_async and waits for the futures afterwards (or a few iterations late) keeps
+ * several iterations in flight. Futures belong to the context, must be destroyed before it (SKEL_ERR_BUSY otherwise),
+ * and at most 1024 may be outstanding per context (SKEL_ERR_BUSY). Same checks and results as the blocking forms. */
+skel_status skel_reduce_async(skel_ctx* ctx, skel_fn op, const skel_vector* in, skel_future** out);
+skel_status skel_mapreduce_async(skel_ctx* ctx, skel_fn map_f, skel_fn red_op, double c, const skel_vector* in0,
+                                 const skel_vector* in1, skel_future** out);
+skel_status skel_future_wait(skel_future* f, void* host_result);
+skel_status skel_future_ready(skel_future* f, int* ready);
+skel_status skel_future_destroy(skel_future* f);
 
 /* Row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] for every row i.
  * `out` has `rows` elements of the matrix's element type (f32 or i32; i32 add / mult wrap modulo 2^32);

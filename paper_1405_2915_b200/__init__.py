@@ -7,4 +7,4 @@ loudly if it has not been built. The seeded input generators live OUTSIDE the pa
 arm of ``bench.py`` never map the library they check.
 """
 from . import binding as skel  # noqa: F401  (raises ImportError when libskel.so is missing)
-from .binding import Context, Matrix, SkelError, SkelInstance, Vector  # noqa: F401
+from .binding import Context, Future, Matrix, SkelError, SkelInstance, Vector  # noqa: F401

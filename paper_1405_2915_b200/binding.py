@@ -98,6 +98,11 @@ _SIGS = {
     "skel_mapreduce_to": ([_vp, _i, _i, _d, _vp, _vp, _vp, _sz], _i),
     "skel_map3": ([_vp, _i, _vp, _vp, _vp, _vp], _i),
     "skel_reduce_rows": ([_vp, _i, _vp, _vp], _i),
+    "skel_reduce_async": ([_vp, _i, _vp, _pp], _i),
+    "skel_mapreduce_async": ([_vp, _i, _i, _d, _vp, _vp, _pp], _i),
+    "skel_future_wait": ([_vp, _vp], _i),
+    "skel_future_ready": ([_vp, C.POINTER(_i)], _i),
+    "skel_future_destroy": ([_vp], _i),
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
@@ -142,6 +147,34 @@ def coherence_step(state: int, actor: int, access: int, mode: int = LAZY):
 
 def variant_names(skeleton: int) -> list[str]:
     return [lib.skel_variant_name(skeleton, v).decode() for v in range(lib.skel_variant_count(skeleton))]
+
+
+class Future:
+    """skel_future: the scalar of a skel_reduce_async / skel_mapreduce_async call (marshalling only)."""
+
+    def __init__(self, ctx: "Context", h, dtype: int):
+        self.ctx, self.h, self.dtype = ctx, h, dtype
+
+    def wait(self):
+        res = (C.c_float if self.dtype == F32 else C.c_int32)()
+        self.ctx.check(lib.skel_future_wait(self.h, C.byref(res)))
+        return res.value
+
+    def ready(self) -> bool:
+        r = C.c_int()
+        self.ctx.check(lib.skel_future_ready(self.h, C.byref(r)))
+        return bool(r.value)
+
+    def destroy(self):
+        if self.h:
+            self.ctx.check(lib.skel_future_destroy(self.h))
+            self.h = None
+
+    def result(self):
+        """wait + destroy"""
+        v = self.wait()
+        self.destroy()
+        return v
 
 
 class Context:
@@ -290,6 +323,16 @@ class Context:
 
     def mapreduce_to(self, map_f: int, red_op: int, c: float, in0, in1, out: "Vector", out_index: int = 0):
         self.check(lib.skel_mapreduce_to(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, out.h, out_index))
+
+    def reduce_async(self, op: int, x: "Vector") -> "Future":
+        h = C.c_void_p()
+        self.check(lib.skel_reduce_async(self.h, op, x.h, C.byref(h)))
+        return Future(self, h, x.dtype)
+
+    def mapreduce_async(self, map_f: int, red_op: int, c: float, in0: "Vector", in1: "Vector | None") -> "Future":
+        h = C.c_void_p()
+        self.check(lib.skel_mapreduce_async(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, C.byref(h)))
+        return Future(self, h, in0.dtype)
 
     def reduce_rows(self, op: int, x: "Matrix", out: "Vector"):
         self.check(lib.skel_reduce_rows(self.h, op, x.h, out.h))

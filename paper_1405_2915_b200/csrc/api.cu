@@ -22,7 +22,8 @@ using namespace skel;
 
 namespace {
 
-constexpr uint32_t MAGIC_CTX = 0x534b4358, MAGIC_VEC = 0x534b5645, MAGIC_MAT = 0x534b4d41;
+constexpr uint32_t MAGIC_CTX = 0x534b4358, MAGIC_VEC = 0x534b5645, MAGIC_MAT = 0x534b4d41, MAGIC_FUT = 0x534b4655;
+constexpr int FUTURE_SLOTS = 1024;  // outstanding skel_future per context (8-byte pinned slots)
 constexpr int FN_IDENT_ = 100;  // same value as skel::FN_IDENT in common.cuh (identity map of plain Reduce)
 
 struct Storage {
@@ -35,7 +36,11 @@ struct Storage {
   int state = ST_UNINIT;
   bool host_held = false;
   int refs = 1;
-  uint64_t last_seq = 0;  // ctx->seq of the last enqueued device operation that touched it
+  // data-dependence tracking: ctx->seq of the last enqueued stream operation that touched the
+  // container in any way / that wrote one of its copies. A host READ waits for the last writer only, a host WRITE
+  // for both; the wait is on the event recorded after THAT operation (EventRing), never on the whole stream.
+  uint64_t last_seq = 0;
+  uint64_t last_write_seq = 0;
   // range-granular coherence: element ranges whose HOST copy is newer than the (otherwise valid) device copy.
   // Non-empty only while the device-valid bit of `state` is set.
   std::vector<ElemRange> host_newer;
@@ -52,7 +57,25 @@ struct Handle {
 
 }  // namespace
 
+// One event per enqueued operation, kept in a ring: slot i holds an event recorded on the context's stream when every
+// operation with sequence number <= seq[i] had been enqueued. To wait for operation q, synchronise on the recorded slot
+// with the smallest seq >= q (the stream is in order: a later event implies the earlier operations). A slot that has
+// been reused only makes the wait conservative, never wrong.
+struct EventRing {
+  static constexpr int N = 64;
+  cudaEvent_t ev[N] = {};
+  uint64_t seq[N] = {};
+  int head = 0;
+};
+
 struct PendingCall;
+struct skel_future {
+  uint32_t magic;
+  skel_ctx* ctx;
+  int slot;      // index of its pinned scalar slot
+  int dtype;
+  uint64_t seq;  // sequence number of the reducing operation
+};
 struct skel_vector : Handle {};
 struct skel_matrix : Handle {};
 
@@ -74,7 +97,14 @@ struct skel_ctx {
   void* d_result = nullptr;  // device slot for scalars returned to the host
   void* h_result = nullptr;      // pinned, mapped host slot for scalars returned to the host ...
   void* h_result_dev = nullptr;  // ... and its device-side address: the reducing kernel stores the scalar straight into it
-  uint64_t seq = 0, synced_seq = 0;
+  uint64_t seq = 0;           // sequence number of the last stream operation issued (launch or copy)
+  uint64_t done_seq = 0;      // every operation <= done_seq is known to have finished
+  uint64_t recorded_seq = 0;  // every operation <= recorded_seq is covered by an event of the ring
+  EventRing ring;
+  // skel_*_async: pinned, mapped scalar slots the reducing kernels write their result into (zero-copy)
+  void* h_slots = nullptr;
+  void* h_slots_dev = nullptr;
+  std::vector<int> free_slots;
   bool sticky = false;
   Plan plan;
   int forced[SKEL_SK_COUNT];
@@ -197,6 +227,8 @@ skel_status ensure_host(skel_ctx* c, Storage* s) {
 }
 
 skel_status flush_pending(skel_ctx* c);
+bool has_pending(const skel_ctx* c);
+skel_status mark_enqueued(skel_ctx* c);
 
 // a prefetch download in flight: block the host until it has landed
 skel_status finish_prefetch(skel_ctx* c, Storage* s) {
@@ -239,13 +271,76 @@ void add_host_newer(Storage* s, size_t begin, size_t end) {
   s->host_newer.resize(cnt);
 }
 
-// wait until every enqueued device operation that touched `s` has finished
-skel_status wait_for(skel_ctx* c, Storage* s) {
-  if (s->last_seq > c->synced_seq) {
-    CU(c, cudaStreamSynchronize(c->stream));
-    c->synced_seq = c->seq;
-  }
+// Every operation issued so far has been enqueued on the stream (nothing is held back): cover them with an event.
+skel_status mark_enqueued(skel_ctx* c) {
+  if (c->recorded_seq == c->seq || has_pending(c)) return SKEL_OK;
+  EventRing& r = c->ring;
+  if (!r.ev[r.head]) CU(c, cudaEventCreateWithFlags(&r.ev[r.head], cudaEventDisableTiming));
+  CU(c, cudaEventRecord(r.ev[r.head], c->stream));
+  r.seq[r.head] = c->seq;
+  c->recorded_seq = c->seq;
+  r.head = (r.head + 1) % EventRing::N;
   return SKEL_OK;
+}
+
+// the recorded event that covers operation q (the one with the smallest seq >= q), or nullptr when q is known to have
+// finished; operations not yet covered by an event are launched / covered first
+skel_status event_for(skel_ctx* c, uint64_t q, cudaEvent_t* ev, uint64_t* ev_seq) {
+  *ev = nullptr;
+  *ev_seq = 0;
+  if (q <= c->done_seq) return SKEL_OK;
+  if (q > c->recorded_seq) {
+    skel_status st = flush_pending(c);
+    if (st != SKEL_OK) return st;
+    st = mark_enqueued(c);
+    if (st != SKEL_OK) return st;
+  }
+  const EventRing& r = c->ring;
+  int best = -1;
+  for (int i = 0; i < EventRing::N; ++i)
+    if (r.ev[i] && r.seq[i] >= q && (best < 0 || r.seq[i] < r.seq[best])) best = i;
+  if (best < 0) return fail(c, SKEL_ERR_CUDA, "internal: no event covers a pending operation");
+  *ev = r.ev[best];
+  *ev_seq = r.seq[best];
+  return SKEL_OK;
+}
+
+// block the host until operation `q` (and, the stream being in order, everything before it) has finished
+skel_status wait_seq(skel_ctx* c, uint64_t q) {
+  cudaEvent_t ev;
+  uint64_t ev_seq;
+  skel_status st = event_for(c, q, &ev, &ev_seq);
+  if (st != SKEL_OK || !ev) return st;
+  CU(c, cudaEventSynchronize(ev));
+  if (ev_seq > c->done_seq) c->done_seq = ev_seq;
+  return SKEL_OK;
+}
+
+// Download elements [offset, offset + count) of `s` to its host copy on the context's COPY stream, ordered after the
+// last operation that wrote the container (its event), not after everything enqueued on the compute stream: a host
+// read of a container whose producer has finished does not wait for unrelated kernels enqueued since. s->d2h_done
+// fires when the data has landed; until then a device write to the container waits for it (order_after_prefetch).
+skel_status start_download(skel_ctx* c, Storage* s, size_t offset, size_t count) {
+  if (!c->copy_stream) CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+  cudaEvent_t produced;
+  uint64_t produced_seq;
+  skel_status st = event_for(c, s->last_write_seq, &produced, &produced_seq);
+  if (st != SKEL_OK) return st;
+  if (produced) CU(c, cudaStreamWaitEvent(c->copy_stream, produced, 0));
+  const size_t es = esize(s->dtype);
+  CU(c, cudaMemcpyAsync(static_cast<char*>(s->host) + offset * es, static_cast<char*>(s->dev) + offset * es, count * es,
+                        cudaMemcpyDeviceToHost, c->copy_stream));
+  if (!s->d2h_done) CU(c, cudaEventCreateWithFlags(&s->d2h_done, cudaEventDisableTiming));
+  CU(c, cudaEventRecord(s->d2h_done, c->copy_stream));
+  c->stats.d2h_bytes += count * es;
+  c->stats.d2h_count += 1;
+  return SKEL_OK;
+}
+
+// host access to `s`: a read waits for the last operation that wrote one of its copies, a write for the last one
+// that touched it at all (a device read of the buffer the host is about to overwrite included)
+skel_status wait_for(skel_ctx* c, Storage* s, bool host_writes = true) {
+  return wait_seq(c, host_writes ? s->last_seq : s->last_write_seq);
 }
 
 // ---- containers --------------------------------------------------------------------------------
@@ -284,10 +379,7 @@ skel_status release_handle(Handle* h) {
   flush_pending(c);  // a held-back launch may still reference this container
   if (s->refs == 1) finish_prefetch(c, s);
   if (--s->refs == 0) {
-    if (s->last_seq > c->synced_seq && !c->sticky) {
-      cudaStreamSynchronize(c->stream);
-      c->synced_seq = c->seq;
-    }
+    if (!c->sticky) wait_seq(c, s->last_seq);
     if (s->dev_owned) dev_free(c, s->dev);
     if (s->host) cudaFreeHost(s->host);
     delete s;
@@ -345,12 +437,12 @@ skel_status host_acquire(Handle* h, skel_access mode, void** host_ptr) {
     st = ensure_host(c, s);
     if (st != SKEL_OK) return st;
     if (step.transfer & XFER_D2H) {
-      CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->stream));
-      c->stats.d2h_bytes += s->n * esize(s->dtype);
-      c->stats.d2h_count += 1;
-      s->last_seq = ++c->seq;
+      st = start_download(c, s, 0, s->n);
+      if (st != SKEL_OK) return st;
+      st = finish_prefetch(c, s);
+      if (st != SKEL_OK) return st;
     }
-    st = wait_for(c, s);
+    st = wait_for(c, s, mode != SKEL_READ);
     if (st != SKEL_OK) return st;
   }
   s->state = step.new_state;
@@ -382,17 +474,8 @@ skel_status prefetch_host(Handle* h) {
   if (st != SKEL_OK) return st;
   st = upload_host_newer(c, s);  // ranges the host wrote must not be overwritten by the download
   if (st != SKEL_OK) return st;
-  if (!c->copy_stream) CU(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-  cudaEvent_t produced;
-  CU(c, cudaEventCreateWithFlags(&produced, cudaEventDisableTiming));
-  CU(c, cudaEventRecord(produced, c->stream));            // everything enqueued so far (the producing kernel)
-  CU(c, cudaStreamWaitEvent(c->copy_stream, produced, 0));
-  cudaEventDestroy(produced);                               // released once it has completed
-  CU(c, cudaMemcpyAsync(s->host, s->dev, s->n * esize(s->dtype), cudaMemcpyDeviceToHost, c->copy_stream));
-  CU(c, cudaEventCreateWithFlags(&s->d2h_done, cudaEventDisableTiming));
-  CU(c, cudaEventRecord(s->d2h_done, c->copy_stream));
-  c->stats.d2h_bytes += s->n * esize(s->dtype);
-  c->stats.d2h_count += 1;
+  st = start_download(c, s, 0, s->n);  // ordered after the container's last writer (the producing kernel)
+  if (st != SKEL_OK) return st;
   s->state = ST_SHARED;  // valid once d2h_done has fired: every host access waits for it
   return SKEL_OK;
 }
@@ -425,13 +508,12 @@ skel_status host_acquire_range(Handle* h, skel_access mode, size_t offset, size_
         if (st != SKEL_OK) return st;
         break;
       }
-    CU(c, cudaMemcpyAsync(static_cast<char*>(s->host) + offset * es, static_cast<char*>(s->dev) + offset * es, count * es,
-                          cudaMemcpyDeviceToHost, c->stream));
-    c->stats.d2h_bytes += count * es;
-    c->stats.d2h_count += 1;
-    s->last_seq = ++c->seq;
+    st = start_download(c, s, offset, count);
+    if (st != SKEL_OK) return st;
+    st = finish_prefetch(c, s);
+    if (st != SKEL_OK) return st;
   }
-  st = wait_for(c, s);  // also orders a host write after device reads of the host buffer that are still in flight
+  st = wait_for(c, s, mode != SKEL_READ);  // a host write also waits for device reads of the host buffer still in flight
   if (st != SKEL_OK) return st;
   if (mode != SKEL_READ && dev_valid) add_host_newer(s, offset, offset + count);
   s->host_held = true;
@@ -520,10 +602,11 @@ skel_status publish_all(skel_ctx* c, OperandSet& set) {
     }
     s->state = o.step.new_state;
     s->last_seq = seq;
+    if (o.access != ACC_READ || (o.step.transfer & (XFER_H2D | XFER_D2H))) s->last_write_seq = seq;
   }
   c->stats.launches += c->launches;
   c->launches = 0;
-  return SKEL_OK;
+  return mark_enqueued(c);  // no-op while the launch is held back (fusion): flush_pending records it
 }
 
 // ---- calls, variants ---------------------------------------------------------------------------
@@ -748,6 +831,8 @@ int chain_kind(const skel_ctx* c, const Call& k) {
   return 0;
 }
 
+bool has_pending(const skel_ctx* c) { return !c->pending.empty(); }
+
 skel_status flush_pending(skel_ctx* c) {
   if (c->pending.empty()) return SKEL_OK;
   std::vector<PendingCall> q;
@@ -804,7 +889,7 @@ skel_status flush_pending(skel_ctx* c) {
       c->stats.fused_calls += q.size();
       c->stats.launches += c->launches;
       c->launches = 0;
-      return SKEL_OK;
+      return mark_enqueued(c);
     }
   }
   for (const PendingCall& p : q) {
@@ -813,7 +898,7 @@ skel_status flush_pending(skel_ctx* c) {
   }
   c->stats.launches += c->launches;
   c->launches = 0;
-  return SKEL_OK;
+  return mark_enqueued(c);
 }
 
 skel_status run_call(skel_ctx* c, const Call& k) {
@@ -859,19 +944,21 @@ skel_status scalar_to_host(skel_ctx* c, int dtype, void* host_result) {
   skel_status fst = flush_pending(c);
   if (fst != SKEL_OK) return fst;
   // zero-copy: the kernel's last block wrote the scalar into the mapped host slot (no device-to-host copy to
-  // enqueue and wait for); visible to the host once the stream has drained
-  CU(c, cudaStreamSynchronize(c->stream));
-  c->synced_seq = c->seq;
+  // enqueue and wait for); visible to the host once the event recorded after the reducing kernel has fired
+  skel_status wst = wait_seq(c, c->seq);
+  if (wst != SKEL_OK) return wst;
   memcpy(host_result, c->h_result, esize(dtype));
   c->stats.scalar_d2h_count += 1;
   return SKEL_OK;
 }
 
 skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op, double cval, const skel_vector* in0,
-                           const skel_vector* in1, void* host_result, skel_vector* out, size_t out_index) {
+                           const skel_vector* in1, void* host_result, skel_vector* out, size_t out_index,
+                           skel_future** fut = nullptr) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (fut) *fut = nullptr;
   if (!vec_ok(in0) || (in1 && !vec_ok(in1))) return fail(c, SKEL_ERR_INVALID_ARG, "bad input handle");
-  if (!host_result && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "no result destination");
+  if (!host_result && !fut && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "no result destination");
   if (!red_op_ok(red_op)) return fail(c, SKEL_ERR_UNSUPPORTED, "reduce operator must be ADD, MULT or MAX");
   if (!plain_reduce && !map_fn_ok(map_f)) return fail(c, SKEL_ERR_UNSUPPORTED, "map function must be ADD, MULT, MAX or SAXPY");
   if (!plain_reduce && map_f == SKEL_FN_SAXPY && !in1) return fail(c, SKEL_ERR_INVALID_ARG, "SAXPY needs in1");
@@ -902,16 +989,35 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   if (out) set.add(out->st, (out->st->n == 1 || out->st->state == ST_UNINIT) ? ACC_WRITE : ACC_READWRITE);
   st = acquire_all(c, set);
   if (st != SKEL_OK) return st;
+  int slot = -1;
+  if (fut) {  // a pinned, mapped 8-byte slot of the context's pool for this result
+    if (!c->h_slots) {
+      CU(c, cudaHostAlloc(&c->h_slots, size_t(FUTURE_SLOTS) * 8, cudaHostAllocMapped));
+      CU(c, cudaHostGetDevicePointer(&c->h_slots_dev, c->h_slots, 0));
+      for (int i = FUTURE_SLOTS - 1; i >= 0; --i) c->free_slots.push_back(i);
+    }
+    if (c->free_slots.empty()) return fail(c, SKEL_ERR_BUSY, "too many outstanding futures (destroy some)");
+    slot = c->free_slots.back();
+  }
   k.in0 = a->dev;
   k.in1 = b ? b->dev : nullptr;
   k.n = a->n;
-  k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype)) : c->h_result_dev;
+  k.out = out ? static_cast<void*>(static_cast<char*>(out->st->dev) + out_index * esize(a->dtype))
+              : (fut ? static_cast<void*>(static_cast<char*>(c->h_slots_dev) + size_t(slot) * 8) : c->h_result_dev);
   k.in_st = a;
   k.out_st = out ? out->st : nullptr;
   st = run_call(c, k);
   if (st != SKEL_OK) return st;
   st = publish_all(c, set);
   if (st != SKEL_OK) return st;
+  if (fut) {
+    skel_future* f = new (std::nothrow) skel_future{MAGIC_FUT, c, slot, a->dtype, c->seq};
+    if (!f) return fail(c, SKEL_ERR_OOM, "host allocation failed");
+    c->free_slots.pop_back();
+    ++c->live;
+    *fut = f;
+    return SKEL_OK;
+  }
   if (host_result) return scalar_to_host(c, a->dtype, host_result);
   return SKEL_OK;
 }
@@ -969,7 +1075,7 @@ skel_status skel_ctx_create(void* cuda_stream, skel_alloc_fn alloc, skel_free_fn
 
 skel_status skel_ctx_destroy(skel_ctx* c) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
-  if (c->live > 0) return fail(c, SKEL_ERR_BUSY, "containers of this context are still alive");
+  if (c->live > 0) return fail(c, SKEL_ERR_BUSY, "containers or futures of this context are still alive");
   if (c->dev_ready) {
     flush_pending(c);
     cudaStreamSynchronize(c->stream);
@@ -982,6 +1088,9 @@ skel_status skel_ctx_destroy(skel_ctx* c) {
     cudaFree(c->scratch.partials);
     if (c->scratch.scan_state) cudaFree(c->scratch.scan_state);
     cudaFreeHost(c->h_result);
+    if (c->h_slots) cudaFreeHost(c->h_slots);
+    for (cudaEvent_t e : c->ring.ev)
+      if (e) cudaEventDestroy(e);
   }
   c->magic = 0;
   delete c;
@@ -996,7 +1105,7 @@ skel_status skel_ctx_sync(skel_ctx* c) {
   if (st != SKEL_OK) return st;
   CU(c, cudaStreamSynchronize(c->stream));
   if (c->copy_stream) CU(c, cudaStreamSynchronize(c->copy_stream));  // prefetch downloads in flight
-  c->synced_seq = c->seq;
+  c->done_seq = c->seq;
   return SKEL_OK;
 }
 
@@ -1266,6 +1375,68 @@ skel_status skel_mapreduce_to(skel_ctx* c, skel_fn map_f, skel_fn red_op, double
                               const skel_vector* in1, skel_vector* out, size_t out_index) {
   if (ctx_ok(c) && !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad result vector");
   return mapreduce_impl(c, false, map_f, red_op, cval, in0, in1, nullptr, out, out_index);
+}
+
+skel_status skel_reduce_async(skel_ctx* c, skel_fn op, const skel_vector* in, skel_future** out) {
+  if (ctx_ok(c) && !out) return fail(c, SKEL_ERR_INVALID_ARG, "out is NULL");
+  return mapreduce_impl(c, true, 0, op, 0.0, in, nullptr, nullptr, nullptr, 0, out);
+}
+
+skel_status skel_mapreduce_async(skel_ctx* c, skel_fn map_f, skel_fn red_op, double cval, const skel_vector* in0,
+                                 const skel_vector* in1, skel_future** out) {
+  if (ctx_ok(c) && !out) return fail(c, SKEL_ERR_INVALID_ARG, "out is NULL");
+  return mapreduce_impl(c, false, map_f, red_op, cval, in0, in1, nullptr, nullptr, 0, out);
+}
+
+skel_status skel_future_wait(skel_future* f, void* host_result) {
+  if (!f || f->magic != MAGIC_FUT) return SKEL_ERR_INVALID_ARG;
+  skel_ctx* c = f->ctx;
+  if (!host_result) return fail(c, SKEL_ERR_INVALID_ARG, "host_result is NULL");
+  if (c->sticky) return SKEL_ERR_CUDA;
+  skel_status st = wait_seq(c, f->seq);  // the event recorded after the reducing kernel, not the whole stream
+  if (st != SKEL_OK) return st;
+  memcpy(host_result, static_cast<char*>(c->h_slots) + size_t(f->slot) * 8, esize(f->dtype));
+  c->stats.scalar_d2h_count += 1;
+  return SKEL_OK;
+}
+
+skel_status skel_future_ready(skel_future* f, int* ready) {
+  if (!f || f->magic != MAGIC_FUT) return SKEL_ERR_INVALID_ARG;
+  skel_ctx* c = f->ctx;
+  if (!ready) return fail(c, SKEL_ERR_INVALID_ARG, "ready is NULL");
+  *ready = 0;
+  if (f->seq <= c->done_seq) {
+    *ready = 1;
+    return SKEL_OK;
+  }
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  st = mark_enqueued(c);
+  if (st != SKEL_OK) return st;
+  const EventRing& r = c->ring;
+  int best = -1;
+  for (int i = 0; i < EventRing::N; ++i)
+    if (r.ev[i] && r.seq[i] >= f->seq && (best < 0 || r.seq[i] < r.seq[best])) best = i;
+  if (best < 0) return SKEL_OK;
+  const cudaError_t e = cudaEventQuery(r.ev[best]);
+  if (e == cudaSuccess) {
+    if (r.seq[best] > c->done_seq) c->done_seq = r.seq[best];
+    *ready = 1;
+  } else if (e != cudaErrorNotReady) {
+    return cuda_fail(c, e, "cudaEventQuery");
+  }
+  return SKEL_OK;
+}
+
+skel_status skel_future_destroy(skel_future* f) {
+  if (!f || f->magic != MAGIC_FUT) return SKEL_ERR_INVALID_ARG;
+  skel_ctx* c = f->ctx;
+  if (!c->sticky) wait_seq(c, f->seq);  // the kernel may still be about to write the slot
+  c->free_slots.push_back(f->slot);
+  --c->live;
+  f->magic = 0;
+  delete f;
+  return SKEL_OK;
 }
 
 skel_status skel_reduce_rows(skel_ctx* c, skel_fn op, const skel_matrix* in, skel_vector* out) {

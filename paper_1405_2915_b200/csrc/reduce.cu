@@ -5,7 +5,10 @@
 // one partial per block; the block that draws the last ticket folds the partials in a fixed order
 // (bitwise deterministic for a given n and variant; no floating-point atomics). The ticket is an
 // atomicInc that wraps to 0, so no memset is needed between calls. The "two_pass" variants write
-// the partials and fold them in a second tiny kernel instead.
+// the partials and fold them in a second tiny kernel instead. The "chunk*" variants launch one block per contiguous
+// chunk of the input (32 / 64 / 128 KB per operand, at most MAX_PARTIALS chunks) instead of 148 x k persistent blocks
+// with a strided tile walk: the hardware block scheduler then balances the SMs (co-resident persistent blocks drift
+// apart and an SM ends the kernel half empty), and the partial of a chunk depends on (n, variant) only: deterministic.
 #include "common.cuh"
 #include "kernels.hpp"
 #include <string.h>
@@ -26,7 +29,8 @@ __device__ __forceinline__ void fold_partials(const T* partials, unsigned count,
 
 template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U, bool SINGLE_PASS>
 __global__ void __launch_bounds__(RED_THREADS)
-mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigned* ticket, T* result) {
+mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigned* ticket, T* result,
+                 unsigned tiles_per_block /* 0: strided walk of a persistent grid; k: block b owns tiles b k .. b k + k - 1 */) {
   __shared__ T smem[32];
   __shared__ bool is_last;
   constexpr size_t TILE = size_t(RED_THREADS) * V * U;
@@ -35,7 +39,10 @@ mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigne
 #pragma unroll
   for (int j = 0; j < V; ++j) acc[j] = identity<T, OP>();
 
-  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  const size_t first = tiles_per_block ? size_t(blockIdx.x) * tiles_per_block : blockIdx.x;
+  const size_t step = tiles_per_block ? 1 : gridDim.x;
+  const size_t last = tiles_per_block ? (first + tiles_per_block < ntiles ? first + tiles_per_block : ntiles) : ntiles;
+  for (size_t tile = first; tile < last; tile += step) {
     const size_t base = tile * TILE + size_t(threadIdx.x) * V;
     if (base + (U - 1) * size_t(RED_THREADS) * V + V <= n) {
       uint32_t a[U][V], b[U][V];
@@ -96,7 +103,7 @@ __global__ void __launch_bounds__(RED_THREADS) fold_kernel(const T* partials, un
   fold_partials<T, OP>(partials, count, result, smem);
 }
 
-struct RedVariant { const char* name; int v, u; bool single; int blocks_per_sm; };
+struct RedVariant { const char* name; int v, u; bool single; int blocks_per_sm; unsigned chunk_bytes = 0; };
 const RedVariant kRedVariants[] = {
     {"scalar_single_pass", 1, 4, true, 8},
     {"v4_u4_single_pass", 4, 4, true, 8},
@@ -104,6 +111,10 @@ const RedVariant kRedVariants[] = {
     {"v4_u4_two_pass", 4, 4, false, 8},
     {"v8_u2_two_pass", 8, 2, false, 8},
     {"v4_u4_single_pass_4bps", 4, 4, true, 4},
+    {"v4_u4_chunk32k", 4, 4, true, 0, 32768},
+    {"v4_u4_chunk64k", 4, 4, true, 0, 65536},
+    {"v4_u4_chunk128k", 4, 4, true, 0, 131072},
+    {"v8_u2_chunk64k", 8, 2, true, 0, 65536},
 };
 constexpr int kNumRedVariants = sizeof(kRedVariants) / sizeof(kRedVariants[0]);
 
@@ -115,16 +126,25 @@ cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, 
   constexpr size_t TILE = size_t(RED_THREADS) * V * U;
   size_t ntiles = (n + TILE - 1) / TILE;
   size_t grid = size_t(L.sms) * rv.blocks_per_sm;
+  unsigned tpb = 0;
+  if (rv.chunk_bytes) {  // one block per chunk; chunks grow when there would be more than MAX_PARTIALS of them
+    size_t t = rv.chunk_bytes / (TILE * sizeof(T));
+    if (t < 1) t = 1;
+    const size_t need = (ntiles + MAX_PARTIALS - 1) / MAX_PARTIALS;
+    if (t < need) t = need;
+    tpb = (unsigned)t;
+    grid = (ntiles + t - 1) / t;
+  }
   if (grid > ntiles) grid = ntiles;
   if (grid > MAX_PARTIALS) grid = MAX_PARTIALS;
   T* partials = static_cast<T*>(S.partials);
   if (rv.single) {
     mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, true>
-        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result);
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
     ++*L.launches;
   } else {
     mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, false>
-        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result);
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
     fold_kernel<T, OP><<<1, RED_THREADS, 0, L.stream>>>(partials, (unsigned)grid, result);
     *L.launches += 2;
   }

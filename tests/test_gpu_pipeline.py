@@ -199,3 +199,114 @@ def test_uninitialised_read_and_alias_errors(ctx):
         ctx.mapoverlap_1d(np.ones(3, np.float32), 1, S.EDGE_DUPLICATE, 0.0, a, a)  # output aliases input
     a.destroy()
     b.destroy()
+
+
+# ------------------------------------------------------------------ per-container events, asynchronous Reduce
+def test_host_read_waits_for_its_own_producer_not_for_the_stream(ctx):
+    """PAPER.md L116 / L135 (data-dependence tracking, asynchronous calls): a host read of container A returns while
+    long-running work on unrelated containers, enqueued AFTER A's producer, is still in flight."""
+    import torch
+    n_small, n_big = 1000, 1 << 26
+    a, a2 = ctx.vector_from(np.arange(n_small, dtype=np.float32)), ctx.vector(n_small)
+    big = ctx.vector_from(I.uniform_int_i32(5, n_big, 15))
+    out = ctx.vector(n_big, S.I32)
+    ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, big, out)   # upload + warm-up
+    ctx.sync()
+    ctx.map(S.FN_ADD, 1.0, a, None, a2)                 # A's producer: microseconds
+    for _ in range(40):                                 # ~4 ms of unrelated device work behind it
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, big, out)
+    got = a2.numpy()                                    # host READ of a2: waits for the Map's event only
+    still_busy = not torch.cuda.current_stream().query()
+    assert np.array_equal(got, np.arange(n_small, dtype=np.float32) + 1.0)
+    assert still_busy, "the host read drained the whole stream"
+    # a host WRITE of `a` (read by the Map) likewise only waits for the Map
+    a.write(np.zeros(n_small, np.float32))
+    assert not torch.cuda.current_stream().query()
+    ctx.sync()
+    ref = O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, I.uniform_int_i32(5, n_big, 15))
+    assert np.array_equal(out.numpy(), ref)
+    for v in (a, a2, big, out):
+        v.destroy()
+
+
+def test_reduce_async_futures(ctx):
+    import torch
+    n = 300007
+    x = I.uniform_pm1_f32(7001, n)
+    y = I.uniform_pm1_f32(7002, n)
+    v = I.uniform_int_i32(7003, n, 1000)
+    vx, vy, vi = ctx.vector_from(x), ctx.vector_from(y), ctx.vector_from(v)
+    ctx.reset_stats()
+    futs = [ctx.reduce_async(S.FN_ADD, vi), ctx.reduce_async(S.FN_MAX, vi), ctx.reduce_async(S.FN_ADD, vx),
+            ctx.mapreduce_async(S.FN_MULT, S.FN_ADD, 0.0, vx, vy), ctx.mapreduce_async(S.FN_MULT, S.FN_ADD, 2.0, vi, None)]
+    assert ctx.stats()["scalar_d2h_count"] == 0          # nothing has been read back yet
+    assert futs[0].wait() == O.reduce_i32(O.FN_ADD, v)[0]
+    assert futs[0].wait() == O.reduce_i32(O.FN_ADD, v)[0]   # may be waited for again
+    assert futs[1].wait() == O.reduce_i32(O.FN_MAX, v)[0]
+    r, ab = O.reduce_f32(O.FN_ADD, x)
+    assert_reduce_f32(futs[2].wait(), r, ab)
+    r, ab = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, y)
+    assert_reduce_f32(futs[3].wait(), r, ab)
+    assert futs[4].wait() == O.mapreduce_i32(O.FN_MULT, O.FN_ADD, 2, v)
+    assert all(f.ready() for f in futs)
+    assert ctx.stats()["scalar_d2h_count"] == 6
+    # the blocking form still works next to outstanding futures and gives the same bits
+    assert ctx.reduce(S.FN_ADD, vx) == futs[2].wait()
+    # a context with a live future cannot be destroyed; destroying the future releases its slot
+    with pytest.raises(S.SkelError):
+        ctx.check(S.lib.skel_ctx_destroy(ctx.h))
+    for f in futs:
+        f.destroy()
+    # the pool: 1024 outstanding futures, the next one is refused with SKEL_ERR_BUSY and leaves no trace
+    small = ctx.vector_from(np.ones(64, np.float32))
+    many = [ctx.reduce_async(S.FN_ADD, small) for _ in range(1024)]
+    with pytest.raises(S.SkelError):
+        ctx.reduce_async(S.FN_ADD, small)
+    assert all(f.result() == 64.0 for f in many)
+    assert ctx.reduce_async(S.FN_ADD, small).result() == 64.0
+    # ready() turns true without a wait
+    big = ctx.vector_from(I.uniform_int_i32(7004, 1 << 24, 15))
+    f = ctx.reduce_async(S.FN_ADD, big)
+    torch.cuda.synchronize()
+    assert f.ready() and f.result() == O.reduce_i32(O.FN_ADD, I.uniform_int_i32(7004, 1 << 24, 15))[0]
+    for c in (vx, vy, vi, small, big):
+        c.destroy()
+
+
+@pytest.mark.parametrize("fusion", [False, True])
+def test_pipeline_with_futures_keeps_iterations_in_flight_and_gives_the_same_scalars(ctx, fusion):
+    n, iters = (1 << 20) + 37, 12
+    x0 = I.uniform01_f32(I.config_seed(5, 1), n)
+    w = I.positive_weights_f32(I.config_seed(3, 14), 9)
+
+    def run(use_futures):
+        a, b = ctx.vector_from(x0), ctx.vector(n)
+        ctx.reset_stats()
+        out, futs = [], []
+        for _ in range(iters):
+            ctx.map(S.FN_MULT, 1.0001, a, None, a)
+            ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
+            if use_futures:
+                futs.append(ctx.reduce_async(S.FN_ADD, b))
+            else:
+                out.append(ctx.reduce(S.FN_ADD, b))
+            a, b = b, a
+        st_before_wait = ctx.stats()
+        out += [f.result() for f in futs]
+        st = ctx.stats()
+        final = a.numpy().copy()
+        a.destroy()
+        b.destroy()
+        return out, st_before_wait, st, final
+
+    ctx.set_fusion(fusion)
+    try:
+        blocking, _, st_b, final_b = run(False)
+        asynch, st_mid, st_a, final_a = run(True)
+    finally:
+        ctx.set_fusion(False)
+    assert asynch == blocking, "async scalars differ from the blocking ones"
+    assert np.array_equal(final_a, final_b)
+    assert st_mid["scalar_d2h_count"] == 0 and st_a["scalar_d2h_count"] == iters == st_b["scalar_d2h_count"]
+    assert st_a["h2d_count"] == 1 and st_a["d2h_count"] == 0 and st_a["h2d_elided"] == st_b["h2d_elided"]
+    assert st_a["launches"] == st_b["launches"] == (iters if fusion else 3 * iters)
