@@ -549,6 +549,7 @@ def main():
             e1.synchronize()
             ts.append(e0.elapsed_time(e1) * 1e3)
         us = float(np.median(ts))
+        rows_variant = S.variant_names(S.SK_REDUCE_ROWS)[ctx.last_variant()[1]]
         got = rr.numpy()
         ref = d["X"].astype(np.float64).sum(axis=1)
         assert np.all(np.abs(got - ref) <= 1e-5 * np.abs(d["X"]).astype(np.float64).sum(axis=1)), "reduce_rows mismatch"
@@ -568,7 +569,7 @@ def main():
         us3 = float(np.median(t3))
         map3 = {"us": round(us3, 2), "variant": S.variant_names(S.SK_MAP)[ctx.last_variant()[1]], "bytes_per_elem": 16,
                 "GB/s": round(16 * n26 / us3 / 1e3, 1), "frac_measured_hbm": round(16 * n26 / us3 / 1e3 / peak, 4)}
-        reduce_rows = {"us": round(us, 2), "variant": S.variant_names(S.SK_REDUCE_ROWS)[ctx.last_variant()[1]],
+        reduce_rows = {"us": round(us, 2), "variant": rows_variant,
                        "bytes_per_elem": 4, "GB/s": round(4 * m / us / 1e3, 1), "frac_measured_hbm": round(4 * m / us / 1e3 / peak, 4)}
         rr.destroy()
 

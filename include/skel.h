@@ -273,15 +273,25 @@ typedef struct {
   int32_t r0;       /* MapOverlap 1D: r; 2D: ry */
   int32_t r1;       /* 2D: rx */
   int32_t edge;     /* skel_edge */
-  int32_t mode;     /* Scan: skel_scan_mode; Map/MapReduce: 1 if in1 is a vector, 0 if it is the constant */
+  int32_t mode;     /* Scan: skel_scan_mode; Map/MapReduce: 1 if in1 is a vector, 0 if it is the constant;
+                       MapOverlap 1D (row-wise): shape class, 0 = vector, 1 = rows of a matrix */
 } skel_instance;
 
 /* Number of kernel variants of a skeleton and the name of one (static string). */
 int skel_variant_count(int skeleton);
 const char* skel_variant_name(int skeleton, int variant);
-/* Measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), median
- * of `reps` launches timed with CUDA events on the context stream, and store size breakpoints
- * in the context's plan. Where the winner changes between two sampled sizes the interval is
+/* The plan is a dispatch TREE over the call context ("tree-based dispatch structure for fast runtime
+ * lookup"): skeleton -> dtype -> (fn, fn2) -> mode / shape class -> r0 -> r1 -> edge -> size breakpoints. A call whose
+ * own context was never tuned takes, level by level, the nearest tuned child (radii: nearest in log2(r + 1), ties to
+ * the larger one; categorical levels: the first child); skeleton and dtype must match. So r = 5 runs what was tuned
+ * for r = 4, r = 12 what was tuned for r = 16, and only a (skeleton, dtype) without any tuned point falls back to
+ * the built-in preference list. The variant found is used if it is applicable to the call (alignment, shape).
+ *
+ * skel_tune_instance: measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), median
+ * of `reps` launches, variants interleaved, timed with CUDA events on the context stream UNDER THE CONDITIONS OF A
+ * SUSTAINED RUN: operands rotate through arenas larger than the L2 cache (so no launch finds its input there) and
+ * every timed launch is preceded by a writer that leaves the L2 full of dirty lines, as the previous skeleton call
+ * of a real sequence does. Size breakpoints are stored in the context's plan. Where the winner changes between two sampled sizes the interval is
  * bisected (only the two contenders are timed) until it is narrower than 2^(1/4), so breakpoints
  * are not confined to powers of two (adaptive sampling). For matrix skeletons `cols`
  * gives the row length (rows = n/cols); pass 0 for vectors. Blocks. */
@@ -293,6 +303,11 @@ skel_status skel_plan_clear(skel_ctx* ctx);
  * Alignment- or radius-driven fallbacks are applied at launch time and reported by
  * skel_last_variant. */
 skel_status skel_plan_lookup(skel_ctx* ctx, const skel_instance* inst, size_t n, int* variant);
+/* The same, and how it was found: *exact = 1 if the instance's own key has a tuned entry, 0 if the variant was
+ * inherited from the nearest tuned neighbour in the dispatch tree or comes from the preference list
+ * (*variant_from_plan = 0 in the latter case). Pure host code. */
+skel_status skel_plan_explain(skel_ctx* ctx, const skel_instance* inst, size_t n, int* variant, int* exact,
+                              int* variant_from_plan);
 /* Insert one breakpoint by hand: variant `variant` from n >= n_min (until the next breakpoint). */
 skel_status skel_plan_set(skel_ctx* ctx, const skel_instance* inst, size_t n_min, int variant);
 /* Timing table of the last skel_tune_instance: times_us[(k-log2_lo)*nvariants + v], NaN where a

@@ -116,6 +116,7 @@ _SIGS = {
     "skel_plan_clear": ([_vp], _i),
     "skel_plan_lookup": ([_vp, C.POINTER(SkelInstance), _sz, C.POINTER(_i)], _i),
     "skel_plan_set": ([_vp, C.POINTER(SkelInstance), _sz, _i], _i),
+    "skel_plan_explain": ([_vp, C.POINTER(SkelInstance), _sz, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)], _i),
     "skel_tune_table": ([_vp, C.POINTER(C.c_float), _sz, C.POINTER(_sz)], _i),
     "skel_force_variant": ([_vp, _i, _i], _i),
     "skel_last_variant": ([_vp, C.POINTER(_i), C.POINTER(_i)], _i),
@@ -376,6 +377,12 @@ class Context:
         v = C.c_int()
         self.check(lib.skel_plan_lookup(self.h, C.byref(inst), n, C.byref(v)))
         return v.value
+
+    def plan_explain(self, inst: SkelInstance, n: int):
+        """-> (variant, exact key tuned?, variant comes from the plan (not the preference list)?)"""
+        v, ex, fp = C.c_int(), C.c_int(), C.c_int()
+        self.check(lib.skel_plan_explain(self.h, C.byref(inst), n, C.byref(v), C.byref(ex), C.byref(fp)))
+        return v.value, bool(ex.value), bool(fp.value)
 
     def plan_set(self, inst: SkelInstance, n_min: int, variant: int):
         self.check(lib.skel_plan_set(self.h, C.byref(inst), n_min, variant))

@@ -212,7 +212,7 @@ inline bool al32(const void* p) { return reinterpret_cast<uintptr_t>(p) % 32 == 
 }  // namespace
 
 bool fused_chain_ok(int map_fn, int r, int red_op, const void* in, const void* map_out, const void* ov_out, size_t n) {
-  const bool rt = r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16;
+  const bool rt = r >= 0 && r <= 16;  // radii between the instantiated ones run zero-padded (kernels.hpp)
   const bool mf = map_fn == FN_IDENT || map_fn == FN_ADD || map_fn == FN_MULT || map_fn == FN_MAX;
   const bool ro = red_op == FUSED_NO_REDUCE || red_op == FN_ADD || red_op == FN_MAX;
   if (!rt || !mf || !ro || n == 0) return false;
@@ -227,6 +227,10 @@ cudaError_t launch_fused_chain(const Launch& L, const Scratch& S, int map_fn, ui
                                float* result) {
   float c;
   memcpy(&c, &cbits, 4);
+  if (const int R = padded_radius_1d(r); R != r) {
+    if (R < 0) return cudaErrorInvalidValue;
+    return launch_fused_chain(L, S, map_fn, cbits, pad_weights_1d(w, r, R), R, edge, pad, red_op, in, map_out, ov_out, n, result);
+  }
   switch (r) {
     case 1: return launch_r<1>(L, S, map_fn, red_op, w, edge, pad, c, in, map_out, ov_out, n, result);
     case 2: return launch_r<2>(L, S, map_fn, red_op, w, edge, pad, c, in, map_out, ov_out, n, result);

@@ -67,6 +67,27 @@ size_t scan_tiles_needed(size_t n);
 struct Weights1D { float w[129]; };   // 2r+1 <= 129 taps, passed by value (constant bank)
 struct Weights2D { float w[17 * 17]; };
 
+// Radii the tiled kernels are instantiated for: {1, 2, 3, 4, 8, 16} in 1D, square {1..4} in 2D, {1, 2, 3, 4, 8} for the
+// fused separable pair. Any other radius up to the largest runs the NEXT instantiated one with the weights zero-padded
+// at both ends (a radius-5 filter IS a radius-8 filter whose outer taps are 0): every tap keeps its place in the
+// ascending order, the extra fused multiply-adds add 0 * x~ = 0, so for finite data the result has the same bits
+// (a non-finite x~ within the padded reach of an output, but outside its real reach, would turn it into NaN: the
+// direct variant is the one to force for such data).
+inline int padded_radius_1d(int r) { return r <= 4 ? (r < 1 ? 1 : r) : (r <= 8 ? 8 : (r <= 16 ? 16 : -1)); }
+inline Weights1D pad_weights_1d(const Weights1D& w, int r, int R) {
+  Weights1D o;
+  for (float& x : o.w) x = 0.f;
+  for (int k = 0; k <= 2 * r; ++k) o.w[k + (R - r)] = w.w[k];
+  return o;
+}
+inline Weights2D pad_weights_2d(const Weights2D& w, int ry, int rx, int R) {  // (2ry+1) x (2rx+1) -> (2R+1)^2
+  Weights2D o;
+  for (float& x : o.w) x = 0.f;
+  for (int a = 0; a <= 2 * ry; ++a)
+    for (int b = 0; b <= 2 * rx; ++b) o.w[(a + R - ry) * (2 * R + 1) + (b + R - rx)] = w.w[a * (2 * rx + 1) + b];
+  return o;
+}
+
 int overlap1d_variant_count();
 const char* overlap1d_variant_name(int v);
 bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols);
@@ -98,8 +119,8 @@ cudaError_t launch_fused_chain(const Launch& L, const Scratch& S, int map_fn, ui
 int separable_variant_count();
 const char* separable_variant_name(int v);
 bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const void* out, size_t rows, size_t cols);
-cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r, int edge,
-                                   float pad, const float* in, float* out, size_t rows, size_t cols);
+cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r_row,
+                                   int r_col, int edge, float pad, const float* in, float* out, size_t rows, size_t cols);
 
 // ---- FP32 FMA roofline probe (probe.cu) ------------------------------------------------------------
 cudaError_t launch_fma_probe(const Launch& L, float* scratch /* device, >= 1 float */, double* fma_count);

@@ -770,7 +770,7 @@ const char* overlap1d_variant_name(int v) { return (v >= 0 && v < kNumVariants) 
 bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumVariants) return false;
   if (kVariants[v].o == 0) return true;
-  if (!templated_radius(r)) return false;
+  if (r < 0 || r > 16) return false;  // radii between the instantiated ones run zero-padded (kernels.hpp)
   if (kVariants[v].o == -8 && r > 8) return false;
   if (kVariants[v].o >= 300 && rows != 1 && cols % 32 != 0) return false;  // a matrix row must be whole 128-byte rows
   const bool al = reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
@@ -780,6 +780,11 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
 cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
+  if (kVariants[v].o != 0 && !templated_radius(r)) {
+    const int R = padded_radius_1d(r);
+    if (R < 0) return cudaErrorInvalidValue;
+    return launch_overlap1d_rows(L, v, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
+  }
   switch (kVariants[v].o) {
     case 0: {
       const size_t total = rows * cols;

@@ -84,14 +84,17 @@ const char* overlap1d_col_variant_name(int v) { return (v >= 0 && v < kNumColVar
 bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumColVariants) return false;
   if (v == 0) return true;
-  const bool templated = r == 1 || r == 2 || r == 3 || r == 4 || r == 8 || r == 16;
-  return templated && tiled_alignment_ok(in, out, rows, cols);
+  return r >= 0 && r <= 16 && tiled_alignment_ok(in, out, rows, cols);  // other radii run zero-padded (kernels.hpp)
 }
 
 cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
   if (v == 0) return launch_direct2<Weights1D>(L, w, r, 0, edge, pad, in, out, rows, cols);
+  if (const int R = padded_radius_1d(r); R != r) {
+    if (R < 0) return cudaErrorInvalidValue;
+    return launch_overlap1d_cols(L, v, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
+  }
   switch (r) {
     case 1: return launch_overlap1d_cols_tiled<1>(L, v, w, edge, pad, in, out, rows, cols);
     case 2: return launch_overlap1d_cols_tiled<2>(L, v, w, edge, pad, in, out, rows, cols);
@@ -109,15 +112,19 @@ const char* overlap2d_variant_name(int v) { return (v >= 0 && v < kNumVariants) 
 bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumVariants) return false;
   if (v == 0) return true;
-  const bool templated = ry == rx && ry >= 1 && ry <= 4;
-  return templated && tiled_alignment_ok(in, out, rows, cols);
+  // rectangular filters and ry = rx = 0 run the square filter of radius max(ry, rx, 1) zero-padded (kernels.hpp)
+  return ry >= 0 && rx >= 0 && ry <= 4 && rx <= 4 && tiled_alignment_ok(in, out, rows, cols);
 }
 
 cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
                              const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
   if (v == 0) return launch_direct2<Weights2D>(L, w, ry, rx, edge, pad, in, out, rows, cols);
-  if (ry != rx) return cudaErrorInvalidValue;
+  if (ry != rx || ry < 1) {
+    const int R = ry > rx ? ry : (rx > 1 ? rx : 1);
+    if (R > 4) return cudaErrorInvalidValue;
+    return launch_overlap2d(L, v, pad_weights_2d(w, ry, rx, R), R, R, edge, pad, in, out, rows, cols);
+  }
   switch (ry) {
     case 1: return launch_overlap2d_tiled<1>(L, v, w, edge, pad, in, out, rows, cols);
     case 2: return launch_overlap2d_tiled<2>(L, v, w, edge, pad, in, out, rows, cols);

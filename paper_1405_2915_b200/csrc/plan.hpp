@@ -1,12 +1,22 @@
 // Execution plans ("a run-time data structure ... for fast lookup of the expected
-// best back-end ... and tunable parameters"; L53: dispatch structures precomputed off-line from
-// sample executions). Here: per skeleton instance, sorted size breakpoints -> kernel variant. Pure host
-// code, no CUDA.
+// best back-end ... and tunable parameters"; L53: "precomputing a tree-based dispatch structure for fast
+// runtime lookup" from off-line sample executions). Pure host code, no CUDA.
+//
+// A tuned point is (instance key) -> sorted size breakpoints -> kernel variant. The keys form a DISPATCH TREE over the
+// call context, one level per dimension, in this order:
+//     skeleton -> dtype -> (fn, fn2) -> shape class / mode -> r0 -> r1 -> edge policy -> size breakpoints
+// A lookup walks the tree from the root. Where the call's value has a child, it takes it; where it has not
+// (a radius, edge policy, user function or shape class that was never tuned), it takes the NEAREST tuned child:
+// for the radii the one closest in log2(r + 1), ties to the larger radius; for the categorical levels the first
+// child. skeleton and dtype must match exactly. So r = 5, 6, 12 inherit the plan of r = 4, 8, 16, CYCLIC edges
+// inherit DUPLICATE's, and only a (skeleton, dtype) pair with no tuned point at all falls back to the static
+// preference list. The caller still checks that the inherited variant is applicable to the call.
 #pragma once
 #include <stddef.h>
 #include <stdint.h>
 #include <array>
 #include <map>
+#include <memory>
 #include <string>
 #include <vector>
 
@@ -21,34 +31,30 @@ struct Breakpoint { size_t n_min; int variant; };
 
 class Plan {
  public:
-  // variant for n, or -1 if the instance has no entry (binary search over the breakpoints;
-  // below the first breakpoint -> the first entry's variant)
-  int lookup(const InstanceKey& k, size_t n) const {
-    auto it = table_.find(k);
-    if (it == table_.end() || it->second.empty()) return -1;
-    const std::vector<Breakpoint>& b = it->second;
-    size_t lo = 0, hi = b.size();  // last entry with n_min <= n
-    while (hi - lo > 1) {
-      const size_t mid = (lo + hi) / 2;
-      if (b[mid].n_min <= n) lo = mid; else hi = mid;
-    }
-    return b[lo].variant;
-  }
-  void set(const InstanceKey& k, size_t n_min, int variant) {
-    std::vector<Breakpoint>& b = table_[k];
-    size_t i = 0;
-    while (i < b.size() && b[i].n_min < n_min) ++i;
-    if (i < b.size() && b[i].n_min == n_min) b[i].variant = variant;
-    else b.insert(b.begin() + i, Breakpoint{n_min, variant});
-  }
-  void erase(const InstanceKey& k) { table_.erase(k); }
-  void clear() { table_.clear(); }
+  // variant for n, or -1 if no tuned point shares the call's skeleton and dtype. *exact (optional) tells whether the
+  // call's own key was tuned (true) or a neighbour's breakpoints were inherited (false). Binary search over the
+  // breakpoints; below the first breakpoint -> the first entry's variant.
+  int lookup(const InstanceKey& k, size_t n, bool* exact = nullptr) const;
+  void set(const InstanceKey& k, size_t n_min, int variant);
+  void erase(const InstanceKey& k);
+  void clear();
   bool save(const char* path) const;
-  bool load(const char* path);
+  bool load(const char* path);  // lines starting with '#' are comments (provenance)
   size_t size() const { return table_.size(); }
+  // number of tree levels below the root (diagnostic)
+  static constexpr int kLevels = 7;
 
  private:
+  // level order of the tree: indices into InstanceKey::f, fn and fn2 merged into one level
+  struct Node {
+    std::map<int64_t, std::unique_ptr<Node>> child;
+    const std::vector<Breakpoint>* leaf = nullptr;  // set on the last level
+  };
+  static int64_t level_value(const InstanceKey& k, int level);
+  static bool level_is_radius(int level) { return level == 4 || level == 5; }
+  void rebuild();
   std::map<InstanceKey, std::vector<Breakpoint>> table_;
+  Node root_;
 };
 
 }  // namespace skel

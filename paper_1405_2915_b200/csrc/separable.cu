@@ -181,15 +181,21 @@ const char* separable_variant_name(int v) { return (v >= 0 && v < kNumSep) ? kSe
 bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumSep) return false;
   if (v == 0) return true;
-  const bool templated = r_row == r_col && (r_row == 1 || r_row == 2 || r_row == 3 || r_row == 4 || r_row == 8);
+  // unequal radii and radii between the instantiated ones run zero-padded to the next of {1, 2, 3, 4, 8} (kernels.hpp)
+  const bool templated = r_row >= 0 && r_col >= 0 && r_row <= 8 && r_col <= 8;
   return templated && reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0 &&
          cols % 4 == 0 && rows < (size_t(1) << 30) && cols < (size_t(1) << 30) &&
          ((rows + 31) / 32) * ((cols + 127) / 128) < (size_t(1) << 30);
 }
 
-cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r, int edge,
-                                   float pad, const float* in, float* out, size_t rows, size_t cols) {
+cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r_row,
+                                   int r_col, int edge, float pad, const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
+  const int rmax = r_row > r_col ? r_row : r_col;
+  const int r = rmax <= 4 ? (rmax < 1 ? 1 : rmax) : (rmax <= 8 ? 8 : -1);
+  if (r != r_row || r != r_col)  // zero-padded to the next instantiated radius (kernels.hpp)
+    return launch_separable_fused(L, v, pad_weights_1d(wrow, r_row, r), pad_weights_1d(wcol, r_col, r), r, r, edge, pad, in,
+                                  out, rows, cols);
   switch (r) {
     case 1: return launch_sep_r<1>(L, v, wrow, wcol, edge, pad, in, out, rows, cols);
     case 2: return launch_sep_r<2>(L, v, wrow, wcol, edge, pad, in, out, rows, cols);

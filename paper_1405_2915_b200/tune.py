@@ -3,9 +3,13 @@ for each new target system"; L53: dispatch structures precomputed from sample ex
 
   python -m paper_1405_2915_b200.tune [--out plans/b200.plan] [--reps 7]
 
-Times every applicable kernel variant of the skeleton instances the bench configs use at
-n = 2^k, stores the per-size winners as breakpoints, prints the timing tables (microseconds) and
-writes the plan file that bench.py and users load with skel_plan_load.
+Times every applicable kernel variant of the skeleton instances the bench configs use (and a few
+neighbours, so that the plan's dispatch tree has more than one tuned radius per skeleton) at
+n = 2^k under the conditions of a sustained run (skel_tune_instance: operands rotate through arenas
+larger than L2, every timed launch follows a writer that leaves L2 dirty), stores the per-size
+winners as breakpoints, prints the timing tables (microseconds) and writes the plan file that
+bench.py and users load with skel_plan_load. The file is written by this program only: its first
+line is a '#' comment that names the command, the GPU and the date; nobody edits breakpoints by hand.
 """
 from __future__ import annotations
 
@@ -32,9 +36,12 @@ def instances(S):
     for r in (1, 4, 16):
         for edge in (S.EDGE_CONSTANT, S.EDGE_DUPLICATE):
             out.append((f"overlap1d_r{r}_e{edge}", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, edge=edge), 12, 26, 0))
-    out.append(("overlap1d_rows_r8", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    for r in (2, 8):  # neighbours for the dispatch tree (not in a bench config)
+        out.append((f"overlap1d_r{r}_e1", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, edge=S.EDGE_DUPLICATE), 12, 26, 0))
+    # rows of a matrix: shape class 1 of the dispatch tree (skel_instance.mode)
+    out.append(("overlap1d_rows_r8", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE, mode=1), 20, 26, 8192))
     out.append(("overlap1d_cols_r8", I(skeleton=S.SK_OVERLAP1D_COL, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
-    for r in (2, 4):
+    for r in (1, 2, 4):
         out.append((f"overlap2d_{2*r+1}x{2*r+1}", I(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, r1=r, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
     out.append(("reduce_rows_add_f32", I(skeleton=S.SK_REDUCE_ROWS, fn=S.FN_ADD, dtype=S.F32), 20, 26, 8192))
     out.append(("separable_r8", I(skeleton=S.SK_SEPARABLE, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, r1=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
@@ -70,6 +77,15 @@ def main():
             print(f"  2^{lo + k:2d}  " + " ".join(f"{x:9.1f}" for x in row) + f"   -> {best}")
     os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
     ctx.plan_save(args.out)
+    # provenance: '#' lines are comments for the loader
+    import datetime
+    import torch
+    body = open(args.out).read()
+    cmd = "python -m paper_1405_2915_b200.tune " + " ".join(sys.argv[1:])
+    note = (f"# generated by: {cmd.strip()}  (skel_tune_instance, reps={args.reps}; {torch.cuda.get_device_name(0)}, "
+            f"{datetime.datetime.now(datetime.timezone.utc).strftime('%Y-%m-%d %H:%M UTC')}); not edited by hand\n")
+    with open(args.out, "w") as f:
+        f.write(note + body)
     if args.tables:
         with open(args.tables, "w") as f:
             json.dump(tables, f)

@@ -126,7 +126,12 @@ def test_plan_lookup_set_save_load(tmp_path):
     ctx.plan_set(inst, 1 << 22, 3)
     for n, v in [(0, 0), (1, 0), ((1 << 16) - 1, 0), (1 << 16, 1), ((1 << 22) - 1, 1), (1 << 22, 3), (1 << 30, 3)]:
         assert ctx.plan_lookup(inst, n) == v
-    assert ctx.plan_lookup(other, 1 << 20) == default  # another instance is untouched
+    # a radius that was never tuned inherits its nearest tuned neighbour (the dispatch tree, see below);
+    # another skeleton / element type is untouched
+    assert ctx.plan_lookup(other, 1 << 20) == 1 and ctx.plan_explain(other, 1 << 20) == (1, False, True)
+    assert ctx.plan_explain(inst, 1 << 20) == (1, True, True)
+    col = S.SkelInstance(skeleton=S.SK_OVERLAP1D_COL, fn=S.FN_WSTENCIL, dtype=S.F32, r0=4, edge=S.EDGE_DUPLICATE)
+    assert ctx.plan_explain(col, 1 << 20)[1:] == (False, False)
     ctx.plan_set(inst, 1 << 16, 2)  # overwrite a breakpoint
     assert ctx.plan_lookup(inst, 1 << 17) == 2
     path = str(tmp_path / "b.plan")
@@ -150,6 +155,76 @@ def test_plan_lookup_set_save_load(tmp_path):
         ctx.plan_load(str(bad))
     assert ctx.plan_lookup(inst, 1 << 23) == 3  # a failed load leaves the plan as it was
     ctx.close()
+
+
+def test_plan_dispatch_tree_inherits_the_nearest_tuned_neighbour(tmp_path):
+    """SURVEY.md 8(f) f3 / PAPER.md L53 "tree-based dispatch structure": skeleton -> dtype -> (fn, fn2) -> shape class ->
+    r0 -> r1 -> edge -> size breakpoints. An untuned context takes the nearest tuned child at the first level where it
+    has none (radii: nearest in log2(r + 1), ties to the larger radius); skeleton and dtype must match."""
+    ctx = S.Context(lazy_cuda=True)
+    o1 = lambda r, edge=S.EDGE_DUPLICATE, mode=0, dt=S.F32: S.SkelInstance(  # noqa: E731
+        skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=dt, r0=r, edge=edge, mode=mode)
+    ctx.plan_set(o1(4), 0, 8)
+    ctx.plan_set(o1(4), 1 << 20, 10)
+    ctx.plan_set(o1(16), 0, 9)
+    ctx.plan_set(o1(1, S.EDGE_CONSTANT), 0, 4)
+    n = 1 << 22
+    assert ctx.plan_explain(o1(4), n) == (10, True, True) and ctx.plan_explain(o1(4), 5) == (8, True, True)
+    # radii: log2(r+1) distance. r=5,6 -> 4; r=8: |log2 9 - log2 5| = 0.848 < |log2 17 - log2 9| = 0.918 -> 4;
+    # r=12 -> 16; r=2 -> log2 3: 0.585 from r=1, 0.737 from r=4 -> 1; r=64 -> 16; r=0 -> 1
+    expect = {5: 10, 6: 10, 8: 10, 9: 9, 12: 9, 64: 9, 3: 10, 2: 4, 0: 4}
+    for r, v in expect.items():
+        assert ctx.plan_explain(o1(r), n) == (v, False, True), r
+    # the breakpoints of the neighbour are inherited, not just its last variant
+    assert ctx.plan_lookup(o1(5), 1000) == 8 and ctx.plan_lookup(o1(5), n) == 10
+    # edge policy never tuned for this radius: the first tuned policy of that radius
+    assert ctx.plan_explain(o1(4, S.EDGE_CYCLIC), n) == (10, False, True)
+    assert ctx.plan_explain(o1(1, S.EDGE_DUPLICATE), n) == (4, False, True)
+    # shape class never tuned (rows of a matrix): inherits the vector's subtree; once tuned, it is its own
+    assert ctx.plan_explain(o1(4, mode=1), n) == (10, False, True)
+    ctx.plan_set(o1(8, mode=1), 0, 7)
+    assert ctx.plan_explain(o1(4, mode=1), n) == (7, False, True) and ctx.plan_explain(o1(4), n) == (10, True, True)
+    # skeleton and element type must match: nothing is inherited across them
+    assert ctx.plan_explain(o1(4, dt=S.I32), n)[2] is False
+    red = S.SkelInstance(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.F32)
+    assert ctx.plan_explain(red, n)[2] is False
+    # user function never tuned: the first tuned function of that skeleton and element type
+    ctx.plan_set(S.SkelInstance(skeleton=S.SK_REDUCE, fn=S.FN_ADD, dtype=S.I32), 0, 5)
+    assert ctx.plan_explain(S.SkelInstance(skeleton=S.SK_REDUCE, fn=S.FN_MAX, dtype=S.I32), n) == (5, False, True)
+    # 2D: both radii walk the tree
+    o2 = lambda ry, rx: S.SkelInstance(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=ry, r1=rx, edge=S.EDGE_DUPLICATE)  # noqa: E731
+    ctx.plan_set(o2(2, 2), 0, 7)
+    ctx.plan_set(o2(4, 4), 0, 5)
+    assert ctx.plan_lookup(o2(3, 3), n) == 5 and ctx.plan_lookup(o2(1, 1), n) == 7 and ctx.plan_lookup(o2(2, 4), n) == 7
+    # save / load round trip keeps the tree; '#' lines (provenance) are comments
+    path = tmp_path / "tree.plan"
+    ctx.plan_save(str(path))
+    text = path.read_text().splitlines()
+    path.write_text("\n".join(["# generated by: a test", text[0], "# another comment"] + text[1:]) + "\n")
+    ctx.plan_clear()
+    assert ctx.plan_explain(o1(5), n)[2] is False
+    ctx.plan_load(str(path))
+    for r, v in expect.items():
+        assert ctx.plan_explain(o1(r), n) == (v, False, True), r
+    ctx.close()
+
+
+def test_plan_file_from_the_environment_reports_a_failed_load(tmp_path):
+    import subprocess
+    import sys
+    code = ("import os, sys; sys.path.insert(0, %r)\n"
+            "from paper_1405_2915_b200 import skel as S\n"
+            "c = S.Context(lazy_cuda=True)\n"
+            "print(S.lib.skel_last_error(c.h).decode())\n" % ROOT)
+    bad = tmp_path / "bad.plan"
+    bad.write_text("garbage\n")
+    out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, SKEL_PLAN_FILE=str(bad)),
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0 and "SKEL_PLAN_FILE" in out.stdout and "bad.plan" in out.stdout, out.stderr
+    good = os.path.join(ROOT, "paper_1405_2915_b200", "plans", "b200.plan")
+    out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, SKEL_PLAN_FILE=good),
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0 and "SKEL_PLAN_FILE" not in out.stdout, out.stderr
 
 
 def test_plan_lookup_is_fast():
@@ -212,7 +287,7 @@ def test_shipped_plan_is_consistent_with_the_variant_tables():
     import os
 
     path = os.path.join(os.path.dirname(os.path.abspath(S.__file__)), "plans", "b200.plan")
-    lines = open(path).read().split("\n")
+    lines = [ln for ln in open(path).read().split("\n") if not ln.lstrip().startswith("#")]   # '#': provenance comments
     assert lines[0].strip() == "skelplan 1"
     ctx = S.Context(lazy_cuda=True)
     ctx.plan_load(path)

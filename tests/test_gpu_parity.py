@@ -27,12 +27,13 @@ def variants(sk):
 
 
 def o1_radius_ok(v, r):
-    """Radii a MapOverlap 1D variant is instantiated for (direct: any; regshfl_2x8: r <= 8)."""
+    """Radii a MapOverlap 1D variant runs (direct: any; tiled: r <= 16, radii between the instantiated ones
+    {1,2,3,4,8,16} zero-padded to the next one, csrc/kernels.hpp; regshfl_2x8: r <= 8)."""
     if v == 0:
         return True
     if S.variant_names(S.SK_OVERLAP1D)[v] == "regshfl_2x8":
-        return r in (1, 2, 3, 4, 8)
-    return r in (1, 2, 3, 4, 8, 16)
+        return 0 <= r <= 8
+    return 0 <= r <= 16
 
 
 class forced:
@@ -338,11 +339,9 @@ EDGE_CASES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICAT
 O1_SIZES = [1, 2, 3, 5, 16, 17, 33, 100, 1023, 4096, 4097, 8200, 12320, 16385, 65537, 300001]
 
 
-@pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
-@pytest.mark.parametrize("r", [0, 1, 2, 3, 4, 5, 8, 16, 17, 64])
+@pytest.mark.parametrize("v,r", [(v, r) for r in [0, 1, 2, 3, 4, 5, 6, 8, 12, 16, 17, 64]
+                                  for v in variants(S.SK_OVERLAP1D) if o1_radius_ok(v, r)])
 def test_overlap1d_vector(ctx, v, r):
-    if not o1_radius_ok(v, r):
-        pytest.skip("tiled variants are instantiated for r in {1,2,3,4,8,16} (regshfl_2x8: r <= 8)")
     w = I.positive_weights_f32(500 + r, 2 * r + 1)
     ws = I.signed_weights_f32(501 + r, 2 * r + 1)
     with forced(ctx, S.SK_OVERLAP1D, v):
@@ -364,7 +363,7 @@ def test_overlap1d_vector(ctx, v, r):
 @pytest.mark.parametrize("v", variants(S.SK_OVERLAP1D))
 def test_overlap1d_one_hot_weights_shift_bit_exact(ctx, v):
     with forced(ctx, S.SK_OVERLAP1D, v):
-        for r in (1, 4, 16):
+        for r in (1, 4, 5, 12, 16):   # 5 and 12 run zero-padded to 8 and 16: the shift must not move
             if not o1_radius_ok(v, r):
                 continue
             for n in (3, 50, 4099, 8193):
@@ -477,7 +476,7 @@ def test_overlap1d_matrix_cols(ctx, v, r):
     for rows, cols in MAT_SHAPES:
         X = I.uniform01_f32(541 + rows, rows * cols).reshape(rows, cols)
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
-        tiled_ok = r in (1, 2, 3, 4, 8, 16) and cols % 4 == 0
+        tiled_ok = 0 <= r <= 16 and cols % 4 == 0   # radii between the instantiated ones run zero-padded
         with forced(ctx, S.SK_OVERLAP1D_COL, v):
             for edge, pad in EDGE_CASES:
                 if v != 0 and not tiled_ok:
@@ -494,7 +493,7 @@ def test_overlap1d_matrix_cols(ctx, v, r):
 
 # ------------------------------------------------------------------ MapOverlap 2D
 @pytest.mark.parametrize("v", variants(S.SK_OVERLAP2D))
-@pytest.mark.parametrize("radii", [(0, 0), (1, 1), (2, 2), (3, 3), (4, 4), (2, 4), (1, 0), (0, 3), (8, 8)])
+@pytest.mark.parametrize("radii", [(0, 0), (1, 1), (2, 2), (3, 3), (4, 4), (2, 4), (1, 0), (0, 3), (4, 1), (8, 8), (5, 2)])
 def test_overlap2d(ctx, v, radii):
     ry, rx = radii
     W = I.positive_weights_f32(600 + ry * 9 + rx, (2 * ry + 1) * (2 * rx + 1))
@@ -502,7 +501,7 @@ def test_overlap2d(ctx, v, radii):
     for rows, cols in MAT_SHAPES:
         X = I.uniform01_f32(602 + rows, rows * cols).reshape(rows, cols)
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
-        tiled_ok = ry == rx and 1 <= ry <= 4 and cols % 4 == 0
+        tiled_ok = ry <= 4 and rx <= 4 and cols % 4 == 0   # rectangular filters run the zero-padded square one
         with forced(ctx, S.SK_OVERLAP2D, v):
             for edge, pad in EDGE_CASES:
                 if v != 0 and not tiled_ok:

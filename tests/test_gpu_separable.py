@@ -37,7 +37,7 @@ def oracle_separable(wr, rr, wc, rc, oe, pad, X):
 
 
 @pytest.mark.parametrize("v", [0, 1, 2, 3, 4])
-@pytest.mark.parametrize("radii", [(1, 1), (2, 2), (3, 3), (4, 4), (8, 8), (0, 0), (8, 2), (5, 5), (16, 16)])
+@pytest.mark.parametrize("radii", [(1, 1), (2, 2), (3, 3), (4, 4), (8, 8), (0, 0), (8, 2), (5, 5), (3, 6), (16, 16), (9, 1)])
 def test_separable_matches_oracle(ctx, v, radii):
     rr, rc = radii
     wr = I.positive_weights_f32(700 + rr, 2 * rr + 1)
@@ -46,7 +46,7 @@ def test_separable_matches_oracle(ctx, v, radii):
     for rows, cols in SHAPES:
         X = I.uniform01_f32(702 + rows, rows * cols).reshape(rows, cols)
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols)
-        fused_ok = rr == rc and rr in (1, 2, 3, 4, 8) and cols % 4 == 0
+        fused_ok = rr <= 8 and rc <= 8 and cols % 4 == 0   # unequal / other radii run zero-padded (csrc/kernels.hpp)
         ctx.force_variant(S.SK_SEPARABLE, v)
         try:
             for ge, oe, pad in EDGES:
