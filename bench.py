@@ -29,9 +29,21 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernels at full size, from the
-# `ncu --set full` captures summarised in profiles/r01_ncu_scan.md (bytes)
-NCU_DRAM_BYTES_PER_LAUNCH = {"scan": 2152857000}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch at full size, per kernel VARIANT, from the `ncu --set full`
+# captures listed in profiles/r02_ncu_traffic.csv (command: profiles/r02_ncu_traffic.md). A variant that has no row
+# there reports "traffic": null instead of a stale number.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
+
+
+def ncu_traffic(op_name: str, variant: str):
+    if not os.path.exists(TRAFFIC_CSV):
+        return None
+    import csv
+    with open(TRAFFIC_CSV) as f:
+        for row in csv.DictReader(f):
+            if row["bench_op"] == op_name and row["variant"] == variant:
+                return int(float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]))
+    return None
 
 METRIC = "skeleton throughput (algorithmic GB/s over one pass of all skeletons at their largest config)"
 UNIT = "GB/s"
@@ -465,8 +477,12 @@ def main():
     dom = max(kern_time, key=lambda f: kern_time[f][0])
     dt_ms, dbytes, dcount = kern_time[dom]
     achieved = dbytes / (dt_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                "frac": round(achieved / peak, 4), "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if args.scale == 1.0 else None,
+    dom_ops = [name for name, *_ in wl.ops if kernel_key(name) == dom]
+    dom_variant = per[dom_ops[0]]["variant"]
+    roofline = {"bound": "hbm", "kernel": dom, "variant": dom_variant, "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4),
+                "traffic": ncu_traffic(dom_ops[0], dom_variant) if args.scale == 1.0 else None,
+                "traffic_source": "profiles/r02_ncu_traffic.csv (ncu --set full, per launch, keyed by variant)",
                 "algorithmic_bytes_per_launch": dbytes // dcount,
                 "peak_source": peak_src, "launches_per_step": dcount, "avg_launch_us": round(dt_ms * 1e3 / dcount, 2),
                 "share_of_step": round(dt_ms / ms_per_step, 4)}
@@ -619,11 +635,34 @@ def main():
             enq.append(time.perf_counter() - t0)
             torch.cuda.synchronize()
         host_ms = float(np.median(enq)) * 1e3
-        container_layer = {"host_us_per_call": round(host_ms * 1e3 / nops, 2), "host_ms_per_step": round(host_ms, 4),
-                           "device_ms_per_step": round(ms_per_step, 4),
-                           "host_fraction_of_device_time": round(host_ms / ms_per_step, 4),
-                           "note": "argument checks + coherence look-up + plan look-up + launch + publish, through ctypes; "
-                                   "calls are asynchronous, so this host time overlaps the device time of earlier calls"}
+        # SURVEY.md 8(d)(4) / PAPER.md L123 ("negligible (less than 1 %)"): the SAME 16 kernel launches through the
+        # container layer against bare launches on raw device pointers, both timed inside the library (no Python, no
+        # ctypes): skel_replay_* records the step's calls and replays them either way.
+        ctx.replay_begin()
+        wl.step()
+        ncalls = ctx.replay_end()
+        for raw in (False, True):
+            ctx.replay_run(raw, 3)
+        hc, dc, hr, dr = [], [], [], []
+        for _ in range(5):  # interleaved: clock / power drift hits both alike
+            h, dv = ctx.replay_run(False, 10)
+            hc.append(h), dc.append(dv)
+            h, dv = ctx.replay_run(True, 10)
+            hr.append(h), dr.append(dv)
+        hc, dc, hr, dr = (float(np.median(v)) for v in (hc, dc, hr, dr))
+        container_layer = {
+            "definition": "time of one step (16 calls) through skel_* on containers / time of the same 16 kernel "
+                          "launches on raw device pointers - 1 (SURVEY.md 8(d)(4)); timed in C inside libskel.so",
+            "calls": ncalls,
+            "device_us_per_step_containers": round(dc, 2), "device_us_per_step_raw": round(dr, 2),
+            "device_overhead": round(dc / dr - 1.0, 5),
+            "host_us_per_step_containers": round(hc, 2), "host_us_per_step_raw": round(hr, 2),
+            "host_us_per_call_containers": round(hc / ncalls, 3), "host_us_per_call_raw": round(hr / ncalls, 3),
+            "host_overhead_us_per_call": round((hc - hr) / ncalls, 3),
+            "host_enqueue_fraction_of_device_time": round(hc / dc, 5),
+            "paper_claim": "< 1 % (PAPER.md L123)",
+            "through_python_ctypes": {"host_us_per_call": round(host_ms * 1e3 / nops, 2), "host_ms_per_step": round(host_ms, 4),
+                                      "note": "the same step enqueued from Python: ctypes marshalling included"}}
         nmax = 1 << 28
         tx, ty = torch.rand(nmax, device="cuda") * 2 - 1, torch.rand(nmax, device="cuda") * 2 - 1
         res = ctx.vector(1)

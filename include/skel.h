@@ -310,6 +310,21 @@ skel_status skel_plan_explain(skel_ctx* ctx, const skel_instance* inst, size_t n
                               int* variant_from_plan);
 /* Insert one breakpoint by hand: variant `variant` from n >= n_min (until the next breakpoint). */
 skel_status skel_plan_set(skel_ctx* ctx, const skel_instance* inst, size_t n_min, int variant);
+/* Measurement hook for the overhead of the container layer (the smart containers' overhead is
+ * "negligible (less than 1 %)"; time through skel_* on containers / time of the same kernel
+ * launches on raw pointers - 1). skel_replay_begin starts recording the skeleton calls made on the context
+ * (fusion must be off), skel_replay_end stops (*ncalls = calls recorded). skel_replay_run then runs the recorded
+ * sequence `reps` times, timed inside the library (host: clock around the enqueue loop; device: CUDA events on the
+ * context's stream), either
+ *   raw = 0: through the container layer - operand acquisition (coherence look-up, transfers if a copy is stale),
+ *            execution-plan look-up, launch, publish, event record - i.e. what the public calls do after argument
+ *            validation, or
+ *   raw = 1: as bare kernel launches on the recorded device pointers with the recorded variants.
+ * The containers of the recorded calls must still be alive. Blocks until the sequence has finished. */
+skel_status skel_replay_begin(skel_ctx* ctx);
+skel_status skel_replay_end(skel_ctx* ctx, int* ncalls);
+skel_status skel_replay_run(skel_ctx* ctx, int raw, int reps, double* host_us_per_pass, double* device_us_per_pass);
+
 /* Timing table of the last skel_tune_instance: times_us[(k-log2_lo)*nvariants + v], NaN where a
  * variant is not applicable. Copies at most `capacity` floats; *count = number available. */
 skel_status skel_tune_table(skel_ctx* ctx, float* times_us, size_t capacity, size_t* count);

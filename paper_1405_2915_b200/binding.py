@@ -117,6 +117,9 @@ _SIGS = {
     "skel_plan_lookup": ([_vp, C.POINTER(SkelInstance), _sz, C.POINTER(_i)], _i),
     "skel_plan_set": ([_vp, C.POINTER(SkelInstance), _sz, _i], _i),
     "skel_plan_explain": ([_vp, C.POINTER(SkelInstance), _sz, C.POINTER(_i), C.POINTER(_i), C.POINTER(_i)], _i),
+    "skel_replay_begin": ([_vp], _i),
+    "skel_replay_end": ([_vp, C.POINTER(_i)], _i),
+    "skel_replay_run": ([_vp, _i, _i, C.POINTER(_d), C.POINTER(_d)], _i),
     "skel_tune_table": ([_vp, C.POINTER(C.c_float), _sz, C.POINTER(_sz)], _i),
     "skel_force_variant": ([_vp, _i, _i], _i),
     "skel_last_variant": ([_vp, C.POINTER(_i), C.POINTER(_i)], _i),
@@ -377,6 +380,20 @@ class Context:
         v = C.c_int()
         self.check(lib.skel_plan_lookup(self.h, C.byref(inst), n, C.byref(v)))
         return v.value
+
+    def replay_begin(self):
+        self.check(lib.skel_replay_begin(self.h))
+
+    def replay_end(self) -> int:
+        n = C.c_int()
+        self.check(lib.skel_replay_end(self.h, C.byref(n)))
+        return n.value
+
+    def replay_run(self, raw: bool, reps: int):
+        """-> (host enqueue microseconds, device microseconds) per pass over the recorded calls"""
+        h, d = C.c_double(), C.c_double()
+        self.check(lib.skel_replay_run(self.h, 1 if raw else 0, reps, C.byref(h), C.byref(d)))
+        return h.value, d.value
 
     def plan_explain(self, inst: SkelInstance, n: int):
         """-> (variant, exact key tuned?, variant comes from the plan (not the preference list)?)"""

@@ -17,6 +17,7 @@
 #include "coherence.hpp"
 #include "kernels.hpp"
 #include "plan.hpp"
+#include <time.h>
 
 using namespace skel;
 
@@ -69,6 +70,7 @@ struct EventRing {
 };
 
 struct PendingCall;
+struct RecordedCall;
 struct skel_future {
   uint32_t magic;
   skel_ctx* ctx;
@@ -114,6 +116,9 @@ struct skel_ctx {
   // cross-call fusion (skel_ctx_set_fusion): launches of a fusible chain are held back here
   bool fusion = false;
   std::vector<struct PendingCall> pending;
+  // skel_replay_*: the calls recorded between _begin and _end (call, operands, variant)
+  bool recording = false;
+  std::vector<struct RecordedCall> recorded;
   cudaStream_t copy_stream = nullptr;  // skel_*_prefetch_host: downloads that overlap the compute stream's work
   void* sep_tmp = nullptr;  // intermediate matrix of the two-pass separable MapOverlap
   size_t sep_tmp_bytes = 0;
@@ -541,6 +546,8 @@ struct OperandSet {
   }
 };
 
+void record_call(skel_ctx* c, const OperandSet& set);  // skel_replay_*: defined next to run_call
+
 skel_status acquire_all(skel_ctx* c, OperandSet& set) {
   skel_status st = ensure_device(c);
   if (st != SKEL_OK) return st;
@@ -606,6 +613,7 @@ skel_status publish_all(skel_ctx* c, OperandSet& set) {
   }
   c->stats.launches += c->launches;
   c->launches = 0;
+  if (c->recording) record_call(c, set);
   return mark_enqueued(c);  // no-op while the launch is held back (fusion): flush_pending records it
 }
 
@@ -627,6 +635,7 @@ struct Call {
 };
 }  // namespace
 struct PendingCall { Call k; };
+struct RecordedCall { Call k; OperandSet set; int variant; };
 namespace {
 
 InstanceKey key_of(const skel_instance& i) {
@@ -900,7 +909,17 @@ skel_status flush_pending(skel_ctx* c) {
   return mark_enqueued(c);
 }
 
+void record_call(skel_ctx* c, const OperandSet& set) {
+  if (c->recorded.empty() || c->recorded.back().variant != -1000) return;  // run_call left a slot only when recording
+  c->recorded.back().set = set;
+  c->recorded.back().variant = c->last_var;
+}
+
 skel_status run_call(skel_ctx* c, const Call& k) {
+  if (c->recording) {
+    if (c->fusion) return fail(c, SKEL_ERR_UNSUPPORTED, "skel_replay_begin: recording needs cross-call fusion off");
+    c->recorded.push_back(RecordedCall{k, OperandSet{}, -1000});
+  }
   if (!c->fusion) return launch_now(c, k);
   const int kind = chain_kind(c, k);
   bool extends = false;
@@ -1863,6 +1882,73 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
     c->launches = 0;
   }
   return result;
+}
+
+// ---- container-layer overhead measurement (skel.h skel_replay_*) ------------------------------------------
+skel_status skel_replay_begin(skel_ctx* c) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (c->fusion) return fail(c, SKEL_ERR_UNSUPPORTED, "recording needs cross-call fusion off");
+  skel_status st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  c->recorded.clear();
+  c->recording = true;
+  return SKEL_OK;
+}
+
+skel_status skel_replay_end(skel_ctx* c, int* ncalls) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  c->recording = false;
+  while (!c->recorded.empty() && c->recorded.back().variant == -1000) c->recorded.pop_back();  // a call that failed
+  if (ncalls) *ncalls = static_cast<int>(c->recorded.size());
+  return SKEL_OK;
+}
+
+skel_status skel_replay_run(skel_ctx* c, int raw, int reps, double* host_us, double* dev_us) {
+  if (!ctx_ok(c) || !host_us || !dev_us || reps < 1) return SKEL_ERR_INVALID_ARG;
+  if (c->recording) return fail(c, SKEL_ERR_BUSY, "still recording: call skel_replay_end first");
+  if (c->recorded.empty()) return fail(c, SKEL_ERR_INVALID_ARG, "nothing recorded");
+  if (c->fusion) return fail(c, SKEL_ERR_UNSUPPORTED, "replay needs cross-call fusion off");
+  skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  CU(c, cudaStreamSynchronize(c->stream));
+  cudaEvent_t e0, e1;
+  CU(c, cudaEventCreate(&e0));
+  CU(c, cudaEventCreate(&e1));
+  skel_status result = SKEL_OK;
+  timespec t0, t1;
+  clock_gettime(CLOCK_MONOTONIC, &t0);
+  cudaEventRecord(e0, c->stream);
+  for (int rep = 0; rep < reps && result == SKEL_OK; ++rep) {
+    for (RecordedCall& r : c->recorded) {
+      if (raw) {
+        if (r.k.inst.skeleton == SKEL_SK_SCAN) result = ensure_scan_state(c, r.k.n);
+        if (result == SKEL_OK && launch_call(c, r.k, r.variant) != cudaSuccess)
+          result = cuda_fail(c, cudaGetLastError(), "replay launch");
+        c->stats.launches += c->launches;
+        c->launches = 0;
+      } else {
+        OperandSet set = r.set;
+        result = acquire_all(c, set);
+        if (result == SKEL_OK) result = run_call(c, r.k);
+        if (result == SKEL_OK) result = publish_all(c, set);
+      }
+      if (result != SKEL_OK) break;
+    }
+  }
+  cudaEventRecord(e1, c->stream);
+  clock_gettime(CLOCK_MONOTONIC, &t1);  // enqueue time: the calls are asynchronous
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (result != SKEL_OK) return result;
+  if (e != cudaSuccess) return cuda_fail(c, e, "replay");
+  *host_us = ((t1.tv_sec - t0.tv_sec) * 1e9 + (t1.tv_nsec - t0.tv_nsec)) / 1e3 / reps;
+  *dev_us = double(ms) * 1e3 / reps;
+  return SKEL_OK;
 }
 
 // ---- observability ------------------------------------------------------------------------------------

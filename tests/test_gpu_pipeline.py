@@ -310,3 +310,39 @@ def test_pipeline_with_futures_keeps_iterations_in_flight_and_gives_the_same_sca
     assert st_mid["scalar_d2h_count"] == 0 and st_a["scalar_d2h_count"] == iters == st_b["scalar_d2h_count"]
     assert st_a["h2d_count"] == 1 and st_a["d2h_count"] == 0 and st_a["h2d_elided"] == st_b["h2d_elided"]
     assert st_a["launches"] == st_b["launches"] == (iters if fusion else 3 * iters)
+
+
+def test_replay_hook_runs_the_recorded_calls_both_ways(ctx):
+    """skel_replay_* (include/skel.h): the measurement hook behind bench.py's container_layer figure replays recorded
+    calls through the container layer or as bare launches; both leave the same results in the containers."""
+    n = 200003
+    x, v = I.uniform01_f32(8801, n), I.uniform_int_i32(8802, n, 1000)
+    w = I.positive_weights_f32(8803, 9)
+    vx, vo, vi, vs, res = ctx.vector_from(x), ctx.vector(n), ctx.vector_from(v), ctx.vector(n, S.I32), ctx.vector(4, S.I32)
+    ctx.replay_begin()
+    ctx.map(S.FN_MULT, 1.0001, vx, None, vo)
+    ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, vx, vo)
+    ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0, vi, vs)
+    ctx.reduce_to(S.FN_ADD, vi, res, 2)
+    assert ctx.replay_end() == 4
+    ref, ab = O.mapoverlap_1d(w, 4, O.EDGE_DUPLICATE, 0.0, x)
+    for raw in (False, True):
+        vo.write(np.zeros(n, np.float32))
+        vs.write(np.zeros(n, np.int32))
+        ctx.reset_stats()
+        host_us, dev_us = ctx.replay_run(raw, 3)
+        assert host_us > 0 and dev_us > 0
+        st = ctx.stats()
+        assert st["launches"] >= 12
+        if raw:   # bare launches: the coherence layer saw nothing, the containers still say "host copy valid"
+            assert st["h2d_count"] == 0 and vo.state() == S.ST_HOST
+            continue
+        assert st["h2d_count"] == 0 and st["h2d_elided"] >= 9      # inputs stayed on the device
+        assert_overlap(vo.numpy(), ref, ab)
+        assert np.array_equal(vs.numpy(), O.scan_i32(O.FN_ADD, O.SCAN_INCLUSIVE, 0, v))
+        assert res.numpy()[2] == O.reduce_i32(O.FN_ADD, v)[0]
+    with pytest.raises(S.SkelError):
+        ctx.replay_begin(), ctx.replay_run(False, 1)   # still recording
+    ctx.replay_end()
+    for c in (vx, vo, vi, vs, res):
+        c.destroy()
