@@ -77,6 +77,9 @@ def _lib() -> C.CDLL:
         L.oracle_mapoverlap_1d_matrix_f32.argtypes = [_f32p, i, i, dbl, i, _f32p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_1d_matrix_f64.argtypes = [_f32p, i, i, dbl, i, _f64p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_2d_f32.argtypes = [_f32p, i, i, i, dbl, _f32p, sz, sz, sz, sz, _f64p, _f64p]
+        L.oracle_mapoverlap_1d_i32.argtypes = [_i32p, i, i, C.c_int32, _i32p, sz, sz, sz, _i32p]
+        L.oracle_mapoverlap_1d_matrix_i32.argtypes = [_i32p, i, i, C.c_int32, i, _i32p, sz, sz, _i32p]
+        L.oracle_mapoverlap_2d_i32.argtypes = [_i32p, i, i, i, C.c_int32, _i32p, sz, sz, _i32p]
         for name in ("oracle_reduce_f32", "oracle_reduce_i32", "oracle_mapreduce_f32", "oracle_mapreduce_i32",
                      "oracle_reduce_rows_f32", "oracle_reduce_rows_i32"):
             getattr(L, name).restype = i
@@ -234,3 +237,34 @@ def mapoverlap_2d(W, ry: int, rx: int, edge: int, pad: float, X, row0: int = 0, 
     ab = np.empty((row1 - row0, cols), np.float64)
     _lib().oracle_mapoverlap_2d_f32(W, ry, rx, edge, float(pad), X, rows, cols, row0, row1, out, ab)
     return out, ab
+
+
+# ---------------------------------------------------------------- int32 MapOverlap (wraps modulo 2^32)
+def mapoverlap_1d_i32(w, r: int, edge: int, pad: int, x, i0: int = 0, i1: int | None = None) -> np.ndarray:
+    w = _c(w, np.int32)
+    x = _c(x, np.int32)
+    assert w.size == 2 * r + 1
+    i1 = x.size if i1 is None else i1
+    out = np.empty(i1 - i0, np.int32)
+    _lib().oracle_mapoverlap_1d_i32(w, r, edge, int(pad), x, x.size, i0, i1, out)
+    return out
+
+
+def mapoverlap_1d_matrix_i32(w, r: int, edge: int, pad: int, axis: int, X) -> np.ndarray:
+    w = _c(w, np.int32)
+    X = _c(X, np.int32)
+    assert w.size == 2 * r + 1 and X.ndim == 2
+    rows, cols = X.shape
+    out = np.empty((rows, cols), np.int32)
+    _lib().oracle_mapoverlap_1d_matrix_i32(w, r, edge, int(pad), axis, X.reshape(-1), rows, cols, out.reshape(-1))
+    return out
+
+
+def mapoverlap_2d_i32(W, ry: int, rx: int, edge: int, pad: int, X) -> np.ndarray:
+    W = _c(W, np.int32).reshape(-1)
+    X = _c(X, np.int32)
+    assert W.size == (2 * ry + 1) * (2 * rx + 1) and X.ndim == 2
+    rows, cols = X.shape
+    out = np.empty((rows, cols), np.int32)
+    _lib().oracle_mapoverlap_2d_i32(W, ry, rx, edge, int(pad), X.reshape(-1), rows, cols, out.reshape(-1))
+    return out

@@ -22,7 +22,9 @@
 // impulse / one-hot-weight shift tests (orientation, indexing, edge policy, bit-exact), split and
 // permutation invariants, the separable identity (row pass . col pass == dense outer-product
 // filter), transpose symmetry, library special cases (numpy cumsum / correlate / math.fsum), and
-// brute-force pure-Python loops on tiny inputs. No function here is "parity unpinned".
+// brute-force pure-Python loops on tiny inputs; the int32 MapOverlap functions against exact Python integers,
+// numpy.correlate on int64, one-hot shifts and the fp64 functions above on small values (where both are exact).
+// No function here is "parity unpinned".
 //
 // The `#pragma omp parallel for` lines only take effect in the -fopenmp build (liboracle_omp.so),
 // which runs the SAME loops over independent outputs in parallel; it is used for timing and for
@@ -151,11 +153,35 @@ void overlap2_rows(const float* W, int ry, int rx, int edge, double pad, const T
     }
 }
 
+// ---- int32 MapOverlap ("i32 element types for all skeletons"; reading 26): the same
+// definitions with int32 data, int32 weights and an int32 pad value; every product and every sum wraps modulo 2^32
+// (computed on uint32_t, like the int32 Map / Reduce / Scan: reading (c).2 ii). x~ follows the same edge policies.
+inline uint32_t iext1(const int32_t* x, ptrdiff_t n, ptrdiff_t stride, ptrdiff_t j, int edge, int32_t pad) {
+  if (j >= 0 && j < n) return u32(x[j * stride]);
+  if (edge == EDGE_CONSTANT) return u32(pad);
+  if (edge == EDGE_CYCLIC) return u32(x[wrapi(j, n) * stride]);
+  return u32(x[clampi(j, 0, n - 1) * stride]);
+}
+
+inline int32_t ioverlap1_at(const int32_t* w, int r, int edge, int32_t pad, const int32_t* x, ptrdiff_t n,
+                            ptrdiff_t stride, ptrdiff_t i) {
+  uint32_t acc = 0;
+  for (int k = -r; k <= r; ++k) acc += u32(w[k + r]) * iext1(x, n, stride, i + k, edge, pad);
+  return i32(acc);
+}
+
+inline uint32_t iext2(const int32_t* X, ptrdiff_t rows, ptrdiff_t cols, ptrdiff_t p, ptrdiff_t q, int edge, int32_t pad) {
+  if (p >= 0 && p < rows && q >= 0 && q < cols) return u32(X[p * cols + q]);
+  if (edge == EDGE_CONSTANT) return u32(pad);
+  if (edge == EDGE_CYCLIC) return u32(X[wrapi(p, rows) * cols + wrapi(q, cols)]);
+  return u32(X[clampi(p, 0, rows - 1) * cols + clampi(q, 0, cols - 1)]);
+}
+
 }  // namespace
 
 extern "C" {
 
-int oracle_abi_version(void) { return 1; }
+int oracle_abi_version(void) { return 2; }
 
 // ---- Map (reading (c).1). out[i] = f(in0[i], b_i), b_i = in1[i] or the constant c (rounded to
 // fp32 first, reading (c).1 iii). Result in fp64.
@@ -345,6 +371,39 @@ void oracle_mapoverlap_2d_f32(const float* W, int ry, int rx, int edge, double p
                               double* absout) {
   overlap2_rows(W, ry, rx, edge, pad, X, static_cast<ptrdiff_t>(rows), static_cast<ptrdiff_t>(cols),
                 static_cast<ptrdiff_t>(row0), static_cast<ptrdiff_t>(row1), out, absout);
+}
+
+// ---- int32 MapOverlap: 1D on a vector (outputs [i0, i1)), 1D along the rows / columns of a matrix, 2D
+void oracle_mapoverlap_1d_i32(const int32_t* w, int r, int edge, int32_t pad, const int32_t* x, size_t n, size_t i0,
+                              size_t i1, int32_t* out) {
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = static_cast<ptrdiff_t>(i0); i < static_cast<ptrdiff_t>(i1); ++i)
+    out[i - i0] = ioverlap1_at(w, r, edge, pad, x, static_cast<ptrdiff_t>(n), 1, i);
+}
+
+void oracle_mapoverlap_1d_matrix_i32(const int32_t* w, int r, int edge, int32_t pad, int axis, const int32_t* X,
+                                     size_t rows_, size_t cols_, int32_t* out) {
+  const ptrdiff_t rows = static_cast<ptrdiff_t>(rows_), cols = static_cast<ptrdiff_t>(cols_);
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < rows; ++i)
+    for (ptrdiff_t j = 0; j < cols; ++j)
+      out[i * cols + j] = axis == AXIS_ROW ? ioverlap1_at(w, r, edge, pad, X + i * cols, cols, 1, j)
+                                           : ioverlap1_at(w, r, edge, pad, X + j, rows, cols, i);
+}
+
+void oracle_mapoverlap_2d_i32(const int32_t* W, int ry, int rx, int edge, int32_t pad, const int32_t* X, size_t rows_,
+                              size_t cols_, int32_t* out) {
+  const ptrdiff_t rows = static_cast<ptrdiff_t>(rows_), cols = static_cast<ptrdiff_t>(cols_);
+  const int fw = 2 * rx + 1;
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < rows; ++i)
+    for (ptrdiff_t j = 0; j < cols; ++j) {
+      uint32_t acc = 0;
+      for (int a = -ry; a <= ry; ++a)
+        for (int b = -rx; b <= rx; ++b)
+          acc += u32(W[(a + ry) * fw + (b + rx)]) * iext2(X, rows, cols, i + a, j + b, edge, pad);
+      out[i * cols + j] = i32(acc);
+    }
 }
 
 }  // extern "C"

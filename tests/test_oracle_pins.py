@@ -719,3 +719,119 @@ def test_overlap2d_cyclic_matches_rolls_and_constant_input():
     a1, _ = O.mapoverlap_1d_matrix(wc, 2, O.EDGE_CYCLIC, 0.0, O.AXIS_COL, X)
     a2, _ = O.mapoverlap_2d(wc, 2, 0, O.EDGE_CYCLIC, 0.0, X)
     assert np.array_equal(a1, a2)
+
+
+# ------------------------------------------------------------------ int32 MapOverlap (wraps mod 2^32)
+def _py_ext(x, j, edge, pad):
+    n = len(x)
+    if 0 <= j < n:
+        return int(x[j])
+    if edge == O.EDGE_CONSTANT:
+        return int(pad)
+    if edge == O.EDGE_CYCLIC:
+        return int(x[j % n])
+    return int(x[min(max(j, 0), n - 1)])
+
+
+ALL_EDGES = [O.EDGE_CONSTANT, O.EDGE_DUPLICATE, O.EDGE_CYCLIC]
+
+
+@pytest.mark.parametrize("edge", ALL_EDGES)
+def test_overlap1d_i32_brute_force_python_ints(edge):
+    """Exact Python integers, full-range data and weights (every product and the sum overflow): a dropped tap, a
+    flipped filter, a wrong clamp or a missing wrap fails."""
+    for r in (0, 1, 2, 5, 16):
+        w = I.full_range_i32(300 + r, 2 * r + 1)
+        for n in (1, 2, 3, 7, 33, 70):   # n < r included: the index clamps / wraps more than once
+            x = I.full_range_i32(301 + n + r, n)
+            pad = -123456789
+            got = O.mapoverlap_1d_i32(w, r, edge, pad, x)
+            exp = [wrap32(sum(int(w[k + r]) * _py_ext(x, i + k, edge, pad) for k in range(-r, r + 1))) for i in range(n)]
+            assert got.tolist() == exp, (r, n)
+            # a sub-range of the outputs is the same numbers
+            if n > 4:
+                assert O.mapoverlap_1d_i32(w, r, edge, pad, x, 2, n - 1).tolist() == exp[2:n - 1]
+
+
+def test_overlap1d_i32_one_hot_shift_impulse_constant_and_library():
+    n, r = 257, 4
+    x = I.full_range_i32(310, n)
+    for m in range(2 * r + 1):                       # one-hot weights: a pure shift, bit-exact, no flip
+        w = np.zeros(2 * r + 1, np.int32)
+        w[m] = 1
+        j = np.arange(n) + m - r
+        assert np.array_equal(O.mapoverlap_1d_i32(w, r, O.EDGE_DUPLICATE, 0, x), x[np.clip(j, 0, n - 1)])
+        assert np.array_equal(O.mapoverlap_1d_i32(w, r, O.EDGE_CYCLIC, 0, x), x[j % n])
+        exp = np.where((j >= 0) & (j < n), x[np.clip(j, 0, n - 1)], np.int32(77))
+        assert np.array_equal(O.mapoverlap_1d_i32(w, r, O.EDGE_CONSTANT, 77, x), exp)
+    w = I.uniform_int_i32(311, 2 * r + 1, 1000) - 500
+    e = np.zeros(n, np.int32)                        # impulse at j: out[i] = w[(j - i) + r] (orientation)
+    e[100] = 1
+    out = O.mapoverlap_1d_i32(w, r, O.EDGE_CONSTANT, 0, e)
+    assert out[100 - r:100 + r + 1].tolist() == w[::-1].tolist() and out.sum() == w.sum()
+    K = 123457                                        # constant input: K * sum(w) mod 2^32 everywhere (DUPLICATE)
+    assert O.mapoverlap_1d_i32(w, r, O.EDGE_DUPLICATE, 0, np.full(n, K, np.int32)).tolist() == [wrap32(K * int(w.sum()))] * n
+    # library special case: numpy.correlate on int64 (no overflow for small values) == interior outputs
+    xs = I.uniform_int_i32(312, n, 1000)
+    lib = np.correlate(xs.astype(np.int64), w.astype(np.int64), mode="valid")
+    assert np.array_equal(O.mapoverlap_1d_i32(w, r, O.EDGE_CONSTANT, 0, xs)[r:n - r].astype(np.int64), lib)
+    # small values: the fp64 oracle of the same numbers is exact and must agree, every edge policy
+    for edge in ALL_EDGES:
+        f, _ = O.mapoverlap_1d(w.astype(np.float32), r, edge, 3.0, xs.astype(np.float32))
+        assert np.array_equal(O.mapoverlap_1d_i32(w, r, edge, 3, xs).astype(np.float64), f)
+
+
+@pytest.mark.parametrize("edge", ALL_EDGES)
+def test_overlap_matrix_and_2d_i32(edge):
+    rows, cols = 9, 13
+    X = I.full_range_i32(320, rows * cols).reshape(rows, cols)
+    pad = 40000
+    for r in (1, 3, 10):                              # 10 > rows: clamps / wraps through the whole matrix
+        w = I.full_range_i32(321 + r, 2 * r + 1)
+        got_r = O.mapoverlap_1d_matrix_i32(w, r, edge, pad, O.AXIS_ROW, X)
+        got_c = O.mapoverlap_1d_matrix_i32(w, r, edge, pad, O.AXIS_COL, X)
+        for i in range(rows):                          # every row / column is the vector call on that row / column
+            assert np.array_equal(got_r[i], O.mapoverlap_1d_i32(w, r, edge, pad, X[i]))
+        for j in range(cols):
+            assert np.array_equal(got_c[:, j], O.mapoverlap_1d_i32(w, r, edge, pad, np.ascontiguousarray(X[:, j])))
+        assert np.array_equal(got_c, O.mapoverlap_1d_matrix_i32(w, r, edge, pad, O.AXIS_ROW, np.ascontiguousarray(X.T)).T)
+    for ry, rx in ((0, 0), (1, 2), (2, 2), (4, 1)):
+        W = I.full_range_i32(330 + 9 * ry + rx, (2 * ry + 1) * (2 * rx + 1)).reshape(2 * ry + 1, 2 * rx + 1)
+        got = O.mapoverlap_2d_i32(W, ry, rx, edge, pad, X)
+
+        def ext(p, q):
+            if 0 <= p < rows and 0 <= q < cols:
+                return int(X[p, q])
+            if edge == O.EDGE_CONSTANT:
+                return pad
+            if edge == O.EDGE_CYCLIC:
+                return int(X[p % rows, q % cols])
+            return int(X[min(max(p, 0), rows - 1), min(max(q, 0), cols - 1)])
+
+        exp = [[wrap32(sum(int(W[a + ry, b + rx]) * ext(i + a, j + b) for a in range(-ry, ry + 1) for b in range(-rx, rx + 1)))
+                for j in range(cols)] for i in range(rows)]
+        assert got.tolist() == exp, (ry, rx)
+    # degenerate axes: ry = 0 is the row-wise 1D call, rx = 0 the column-wise one; one-hot 2D weights shift both ways
+    w = I.full_range_i32(340, 5)
+    assert np.array_equal(O.mapoverlap_2d_i32(w.reshape(1, 5), 0, 2, edge, pad, X), O.mapoverlap_1d_matrix_i32(w, 2, edge, pad, O.AXIS_ROW, X))
+    assert np.array_equal(O.mapoverlap_2d_i32(w.reshape(5, 1), 2, 0, edge, pad, X), O.mapoverlap_1d_matrix_i32(w, 2, edge, pad, O.AXIS_COL, X))
+    W = np.zeros((3, 3), np.int32)
+    W[0, 2] = 1                                       # out[i][j] = X~[i-1][j+1]
+    p, q = np.arange(rows)[:, None] - 1, np.arange(cols)[None, :] + 1
+    if edge == O.EDGE_DUPLICATE:
+        exp = X[np.clip(p, 0, rows - 1), np.clip(q, 0, cols - 1)]
+    elif edge == O.EDGE_CYCLIC:
+        exp = X[p % rows, q % cols]
+    else:
+        exp = np.where((p >= 0) & (q < cols), X[np.clip(p, 0, rows - 1), np.clip(q, 0, cols - 1)], np.int32(pad))
+    assert np.array_equal(O.mapoverlap_2d_i32(W, 1, 1, edge, pad, X), exp)
+    # small values agree with the (exact) fp64 oracle; the OpenMP build computes the same numbers
+    Xs = I.uniform_int_i32(341, rows * cols, 100).reshape(rows, cols)
+    Ws = (I.uniform_int_i32(342, 25, 20) - 10).reshape(5, 5)
+    f, _ = O.mapoverlap_2d(Ws.astype(np.float32), 2, 2, edge, 7.0, Xs.astype(np.float32))
+    assert np.array_equal(O.mapoverlap_2d_i32(Ws, 2, 2, edge, 7, Xs).astype(np.float64), f)
+    O.use_openmp(True)
+    try:
+        assert np.array_equal(O.mapoverlap_2d_i32(Ws, 2, 2, edge, 7, Xs).astype(np.float64), f)
+    finally:
+        O.use_openmp(False)
