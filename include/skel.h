@@ -248,6 +248,19 @@ skel_status skel_mapoverlap_1d_matrix(skel_ctx* ctx, const float* w, int r, skel
  * W: HOST pointer, (2ry+1)*(2rx+1) floats row-major. 0 <= ry, rx <= SKEL_MAX_RADIUS_2D. */
 skel_status skel_mapoverlap_2d(skel_ctx* ctx, const float* W, int ry, int rx, skel_edge edge, double pad,
                                const skel_matrix* in, skel_matrix* out);
+
+/* MapOverlap on int32 containers (the skeletons are generic in the element type, PAPER.md L75, L81;
+ * DESIGN.md reading 26): the same three calls with int32 data, int32 weights (HOST pointer, copied at call time)
+ * and an int32 pad value. Every product and every sum wraps modulo 2^32 (like the int32 Map / Reduce / Scan), so the
+ * result does not depend on the summation order and is bit-exact against the definition. Same radii, edge policies,
+ * aliasing and shape rules; f32 containers -> SKEL_ERR_DTYPE (and int32 containers in the f32 calls likewise).
+ * Kernels: the direct, register-window and TMA-fed variants with an integer multiply-add. */
+skel_status skel_mapoverlap_1d_i32(skel_ctx* ctx, const int32_t* w, int r, skel_edge edge, int32_t pad,
+                                   const skel_vector* in, skel_vector* out);
+skel_status skel_mapoverlap_1d_matrix_i32(skel_ctx* ctx, const int32_t* w, int r, skel_edge edge, int32_t pad,
+                                          skel_axis axis, const skel_matrix* in, skel_matrix* out);
+skel_status skel_mapoverlap_2d_i32(skel_ctx* ctx, const int32_t* W, int ry, int rx, skel_edge edge, int32_t pad,
+                                   const skel_matrix* in, skel_matrix* out);
 /* Separable MapOverlap (BASELINE.json configs[3] "separable row-then-column 1D
  * passes"): out = colpass(w_col, r_col, T), T = RN_f32(rowpass(w_row, r_row, in)), each pass with the
  * edge policy, i.e. by definition the result of skel_mapoverlap_1d_matrix(ROW) into a temporary

@@ -106,6 +106,9 @@ _SIGS = {
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
+    "skel_mapoverlap_1d_i32": ([_vp, _vp, _i, _i, C.c_int32, _vp, _vp], _i),
+    "skel_mapoverlap_1d_matrix_i32": ([_vp, _vp, _i, _i, C.c_int32, _i, _vp, _vp], _i),
+    "skel_mapoverlap_2d_i32": ([_vp, _vp, _i, _i, _i, C.c_int32, _vp, _vp], _i),
     "skel_mapoverlap_separable": ([_vp, _vp, _i, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_scan": ([_vp, _i, _i, _d, _vp, _vp], _i),
     "skel_variant_count": ([_i], _i),
@@ -355,6 +358,21 @@ class Context:
         W = np.ascontiguousarray(W, np.float32)
         assert W.size == (2 * ry + 1) * (2 * rx + 1)
         self.check(lib.skel_mapoverlap_2d(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
+
+    def mapoverlap_1d_i32(self, w, r: int, edge: int, pad: int, x: "Vector", out: "Vector"):
+        w = np.ascontiguousarray(w, np.int32)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d_i32(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, x.h, out.h))
+
+    def mapoverlap_1d_matrix_i32(self, w, r: int, edge: int, pad: int, axis: int, x: "Matrix", out: "Matrix"):
+        w = np.ascontiguousarray(w, np.int32)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d_matrix_i32(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, axis, x.h, out.h))
+
+    def mapoverlap_2d_i32(self, W, ry: int, rx: int, edge: int, pad: int, x: "Matrix", out: "Matrix"):
+        W = np.ascontiguousarray(W, np.int32)
+        assert W.size == (2 * ry + 1) * (2 * rx + 1)
+        self.check(lib.skel_mapoverlap_2d_i32(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
 
     def mapoverlap_separable(self, w_row, r_row: int, w_col, r_col: int, edge: int, pad: float, x: "Matrix", out: "Matrix"):
         wr, wc = np.ascontiguousarray(w_row, np.float32), np.ascontiguousarray(w_col, np.float32)

@@ -681,9 +681,9 @@ bool variant_ok(const Call& k, int v) {
     case SKEL_SK_REDUCE:
     case SKEL_SK_MAPREDUCE: return reduce_variant_ok(v, k.in0, k.in1, k.n);
     case SKEL_SK_SCAN: return scan_variant_ok(v, k.inst.dtype, k.in0, k.out, k.n);
-    case SKEL_SK_OVERLAP1D: return overlap1d_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
-    case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_ok(v, k.inst.r0, k.in0, k.out, k.rows, k.cols);
-    case SKEL_SK_OVERLAP2D: return overlap2d_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_OVERLAP1D: return overlap1d_variant_ok(v, k.inst.dtype, k.inst.r0, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_OVERLAP1D_COL: return overlap1d_col_variant_ok(v, k.inst.dtype, k.inst.r0, k.in0, k.out, k.rows, k.cols);
+    case SKEL_SK_OVERLAP2D: return overlap2d_variant_ok(v, k.inst.dtype, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_SEPARABLE: return separable_variant_ok(v, k.inst.r0, k.inst.r1, k.in0, k.out, k.rows, k.cols);
     case SKEL_SK_REDUCE_ROWS: return reduce_rows_variant_ok(v, k.in0, k.rows, k.cols);
   }
@@ -697,6 +697,8 @@ const int* preference(int sk, int dtype, int* count) {
   static const int scan_i[] = {15, 3, 0, 4, 5};
   static const int scan_f[] = {4, 5};
   static const int o1_p[] = {2, 1, 0};
+  static const int o1_i[] = {10, 8, 4, 0};  // int32 elements: tma_swz_o16_s3, regshfl_2x8, regshfl_o16, direct
+  static const int tma_i[] = {5, 0};        // int32 columns / 2D: tma_oy4, direct
   static const int col_p[] = {2, 0};
   static const int o2_p[] = {1, 0};
   static const int sep_p[] = {4, 1, 0};
@@ -708,9 +710,15 @@ const int* preference(int sk, int dtype, int* count) {
     case SKEL_SK_SCAN:
       if (dtype == SKEL_I32) { *count = 5; return scan_i; }
       *count = 2; return scan_f;
-    case SKEL_SK_OVERLAP1D: *count = 3; return o1_p;
-    case SKEL_SK_OVERLAP1D_COL: *count = 2; return col_p;
-    case SKEL_SK_OVERLAP2D: *count = 2; return o2_p;
+    case SKEL_SK_OVERLAP1D:
+      if (dtype == SKEL_I32) { *count = 4; return o1_i; }
+      *count = 3; return o1_p;
+    case SKEL_SK_OVERLAP1D_COL:
+      if (dtype == SKEL_I32) { *count = 2; return tma_i; }
+      *count = 2; return col_p;
+    case SKEL_SK_OVERLAP2D:
+      if (dtype == SKEL_I32) { *count = 2; return tma_i; }
+      *count = 2; return o2_p;
     case SKEL_SK_SEPARABLE: *count = 3; return sep_p;
     case SKEL_SK_REDUCE_ROWS: *count = 2; return rows_p;
   }
@@ -793,13 +801,13 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
     case SKEL_SK_SCAN:
       return launch_scan(L, c->scratch, v, i.dtype, i.fn, i.mode == SKEL_SCAN_EXCLUSIVE, k.cbits, k.in0, k.out, k.n);
     case SKEL_SK_OVERLAP1D:
-      return launch_overlap1d_rows(L, v, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
+      return launch_overlap1d_rows(L, v, i.dtype, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
                                    static_cast<float*>(k.out), k.rows, k.cols);
     case SKEL_SK_OVERLAP1D_COL:
-      return launch_overlap1d_cols(L, v, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
+      return launch_overlap1d_cols(L, v, i.dtype, k.w1, i.r0, i.edge, k.pad, static_cast<const float*>(k.in0),
                                    static_cast<float*>(k.out), k.rows, k.cols);
     case SKEL_SK_OVERLAP2D:
-      return launch_overlap2d(L, v, k.w2, i.r0, i.r1, i.edge, k.pad, static_cast<const float*>(k.in0),
+      return launch_overlap2d(L, v, i.dtype, k.w2, i.r0, i.r1, i.edge, k.pad, static_cast<const float*>(k.in0),
                               static_cast<float*>(k.out), k.rows, k.cols);
   }
   return cudaErrorInvalidValue;
@@ -834,7 +842,7 @@ int chain_kind(const skel_ctx* c, const Call& k) {
   if (i.skeleton == SKEL_SK_MAP && i.dtype == SKEL_F32 && i.mode == 0 &&
       (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MULT || i.fn == SKEL_FN_MAX))
     return 1;
-  if (i.skeleton == SKEL_SK_OVERLAP1D && k.rows == 1 && i.r0 >= 0 && i.r0 <= 16) return 2;
+  if (i.skeleton == SKEL_SK_OVERLAP1D && i.dtype == SKEL_F32 && k.rows == 1 && i.r0 >= 0 && i.r0 <= 16) return 2;
   if (i.skeleton == SKEL_SK_REDUCE && i.dtype == SKEL_F32 && (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MAX)) return 3;
   return 0;
 }
@@ -1040,8 +1048,10 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   return SKEL_OK;
 }
 
-skel_status overlap_check(skel_ctx* c, const Handle* in, const Handle* out, int edge) {
-  if (in->st->dtype != SKEL_F32 || out->st->dtype != SKEL_F32) return fail(c, SKEL_ERR_DTYPE, "MapOverlap is defined for f32 only");
+skel_status overlap_check(skel_ctx* c, const Handle* in, const Handle* out, int edge, int dtype = SKEL_F32) {
+  if (in->st->dtype != dtype || out->st->dtype != dtype)
+    return fail(c, SKEL_ERR_DTYPE, dtype == SKEL_F32 ? "skel_mapoverlap_*: f32 containers expected (int32: skel_mapoverlap_*_i32)"
+                                                    : "skel_mapoverlap_*_i32: int32 containers expected");
   if (in->rows != out->rows || in->cols != out->cols) return fail(c, SKEL_ERR_SIZE_MISMATCH, "input and output shapes differ");
   if (in->st == out->st) return fail(c, SKEL_ERR_ALIAS, "MapOverlap output must not alias its input");
   if (edge != SKEL_EDGE_CONSTANT && edge != SKEL_EDGE_DUPLICATE && edge != SKEL_EDGE_CYCLIC) return fail(c, SKEL_ERR_INVALID_ARG, "bad edge policy");
@@ -1490,68 +1500,98 @@ skel_status skel_reduce_rows(skel_ctx* c, skel_fn op, const skel_matrix* in, ske
 }
 
 // ---- MapOverlap -----------------------------------------------------------------------------------
+namespace {
+// dtype: SKEL_F32 (w: floats, pad rounded to f32) or SKEL_I32 (w: int32, pad an int32): 32-bit images either way
+skel_status overlap1d_impl(skel_ctx* c, int dtype, const void* w, int r, skel_edge edge, uint32_t pad_bits, int axis,
+                           const Handle* in, Handle* out, bool is_matrix) {
+  if (!w) return fail(c, SKEL_ERR_INVALID_ARG, "NULL weights");
+  if (is_matrix && axis != SKEL_AXIS_ROW && axis != SKEL_AXIS_COL) return fail(c, SKEL_ERR_INVALID_ARG, "bad axis");
+  if (r < 0 || r > SKEL_MAX_RADIUS_1D) return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge, dtype);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = (!is_matrix || axis == SKEL_AXIS_ROW) ? SKEL_SK_OVERLAP1D : SKEL_SK_OVERLAP1D_COL;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = dtype;
+  k.inst.r0 = r;
+  k.inst.edge = edge;
+  k.inst.mode = (is_matrix && axis == SKEL_AXIS_ROW && in->rows > 1) ? 1 : 0;  // shape class of the plan's dispatch tree
+  memcpy(&k.pad, &pad_bits, 4);
+  memcpy(k.w1.w, w, 4 * size_t(2 * r + 1));
+  k.rows = is_matrix ? in->rows : 1;
+  k.cols = is_matrix ? in->cols : in->st->n;
+  return overlap_run(c, k, in, out);
+}
+
+skel_status overlap2d_impl(skel_ctx* c, int dtype, const void* W, int ry, int rx, skel_edge edge, uint32_t pad_bits,
+                           const skel_matrix* in, skel_matrix* out) {
+  if (!W) return fail(c, SKEL_ERR_INVALID_ARG, "NULL weights");
+  if (ry < 0 || rx < 0 || ry > SKEL_MAX_RADIUS_2D || rx > SKEL_MAX_RADIUS_2D)
+    return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge, dtype);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = SKEL_SK_OVERLAP2D;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = dtype;
+  k.inst.r0 = ry;
+  k.inst.r1 = rx;
+  k.inst.edge = edge;
+  memcpy(&k.pad, &pad_bits, 4);
+  memcpy(k.w2.w, W, 4 * size_t(2 * ry + 1) * size_t(2 * rx + 1));
+  k.rows = in->rows;
+  k.cols = in->cols;
+  return overlap_run(c, k, in, out);
+}
+
+uint32_t f32_bits(double v) {
+  const float f = static_cast<float>(v);
+  uint32_t b;
+  memcpy(&b, &f, 4);
+  return b;
+}
+}  // namespace
+
 skel_status skel_mapoverlap_1d(skel_ctx* c, const float* w, int r, skel_edge edge, double pad, const skel_vector* in,
                                skel_vector* out) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
-  if (!vec_ok(in) || !vec_ok(out) || !w) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
-  if (r < 0 || r > SKEL_MAX_RADIUS_1D) return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
-  skel_status st = overlap_check(c, in, out, edge);
-  if (st != SKEL_OK) return st;
-  Call k;
-  k.inst.skeleton = SKEL_SK_OVERLAP1D;
-  k.inst.fn = SKEL_FN_WSTENCIL;
-  k.inst.dtype = SKEL_F32;
-  k.inst.r0 = r;
-  k.inst.edge = edge;
-  k.pad = static_cast<float>(pad);
-  memcpy(k.w1.w, w, sizeof(float) * (2 * r + 1));
-  k.rows = 1;
-  k.cols = in->st->n;
-  return overlap_run(c, k, in, out);
+  if (!vec_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap1d_impl(c, SKEL_F32, w, r, edge, f32_bits(pad), SKEL_AXIS_ROW, in, out, false);
 }
 
 skel_status skel_mapoverlap_1d_matrix(skel_ctx* c, const float* w, int r, skel_edge edge, double pad, skel_axis axis,
                                       const skel_matrix* in, skel_matrix* out) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
-  if (!mat_ok(in) || !mat_ok(out) || !w) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
-  if (axis != SKEL_AXIS_ROW && axis != SKEL_AXIS_COL) return fail(c, SKEL_ERR_INVALID_ARG, "bad axis");
-  if (r < 0 || r > SKEL_MAX_RADIUS_1D) return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
-  skel_status st = overlap_check(c, in, out, edge);
-  if (st != SKEL_OK) return st;
-  Call k;
-  k.inst.skeleton = axis == SKEL_AXIS_ROW ? SKEL_SK_OVERLAP1D : SKEL_SK_OVERLAP1D_COL;
-  k.inst.fn = SKEL_FN_WSTENCIL;
-  k.inst.dtype = SKEL_F32;
-  k.inst.r0 = r;
-  k.inst.edge = edge;
-  k.inst.mode = (axis == SKEL_AXIS_ROW && in->rows > 1) ? 1 : 0;  // shape class of the plan's dispatch tree
-  k.pad = static_cast<float>(pad);
-  memcpy(k.w1.w, w, sizeof(float) * (2 * r + 1));
-  k.rows = in->rows;
-  k.cols = in->cols;
-  return overlap_run(c, k, in, out);
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap1d_impl(c, SKEL_F32, w, r, edge, f32_bits(pad), axis, in, out, true);
 }
 
 skel_status skel_mapoverlap_2d(skel_ctx* c, const float* W, int ry, int rx, skel_edge edge, double pad,
                                const skel_matrix* in, skel_matrix* out) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
-  if (!mat_ok(in) || !mat_ok(out) || !W) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle or NULL weights");
-  if (ry < 0 || rx < 0 || ry > SKEL_MAX_RADIUS_2D || rx > SKEL_MAX_RADIUS_2D)
-    return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
-  skel_status st = overlap_check(c, in, out, edge);
-  if (st != SKEL_OK) return st;
-  Call k;
-  k.inst.skeleton = SKEL_SK_OVERLAP2D;
-  k.inst.fn = SKEL_FN_WSTENCIL;
-  k.inst.dtype = SKEL_F32;
-  k.inst.r0 = ry;
-  k.inst.r1 = rx;
-  k.inst.edge = edge;
-  k.pad = static_cast<float>(pad);
-  memcpy(k.w2.w, W, sizeof(float) * (2 * ry + 1) * (2 * rx + 1));
-  k.rows = in->rows;
-  k.cols = in->cols;
-  return overlap_run(c, k, in, out);
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap2d_impl(c, SKEL_F32, W, ry, rx, edge, f32_bits(pad), in, out);
+}
+
+skel_status skel_mapoverlap_1d_i32(skel_ctx* c, const int32_t* w, int r, skel_edge edge, int32_t pad,
+                                   const skel_vector* in, skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap1d_impl(c, SKEL_I32, w, r, edge, static_cast<uint32_t>(pad), SKEL_AXIS_ROW, in, out, false);
+}
+
+skel_status skel_mapoverlap_1d_matrix_i32(skel_ctx* c, const int32_t* w, int r, skel_edge edge, int32_t pad, skel_axis axis,
+                                          const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap1d_impl(c, SKEL_I32, w, r, edge, static_cast<uint32_t>(pad), axis, in, out, true);
+}
+
+skel_status skel_mapoverlap_2d_i32(skel_ctx* c, const int32_t* W, int ry, int rx, skel_edge edge, int32_t pad,
+                                   const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap2d_impl(c, SKEL_I32, W, ry, rx, edge, static_cast<uint32_t>(pad), in, out);
 }
 
 skel_status skel_mapoverlap_separable(skel_ctx* c, const float* w_row, int r_row, const float* w_col, int r_col,

@@ -158,6 +158,26 @@ template <int FN> __device__ __forceinline__ int32_t apply_fn(int32_t c, int32_t
   else return a;
 }
 
+// ---- MapOverlap element arithmetic ---------------------------------------------------------------
+// The stencil kernels move 32-bit register images typed `float` whatever the element type (loads, shared memory, TMA,
+// shuffles and stores do not look at the bits); only the multiply-add of a tap and the addition of two partial sums
+// interpret them. f32: one fused multiply-add (FFMA); i32: multiply-add modulo 2^32 on uint32_t (IMAD), DESIGN.md
+// reading 26. The packed FFMA2 forms exist for f32 only.
+template <typename T> struct StencilOps;
+template <> struct StencilOps<float> {
+  static constexpr bool kFloat = true;
+  static __device__ __forceinline__ float mad(float w, float x, float acc) { return fmaf(w, x, acc); }
+  static __device__ __forceinline__ float add(float a, float b) { return a + b; }
+};
+template <> struct StencilOps<int32_t> {
+  static constexpr bool kFloat = false;
+  static __device__ __forceinline__ float mad(float w, float x, float acc) {
+    return __uint_as_float(__float_as_uint(w) * __float_as_uint(x) + __float_as_uint(acc));
+  }
+  static __device__ __forceinline__ float add(float a, float b) { return __uint_as_float(__float_as_uint(a) + __float_as_uint(b)); }
+};
+__device__ __forceinline__ bool bits_are_zero(float v) { return __float_as_uint(v) == 0u; }
+
 // identity element of a reduction operator
 template <typename T, int OP> __device__ __forceinline__ T identity() {
   if constexpr (OP == FN_ADD) return T(0);

@@ -64,6 +64,8 @@ cudaError_t launch_scan(const Launch& L, Scratch& S, int v, int dtype, int op, b
 size_t scan_tiles_needed(size_t n);
 
 // ---- MapOverlap ---------------------------------------------------------------------------------
+// Weights travel as 32-bit images typed float: for int32 elements (dtype = DT_I32) w[] holds the int32 bit patterns
+// and so does `pad`; the data pointers are typed float* for the same reason (common.cuh StencilOps).
 struct Weights1D { float w[129]; };   // 2r+1 <= 129 taps, passed by value (constant bank)
 struct Weights2D { float w[17 * 17]; };
 
@@ -90,21 +92,21 @@ inline Weights2D pad_weights_2d(const Weights2D& w, int ry, int rx, int R) {  //
 
 int overlap1d_variant_count();
 const char* overlap1d_variant_name(int v);
-bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols);
+bool overlap1d_variant_ok(int v, int dtype, int r, const void* in, const void* out, size_t rows, size_t cols);
 // vector: rows = 1. Row-wise on a matrix: every row independently.
-cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+cudaError_t launch_overlap1d_rows(const Launch& L, int v, int dtype, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols);
 
 int overlap1d_col_variant_count();
 const char* overlap1d_col_variant_name(int v);
-bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols);
-cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+bool overlap1d_col_variant_ok(int v, int dtype, int r, const void* in, const void* out, size_t rows, size_t cols);
+cudaError_t launch_overlap1d_cols(const Launch& L, int v, int dtype, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols);
 
 int overlap2d_variant_count();
 const char* overlap2d_variant_name(int v);
-bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols);
-cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
+bool overlap2d_variant_ok(int v, int dtype, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols);
+cudaError_t launch_overlap2d(const Launch& L, int v, int dtype, const Weights2D& w, int ry, int rx, int edge, float pad,
                              const float* in, float* out, size_t rows, size_t cols);
 
 // ---- fused chain [Map(f, c)] -> MapOverlap1D -> [Reduce(op)] on one f32 vector (fused.cu) -----------
@@ -127,10 +129,10 @@ cudaError_t launch_fma_probe(const Launch& L, float* scratch /* device, >= 1 flo
 
 // tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
 template <int R>
-cudaError_t launch_overlap2d_tiled(const Launch& L, int v, const Weights2D& w, int edge, float pad, const float* in,
-                                   float* out, size_t rows, size_t cols);
+cudaError_t launch_overlap2d_tiled(const Launch& L, int v, int dtype, const Weights2D& w, int edge, float pad,
+                                   const float* in, float* out, size_t rows, size_t cols);
 template <int R>
-cudaError_t launch_overlap1d_cols_tiled(const Launch& L, int v, const Weights1D& w, int edge, float pad,
+cudaError_t launch_overlap1d_cols_tiled(const Launch& L, int v, int dtype, const Weights1D& w, int edge, float pad,
                                         const float* in, float* out, size_t rows, size_t cols);
 
 }  // namespace skel

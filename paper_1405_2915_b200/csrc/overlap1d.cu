@@ -36,6 +36,7 @@ __device__ __forceinline__ float ext_row(const float* row, long long cols, long 
 // Up to 33 taps (r <= 16) are ONE chain in ascending tap order, like every tiled variant (so all variants, and the
 // fused separable kernel, give the same bits; bound 33 * 2^-24 = 1.97e-6 of sum|w x|). Longer filters are chained in
 // groups of 16 taps and the group sums added: (16 + #groups - 1) * 2^-24 <= 1.44e-6.
+template <typename T>
 __global__ void __launch_bounds__(256)
 overlap1d_direct_kernel(const __grid_constant__ Weights1D W, int r, int edge, float pad, const float* in, float* out,
                         size_t rows, size_t cols) {
@@ -51,11 +52,11 @@ overlap1d_direct_kernel(const __grid_constant__ Weights1D W, int r, int edge, fl
       const int k1 = min(k0 + chain, 2 * r + 1);
       float acc = 0.f;
       if (interior) {
-        for (int k = k0; k < k1; ++k) acc = fmaf(W.w[k], __ldg(x + j + k - r), acc);
+        for (int k = k0; k < k1; ++k) acc = StencilOps<T>::mad(W.w[k], __ldg(x + j + k - r), acc);
       } else {
-        for (int k = k0; k < k1; ++k) acc = fmaf(W.w[k], ext_row(x, (long long)cols, j + k - r, edge, pad), acc);
+        for (int k = k0; k < k1; ++k) acc = StencilOps<T>::mad(W.w[k], ext_row(x, (long long)cols, j + k - r, edge, pad), acc);
       }
-      total_acc = k0 == 0 ? acc : total_acc + acc;
+      total_acc = k0 == 0 ? acc : StencilOps<T>::add(total_acc, acc);
     }
     out[idx] = total_acc;
   }
@@ -117,10 +118,11 @@ __device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x
 // chunk c ^ (q & 7)); the thread's first group is chunk threadIdx.x * O / 4 + SWZ of the window. With u = t + a
 // (a = (SWZ + g) / 4, b = (SWZ + g) % 4; O = 16) the group's byte address is ((u >> 1) * 128 | (((u & 1) * 4) ^
 // ((u >> 1) & 7)) * 16) ^ (b * 16): one XOR per group on top of five integer instructions per a.
-template <int R, int O, bool PK = false, int SWZ = -1>
+template <int R, int O, bool PK_ = false, int SWZ = -1, typename T = float>
 __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& W, float* orow, long long cols, long long c0) {
   constexpr int HP = (R + 3) / 4 * 4;
   constexpr int NG = (O + 2 * HP) / 4;  // 128-bit groups a thread reads
+  constexpr bool PK = PK_ && StencilOps<T>::kFloat;
   static_assert(SWZ < 0 || O == 16, "the swizzled window form is written for 16 outputs per thread");
   float acc[O];
 #pragma unroll
@@ -151,7 +153,7 @@ __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& 
 #pragma unroll
         for (int o = 1; o < O; o += 2) {  // x[p] -> odd outputs (scalar), before their paired tap p+1
           const int k = 4 * g + e - HP - o + R;
-          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+          if (k >= 0 && k <= 2 * R) acc[o] = StencilOps<T>::mad(W.w[k], v[e], acc[o]);
         }
 #pragma unroll
         for (int o = 0; o < O; o += 2) {  // (x[p], x[p+1]) -> (o, o+1): one FFMA2
@@ -161,7 +163,7 @@ __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& 
 #pragma unroll
         for (int o = 0; o < O; o += 2) {  // x[p+1] -> even outputs (scalar)
           const int k = 4 * g + e + 1 - HP - o + R;
-          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e + 1], acc[o]);
+          if (k >= 0 && k <= 2 * R) acc[o] = StencilOps<T>::mad(W.w[k], v[e + 1], acc[o]);
         }
       }
     } else {
@@ -170,7 +172,7 @@ __device__ __forceinline__ void compute_tile1(const float* sm, const Weights1D& 
 #pragma unroll
         for (int o = 0; o < O; ++o) {
           const int k = 4 * g + e - HP - o + R;
-          if (k >= 0 && k <= 2 * R) acc[o] = fmaf(W.w[k], v[e], acc[o]);
+          if (k >= 0 && k <= 2 * R) acc[o] = StencilOps<T>::mad(W.w[k], v[e], acc[o]);
         }
       }
     }
@@ -307,7 +309,7 @@ __device__ __forceinline__ void tma_load_rows(void* smem_dst, const CUtensorMap*
       : "memory");
 }
 
-template <int R, bool PK, int STAGES>
+template <int R, bool PK, int STAGES, typename T = float>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
                      const float* in, float* out, long long rows, long long cols, unsigned tiles_per_row, int ntiles,
@@ -355,7 +357,7 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
   }
   // Outside the vector the copy delivers zeros (what CONSTANT with pad 0 wants); outside a row of a matrix it delivers
   // the neighbouring rows. pb: the first column the 128-byte-row view does not hold as part of this row.
-  const bool zeros_ok = rows == 1 && edge == EDGE_CONSTANT && pad == 0.f;
+  const bool zeros_ok = rows == 1 && edge == EDGE_CONSTANT && bits_are_zero(pad);
   const long long pb = cols & ~31ll;
   const bool back_always = !zeros_ok || pb != cols;
   int s = 0, ph = 0;
@@ -399,7 +401,7 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next TMA refill
       __syncwarp();
     }
-    compute_tile1<R, 16, PK, SWZ>(sm, W, out + row * cols, cols, c0);
+    compute_tile1<R, 16, PK, SWZ, T>(sm, W, out + row * cols, cols, c0);
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
     s = s + 1 == STAGES ? 0 : s + 1;
@@ -412,7 +414,7 @@ overlap1d_tma_kernel(const __grid_constant__ Weights1D W, const __grid_constant_
 // full 32-byte sector each, all issued before the first use, like the Map kernel) and gets the r
 // halo values on each side from the neighbouring lanes by shuffles; only lanes 0 and 31 read
 // their outer halo from memory (those lines are being fetched by the neighbouring warp anyway).
-template <int R>
+template <int R, typename T = float>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
                       size_t rows, size_t cols) {
@@ -459,7 +461,7 @@ overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, 
     // Taps k with k - R even address window pairs (win[o+k], win[o+k+1]), o even, that are aligned
     // register pairs of the 256-bit loads: one FFMA2 per output pair (only worth it when the kernel
     // is issue bound, r >= 8). Per output the taps still accumulate in ascending k: bit-identical.
-    constexpr bool PK = R >= 8;
+    constexpr bool PK = R >= 8 && StencilOps<T>::kFloat;
 #pragma unroll
     for (int k = 0; k <= 2 * R; ++k) {
       if (PK && (k + R) % 2 == 0) {
@@ -467,7 +469,7 @@ overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, 
         for (int o = 0; o < O; o += 2) fma2_into(acc[o], acc[o + 1], W.w[k], win[o + k], win[o + k + 1]);
       } else {
 #pragma unroll
-        for (int o = 0; o < O; ++o) acc[o] = fmaf(W.w[k], win[o + k], acc[o]);
+        for (int o = 0; o < O; ++o) acc[o] = StencilOps<T>::mad(W.w[k], win[o + k], acc[o]);
       }
     }
     if (c0 + O <= lc) {
@@ -485,13 +487,13 @@ overlap1d_shfl_kernel(const __grid_constant__ Weights1D W, int edge, float pad, 
   }
 }
 
-template <int R>
+template <int R, typename T = float>
 cudaError_t launch_shfl(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
                         size_t rows, size_t cols) {
   constexpr int TILE = T1_THREADS * 16;
   const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
   const size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
-  overlap1d_shfl_kernel<R><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  overlap1d_shfl_kernel<R, T><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -502,7 +504,7 @@ cudaError_t launch_shfl(const Launch& L, const Weights1D& w, int edge, float pad
 // 32-byte sector of 2048 bytes. Halos by shuffles with wrap-around: the right neighbour of lane 31's chunk A is lane
 // 0's chunk B, the left neighbour of lane 0's chunk B is lane 31's chunk A; only A's left halo at lane 0 and B's right
 // halo at lane 31 come from memory. r <= 8.
-template <int R>
+template <int R, typename T = float>
 __global__ void __launch_bounds__(T1_THREADS)
 overlap1d_shfl2_kernel(const __grid_constant__ Weights1D W, int edge, float pad, const float* in, float* out,
                        size_t rows, size_t cols) {
@@ -556,7 +558,7 @@ overlap1d_shfl2_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
     float accA[C], accB[C];
 #pragma unroll
     for (int o = 0; o < C; ++o) accA[o] = accB[o] = 0.f;
-    constexpr bool PK = R >= 8;  // as in overlap1d_shfl_kernel: per output the taps accumulate in ascending k
+    constexpr bool PK = R >= 8 && StencilOps<T>::kFloat;  // as in overlap1d_shfl_kernel: per output the taps accumulate in ascending k
 #pragma unroll
     for (int k = 0; k <= 2 * R; ++k) {
       if (PK && (k + R) % 2 == 0) {
@@ -568,8 +570,8 @@ overlap1d_shfl2_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
       } else {
 #pragma unroll
         for (int o = 0; o < C; ++o) {
-          accA[o] = fmaf(W.w[k], wa[o + k], accA[o]);
-          accB[o] = fmaf(W.w[k], wb[o + k], accB[o]);
+          accA[o] = StencilOps<T>::mad(W.w[k], wa[o + k], accA[o]);
+          accB[o] = StencilOps<T>::mad(W.w[k], wb[o + k], accB[o]);
         }
       }
     }
@@ -590,13 +592,13 @@ overlap1d_shfl2_kernel(const __grid_constant__ Weights1D W, int edge, float pad,
   }
 }
 
-template <int R>
+template <int R, typename T = float>
 cudaError_t launch_shfl2(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out,
                          size_t rows, size_t cols) {
   constexpr int TILE = T1_THREADS * 16;
   const size_t ntiles = rows * ((cols + TILE - 1) / TILE);
   const size_t grid = ntiles < 0x7fffffffu ? ntiles : 0x7fffffffu;
-  overlap1d_shfl2_kernel<R><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
+  overlap1d_shfl2_kernel<R, T><<<(unsigned)grid, T1_THREADS, 0, L.stream>>>(w, edge, pad, in, out, rows, cols);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -693,15 +695,17 @@ inline cudaError_t make_tmap_rows(CUtensorMap* out, const float* base, size_t nr
 }
 
 // vectors shorter than one tile (and anything the tensor map cannot describe) take the cp.async form
-template <int R, int STAGES>
+template <int R, int STAGES, typename T = float>
 cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad, const float* in, float* out, size_t rows,
                         size_t cols) {
   const size_t tpr = (cols + T1W_TILE - 1) / T1W_TILE;
   const size_t ntiles = rows * tpr;
-  if ((rows == 1 && cols < size_t(T1W_TILE)) || cols < 32 || rows * cols / 32 >= (size_t(1) << 31) - 1 || ntiles >= (size_t(1) << 30))
-    return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, rows, cols);
+  if ((rows == 1 && cols < size_t(T1W_TILE)) || cols < 32 || rows * cols / 32 >= (size_t(1) << 31) - 1 || ntiles >= (size_t(1) << 30)) {
+    if constexpr (StencilOps<T>::kFloat) return launch_tiled_db<R, 16, true>(L, w, edge, pad, in, out, rows, cols);
+    else return launch_shfl<R, T>(L, w, edge, pad, in, out, rows, cols);
+  }
   constexpr size_t smem = size_t(STAGES) * T1W_STAGE_STRIDE + 3 * STAGES * sizeof(uint64_t) + 1024;  // stages, full/empty, coord
-  auto kern = overlap1d_tma_kernel<R, true, STAGES>;
+  auto kern = overlap1d_tma_kernel<R, true, STAGES, T>;
   static int per_sm = 0;
   if (per_sm == 0) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -720,16 +724,55 @@ cudaError_t launch_tma1(const Launch& L, const Weights1D& w, int edge, float pad
   return cudaGetLastError();
 }
 
-template <int STAGES>
+template <int STAGES, typename T = float>
 cudaError_t launch_tma1_r(const Launch& L, const Weights1D& w, int r, int edge, float pad, const float* in, float* out,
                           size_t rows, size_t cols) {
   switch (r) {
-    case 1: return launch_tma1<1, STAGES>(L, w, edge, pad, in, out, rows, cols);
-    case 2: return launch_tma1<2, STAGES>(L, w, edge, pad, in, out, rows, cols);
-    case 3: return launch_tma1<3, STAGES>(L, w, edge, pad, in, out, rows, cols);
-    case 4: return launch_tma1<4, STAGES>(L, w, edge, pad, in, out, rows, cols);
-    case 8: return launch_tma1<8, STAGES>(L, w, edge, pad, in, out, rows, cols);
-    case 16: return launch_tma1<16, STAGES>(L, w, edge, pad, in, out, rows, cols);
+    case 1: return launch_tma1<1, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_tma1<2, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_tma1<3, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_tma1<4, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_tma1<8, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_tma1<16, STAGES, T>(L, w, edge, pad, in, out, rows, cols);
+  }
+  return cudaErrorInvalidValue;
+}
+
+// int32 elements (reading 26): the direct, register-window and TMA-fed variants
+cudaError_t launch_overlap1d_rows_i32(const Launch& L, int o, const Weights1D& w, int r, int edge, float pad,
+                                      const float* in, float* out, size_t rows, size_t cols) {
+  using T = int32_t;
+  switch (o) {
+    case 0: {
+      const size_t total = rows * cols;
+      size_t grid = (total + 255) / 256;
+      const size_t cap = size_t(L.sms) * 64;
+      if (grid > cap) grid = cap;
+      overlap1d_direct_kernel<T><<<(unsigned)grid, 256, 0, L.stream>>>(w, r, edge, pad, in, out, rows, cols);
+      ++*L.launches;
+      return cudaGetLastError();
+    }
+    case 302: return launch_tma1_r<2, T>(L, w, r, edge, pad, in, out, rows, cols);
+    case 303: return launch_tma1_r<3, T>(L, w, r, edge, pad, in, out, rows, cols);
+    case -8:
+      switch (r) {
+        case 1: return launch_shfl2<1, T>(L, w, edge, pad, in, out, rows, cols);
+        case 2: return launch_shfl2<2, T>(L, w, edge, pad, in, out, rows, cols);
+        case 3: return launch_shfl2<3, T>(L, w, edge, pad, in, out, rows, cols);
+        case 4: return launch_shfl2<4, T>(L, w, edge, pad, in, out, rows, cols);
+        case 8: return launch_shfl2<8, T>(L, w, edge, pad, in, out, rows, cols);
+      }
+      return cudaErrorInvalidValue;
+    case -16:
+      switch (r) {
+        case 1: return launch_shfl<1, T>(L, w, edge, pad, in, out, rows, cols);
+        case 2: return launch_shfl<2, T>(L, w, edge, pad, in, out, rows, cols);
+        case 3: return launch_shfl<3, T>(L, w, edge, pad, in, out, rows, cols);
+        case 4: return launch_shfl<4, T>(L, w, edge, pad, in, out, rows, cols);
+        case 8: return launch_shfl<8, T>(L, w, edge, pad, in, out, rows, cols);
+        case 16: return launch_shfl<16, T>(L, w, edge, pad, in, out, rows, cols);
+      }
+      return cudaErrorInvalidValue;
   }
   return cudaErrorInvalidValue;
 }
@@ -767,9 +810,10 @@ cudaError_t launch_tiled_r(const Launch& L, const Weights1D& w, int r, int edge,
 int overlap1d_variant_count() { return kNumVariants; }
 const char* overlap1d_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kVariants[v].name : nullptr; }
 
-bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
+bool overlap1d_variant_ok(int v, int dtype, int r, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumVariants) return false;
   if (kVariants[v].o == 0) return true;
+  if (dtype != DT_F32 && kVariants[v].o > 0 && kVariants[v].o < 300) return false;  // i32: direct, regshfl_*, tma_* only
   if (r < 0 || r > 16) return false;  // radii between the instantiated ones run zero-padded (kernels.hpp)
   if (kVariants[v].o == -8 && r > 8) return false;
   if (kVariants[v].o >= 300 && rows != 1 && cols % 32 != 0) return false;  // a matrix row must be whole 128-byte rows
@@ -777,21 +821,22 @@ bool overlap1d_variant_ok(int v, int r, const void* in, const void* out, size_t 
   return al && (rows == 1 || cols % 8 == 0);
 }
 
-cudaError_t launch_overlap1d_rows(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+cudaError_t launch_overlap1d_rows(const Launch& L, int v, int dtype, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
   if (kVariants[v].o != 0 && !templated_radius(r)) {
     const int R = padded_radius_1d(r);
     if (R < 0) return cudaErrorInvalidValue;
-    return launch_overlap1d_rows(L, v, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
+    return launch_overlap1d_rows(L, v, dtype, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
   }
+  if (dtype != DT_F32) return launch_overlap1d_rows_i32(L, kVariants[v].o, w, r, edge, pad, in, out, rows, cols);
   switch (kVariants[v].o) {
     case 0: {
       const size_t total = rows * cols;
       size_t grid = (total + 255) / 256;
       const size_t cap = size_t(L.sms) * 64;
       if (grid > cap) grid = cap;
-      overlap1d_direct_kernel<<<(unsigned)grid, 256, 0, L.stream>>>(w, r, edge, pad, in, out, rows, cols);
+      overlap1d_direct_kernel<float><<<(unsigned)grid, 256, 0, L.stream>>>(w, r, edge, pad, in, out, rows, cols);
       ++*L.launches;
       return cudaGetLastError();
     }

@@ -14,7 +14,7 @@ namespace {
 
 // ---- direct --------------------------------------------------------------------------------
 // Filter rows are summed separately in chains of at most 17 taps, then added.
-template <typename WT>
+template <typename WT, typename T>
 __global__ void __launch_bounds__(256)
 overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, float pad, const float* in, float* out,
                         size_t rows, size_t cols) {
@@ -33,9 +33,9 @@ overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, 
         for (int a = a0; a < a1; ++a) {
           const float v = interior ? __ldg(in + (i + a - ry) * (long long)cols + j)
                                    : ext2(in, rows, cols, i + a - ry, j, edge, pad);
-          p = fmaf(W.w[a], v, p);
+          p = StencilOps<T>::mad(W.w[a], v, p);
         }
-        acc = a0 == 0 ? p : acc + p;
+        acc = a0 == 0 ? p : StencilOps<T>::add(acc, p);
       }
     } else {
       for (int a = 0; a <= 2 * ry; ++a) {
@@ -43,9 +43,9 @@ overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, 
         for (int b = 0; b <= 2 * rx; ++b) {
           const float v = interior ? __ldg(in + (i + a - ry) * (long long)cols + (j + b - rx))
                                    : ext2(in, rows, cols, i + a - ry, j + b - rx, edge, pad);
-          p = fmaf(W.w[a * fw + b], v, p);
+          p = StencilOps<T>::mad(W.w[a * fw + b], v, p);
         }
-        acc = a == 0 ? p : acc + p;
+        acc = a == 0 ? p : StencilOps<T>::add(acc, p);
       }
     }
     out[idx] = acc;
@@ -53,13 +53,16 @@ overlap2d_direct_kernel(const __grid_constant__ WT W, int ry, int rx, int edge, 
 }
 
 template <typename WT>
-cudaError_t launch_direct2(const Launch& L, const WT& w, int ry, int rx, int edge, float pad, const float* in,
+cudaError_t launch_direct2(const Launch& L, int dtype, const WT& w, int ry, int rx, int edge, float pad, const float* in,
                            float* out, size_t rows, size_t cols) {
   const size_t total = rows * cols;
   size_t grid = (total + 255) / 256;
   const size_t cap = size_t(L.sms) * 64;
   if (grid > cap) grid = cap;
-  overlap2d_direct_kernel<WT><<<(unsigned)grid, 256, 0, L.stream>>>(w, ry, rx, edge, pad, in, out, rows, cols);
+  if (dtype == DT_F32)
+    overlap2d_direct_kernel<WT, float><<<(unsigned)grid, 256, 0, L.stream>>>(w, ry, rx, edge, pad, in, out, rows, cols);
+  else
+    overlap2d_direct_kernel<WT, int32_t><<<(unsigned)grid, 256, 0, L.stream>>>(w, ry, rx, edge, pad, in, out, rows, cols);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -81,27 +84,28 @@ inline bool tiled_alignment_ok(const void* in, const void* out, size_t rows, siz
 // ---- column-wise 1D ----------------------------------------------------------------------------
 int overlap1d_col_variant_count() { return kNumColVariants; }
 const char* overlap1d_col_variant_name(int v) { return (v >= 0 && v < kNumColVariants) ? kNames[v] : nullptr; }
-bool overlap1d_col_variant_ok(int v, int r, const void* in, const void* out, size_t rows, size_t cols) {
+bool overlap1d_col_variant_ok(int v, int dtype, int r, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumColVariants) return false;
   if (v == 0) return true;
+  if (dtype != DT_F32 && (v < 5 || v > 7)) return false;  // i32: direct and the TMA-fed variants
   return r >= 0 && r <= 16 && tiled_alignment_ok(in, out, rows, cols);  // other radii run zero-padded (kernels.hpp)
 }
 
-cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, int r, int edge, float pad,
+cudaError_t launch_overlap1d_cols(const Launch& L, int v, int dtype, const Weights1D& w, int r, int edge, float pad,
                                   const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
-  if (v == 0) return launch_direct2<Weights1D>(L, w, r, 0, edge, pad, in, out, rows, cols);
+  if (v == 0) return launch_direct2<Weights1D>(L, dtype, w, r, 0, edge, pad, in, out, rows, cols);
   if (const int R = padded_radius_1d(r); R != r) {
     if (R < 0) return cudaErrorInvalidValue;
-    return launch_overlap1d_cols(L, v, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
+    return launch_overlap1d_cols(L, v, dtype, pad_weights_1d(w, r, R), R, edge, pad, in, out, rows, cols);
   }
   switch (r) {
-    case 1: return launch_overlap1d_cols_tiled<1>(L, v, w, edge, pad, in, out, rows, cols);
-    case 2: return launch_overlap1d_cols_tiled<2>(L, v, w, edge, pad, in, out, rows, cols);
-    case 3: return launch_overlap1d_cols_tiled<3>(L, v, w, edge, pad, in, out, rows, cols);
-    case 4: return launch_overlap1d_cols_tiled<4>(L, v, w, edge, pad, in, out, rows, cols);
-    case 8: return launch_overlap1d_cols_tiled<8>(L, v, w, edge, pad, in, out, rows, cols);
-    case 16: return launch_overlap1d_cols_tiled<16>(L, v, w, edge, pad, in, out, rows, cols);
+    case 1: return launch_overlap1d_cols_tiled<1>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_overlap1d_cols_tiled<2>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_overlap1d_cols_tiled<3>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_overlap1d_cols_tiled<4>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 8: return launch_overlap1d_cols_tiled<8>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 16: return launch_overlap1d_cols_tiled<16>(L, v, dtype, w, edge, pad, in, out, rows, cols);
   }
   return cudaErrorInvalidValue;
 }
@@ -109,27 +113,28 @@ cudaError_t launch_overlap1d_cols(const Launch& L, int v, const Weights1D& w, in
 // ---- 2D ----------------------------------------------------------------------------------------
 int overlap2d_variant_count() { return kNumVariants; }
 const char* overlap2d_variant_name(int v) { return (v >= 0 && v < kNumVariants) ? kNames[v] : nullptr; }
-bool overlap2d_variant_ok(int v, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols) {
+bool overlap2d_variant_ok(int v, int dtype, int ry, int rx, const void* in, const void* out, size_t rows, size_t cols) {
   if (v < 0 || v >= kNumVariants) return false;
   if (v == 0) return true;
+  if (dtype != DT_F32 && (v < 5 || v > 7)) return false;  // i32: direct and the TMA-fed variants
   // rectangular filters and ry = rx = 0 run the square filter of radius max(ry, rx, 1) zero-padded (kernels.hpp)
   return ry >= 0 && rx >= 0 && ry <= 4 && rx <= 4 && tiled_alignment_ok(in, out, rows, cols);
 }
 
-cudaError_t launch_overlap2d(const Launch& L, int v, const Weights2D& w, int ry, int rx, int edge, float pad,
+cudaError_t launch_overlap2d(const Launch& L, int v, int dtype, const Weights2D& w, int ry, int rx, int edge, float pad,
                              const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
-  if (v == 0) return launch_direct2<Weights2D>(L, w, ry, rx, edge, pad, in, out, rows, cols);
+  if (v == 0) return launch_direct2<Weights2D>(L, dtype, w, ry, rx, edge, pad, in, out, rows, cols);
   if (ry != rx || ry < 1) {
     const int R = ry > rx ? ry : (rx > 1 ? rx : 1);
     if (R > 4) return cudaErrorInvalidValue;
-    return launch_overlap2d(L, v, pad_weights_2d(w, ry, rx, R), R, R, edge, pad, in, out, rows, cols);
+    return launch_overlap2d(L, v, dtype, pad_weights_2d(w, ry, rx, R), R, R, edge, pad, in, out, rows, cols);
   }
   switch (ry) {
-    case 1: return launch_overlap2d_tiled<1>(L, v, w, edge, pad, in, out, rows, cols);
-    case 2: return launch_overlap2d_tiled<2>(L, v, w, edge, pad, in, out, rows, cols);
-    case 3: return launch_overlap2d_tiled<3>(L, v, w, edge, pad, in, out, rows, cols);
-    case 4: return launch_overlap2d_tiled<4>(L, v, w, edge, pad, in, out, rows, cols);
+    case 1: return launch_overlap2d_tiled<1>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 2: return launch_overlap2d_tiled<2>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 3: return launch_overlap2d_tiled<3>(L, v, dtype, w, edge, pad, in, out, rows, cols);
+    case 4: return launch_overlap2d_tiled<4>(L, v, dtype, w, edge, pad, in, out, rows, cols);
   }
   return cudaErrorInvalidValue;
 }

@@ -11,15 +11,15 @@ namespace skel {
 
 #define SKEL_DEF_2D(R)                                                                                              \
   template <>                                                                                                       \
-  cudaError_t launch_overlap2d_tiled<R>(const Launch& L, int v, const Weights2D& w, int edge, float pad,            \
+  cudaError_t launch_overlap2d_tiled<R>(const Launch& L, int v, int dtype, const Weights2D& w, int edge, float pad, \
                                         const float* in, float* out, size_t rows, size_t cols) {                    \
-    return launch_tiled_any<R, R, Weights2D>(L, v, w, edge, pad, in, out, rows, cols);                              \
+    return launch_tiled_any<R, R, Weights2D>(L, v, dtype, w, edge, pad, in, out, rows, cols);                       \
   }
 #define SKEL_DEF_COL(R)                                                                                             \
   template <>                                                                                                       \
-  cudaError_t launch_overlap1d_cols_tiled<R>(const Launch& L, int v, const Weights1D& w, int edge, float pad,       \
-                                             const float* in, float* out, size_t rows, size_t cols) {               \
-    return launch_tiled_any<R, 0, Weights1D>(L, v, w, edge, pad, in, out, rows, cols);                              \
+  cudaError_t launch_overlap1d_cols_tiled<R>(const Launch& L, int v, int dtype, const Weights1D& w, int edge,       \
+                                             float pad, const float* in, float* out, size_t rows, size_t cols) {    \
+    return launch_tiled_any<R, 0, Weights1D>(L, v, dtype, w, edge, pad, in, out, rows, cols);                       \
   }
 
 #if SKEL_INST == 0

@@ -235,9 +235,10 @@ __device__ __forceinline__ void compute_tile2_bx(const float* sm, const WPairs2D
 // a thread's 4 (x) by OY (y) outputs from the staged tile, written to `out`.
 // full_tile = the caller knows that the whole tile lies inside the matrix: the row and column checks
 // vanish and the output address is advanced by `cols` per row.
-template <int RY, int RX, int OY, typename WT, bool PK>
+template <int RY, int RX, int OY, typename WT, bool PK_, typename T = float>
 __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, float* out, long long rows, long long cols,
                                               long long r0, long long c0, bool full_tile = false) {
+  constexpr bool PK = PK_ && StencilOps<T>::kFloat;
   constexpr int RXP = (RX + 3) / 4 * 4;
   constexpr int SW = T2_TW + 2 * RXP;
   constexpr int NGX = (4 + 2 * RXP) / 4;
@@ -280,12 +281,12 @@ __device__ __forceinline__ void compute_tile2(const float* sm, const WT& W, floa
             fma2_into(dstp[2], dstp[3], W.w[a * FW + b], v[RXP - RX + b + 2], v[RXP - RX + b + 3]);
           } else {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) dstp[e] = fmaf(W.w[a * FW + b], v[RXP - RX + b + e], dstp[e]);
+            for (int e = 0; e < 4; ++e) dstp[e] = StencilOps<T>::mad(W.w[a * FW + b], v[RXP - RX + b + e], dstp[e]);
           }
         }
         if (GROUPED && (a % GR == GR - 1 || a == 2 * RY)) {  // the group is complete
 #pragma unroll
-          for (int e = 0; e < 4; ++e) acc[o][e] = a < GR ? dstp[e] : acc[o][e] + dstp[e];
+          for (int e = 0; e < 4; ++e) acc[o][e] = a < GR ? dstp[e] : StencilOps<T>::add(acc[o][e], dstp[e]);
         }
       }
     }
@@ -427,7 +428,8 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
 
 
 // XS > 1 / BX: the broadcast form (compute_tile2_bx; WT = WPairs2D<RY, RX>), XS TMA boxes per stage.
-template <int RY, int RX, int OY, typename WT, bool PK, int STAGES, int XS = 1, bool BX = false, int MINB = 0>
+template <int RY, int RX, int OY, typename WT, bool PK, int STAGES, int XS = 1, bool BX = false, int MINB = 0,
+          typename T = float>
 __global__ void __launch_bounds__(T2_THREADS, MINB)
 overlap2d_tma_kernel(const __grid_constant__ WT W, const __grid_constant__ CUtensorMap tmap, int edge, float pad,
                      const float* in, float* out, int rows, int cols, int tiles_x, int ntiles, unsigned* tile_ctr,
@@ -476,7 +478,7 @@ overlap2d_tma_kernel(const __grid_constant__ WT W, const __grid_constant__ CUten
     for (int d = 0; d < STAGES - 1; ++d) produce(d);
   }
   // zeros are what CONSTANT with pad = 0 wants; any other policy patches the cells outside the matrix
-  const bool patch_needed = !(edge == EDGE_CONSTANT && pad == 0.f);
+  const bool patch_needed = !(edge == EDGE_CONSTANT && bits_are_zero(pad));
   int s = 0, ph = 0;           // stage and parity of this iteration's `full` wait
   int tgt = STAGES - 1, tph = 1;  // thread 0: stage to refill and parity of its `empty` wait
   for (int it = 0;; ++it) {
@@ -505,7 +507,7 @@ overlap2d_tma_kernel(const __grid_constant__ WT W, const __grid_constant__ CUten
     if constexpr (BX)
       compute_tile2_bx<RY, RX, OY, XS>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + TW <= cols);
     else
-      compute_tile2<RY, RX, OY, WT, PK>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
+      compute_tile2<RY, RX, OY, WT, PK, T>(sm, W, out, rows, cols, r0, c0, r0 + TH <= rows && c0 + T2_TW <= cols);
     __syncwarp();
     if (lane == 0) mbar_arrive(empty + s);
     s = s + 1 == STAGES ? 0 : s + 1;
@@ -590,13 +592,13 @@ inline cudaError_t make_tmap_2d(CUtensorMap* out, const float* base, size_t rows
   return cudaSuccess;
 }
 
-template <int RY, int RX, int OY, typename WT, bool PK, int STAGES>
+template <int RY, int RX, int OY, typename WT, bool PK, int STAGES, typename T = float>
 cudaError_t launch_tma2(const Launch& L, const WT& w, int edge, float pad, const float* in, float* out, size_t rows,
                         size_t cols) {
   using G = Tile2Geom<RY, RX, OY>;
   constexpr size_t smem = size_t(STAGES) * G::STAGE_STRIDE + 3 * STAGES * sizeof(uint64_t);  // stages, full/empty, coord
   static_assert(smem <= 227 * 1024, "stages do not fit");
-  auto kern = overlap2d_tma_kernel<RY, RX, OY, WT, PK, STAGES>;
+  auto kern = overlap2d_tma_kernel<RY, RX, OY, WT, PK, STAGES, 1, false, 0, T>;
   static int per_sm = 0;
   if (per_sm == 0) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -650,9 +652,17 @@ cudaError_t launch_tma2_bx(const Launch& L, const Weights2D& w, int edge, float 
 
 // every tiled variant of one (RY, RX) pair; v = variant id of overlap2d.cu's table (v >= 1)
 template <int RY, int RX, typename WT>
-cudaError_t launch_tiled_any(const Launch& L, int v, const WT& w, int edge, float pad, const float* in, float* out,
-                             size_t rows, size_t cols) {
+cudaError_t launch_tiled_any(const Launch& L, int v, int dtype, const WT& w, int edge, float pad, const float* in,
+                             float* out, size_t rows, size_t cols) {
   constexpr bool PK = RX > 0;  // FFMA2 pays when a row feeds several taps; the column form has one tap per row
+  if (dtype != DT_F32) {  // int32 elements: the TMA-fed variants (scalar multiply-add modulo 2^32)
+    switch (v) {
+      case 5: return launch_tma2<RY, RX, 4, WT, false, 3, int32_t>(L, w, edge, pad, in, out, rows, cols);
+      case 6: return launch_tma2<RY, RX, 8, WT, false, RX == 0 ? 3 : 2, int32_t>(L, w, edge, pad, in, out, rows, cols);
+      case 7: return launch_tma2<RY, RX, 4, WT, false, 2, int32_t>(L, w, edge, pad, in, out, rows, cols);
+    }
+    return cudaErrorInvalidValue;
+  }
   switch (v) {
     case 1: return launch_tiled2<RY, RX, 4, WT>(L, w, edge, pad, in, out, rows, cols);
     case 2: return launch_tiled2<RY, RX, 8, WT>(L, w, edge, pad, in, out, rows, cols);

@@ -70,7 +70,7 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
     }
   };
   if (threadIdx.x == 0) produce(0);
-  const bool patch_needed = !(edge == EDGE_CONSTANT && pad == 0.f);
+  const bool patch_needed = !(edge == EDGE_CONSTANT && bits_are_zero(pad));
   int s = 0, ph = 0, tph = 1;
   for (int it = 0;; ++it) {
     if (STAGES == 2 && threadIdx.x == 0) {
