@@ -558,6 +558,20 @@ skel_status acquire_all(skel_ctx* c, OperandSet& set) {
     o.step = coherence_step(o.st->state, ACTOR_DEVICE, o.access, c->mode);
     if (!o.step.ok) return fail(c, SKEL_ERR_UNINIT, "skeleton input was never written");
   }
+  // Two DIFFERENT containers of a call must not share device memory when one of them is written (possible only with
+  // skel_*_adopt_device over overlapping buffers): the kernels choose non-coherent loads, halo reads and in-place
+  // forms by container identity, so such a call would race silently. One handle used as input and output is fine.
+  for (int i = 0; i < set.count; ++i)
+    for (int j = i + 1; j < set.count; ++j) {
+      const Storage* a = set.ops[i].st;
+      const Storage* b = set.ops[j].st;
+      if (!a->dev || !b->dev || a->n == 0 || b->n == 0) continue;
+      if (set.ops[i].access == ACC_READ && set.ops[j].access == ACC_READ) continue;
+      const char* a0 = static_cast<const char*>(a->dev);
+      const char* b0 = static_cast<const char*>(b->dev);
+      if (a0 < b0 + b->n * esize(b->dtype) && b0 < a0 + a->n * esize(a->dtype))
+        return fail(c, SKEL_ERR_ALIAS, "two containers of this call overlap in device memory (adopted buffers)");
+    }
   for (int i = 0; i < set.count; ++i) {
     Operand& o = set.ops[i];
     Storage* s = o.st;

@@ -346,3 +346,29 @@ def test_replay_hook_runs_the_recorded_calls_both_ways(ctx):
     ctx.replay_end()
     for c in (vx, vo, vi, vs, res):
         c.destroy()
+
+
+def test_adopted_buffers_that_overlap_are_rejected(ctx):
+    """alias checks go by device address range, not by handle identity."""
+    import torch
+    t = torch.rand(3000, device="cuda")
+    a = ctx.vector_adopt(t[:2000])
+    b = ctx.vector_adopt(t[1000:3000])       # overlaps a
+    b2 = ctx.vector_adopt(t[:2000])          # the same memory as a, another handle
+    cfree = ctx.vector_adopt(t[2000:3000])   # disjoint from the first 1000 elements only
+    a1 = ctx.vector_adopt(t[:1000])
+    w = np.ones(3, np.float32)
+    for out in (b, b2):
+        with pytest.raises(S.SkelError) as ei:
+            ctx.mapoverlap_1d(w, 1, S.EDGE_DUPLICATE, 0.0, a, out)
+        assert ei.value.status == S.ERR_ALIAS
+        with pytest.raises(S.SkelError) as ei:
+            ctx.map(S.FN_MULT, 2.0, a, None, out)
+        assert ei.value.status == S.ERR_ALIAS
+    ctx.map(S.FN_MULT, 2.0, a1, None, cfree)           # disjoint: fine
+    ctx.map(S.FN_MULT, 2.0, a, None, a)                # one handle in place: fine
+    s1 = ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, a, b2)  # both only read: fine (dot of a with itself)
+    assert s1 > 0
+    ctx.sync()
+    for v in (a, b, b2, cfree, a1):
+        v.destroy()
