@@ -856,7 +856,7 @@ int chain_kind(const skel_ctx* c, const Call& k) {
   if (i.skeleton == SKEL_SK_MAP && i.dtype == SKEL_F32 && i.mode == 0 &&
       (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MULT || i.fn == SKEL_FN_MAX))
     return 1;
-  if (i.skeleton == SKEL_SK_OVERLAP1D && i.dtype == SKEL_F32 && k.rows == 1 && i.r0 >= 0 && i.r0 <= 16) return 2;
+  if (i.skeleton == SKEL_SK_OVERLAP1D && i.dtype == SKEL_F32 && k.rows == 1 && i.r0 >= 0 && i.r0 <= 8) return 2;
   if (i.skeleton == SKEL_SK_REDUCE && i.dtype == SKEL_F32 && (i.fn == SKEL_FN_ADD || i.fn == SKEL_FN_MAX)) return 3;
   return 0;
 }

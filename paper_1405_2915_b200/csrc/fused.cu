@@ -171,6 +171,152 @@ fused_chain_kernel(const __grid_constant__ Weights1D W, int edge, float pad, flo
   }
 }
 
+// The same chain in the "regshfl_2x8" layout (overlap1d.cu): a warp owns 512 consecutive elements, lane l the two
+// 8-element chunks A = [8l, 8l+8) and B = [256+8l, 256+8l+8), so every 256-bit load and store of a warp covers 1024
+// contiguous bytes (whole 128-byte lines) instead of every other 32-byte sector of 2048 bytes. Halos by wrap-around
+// shuffles (lane 31's chunk A borders lane 0's chunk B). r <= 8. Same arithmetic per element as fused_chain_kernel.
+template <int R, int MAPF, int OP>
+__global__ void __launch_bounds__(FU_THREADS)
+fused_chain2_kernel(const __grid_constant__ Weights1D W, int edge, float pad, float c, const float* in, float* map_out,
+                    float* ov_out, size_t n, float* partials, unsigned* ticket, float* result) {
+  constexpr int C = 8, TILE = FU_THREADS * 2 * C;
+  constexpr int ROP = OP == OP_NONE ? FN_ADD : OP;
+  static_assert(R >= 1 && R <= C, "halo comes from the direct neighbours only");
+  constexpr unsigned FULLM = 0xffffffffu;
+  __shared__ float smem[32];
+  __shared__ bool is_last;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const long long ln = static_cast<long long>(n);
+  const size_t ntiles = (n + TILE - 1) / TILE;
+  float red[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) red[q] = identity<float, ROP>();
+
+  for (size_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const long long wbase = static_cast<long long>(tile * TILE) + warp * (64 * C);
+    const long long cA = wbase + C * lane, cB = cA + 32 * C;
+    const bool full = wbase + 64 * C <= ln;  // warp-uniform
+    float wa[C + 2 * R], wb[C + 2 * R];
+    if (full) {
+      uint32_t a[8], b[8];
+      ld_stream<8, true>(a, in + cA);
+      ld_stream<8, true>(b, in + cB);
+#pragma unroll
+      for (int j = 0; j < C; ++j) {
+        wa[R + j] = map1<MAPF>(c, __uint_as_float(a[j]));
+        wb[R + j] = map1<MAPF>(c, __uint_as_float(b[j]));
+      }
+      if constexpr (MAPF != FN_IDENT) {
+        uint32_t m0[8], m1[8];
+#pragma unroll
+        for (int j = 0; j < C; ++j) { m0[j] = __float_as_uint(wa[R + j]); m1[j] = __float_as_uint(wb[R + j]); }
+        st_stream<8>(map_out + cA, m0);
+        st_stream<8>(map_out + cB, m1);
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < C; ++j) {
+        wa[R + j] = ext_mapped<MAPF>(in, ln, cA + j, edge, pad, c);
+        wb[R + j] = ext_mapped<MAPF>(in, ln, cB + j, edge, pad, c);
+        if constexpr (MAPF != FN_IDENT) {
+          if (cA + j < ln) map_out[cA + j] = wa[R + j];
+          if (cB + j < ln) map_out[cB + j] = wb[R + j];
+        }
+      }
+    }
+    const int prev = (lane + 31) & 31, next = (lane + 1) & 31;
+#pragma unroll
+    for (int j = 0; j < R; ++j) {
+      const float tA = __shfl_sync(FULLM, wa[C + j], prev);
+      const float hA = __shfl_sync(FULLM, wa[R + j], next);
+      const float tB = __shfl_sync(FULLM, wb[C + j], prev);
+      const float hB = __shfl_sync(FULLM, wb[R + j], next);
+      wa[j] = tA;
+      wa[R + C + j] = lane == 31 ? hB : hA;
+      wb[j] = lane == 0 ? tA : tB;
+      wb[R + C + j] = hB;
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) wa[j] = ext_mapped<MAPF>(in, ln, cA - R + j, edge, pad, c);
+    }
+    if (lane == 31) {
+#pragma unroll
+      for (int j = 0; j < R; ++j) wb[R + C + j] = ext_mapped<MAPF>(in, ln, cB + C + j, edge, pad, c);
+    }
+    float accA[C], accB[C];
+#pragma unroll
+    for (int o = 0; o < C; ++o) accA[o] = accB[o] = 0.f;
+    constexpr bool PK = R >= 8;
+#pragma unroll
+    for (int k = 0; k <= 2 * R; ++k) {
+      if (PK && (k + R) % 2 == 0) {
+#pragma unroll
+        for (int o = 0; o < C; o += 2) {
+          fma2_into(accA[o], accA[o + 1], W.w[k], wa[o + k], wa[o + k + 1]);
+          fma2_into(accB[o], accB[o + 1], W.w[k], wb[o + k], wb[o + k + 1]);
+        }
+      } else {
+#pragma unroll
+        for (int o = 0; o < C; ++o) {
+          accA[o] = fmaf(W.w[k], wa[o + k], accA[o]);
+          accB[o] = fmaf(W.w[k], wb[o + k], accB[o]);
+        }
+      }
+    }
+    if (full) {
+      uint32_t r0[8], r1[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { r0[e] = __float_as_uint(accA[e]); r1[e] = __float_as_uint(accB[e]); }
+      st_stream<8>(ov_out + cA, r0);
+      st_stream<8>(ov_out + cB, r1);
+      if constexpr (OP != OP_NONE) {
+#pragma unroll
+        for (int o = 0; o < C; ++o) {
+          red[o & 3] = apply_fn<ROP>(0.f, red[o & 3], accA[o]);
+          red[o & 3] = apply_fn<ROP>(0.f, red[o & 3], accB[o]);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int o = 0; o < C; ++o) {
+        if (cA + o < ln) {
+          ov_out[cA + o] = accA[o];
+          if constexpr (OP != OP_NONE) red[o & 3] = apply_fn<ROP>(0.f, red[o & 3], accA[o]);
+        }
+        if (cB + o < ln) {
+          ov_out[cB + o] = accB[o];
+          if constexpr (OP != OP_NONE) red[o & 3] = apply_fn<ROP>(0.f, red[o & 3], accB[o]);
+        }
+      }
+    }
+  }
+
+  if constexpr (OP != OP_NONE) {
+    float v = apply_fn<ROP>(0.f, apply_fn<ROP>(0.f, red[0], red[1]), apply_fn<ROP>(0.f, red[2], red[3]));
+    v = block_reduce<float, ROP>(v, smem);
+    if (gridDim.x == 1) {
+      if (threadIdx.x == 0) *result = v;
+      return;
+    }
+    if (threadIdx.x == 0) {
+      partials[blockIdx.x] = v;
+      __threadfence();
+      const unsigned t = atomicInc(ticket, gridDim.x - 1);
+      is_last = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (is_last) {
+      __threadfence();
+      float a = identity<float, ROP>();
+      for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) a = apply_fn<ROP>(0.f, a, partials[i]);
+      __syncthreads();
+      a = block_reduce<float, ROP>(a, smem);
+      if (threadIdx.x == 0) *result = a;
+    }
+  }
+}
+
 template <int R, int MAPF, int OP>
 cudaError_t launch_rmo(const Launch& L, const Scratch& S, const Weights1D& w, int edge, float pad, float c,
                        const float* in, float* map_out, float* ov_out, size_t n, float* result) {
@@ -178,8 +324,12 @@ cudaError_t launch_rmo(const Launch& L, const Scratch& S, const Weights1D& w, in
   size_t grid = (n + TILE - 1) / TILE;
   if (OP != OP_NONE && grid > MAX_PARTIALS) grid = MAX_PARTIALS;
   if (grid > 0x7fffffffu) grid = 0x7fffffffu;
-  fused_chain_kernel<R, MAPF, OP><<<(unsigned)grid, FU_THREADS, 0, L.stream>>>(
-      w, edge, pad, c, in, map_out, ov_out, n, static_cast<float*>(S.partials), S.ticket, result);
+  if constexpr (R <= 8)  // warp-contiguous layout (fewer halo shuffles than loads saved only up to r = 8)
+    fused_chain2_kernel<R, MAPF, OP><<<(unsigned)grid, FU_THREADS, 0, L.stream>>>(
+        w, edge, pad, c, in, map_out, ov_out, n, static_cast<float*>(S.partials), S.ticket, result);
+  else
+    fused_chain_kernel<R, MAPF, OP><<<(unsigned)grid, FU_THREADS, 0, L.stream>>>(
+        w, edge, pad, c, in, map_out, ov_out, n, static_cast<float*>(S.partials), S.ticket, result);
   ++*L.launches;
   return cudaGetLastError();
 }
@@ -212,7 +362,9 @@ inline bool al32(const void* p) { return reinterpret_cast<uintptr_t>(p) % 32 == 
 }  // namespace
 
 bool fused_chain_ok(int map_fn, int r, int red_op, const void* in, const void* map_out, const void* ov_out, size_t n) {
-  const bool rt = r >= 0 && r <= 16;  // radii between the instantiated ones run zero-padded (kernels.hpp)
+  // radii between the instantiated ones run zero-padded (kernels.hpp); beyond r = 8 the register-window form loses
+  // to the separate TMA-fed MapOverlap kernel (225 against 210 us per iteration at r = 16, n = 2^26): not fused
+  const bool rt = r >= 0 && r <= 8;
   const bool mf = map_fn == FN_IDENT || map_fn == FN_ADD || map_fn == FN_MULT || map_fn == FN_MAX;
   const bool ro = red_op == FUSED_NO_REDUCE || red_op == FN_ADD || red_op == FN_MAX;
   if (!rt || !mf || !ro || n == 0) return false;

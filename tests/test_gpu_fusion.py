@@ -58,7 +58,7 @@ def check_chain(got_a, got_b, got_s, ref, redop):
 
 
 @pytest.mark.parametrize("n", [1, 5, 33, 4097, 100003, (1 << 20) + 1])
-@pytest.mark.parametrize("r", [1, 4, 16])
+@pytest.mark.parametrize("r", [1, 4, 5, 8, 16])
 def test_fused_inplace_chain_matches_oracle(ctx, n, r):
     x = I.uniform01_f32(I.config_seed(5, 1) + n + r, n)
     w = I.positive_weights_f32(I.config_seed(3, 20 + r), 2 * r + 1)
@@ -69,8 +69,11 @@ def test_fused_inplace_chain_matches_oracle(ctx, n, r):
         ctx.mapoverlap_1d(w, r, ge, pad, a, b)
         s = ctx.reduce(gr, b)
         st = ctx.stats()
-        assert st["fused_launches"] == 1 and st["fused_calls"] == 3 and st["launches"] == 1, st
-        assert ctx.last_variant() == (S.SK_OVERLAP1D, -2)
+        if r <= 8:   # r = 5 runs the r = 8 kernel zero-padded
+            assert st["fused_launches"] == 1 and st["fused_calls"] == 3 and st["launches"] == 1, st
+            assert ctx.last_variant() == (S.SK_OVERLAP1D, -2)
+        else:        # beyond r = 8 the chain runs call by call (the separate TMA-fed MapOverlap kernel is faster)
+            assert st["fused_launches"] == 0 and st["launches"] == 3, st
         check_chain(a.numpy(), b.numpy(), s, oracle_chain(x, om, c, w, r, oe, pad, orr), orr)
         a.destroy()
         b.destroy()
