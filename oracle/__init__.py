@@ -77,6 +77,13 @@ def _lib() -> C.CDLL:
         L.oracle_mapoverlap_1d_matrix_f32.argtypes = [_f32p, i, i, dbl, i, _f32p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_1d_matrix_f64.argtypes = [_f32p, i, i, dbl, i, _f64p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_2d_f32.argtypes = [_f32p, i, i, i, dbl, _f32p, sz, sz, sz, sz, _f64p, _f64p]
+        L.oracle_map_f64.argtypes = [i, dbl, _f64p, vp, sz, _f64p]
+        L.oracle_map3_f64.argtypes = [_f64p, _f64p, _f64p, sz, _f64p]
+        L.oracle_mapreduce_f64.argtypes = [i, i, dbl, _f64p, vp, sz, C.POINTER(dbl), C.POINTER(dbl)]
+        L.oracle_mapreduce_f64.restype = i
+        L.oracle_scan_f64.argtypes = [i, i, dbl, _f64p, sz, _f64p, _f64p]
+        L.oracle_mapoverlap_1d_matrix_f64w.argtypes = [_f64p, i, i, dbl, i, _f64p, sz, sz, _f64p, _f64p]
+        L.oracle_mapoverlap_2d_f64w.argtypes = [_f64p, i, i, i, dbl, _f64p, sz, sz, _f64p, _f64p]
         L.oracle_mapoverlap_1d_i32.argtypes = [_i32p, i, i, C.c_int32, _i32p, sz, sz, sz, _i32p]
         L.oracle_mapoverlap_1d_matrix_i32.argtypes = [_i32p, i, i, C.c_int32, i, _i32p, sz, sz, _i32p]
         L.oracle_mapoverlap_2d_i32.argtypes = [_i32p, i, i, i, C.c_int32, _i32p, sz, sz, _i32p]
@@ -268,3 +275,63 @@ def mapoverlap_2d_i32(W, ry: int, rx: int, edge: int, pad: int, X) -> np.ndarray
     out = np.empty((rows, cols), np.int32)
     _lib().oracle_mapoverlap_2d_i32(W, ry, rx, edge, int(pad), X.reshape(-1), rows, cols, out.reshape(-1))
     return out
+
+
+# ---------------------------------------------------------------- fp64 elements (binary128 arithmetic, rounded once)
+def map_f64(fn: int, c: float, in0, in1=None) -> np.ndarray:
+    in0 = _c(in0, np.float64)
+    in1 = None if in1 is None else _c(in1, np.float64)
+    out = np.empty(in0.size, np.float64)
+    _lib().oracle_map_f64(fn, float(c), in0, _opt(in1), in0.size, out)
+    return out
+
+
+def map3_muladd_f64(in0, in1, in2) -> np.ndarray:
+    a, b, c = _c(in0, np.float64), _c(in1, np.float64), _c(in2, np.float64)
+    out = np.empty(a.size, np.float64)
+    _lib().oracle_map3_f64(a, b, c, a.size, out)
+    return out
+
+
+def reduce_f64(op: int, x):
+    """-> (result rounded to fp64, sum |x|)."""
+    return mapreduce_f64(-1, op, 0.0, x, None)
+
+
+def mapreduce_f64(map_f: int, red_op: int, c: float, in0, in1=None):
+    in0 = _c(in0, np.float64)
+    in1 = None if in1 is None else _c(in1, np.float64)
+    r, a = C.c_double(), C.c_double()
+    if _lib().oracle_mapreduce_f64(map_f, red_op, float(c), in0, _opt(in1), in0.size, C.byref(r), C.byref(a)) != 0:
+        raise ValueError("reduce of an empty vector")
+    return r.value, a.value
+
+
+def scan_f64(op: int, mode: int, init: float, x):
+    x = _c(x, np.float64)
+    out, ab = np.empty(x.size, np.float64), np.empty(x.size, np.float64)
+    _lib().oracle_scan_f64(op, mode, float(init), x, x.size, out, ab)
+    return out, ab
+
+
+def mapoverlap_1d_f64(w, r: int, edge: int, pad: float, x):
+    out, ab = mapoverlap_1d_matrix_f64(w, r, edge, pad, AXIS_ROW, _c(x, np.float64).reshape(1, -1))
+    return out.reshape(-1), ab.reshape(-1)
+
+
+def mapoverlap_1d_matrix_f64(w, r: int, edge: int, pad: float, axis: int, X):
+    w, X = _c(w, np.float64), _c(X, np.float64)
+    assert w.size == 2 * r + 1 and X.ndim == 2
+    rows, cols = X.shape
+    out, ab = np.empty((rows, cols), np.float64), np.empty((rows, cols), np.float64)
+    _lib().oracle_mapoverlap_1d_matrix_f64w(w, r, edge, float(pad), axis, X.reshape(-1), rows, cols, out.reshape(-1), ab.reshape(-1))
+    return out, ab
+
+
+def mapoverlap_2d_f64(W, ry: int, rx: int, edge: int, pad: float, X):
+    W, X = _c(W, np.float64).reshape(-1), _c(X, np.float64)
+    assert W.size == (2 * ry + 1) * (2 * rx + 1) and X.ndim == 2
+    rows, cols = X.shape
+    out, ab = np.empty((rows, cols), np.float64), np.empty((rows, cols), np.float64)
+    _lib().oracle_mapoverlap_2d_f64w(W, ry, rx, edge, float(pad), X.reshape(-1), rows, cols, out.reshape(-1), ab.reshape(-1))
+    return out, ab

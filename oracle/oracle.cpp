@@ -24,6 +24,8 @@
 // filter), transpose symmetry, library special cases (numpy cumsum / correlate / math.fsum), and
 // brute-force pure-Python loops on tiny inputs; the int32 MapOverlap functions against exact Python integers,
 // numpy.correlate on int64, one-hot shifts and the fp64 functions above on small values (where both are exact).
+// The fp64-element functions (binary128 arithmetic) against exact rationals (Python Fraction), cancellation cases a
+// plain fp64 loop gets wrong, and the fp32-element functions on fp32-representable data.
 // No function here is "parity unpinned".
 //
 // The `#pragma omp parallel for` lines only take effect in the -fopenmp build (liboracle_omp.so),
@@ -177,11 +179,52 @@ inline uint32_t iext2(const int32_t* X, ptrdiff_t rows, ptrdiff_t cols, ptrdiff_
   return u32(X[clampi(p, 0, rows - 1) * cols + clampi(q, 0, cols - 1)]);
 }
 
+// ---- fp64 elements (SURVEY.md 8(f) f2 "f64 element types for all skeletons"; reading 27) ------------------
+// The oracle of an fp64 path cannot be fp64: it computes in binary128 (__float128, 113-bit significand; plain
+// arithmetic only, no libquadmath call). The product of two fp64 values (106 bits) is EXACT in binary128, sums carry
+// ~1e-34 relative error per step, and the result is rounded to fp64 once at the end. Pinned against exact rational
+// arithmetic (Python Fraction) in tests/test_oracle_pins.py.
+typedef __float128 q128;
+inline q128 q_apply(int fn, q128 c, q128 a, q128 b) {
+  switch (fn) {
+    case FN_ADD: return a + b;
+    case FN_MULT: return a * b;
+    case FN_MAX: return a < b ? b : a;
+    case FN_SAXPY: return c * a + b;
+  }
+  return 0;
+}
+inline q128 q_abs(q128 v) { return v < 0 ? -v : v; }
+
+inline q128 qext1(const double* x, ptrdiff_t n, ptrdiff_t stride, ptrdiff_t j, int edge, double pad) {
+  if (j >= 0 && j < n) return x[j * stride];
+  if (edge == EDGE_CONSTANT) return pad;
+  if (edge == EDGE_CYCLIC) return x[wrapi(j, n) * stride];
+  return x[clampi(j, 0, n - 1) * stride];
+}
+inline void qoverlap1_at(const double* w, int r, int edge, double pad, const double* x, ptrdiff_t n, ptrdiff_t stride,
+                         ptrdiff_t i, double* out, double* absout) {
+  q128 acc = 0, aacc = 0;
+  for (int k = -r; k <= r; ++k) {
+    const q128 t = q128(w[k + r]) * qext1(x, n, stride, i + k, edge, pad);  // exact
+    acc += t;
+    aacc += q_abs(t);
+  }
+  *out = static_cast<double>(acc);
+  if (absout) *absout = static_cast<double>(aacc);
+}
+inline q128 qext2(const double* X, ptrdiff_t rows, ptrdiff_t cols, ptrdiff_t p, ptrdiff_t q, int edge, double pad) {
+  if (p >= 0 && p < rows && q >= 0 && q < cols) return X[p * cols + q];
+  if (edge == EDGE_CONSTANT) return pad;
+  if (edge == EDGE_CYCLIC) return X[wrapi(p, rows) * cols + wrapi(q, cols)];
+  return X[clampi(p, 0, rows - 1) * cols + clampi(q, 0, cols - 1)];
+}
+
 }  // namespace
 
 extern "C" {
 
-int oracle_abi_version(void) { return 2; }
+int oracle_abi_version(void) { return 3; }
 
 // ---- Map (reading (c).1). out[i] = f(in0[i], b_i), b_i = in1[i] or the constant c (rounded to
 // fp32 first, reading (c).1 iii). Result in fp64.
@@ -403,6 +446,81 @@ void oracle_mapoverlap_2d_i32(const int32_t* W, int ry, int rx, int edge, int32_
         for (int b = -rx; b <= rx; ++b)
           acc += u32(W[(a + ry) * fw + (b + rx)]) * iext2(X, rows, cols, i + a, j + b, edge, pad);
       out[i * cols + j] = i32(acc);
+    }
+}
+
+// ---- fp64 elements: every function returns the binary128 result rounded ONCE to fp64 -------------------------------
+void oracle_map_f64(int fn, double c, const double* in0, const double* in1, size_t n, double* out) {
+  const ptrdiff_t N = static_cast<ptrdiff_t>(n);
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < N; ++i) out[i] = static_cast<double>(q_apply(fn, c, in0[i], in1 ? q128(in1[i]) : q128(c)));
+}
+
+void oracle_map3_f64(const double* in0, const double* in1, const double* in2, size_t n, double* out) {
+  const ptrdiff_t N = static_cast<ptrdiff_t>(n);
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < N; ++i) out[i] = static_cast<double>(q128(in0[i]) * q128(in1[i]) + q128(in2[i]));
+}
+
+int oracle_mapreduce_f64(int map_f /* -1: plain Reduce */, int red_op, double c, const double* in0, const double* in1,
+                         size_t n, double* result, double* abs_sum) {
+  if (n == 0) return -1;
+  q128 acc = 0, aacc = 0;
+  for (size_t i = 0; i < n; ++i) {
+    const q128 t = map_f < 0 ? q128(in0[i]) : q_apply(map_f, c, in0[i], in1 ? q128(in1[i]) : q128(c));
+    acc = i == 0 ? t : q_apply(red_op, 0, acc, t);
+    aacc += q_abs(t);
+  }
+  *result = static_cast<double>(acc);
+  if (abs_sum) *abs_sum = static_cast<double>(aacc);
+  return 0;
+}
+
+void oracle_scan_f64(int op, int mode, double init, const double* x, size_t n, double* out, double* abs_prefix) {
+  q128 acc = mode == SCAN_INCLUSIVE ? q128(0) : q128(init), aacc = mode == SCAN_INCLUSIVE ? q128(0) : q_abs(init);
+  for (size_t i = 0; i < n; ++i) {
+    if (mode == SCAN_INCLUSIVE) {
+      acc = i == 0 ? q128(x[0]) : q_apply(op, 0, acc, x[i]);
+      aacc += q_abs(x[i]);
+      out[i] = static_cast<double>(acc);
+      if (abs_prefix) abs_prefix[i] = static_cast<double>(aacc);
+    } else {
+      out[i] = static_cast<double>(acc);
+      if (abs_prefix) abs_prefix[i] = static_cast<double>(aacc);
+      acc = q_apply(op, 0, acc, x[i]);
+      aacc += q_abs(x[i]);
+    }
+  }
+}
+
+void oracle_mapoverlap_1d_matrix_f64w(const double* w, int r, int edge, double pad, int axis, const double* X, size_t rows_,
+                                      size_t cols_, double* out, double* absout) {
+  const ptrdiff_t rows = static_cast<ptrdiff_t>(rows_), cols = static_cast<ptrdiff_t>(cols_);
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < rows; ++i)
+    for (ptrdiff_t j = 0; j < cols; ++j) {
+      double* a = absout ? absout + i * cols + j : nullptr;
+      if (axis == AXIS_ROW) qoverlap1_at(w, r, edge, pad, X + i * cols, cols, 1, j, out + i * cols + j, a);
+      else qoverlap1_at(w, r, edge, pad, X + j, rows, cols, i, out + i * cols + j, a);
+    }
+}
+
+void oracle_mapoverlap_2d_f64w(const double* W, int ry, int rx, int edge, double pad, const double* X, size_t rows_,
+                               size_t cols_, double* out, double* absout) {
+  const ptrdiff_t rows = static_cast<ptrdiff_t>(rows_), cols = static_cast<ptrdiff_t>(cols_);
+  const int fw = 2 * rx + 1;
+#pragma omp parallel for schedule(static)
+  for (ptrdiff_t i = 0; i < rows; ++i)
+    for (ptrdiff_t j = 0; j < cols; ++j) {
+      q128 acc = 0, aacc = 0;
+      for (int a = -ry; a <= ry; ++a)
+        for (int b = -rx; b <= rx; ++b) {
+          const q128 t = q128(W[(a + ry) * fw + (b + rx)]) * qext2(X, rows, cols, i + a, j + b, edge, pad);
+          acc += t;
+          aacc += q_abs(t);
+        }
+      out[i * cols + j] = static_cast<double>(acc);
+      if (absout) absout[i * cols + j] = static_cast<double>(aacc);
     }
 }
 

@@ -66,6 +66,15 @@ def uniform_pm1_f32(seed: int, n: int) -> np.ndarray:
     return (2.0 * _unit24(seed, n) - 1.0).astype(np.float32)
 
 
+def uniform_pm1_f64(seed: int, n: int) -> np.ndarray:
+    """fp64 uniform on [-1,1) with a full 53-bit significand (fp64 element tests; not a BASELINE.json config)."""
+    out = np.empty(n, dtype=np.float64)
+    for lo in range(0, n, _CHUNK):
+        hi = min(n, lo + _CHUNK)
+        out[lo:hi] = (raw_u64(seed, hi - lo, lo) >> np.uint64(11)).astype(np.float64) * 2.0 ** -52 - 1.0
+    return out
+
+
 def uniform_int_i32(seed: int, n: int, hi_inclusive: int) -> np.ndarray:
     """int32 uniform on {0..hi_inclusive} (BJ:L8 'uniform[0,1000]', BJ:L11 'uniform[0,15]')."""
     out = np.empty(n, dtype=np.int32)

@@ -36,7 +36,7 @@ def oracle_separable(wr, rr, wc, rc, oe, pad, X):
     return ref, ab + np.abs(carried) * 1.000001
 
 
-@pytest.mark.parametrize("v", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("v", list(range(S.lib.skel_variant_count(S.SK_SEPARABLE))))
 @pytest.mark.parametrize("radii", [(1, 1), (2, 2), (3, 3), (4, 4), (8, 8), (0, 0), (8, 2), (5, 5), (3, 6), (16, 16), (9, 1)])
 def test_separable_matches_oracle(ctx, v, radii):
     rr, rc = radii
@@ -72,7 +72,7 @@ def test_separable_fused_is_bit_identical_to_the_two_passes_and_plan_default(ctx
     wr, wc = I.positive_weights_f32(711, 17), I.positive_weights_f32(712, 17)
     mx, mt, mo = ctx.matrix_from(X), ctx.matrix(rows, cols), ctx.matrix(rows, cols)
     outs = []
-    for v in (0, 1, 2, 3, 4, -1):
+    for v in list(range(S.lib.skel_variant_count(S.SK_SEPARABLE))) + [-1]:
         ctx.force_variant(S.SK_SEPARABLE, v)
         ctx.reset_stats()
         ctx.mapoverlap_separable(wr, r, wc, r, S.EDGE_DUPLICATE, 0.0, mx, mo)

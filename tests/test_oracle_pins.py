@@ -835,3 +835,146 @@ def test_overlap_matrix_and_2d_i32(edge):
         assert np.array_equal(O.mapoverlap_2d_i32(Ws, 2, 2, edge, 7, Xs).astype(np.float64), f)
     finally:
         O.use_openmp(False)
+
+
+# ------------------------------------------------------------------ fp64 elements (binary128 oracle)
+from fractions import Fraction  # noqa: E402
+
+
+def _rn(fr: Fraction) -> float:
+    """Exact rational -> nearest fp64 (Python's int / int true division is correctly rounded)."""
+    return fr.numerator / fr.denominator
+
+
+def test_f64_map_is_the_exact_result_rounded_once():
+    n = 300
+    x, y = I.uniform_pm1_f64(400, n), I.uniform_pm1_f64(401, n)
+    c = 2.5000000000000004   # not a short binary fraction
+    for fn, f in ((O.FN_ADD, lambda a, b: a + b), (O.FN_MULT, lambda a, b: a * b), (O.FN_SAXPY, lambda a, b: Fraction(c) * a + b)):
+        got = O.map_f64(fn, c, x, y)
+        assert got.tolist() == [_rn(f(Fraction(float(a)), Fraction(float(b)))) for a, b in zip(x, y)], fn
+    assert np.array_equal(O.map_f64(O.FN_MAX, 0.0, x, y), np.maximum(x, y))
+    assert O.map_f64(O.FN_MULT, c, x).tolist() == [_rn(Fraction(float(a)) * Fraction(c)) for a in x]   # constant operand
+    # cancellation: c*x + y with y = -RN(c*x): the exact residual, which a separate multiply and add returns as 0
+    yc = -(c * x)
+    res = O.map_f64(O.FN_SAXPY, c, x, yc)
+    assert res.tolist() == [_rn(Fraction(c) * Fraction(float(a)) + Fraction(float(b))) for a, b in zip(x, yc)]
+    assert np.count_nonzero(res) > n // 2
+    z = I.uniform_pm1_f64(402, n)
+    assert O.map3_muladd_f64(x, y, z).tolist() == [_rn(Fraction(float(a)) * Fraction(float(b)) + Fraction(float(d))) for a, b, d in zip(x, y, z)]
+
+
+def test_f64_reduce_mapreduce_against_exact_rationals_and_cancellation():
+    assert O.reduce_f64(O.FN_ADD, np.array([1e16, 1.0, -1e16]))[0] == 1.0          # a plain fp64 loop returns 0
+    r, a = O.mapreduce_f64(O.FN_MULT, O.FN_ADD, 0.0, np.array([2.0 ** 27 + 1, -2.0 ** 54]), np.array([2.0 ** 27 + 1, 1.0]))
+    assert r == 2.0 ** 28 + 1                                                       # the product needs 55 bits
+    for n in BOUNDARY_N:
+        x, y = I.uniform_pm1_f64(410 + n, n), I.uniform_pm1_f64(411 + n, n)
+        fx, fy = [Fraction(float(t)) for t in x], [Fraction(float(t)) for t in y]
+        r, a = O.reduce_f64(O.FN_ADD, x)
+        assert r == _rn(sum(fx)) and a == _rn(sum(abs(t) for t in fx))
+        assert O.reduce_f64(O.FN_MAX, x)[0] == float(x.max())
+        r, a = O.mapreduce_f64(O.FN_MULT, O.FN_ADD, 0.0, x, y)
+        assert r == _rn(sum(p * q for p, q in zip(fx, fy))) and a == _rn(sum(abs(p * q) for p, q in zip(fx, fy)))
+        r, _ = O.mapreduce_f64(O.FN_SAXPY, O.FN_ADD, 0.75, x, y)
+        assert r == _rn(sum(Fraction(0.75) * p + q for p, q in zip(fx, fy)))
+        r, _ = O.mapreduce_f64(O.FN_MULT, O.FN_ADD, 3.0, x)                        # constant second operand
+        assert r == _rn(3 * sum(fx))
+    n = 1 << 16                                                                    # closed form: sum i = n (n - 1) / 2
+    assert O.reduce_f64(O.FN_ADD, np.arange(n, dtype=np.float64))[0] == n * (n - 1) // 2
+    assert O.mapreduce_f64(O.FN_MULT, O.FN_ADD, 0.0, np.arange(n, dtype=np.float64), np.ones(n))[0] == n * (n - 1) // 2
+    p = 1.0 + 1e-3 * I.uniform_pm1_f64(412, 40)
+    prod = Fraction(1)
+    for t in p:
+        prod *= Fraction(float(t))
+    assert O.reduce_f64(O.FN_MULT, p)[0] == pytest.approx(_rn(prod), rel=1e-30, abs=0)  # ~1e-34 per step
+    with pytest.raises(ValueError):
+        O.reduce_f64(O.FN_ADD, np.zeros(0))
+
+
+def test_f64_scan_against_exact_rationals():
+    for n in (0, 1, 2, 3, 33, 257):
+        x = I.uniform_pm1_f64(420 + n, n)
+        fx = [Fraction(float(t)) for t in x]
+        inc, ab = O.scan_f64(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, x)
+        acc, exp, expa, aa = Fraction(0), [], [], Fraction(0)
+        for t in fx:
+            acc += t
+            aa += abs(t)
+            exp.append(_rn(acc))
+            expa.append(_rn(aa))
+        assert inc.tolist() == exp and ab.tolist() == expa
+        exc, abe = O.scan_f64(O.FN_ADD, O.SCAN_EXCLUSIVE, 0.3, x)
+        init = Fraction(0.3)
+        assert exc.tolist() == [_rn(init + sum(fx[:i])) for i in range(n)]
+        assert abe.tolist() == [_rn(abs(init) + sum(abs(t) for t in fx[:i])) for i in range(n)]
+        if n:
+            assert np.array_equal(O.scan_f64(O.FN_MAX, O.SCAN_INCLUSIVE, 0.0, x)[0], np.maximum.accumulate(x))
+            mxe = O.scan_f64(O.FN_MAX, O.SCAN_EXCLUSIVE, -0.25, x)[0]
+            assert mxe[0] == -0.25 and np.array_equal(mxe[1:], np.maximum(np.maximum.accumulate(x)[:-1], -0.25))
+    big = np.array([1e16, 1.0, 1.0, -1e16, 1.0])
+    assert O.scan_f64(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, big)[0].tolist() == [1e16, 1e16, 1e16 + 2, 2.0, 3.0]
+    two = np.full(60, 2.0)
+    assert O.scan_f64(O.FN_MULT, O.SCAN_INCLUSIVE, 0.0, two)[0].tolist() == [2.0 ** (k + 1) for k in range(60)]
+    assert O.scan_f64(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, np.ones(5000))[0].tolist() == list(range(1, 5001))
+
+
+@pytest.mark.parametrize("edge", ALL_EDGES)
+def test_f64_overlap_against_exact_rationals_shifts_and_the_f32_oracle(edge):
+    pad = 0.37
+    fpad = Fraction(pad)
+
+    def ext(x, j):
+        n = len(x)
+        if 0 <= j < n:
+            return Fraction(float(x[j]))
+        if edge == O.EDGE_CONSTANT:
+            return fpad
+        if edge == O.EDGE_CYCLIC:
+            return Fraction(float(x[j % n]))
+        return Fraction(float(x[min(max(j, 0), n - 1)]))
+
+    for r in (0, 1, 3, 16):
+        w = I.uniform_pm1_f64(430 + r, 2 * r + 1)
+        fw = [Fraction(float(t)) for t in w]
+        for n in (1, 2, 5, 40):
+            x = I.uniform_pm1_f64(431 + n + r, n)
+            got, ab = O.mapoverlap_1d_f64(w, r, edge, pad, x)
+            assert got.tolist() == [_rn(sum(fw[k + r] * ext(x, i + k) for k in range(-r, r + 1))) for i in range(n)], (r, n)
+            assert ab.tolist() == [_rn(sum(abs(fw[k + r] * ext(x, i + k)) for k in range(-r, r + 1))) for i in range(n)]
+    rows, cols = 7, 9
+    X = I.uniform_pm1_f64(440, rows * cols).reshape(rows, cols)
+    w = I.uniform_pm1_f64(441, 5)
+    got_r, _ = O.mapoverlap_1d_matrix_f64(w, 2, edge, pad, O.AXIS_ROW, X)
+    got_c, _ = O.mapoverlap_1d_matrix_f64(w, 2, edge, pad, O.AXIS_COL, X)
+    for i in range(rows):
+        assert np.array_equal(got_r[i], O.mapoverlap_1d_f64(w, 2, edge, pad, X[i])[0])
+    for j in range(cols):
+        assert np.array_equal(got_c[:, j], O.mapoverlap_1d_f64(w, 2, edge, pad, np.ascontiguousarray(X[:, j]))[0])
+    W = I.uniform_pm1_f64(442, 15).reshape(3, 5)
+
+    def ext2(p, q):
+        if 0 <= p < rows and 0 <= q < cols:
+            return Fraction(float(X[p, q]))
+        if edge == O.EDGE_CONSTANT:
+            return fpad
+        if edge == O.EDGE_CYCLIC:
+            return Fraction(float(X[p % rows, q % cols]))
+        return Fraction(float(X[min(max(p, 0), rows - 1), min(max(q, 0), cols - 1)]))
+
+    got, _ = O.mapoverlap_2d_f64(W, 1, 2, edge, pad, X)
+    exp = [[_rn(sum(Fraction(float(W[a + 1, b + 2])) * ext2(i + a, j + b) for a in (-1, 0, 1) for b in range(-2, 3)))
+            for j in range(cols)] for i in range(rows)]
+    assert got.tolist() == exp
+    # one-hot weights: a pure shift (orientation, edge policy), bit-exact; degenerate axes
+    W1 = np.zeros((3, 3))
+    W1[2, 0] = 1.0                                  # out[i][j] = X~[i+1][j-1]
+    sh, _ = O.mapoverlap_2d_f64(W1, 1, 1, edge, pad, X)
+    assert sh.tolist() == [[float(ext2(i + 1, j - 1)) for j in range(cols)] for i in range(rows)]
+    assert np.array_equal(O.mapoverlap_2d_f64(w.reshape(1, 5), 0, 2, edge, pad, X)[0], got_r)
+    assert np.array_equal(O.mapoverlap_2d_f64(w.reshape(5, 1), 2, 0, edge, pad, X)[0], got_c)
+    # fp32-representable data: the fp32-element oracle (fp64 accumulation) and this one agree to ~1e-16 relative
+    Xs, Ws = X.astype(np.float32), W.astype(np.float32)
+    a32, ab32 = O.mapoverlap_2d(Ws, 1, 2, edge, float(np.float32(pad)), Xs)
+    a64, _ = O.mapoverlap_2d_f64(Ws.astype(np.float64), 1, 2, edge, float(np.float32(pad)), Xs.astype(np.float64))
+    assert np.all(np.abs(a32 - a64) <= 4e-16 * ab32)
