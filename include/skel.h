@@ -52,7 +52,11 @@ typedef enum {
   SKEL_ERR_IO = 11            /* plan file could not be read / written / parsed */
 } skel_status;
 
-typedef enum { SKEL_F32 = 0, SKEL_I32 = 1 } skel_dtype;
+/* SKEL_F64: 8-byte elements; every skeleton has ONE kernel for them (no variants to select, nothing
+ * to tune): Map, skel_map3, Reduce, MapReduce (blocking, _to and _async forms; the scalar is a double), Scan, MapOverlap
+ * through skel_mapoverlap_*_f64. Not offered for fp64: skel_reduce_rows, skel_mapoverlap_separable, cross-call fusion
+ * (such chains run call by call). Tolerances: DESIGN.md section 7. */
+typedef enum { SKEL_F32 = 0, SKEL_I32 = 1, SKEL_F64 = 2 } skel_dtype;
 
 /* user functions (BASELINE.json L5: "add, mult, max, saxpy, weighted stencil").
  * Map:      ADD a+b, MULT a*b, MAX max(a,b), SAXPY c*a+b (one fused multiply-add for f32).
@@ -260,6 +264,16 @@ skel_status skel_mapoverlap_1d_i32(skel_ctx* ctx, const int32_t* w, int r, skel_
 skel_status skel_mapoverlap_1d_matrix_i32(skel_ctx* ctx, const int32_t* w, int r, skel_edge edge, int32_t pad,
                                           skel_axis axis, const skel_matrix* in, skel_matrix* out);
 skel_status skel_mapoverlap_2d_i32(skel_ctx* ctx, const int32_t* W, int ry, int rx, skel_edge edge, int32_t pad,
+                                   const skel_matrix* in, skel_matrix* out);
+
+/* MapOverlap on fp64 containers (SKEL_F64): fp64 data, fp64 weights (HOST pointer, copied at call time), fp64 pad.
+ * One fused multiply-add (DFMA) per tap in ascending tap order, chains of at most 33 taps (2D: one chain per filter
+ * row, the row sums added): |error| <= 33 * 2^-53 * sum|w x~| against the exact value. One kernel each (direct form). */
+skel_status skel_mapoverlap_1d_f64(skel_ctx* ctx, const double* w, int r, skel_edge edge, double pad, const skel_vector* in,
+                                   skel_vector* out);
+skel_status skel_mapoverlap_1d_matrix_f64(skel_ctx* ctx, const double* w, int r, skel_edge edge, double pad, skel_axis axis,
+                                          const skel_matrix* in, skel_matrix* out);
+skel_status skel_mapoverlap_2d_f64(skel_ctx* ctx, const double* W, int ry, int rx, skel_edge edge, double pad,
                                    const skel_matrix* in, skel_matrix* out);
 /* Separable MapOverlap (BASELINE.json configs[3] "separable row-then-column 1D
  * passes"): out = colpass(w_col, r_col, T), T = RN_f32(rowpass(w_row, r_row, in)), each pass with the

@@ -28,7 +28,7 @@ OK, ERR_INVALID_ARG, ERR_SIZE_MISMATCH, ERR_DTYPE, ERR_UNSUPPORTED, ERR_EMPTY, E
     ERR_OOM, ERR_CUDA, ERR_BUSY, ERR_IO = range(12)
 STATUS_NAMES = ["OK", "INVALID_ARG", "SIZE_MISMATCH", "DTYPE", "UNSUPPORTED", "EMPTY", "ALIAS", "UNINIT", "OOM",
                 "CUDA", "BUSY", "IO"]
-F32, I32 = 0, 1
+F32, I32, F64 = 0, 1, 2
 FN_ADD, FN_MULT, FN_MAX, FN_SAXPY, FN_WSTENCIL, FN_MULADD = 0, 1, 2, 3, 4, 5
 EDGE_CONSTANT, EDGE_DUPLICATE, EDGE_CYCLIC = 0, 1, 2
 SCAN_INCLUSIVE, SCAN_EXCLUSIVE = 0, 1
@@ -38,7 +38,9 @@ LAZY, EAGER = 0, 1
 SK_MAP, SK_REDUCE, SK_MAPREDUCE, SK_SCAN, SK_OVERLAP1D, SK_OVERLAP1D_COL, SK_OVERLAP2D, SK_SEPARABLE, SK_REDUCE_ROWS, SK_COUNT = range(10)
 ST_UNINIT, ST_HOST, ST_DEVICE, ST_SHARED = 0, 1, 2, 3
 
-_NP = {F32: np.float32, I32: np.int32}
+_NP = {F32: np.float32, I32: np.int32, F64: np.float64}
+_CT = {F32: C.c_float, I32: C.c_int32, F64: C.c_double}
+_FROM_NP = {np.dtype(np.float32): F32, np.dtype(np.int32): I32, np.dtype(np.float64): F64}
 
 
 class SkelInstance(C.Structure):
@@ -106,6 +108,9 @@ _SIGS = {
     "skel_mapoverlap_1d": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
+    "skel_mapoverlap_1d_f64": ([_vp, _vp, _i, _i, _d, _vp, _vp], _i),
+    "skel_mapoverlap_1d_matrix_f64": ([_vp, _vp, _i, _i, _d, _i, _vp, _vp], _i),
+    "skel_mapoverlap_2d_f64": ([_vp, _vp, _i, _i, _i, _d, _vp, _vp], _i),
     "skel_mapoverlap_1d_i32": ([_vp, _vp, _i, _i, C.c_int32, _vp, _vp], _i),
     "skel_mapoverlap_1d_matrix_i32": ([_vp, _vp, _i, _i, C.c_int32, _i, _vp, _vp], _i),
     "skel_mapoverlap_2d_i32": ([_vp, _vp, _i, _i, _i, C.c_int32, _vp, _vp], _i),
@@ -163,7 +168,7 @@ class Future:
         self.ctx, self.h, self.dtype = ctx, h, dtype
 
     def wait(self):
-        res = (C.c_float if self.dtype == F32 else C.c_int32)()
+        res = _CT[self.dtype]()
         self.ctx.check(lib.skel_future_wait(self.h, C.byref(res)))
         return res.value
 
@@ -267,8 +272,7 @@ class Context:
 
     def vector_from(self, arr: np.ndarray) -> "Vector":
         arr = np.ascontiguousarray(arr)
-        dtype = F32 if arr.dtype == np.float32 else I32
-        assert arr.dtype in (np.float32, np.int32)
+        dtype = _FROM_NP[arr.dtype]
         h = C.c_void_p()
         self.check(lib.skel_vector_create_from(self.h, dtype, arr.size, arr.ctypes.data_as(C.c_void_p), C.byref(h)))
         return Vector(self, h, dtype, arr.size)
@@ -277,8 +281,7 @@ class Context:
         """Wrap a contiguous 1-D torch CUDA tensor (float32 / int32); keeps a reference to it."""
         import torch
         assert tensor.is_cuda and tensor.is_contiguous()
-        dtype = F32 if tensor.dtype == torch.float32 else I32
-        assert tensor.dtype in (torch.float32, torch.int32)
+        dtype = {torch.float32: F32, torch.int32: I32, torch.float64: F64}[tensor.dtype]
         h = C.c_void_p()
         self.check(lib.skel_vector_adopt_device(self.h, dtype, tensor.numel(), C.c_void_p(tensor.data_ptr()), C.byref(h)))
         v = Vector(self, h, dtype, tensor.numel())
@@ -292,8 +295,8 @@ class Context:
 
     def matrix_from(self, arr: np.ndarray) -> "Matrix":
         arr = np.ascontiguousarray(arr)
-        assert arr.ndim == 2 and arr.dtype in (np.float32, np.int32)
-        dtype = F32 if arr.dtype == np.float32 else I32
+        assert arr.ndim == 2
+        dtype = _FROM_NP[arr.dtype]
         h = C.c_void_p()
         self.check(lib.skel_matrix_create_from(self.h, dtype, arr.shape[0], arr.shape[1], arr.ctypes.data_as(C.c_void_p), C.byref(h)))
         return Matrix(self, h, dtype, arr.shape[0], arr.shape[1])
@@ -301,7 +304,7 @@ class Context:
     def matrix_adopt(self, tensor) -> "Matrix":
         import torch
         assert tensor.is_cuda and tensor.is_contiguous() and tensor.dim() == 2
-        dtype = F32 if tensor.dtype == torch.float32 else I32
+        dtype = {torch.float32: F32, torch.int32: I32, torch.float64: F64}[tensor.dtype]
         h = C.c_void_p()
         self.check(lib.skel_matrix_adopt_device(self.h, dtype, tensor.shape[0], tensor.shape[1], C.c_void_p(tensor.data_ptr()), C.byref(h)))
         m = Matrix(self, h, dtype, tensor.shape[0], tensor.shape[1])
@@ -316,7 +319,7 @@ class Context:
         self.check(lib.skel_map3(self.h, f, in0.h, in1.h, in2.h, out.h))
 
     def reduce(self, op: int, x: "Vector"):
-        res = (C.c_float if x.dtype == F32 else C.c_int32)()
+        res = _CT[x.dtype]()
         self.check(lib.skel_reduce(self.h, op, x.h, C.byref(res)))
         return res.value
 
@@ -324,7 +327,7 @@ class Context:
         self.check(lib.skel_reduce_to(self.h, op, x.h, out.h, out_index))
 
     def mapreduce(self, map_f: int, red_op: int, c: float, in0: "Vector", in1: "Vector | None"):
-        res = (C.c_float if in0.dtype == F32 else C.c_int32)()
+        res = _CT[in0.dtype]()
         self.check(lib.skel_mapreduce(self.h, map_f, red_op, c, in0.h, in1.h if in1 is not None else None, C.byref(res)))
         return res.value
 
@@ -358,6 +361,21 @@ class Context:
         W = np.ascontiguousarray(W, np.float32)
         assert W.size == (2 * ry + 1) * (2 * rx + 1)
         self.check(lib.skel_mapoverlap_2d(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
+
+    def mapoverlap_1d_f64(self, w, r: int, edge: int, pad: float, x: "Vector", out: "Vector"):
+        w = np.ascontiguousarray(w, np.float64)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d_f64(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, x.h, out.h))
+
+    def mapoverlap_1d_matrix_f64(self, w, r: int, edge: int, pad: float, axis: int, x: "Matrix", out: "Matrix"):
+        w = np.ascontiguousarray(w, np.float64)
+        assert w.size == 2 * r + 1
+        self.check(lib.skel_mapoverlap_1d_matrix_f64(self.h, w.ctypes.data_as(C.c_void_p), r, edge, pad, axis, x.h, out.h))
+
+    def mapoverlap_2d_f64(self, W, ry: int, rx: int, edge: int, pad: float, x: "Matrix", out: "Matrix"):
+        W = np.ascontiguousarray(W, np.float64)
+        assert W.size == (2 * ry + 1) * (2 * rx + 1)
+        self.check(lib.skel_mapoverlap_2d_f64(self.h, W.ctypes.data_as(C.c_void_p), ry, rx, edge, pad, x.h, out.h))
 
     def mapoverlap_1d_i32(self, w, r: int, edge: int, pad: int, x: "Vector", out: "Vector"):
         w = np.ascontiguousarray(w, np.int32)
@@ -449,7 +467,7 @@ class _Container:
         self.ctx.check(self._acquire(self.h, mode, C.byref(p)))
         if self.size == 0:
             return np.empty(self.shape, _NP[self.dtype])
-        buf = (C.c_byte * (self.size * 4)).from_address(p.value)
+        buf = (C.c_byte * (self.size * np.dtype(_NP[self.dtype]).itemsize)).from_address(p.value)
         return np.frombuffer(buf, dtype=_NP[self.dtype]).reshape(self.shape)
 
     def release(self):
@@ -462,7 +480,7 @@ class _Container:
     def _range_view(self, fn, mode: int, a: int, b: int, count: int, shape) -> np.ndarray:
         p = C.c_void_p()
         self.ctx.check(fn(self.h, mode, a, b, C.byref(p)))
-        buf = (C.c_byte * (count * 4)).from_address(p.value)
+        buf = (C.c_byte * (count * np.dtype(_NP[self.dtype]).itemsize)).from_address(p.value)
         return np.frombuffer(buf, dtype=_NP[self.dtype]).reshape(shape)
 
     def read_range(self, offset: int, count: int) -> np.ndarray:

@@ -17,6 +17,7 @@
 #include "coherence.hpp"
 #include "kernels.hpp"
 #include "plan.hpp"
+#include <memory>
 #include <time.h>
 
 using namespace skel;
@@ -149,7 +150,7 @@ bool ctx_ok(const skel_ctx* c) { return c && c->magic == MAGIC_CTX; }
 bool vec_ok(const skel_vector* v) { return v && v->magic == MAGIC_VEC && v->st; }
 bool mat_ok(const skel_matrix* m) { return m && m->magic == MAGIC_MAT && m->st; }
 
-size_t esize(int) { return 4; }
+size_t esize(int dtype) { return dtype == SKEL_F64 ? 8 : 4; }
 
 skel_status ensure_device(skel_ctx* c) {
   if (c->sticky) return SKEL_ERR_CUDA;
@@ -353,7 +354,7 @@ template <typename H>
 skel_status make_handle(skel_ctx* c, uint32_t magic, int dt, size_t rows, size_t cols, H** out) {
   if (!ctx_ok(c) || !out) return fail(ctx_ok(c) ? c : nullptr, SKEL_ERR_INVALID_ARG, "NULL context or out pointer");
   *out = nullptr;
-  if (dt != SKEL_F32 && dt != SKEL_I32) return fail(c, SKEL_ERR_INVALID_ARG, "unknown dtype");
+  if (dt != SKEL_F32 && dt != SKEL_I32 && dt != SKEL_F64) return fail(c, SKEL_ERR_INVALID_ARG, "unknown dtype");
   if (cols != 0 && rows > std::numeric_limits<size_t>::max() / 8 / cols)
     return fail(c, SKEL_ERR_INVALID_ARG, "size overflow");
   Storage* s = new (std::nothrow) Storage;
@@ -639,8 +640,12 @@ struct Call {
   const void* in2 = nullptr;  // three-vector Map
   void* out = nullptr;
   size_t n = 0, rows = 1, cols = 0;
-  uint32_t cbits = 0;  // constant c / scan init, as the element type's bits
+  uint32_t cbits = 0;  // constant c / scan init, as the element type's bits (32-bit element types)
   float pad = 0.f;
+  // fp64 elements (f64.cu): constant / scan init / pad as doubles, weights behind a pointer (the struct stays small)
+  double c64 = 0.0, pad64 = 0.0;
+  std::shared_ptr<const Weights1D64> w1_64;
+  std::shared_ptr<const Weights2D64> w2_64;
   Weights1D w1;
   Weights2D w2;
   Weights1D w1b;  // separable: the column filter (w1 = the row filter, r0 / r1 = their radii)
@@ -827,8 +832,43 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
   return cudaErrorInvalidValue;
 }
 
+cudaError_t launch_call_f64(skel_ctx* c, const Call& k) {
+  Launch L{c->stream, c->sms, &c->launches, c->tile_ctr, &c->tile_next};
+  const skel_instance& i = k.inst;
+  const double* in0 = static_cast<const double*>(k.in0);
+  const double* in1 = static_cast<const double*>(k.in1);
+  double* out = static_cast<double*>(k.out);
+  switch (i.skeleton) {
+    case SKEL_SK_MAP:
+      return launch_map_f64(L, i.fn, i.mode != 0, k.c64, in0, in1, static_cast<const double*>(k.in2), out, k.n);
+    case SKEL_SK_REDUCE:
+      return launch_mapreduce_f64(L, c->scratch, FN_IDENT_, false, i.fn, 0.0, in0, nullptr, k.n, out);
+    case SKEL_SK_MAPREDUCE:
+      return launch_mapreduce_f64(L, c->scratch, i.fn, i.mode != 0, i.fn2, k.c64, in0, in1, k.n, out);
+    case SKEL_SK_SCAN:
+      return launch_scan_f64(L, c->scratch, i.fn, i.mode == SKEL_SCAN_EXCLUSIVE, k.c64, in0, out, k.n);
+    case SKEL_SK_OVERLAP1D:
+      return k.w1_64 ? launch_overlap1d_f64(L, *k.w1_64, i.r0, i.edge, k.pad64, 0, in0, out, k.rows, k.cols) : cudaErrorInvalidValue;
+    case SKEL_SK_OVERLAP1D_COL:
+      return k.w1_64 ? launch_overlap1d_f64(L, *k.w1_64, i.r0, i.edge, k.pad64, 1, in0, out, k.rows, k.cols) : cudaErrorInvalidValue;
+    case SKEL_SK_OVERLAP2D:
+      return k.w2_64 ? launch_overlap2d_f64(L, *k.w2_64, i.r0, i.r1, i.edge, k.pad64, in0, out, k.rows, k.cols) : cudaErrorInvalidValue;
+  }
+  return cudaErrorInvalidValue;
+}
+
 // choose + launch + bookkeeping
+cudaError_t launch_call_f64(skel_ctx* c, const Call& k);
+
 skel_status launch_now(skel_ctx* c, const Call& k) {
+  if (k.inst.dtype == SKEL_F64) {  // one kernel per skeleton (f64.cu): nothing to select
+    if (c->forced[k.inst.skeleton] > 0) return fail(c, SKEL_ERR_UNSUPPORTED, "fp64 elements have one variant (0) per skeleton");
+    cudaError_t e = launch_call_f64(c, k);
+    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch (fp64)");
+    c->last_sk = k.inst.skeleton;
+    c->last_var = 0;
+    return SKEL_OK;
+  }
   int v = -1;
   skel_status st = choose_variant(c, k, &v);
   if (st != SKEL_OK) return st;
@@ -968,6 +1008,10 @@ bool map_fn_ok(int f) { return f == SKEL_FN_ADD || f == SKEL_FN_MULT || f == SKE
 
 // convert the scalar constant to the element type's bits
 skel_status const_bits(skel_ctx* c, int dtype, double v, uint32_t* bits) {
+  if (dtype == SKEL_F64) {  // the constant travels as a double (Call::c64)
+    *bits = 0;
+    return SKEL_OK;
+  }
   if (dtype == SKEL_F32) {
     const float f = static_cast<float>(v);
     memcpy(bits, &f, 4);
@@ -1022,6 +1066,7 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
   if (!plain_reduce) {
     st = const_bits(c, a->dtype, cval, &k.cbits);
     if (st != SKEL_OK) return st;
+    k.c64 = cval;
   }
   OperandSet set;
   set.add(a, ACC_READ);
@@ -1064,8 +1109,9 @@ skel_status mapreduce_impl(skel_ctx* c, bool plain_reduce, int map_f, int red_op
 
 skel_status overlap_check(skel_ctx* c, const Handle* in, const Handle* out, int edge, int dtype = SKEL_F32) {
   if (in->st->dtype != dtype || out->st->dtype != dtype)
-    return fail(c, SKEL_ERR_DTYPE, dtype == SKEL_F32 ? "skel_mapoverlap_*: f32 containers expected (int32: skel_mapoverlap_*_i32)"
-                                                    : "skel_mapoverlap_*_i32: int32 containers expected");
+    return fail(c, SKEL_ERR_DTYPE, dtype == SKEL_F32   ? "skel_mapoverlap_*: f32 containers expected (int32: *_i32, fp64: *_f64)"
+                                   : dtype == SKEL_I32 ? "skel_mapoverlap_*_i32: int32 containers expected"
+                                                       : "skel_mapoverlap_*_f64: fp64 containers expected");
   if (in->rows != out->rows || in->cols != out->cols) return fail(c, SKEL_ERR_SIZE_MISMATCH, "input and output shapes differ");
   if (in->st == out->st) return fail(c, SKEL_ERR_ALIAS, "MapOverlap output must not alias its input");
   if (edge != SKEL_EDGE_CONSTANT && edge != SKEL_EDGE_DUPLICATE && edge != SKEL_EDGE_CYCLIC) return fail(c, SKEL_ERR_INVALID_ARG, "bad edge policy");
@@ -1342,6 +1388,7 @@ skel_status skel_map(skel_ctx* c, skel_fn f, double cval, const skel_vector* in0
   k.inst.fn = f;
   k.inst.dtype = a->dtype;
   k.inst.mode = b ? 1 : 0;
+  k.c64 = cval;
   skel_status st = const_bits(c, a->dtype, cval, &k.cbits);
   if (st != SKEL_OK) return st;
   OperandSet set;
@@ -1487,6 +1534,7 @@ skel_status skel_reduce_rows(skel_ctx* c, skel_fn op, const skel_matrix* in, ske
   if (!mat_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
   if (!red_op_ok(op)) return fail(c, SKEL_ERR_UNSUPPORTED, "reduce operator must be ADD, MULT or MAX");
   if (out->st->dtype != in->st->dtype) return fail(c, SKEL_ERR_DTYPE, "result element type differs");
+  if (in->st->dtype == SKEL_F64) return fail(c, SKEL_ERR_DTYPE, "skel_reduce_rows: f32 and i32 matrices only");
   if (out->st->n != in->rows) return fail(c, SKEL_ERR_SIZE_MISMATCH, "result vector must have one element per row");
   if (out->st == in->st) return fail(c, SKEL_ERR_ALIAS, "result vector aliases the input");
   if (in->rows > 0 && in->cols == 0) return fail(c, SKEL_ERR_EMPTY, "reduce of empty rows");
@@ -1558,6 +1606,36 @@ skel_status overlap2d_impl(skel_ctx* c, int dtype, const void* W, int ry, int rx
   return overlap_run(c, k, in, out);
 }
 
+skel_status overlap_f64_impl(skel_ctx* c, int skeleton, const double* w, int ry, int rx, skel_edge edge, double pad,
+                             const Handle* in, Handle* out, bool is_matrix) {
+  if (!w) return fail(c, SKEL_ERR_INVALID_ARG, "NULL weights");
+  const bool two_d = skeleton == SKEL_SK_OVERLAP2D;
+  if (two_d ? (ry < 0 || rx < 0 || ry > SKEL_MAX_RADIUS_2D || rx > SKEL_MAX_RADIUS_2D) : (ry < 0 || ry > SKEL_MAX_RADIUS_1D))
+    return fail(c, SKEL_ERR_UNSUPPORTED, "radius out of range");
+  skel_status st = overlap_check(c, in, out, edge, SKEL_F64);
+  if (st != SKEL_OK) return st;
+  Call k;
+  k.inst.skeleton = skeleton;
+  k.inst.fn = SKEL_FN_WSTENCIL;
+  k.inst.dtype = SKEL_F64;
+  k.inst.r0 = ry;
+  k.inst.r1 = two_d ? rx : 0;
+  k.inst.edge = edge;
+  k.pad64 = pad;
+  if (two_d) {
+    auto p = std::make_shared<Weights2D64>();
+    memcpy(p->w, w, sizeof(double) * size_t(2 * ry + 1) * size_t(2 * rx + 1));
+    k.w2_64 = p;
+  } else {
+    auto p = std::make_shared<Weights1D64>();
+    memcpy(p->w, w, sizeof(double) * size_t(2 * ry + 1));
+    k.w1_64 = p;
+  }
+  k.rows = is_matrix ? in->rows : 1;
+  k.cols = is_matrix ? in->cols : in->st->n;
+  return overlap_run(c, k, in, out);
+}
+
 uint32_t f32_bits(double v) {
   const float f = static_cast<float>(v);
   uint32_t b;
@@ -1608,6 +1686,28 @@ skel_status skel_mapoverlap_2d_i32(skel_ctx* c, const int32_t* W, int ry, int rx
   return overlap2d_impl(c, SKEL_I32, W, ry, rx, edge, static_cast<uint32_t>(pad), in, out);
 }
 
+skel_status skel_mapoverlap_1d_f64(skel_ctx* c, const double* w, int r, skel_edge edge, double pad, const skel_vector* in,
+                                   skel_vector* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!vec_ok(in) || !vec_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap_f64_impl(c, SKEL_SK_OVERLAP1D, w, r, 0, edge, pad, in, out, false);
+}
+
+skel_status skel_mapoverlap_1d_matrix_f64(skel_ctx* c, const double* w, int r, skel_edge edge, double pad, skel_axis axis,
+                                          const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  if (axis != SKEL_AXIS_ROW && axis != SKEL_AXIS_COL) return fail(c, SKEL_ERR_INVALID_ARG, "bad axis");
+  return overlap_f64_impl(c, axis == SKEL_AXIS_ROW ? SKEL_SK_OVERLAP1D : SKEL_SK_OVERLAP1D_COL, w, r, 0, edge, pad, in, out, true);
+}
+
+skel_status skel_mapoverlap_2d_f64(skel_ctx* c, const double* W, int ry, int rx, skel_edge edge, double pad,
+                                   const skel_matrix* in, skel_matrix* out) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  if (!mat_ok(in) || !mat_ok(out)) return fail(c, SKEL_ERR_INVALID_ARG, "bad handle");
+  return overlap_f64_impl(c, SKEL_SK_OVERLAP2D, W, ry, rx, edge, pad, in, out, true);
+}
+
 skel_status skel_mapoverlap_separable(skel_ctx* c, const float* w_row, int r_row, const float* w_col, int r_col,
                                       skel_edge edge, double pad, const skel_matrix* in, skel_matrix* out) {
   if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
@@ -1646,6 +1746,7 @@ skel_status skel_scan(skel_ctx* c, skel_fn op, skel_scan_mode mode, double init,
   k.inst.fn = op;
   k.inst.dtype = a->dtype;
   k.inst.mode = mode;
+  k.c64 = mode == SKEL_SCAN_EXCLUSIVE ? init : 0.0;
   skel_status st = const_bits(c, a->dtype, mode == SKEL_SCAN_EXCLUSIVE ? init : 0.0, &k.cbits);
   if (st != SKEL_OK) return st;
   OperandSet set;
@@ -1766,6 +1867,7 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
   const int sk = inst->skeleton;
   if (sk < 0 || sk >= SKEL_SK_COUNT) return fail(c, SKEL_ERR_INVALID_ARG, "bad skeleton id");
   if (log2_lo < 0 || log2_hi > 32 || log2_lo > log2_hi || reps < 1) return fail(c, SKEL_ERR_INVALID_ARG, "bad tuning range");
+  if (inst->dtype == SKEL_F64) return fail(c, SKEL_ERR_UNSUPPORTED, "fp64 elements have one kernel per skeleton: nothing to tune");
   const bool matrix = sk == SKEL_SK_OVERLAP1D_COL || sk == SKEL_SK_OVERLAP2D || sk == SKEL_SK_SEPARABLE ||
                       sk == SKEL_SK_REDUCE_ROWS ||
                       (sk == SKEL_SK_OVERLAP1D && cols > 0);
@@ -1978,7 +2080,7 @@ skel_status skel_replay_run(skel_ctx* c, int raw, int reps, double* host_us, dou
     for (RecordedCall& r : c->recorded) {
       if (raw) {
         if (r.k.inst.skeleton == SKEL_SK_SCAN) result = ensure_scan_state(c, r.k.n);
-        if (result == SKEL_OK && launch_call(c, r.k, r.variant) != cudaSuccess)
+        if (result == SKEL_OK && (r.k.inst.dtype == SKEL_F64 ? launch_call_f64(c, r.k) : launch_call(c, r.k, r.variant)) != cudaSuccess)
           result = cuda_fail(c, cudaGetLastError(), "replay launch");
         c->stats.launches += c->launches;
         c->launches = 0;

@@ -6,7 +6,7 @@
 
 namespace skel {
 
-enum : int { DT_F32 = 0, DT_I32 = 1 };
+enum : int { DT_F32 = 0, DT_I32 = 1, DT_F64 = 2 };
 
 struct Launch {
   cudaStream_t stream;
@@ -123,6 +123,22 @@ const char* separable_variant_name(int v);
 bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const void* out, size_t rows, size_t cols);
 cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r_row,
                                    int r_col, int edge, float pad, const float* in, float* out, size_t rows, size_t cols);
+
+// ---- fp64 elements (f64.cu; dtype = DT_F64): one kernel per skeleton, no variant table ---------------------------
+struct Weights1D64 { double w[129]; };
+struct Weights2D64 { double w[17 * 17]; };
+// in2 != NULL: three-vector MULADD (fn ignored); else out = f(in0, in1 or c)
+cudaError_t launch_map_f64(const Launch& L, int fn, bool has_in1, double c, const double* in0, const double* in1,
+                           const double* in2, double* out, size_t n);
+cudaError_t launch_mapreduce_f64(const Launch& L, const Scratch& S, int map_fn, bool has_in1, int red_op, double c,
+                                 const double* in0, const double* in1, size_t n, double* result /* device */);
+cudaError_t launch_scan_f64(const Launch& L, const Scratch& S, int op, bool exclusive, double init, const double* in,
+                            double* out, size_t n);
+// axis 0: along the rows (a vector is rows = 1), 1: along the columns
+cudaError_t launch_overlap1d_f64(const Launch& L, const Weights1D64& w, int r, int edge, double pad, int axis,
+                                 const double* in, double* out, size_t rows, size_t cols);
+cudaError_t launch_overlap2d_f64(const Launch& L, const Weights2D64& w, int ry, int rx, int edge, double pad,
+                                 const double* in, double* out, size_t rows, size_t cols);
 
 // ---- FP32 FMA roofline probe (probe.cu) ------------------------------------------------------------
 cudaError_t launch_fma_probe(const Launch& L, float* scratch /* device, >= 1 float */, double* fma_count);
