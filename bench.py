@@ -275,13 +275,15 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
         flight and the host never drains the stream."""
         a, b = ctx.vector_from(x0), ctx.vector(n)
         ctx.reset_stats()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0, e1, es = (torch.cuda.Event(enable_timing=True) for _ in range(3))
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         e0.record()
         s = 0.0
         futs = []
-        for _ in range(k):
+        for it in range(k):
+            if it == 1:
+                es.record()  # iteration 1 carried the one upload of A (256 MiB over PCIe): steady state starts here
             ctx.map(S.FN_MULT, 1.0001, a, None, a)
             ctx.mapoverlap_1d(w, 4, S.EDGE_DUPLICATE, 0.0, a, b)
             if lag:
@@ -299,20 +301,25 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
         st = ctx.stats()
         a.destroy()
         b.destroy()
+        run.steady_ms = es.elapsed_time(e1) / (k - 1) if k > 1 else float("nan")
         return wall, e0.elapsed_time(e1), st, s
 
     run(3)  # warm-up (allocations, first-use kernel loads)
     wall_l, dev_l, st_l, s_l = run(iters)
+    steady_l = run.steady_ms
     # the same loop with cross-call fusion on (skel_ctx_set_fusion): Map -> MapOverlap1D -> Reduce is ONE
     # kernel, 12 instead of 20 bytes per element (every reduce() ends with a scalar read-back, which also
     # flushes: the events above see every launch)
     wall_la, dev_la, st_la, s_la = run(iters, lag=2)
+    steady_la = run.steady_ms
     ctx.set_fusion(True)
     try:
         run(3)
         wall_f, dev_f, st_f, s_f = run(iters)
+        steady_f = run.steady_ms
         run(3, lag=2)
         wall_fa, dev_fa, st_fa, s_fa = run(iters, lag=2)
+        steady_fa = run.steady_ms
     finally:
         ctx.set_fusion(False)
     ctx.set_coherence(S.EAGER)
@@ -323,22 +330,29 @@ def pipeline_experiment(S, ctx, n, iters=100, eager_iters=10):
     per_iter_bytes = 20 * n  # Map 8 + MapOverlap 8 + Reduce 4 bytes per element
     return {
         "n": n, "iterations": iters,
+        "note": "wall / device per iteration include the ONE upload of A (256 MiB over PCIe, ~5 ms) spread over the "
+                "iterations; steady_device_ms_per_iter is iterations 2..100 only",
         "lazy": {"wall_ms_per_iter": round(wall_l / iters * 1e3, 4), "device_ms_per_iter": round(dev_l / iters, 4),
+                 "steady_device_ms_per_iter": round(steady_l, 4),
                  "GB/s_device": round(per_iter_bytes / (dev_l / iters * 1e-3) / 1e9, 1),
                  "h2d_bytes_total": st_l["h2d_bytes"], "d2h_bytes_total": st_l["d2h_bytes"],
                  "h2d_count": st_l["h2d_count"], "d2h_count": st_l["d2h_count"],
                  "scalar_readbacks": st_l["scalar_d2h_count"], "h2d_elided": st_l["h2d_elided"]},
         "lazy_async": {"wall_ms_per_iter": round(wall_la / iters * 1e3, 4), "device_ms_per_iter": round(dev_la / iters, 4),
+                       "steady_device_ms_per_iter": round(steady_la, 4),
                        "iterations_in_flight": 2, "scalar_readbacks": st_la["scalar_d2h_count"],
                        "same_scalar_as_blocking": bool(s_la == s_l),
                        "note": "skel_reduce_async + skel_future_wait two iterations late: the host waits on the event "
                                "behind each reducing kernel, never on the whole stream"},
         "fused": {"wall_ms_per_iter": round(wall_f / iters * 1e3, 4), "device_ms_per_iter": round(dev_f / iters, 4),
+                  "steady_device_ms_per_iter": round(steady_f, 4),
                   "bytes_per_elem": 12, "GB/s_device_at_12B": round(12 * n / (dev_f / iters * 1e-3) / 1e9, 1),
                   "launches_per_iter": st_f["launches"] / iters, "fused_launches": st_f["fused_launches"],
                   "h2d_count": st_f["h2d_count"], "d2h_count": st_f["d2h_count"],
                   "speedup_over_unfused_device": round(dev_l / dev_f, 3), "last_scalar": s_f},
         "fused_async": {"wall_ms_per_iter": round(wall_fa / iters * 1e3, 4), "device_ms_per_iter": round(dev_fa / iters, 4),
+                        "steady_device_ms_per_iter": round(steady_fa, 4),
+                        "steady_GB/s_at_12B": round(12 * n / (steady_fa * 1e-3) / 1e9, 1),
                         "iterations_in_flight": 2, "launches_per_iter": st_fa["launches"] / iters,
                         "scalar_readbacks": st_fa["scalar_d2h_count"], "same_scalar_as_blocking": bool(s_fa == s_f),
                         "GB/s_wall_at_12B": round(12 * n / (wall_fa / iters) / 1e9, 1)},
@@ -589,6 +603,60 @@ def main():
                        "bytes_per_elem": 4, "GB/s": round(4 * m / us / 1e3, 1), "frac_measured_hbm": round(4 * m / us / 1e3 / peak, 4)}
         rr.destroy()
 
+    # ---- the other element types: int32 MapOverlap and fp64 skeletons at the bench sizes. Not part
+    # of `value` (BASELINE.json's configs are f32 / i32 Reduce / i32 Scan); same timing protocol, each call preceded
+    # by nothing but its own previous launch (working sets > L2).
+    other_dtypes = None
+    if rank == 0 and not args.no_pipeline:
+        import torch
+        import skel_inputs as I
+
+        def timed(call, reps=15):
+            for _ in range(3):
+                call()
+            ts = []
+            for _ in range(reps):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                call()
+                e1.record()
+                e1.synchronize()
+                ts.append(e0.elapsed_time(e1) * 1e3)
+            return float(np.median(ts))
+
+        def row(us, nbytes, sk, f64=False):
+            return {"us": round(us, 2), "GB/s": round(nbytes / us / 1e3, 1), "frac_measured_hbm": round(nbytes / us / 1e3 / peak, 4),
+                    "variant": "f64 (one kernel per skeleton, csrc/f64.cu)" if f64 else S.variant_names(sk)[ctx.last_variant()[1]]}
+
+        other_dtypes = {}
+        n26, side = sz["n26"], sz["side"]
+        vi_o = ctx.vector(n26, S.I32)
+        wi4 = (I.uniform_int_i32(31, 9, 200) - 100).astype(np.int32)
+        us = timed(lambda: ctx.mapoverlap_1d_i32(wi4, 4, S.EDGE_DUPLICATE, 0, wl.vi, vi_o))
+        other_dtypes["overlap1d_r4_dup_i32"] = row(us, 8 * n26, S.SK_OVERLAP1D)
+        vi_o.destroy()
+        Xi = I.uniform_int_i32(32, side * side, 1000).reshape(side, side)
+        mi, mio = ctx.matrix_from(Xi), ctx.matrix(side, side, S.I32)
+        Wi = (I.uniform_int_i32(33, 25, 200) - 100).astype(np.int32)
+        us = timed(lambda: ctx.mapoverlap_2d_i32(Wi, 2, 2, S.EDGE_DUPLICATE, 0, mi, mio))
+        other_dtypes["overlap2d_5x5_dup_i32"] = row(us, 8 * side * side, S.SK_OVERLAP2D)
+        mi.destroy()
+        mio.destroy()
+        n25 = n26 // 2   # the same bytes per operand as the f32 vectors
+        xd, yd = ctx.vector_from(I.uniform_pm1_f64(34, n25)), ctx.vector_from(I.uniform_pm1_f64(35, n25))
+        od, rd = ctx.vector(n25, S.F64), ctx.vector(2, S.F64)
+        us = timed(lambda: ctx.map(S.FN_SAXPY, 2.5, xd, yd, od))
+        other_dtypes["map_saxpy_f64"] = row(us, 24 * n25, S.SK_MAP, True)
+        us = timed(lambda: ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, xd, yd, rd, 0))
+        other_dtypes["mapreduce_dot_f64"] = row(us, 16 * n25, S.SK_MAPREDUCE, True)
+        us = timed(lambda: ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, xd, od))
+        other_dtypes["scan_inclusive_f64"] = dict(row(us, 16 * n25, S.SK_SCAN, True), note="three kernels, 24 B/elem moved for 16 algorithmic")
+        wd = I.uniform_pm1_f64(36, 9)
+        us = timed(lambda: ctx.mapoverlap_1d_f64(wd, 4, S.EDGE_DUPLICATE, 0.0, xd, od))
+        other_dtypes["overlap1d_r4_dup_f64"] = dict(row(us, 16 * n25, S.SK_OVERLAP1D, True), note="direct form")
+        for c in (xd, yd, od, rd):
+            c.destroy()
+
     # ---- range-granular host access (PAPER.md L123 partial copies): the host updates 1 MiB of a
     # 256 MiB vector between two Reduce calls; with a range access only that MiB is uploaded, with the whole-container
     # protocol (READWRITE access to the container) the device copy is invalidated and 256 MiB go up again
@@ -738,7 +806,7 @@ def main():
                 "Gelem/s": round(world * wl.elems_per_step / (ms_per_step * 1e-3) / 1e9, 1),
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3, "range_update": range_update,
+                "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3, "other_element_types": other_dtypes, "range_update": range_update,
                 "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)

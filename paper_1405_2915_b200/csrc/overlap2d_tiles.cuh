@@ -138,7 +138,7 @@ template <int RY, int RX, int OY, int XS>
 __device__ __forceinline__ void compute_tile2_bx(const float* sm, const WPairs2D<RY, RX>& P, float* out, long long rows,
                                                  long long cols, long long r0, long long c0, bool full_tile) {
   constexpr int RXP = (RX + 3) / 4 * 4;
-  constexpr int SW = T2_TW + 2 * RXP, SH = 8 * OY + 2 * RY;
+  constexpr int SW = T2_TW + 2 * RXP;
   constexpr int NGX = (4 + 2 * RXP) / 4;
   constexpr int FW = 2 * RX + 1, OFF = RXP - RX;
   constexpr bool GROUPED = (2 * RY + 1) * FW > 33;
