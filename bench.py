@@ -504,6 +504,8 @@ def main():
     # ---- arithmetic roofline of the MapOverlap rows: FMAs per element over the FP32 FMA rate
     # measured in this run by a register-only FFMA kernel; "bound" = the larger of the two floors
     fma_peak = ctx.probe_fma_peak(5)  # FMA/s
+    # what a shared-memory load costs the FMA pipe: FFMA2 stream + NL LDS.128 per 144 pipe cycles
+    fma_vs_loads = {f"lds128_per_144_cycles={nl}": round(ctx.probe_fma_with_loads(nl, 5) / 1e12, 2) for nl in (0, 1, 2, 4, 8)}
     fma_per_elem = {"overlap1d_r1": 3, "overlap1d_r4": 9, "overlap1d_r16": 33, "overlap2d_5x5": 25, "overlap2d_9x9": 81,
                     "overlap1d_rows_r8": 17, "overlap1d_cols_r8": 17}
     for name, _, _, nbytes, elems in wl.ops:
@@ -807,7 +809,7 @@ def main():
                 "frac_measured_hbm": round(value / world / peak, 4), "frac_8TBs": round(value / world / 8000.0, 4),
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
                 "dot_2p20_us_l2_resident": round(dot20_us, 2), "pipeline": pipeline, "separable_fused": separable, "reduce_rows": reduce_rows, "map3_muladd": map3, "other_element_types": other_dtypes, "range_update": range_update,
-                "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
+                "fma_peak_tfma_s": round(fma_peak / 1e12, 2), "fma_tfma_s_vs_shared_loads": fma_vs_loads, "container_layer": container_layer, "dot_sweep": dot_sweep, "cpu_baseline_omp": cpu_omp,
                 "per_skeleton": per}
         print(json.dumps(line), flush=True)
     wl.destroy()

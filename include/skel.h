@@ -376,6 +376,11 @@ skel_status skel_get_stats(skel_ctx* ctx, skel_stats* out);
  * (median of `reps` launches, CUDA events on the context's stream; synchronises): *fma_per_s = FMAs per
  * second (x 2 = FLOP/s). The roofline of the arithmetic-bound MapOverlap instances. */
 skel_status skel_probe_fma_peak(skel_ctx* ctx, int reps, double* fma_per_s);
+/* The same for a stream of packed FFMA2 (72 per iteration = 144 FMA-pipe cycles per warp) interleaved with
+ * `lds128_per_iter` in {0, 1, 2, 4, 8} 128-bit shared-memory loads per iteration, three resident blocks per SM:
+ * measures what a load returning into the register file costs the FMA pipe (the ceiling of the arithmetic-bound
+ * dense 9x9 MapOverlap). Any other count -> SKEL_ERR_INVALID_ARG. */
+skel_status skel_probe_fma_with_loads(skel_ctx* ctx, int lds128_per_iter, int reps, double* fma_per_s);
 skel_status skel_reset_stats(skel_ctx* ctx);
 
 /* The range list of the range-granular host access as a pure function (no GPU needed): merges [begin, end) into

@@ -68,6 +68,7 @@ _SIGS = {
     "skel_ctx_sync": ([_vp], _i),
     "skel_ctx_set_coherence": ([_vp, _i], _i),
     "skel_probe_fma_peak": ([_vp, _i, C.POINTER(C.c_double)], _i),
+    "skel_probe_fma_with_loads": ([_vp, _i, _i, C.POINTER(C.c_double)], _i),
     "skel_ctx_set_fusion": ([_vp, _i], _i),
     "skel_ctx_flush": ([_vp], _i),
     "skel_last_error": ([_vp], C.c_char_p),
@@ -235,6 +236,12 @@ class Context:
 
     def set_coherence(self, mode: int):
         self.check(lib.skel_ctx_set_coherence(self.h, mode))
+
+    def probe_fma_with_loads(self, lds128_per_iter: int, reps: int = 5) -> float:
+        """FMAs per second of an FFMA2 stream with `lds128_per_iter` LDS.128 per 144 FMA-pipe cycles."""
+        out = C.c_double(0.0)
+        self.check(lib.skel_probe_fma_with_loads(self.h, lds128_per_iter, reps, C.byref(out)))
+        return out.value
 
     def probe_fma_peak(self, reps: int = 5) -> float:
         """FP32 FMAs per second of the device (register-only FFMA kernel)."""

@@ -2114,6 +2114,40 @@ skel_status skel_get_stats(skel_ctx* c, skel_stats* out) {
   return SKEL_OK;
 }
 
+skel_status skel_probe_fma_with_loads(skel_ctx* c, int nl, int reps, double* fma_per_s) {
+  if (!ctx_ok(c) || !fma_per_s || reps < 1) return SKEL_ERR_INVALID_ARG;
+  if (nl != 0 && nl != 1 && nl != 2 && nl != 4 && nl != 8) return fail(c, SKEL_ERR_INVALID_ARG, "lds128_per_iter must be 0, 1, 2, 4 or 8");
+  skel_status st = ensure_device(c);
+  if (st != SKEL_OK) return st;
+  st = flush_pending(c);
+  if (st != SKEL_OK) return st;
+  cudaEvent_t e0, e1;
+  CU(c, cudaEventCreate(&e0));
+  CU(c, cudaEventCreate(&e1));
+  Launch L{c->stream, c->sms, &c->launches, c->tile_ctr, &c->tile_next};
+  std::vector<float> ms(reps);
+  double count = 0;
+  cudaError_t e = cudaSuccess;
+  const float* in64 = static_cast<const float*>(c->scratch.partials);  // any 64 readable floats
+  for (int r = -1; r < reps && e == cudaSuccess; ++r) {  // r = -1 warms up
+    cudaEventRecord(e0, c->stream);
+    e = launch_fma_lds_probe(L, nl, in64, static_cast<float*>(c->d_result), &count);
+    cudaEventRecord(e1, c->stream);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float t = 0.f;
+    if (e == cudaSuccess) cudaEventElapsedTime(&t, e0, e1);
+    if (r >= 0) ms[r] = t;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  c->stats.launches += c->launches;
+  c->launches = 0;
+  if (e != cudaSuccess) return cuda_fail(c, e, "FMA + LDS probe");
+  std::sort(ms.begin(), ms.end());
+  *fma_per_s = count / (double(ms[reps / 2]) * 1e-3);
+  return SKEL_OK;
+}
+
 skel_status skel_probe_fma_peak(skel_ctx* c, int reps, double* fma_per_s) {
   if (!ctx_ok(c) || !fma_per_s || reps < 1) return SKEL_ERR_INVALID_ARG;
   skel_status st = ensure_device(c);

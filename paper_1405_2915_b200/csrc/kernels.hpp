@@ -142,6 +142,8 @@ cudaError_t launch_overlap2d_f64(const Launch& L, const Weights2D64& w, int ry, 
 
 // ---- FP32 FMA roofline probe (probe.cu) ------------------------------------------------------------
 cudaError_t launch_fma_probe(const Launch& L, float* scratch /* device, >= 1 float */, double* fma_count);
+// FFMA2 stream with nl in {0, 1, 2, 4, 8} LDS.128 per 144 FMA-pipe cycles; in64: device, 64 floats
+cudaError_t launch_fma_lds_probe(const Launch& L, int nl, const float* in64, float* scratch, double* fma_count);
 
 // tiled variants (v >= 1) of one radius; specialised in overlap2d_inst.cu, one translation unit per radius
 template <int R>

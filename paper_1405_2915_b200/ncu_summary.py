@@ -67,7 +67,7 @@ def main():
         stalls.sort(reverse=True)
         out_rows.append([op, info["variant"], kern, int(rd), int(wr)])
         md.append(f"| {op} | `{info['variant']}` | `{kern}` | {us:.1f} | {rd / 1e6:.1f} | {wr / 1e6:.1f} | {(rd + wr) / alg:.3f} | "
-                  f"{num(get(r, 'FBSP.TriageCompute.dram__throughput.avg.pct_of_peak_sustained_elapsed') or get(r, 'dram__throughput.avg.pct_of_peak_sustained_elapsed')):.0f} | "
+                  f"{num(get(r, 'gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed')):.0f} | "
                   f"{num(get(r, 'sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active')):.0f} | "
                   f"{num(get(r, 'smsp__issue_active.avg.pct_of_peak_sustained_active')):.0f} | "
                   f"{num(get(r, 'smsp__warps_active.avg.per_cycle_active')):.1f} | {get(r, 'launch__registers_per_thread')} | "
