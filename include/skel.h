@@ -383,6 +383,27 @@ skel_status skel_probe_fma_peak(skel_ctx* ctx, int reps, double* fma_per_s);
 skel_status skel_probe_fma_with_loads(skel_ctx* ctx, int lds128_per_iter, int reps, double* fma_per_s);
 skel_status skel_reset_stats(skel_ctx* ctx);
 
+/* ---- no-allocation entry point ----------------------------------------------------------------
+ * Reduce (PAPER.md L81 skeleton list; reading 2) for callers that may not allocate: code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc. Needs no context. The scratch of the reduction
+ * (one partial per block + the ticket) lives in a file-scope __device__ array of skel_noalloc_scratch_bytes() = 33 024
+ * bytes, which every GPU that loads the library holds until the process exits; the call itself calls no cudaMalloc,
+ * cudaFree or allocating library routine.
+ *   op             SKEL_FN_ADD, SKEL_FN_MULT or SKEL_FN_MAX (anything else -> SKEL_ERR_INVALID_ARG)
+ *   device_in      DEVICE pointer, n floats, owned by the caller, read only (any 4-byte alignment)
+ *   n              1 .. skel_noalloc_max_elements() = 2^26; 0 -> SKEL_ERR_EMPTY; more -> SKEL_ERR_UNSUPPORTED
+ *   device_result  DEVICE pointer to one float, owned by the caller, written by the kernel
+ *   cuda_stream    a cudaStream_t (NULL = the legacy default stream); the call is asynchronous on it
+ * The device of the call is the CURRENT device. Same arithmetic as skel_reduce (f32 accumulators, fixed order,
+ * deterministic for a given n), within the Reduce tolerance of DESIGN.md section 7; not bitwise equal to skel_reduce,
+ * whose order depends on the tuned variant. Every call shares the one array: calls on one stream are ordered and
+ * safe, calls that overlap on the GPU (two streams, two host threads) RACE on it. skel_noalloc_last_error() returns
+ * the calling thread's message of its last failed no-alloc call (static storage). */
+skel_status skel_reduce_f32_noalloc(skel_fn op, const float* device_in, size_t n, float* device_result, void* cuda_stream);
+size_t skel_noalloc_max_elements(void);
+size_t skel_noalloc_scratch_bytes(void);
+const char* skel_noalloc_last_error(void);
+
 /* The range list of the range-granular host access as a pure function (no GPU needed): merges [begin, end) into
  * the sorted list of `*count` disjoint ranges stored as pairs ranges[2k], ranges[2k+1] (capacity in pairs). */
 skel_status skel_ranges_add(uint64_t* ranges, size_t* count, size_t capacity, uint64_t begin, uint64_t end);

@@ -135,6 +135,10 @@ _SIGS = {
     "skel_get_stats": ([_vp, C.POINTER(SkelStats)], _i),
     "skel_reset_stats": ([_vp], _i),
     "skel_coherence_step": ([_i, _i, _i, _i, C.POINTER(_i), C.POINTER(_i)], _i),
+    "skel_reduce_f32_noalloc": ([_i, _vp, _sz, _vp, _vp], _i),
+    "skel_noalloc_max_elements": ([], _sz),
+    "skel_noalloc_scratch_bytes": ([], _sz),
+    "skel_noalloc_last_error": ([], C.c_char_p),
 }
 EXPORTS = sorted(_SIGS)
 for _name, (_args, _res) in _SIGS.items():
@@ -156,6 +160,19 @@ def coherence_step(state: int, actor: int, access: int, mode: int = LAZY):
     ns, tr = C.c_int(), C.c_int()
     st = lib.skel_coherence_step(state, actor, access, mode, C.byref(ns), C.byref(tr))
     return st, ns.value, tr.value
+
+
+def reduce_f32_noalloc(op: int, device_in: int, n: int, device_result: int, stream: int = 0) -> None:
+    """skel_reduce_f32_noalloc: Reduce of n floats at DEVICE address `device_in` into the float at DEVICE address
+    `device_result`, asynchronous on `stream` (a cudaStream_t as an integer), scratch in a static device array:
+    no allocation, no context. n <= noalloc_max_elements()."""
+    st = lib.skel_reduce_f32_noalloc(op, device_in, n, device_result, stream)
+    if st != OK:
+        raise SkelError(st, (lib.skel_noalloc_last_error() or b"").decode())
+
+
+def noalloc_max_elements() -> int:
+    return int(lib.skel_noalloc_max_elements())
 
 
 def variant_names(skeleton: int) -> list[str]:

@@ -14,7 +14,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 # the slowest ones first so that the parallel build ends early
 SOURCES = ([("overlap2d_inst.cu", f"overlap2d_inst{k}", [f"-DSKEL_INST={k}"]) for k in (3, 9, 8, 2, 1, 7, 6, 5, 0, 4)] +
            [(f, os.path.splitext(f)[0], []) for f in
-            ("separable.cu", "fused.cu", "f64.cu", "scan.cu", "overlap1d.cu", "api.cu", "overlap2d.cu", "reduce.cu", "map.cu", "probe.cu", "plan.cpp")])
+            ("separable.cu", "fused.cu", "f64.cu", "scan.cu", "overlap1d.cu", "api.cu", "overlap2d.cu", "reduce.cu", "map.cu", "probe.cu", "noalloc.cu", "plan.cpp")])
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 
