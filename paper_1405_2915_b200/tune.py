@@ -84,8 +84,12 @@ def main():
     cmd = "python -m paper_1405_2915_b200.tune " + " ".join(sys.argv[1:])
     note = (f"# generated by: {cmd.strip()}  (skel_tune_instance, reps={args.reps}; {torch.cuda.get_device_name(0)}, "
             f"{datetime.datetime.now(datetime.timezone.utc).strftime('%Y-%m-%d %H:%M UTC')}); not edited by hand\n")
+    # a partial re-tune (--only with --base) keeps the provenance lines of the plan it started from below its own
+    earlier = ""
+    if args.base and os.path.exists(args.base):
+        earlier = "".join(ln for ln in open(args.base) if ln.startswith("#"))
     with open(args.out, "w") as f:
-        f.write(note + body)
+        f.write(note + earlier + body)
     if args.tables:
         with open(args.tables, "w") as f:
             json.dump(tables, f)
