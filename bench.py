@@ -654,7 +654,7 @@ def main():
         us = timed(lambda: ctx.mapreduce_to(S.FN_MULT, S.FN_ADD, 0.0, xd, yd, rd, 0))
         other_dtypes["mapreduce_dot_f64"] = row(us, 16 * n25, S.SK_MAPREDUCE, True)
         us = timed(lambda: ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, xd, od))
-        other_dtypes["scan_inclusive_f64"] = dict(row(us, 16 * n25, S.SK_SCAN, True), note="three kernels, 24 B/elem moved for 16 algorithmic")
+        other_dtypes["scan_inclusive_f64"] = dict(row(us, 16 * n25, S.SK_SCAN, True), note="single pass over HBM (l2ahead form, f64.cu), the tile is re-read from L2")
         wd = I.uniform_pm1_f64(36, 9)
         us = timed(lambda: ctx.mapoverlap_1d_f64(wd, 4, S.EDGE_DUPLICATE, 0.0, xd, od))
         other_dtypes["overlap1d_r4_dup_f64"] = dict(row(us, 16 * n25, S.SK_OVERLAP1D, True), note="direct form")

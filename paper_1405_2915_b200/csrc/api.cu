@@ -195,6 +195,25 @@ skel_status ensure_scan_state(skel_ctx* c, size_t n) {
   return SKEL_OK;
 }
 
+// fp64 single-pass scan: 16 bytes of state per 4096-element tile (f64.cu). The array is zero-filled once and never
+// cleared: states are tagged with a launch number that never repeats. Growing it waits for the stream (rare).
+skel_status ensure_scan_state64(skel_ctx* c, size_t n) {
+  const size_t need = scan_f64_state_words(n);
+  if (need <= c->scratch.scan_state64_words) return SKEL_OK;
+  if (c->scratch.scan_state64) {
+    CU(c, cudaStreamSynchronize(c->stream));
+    CU(c, cudaFree(c->scratch.scan_state64));
+    c->scratch.scan_state64 = nullptr;
+    c->scratch.scan_state64_words = 0;
+  }
+  size_t cap = 2048;
+  while (cap < need) cap *= 2;
+  CU(c, cudaMalloc(reinterpret_cast<void**>(&c->scratch.scan_state64), cap * 8));
+  CU(c, cudaMemsetAsync(c->scratch.scan_state64, 0, cap * 8, c->stream));
+  c->scratch.scan_state64_words = cap;
+  return SKEL_OK;
+}
+
 skel_status dev_alloc(skel_ctx* c, size_t bytes, void** out) {
   *out = nullptr;
   if (bytes == 0) return SKEL_OK;
@@ -863,6 +882,10 @@ cudaError_t launch_call_f64(skel_ctx* c, const Call& k);
 skel_status launch_now(skel_ctx* c, const Call& k) {
   if (k.inst.dtype == SKEL_F64) {  // one kernel per skeleton (f64.cu): nothing to select
     if (c->forced[k.inst.skeleton] > 0) return fail(c, SKEL_ERR_UNSUPPORTED, "fp64 elements have one variant (0) per skeleton");
+    if (k.inst.skeleton == SKEL_SK_SCAN) {
+      skel_status st64 = ensure_scan_state64(c, k.n);
+      if (st64 != SKEL_OK) return st64;
+    }
     cudaError_t e = launch_call_f64(c, k);
     if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch (fp64)");
     c->last_sk = k.inst.skeleton;
@@ -1176,6 +1199,7 @@ skel_status skel_ctx_destroy(skel_ctx* c) {
     if (c->sep_tmp) dev_free(c, c->sep_tmp);
     cudaFree(c->scratch.partials);
     if (c->scratch.scan_state) cudaFree(c->scratch.scan_state);
+    if (c->scratch.scan_state64) cudaFree(c->scratch.scan_state64);
     cudaFreeHost(c->h_result);
     if (c->h_slots) cudaFreeHost(c->h_slots);
     for (cudaEvent_t e : c->ring.ev)
@@ -2079,7 +2103,8 @@ skel_status skel_replay_run(skel_ctx* c, int raw, int reps, double* host_us, dou
   for (int rep = 0; rep < reps && result == SKEL_OK; ++rep) {
     for (RecordedCall& r : c->recorded) {
       if (raw) {
-        if (r.k.inst.skeleton == SKEL_SK_SCAN) result = ensure_scan_state(c, r.k.n);
+        if (r.k.inst.skeleton == SKEL_SK_SCAN)
+          result = r.k.inst.dtype == SKEL_F64 ? ensure_scan_state64(c, r.k.n) : ensure_scan_state(c, r.k.n);
         if (result == SKEL_OK && (r.k.inst.dtype == SKEL_F64 ? launch_call_f64(c, r.k) : launch_call(c, r.k, r.variant)) != cudaSuccess)
           result = cuda_fail(c, cudaGetLastError(), "replay launch");
         c->stats.launches += c->launches;

@@ -5,8 +5,10 @@
 //   Reduce / MapReduce       one block per contiguous chunk (hardware-balanced), 4 accumulators per thread, fixed
 //                            shuffle + shared-memory trees, last block (ticket) folds the partials in index order:
 //                            bitwise deterministic for a given n, no floating-point atomics.
-//   Scan                     three kernels in a fixed order (chunk totals, exclusive scan of the totals by one block,
-//                            chunk-local scans with their offsets): deterministic, 3 passes over the data.
+//   Scan                     n >= 2^20: ONE pass over HBM ("l2ahead": a reduce pass runs two tiles ahead and publishes
+//                            tile aggregates, the scan pass re-reads the tile from L2; 16 B/elem of HBM traffic);
+//                            smaller n: three kernels in a fixed order (chunk totals, exclusive scan of the totals
+//                            by one block, chunk-local scans with their offsets). Both deterministic run to run.
 //   MapOverlap 1D / 2D       one output per thread, taps in ascending order, one DFMA each; chains of at most 33 taps
 //                            (2D: one chain per filter row, the row sums added): bound 33 * 2^-53 of sum|w x|.
 // All of them are bound by HBM (fp64 arithmetic is far from its limit at these intensities).
@@ -333,6 +335,275 @@ overlap2d_f64_kernel(const __grid_constant__ Weights2D64 W, int ry, int rx, int 
   }
 }
 
+// ---- Scan, single pass over HBM ("l2ahead", the structure of scan.cu's scan_l2_kernel for 8-byte elements) ------------
+// CTA b owns tiles b, b + G, ... (static, cooperative launch). Worker warps: a ring of S bulk async copies (evict_last)
+// feeds a REDUCE pass that runs D tiles ahead and publishes each tile's aggregate; the SCAN pass re-reads the tile (an
+// L2 hit), scans it in registers, adds the carry and streams it out. One PREFIX warp per CTA computes the carry of the
+// CTA's next tile as the carry of its previous tile (+) the G aggregates in between, all loads of the window in flight.
+// A tile's state is 16 bytes, (aggregate bits, launch number), written and read with ONE 128-bit relaxed.gpu access
+// (single-copy atomic): a reader that sees this launch's number sees this launch's aggregate. The launch number never
+// repeats (64 bits), so the array is never cleared. The grouping of every sum depends on (n, G) only: bitwise
+// deterministic run to run on a given GPU, like the three-kernel form (whose rounding it does not share).
+__device__ __forceinline__ void ld_state128(const unsigned long long* p, unsigned long long& value, unsigned long long& tag) {
+  asm volatile("{\n.reg .b128 t;\nld.relaxed.gpu.global.b128 t, [%2];\nmov.b128 {%0, %1}, t;\n}"
+               : "=l"(value), "=l"(tag) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st_state128(unsigned long long* p, unsigned long long value, unsigned long long tag) {
+  asm volatile("{\n.reg .b128 t;\nmov.b128 t, {%1, %2};\nst.relaxed.gpu.global.b128 [%0], t;\n}" ::"l"(p), "l"(value), "l"(tag)
+               : "memory");
+}
+__device__ __forceinline__ unsigned ld_acq_sh(const unsigned* p) {
+  unsigned v;
+  asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_rel_sh(unsigned* p, unsigned v) {
+  asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void ld2_hint(double (&d)[2], const double* p, uint64_t policy) {
+  uint32_t r[4];
+  ld_hint4(r, p, policy);
+  d[0] = __hiloint2double(int(r[1]), int(r[0]));
+  d[1] = __hiloint2double(int(r[3]), int(r[2]));
+}
+__device__ __forceinline__ void st2_hint(double* p, const double (&d)[2], uint64_t policy) {
+  const uint32_t r[4] = {uint32_t(__double2loint(d[0])), uint32_t(__double2hiint(d[0])), uint32_t(__double2loint(d[1])),
+                         uint32_t(__double2hiint(d[1]))};
+  st_hint4(p, r, policy);
+}
+
+constexpr int L2_NW = 8, L2_D = 2, L2_S = 2, L2_KW = 10;   // the operating point of the i32 kernel
+constexpr int L2_WT = L2_NW * 32;
+// tile = 256 threads x 2 doubles x U: U = 4 -> 16 KB tiles, 3 CTAs per SM (U = 8: 32 KB tiles, 2 CTAs per SM)
+template <int U> struct L2Geom {
+  static constexpr size_t TILE = size_t(L2_WT) * 2 * U;
+  static constexpr size_t SMEM = L2_S * TILE * 8 + L2_S * 8 + 16;
+};
+constexpr size_t L2_TILE_MIN = L2Geom<4>::TILE;   // the state array is sized for the smaller tile
+
+template <int OP, int U, int MINB>
+__global__ void __launch_bounds__((L2_NW + 1) * 32, MINB)
+scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exclusive, unsigned long long* state,
+                   unsigned long long launch_no, unsigned ntiles) {
+  constexpr int NW = L2_NW, D = L2_D, S = L2_S, KW = L2_KW, WT = L2_WT, E = U * NW, Q = D + 2;
+  constexpr size_t TILE = L2Geom<U>::TILE;
+  constexpr unsigned FULL = 0xffffffffu;
+  __shared__ double sm[2 * E + 1];
+  __shared__ double red[2][NW];
+  __shared__ double cq[Q];
+  __shared__ unsigned cq_head, cq_tail;  // carries produced / consumed
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned long long G = gridDim.x;
+  const double ident = didentity<OP>();
+  if (threadIdx.x == 0) {
+    cq_head = 0;
+    cq_tail = 0;
+  }
+  __syncthreads();
+
+  if (warp == NW) {  // ---------------- prefix warp ----------------
+    double carry = exclusive ? init : ident;
+    unsigned long long lo = 0;
+    unsigned j = 0;
+    for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++j) {
+      double acc = ident;  // carry(tile) = carry(previous own tile) (+) aggregates of tiles [lo, tile), fixed grouping
+      for (unsigned long long c0 = lo; c0 < tile; c0 += 32ull * KW) {
+        bool pending = true;
+        unsigned long long val[KW], tag[KW];
+        while (pending) {
+          pending = false;
+#pragma unroll
+          for (int k = 0; k < KW; ++k) {
+            const unsigned long long idx = c0 + 32ull * k + lane;
+            if (idx < tile) {
+              ld_state128(state + 2 * idx, val[k], tag[k]);
+            } else {
+              val[k] = static_cast<unsigned long long>(__double_as_longlong(ident));
+              tag[k] = launch_no;
+            }
+          }
+#pragma unroll
+          for (int k = 0; k < KW; ++k) pending |= tag[k] != launch_no;
+          pending = __any_sync(FULL, pending);
+        }
+#pragma unroll
+        for (int k = 0; k < KW; ++k) acc = dapply<OP>(0.0, acc, __longlong_as_double(static_cast<long long>(val[k])));
+      }
+      carry = dapply<OP>(0.0, carry, dwarp_reduce<OP>(acc));
+      lo = tile;
+      while (j - ld_acq_sh(&cq_tail) >= unsigned(Q)) {}  // queue full: wait for the workers
+      if (lane == 0) {
+        cq[j % Q] = carry;
+        st_rel_sh(&cq_head, j + 1);
+      }
+      __syncwarp();
+    }
+    return;
+  }
+
+  // ---------------- worker warps ----------------
+  constexpr unsigned TILE_BYTES = unsigned(TILE) * 8u;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double* ring = reinterpret_cast<double*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + size_t(S) * TILE_BYTES);
+  const uint64_t keep = l2_policy_evict_last(), stream = l2_policy_evict_first();
+  auto bar_workers = [] { asm volatile("bar.sync 1, %0;" ::"n"(WT) : "memory"); };
+  auto red_tile = [&](unsigned j) { return blockIdx.x + (unsigned long long)j * G; };
+  auto issue = [&](unsigned j) {  // thread 0: arm stage j % S with reduce-tile j (whole tiles only)
+    const unsigned long long t = red_tile(j);
+    if (t < ntiles && (t + 1) * TILE <= n) {
+      mbar_arrive_expect_tx(&full[j % S], TILE_BYTES);
+      bulk_load_hint(ring + size_t(j % S) * TILE, in + size_t(t) * TILE, TILE_BYTES, &full[j % S], keep);
+    }
+  };
+  if (threadIdx.x == 0) {
+    for (int st = 0; st < S; ++st) mbar_init(&full[st], 1);
+    mbar_fence_init();
+    for (unsigned j = 0; j < unsigned(S); ++j) issue(j);
+  }
+  bar_workers();
+  unsigned par = 0;
+  auto reduce_tile = [&](unsigned j) {  // fold reduce-tile j, publish its aggregate, refill its stage
+    const unsigned long long tile = red_tile(j);
+    const size_t base = size_t(tile) * TILE;
+    double a = ident;
+    if (base + TILE <= n) {
+      mbar_wait(&full[j % S], (j / S) & 1u);
+      const double* stage = ring + size_t(j % S) * TILE;
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const double2 q = *reinterpret_cast<const double2*>(stage + (u * WT + threadIdx.x) * 2);
+        a = dapply<OP>(0.0, a, dapply<OP>(0.0, q.x, q.y));
+      }
+    } else {  // ragged last tile: guarded loads
+      for (size_t i = base + threadIdx.x; i < n; i += WT) a = dapply<OP>(0.0, a, in[i]);
+    }
+    a = dwarp_reduce<OP>(a);
+    if (lane == 0) red[par][warp] = a;
+    bar_workers();  // every worker has read the stage
+    if (warp == 0) {
+      double v = lane < NW ? red[par][lane] : ident;
+      v = dwarp_reduce<OP>(v);
+      if (lane == 0) {
+        st_state128(state + 2 * tile, static_cast<unsigned long long>(__double_as_longlong(v)), launch_no);
+        issue(j + S);
+      }
+    }
+    par ^= 1u;  // red[par] is rewritten two reduces later, with worker barriers in between
+  };
+
+  for (unsigned j = 0; j < unsigned(D); ++j) {  // prologue: run D tiles ahead
+    if (red_tile(j) >= ntiles) break;
+    reduce_tile(j);
+  }
+  unsigned it = 0;
+  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+    const size_t base = size_t(tile) * TILE;
+    double x[U][2], lane_excl[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {  // second read of the tile: an L2 hit
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * 2;
+      if (i0 + 2 <= n) {
+        ld2_hint(x[u], in + i0, stream);
+      } else {
+        x[u][0] = i0 < n ? in[i0] : ident;
+        x[u][1] = ident;
+      }
+    }
+    if (red_tile(it + D) < ntiles) reduce_tile(it + D);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {  // local scan of the tile (registers)
+      x[u][1] = dapply<OP>(0.0, x[u][0], x[u][1]);
+      double ws = x[u][1];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const double y = __shfl_up_sync(FULL, ws, o);
+        if (lane >= o) ws = dapply<OP>(0.0, y, ws);
+      }
+      const double ex = __shfl_up_sync(FULL, ws, 1);
+      lane_excl[u] = lane == 0 ? ident : ex;
+      if (lane == 31) sm[u * NW + warp] = ws;
+    }
+    bar_workers();
+    if (warp == 0) {  // exclusive scan of the E = 64 (u, warp) totals, two per lane
+      constexpr int EPL = (E + 31) / 32;
+      double v[EPL];
+      double run = ident;
+#pragma unroll
+      for (int k = 0; k < EPL; ++k) {
+        const int e = lane * EPL + k;
+        v[k] = e < E ? sm[e] : ident;
+        run = dapply<OP>(0.0, run, v[k]);
+      }
+      double ws = run;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const double y = __shfl_up_sync(FULL, ws, o);
+        if (lane >= o) ws = dapply<OP>(0.0, y, ws);
+      }
+      double ex = __shfl_up_sync(FULL, ws, 1);
+      ex = lane == 0 ? ident : ex;
+#pragma unroll
+      for (int k = 0; k < EPL; ++k) {
+        const int e = lane * EPL + k;
+        if (e < E) sm[E + e] = ex;
+        ex = dapply<OP>(0.0, ex, v[k]);
+      }
+    }
+    while (ld_acq_sh(&cq_head) <= it) {}  // carry of this tile (normally long there)
+    const double carry = cq[it % Q];
+    bar_workers();
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const double p = dapply<OP>(0.0, dapply<OP>(0.0, carry, sm[E + u * NW + warp]), lane_excl[u]);
+      double o[2];
+      if (exclusive) {
+        o[0] = p;
+        o[1] = dapply<OP>(0.0, p, x[u][0]);
+      } else {
+        o[0] = dapply<OP>(0.0, p, x[u][0]);
+        o[1] = dapply<OP>(0.0, p, x[u][1]);
+      }
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * 2;
+      if (i0 + 2 <= n) {
+        st2_hint(out + i0, o, stream);
+      } else if (i0 < n) {
+        out[i0] = o[0];
+      }
+    }
+    bar_workers();  // sm is reused; every worker has read its carry
+    if (threadIdx.x == 0) st_rel_sh(&cq_tail, it + 1);
+  }
+}
+
+template <int OP, int U, int MINB>
+cudaError_t scan_l2_f64(const Launch& L, Scratch& Sc, bool exclusive, double init, const double* in, double* out, size_t n) {
+  constexpr size_t L2_TILE = L2Geom<U>::TILE, L2_SMEM = L2Geom<U>::SMEM;
+  const size_t ntiles = (n + L2_TILE - 1) / L2_TILE;
+  if (2 * ntiles > Sc.scan_state64_words || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
+  auto kern = scan_l2_f64_kernel<OP, U, MINB>;
+  static int ctas_per_sm = 0;
+  if (ctas_per_sm == 0) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L2_SMEM);
+    if (e != cudaSuccess) return e;
+    int per = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, (L2_NW + 1) * 32, L2_SMEM);
+    if (e != cudaSuccess) return e;
+    if (per < 1) return cudaErrorInvalidValue;
+    ctas_per_sm = per;
+  }
+  size_t grid = size_t(L.sms) * ctas_per_sm;
+  if (grid > ntiles) grid = ntiles;
+  int excl = exclusive ? 1 : 0;
+  unsigned long long launch_no = ++Sc.scan_launch64;  // starts at 1: the zero-initialised array holds no valid tag
+  unsigned nt = (unsigned)ntiles;
+  void* args[] = {&in, &out, &n, &init, &excl, &Sc.scan_state64, &launch_no, &nt};
+  cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(kern), dim3((unsigned)grid), dim3((L2_NW + 1) * 32), args,
+                                              L2_SMEM, L.stream);
+  ++*L.launches;
+  return e;
+}
+
 size_t f64_chunk(size_t n) {  // elements per block of the chunked kernels: a multiple of 1024, at most MAX_PARTIALS chunks
   size_t chunk = 8192;
   const size_t need = (n + MAX_PARTIALS - 1) / MAX_PARTIALS;
@@ -415,9 +686,25 @@ cudaError_t launch_mapreduce_f64(const Launch& L, const Scratch& S, int map_fn, 
   return cudaErrorInvalidValue;
 }
 
-cudaError_t launch_scan_f64(const Launch& L, const Scratch& S, int op, bool exclusive, double init, const double* in,
+size_t scan_f64_state_words(size_t n) { return n >= SCAN_F64_L2_MIN ? 2 * ((n + L2_TILE_MIN - 1) / L2_TILE_MIN) : 0; }
+
+// 16 KB tiles with three CTAs per SM measured 4 - 5 % faster than 32 KB tiles with two at every size from 2^24 to 2^27
+template <int OP>
+cudaError_t scan_l2_f64_any(const Launch& L, Scratch& S, bool exclusive, double init, const double* in, double* out, size_t n) {
+  return scan_l2_f64<OP, 4, 3>(L, S, exclusive, init, in, out, n);
+}
+
+cudaError_t launch_scan_f64(const Launch& L, Scratch& S, int op, bool exclusive, double init, const double* in,
                             double* out, size_t n) {
   if (n == 0) return cudaSuccess;
+  if (n >= SCAN_F64_L2_MIN && reinterpret_cast<uintptr_t>(in) % 16 == 0 && reinterpret_cast<uintptr_t>(out) % 16 == 0) {
+    switch (op) {
+      case FN_ADD: return scan_l2_f64_any<FN_ADD>(L, S, exclusive, init, in, out, n);
+      case FN_MULT: return scan_l2_f64_any<FN_MULT>(L, S, exclusive, init, in, out, n);
+      case FN_MAX: return scan_l2_f64_any<FN_MAX>(L, S, exclusive, init, in, out, n);
+    }
+    return cudaErrorInvalidValue;
+  }
   switch (op) {
     case FN_ADD: return scan_op<FN_ADD>(L, S, exclusive, init, in, out, n);
     case FN_MULT: return scan_op<FN_MULT>(L, S, exclusive, init, in, out, n);

@@ -25,6 +25,9 @@ struct Scratch {       // device scratch owned by the context (see api.cu)
   unsigned long long* scan_state;  // scan: per-tile (epoch|status|value) words, zero-initialised
   size_t scan_state_tiles;      // capacity of scan_state in tiles
   uint32_t scan_epoch;          // incremented per look-back launch (host side)
+  unsigned long long* scan_state64 = nullptr;  // fp64 single-pass scan: 16 bytes per tile (aggregate, launch number)
+  size_t scan_state64_words = 0;               // capacity in 8-byte words, zero-initialised, never cleared
+  unsigned long long scan_launch64 = 0;        // launch number of the last fp64 single-pass scan (tags the states)
 };
 constexpr int MAX_PARTIALS = 8192;
 
@@ -132,7 +135,11 @@ cudaError_t launch_map_f64(const Launch& L, int fn, bool has_in1, double c, cons
                            const double* in2, double* out, size_t n);
 cudaError_t launch_mapreduce_f64(const Launch& L, const Scratch& S, int map_fn, bool has_in1, int red_op, double c,
                                  const double* in0, const double* in1, size_t n, double* result /* device */);
-cudaError_t launch_scan_f64(const Launch& L, const Scratch& S, int op, bool exclusive, double init, const double* in,
+// n >= SCAN_F64_L2_MIN (16-byte aligned operands): single pass ("l2ahead"), needs scan_f64_state_words(n) words of
+// Scratch::scan_state64; smaller n: three kernels.
+constexpr size_t SCAN_F64_L2_MIN = size_t(1) << 20;
+size_t scan_f64_state_words(size_t n);
+cudaError_t launch_scan_f64(const Launch& L, Scratch& S, int op, bool exclusive, double init, const double* in,
                             double* out, size_t n);
 // axis 0: along the rows (a vector is rows = 1), 1: along the columns
 cudaError_t launch_overlap1d_f64(const Launch& L, const Weights1D64& w, int r, int edge, double pad, int axis,

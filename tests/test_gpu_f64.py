@@ -133,6 +133,48 @@ def test_scan_f64(ctx):
         c.destroy()
 
 
+def test_scan_f64_single_pass_path(ctx):
+    """n >= 2^20 takes the single-pass kernel (f64.cu scan_l2_f64_kernel): several tiles per CTA (296 CTAs x 4096
+    elements), ragged tails, all operators, in place, and the tile states of earlier launches (tagged with their launch
+    number, never cleared) must not leak into later launches of other sizes and other data."""
+    sizes = [1 << 20, (1 << 20) + 4096 * 300 + 17, (1 << 23) + 1, (1 << 21) - 3, 1 << 20]
+    for rep, n in enumerate(sizes):
+        x = I.uniform_pm1_f64(9600 + rep, n)
+        vx, vo = ctx.vector_from(x), ctx.vector(n, S.F64)
+        ref, ab = O.scan_f64(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, x)
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        got = vo.numpy().copy()
+        assert np.all(np.abs(got - ref) <= RED_TOL * ab), n
+        for _ in range(3):
+            ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+            assert np.array_equal(vo.numpy(), got)                            # bitwise deterministic
+        ref, ab = O.scan_f64(O.FN_ADD, O.SCAN_EXCLUSIVE, -1.75, x)
+        ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, -1.75, vx, vo)
+        assert np.all(np.abs(vo.numpy() - ref) <= RED_TOL * ab), n
+        ctx.scan(S.FN_MAX, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        assert np.array_equal(vo.numpy(), np.maximum.accumulate(x))
+        ctx.scan(S.FN_MAX, S.SCAN_EXCLUSIVE, 0.5, vx, vo)
+        assert np.array_equal(vo.numpy(), O.scan_f64(O.FN_MAX, O.SCAN_EXCLUSIVE, 0.5, x)[0])
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vx)                     # in place
+        assert np.array_equal(vx.numpy(), got)
+        vx.destroy()
+        vo.destroy()
+    n = (1 << 22) + 4099
+    ones = np.ones(n)
+    vx, vo = ctx.vector_from(ones), ctx.vector(n, S.F64)
+    ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+    assert np.array_equal(vo.numpy(), np.arange(1, n + 1, dtype=np.float64))  # exact integers: any dropped tile shows
+    ctx.scan(S.FN_ADD, S.SCAN_EXCLUSIVE, 7.0, vx, vo)
+    assert np.array_equal(vo.numpy(), np.arange(7, n + 7, dtype=np.float64))
+    p = 1.0 + 1e-7 * I.uniform_pm1_f64(9610, 1 << 21)
+    vp, vq = ctx.vector_from(p), ctx.vector(p.size, S.F64)
+    ctx.scan(S.FN_MULT, S.SCAN_INCLUSIVE, 0.0, vp, vq)
+    ref = O.scan_f64(O.FN_MULT, O.SCAN_INCLUSIVE, 0.0, p)[0]
+    assert np.all(np.abs(vq.numpy() - ref) <= np.arange(1, p.size + 1) * 2.3e-16 * np.abs(ref))   # i roundings at element i
+    for c in (vx, vo, vp, vq):
+        c.destroy()
+
+
 EDGES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICATE, 0.0), (S.EDGE_CYCLIC, 0.0)]
 
 
