@@ -360,33 +360,57 @@ __device__ __forceinline__ unsigned ld_acq_sh(const unsigned* p) {
 __device__ __forceinline__ void st_rel_sh(unsigned* p, unsigned v) {
   asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
 }
-__device__ __forceinline__ void ld2_hint(double (&d)[2], const double* p, uint64_t policy) {
-  uint32_t r[4];
-  ld_hint4(r, p, policy);
-  d[0] = __hiloint2double(int(r[1]), int(r[0]));
-  d[1] = __hiloint2double(int(r[3]), int(r[2]));
+// V = 2 doubles (one 128-bit access) or a multiple of 4 (256-bit accesses) with an L2 eviction-priority policy
+template <int V> __device__ __forceinline__ void ldv_hint(double (&d)[V], const double* p, uint64_t policy) {
+  uint32_t r[2 * V];
+  if constexpr (V == 2) {
+    ld_hint4(*reinterpret_cast<uint32_t(*)[4]>(r), p, policy);
+  } else {
+#pragma unroll
+    for (int c = 0; c < V / 4; ++c)
+      asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8], %9;"
+                   : "=r"(r[8 * c]), "=r"(r[8 * c + 1]), "=r"(r[8 * c + 2]), "=r"(r[8 * c + 3]), "=r"(r[8 * c + 4]),
+                     "=r"(r[8 * c + 5]), "=r"(r[8 * c + 6]), "=r"(r[8 * c + 7])
+                   : "l"(p + 4 * c), "l"(policy)
+                   : "memory");
+  }
+#pragma unroll
+  for (int j = 0; j < V; ++j) d[j] = __hiloint2double(int(r[2 * j + 1]), int(r[2 * j]));
 }
-__device__ __forceinline__ void st2_hint(double* p, const double (&d)[2], uint64_t policy) {
-  const uint32_t r[4] = {uint32_t(__double2loint(d[0])), uint32_t(__double2hiint(d[0])), uint32_t(__double2loint(d[1])),
-                         uint32_t(__double2hiint(d[1]))};
-  st_hint4(p, r, policy);
+template <int V> __device__ __forceinline__ void stv_hint(double* p, const double (&d)[V], uint64_t policy) {
+  uint32_t r[2 * V];
+#pragma unroll
+  for (int j = 0; j < V; ++j) {
+    r[2 * j] = uint32_t(__double2loint(d[j]));
+    r[2 * j + 1] = uint32_t(__double2hiint(d[j]));
+  }
+  if constexpr (V == 2) {
+    st_hint4(p, *reinterpret_cast<const uint32_t(*)[4]>(r), policy);
+  } else {
+#pragma unroll
+    for (int c = 0; c < V / 4; ++c)
+      asm volatile("st.global.L1::no_allocate.L2::cache_hint.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8}, %9;" ::"l"(p + 4 * c),
+                   "r"(r[8 * c]), "r"(r[8 * c + 1]), "r"(r[8 * c + 2]), "r"(r[8 * c + 3]), "r"(r[8 * c + 4]),
+                   "r"(r[8 * c + 5]), "r"(r[8 * c + 6]), "r"(r[8 * c + 7]), "l"(policy)
+                   : "memory");
+  }
 }
 
 constexpr int L2_NW = 8, L2_D = 2, L2_S = 2, L2_KW = 10;   // the operating point of the i32 kernel
 constexpr int L2_WT = L2_NW * 32;
-// tile = 256 threads x 2 doubles x U: U = 4 -> 16 KB tiles, 3 CTAs per SM (U = 8: 32 KB tiles, 2 CTAs per SM)
-template <int U> struct L2Geom {
-  static constexpr size_t TILE = size_t(L2_WT) * 2 * U;
+// tile = 256 threads x V doubles x U
+template <int U, int V = 2> struct L2Geom {
+  static constexpr size_t TILE = size_t(L2_WT) * V * U;
   static constexpr size_t SMEM = L2_S * TILE * 8 + L2_S * 8 + 16;
 };
-constexpr size_t L2_TILE_MIN = L2Geom<4>::TILE;   // the state array is sized for the smaller tile
+constexpr size_t L2_TILE_MIN = L2Geom<4, 2>::TILE;  // the state array is sized for the smaller of the two tiles in use
 
-template <int OP, int U, int MINB>
+template <int OP, int U, int MINB, int V>
 __global__ void __launch_bounds__((L2_NW + 1) * 32, MINB)
 scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exclusive, unsigned long long* state,
                    unsigned long long launch_no, unsigned ntiles) {
   constexpr int NW = L2_NW, D = L2_D, S = L2_S, KW = L2_KW, WT = L2_WT, E = U * NW, Q = D + 2;
-  constexpr size_t TILE = L2Geom<U>::TILE;
+  constexpr size_t TILE = L2Geom<U, V>::TILE;
   constexpr unsigned FULL = 0xffffffffu;
   __shared__ double sm[2 * E + 1];
   __shared__ double red[2][NW];
@@ -471,8 +495,8 @@ scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exc
       mbar_wait(&full[j % S], (j / S) & 1u);
       const double* stage = ring + size_t(j % S) * TILE;
 #pragma unroll
-      for (int u = 0; u < U; ++u) {
-        const double2 q = *reinterpret_cast<const double2*>(stage + (u * WT + threadIdx.x) * 2);
+      for (int k = 0; k < U * V / 2; ++k) {  // any fixed grouping serves for the aggregate: consecutive 16-byte reads
+        const double2 q = *reinterpret_cast<const double2*>(stage + (k * WT + threadIdx.x) * 2);
         a = dapply<OP>(0.0, a, dapply<OP>(0.0, q.x, q.y));
       }
     } else {  // ragged last tile: guarded loads
@@ -499,22 +523,23 @@ scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exc
   unsigned it = 0;
   for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
     const size_t base = size_t(tile) * TILE;
-    double x[U][2], lane_excl[U];
+    double x[U][V], lane_excl[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {  // second read of the tile: an L2 hit
-      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * 2;
-      if (i0 + 2 <= n) {
-        ld2_hint(x[u], in + i0, stream);
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * V;
+      if (i0 + V <= n) {
+        ldv_hint<V>(x[u], in + i0, stream);
       } else {
-        x[u][0] = i0 < n ? in[i0] : ident;
-        x[u][1] = ident;
+#pragma unroll
+        for (int j = 0; j < V; ++j) x[u][j] = i0 + j < n ? in[i0 + j] : ident;
       }
     }
     if (red_tile(it + D) < ntiles) reduce_tile(it + D);
 #pragma unroll
     for (int u = 0; u < U; ++u) {  // local scan of the tile (registers)
-      x[u][1] = dapply<OP>(0.0, x[u][0], x[u][1]);
-      double ws = x[u][1];
+#pragma unroll
+      for (int j = 1; j < V; ++j) x[u][j] = dapply<OP>(0.0, x[u][j - 1], x[u][j]);
+      double ws = x[u][V - 1];
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) {
         const double y = __shfl_up_sync(FULL, ws, o);
@@ -556,19 +581,19 @@ scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exc
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       const double p = dapply<OP>(0.0, dapply<OP>(0.0, carry, sm[E + u * NW + warp]), lane_excl[u]);
-      double o[2];
-      if (exclusive) {
-        o[0] = p;
-        o[1] = dapply<OP>(0.0, p, x[u][0]);
-      } else {
-        o[0] = dapply<OP>(0.0, p, x[u][0]);
-        o[1] = dapply<OP>(0.0, p, x[u][1]);
+      double o[V];
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        if (exclusive) o[j] = j == 0 ? p : dapply<OP>(0.0, p, x[u][j - 1]);
+        else o[j] = dapply<OP>(0.0, p, x[u][j]);
       }
-      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * 2;
-      if (i0 + 2 <= n) {
-        st2_hint(out + i0, o, stream);
-      } else if (i0 < n) {
-        out[i0] = o[0];
+      const size_t i0 = base + (size_t(u) * WT + threadIdx.x) * V;
+      if (i0 + V <= n) {
+        stv_hint<V>(out + i0, o, stream);
+      } else {
+#pragma unroll
+        for (int j = 0; j < V; ++j)
+          if (i0 + j < n) out[i0 + j] = o[j];
       }
     }
     bar_workers();  // sm is reused; every worker has read its carry
@@ -576,12 +601,12 @@ scan_l2_f64_kernel(const double* in, double* out, size_t n, double init, int exc
   }
 }
 
-template <int OP, int U, int MINB>
+template <int OP, int U, int MINB, int V>
 cudaError_t scan_l2_f64(const Launch& L, Scratch& Sc, bool exclusive, double init, const double* in, double* out, size_t n) {
-  constexpr size_t L2_TILE = L2Geom<U>::TILE, L2_SMEM = L2Geom<U>::SMEM;
+  constexpr size_t L2_TILE = L2Geom<U, V>::TILE, L2_SMEM = L2Geom<U, V>::SMEM;
   const size_t ntiles = (n + L2_TILE - 1) / L2_TILE;
   if (2 * ntiles > Sc.scan_state64_words || ntiles > 0x7fffffffu) return cudaErrorInvalidValue;
-  auto kern = scan_l2_f64_kernel<OP, U, MINB>;
+  auto kern = scan_l2_f64_kernel<OP, U, MINB, V>;
   static int ctas_per_sm = 0;
   if (ctas_per_sm == 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L2_SMEM);
@@ -688,10 +713,16 @@ cudaError_t launch_mapreduce_f64(const Launch& L, const Scratch& S, int map_fn, 
 
 size_t scan_f64_state_words(size_t n) { return n >= SCAN_F64_L2_MIN ? 2 * ((n + L2_TILE_MIN - 1) / L2_TILE_MIN) : 0; }
 
-// 16 KB tiles with three CTAs per SM measured 4 - 5 % faster than 32 KB tiles with two at every size from 2^24 to 2^27
+// A thread owns V = 8 contiguous doubles per step (two 256-bit accesses), U = 2 steps per 32 KB tile: the cross-lane
+// scans (10 shuffles of 64-bit values + 5 dependent DADDs each) are what limits the fp64 form, and their number per
+// byte falls with V. Measured at 2^25 (16 B/elem): V = 2, U = 4: 133 us; V = 4, U = 2: 116 us; V = 8, U = 1 (16 KB tiles,
+// 3 CTAs per SM): 112 us; V = 16, U = 1: 113 us; V = 8, U = 2: 103 us. Operands that are only 16-byte aligned (adopted
+// pointers) take V = 2.
 template <int OP>
 cudaError_t scan_l2_f64_any(const Launch& L, Scratch& S, bool exclusive, double init, const double* in, double* out, size_t n) {
-  return scan_l2_f64<OP, 4, 3>(L, S, exclusive, init, in, out, n);
+  if (reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0)
+    return scan_l2_f64<OP, 2, 2, 8>(L, S, exclusive, init, in, out, n);
+  return scan_l2_f64<OP, 4, 3, 2>(L, S, exclusive, init, in, out, n);
 }
 
 cudaError_t launch_scan_f64(const Launch& L, Scratch& S, int op, bool exclusive, double init, const double* in,

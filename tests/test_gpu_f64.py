@@ -159,6 +159,22 @@ def test_scan_f64_single_pass_path(ctx):
         assert np.array_equal(vx.numpy(), got)
         vx.destroy()
         vo.destroy()
+    # operands that are 16- but not 32-byte aligned (adopted pointers) take the 128-bit form of the kernel; 8-byte
+    # aligned ones the three-kernel form
+    import torch
+    n = (1 << 21) + 77
+    x = I.uniform_pm1_f64(9620, n)
+    ref, ab = O.scan_f64(O.FN_ADD, O.SCAN_INCLUSIVE, 0.0, x)
+    for off in (2, 1):
+        t, to = torch.zeros(n + 8, dtype=torch.float64, device="cuda"), torch.zeros(n + 8, dtype=torch.float64, device="cuda")
+        t[off:n + off] = torch.from_numpy(x).cuda()
+        vx, vo = ctx.vector_adopt(t[off:n + off]), ctx.vector_adopt(to[off:n + off])
+        ctx.scan(S.FN_ADD, S.SCAN_INCLUSIVE, 0.0, vx, vo)
+        ctx.sync()
+        assert np.all(np.abs(to[off:n + off].cpu().numpy() - ref) <= RED_TOL * ab), off
+        assert float(to[off - 1]) == 0.0 and float(to[n + off]) == 0.0       # nothing written outside
+        vx.destroy()
+        vo.destroy()
     n = (1 << 22) + 4099
     ones = np.ones(n)
     vx, vo = ctx.vector_from(ones), ctx.vector(n, S.F64)
