@@ -657,7 +657,7 @@ def main():
         other_dtypes["scan_inclusive_f64"] = dict(row(us, 16 * n25, S.SK_SCAN, True), note="single pass over HBM (l2ahead form, f64.cu), the tile is re-read from L2")
         wd = I.uniform_pm1_f64(36, 9)
         us = timed(lambda: ctx.mapoverlap_1d_f64(wd, 4, S.EDGE_DUPLICATE, 0.0, xd, od))
-        other_dtypes["overlap1d_r4_dup_f64"] = dict(row(us, 16 * n25, S.SK_OVERLAP1D, True), note="direct form")
+        other_dtypes["overlap1d_r4_dup_f64"] = dict(row(us, 16 * n25, S.SK_OVERLAP1D, True), note="256-bit row form (f64.cu)")
         for c in (xd, yd, od, rd):
             c.destroy()
 

@@ -304,6 +304,59 @@ overlap1d_f64_kernel(const __grid_constant__ Weights1D64 W, int r, int edge, dou
   }
 }
 
+// Row-wise fast form, radius <= R (the weights arrive zero-padded to 2R+1 taps: a zero weight adds exactly 0, the taps
+// keep their ascending order, reading 28): a thread owns 4 consecutive outputs, reads its 4 + 2R window with
+// 1 + R/2 aligned 256-bit loads (the scalar form above needs 4 + 2R 8-byte loads, and the L1 tag stage, not HBM, is
+// what bounds it) and stores one 256-bit vector; all taps unrolled, weights straight from the constant bank. Groups
+// whose window leaves the row take the per-element path. Needs 32-byte aligned rows: base pointers and cols % 4 == 0.
+__device__ __forceinline__ void ld4_cached(double (&d)[4], const double* p) {  // 256-bit read-only load that allocates in
+  uint32_t r[8];                                                              // L1: neighbours re-read the window
+  asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "l"(p));
+#pragma unroll
+  for (int j = 0; j < 4; ++j) d[j] = __hiloint2double(static_cast<int>(r[2 * j + 1]), static_cast<int>(r[2 * j]));
+}
+
+template <int R>
+__global__ void __launch_bounds__(D_THREADS)
+overlap1d_f64_rows_kernel(const __grid_constant__ Weights1D64 W, int r_true, int edge, double pad, const double* in,
+                          double* out, size_t rows, size_t cols) {
+  const size_t groups_per_row = cols / 4, ngroups = rows * groups_per_row;
+  const long long lc = static_cast<long long>(cols);
+  for (size_t g = blockIdx.x * size_t(D_THREADS) + threadIdx.x; g < ngroups; g += size_t(gridDim.x) * D_THREADS) {
+    const size_t i = g / groups_per_row;
+    const long long j0 = static_cast<long long>(g - i * groups_per_row) * 4;
+    const double* row = in + i * cols;
+    double* dst = out + i * cols + j0;
+    if (j0 - R >= 0 && j0 + 3 + R < lc) {
+      double v[4 + 2 * R];
+#pragma unroll
+      for (int c = 0; c < 1 + R / 2; ++c) ld4_cached(*reinterpret_cast<double(*)[4]>(v + 4 * c), row + j0 - R + 4 * c);
+      double acc[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+      for (int k = 0; k <= 2 * R; ++k)
+#pragma unroll
+        for (int o = 0; o < 4; ++o) acc[o] = __fma_rn(W.w[k], v[o + k], acc[o]);
+      st4(dst, acc);
+    } else {  // the true radius and the unpadded taps sit in the middle of W
+      for (int o = 0; o < 4; ++o) {
+        double a = 0.0;
+        for (int k = 0; k <= 2 * r_true; ++k) {
+          long long q = j0 + o + k - r_true;
+          double x;
+          if (q < 0 || q >= lc) {
+            if (edge == EDGE_CONSTANT) x = pad;
+            else x = row[wrap_index(q, lc, edge)];
+          } else x = row[q];
+          a = __fma_rn(W.w[k + R - r_true], x, a);
+        }
+        dst[o] = a;
+      }
+    }
+  }
+}
+
 __global__ void __launch_bounds__(D_THREADS)
 overlap2d_f64_kernel(const __grid_constant__ Weights2D64 W, int ry, int rx, int edge, double pad, const double* in,
                      double* out, size_t rows, size_t cols) {
@@ -751,7 +804,19 @@ cudaError_t launch_overlap1d_f64(const Launch& L, const Weights1D64& w, int r, i
   size_t grid = (total + D_THREADS - 1) / D_THREADS;
   const size_t cap = size_t(L.sms) * 64;
   if (grid > cap) grid = cap;
-  overlap1d_f64_kernel<<<(unsigned)grid, D_THREADS, 0, L.stream>>>(w, r, edge, pad, axis, in, out, rows, cols);
+  const bool rows_fast = axis == 0 && r >= 0 && r <= 16 && cols % 4 == 0 && cols >= 64 &&
+                         reinterpret_cast<uintptr_t>(in) % 32 == 0 && reinterpret_cast<uintptr_t>(out) % 32 == 0;
+  if (rows_fast) {
+    const int R = r <= 4 ? 4 : (r <= 8 ? 8 : 16);
+    Weights1D64 wp;
+    for (double& x : wp.w) x = 0.0;
+    for (int k = 0; k <= 2 * r; ++k) wp.w[k + R - r] = w.w[k];
+    if (R == 4) overlap1d_f64_rows_kernel<4><<<(unsigned)grid, D_THREADS, 0, L.stream>>>(wp, r, edge, pad, in, out, rows, cols);
+    else if (R == 8) overlap1d_f64_rows_kernel<8><<<(unsigned)grid, D_THREADS, 0, L.stream>>>(wp, r, edge, pad, in, out, rows, cols);
+    else overlap1d_f64_rows_kernel<16><<<(unsigned)grid, D_THREADS, 0, L.stream>>>(wp, r, edge, pad, in, out, rows, cols);
+  } else {
+    overlap1d_f64_kernel<<<(unsigned)grid, D_THREADS, 0, L.stream>>>(w, r, edge, pad, axis, in, out, rows, cols);
+  }
   ++*L.launches;
   return cudaGetLastError();
 }

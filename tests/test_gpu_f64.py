@@ -194,10 +194,11 @@ def test_scan_f64_single_pass_path(ctx):
 EDGES = [(S.EDGE_CONSTANT, 0.0), (S.EDGE_CONSTANT, -0.75), (S.EDGE_DUPLICATE, 0.0), (S.EDGE_CYCLIC, 0.0)]
 
 
-@pytest.mark.parametrize("r", [0, 1, 4, 5, 16, 17, 64])
+@pytest.mark.parametrize("r", [0, 1, 3, 4, 5, 8, 11, 16, 17, 64])
 def test_overlap1d_f64(ctx, r):
     w = I.uniform_pm1_f64(9530 + r, 2 * r + 1)
-    for n in (1, 2, 3, 17, 100, 4097, 100003):
+    # n % 4 == 0 and n >= 64 with r <= 16: the 256-bit row form (zero-padded to radius 4, 8 or 16); everything else: scalar form
+    for n in (1, 2, 3, 17, 64, 100, 4096, 4097, 100003, 100004):
         x = I.uniform_pm1_f64(9531 + n, n)
         vx, vo = ctx.vector_from(x), ctx.vector(n, S.F64)
         for edge, pad in EDGES:
@@ -225,7 +226,7 @@ def test_overlap_matrix_and_2d_f64(ctx):
         X = I.uniform_pm1_f64(9540 + rows, rows * cols).reshape(rows, cols)
         mx, mo = ctx.matrix_from(X), ctx.matrix(rows, cols, S.F64)
         for edge, pad in EDGES:
-            for r in (1, 8):
+            for r in (1, 8, 13):
                 w = I.uniform_pm1_f64(9541 + r, 2 * r + 1)
                 for axis, oax in ((S.AXIS_ROW, O.AXIS_ROW), (S.AXIS_COL, O.AXIS_COL)):
                     ctx.mapoverlap_1d_matrix_f64(w, r, edge, pad, axis, mx, mo)
