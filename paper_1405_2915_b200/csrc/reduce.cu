@@ -9,13 +9,15 @@
 // chunk of the input (32 / 64 / 128 KB per operand, at most MAX_PARTIALS chunks) instead of 148 x k persistent blocks
 // with a strided tile walk: the hardware block scheduler then balances the SMs (co-resident persistent blocks drift
 // apart and an SM ends the kernel half empty), and the partial of a chunk depends on (n, variant) only: deterministic.
-// The "*_iatom" variants replace the ticket + fold of an int32 add / max by atomics on a scratch word (integer add and
-// max are associative and commutative: the result has the same bits in any order): add packs the running sum (high 32
-// bits, wraps modulo 2^32) and the count of arrived blocks (low 32 bits) into ONE 64-bit atomicAdd, so a block pays a
-// single L2 round trip, no fence and no partial; the block that reads count = grid - 1 holds the total and zeroes the
-// word. max uses atomicMax on the order-preserving image v ^ 0x80000000 (identity 0) + fence + ticket. Measured on
-// B200 at n = 2^26 in a stand-alone probe: fold 48.4 us, add + fence + ticket 46.5 us, no end chain at all 43.9 us.
-// Every other case (fp32, mult) takes the ordinary fold inside these variants.
+// The "*_iatom" variants replace the ticket + fold of an int32 ADD by ONE packed 64-bit atomicAdd per block (integer add
+// is associative and commutative: the result has the same bits in any order): the running sum sits in the high 32 bits
+// (wraps modulo 2^32), the count of arrived blocks in the low 32 bits, so a block pays a single L2 round trip, no fence
+// and no partial; the block that reads count = grid - 1 holds the total and zeroes the word. Measured on B200 at
+// n = 2^26: 43.3 us against 47.5 us for the fold in bench.py (46.0 -> 42-43 us back to back). The same idea for max
+// (atomicMax on a scratch word + fence + ticket) was measured and dropped: two atomics per block on one 32-byte sector
+// are 16 384 same-address atomics per launch, and their rate depends on where the scratch word lands (45.4 us in one
+// process, 55.6 us in bench.py, against 47.5 us for the fold). Every other case (max, mult, fp32) takes the ordinary
+// fold inside these variants.
 #include "common.cuh"
 #include "kernels.hpp"
 #include <string.h>
@@ -86,25 +88,16 @@ mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigne
   for (int j = 1; j < V; ++j) v = apply_fn<OP>(T(0), v, acc[j]);
   v = block_reduce<T, OP>(v, smem);
 
-  if constexpr (END == END_ATOMIC) {  // int32 add / max only (launch_one)
+  if constexpr (END == END_ATOMIC) {  // int32 add only (launch_one)
     if (threadIdx.x == 0) {
       if (gridDim.x == 1) {
         *result = v;
-      } else if constexpr (OP == FN_ADD) {
+      } else {
         unsigned long long* word = reinterpret_cast<unsigned long long*>(ticket + 2);
         const unsigned long long old = atomicAdd(word, ((unsigned long long)(uint32_t)v << 32) | 1ull);
         if (uint32_t(old) == gridDim.x - 1) {  // every other block has arrived: old carries their sum
           *result = T(uint32_t(old >> 32) + uint32_t(v));
           *word = 0;  // nobody else touches it in this launch; the next launch is ordered behind this one
-        }
-      } else {
-        unsigned* best = ticket + 4;
-        atomicMax(best, uint32_t(v) ^ 0x80000000u);
-        __threadfence();
-        const unsigned t = atomicInc(ticket, gridDim.x - 1);
-        if (t == gridDim.x - 1) {
-          __threadfence();
-          *result = T(atomicExch(best, 0u) ^ 0x80000000u);
         }
       }
     }
@@ -172,7 +165,7 @@ cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, 
   if (grid > ntiles) grid = ntiles;
   if (grid > MAX_PARTIALS) grid = MAX_PARTIALS;
   T* partials = static_cast<T*>(S.partials);
-  if constexpr (std::is_same<T, int32_t>::value && (OP == FN_ADD || OP == FN_MAX) && V == 4) {
+  if constexpr (std::is_same<T, int32_t>::value && OP == FN_ADD && V == 4) {
     if (rv.iatom) {
       mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, END_ATOMIC>
           <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
