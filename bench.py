@@ -564,6 +564,21 @@ def main():
                      "bytes_per_elem": 8, "GB/s_at_8B": round(8 * m / us / 1e3, 1),
                      "frac_measured_hbm": round(8 * m / us / 1e3 / peak, 4),
                      "two_calls_us": round(two, 2), "speedup_over_two_calls": round(two / us, 3)}
+        # the same pair with CONSTANT 0 edges: the register-marching form (csrc/separable.cu "march_r8") needs no border pass there
+        callc = lambda: ctx.mapoverlap_separable(d["wr8"], 8, d["wc8"], 8, S.EDGE_CONSTANT, 0.0, wl.mX, wl.mO)  # noqa: E731
+        for _ in range(3):
+            callc()
+        ts = []
+        for _ in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            callc()
+            e1.record()
+            e1.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        usc = float(np.median(ts))
+        separable["const0_edges"] = {"us": round(usc, 2), "variant": S.variant_names(S.SK_SEPARABLE)[ctx.last_variant()[1]],
+                                     "GB/s_at_8B": round(8 * m / usc / 1e3, 1), "frac_measured_hbm": round(8 * m / usc / 1e3 / peak, 4)}
 
     # ---- row-wise Reduce on the 8192^2 matrix (reported, not part of `value`)
     reduce_rows = map3 = None

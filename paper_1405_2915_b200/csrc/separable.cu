@@ -13,6 +13,7 @@
 // row pass of the clamped / wrapped row, which is what the patched window holds.
 // Taps accumulate in ascending order from zero in both passes, like the 1D kernels.
 #include "overlap2d_tiles.cuh"
+#include <string.h>
 
 namespace skel {
 namespace {
@@ -31,7 +32,8 @@ template <int R, int OY, int STAGES>
 __global__ void __launch_bounds__(T2_THREADS)
 separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_constant__ Weights1D Wcol,
                        const __grid_constant__ CUtensorMap tmap, int edge, float pad, const float* in, float* out,
-                       int rows, int cols, int tiles_x, int ntiles, unsigned* tile_ctr, unsigned tile_base) {
+                       int rows, int cols, int tiles_x, int ntiles, unsigned* tile_ctr, unsigned tile_base,
+                       int frame_tiles_y /* 0: all tiles; > 2: only the tiles on the border of a tiles_x x frame_tiles_y grid */) {
   using S = SepGeom<R, OY, STAGES>;
   using G = typename S::G;
   constexpr int RXP = S::RXP, TH = S::TH, SW = S::SW, SH = S::SH;
@@ -60,7 +62,15 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
     if (!exhausted) exhausted = t >= unsigned(ntiles);
     if (!exhausted) t_next = atomicAdd(tile_ctr, 1u) - tile_base + gridDim.x;
     if (!exhausted) {
-      const int y = int(t) / tiles_x, x = int(t) - y * tiles_x;
+      int y = int(t) / tiles_x, x = int(t) - y * tiles_x;
+      if (frame_tiles_y) {  // t counts the border tiles: first row, last row, then (left, right) of every row between
+        if (y == 1) y = frame_tiles_y - 1;
+        else if (y >= 2) {
+          const int g = int(t) - 2 * tiles_x;
+          y = 1 + g / 2;
+          x = (g & 1) ? tiles_x - 1 : 0;
+        }
+      }
       coord[s] = make_int2(y * TH, x * T2_TW);
       mbar_arrive_expect_tx(full + s, G::STAGE_BYTES);
       tma_load_2d(stage_ptr(s), &tmap, x * T2_TW - RXP, y * TH - R, full + s);
@@ -137,7 +147,7 @@ separable_fused_kernel(const __grid_constant__ Weights1D Wrow, const __grid_cons
 
 template <int R, int OY, int STAGES>
 cudaError_t launch_sep(const Launch& L, const Weights1D& wrow, const Weights1D& wcol, int edge, float pad, const float* in,
-                       float* out, size_t rows, size_t cols) {
+                       float* out, size_t rows, size_t cols, bool frame_only = false) {
   using S = SepGeom<R, OY, STAGES>;
   static_assert(S::SMEM <= 227 * 1024, "does not fit");
   auto kern = separable_fused_kernel<R, OY, STAGES>;
@@ -150,14 +160,192 @@ cudaError_t launch_sep(const Launch& L, const Weights1D& wrow, const Weights1D& 
   CUtensorMap tmap;
   cudaError_t e = make_tmap_2d(&tmap, in, rows, cols, S::SW, S::SH);
   if (e != cudaSuccess) return e;
-  const size_t tiles_x = (cols + T2_TW - 1) / T2_TW;
-  const size_t ntiles = tiles_x * ((rows + S::TH - 1) / S::TH);
+  const size_t tiles_x = (cols + T2_TW - 1) / T2_TW, tiles_y = (rows + S::TH - 1) / S::TH;
+  const bool frame = frame_only && tiles_x > 2 && tiles_y > 2;   // small matrices: every tile touches the border anyway
+  const size_t ntiles = frame ? 2 * tiles_x + 2 * (tiles_y - 2) : tiles_x * tiles_y;
   size_t grid = size_t(L.sms) * per_sm;
   if (grid > ntiles) grid = ntiles;
   kern<<<(unsigned)grid, T2_THREADS, S::SMEM, L.stream>>>(wrow, wcol, tmap, edge, pad, in, out, (int)rows, (int)cols,
-                                                          (int)tiles_x, (int)ntiles, L.tile_ctr, *L.tile_next);
+                                                          (int)tiles_x, (int)ntiles, L.tile_ctr, *L.tile_next,
+                                                          frame ? (int)tiles_y : 0);
   *L.tile_next += unsigned(ntiles);  // ntiles - grid ids fetched from the counter + one failing fetch per block
   ++*L.launches;
+  return cudaGetLastError();
+}
+
+// ---- register-marching form ("march_r8") ----------------------------------------------------------------------------
+// One WARP per 128-column strip walks down a segment of L output rows; nothing of the intermediate T ever touches shared
+// memory. Per window row the warp reads its 4 + 16 window columns from its own ring of bulk tensor copies (3 stages of
+// 8 rows x 144 columns per warp, TMA; the warp that consumes a stage re-arms it, so there is no `empty` barrier and no
+// block barrier at all), computes the row pass of 4 columns per lane (broadcast FFMA2, two chains), and feeds the 4
+// values into the 17 column-pass accumulators of the 17 output rows that are in flight (68 registers; the row that
+// receives its last tap is stored). The accumulator a T row goes to depends on (row mod 17), so the row loop is unrolled
+// 17 times and the rotation costs no moves. Every output receives the same taps in the same order as the two 1D calls
+// (row pass ascending from zero, rounded to fp32, column pass ascending from zero): bit-identical to them. The row pass
+// is recomputed for the 16 halo rows of a segment only (L = 222 at 8192^2: 7 %), against 25 - 50 % for the tiled forms.
+// Borders: the marching kernel sees zeros outside the matrix (the tensor copy's fill) and T = 0 in rows outside it,
+// which IS the CONSTANT policy with pad = 0; for every other policy the outputs within MR rows / columns of the border
+// (the only ones that see cells outside the matrix) are wrong, and a second launch recomputes the 32 x 128 tiles on
+// the border of the matrix with the tiled fused kernel above, which patches its windows with the edge policy (4 % of
+// the tiles at 8192^2). Patching inside the marching loop would need calls, and a call with 100 live registers
+// spills them.
+constexpr int MR = 8, MFW = 2 * MR + 1, M_KROWS = 8, M_NS = 3, M_SWC = 128 + 2 * MR;   // 144 floats per staged row
+constexpr unsigned M_STAGE_BYTES = M_KROWS * M_SWC * 4;                                  // 4608
+struct WPairs1D { float2 p[MFW + 1]; };  // p[d] = (w[d], w[d-1]) with w[-1] = w[17] = 0
+
+__device__ __forceinline__ void mbar_wait_s(uint32_t bar, unsigned parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_LOOP:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra WAIT_DONE;\nbra WAIT_LOOP;\nWAIT_DONE:\n}\n" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void march_refill(uint32_t dst, uint32_t bar, const CUtensorMap* map, int x, int y) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(M_STAGE_BYTES) : "memory");
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+               "l"(map), "r"(x), "r"(y), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ float4 lds128_s(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__global__ void __launch_bounds__(256, 2)
+separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constant__ Weights1D Wc,
+                       const __grid_constant__ CUtensorMap tmap, float* out, int rows, int cols, int L, int nstrips,
+                       int ntasks) {
+  constexpr int R = MR, FW = MFW, KROWS = M_KROWS, NS = M_NS, SWC = M_SWC;
+  constexpr unsigned STAGE_BYTES = M_STAGE_BYTES;
+  extern __shared__ __align__(128) unsigned char smraw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  unsigned char* ring = smraw + warp * (NS * STAGE_BYTES);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smraw + 8 * NS * STAGE_BYTES) + warp * NS;
+  const int task = blockIdx.x * 8 + warp;
+  if (task >= ntasks) return;   // no block-wide barrier anywhere below
+  const int seg = task / nstrips, strip = task - seg * nstrips;
+  const int r0 = seg * L, c0 = strip * 128;
+  const int nout = min(L, rows - r0);
+  const int nwin = nout + 2 * R;                  // window rows r0 - R .. r0 + nout + R - 1
+  const int nchunks = (nwin + KROWS - 1) / KROWS;
+  const uint32_t ring32 = smem_u32(ring), sbase = ring32 + lane * 16, full32 = smem_u32(full);
+  if (lane == 0) {
+    for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
+    mbar_fence_init();
+    for (int s = 0; s < NS && s < nchunks; ++s) march_refill(ring32 + s * STAGE_BYTES, full32 + 8 * s, &tmap, c0 - R, r0 - R + s * KROWS);
+  }
+  __syncwarp();
+  const bool col_ok = c0 + lane * 4 < cols;       // cols % 4 == 0: a lane's 4 columns are inside or outside together
+  float acc[FW][4];
+#pragma unroll
+  for (int s = 0; s < FW; ++s)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) acc[s][e] = 0.f;
+  float* optr = out + (static_cast<long long>(r0) - 2 * R) * cols + c0 + lane * 4;  // output row of window row `row`, minus 2R
+  uint32_t off = 0, st_off = 0;   // byte offsets in the ring of the current row and of the current stage
+  int rin = 0, chunk = 0;
+  uint32_t bar = full32;
+  unsigned ph = 0;
+  int prow = r0 - R;
+  for (int q = 0; q < nwin; q += FW) {
+#pragma unroll
+    for (int k = 0; k < FW; ++k) {
+      const int row = q + k;
+      if (row < nwin) {
+        if (rin == 0) mbar_wait_s(bar, ph);
+        float v[20];
+#pragma unroll
+        for (int g = 0; g < 5; ++g) {
+          const float4 t4 = lds128_s(sbase + off + 16 * g);
+          v[4 * g] = t4.x; v[4 * g + 1] = t4.y; v[4 * g + 2] = t4.z; v[4 * g + 3] = t4.w;
+        }
+        if (rin == KROWS - 1) {  // the warp is done with this stage: re-arm it with chunk + NS
+          __syncwarp();
+          if (lane == 0 && chunk + NS < nchunks) march_refill(ring32 + st_off, bar, &tmap, c0 - R, r0 - R + (chunk + NS) * KROWS);
+          rin = 0; ++chunk; st_off += STAGE_BYTES; bar += 8;
+          if (st_off == NS * STAGE_BYTES) { st_off = 0; bar = full32; ph ^= 1u; }
+        } else {
+          ++rin;
+        }
+        off += SWC * 4;
+        if (off == NS * KROWS * SWC * 4) off = 0;
+        // row pass, broadcast form: outputs (2j, 2j+1) take window element v[d + 2j] with taps d and d - 1
+        float t[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int d = 0; d <= FW; ++d) {
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const float x = v[d + 2 * j];
+            if (d == 0) t[2 * j] = fmaf(Wr.p[0].x, x, t[2 * j]);
+            else if (d == FW) t[2 * j + 1] = fmaf(Wr.p[FW].y, x, t[2 * j + 1]);
+            else fma2_bcast(t[2 * j], t[2 * j + 1], Wr.p[d], x);
+          }
+        }
+        if (prow < 0 || prow >= rows) t[0] = t[1] = t[2] = t[3] = 0.f;   // (cells outside arrive as zeros: CONSTANT 0)
+        ++prow;
+        // column pass: T row `row` is tap a of output m = row - a, accumulator (k - a) mod 17
+#pragma unroll
+        for (int a = 0; a < FW; ++a) {
+          const int slot = (k - a + FW) % FW;
+          if (a == 0) acc[slot][0] = acc[slot][1] = acc[slot][2] = acc[slot][3] = 0.f;
+          fma2_into(acc[slot][0], acc[slot][1], Wc.w[a], t[0], t[1]);
+          fma2_into(acc[slot][2], acc[slot][3], Wc.w[a], t[2], t[3]);
+        }
+        if (row >= 2 * R && col_ok) {
+          const int slot = (k - 2 * R + FW) % FW;
+          uint32_t raw[4] = {__float_as_uint(acc[slot][0]), __float_as_uint(acc[slot][1]), __float_as_uint(acc[slot][2]),
+                             __float_as_uint(acc[slot][3])};
+          st_stream<4>(optr, raw);
+        }
+        optr += cols;
+      }
+    }
+  }
+}
+
+cudaError_t launch_sep_march(const Launch& L, const Weights1D& wrow, const Weights1D& wcol, int edge, float pad, const float* in,
+                             float* out, size_t rows, size_t cols) {
+  constexpr size_t smem = 8 * M_NS * M_STAGE_BYTES + 8 * M_NS * sizeof(uint64_t);
+  uint32_t pad_bits;
+  memcpy(&pad_bits, &pad, 4);
+  const bool zeros_outside = edge == EDGE_CONSTANT && pad_bits == 0u;   // +0.0 only: the fill of the tensor copy
+  // the second launch redoes the border TILES: they cover the frame only if the last (ragged) tile row / column holds
+  // at least MR rows / columns; other shapes, and matrices of at most two tiles in a direction, run the tiled kernel alone
+  const bool frame_in_border_tiles = (rows % 32 == 0 || rows % 32 >= MR) && (cols % T2_TW == 0 || cols % T2_TW >= MR) &&
+                                     (cols + T2_TW - 1) / T2_TW > 2 && (rows + 31) / 32 > 2;
+  if (!zeros_outside && !frame_in_border_tiles) return launch_sep<MR, 4, 1>(L, wrow, wcol, edge, pad, in, out, rows, cols);
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    cudaFuncSetAttribute(separable_march_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, separable_march_kernel, 256, smem) != cudaSuccess || per_sm < 1)
+      return cudaErrorInvalidValue;
+  }
+  CUtensorMap tmap;
+  cudaError_t e = make_tmap_2d(&tmap, in, rows, cols, M_SWC, M_KROWS);
+  if (e != cudaSuccess) return e;
+  WPairs1D P;
+  for (int d = 0; d <= MFW; ++d) {
+    P.p[d].x = d < MFW ? wrow.w[d] : 0.f;
+    P.p[d].y = d >= 1 ? wrow.w[d - 1] : 0.f;
+  }
+  // segments: whole waves of (SMs x resident blocks x 8) warps when the matrix is large enough, segments of about 224
+  // rows (7 % halo), never shorter than 32 rows
+  const size_t nstrips = (cols + 127) / 128;
+  const size_t slots = size_t(L.sms) * per_sm * 8;
+  const size_t per_wave = slots / nstrips > 0 ? slots / nstrips : 1;
+  const size_t want = (rows + 223) / 224;
+  const size_t waves = (want + per_wave - 1) / per_wave;
+  size_t nseg = waves * per_wave;
+  const size_t max_seg = (rows + 31) / 32;
+  if (nseg > max_seg) nseg = max_seg;
+  const size_t Lrows = (rows + nseg - 1) / nseg;
+  nseg = (rows + Lrows - 1) / Lrows;
+  const size_t ntasks = nstrips * nseg;
+  const size_t grid = (ntasks + 7) / 8;
+  separable_march_kernel<<<(unsigned)grid, 256, smem, L.stream>>>(P, wcol, tmap, out, (int)rows, (int)cols, (int)Lrows, (int)nstrips,
+                                                                   (int)ntasks);
+  ++*L.launches;
+  if (!zeros_outside)  // the border tiles again, with the edge policy (they are a superset of the frame)
+    return launch_sep<MR, 4, 1>(L, wrow, wcol, edge, pad, in, out, rows, cols, true);
   return cudaGetLastError();
 }
 
@@ -171,8 +359,8 @@ cudaError_t launch_sep_r(const Launch& L, int v, const Weights1D& wrow, const We
   return cudaErrorInvalidValue;
 }
 
-const char* const kSepNames[] = {"two_pass", "fused_oy4", "fused_oy8", "fused_oy4_s1", "fused_oy8_s1"};
-constexpr int kNumSep = 5;
+const char* const kSepNames[] = {"two_pass", "fused_oy4", "fused_oy8", "fused_oy4_s1", "fused_oy8_s1", "march_r8"};
+constexpr int kNumSep = 6;
 
 }  // namespace
 
@@ -191,6 +379,8 @@ bool separable_variant_ok(int v, int r_row, int r_col, const void* in, const voi
 cudaError_t launch_separable_fused(const Launch& L, int v, const Weights1D& wrow, const Weights1D& wcol, int r_row,
                                    int r_col, int edge, float pad, const float* in, float* out, size_t rows, size_t cols) {
   if (rows * cols == 0) return cudaSuccess;
+  if (v == 5)  // the marching form exists for radius 8; smaller radii run it zero-padded (kernels.hpp)
+    return launch_sep_march(L, pad_weights_1d(wrow, r_row, MR), pad_weights_1d(wcol, r_col, MR), edge, pad, in, out, rows, cols);
   const int rmax = r_row > r_col ? r_row : r_col;
   const int r = rmax <= 4 ? (rmax < 1 ? 1 : rmax) : (rmax <= 8 ? 8 : -1);
   if (r != r_row || r != r_col)  // zero-padded to the next instantiated radius (kernels.hpp)

@@ -45,6 +45,7 @@ def instances(S):
         out.append((f"overlap2d_{2*r+1}x{2*r+1}", I(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, r1=r, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
     out.append(("reduce_rows_add_f32", I(skeleton=S.SK_REDUCE_ROWS, fn=S.FN_ADD, dtype=S.F32), 20, 26, 8192))
     out.append(("separable_r8", I(skeleton=S.SK_SEPARABLE, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, r1=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    out.append(("separable_r8_const", I(skeleton=S.SK_SEPARABLE, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, r1=8, edge=S.EDGE_CONSTANT), 20, 26, 8192))
     return out
 
 

@@ -170,6 +170,29 @@ def test_reduce_f32_tolerance_and_determinism(ctx, v):
             vy.destroy()
 
 
+def test_reduce_i32_atomic_end_chain_resets_its_scratch_word(ctx):
+    """The *_iatom variants keep (sum, count of arrived blocks) in one scratch word that the last block zeroes: launches
+    of different sizes, operators and element types in any order must each start from a clean word."""
+    names = S.variant_names(S.SK_REDUCE)
+    sizes = [(1 << 20) + 5, 8192 * 3, (1 << 22) + 4097, 8193, 1 << 21, 100003, (1 << 23) + 1]
+    data = {n: I.full_range_i32(240 + n, n) for n in sizes}
+    vecs = {n: ctx.vector_from(a) for n, a in data.items()}
+    xf = I.uniform_pm1_f32(241, 1 << 20)
+    vf = ctx.vector_from(xf)
+    reff, abf = O.reduce_f32(O.FN_ADD, xf)
+    for v in [i for i, nm in enumerate(names) if nm.endswith("_iatom")]:
+        with forced(ctx, S.SK_REDUCE, v):
+            for rep in range(3):
+                for n in sizes if rep % 2 == 0 else reversed(sizes):
+                    assert ctx.reduce(S.FN_ADD, vecs[n]) == O.reduce_i32(O.FN_ADD, data[n])[0], (names[v], n)
+                    if n % 3 == 0:
+                        assert ctx.reduce(S.FN_MAX, vecs[n]) == O.reduce_i32(O.FN_MAX, data[n])[0]
+                    if n % 2 == 1:
+                        assert_reduce_f32(ctx.reduce(S.FN_ADD, vf), reff, abf)
+    for c in list(vecs.values()) + [vf]:
+        c.destroy()
+
+
 def test_reduce_closed_forms_and_max_position(ctx):
     for n in [1, 1000, 4096, (1 << 20) + 3]:
         v = ctx.vector_from(np.ones(n, np.float32))
