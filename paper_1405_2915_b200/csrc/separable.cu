@@ -184,11 +184,12 @@ cudaError_t launch_sep(const Launch& L, const Weights1D& wrow, const Weights1D& 
 // (row pass ascending from zero, rounded to fp32, column pass ascending from zero): bit-identical to them. The row pass
 // is recomputed for the 16 halo rows of a segment only (L = 222 at 8192^2: 7 %), against 25 - 50 % for the tiled forms.
 // Borders: the marching kernel sees zeros outside the matrix (the tensor copy's fill) and T = 0 in rows outside it,
-// which IS the CONSTANT policy with pad = 0; for every other policy the outputs within MR rows / columns of the border
-// (the only ones that see cells outside the matrix) are wrong, and a second launch recomputes the 32 x 128 tiles on
-// the border of the matrix with the tiled fused kernel above, which patches its windows with the edge policy (4 % of
-// the tiles at 8192^2). Patching inside the marching loop would need calls, and a call with 100 live registers
-// spills them.
+// which IS the CONSTANT policy with pad = 0. CONSTANT with another pad and DUPLICATE are applied in registers when the
+// columns fill whole strips (kernel MODE 1 / 2 below). For CYCLIC and for ragged column counts the outputs within MR
+// rows / columns of the border (the only ones that see cells outside the matrix) come out wrong, and a second launch
+// recomputes the 32 x 128 tiles on the border of the matrix with the tiled fused kernel above, which patches its windows
+// with the edge policy (4 % of the tiles at 8192^2). Patching the stages inside the marching loop would need calls, and
+// a call with 100 live registers spills them.
 constexpr int MR = 8, MFW = 2 * MR + 1, M_KROWS = 8, M_NS = 3, M_SWC = 128 + 2 * MR;   // 144 floats per staged row
 constexpr unsigned M_STAGE_BYTES = M_KROWS * M_SWC * 4;                                  // 4608
 struct WPairs1D { float2 p[MFW + 1]; };  // p[d] = (w[d], w[d-1]) with w[-1] = w[17] = 0
@@ -205,24 +206,66 @@ __device__ __forceinline__ void march_refill(uint32_t dst, uint32_t bar, const C
                "l"(map), "r"(x), "r"(y), "r"(bar)
                : "memory");
 }
+__device__ __forceinline__ float lds32_s(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts64_s(uint32_t addr, float a, float b) {
+  asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a), "f"(b) : "memory");
+}
 __device__ __forceinline__ float4 lds128_s(uint32_t addr) {
   float4 v;
   asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
   return v;
 }
-__global__ void __launch_bounds__(256, 2)
-separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constant__ Weights1D Wc,
-                       const __grid_constant__ CUtensorMap tmap, float* out, int rows, int cols, int L, int nstrips,
-                       int ntasks) {
+// MODE 0: cells outside the matrix are zeros (what the tensor copy delivers) and T is 0 in rows outside it: CONSTANT 0.
+// MODE 1 (CONSTANT, pad != 0) and MODE 2 (DUPLICATE), cols % 128 == 0: the policy is applied in REGISTERS. Columns: only
+// lanes 0, 1 of the first strip and lanes 30, 31 of the last strip hold window columns outside the matrix, and the
+// element that DUPLICATE repeats (column 0 / cols - 1) is in the lane's own window. Rows: a T row outside the matrix
+// is `pad` (MODE 1) or the T of row 0 / rows - 1 (MODE 2: the last row's T is simply kept; the first row's T is computed
+// before the walk starts, from the second chunk of the ring).
+__device__ __forceinline__ void march_rowpass(const WPairs1D& Wr, const float (&v)[20], float (&t)[4]) {
+  constexpr int FW = MFW;
+  t[0] = t[1] = t[2] = t[3] = 0.f;
+#pragma unroll
+  for (int d = 0; d <= FW; ++d) {   // broadcast form: outputs (2j, 2j+1) take window element v[d + 2j] with taps d and d - 1
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const float x = v[d + 2 * j];
+      if (d == 0) t[2 * j] = fmaf(Wr.p[0].x, x, t[2 * j]);
+      else if (d == FW) t[2 * j + 1] = fmaf(Wr.p[FW].y, x, t[2 * j + 1]);
+      else fma2_bcast(t[2 * j], t[2 * j + 1], Wr.p[d], x);
+    }
+  }
+}
+template <int MODE>
+__device__ __forceinline__ void march_fix_cols(float (&v)[20], int lane, bool left, bool right, float pad) {
+  if (left && lane < 2) {          // lane 0: window columns -8 .. 11, lane 1: -4 .. 15
+    const float x0 = MODE == 1 ? pad : (lane == 0 ? v[8] : v[4]);
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      if (j < 4 || lane == 0) v[j] = x0;
+  }
+  if (right && lane >= 30) {       // lane 30: columns cols - 16 .. cols + 3, lane 31: cols - 12 .. cols + 7
+    const float x1 = MODE == 1 ? pad : (lane == 31 ? v[11] : v[15]);
+#pragma unroll
+    for (int j = 12; j < 20; ++j)
+      if (j >= 16 || lane == 31) v[j] = x1;
+  }
+}
+
+// Columns outside the matrix (MODE 1 / 2): the first and the last strip of a row of strips patch the 8 outside columns of
+// each chunk in their stage when it lands (64 cells, two per lane), then fence.proxy.async before the stage is re-armed.
+// (The same fix-up on the window registers of every row, as predicated selects, cost 12 % of the kernel; a separate copy
+// of the row loop for the border strips made them the stragglers: two 46 KB instruction streams on their SMs.)
+template <int MODE>
+__device__ __forceinline__ void march_strip(const WPairs1D& Wr, const Weights1D& Wc, const CUtensorMap* tmap, float* out, int rows,
+                                            int cols, int L, int nstrips, float pad, unsigned char* ring, uint64_t* full,
+                                            int seg, int strip) {
   constexpr int R = MR, FW = MFW, KROWS = M_KROWS, NS = M_NS, SWC = M_SWC;
   constexpr unsigned STAGE_BYTES = M_STAGE_BYTES;
-  extern __shared__ __align__(128) unsigned char smraw[];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  unsigned char* ring = smraw + warp * (NS * STAGE_BYTES);
-  uint64_t* full = reinterpret_cast<uint64_t*>(smraw + 8 * NS * STAGE_BYTES) + warp * NS;
-  const int task = blockIdx.x * 8 + warp;
-  if (task >= ntasks) return;   // no block-wide barrier anywhere below
-  const int seg = task / nstrips, strip = task - seg * nstrips;
+  const int lane = threadIdx.x & 31;
   const int r0 = seg * L, c0 = strip * 128;
   const int nout = min(L, rows - r0);
   const int nwin = nout + 2 * R;                  // window rows r0 - R .. r0 + nout + R - 1
@@ -231,7 +274,7 @@ separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constan
   if (lane == 0) {
     for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
     mbar_fence_init();
-    for (int s = 0; s < NS && s < nchunks; ++s) march_refill(ring32 + s * STAGE_BYTES, full32 + 8 * s, &tmap, c0 - R, r0 - R + s * KROWS);
+    for (int s = 0; s < NS && s < nchunks; ++s) march_refill(ring32 + s * STAGE_BYTES, full32 + 8 * s, tmap, c0 - R, r0 - R + s * KROWS);
   }
   __syncwarp();
   const bool col_ok = c0 + lane * 4 < cols;       // cols % 4 == 0: a lane's 4 columns are inside or outside together
@@ -246,12 +289,40 @@ separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constan
   uint32_t bar = full32;
   unsigned ph = 0;
   int prow = r0 - R;
+  const bool left = strip == 0, right = strip == nstrips - 1;
+  float tk[4] = {0.f, 0.f, 0.f, 0.f};   // MODE 2: the T a row outside the matrix takes (row 0's before the matrix, the last row's after)
+  if (MODE == 2 && r0 == 0) {           // matrix row 0 is window row R = row 0 of the second chunk (R == KROWS)
+    mbar_wait_s(full32 + 8, 0);
+    float v[20];
+#pragma unroll
+    for (int g = 0; g < 5; ++g) {
+      const float4 t4 = lds128_s(sbase + STAGE_BYTES + 16 * g);
+      v[4 * g] = t4.x; v[4 * g + 1] = t4.y; v[4 * g + 2] = t4.z; v[4 * g + 3] = t4.w;
+    }
+    march_fix_cols<MODE>(v, lane, left, right, pad);   // (chunk 1 is patched in shared memory only when the walk reaches it)
+    march_rowpass(Wr, v, tk);
+  }
   for (int q = 0; q < nwin; q += FW) {
 #pragma unroll
     for (int k = 0; k < FW; ++k) {
       const int row = q + k;
       if (row < nwin) {
-        if (rin == 0) mbar_wait_s(bar, ph);
+        if (rin == 0) {
+          mbar_wait_s(bar, ph);
+          if (MODE != 0 && (left || right)) {   // warp-uniform, once per chunk
+            const uint32_t a = ring32 + st_off + (lane >> 2) * (SWC * 4) + (lane & 3) * 8;   // row lane / 4, cells 2 (lane % 4), + 1
+            if (left) {
+              const float x0 = MODE == 1 ? pad : lds32_s(ring32 + st_off + (lane >> 2) * (SWC * 4) + R * 4);
+              sts64_s(a, x0, x0);
+            }
+            if (right) {
+              const float x1 = MODE == 1 ? pad : lds32_s(ring32 + st_off + (lane >> 2) * (SWC * 4) + (R + 127) * 4);
+              sts64_s(a + (R + 128) * 4, x1, x1);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic writes before the stage is re-armed
+            __syncwarp();
+          }
+        }
         float v[20];
 #pragma unroll
         for (int g = 0; g < 5; ++g) {
@@ -260,7 +331,7 @@ separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constan
         }
         if (rin == KROWS - 1) {  // the warp is done with this stage: re-arm it with chunk + NS
           __syncwarp();
-          if (lane == 0 && chunk + NS < nchunks) march_refill(ring32 + st_off, bar, &tmap, c0 - R, r0 - R + (chunk + NS) * KROWS);
+          if (lane == 0 && chunk + NS < nchunks) march_refill(ring32 + st_off, bar, tmap, c0 - R, r0 - R + (chunk + NS) * KROWS);
           rin = 0; ++chunk; st_off += STAGE_BYTES; bar += 8;
           if (st_off == NS * STAGE_BYTES) { st_off = 0; bar = full32; ph ^= 1u; }
         } else {
@@ -268,19 +339,15 @@ separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constan
         }
         off += SWC * 4;
         if (off == NS * KROWS * SWC * 4) off = 0;
-        // row pass, broadcast form: outputs (2j, 2j+1) take window element v[d + 2j] with taps d and d - 1
-        float t[4] = {0.f, 0.f, 0.f, 0.f};
+        float t[4];
+        march_rowpass(Wr, v, t);
+        if (prow < 0 || prow >= rows) {   // a T row outside the matrix
 #pragma unroll
-        for (int d = 0; d <= FW; ++d) {
+          for (int e = 0; e < 4; ++e) t[e] = MODE == 0 ? 0.f : (MODE == 1 ? pad : tk[e]);
+        } else if (MODE == 2) {
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            const float x = v[d + 2 * j];
-            if (d == 0) t[2 * j] = fmaf(Wr.p[0].x, x, t[2 * j]);
-            else if (d == FW) t[2 * j + 1] = fmaf(Wr.p[FW].y, x, t[2 * j + 1]);
-            else fma2_bcast(t[2 * j], t[2 * j + 1], Wr.p[d], x);
-          }
+          for (int e = 0; e < 4; ++e) tk[e] = t[e];   // rows after the matrix repeat the last row's T
         }
-        if (prow < 0 || prow >= rows) t[0] = t[1] = t[2] = t[3] = 0.f;   // (cells outside arrive as zeros: CONSTANT 0)
         ++prow;
         // column pass: T row `row` is tap a of output m = row - a, accumulator (k - a) mod 17
 #pragma unroll
@@ -302,6 +369,21 @@ separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constan
   }
 }
 
+template <int MODE>
+__global__ void __launch_bounds__(256, 2)
+separable_march_kernel(const __grid_constant__ WPairs1D Wr, const __grid_constant__ Weights1D Wc,
+                       const __grid_constant__ CUtensorMap tmap, float* out, int rows, int cols, int L, int nstrips,
+                       int ntasks, float pad) {
+  extern __shared__ __align__(128) unsigned char smraw[];
+  const int warp = threadIdx.x >> 5;
+  unsigned char* ring = smraw + warp * (M_NS * M_STAGE_BYTES);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smraw + 8 * M_NS * M_STAGE_BYTES) + warp * M_NS;
+  const int task = blockIdx.x * 8 + warp;
+  if (task >= ntasks) return;   // no block-wide barrier anywhere below
+  const int seg = task / nstrips, strip = task - seg * nstrips;
+  march_strip<MODE>(Wr, Wc, &tmap, out, rows, cols, L, nstrips, pad, ring, full, seg, strip);
+}
+
 cudaError_t launch_sep_march(const Launch& L, const Weights1D& wrow, const Weights1D& wcol, int edge, float pad, const float* in,
                              float* out, size_t rows, size_t cols) {
   constexpr size_t smem = 8 * M_NS * M_STAGE_BYTES + 8 * M_NS * sizeof(uint64_t);
@@ -312,11 +394,15 @@ cudaError_t launch_sep_march(const Launch& L, const Weights1D& wrow, const Weigh
   // at least MR rows / columns; other shapes, and matrices of at most two tiles in a direction, run the tiled kernel alone
   const bool frame_in_border_tiles = (rows % 32 == 0 || rows % 32 >= MR) && (cols % T2_TW == 0 || cols % T2_TW >= MR) &&
                                      (cols + T2_TW - 1) / T2_TW > 2 && (rows + 31) / 32 > 2;
-  if (!zeros_outside && !frame_in_border_tiles) return launch_sep<MR, 4, 1>(L, wrow, wcol, edge, pad, in, out, rows, cols);
+  // in-register policy (kernel MODE 1 / 2): CONSTANT and DUPLICATE on matrices whose columns fill whole strips
+  const int mode = zeros_outside ? 0 : (cols % 128 == 0 && edge == EDGE_CONSTANT ? 1 : (cols % 128 == 0 && edge == EDGE_DUPLICATE ? 2 : 0));
+  if (!zeros_outside && mode == 0 && !frame_in_border_tiles) return launch_sep<MR, 4, 1>(L, wrow, wcol, edge, pad, in, out, rows, cols);
   static int per_sm = 0;
   if (per_sm == 0) {
-    cudaFuncSetAttribute(separable_march_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, separable_march_kernel, 256, smem) != cudaSuccess || per_sm < 1)
+    cudaFuncSetAttribute(separable_march_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(separable_march_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(separable_march_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, separable_march_kernel<2>, 256, smem) != cudaSuccess || per_sm < 1)
       return cudaErrorInvalidValue;
   }
   CUtensorMap tmap;
@@ -341,10 +427,17 @@ cudaError_t launch_sep_march(const Launch& L, const Weights1D& wrow, const Weigh
   nseg = (rows + Lrows - 1) / Lrows;
   const size_t ntasks = nstrips * nseg;
   const size_t grid = (ntasks + 7) / 8;
-  separable_march_kernel<<<(unsigned)grid, 256, smem, L.stream>>>(P, wcol, tmap, out, (int)rows, (int)cols, (int)Lrows, (int)nstrips,
-                                                                   (int)ntasks);
+  if (mode == 1)
+    separable_march_kernel<1><<<(unsigned)grid, 256, smem, L.stream>>>(P, wcol, tmap, out, (int)rows, (int)cols, (int)Lrows,
+                                                                        (int)nstrips, (int)ntasks, pad);
+  else if (mode == 2)
+    separable_march_kernel<2><<<(unsigned)grid, 256, smem, L.stream>>>(P, wcol, tmap, out, (int)rows, (int)cols, (int)Lrows,
+                                                                        (int)nstrips, (int)ntasks, pad);
+  else
+    separable_march_kernel<0><<<(unsigned)grid, 256, smem, L.stream>>>(P, wcol, tmap, out, (int)rows, (int)cols, (int)Lrows,
+                                                                        (int)nstrips, (int)ntasks, pad);
   ++*L.launches;
-  if (!zeros_outside)  // the border tiles again, with the edge policy (they are a superset of the frame)
+  if (!zeros_outside && mode == 0)  // the border tiles again, with the edge policy (they are a superset of the frame)
     return launch_sep<MR, 4, 1>(L, wrow, wcol, edge, pad, in, out, rows, cols, true);
   return cudaGetLastError();
 }

@@ -76,10 +76,10 @@ def test_separable_fused_is_bit_identical_to_the_two_passes_and_plan_default(ctx
         ctx.force_variant(S.SK_SEPARABLE, v)
         ctx.reset_stats()
         ctx.mapoverlap_separable(wr, r, wc, r, S.EDGE_DUPLICATE, 0.0, mx, mo)
-        # two_pass: the two 1D kernels; march_r8: the marching kernel + the frame kernel of every policy but CONSTANT 0
-        two = v == 0 or (v >= 0 and S.variant_names(S.SK_SEPARABLE)[v].startswith("march"))
+        # two_pass: the two 1D kernels; every fused form is one launch (march_r8 applies DUPLICATE in registers when
+        # cols % 128 == 0, as here; CYCLIC and ragged column counts would add the border-tile launch)
         if v >= 0:
-            assert ctx.stats()["launches"] == (2 if two else 1)
+            assert ctx.stats()["launches"] == (2 if v == 0 else 1)
         outs.append(mo.numpy().copy())
     ctx.force_variant(S.SK_SEPARABLE, -1)
     # the same taps in the same order with the same fp32 intermediate: every variant gives the same bits
@@ -91,6 +91,38 @@ def test_separable_fused_is_bit_identical_to_the_two_passes_and_plan_default(ctx
     assert np.array_equal(outs[0], mo.numpy())
     for m in (mx, mt, mo):
         m.destroy()
+
+
+def test_separable_march_policies_and_launch_counts(ctx):
+    """march_r8: CONSTANT / DUPLICATE on cols % 128 == 0 are applied in registers (one launch), CYCLIC and ragged column
+    counts take the border-tile launch as well (two), and both give the bits of the two 1D calls; matrices tall enough
+    for several segments per strip and exactly one strip wide (both border fix-ups in the same warp)."""
+    names = S.variant_names(S.SK_SEPARABLE)
+    v = names.index("march_r8")
+    for rows, cols in ((700, 128), (1000, 384), (517, 1024), (300, 1028), (97, 640)):
+        X = I.uniform_pm1_f32(720 + rows, rows * cols).reshape(rows, cols)
+        mx, mt, mo = ctx.matrix_from(X), ctx.matrix(rows, cols), ctx.matrix(rows, cols)
+        for r in (8, 3):
+            wr, wc = I.signed_weights_f32(721 + r, 2 * r + 1), I.signed_weights_f32(722 + r, 2 * r + 1)
+            for ge, oe, pad in EDGES:
+                ctx.mapoverlap_1d_matrix(wr, r, ge, pad, S.AXIS_ROW, mx, mt)
+                ctx.mapoverlap_1d_matrix(wc, r, ge, pad, S.AXIS_COL, mt, mo)
+                want = mo.numpy().copy()
+                ctx.force_variant(S.SK_SEPARABLE, v)
+                try:
+                    ctx.reset_stats()
+                    ctx.mapoverlap_separable(wr, r, wc, r, ge, pad, mx, mo)
+                    launches = ctx.stats()["launches"]
+                finally:
+                    ctx.force_variant(S.SK_SEPARABLE, -1)
+                assert np.array_equal(mo.numpy(), want), (rows, cols, r, ge, pad)
+                in_registers = (ge == S.EDGE_CONSTANT or ge == S.EDGE_DUPLICATE) and cols % 128 == 0
+                zeros = ge == S.EDGE_CONSTANT and pad == 0.0
+                tiled_alone = not zeros and not in_registers and (rows % 32 not in (0,) and rows % 32 < 8 or cols % 128 not in (0,) and cols % 128 < 8
+                                                                  or -(-cols // 128) <= 2 or -(-rows // 32) <= 2)
+                assert launches == (1 if zeros or in_registers or tiled_alone else 2), (rows, cols, r, ge, pad, launches)
+        for m in (mx, mt, mo):
+            m.destroy()
 
 
 def test_separable_errors(ctx):
