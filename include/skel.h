@@ -128,6 +128,13 @@ skel_status skel_ctx_set_coherence(skel_ctx* ctx, skel_coherence mode);
  * until the next skeleton call that writes the container (adopted buffers are never swapped; such a
  * chain runs call by call); (4) skel_last_variant reports variant -2 for a fused launch. */
 skel_status skel_ctx_set_fusion(skel_ctx* ctx, int enable);
+/* L2-aware traversal (default: on). A skeleton kernel streams its operands front to back, so when it ends the L2
+ * (126 MB on B200) holds the TAIL of what it read. With the setting on, a Reduce / MapReduce whose first operand is the
+ * buffer the context's previous launch also read walks that buffer in the OPPOSITE direction, so that its first chunks
+ * hit L2 instead of HBM (chained calls on one smart container, P:L123 / L137: the container layer knows what the last
+ * call touched). The result has the same bits in either direction (a block's partial belongs to its chunk, the fold
+ * order is by chunk). Off: every kernel walks forward. */
+skel_status skel_ctx_set_l2_reuse(skel_ctx* ctx, int enable);
 /* Launch everything that fusion holds back (no synchronisation). */
 skel_status skel_ctx_flush(skel_ctx* ctx);
 const char* skel_last_error(skel_ctx* ctx);
@@ -314,8 +321,8 @@ const char* skel_variant_name(int skeleton, int variant);
  * for r = 4, r = 12 what was tuned for r = 16, and only a (skeleton, dtype) without any tuned point falls back to
  * the built-in preference list. The variant found is used if it is applicable to the call (alignment, shape).
  *
- * skel_tune_instance: measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), median
- * of `reps` launches, variants interleaved, timed with CUDA events on the context stream UNDER THE CONDITIONS OF A
+ * skel_tune_instance: measure every applicable variant of `inst` at n = 2^k, k = log2_lo..log2_hi (vectors), mean of
+ * the middle half of `reps` launches (event timestamps tick in about 2 us steps: a median would be quantised), variants interleaved, timed with CUDA events on the context stream UNDER THE CONDITIONS OF A
  * SUSTAINED RUN: operands rotate through arenas larger than the L2 cache (so no launch finds its input there) and
  * every timed launch is preceded by a writer that leaves the L2 full of dirty lines, as the previous skeleton call
  * of a real sequence does. Size breakpoints are stored in the context's plan. Where the winner changes between two sampled sizes the interval is

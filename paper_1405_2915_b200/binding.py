@@ -70,6 +70,7 @@ _SIGS = {
     "skel_probe_fma_peak": ([_vp, _i, C.POINTER(C.c_double)], _i),
     "skel_probe_fma_with_loads": ([_vp, _i, _i, C.POINTER(C.c_double)], _i),
     "skel_ctx_set_fusion": ([_vp, _i], _i),
+    "skel_ctx_set_l2_reuse": ([_vp, _i], _i),
     "skel_ctx_flush": ([_vp], _i),
     "skel_last_error": ([_vp], C.c_char_p),
     "skel_vector_create": ([_vp, _i, _sz, _pp], _i),
@@ -265,6 +266,9 @@ class Context:
         out = C.c_double(0.0)
         self.check(lib.skel_probe_fma_peak(self.h, reps, C.byref(out)))
         return out.value
+
+    def set_l2_reuse(self, enable: bool):
+        self.check(lib.skel_ctx_set_l2_reuse(self.h, 1 if enable else 0))
 
     def set_fusion(self, enable: bool):
         self.check(lib.skel_ctx_set_fusion(self.h, 1 if enable else 0))

@@ -114,6 +114,10 @@ struct skel_ctx {
   int last_sk = -1, last_var = -1;
   int launches = 0;
   std::vector<float> tune_table;
+  // L2-aware traversal direction of Reduce / MapReduce (launch_now)
+  bool l2_reuse = true, reverse_next = false, walk_reverse = false;
+  const void* walk_in0 = nullptr;   // first operand of the last launch_now launch
+  uint64_t walk_launch = ~0ull;     // kernels launched by the context up to and including it
   // cross-call fusion (skel_ctx_set_fusion): launches of a fusible chain are held back here
   bool fusion = false;
   std::vector<struct PendingCall> pending;
@@ -160,8 +164,10 @@ skel_status ensure_device(skel_ctx* c) {
   CU(c, cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev));
   char* base = nullptr;
   const size_t partial_bytes = size_t(MAX_PARTIALS) * 8;
-  CU(c, cudaMalloc(reinterpret_cast<void**>(&base), partial_bytes + 256));
-  CU(c, cudaMemsetAsync(base, 0, partial_bytes + 256, c->stream));
+  CU(c, cudaMalloc(reinterpret_cast<void**>(&base), 2 * partial_bytes + 512));
+  CU(c, cudaMemsetAsync(base, 0, 2 * partial_bytes + 512, c->stream));
+  c->scratch.red_tagged = reinterpret_cast<unsigned long long*>(base + partial_bytes + 256);
+  c->scratch.red_epoch = 0;
   c->scratch.partials = base;
   c->scratch.ticket = reinterpret_cast<unsigned*>(base + partial_bytes);
   c->scratch.scan_ticket = reinterpret_cast<unsigned*>(base + partial_bytes + 64);
@@ -833,9 +839,9 @@ cudaError_t launch_call(skel_ctx* c, const Call& k, int v) {
       if (i.fn == SKEL_FN_MULADD) return launch_map3(L, v, i.dtype, k.in0, k.in1, k.in2, k.out, k.n);
       return launch_map(L, v, i.dtype, i.fn, i.mode != 0, k.cbits, k.in0, k.in1, k.out, k.n);
     case SKEL_SK_REDUCE:
-      return launch_mapreduce(L, c->scratch, v, i.dtype, FN_IDENT_, false, i.fn, 0, k.in0, nullptr, k.n, k.out);
+      return launch_mapreduce(L, c->scratch, v, i.dtype, FN_IDENT_, false, i.fn, 0, k.in0, nullptr, k.n, k.out, c->reverse_next);
     case SKEL_SK_MAPREDUCE:
-      return launch_mapreduce(L, c->scratch, v, i.dtype, i.fn, i.mode != 0, i.fn2, k.cbits, k.in0, k.in1, k.n, k.out);
+      return launch_mapreduce(L, c->scratch, v, i.dtype, i.fn, i.mode != 0, i.fn2, k.cbits, k.in0, k.in1, k.n, k.out, c->reverse_next);
     case SKEL_SK_SCAN:
       return launch_scan(L, c->scratch, v, i.dtype, i.fn, i.mode == SKEL_SCAN_EXCLUSIVE, k.cbits, k.in0, k.out, k.n);
     case SKEL_SK_OVERLAP1D:
@@ -899,8 +905,19 @@ skel_status launch_now(skel_ctx* c, const Call& k) {
     st = ensure_scan_state(c, k.n);
     if (st != SKEL_OK) return st;
   }
+  // L2-aware traversal (skel_ctx_set_l2_reuse): a kernel that streams an operand front to back leaves the operand's
+  // TAIL in the 126 MB L2. When the launch right before this one read the same operand in one direction, a Reduce /
+  // MapReduce walks it in the other, so its first chunks are L2 hits instead of HBM reads (a forward walk would evict
+  // those lines before reaching them). Same result bits either way (reduce.cu); other kernels always walk forward.
+  const bool red = k.inst.skeleton == SKEL_SK_REDUCE || k.inst.skeleton == SKEL_SK_MAPREDUCE;
+  c->reverse_next = red && c->l2_reuse && c->walk_in0 == k.in0 && c->walk_launch == c->stats.launches + uint64_t(c->launches) && !c->walk_reverse;
   cudaError_t e = launch_call(c, k, v);
+  const bool reversed = c->reverse_next;
+  c->reverse_next = false;
   if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+  c->walk_in0 = k.in0;
+  c->walk_reverse = reversed;
+  c->walk_launch = c->stats.launches + uint64_t(c->launches);
   c->last_sk = k.inst.skeleton;
   c->last_var = v;
   return SKEL_OK;
@@ -1219,6 +1236,12 @@ skel_status skel_ctx_sync(skel_ctx* c) {
   CU(c, cudaStreamSynchronize(c->stream));
   if (c->copy_stream) CU(c, cudaStreamSynchronize(c->copy_stream));  // prefetch downloads in flight
   c->done_seq = c->seq;
+  return SKEL_OK;
+}
+
+skel_status skel_ctx_set_l2_reuse(skel_ctx* c, int enable) {
+  if (!ctx_ok(c)) return SKEL_ERR_INVALID_ARG;
+  c->l2_reuse = enable != 0;
   return SKEL_OK;
 }
 
@@ -1971,8 +1994,11 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
     k.in2 = (sk == SKEL_SK_MAP && inst->fn == SKEL_FN_MULADD) ? a0 : nullptr;
     k.out = (sk == SKEL_SK_REDUCE || sk == SKEL_SK_MAPREDUCE) ? c->d_result : static_cast<void*>(a2);
   };
-  // Median of `reps` launches of every variant in `vs`, INTERLEAVED (rep-major): clock and power state drift
-  // during a tuning run (sw_power_cap), and timing one variant after the other mis-ranks near-equal ones.
+  // Mean of the middle half of `reps` launches (the lowest and the highest quarter are dropped) of every variant in
+  // `vs`, INTERLEAVED (rep-major): clock and power state drift during a tuning run (sw_power_cap), and timing one
+  // variant after the other mis-ranks near-equal ones. Not the median: CUDA event timestamps tick in steps of about
+  // 2 us on this driver, so a median of single launches is quantised to that step (4 % of a 47 us Reduce, more than
+  // the differences the plan is about), while the phase of a launch against the tick is random and a mean resolves it.
   std::vector<std::vector<float>> tsamp;
   auto time_variants = [&](Call k, const std::vector<int>& vs, std::vector<float>& med_us) -> bool {
     tsamp.assign(vs.size(), std::vector<float>());
@@ -1992,7 +2018,10 @@ skel_status skel_tune_instance(skel_ctx* c, const skel_instance* inst, int log2_
     med_us.resize(vs.size());
     for (size_t j = 0; j < vs.size(); ++j) {
       std::sort(tsamp[j].begin(), tsamp[j].end());
-      med_us[j] = tsamp[j][reps / 2];
+      const int lo = reps / 4, hi = reps - reps / 4;
+      float sum = 0.f;
+      for (int r = lo; r < hi; ++r) sum += tsamp[j][r];
+      med_us[j] = sum / float(hi - lo);
     }
     return true;
   };

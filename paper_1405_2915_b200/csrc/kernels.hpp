@@ -20,7 +20,9 @@ struct Launch {
 
 struct Scratch {       // device scratch owned by the context (see api.cu)
   void* partials;      // >= MAX_PARTIALS 8-byte slots (reduce partials, scan block sums)
-  unsigned* ticket;    // reduce: atomicInc ticket (self-resetting)
+  unsigned* ticket;    // reduce: atomicInc ticket (self-resetting); +2: packed word of the iatom end; +4: start-order ticket of the tagged end
+  unsigned long long* red_tagged = nullptr;  // reduce, "*_tag" variants: MAX_PARTIALS + 8 (partial bits, launch number) slots (per block, then the 8 second-level ones), zero-initialised
+  mutable uint32_t red_epoch = 0;            // launch number of the last tagged Reduce (host side)
   unsigned* scan_ticket;        // scan: dynamic tile id counter (reset by the last tile)
   unsigned long long* scan_state;  // scan: per-tile (epoch|status|value) words, zero-initialised
   size_t scan_state_tiles;      // capacity of scan_state in tiles
@@ -49,7 +51,9 @@ const char* reduce_variant_name(int v);
 bool reduce_variant_ok(int v, const void* in0, const void* in1, size_t n);
 cudaError_t launch_mapreduce(const Launch& L, const Scratch& S, int v, int dtype, int map_fn, bool has_in1,
                              int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n,
-                             void* result /* device, one element */);
+                             void* result /* device, one element */,
+                             bool reverse = false /* chunk variants: walk the operands from the end to the front (same
+                                                     result bits; api.cu uses it to meet what the previous launch left in L2) */);
 
 // ---- row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] (reduce.cu) ----------------
 int reduce_rows_variant_count();

@@ -18,6 +18,13 @@
 // are 16 384 same-address atomics per launch, and their rate depends on where the scratch word lands (45.4 us in one
 // process, 55.6 us in bench.py, against 47.5 us for the fold). Every other case (max, mult, fp32) takes the ordinary
 // fold inside these variants.
+// The "*_tag" variants keep the iatom end for an int32 ADD and end every other case WITHOUT a fence and without a
+// wait: a block stores (partial bits, launch number) as ONE 64-bit relaxed.gpu word into its slot of a dedicated array
+// (never cleared: the launch number never repeats within 2^32 launches) and exits. The ticket is drawn at the START of
+// a block instead (its latency hides under the loads): the 8 blocks that STARTED last fold, each polling its eighth of
+// the slots for this launch's number, and the very last one folds their 8 sub-totals (fold_tagged); every block they
+// wait for is running or done or will start (8 waiting blocks never fill an SM), so the wait cannot deadlock. The fold
+// order depends on (n, variant) only, like the ticket fold: bitwise deterministic.
 #include "common.cuh"
 #include "kernels.hpp"
 #include <string.h>
@@ -37,21 +44,88 @@ __device__ __forceinline__ void fold_partials(const T* partials, unsigned count,
   if (threadIdx.x == 0) *result = acc;
 }
 
-enum : int { END_PARTIALS = 0, END_FOLD = 1, END_ATOMIC = 2 };
+enum : int { END_PARTIALS = 0, END_FOLD = 1, END_ATOMIC = 2, END_TAGGED = 3 };
 
+// END_TAGGED: 128-bit relaxed.gpu load of two (partial bits, launch number) slots
+__device__ __forceinline__ void ld_tagged2(const unsigned long long* p, unsigned long long& w0, unsigned long long& w1) {
+  asm volatile("{\n.reg .b128 t;\nld.relaxed.gpu.global.b128 t, [%2];\nmov.b128 {%0, %1}, t;\n}"
+               : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+}
+
+// The end of END_TAGGED in two levels. The TAG_P blocks that STARTED last are the pollers: poller j waits for the slots
+// j S .. j S + S - 1 (S = slots per poller, fixed by the grid) to carry this launch's number, folds them in index order
+// (thread t takes the slot pairs t, t + 256, ...; then the block tree) and publishes the sub-total the same way in the
+// second-level slot j; the block that started LAST also waits for the TAG_P second-level slots and folds them in index
+// order. A thread has one 128-bit load in flight per step (a poller reads at most 1024 slots at the usual grids), so the
+// kernel keeps the 32 registers of the streaming loop. Every block stores its own slot BEFORE it waits and at most TAG_P
+// = 8 blocks wait, never more than one SM holds (__launch_bounds__(256, 8)): the waits cannot deadlock. Grouping and
+// order depend on (gridDim) only: the same bits on every run.
+constexpr unsigned TAG_P = 8;
+
+template <typename T, int OP>
+__device__ __forceinline__ void fold_tagged(unsigned long long* tagged, unsigned count, unsigned order, uint32_t epoch,
+                                            T* result, T* smem) {
+  unsigned long long* level2 = tagged + MAX_PARTIALS;  // TAG_P slots behind the per-block slots
+  const unsigned P = count < TAG_P ? count : TAG_P;
+  const unsigned j = order - (count - P);                      // this poller's index, 0 .. P - 1
+  const unsigned per = (((count + P - 1) / P) + 1) & ~1u;      // slots per poller, even: a pair never straddles two pollers
+  const unsigned lo = j * per;
+  const unsigned hi = lo + per < count ? lo + per : count;
+  T acc = identity<T, OP>();
+  for (unsigned s0 = lo + 2 * threadIdx.x; s0 < hi; s0 += 2 * RED_THREADS) {
+    unsigned long long w0, w1;
+    bool ok;
+    do {
+      ld_tagged2(tagged + s0, w0, w1);
+      ok = uint32_t(w0 >> 32) == epoch && (s0 + 1 >= hi || uint32_t(w1 >> 32) == epoch);
+    } while (!ok);
+    acc = apply_fn<OP>(T(0), acc, from_bits<T>(uint32_t(w0)));
+    if (s0 + 1 < hi) acc = apply_fn<OP>(T(0), acc, from_bits<T>(uint32_t(w1)));
+  }
+  __syncthreads();  // smem reuse
+  acc = block_reduce<T, OP>(acc, smem);
+  if (threadIdx.x == 0) {
+    const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)to_bits(acc);
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(level2 + j), "l"(w) : "memory");
+  }
+  if (order != count - 1 || threadIdx.x >= 32) return;
+  // the block that started last: second level, lanes 0 .. P - 1 of warp 0
+  T v = identity<T, OP>();
+  if (threadIdx.x < P) {
+    unsigned long long w;
+    do {
+      asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w) : "l"(level2 + threadIdx.x) : "memory");
+    } while (uint32_t(w >> 32) != epoch);
+    v = from_bits<T>(uint32_t(w));
+  }
+  v = warp_reduce<T, OP>(v);
+  if (threadIdx.x == 0) *result = v;
+}
+
+// END_TAGGED: 8 blocks per SM = at most 32 registers, what the streaming loop needs; the fold of the one folder block
+// may spill (it is one block per launch), the other 8191 keep full occupancy
 template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U, int END>
-__global__ void __launch_bounds__(RED_THREADS)
+__global__ void __launch_bounds__(RED_THREADS, END == END_TAGGED ? 8 : 1)
 mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigned* ticket, T* result,
-                 unsigned tiles_per_block /* 0: strided walk of a persistent grid; k: block b owns tiles b k .. b k + k - 1 */) {
+                 unsigned tiles_per_block /* 0: strided walk of a persistent grid; k: block b owns tiles b k .. b k + k - 1 */,
+                 unsigned reverse /* chunk variants: the blocks take the chunks from the last one down (see launch_mapreduce) */,
+                 unsigned long long* tagged = nullptr, uint32_t epoch = 0) {
   __shared__ T smem[32];
   __shared__ bool is_last;
+  __shared__ unsigned s_order;
+  unsigned order = 0;  // END_TAGGED, thread 0: this block's place in the order in which the blocks STARTED
+  if constexpr (END == END_TAGGED) {
+    if (threadIdx.x == 0 && gridDim.x > 1) order = atomicInc(ticket + 4, gridDim.x - 1);  // wraps to 0: self-resetting
+  }
   constexpr size_t TILE = size_t(RED_THREADS) * V * U;
   const size_t ntiles = (n + TILE - 1) / TILE;
   T acc[V];
 #pragma unroll
   for (int j = 0; j < V; ++j) acc[j] = identity<T, OP>();
 
-  const size_t first = tiles_per_block ? size_t(blockIdx.x) * tiles_per_block : blockIdx.x;
+  // the chunk this block owns (= its partial's slot: the fold order does not depend on the direction)
+  const unsigned chunk = (reverse && tiles_per_block) ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+  const size_t first = tiles_per_block ? size_t(chunk) * tiles_per_block : blockIdx.x;
   const size_t step = tiles_per_block ? 1 : gridDim.x;
   const size_t last = tiles_per_block ? (first + tiles_per_block < ntiles ? first + tiles_per_block : ntiles) : ntiles;
   for (size_t tile = first; tile < last; tile += step) {
@@ -101,13 +175,27 @@ mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigne
         }
       }
     }
+  } else if constexpr (END == END_TAGGED) {
+    if (gridDim.x == 1) {
+      if (threadIdx.x == 0) *result = v;
+      return;
+    }
+    if (threadIdx.x == 0) {
+      // partial and launch number in ONE 64-bit store: no fence, nothing to wait for
+      const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)to_bits(v);
+      asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(tagged + chunk), "l"(w) : "memory");
+      s_order = order;
+    }
+    __syncthreads();
+    const unsigned ord = s_order;
+    if (ord + TAG_P >= gridDim.x) fold_tagged<T, OP>(tagged, gridDim.x, ord, epoch, result, smem);
   } else if constexpr (END == END_FOLD) {
     if (gridDim.x == 1) {
       if (threadIdx.x == 0) *result = v;
       return;
     }
     if (threadIdx.x == 0) {
-      partials[blockIdx.x] = v;
+      partials[chunk] = v;
       __threadfence();
       const unsigned t = atomicInc(ticket, gridDim.x - 1);  // wraps back to 0 on the last arrival
       is_last = (t == gridDim.x - 1);
@@ -118,7 +206,7 @@ mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigne
       fold_partials<T, OP>(partials, gridDim.x, result, smem);
     }
   } else {
-    if (threadIdx.x == 0) partials[blockIdx.x] = v;
+    if (threadIdx.x == 0) partials[chunk] = v;
   }
 }
 
@@ -128,7 +216,7 @@ __global__ void __launch_bounds__(RED_THREADS) fold_kernel(const T* partials, un
   fold_partials<T, OP>(partials, count, result, smem);
 }
 
-struct RedVariant { const char* name; int v, u; bool single; int blocks_per_sm; unsigned chunk_bytes = 0; bool iatom = false; };
+struct RedVariant { const char* name; int v, u; bool single; int blocks_per_sm; unsigned chunk_bytes = 0; bool iatom = false; bool tagged = false; };
 const RedVariant kRedVariants[] = {
     {"scalar_single_pass", 1, 4, true, 8},
     {"v4_u4_single_pass", 4, 4, true, 8},
@@ -142,6 +230,8 @@ const RedVariant kRedVariants[] = {
     {"v8_u2_chunk64k", 8, 2, true, 0, 65536},
     {"v4_u4_chunk32k_iatom", 4, 4, true, 0, 32768, true},
     {"v4_u4_chunk64k_iatom", 4, 4, true, 0, 65536, true},
+    {"v4_u4_chunk32k_tag", 4, 4, true, 0, 32768, true, true},
+    {"v4_u4_chunk64k_tag", 4, 4, true, 0, 65536, true, true},
 };
 constexpr int kNumRedVariants = sizeof(kRedVariants) / sizeof(kRedVariants[0]);
 
@@ -149,7 +239,7 @@ inline bool aligned_to(const void* p, size_t a) { return p == nullptr || (reinte
 
 template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U>
 cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, const T* in0, const T* in1, T c,
-                       size_t n, T* result) {
+                       size_t n, T* result, unsigned rev) {
   constexpr size_t TILE = size_t(RED_THREADS) * V * U;
   size_t ntiles = (n + TILE - 1) / TILE;
   size_t grid = size_t(L.sms) * rv.blocks_per_sm;
@@ -168,18 +258,31 @@ cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, 
   if constexpr (std::is_same<T, int32_t>::value && OP == FN_ADD && V == 4) {
     if (rv.iatom) {
       mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, END_ATOMIC>
-          <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
+          <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb, rev);
+      ++*L.launches;
+      return cudaGetLastError();
+    }
+  }
+  if constexpr (V == 4) {
+    if (rv.tagged) {
+      if (++S.red_epoch == 0) {  // 2^32 launches: start over from cleared slots
+        cudaError_t e = cudaMemsetAsync(S.red_tagged, 0, size_t(MAX_PARTIALS + 8) * 8, L.stream);
+        if (e != cudaSuccess) return e;
+        S.red_epoch = 1;
+      }
+      mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, END_TAGGED>
+          <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb, rev, S.red_tagged, S.red_epoch);
       ++*L.launches;
       return cudaGetLastError();
     }
   }
   if (rv.single) {
     mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, END_FOLD>
-        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb, rev);
     ++*L.launches;
   } else {
     mapreduce_kernel<T, MAPF, HAS_IN1, OP, V, U, END_PARTIALS>
-        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb);
+        <<<(unsigned)grid, RED_THREADS, 0, L.stream>>>(in0, in1, c, n, partials, S.ticket, result, tpb, rev);
     fold_kernel<T, OP><<<1, RED_THREADS, 0, L.stream>>>(partials, (unsigned)grid, result);
     *L.launches += 2;
   }
@@ -188,36 +291,36 @@ cudaError_t launch_one(const Launch& L, const Scratch& S, const RedVariant& rv, 
 
 template <typename T, int MAPF, bool HAS_IN1, int OP>
 cudaError_t launch_vu(const Launch& L, const Scratch& S, const RedVariant& rv, const T* in0, const T* in1, T c,
-                      size_t n, T* result) {
-  if (rv.v == 1) return launch_one<T, MAPF, HAS_IN1, OP, 1, 4>(L, S, rv, in0, in1, c, n, result);
-  if (rv.v == 4) return launch_one<T, MAPF, HAS_IN1, OP, 4, 4>(L, S, rv, in0, in1, c, n, result);
-  return launch_one<T, MAPF, HAS_IN1, OP, 8, 2>(L, S, rv, in0, in1, c, n, result);
+                      size_t n, T* result, unsigned rev) {
+  if (rv.v == 1) return launch_one<T, MAPF, HAS_IN1, OP, 1, 4>(L, S, rv, in0, in1, c, n, result, rev);
+  if (rv.v == 4) return launch_one<T, MAPF, HAS_IN1, OP, 4, 4>(L, S, rv, in0, in1, c, n, result, rev);
+  return launch_one<T, MAPF, HAS_IN1, OP, 8, 2>(L, S, rv, in0, in1, c, n, result, rev);
 }
 
 template <typename T, int MAPF, bool HAS_IN1>
 cudaError_t launch_op(const Launch& L, const Scratch& S, const RedVariant& rv, int op, const T* in0, const T* in1,
-                      T c, size_t n, T* result) {
+                      T c, size_t n, T* result, unsigned rev) {
   switch (op) {
-    case FN_ADD: return launch_vu<T, MAPF, HAS_IN1, FN_ADD>(L, S, rv, in0, in1, c, n, result);
-    case FN_MULT: return launch_vu<T, MAPF, HAS_IN1, FN_MULT>(L, S, rv, in0, in1, c, n, result);
-    case FN_MAX: return launch_vu<T, MAPF, HAS_IN1, FN_MAX>(L, S, rv, in0, in1, c, n, result);
+    case FN_ADD: return launch_vu<T, MAPF, HAS_IN1, FN_ADD>(L, S, rv, in0, in1, c, n, result, rev);
+    case FN_MULT: return launch_vu<T, MAPF, HAS_IN1, FN_MULT>(L, S, rv, in0, in1, c, n, result, rev);
+    case FN_MAX: return launch_vu<T, MAPF, HAS_IN1, FN_MAX>(L, S, rv, in0, in1, c, n, result, rev);
   }
   return cudaErrorInvalidValue;
 }
 
 template <typename T>
 cudaError_t launch_t(const Launch& L, const Scratch& S, const RedVariant& rv, int map_fn, bool has_in1, int op,
-                     T c, const T* in0, const T* in1, size_t n, T* result) {
+                     T c, const T* in0, const T* in1, size_t n, T* result, unsigned rev) {
 #define SKEL_MR_CASE(F)                                                                   \
   case F:                                                                                 \
-    return has_in1 ? launch_op<T, F, true>(L, S, rv, op, in0, in1, c, n, result)          \
-                   : launch_op<T, F, false>(L, S, rv, op, in0, in1, c, n, result);
+    return has_in1 ? launch_op<T, F, true>(L, S, rv, op, in0, in1, c, n, result, rev)     \
+                   : launch_op<T, F, false>(L, S, rv, op, in0, in1, c, n, result, rev);
   switch (map_fn) {
-    case FN_IDENT: return launch_op<T, FN_IDENT, false>(L, S, rv, op, in0, in1, c, n, result);
+    case FN_IDENT: return launch_op<T, FN_IDENT, false>(L, S, rv, op, in0, in1, c, n, result, rev);
     SKEL_MR_CASE(FN_ADD)
     SKEL_MR_CASE(FN_MULT)
     SKEL_MR_CASE(FN_MAX)
-    case FN_SAXPY: return launch_op<T, FN_SAXPY, true>(L, S, rv, op, in0, in1, c, n, result);
+    case FN_SAXPY: return launch_op<T, FN_SAXPY, true>(L, S, rv, op, in0, in1, c, n, result, rev);
   }
 #undef SKEL_MR_CASE
   return cudaErrorInvalidValue;
@@ -225,7 +328,8 @@ cudaError_t launch_t(const Launch& L, const Scratch& S, const RedVariant& rv, in
 
 // ---- row-wise Reduce on a matrix: out[i] = in[i][0] (+) ... (+) in[i][cols-1] --------
 // "warp_*": one warp per row (8 rows per block): a lane folds its V-wide vectors into 4 x V independent chains
-// (4 vectors in flight), then a fixed shuffle tree; "block_v4": 256 threads per row (long rows, few of them).
+// (4 vectors in flight), then a fixed shuffle tree; "block_v4": 256 threads per row (long rows, few of them), 16 x 148
+// persistent blocks; "block_v4_row": the same kernel with one block per row.
 // The combination order depends only on (cols, variant): deterministic run to run.
 template <typename T, int OP, int V>
 __device__ __forceinline__ T fold_row_part(const T* row, size_t cols, int t, int nt) {
@@ -286,13 +390,16 @@ reduce_rows_block_kernel(const T* in, size_t rows, size_t cols, T* out) {
   }
 }
 
-const char* const kRowNames[] = {"warp_scalar", "warp_v4", "block_v4"};
-constexpr int kNumRowVariants = 3;
+const char* const kRowNames[] = {"warp_scalar", "warp_v4", "block_v4", "block_v4_row"};
+constexpr int kNumRowVariants = 4;
 
 template <typename T, int OP>
 cudaError_t launch_rows_op(const Launch& L, int v, const T* in, size_t rows, size_t cols, T* out) {
   const size_t cap = size_t(L.sms) * 16;
-  if (v == 2) {
+  if (v == 3) {  // one block per row: the hardware block scheduler balances the SMs (like Reduce's chunk variants)
+    const unsigned grid = (unsigned)(rows < 0x7fffffffu ? rows : 0x7fffffffu);
+    reduce_rows_block_kernel<T, OP, 4><<<grid, RED_THREADS, 0, L.stream>>>(in, rows, cols, out);
+  } else if (v == 2) {
     const unsigned grid = (unsigned)(rows < cap ? rows : cap);
     reduce_rows_block_kernel<T, OP, 4><<<grid, RED_THREADS, 0, L.stream>>>(in, rows, cols, out);
   } else {
@@ -342,17 +449,19 @@ bool reduce_variant_ok(int v, const void* in0, const void* in1, size_t) {
 }
 
 cudaError_t launch_mapreduce(const Launch& L, const Scratch& S, int v, int dtype, int map_fn, bool has_in1,
-                             int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n, void* result) {
+                             int red_op, uint32_t cbits, const void* in0, const void* in1, size_t n, void* result,
+                             bool reverse) {
   const RedVariant& rv = kRedVariants[v];
+  const unsigned rev = reverse ? 1u : 0u;
   if (dtype == DT_F32) {
     float c;
     memcpy(&c, &cbits, 4);
     return launch_t<float>(L, S, rv, map_fn, has_in1, red_op, c, static_cast<const float*>(in0),
-                           static_cast<const float*>(in1), n, static_cast<float*>(result));
+                           static_cast<const float*>(in1), n, static_cast<float*>(result), rev);
   }
   return launch_t<int32_t>(L, S, rv, map_fn, has_in1, red_op, static_cast<int32_t>(cbits),
                            static_cast<const int32_t*>(in0), static_cast<const int32_t*>(in1), n,
-                           static_cast<int32_t*>(result));
+                           static_cast<int32_t*>(result), rev);
 }
 
 }  // namespace skel

@@ -54,7 +54,7 @@ def main():
     ap.add_argument("--out", default=os.path.join(HERE, "plans", "b200.plan"))
     ap.add_argument("--reps", type=int, default=11)
     ap.add_argument("--tables", default=None, help="write the timing tables as JSON here")
-    ap.add_argument("--only", default=None, help="tune only the instances whose name contains this substring")
+    ap.add_argument("--only", default=None, help="tune only the instances whose name contains this substring (several: comma-separated)")
     ap.add_argument("--base", default=None, help="start from this plan file (instances not tuned keep their entries)")
     args = ap.parse_args()
     sys.path.insert(0, os.path.dirname(HERE))
@@ -65,7 +65,7 @@ def main():
         ctx.plan_load(args.base)
     tables = {}
     for name, inst, lo, hi, cols in instances(S):
-        if args.only and args.only not in name:
+        if args.only and not any(part and part in name for part in args.only.split(",")):
             continue
         t = ctx.tune(inst, lo, hi, cols, args.reps)
         names = S.variant_names(inst.skeleton)
@@ -76,6 +76,11 @@ def main():
                 continue
             best = min((x, i) for i, x in enumerate(row) if x == x)[1]
             print(f"  2^{lo + k:2d}  " + " ".join(f"{x:9.1f}" for x in row) + f"   -> {best}")
+    # a partial re-tune (--only with --base) keeps the provenance lines of the plan it started from below its own
+    # (read before the plan is saved: --out may be the same file as --base)
+    earlier = ""
+    if args.base and os.path.exists(args.base):
+        earlier = "".join(ln for ln in open(args.base) if ln.startswith("#"))
     os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
     ctx.plan_save(args.out)
     # provenance: '#' lines are comments for the loader
@@ -85,10 +90,6 @@ def main():
     cmd = "python -m paper_1405_2915_b200.tune " + " ".join(sys.argv[1:])
     note = (f"# generated by: {cmd.strip()}  (skel_tune_instance, reps={args.reps}; {torch.cuda.get_device_name(0)}, "
             f"{datetime.datetime.now(datetime.timezone.utc).strftime('%Y-%m-%d %H:%M UTC')}); not edited by hand\n")
-    # a partial re-tune (--only with --base) keeps the provenance lines of the plan it started from below its own
-    earlier = ""
-    if args.base and os.path.exists(args.base):
-        earlier = "".join(ln for ln in open(args.base) if ln.startswith("#"))
     with open(args.out, "w") as f:
         f.write(note + earlier + body)
     if args.tables:

@@ -193,6 +193,82 @@ def test_reduce_i32_atomic_end_chain_resets_its_scratch_word(ctx):
         c.destroy()
 
 
+def test_reduce_tagged_end_across_launches(ctx):
+    """The *_tag variants end a max / mult / fp32 Reduce with one (partial, launch number) word per block and a fold by
+    the block that STARTED last; the slots are never cleared. Launches of different sizes (odd and even block counts,
+    more and fewer blocks than the launch before, so stale slots of earlier launches sit beside fresh ones), operators
+    and element types, back to back: exact for int32, fp32 inside the tolerance and bitwise equal run to run."""
+    names = S.variant_names(S.SK_REDUCE)
+    tagged = [i for i, nm in enumerate(names) if nm.endswith("_tag")]
+    assert tagged
+    sizes = [(1 << 23) + 1, 8192 * 3, (1 << 22) + 4097, 8193, 1 << 21, 100003, (1 << 20) + 5, 3 * 8192 + 1, 1 << 24]
+    data = {n: I.full_range_i32(250 + n, n) for n in sizes}
+    vecs = {n: ctx.vector_from(a) for n, a in data.items()}
+    xf = I.uniform_pm1_f32(251, (1 << 22) + 12345)
+    vf, vg = ctx.vector_from(xf), ctx.vector_from(xf[::-1].copy())
+    reff, abf = O.reduce_f32(O.FN_ADD, xf)
+    dref, dabs = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, xf, xf[::-1].copy())
+    for v in tagged:
+        with forced(ctx, S.SK_REDUCE, v), forced(ctx, S.SK_MAPREDUCE, v):
+            first = None
+            for rep in range(4):
+                for n in sizes if rep % 2 == 0 else reversed(sizes):
+                    assert ctx.reduce(S.FN_MAX, vecs[n]) == O.reduce_i32(O.FN_MAX, data[n])[0], (names[v], n)
+                    if n % 2 == 1:
+                        assert ctx.reduce(S.FN_ADD, vecs[n]) == O.reduce_i32(O.FN_ADD, data[n])[0]
+                        got = ctx.reduce(S.FN_ADD, vf)
+                        assert_reduce_f32(got, reff, abf)
+                        first = got if first is None else first
+                        assert got == first
+                    if n % 3 == 0:
+                        assert ctx.reduce(S.FN_MAX, vf) == O.reduce_f32(O.FN_MAX, xf)[0]
+                        d = ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, vf, vg)
+                        assert abs(d - dref) <= 1e-5 * dabs
+            # many launches in a row without a host read in between: futures resolved at the end
+            outs = [ctx.vector(1, S.I32) for _ in range(64)]
+            for k, o in enumerate(outs):
+                ctx.reduce_to(S.FN_MAX, vecs[sizes[k % len(sizes)]], o)
+            for k, o in enumerate(outs):
+                assert int(o.numpy()[0]) == O.reduce_i32(O.FN_MAX, data[sizes[k % len(sizes)]])[0]
+                o.destroy()
+    for c in list(vecs.values()) + [vf, vg]:
+        c.destroy()
+
+
+def test_reduce_l2_aware_direction_keeps_the_bits(ctx):
+    """skel_ctx_set_l2_reuse: a Reduce / MapReduce that follows a launch on the same operand walks it from the end to
+    the front. Every chunk variant, sizes with a ragged last chunk and odd chunk counts: int32 exact, and the fp32 sum
+    and dot product have the SAME BITS with the setting on (directions alternate call by call) and off (all forward)."""
+    names = S.variant_names(S.SK_REDUCE)
+    chunked = [i for i, nm in enumerate(names) if "chunk" in nm]
+    sizes = [(1 << 22) + 4097, 8192 * 3 + 1, (1 << 24) + 5, 100003]
+    for n in sizes:
+        a = I.full_range_i32(260 + n, n)
+        x, y = I.uniform_pm1_f32(261 + n, n), I.uniform_pm1_f32(262 + n, n)
+        va, vx, vy = ctx.vector_from(a), ctx.vector_from(x), ctx.vector_from(y)
+        ref_add, ref_max = O.reduce_i32(O.FN_ADD, a)[0], O.reduce_i32(O.FN_MAX, a)[0]
+        rf, af = O.reduce_f32(O.FN_ADD, x)
+        rd, ad = O.mapreduce_f32(O.FN_MULT, O.FN_ADD, 0.0, x, y)
+        for v in chunked:
+            with forced(ctx, S.SK_REDUCE, v), forced(ctx, S.SK_MAPREDUCE, v):
+                got = {}
+                for on in (False, True):
+                    ctx.set_l2_reuse(on)
+                    for _ in range(3):  # forward, backward, forward when on
+                        assert ctx.reduce(S.FN_ADD, va) == ref_add, (names[v], n, on)
+                        assert ctx.reduce(S.FN_MAX, va) == ref_max, (names[v], n, on)
+                    fs = [ctx.reduce(S.FN_ADD, vx) for _ in range(3)]
+                    ds = [ctx.mapreduce(S.FN_MULT, S.FN_ADD, 0.0, vx, vy) for _ in range(3)]
+                    assert_reduce_f32(fs[0], rf, af)
+                    assert abs(ds[0] - rd) <= 1e-5 * ad
+                    assert fs[0] == fs[1] == fs[2] and ds[0] == ds[1] == ds[2]
+                    got[on] = (fs[0], ds[0])
+                assert got[False] == got[True], (names[v], n)
+        ctx.set_l2_reuse(True)
+        for c in (va, vx, vy):
+            c.destroy()
+
+
 def test_reduce_closed_forms_and_max_position(ctx):
     for n in [1, 1000, 4096, (1 << 20) + 3]:
         v = ctx.vector_from(np.ones(n, np.float32))

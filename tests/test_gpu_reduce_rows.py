@@ -22,10 +22,10 @@ def ctx():
     c.close()
 
 
-@pytest.mark.parametrize("v", [0, 1, 2])
+@pytest.mark.parametrize("v", [0, 1, 2, 3])
 def test_reduce_rows_matches_oracle(ctx, v):
     names = S.variant_names(S.SK_REDUCE_ROWS)
-    assert names == ["warp_scalar", "warp_v4", "block_v4"]
+    assert names == ["warp_scalar", "warp_v4", "block_v4", "block_v4_row"]
     for rows, cols in SHAPES:
         X = I.uniform_pm1_f32(800 + rows, rows * cols).reshape(rows, cols)
         Xi = (I.raw_u64(801 + rows, rows * cols) % np.uint64(1 << 31)).astype(np.int32).reshape(rows, cols)
