@@ -102,10 +102,11 @@ __device__ __forceinline__ void fold_tagged(unsigned long long* tagged, unsigned
   if (threadIdx.x == 0) *result = v;
 }
 
-// END_TAGGED: 8 blocks per SM = at most 32 registers, what the streaming loop needs; the fold of the one folder block
-// may spill (it is one block per launch), the other 8191 keep full occupancy
+// 8 blocks per SM = at most 32 registers, what the streaming loop of the 128-bit forms needs (2048 resident threads:
+// the bytes in flight are what a 268 MB Reduce lives on; at 40 registers the int32 max fold lost 25 % of its warps and
+// 0.8 us). Asked for where it costs no spill in the loop: one-operand V = 4 kernels and the tagged end.
 template <typename T, int MAPF, bool HAS_IN1, int OP, int V, int U, int END>
-__global__ void __launch_bounds__(RED_THREADS, END == END_TAGGED ? 8 : 1)
+__global__ void __launch_bounds__(RED_THREADS, ((V == 4 && !HAS_IN1) || END == END_TAGGED) ? 8 : 1)
 mapreduce_kernel(const T* in0, const T* in1, T c, size_t n, T* partials, unsigned* ticket, T* result,
                  unsigned tiles_per_block /* 0: strided walk of a persistent grid; k: block b owns tiles b k .. b k + k - 1 */,
                  unsigned reverse /* chunk variants: the blocks take the chunks from the last one down (see launch_mapreduce) */,
