@@ -208,4 +208,63 @@ template <typename T, int OP> __device__ __forceinline__ T block_reduce(T v, T* 
   return v;
 }
 
+// ---- the tagged end of the reducing kernels (reduce.cu END_TAGGED, fused.cu) ----------------------------------------
+// 128-bit relaxed.gpu load of two (partial bits, launch number) slots
+__device__ __forceinline__ void ld_tagged2(const unsigned long long* p, unsigned long long& w0, unsigned long long& w1) {
+  asm volatile("{\n.reg .b128 t;\nld.relaxed.gpu.global.b128 t, [%2];\nmov.b128 {%0, %1}, t;\n}"
+               : "=l"(w0), "=l"(w1) : "l"(p) : "memory");
+}
+
+// The end of END_TAGGED in two levels. The TAG_P blocks that STARTED last are the pollers: poller j waits for the slots
+// j S .. j S + S - 1 (S = slots per poller, fixed by the grid) to carry this launch's number, folds them in index order
+// (thread t takes the slot pairs t, t + NT, ...; then the block tree) and publishes the sub-total the same way in the
+// second-level slot j; the block that started LAST also waits for the TAG_P second-level slots and folds them in index
+// order. A thread has one 128-bit load in flight per step (a poller reads at most 1024 slots at the usual grids), so the
+// kernel keeps the 32 registers of the streaming loop. Every block stores its own slot BEFORE it waits and at most TAG_P
+// = 8 blocks wait, fewer than the device holds at once (reduce.cu: 8 per SM by __launch_bounds__(256, 8); fused.cu: 3 or
+// more per SM on 148 SMs), so a block that has not started yet always finds a slot: the waits cannot deadlock. Grouping
+// and order depend on (gridDim) only: the same bits on every run.
+constexpr unsigned TAG_P = 8;
+constexpr unsigned TAG_SLOTS = 8192;  // per-block slots (as many as Reduce partials, kernels.hpp); the TAG_P second-level slots follow them
+
+template <typename T, int OP, int NT /* threads per block */>
+__device__ __forceinline__ void fold_tagged(unsigned long long* tagged, unsigned count, unsigned order, uint32_t epoch,
+                                            T* result, T* smem) {
+  unsigned long long* level2 = tagged + TAG_SLOTS;  // TAG_P slots behind the per-block slots
+  const unsigned P = count < TAG_P ? count : TAG_P;
+  const unsigned j = order - (count - P);                      // this poller's index, 0 .. P - 1
+  const unsigned per = (((count + P - 1) / P) + 1) & ~1u;      // slots per poller, even: a pair never straddles two pollers
+  const unsigned lo = j * per;
+  const unsigned hi = lo + per < count ? lo + per : count;
+  T acc = identity<T, OP>();
+  for (unsigned s0 = lo + 2 * threadIdx.x; s0 < hi; s0 += 2 * NT) {
+    unsigned long long w0, w1;
+    bool ok;
+    do {
+      ld_tagged2(tagged + s0, w0, w1);
+      ok = uint32_t(w0 >> 32) == epoch && (s0 + 1 >= hi || uint32_t(w1 >> 32) == epoch);
+    } while (!ok);
+    acc = apply_fn<OP>(T(0), acc, from_bits<T>(uint32_t(w0)));
+    if (s0 + 1 < hi) acc = apply_fn<OP>(T(0), acc, from_bits<T>(uint32_t(w1)));
+  }
+  __syncthreads();  // smem reuse
+  acc = block_reduce<T, OP>(acc, smem);
+  if (threadIdx.x == 0) {
+    const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)to_bits(acc);
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(level2 + j), "l"(w) : "memory");
+  }
+  if (order != count - 1 || threadIdx.x >= 32) return;
+  // the block that started last: second level, lanes 0 .. P - 1 of warp 0
+  T v = identity<T, OP>();
+  if (threadIdx.x < P) {
+    unsigned long long w;
+    do {
+      asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w) : "l"(level2 + threadIdx.x) : "memory");
+    } while (uint32_t(w >> 32) != epoch);
+    v = from_bits<T>(uint32_t(w));
+  }
+  v = warp_reduce<T, OP>(v);
+  if (threadIdx.x == 0) *result = v;
+}
+
 }  // namespace skel

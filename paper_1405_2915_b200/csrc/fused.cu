@@ -55,13 +55,18 @@ __device__ __forceinline__ void fma2_into(float& lo, float& hi, float w, float x
 template <int R, int MAPF, int OP>
 __global__ void __launch_bounds__(FU_THREADS)
 fused_chain_kernel(const __grid_constant__ Weights1D W, int edge, float pad, float c, const float* in, float* map_out,
-                   float* ov_out, size_t n, float* partials, unsigned* ticket, float* result) {
+                   float* ov_out, size_t n, unsigned long long* tagged, unsigned* ticket, uint32_t epoch, float* result) {
   constexpr int O = 16;
   constexpr int TILE = FU_THREADS * O;
   constexpr int ROP = OP == OP_NONE ? FN_ADD : OP;  // only instantiates the helpers; unused when OP_NONE
   static_assert(R >= 1 && R <= O, "halo comes from the direct neighbours only");
   __shared__ float smem[32];
-  __shared__ bool is_last;
+  __shared__ unsigned s_order;
+  // tagged end (common.cuh): the ticket is drawn when the block STARTS; its latency hides under the loads
+  unsigned order = 0;
+  if constexpr (OP != OP_NONE) {
+    if (threadIdx.x == 0 && gridDim.x > 1) order = atomicInc(ticket + 4, gridDim.x - 1);  // wraps to 0: self-resetting
+  }
   const int lane = threadIdx.x & 31;
   const long long ln = static_cast<long long>(n);
   const size_t ntiles = (n + TILE - 1) / TILE;
@@ -153,21 +158,15 @@ fused_chain_kernel(const __grid_constant__ Weights1D W, int edge, float pad, flo
       if (threadIdx.x == 0) *result = v;
       return;
     }
-    if (threadIdx.x == 0) {
-      partials[blockIdx.x] = v;
-      __threadfence();
-      const unsigned t = atomicInc(ticket, gridDim.x - 1);  // wraps back to 0 on the last arrival
-      is_last = (t == gridDim.x - 1);
+    if (threadIdx.x == 0) {  // partial and launch number in ONE 64-bit store: no fence, nothing to wait for
+      const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)to_bits(v);
+      asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(tagged + blockIdx.x), "l"(w) : "memory");
+      s_order = order;
     }
     __syncthreads();
-    if (is_last) {  // fold the partials in a fixed order (run-to-run deterministic)
-      __threadfence();
-      float a = identity<float, ROP>();
-      for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) a = apply_fn<ROP>(0.f, a, partials[i]);
-      __syncthreads();
-      a = block_reduce<float, ROP>(a, smem);
-      if (threadIdx.x == 0) *result = a;
-    }
+    // the 8 blocks that started last fold the slots in a fixed order (run-to-run deterministic; common.cuh)
+    const unsigned ord = s_order;
+    if (ord + TAG_P >= gridDim.x) fold_tagged<float, ROP, FU_THREADS>(tagged, gridDim.x, ord, epoch, result, smem);
   }
 }
 
@@ -178,13 +177,18 @@ fused_chain_kernel(const __grid_constant__ Weights1D W, int edge, float pad, flo
 template <int R, int MAPF, int OP>
 __global__ void __launch_bounds__(FU_THREADS)
 fused_chain2_kernel(const __grid_constant__ Weights1D W, int edge, float pad, float c, const float* in, float* map_out,
-                    float* ov_out, size_t n, float* partials, unsigned* ticket, float* result) {
+                    float* ov_out, size_t n, unsigned long long* tagged, unsigned* ticket, uint32_t epoch, float* result) {
   constexpr int C = 8, TILE = FU_THREADS * 2 * C;
   constexpr int ROP = OP == OP_NONE ? FN_ADD : OP;
   static_assert(R >= 1 && R <= C, "halo comes from the direct neighbours only");
   constexpr unsigned FULLM = 0xffffffffu;
   __shared__ float smem[32];
-  __shared__ bool is_last;
+  __shared__ unsigned s_order;
+  // tagged end (common.cuh): the ticket is drawn when the block STARTS; its latency hides under the loads
+  unsigned order = 0;
+  if constexpr (OP != OP_NONE) {
+    if (threadIdx.x == 0 && gridDim.x > 1) order = atomicInc(ticket + 4, gridDim.x - 1);  // wraps to 0: self-resetting
+  }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const long long ln = static_cast<long long>(n);
   const size_t ntiles = (n + TILE - 1) / TILE;
@@ -299,21 +303,15 @@ fused_chain2_kernel(const __grid_constant__ Weights1D W, int edge, float pad, fl
       if (threadIdx.x == 0) *result = v;
       return;
     }
-    if (threadIdx.x == 0) {
-      partials[blockIdx.x] = v;
-      __threadfence();
-      const unsigned t = atomicInc(ticket, gridDim.x - 1);
-      is_last = (t == gridDim.x - 1);
+    if (threadIdx.x == 0) {  // partial and launch number in ONE 64-bit store: no fence, nothing to wait for
+      const unsigned long long w = ((unsigned long long)epoch << 32) | (unsigned long long)to_bits(v);
+      asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(tagged + blockIdx.x), "l"(w) : "memory");
+      s_order = order;
     }
     __syncthreads();
-    if (is_last) {
-      __threadfence();
-      float a = identity<float, ROP>();
-      for (unsigned i = threadIdx.x; i < gridDim.x; i += blockDim.x) a = apply_fn<ROP>(0.f, a, partials[i]);
-      __syncthreads();
-      a = block_reduce<float, ROP>(a, smem);
-      if (threadIdx.x == 0) *result = a;
-    }
+    // the 8 blocks that started last fold the slots in a fixed order (run-to-run deterministic; common.cuh)
+    const unsigned ord = s_order;
+    if (ord + TAG_P >= gridDim.x) fold_tagged<float, ROP, FU_THREADS>(tagged, gridDim.x, ord, epoch, result, smem);
   }
 }
 
@@ -324,12 +322,17 @@ cudaError_t launch_rmo(const Launch& L, const Scratch& S, const Weights1D& w, in
   size_t grid = (n + TILE - 1) / TILE;
   if (OP != OP_NONE && grid > MAX_PARTIALS) grid = MAX_PARTIALS;
   if (grid > 0x7fffffffu) grid = 0x7fffffffu;
+  if (OP != OP_NONE && ++S.red_epoch == 0) {  // 2^32 launches: start over from cleared slots (reduce.cu)
+    cudaError_t e = cudaMemsetAsync(S.red_tagged, 0, size_t(MAX_PARTIALS + 8) * 8, L.stream);
+    if (e != cudaSuccess) return e;
+    S.red_epoch = 1;
+  }
   if constexpr (R <= 8)  // warp-contiguous layout (fewer halo shuffles than loads saved only up to r = 8)
     fused_chain2_kernel<R, MAPF, OP><<<(unsigned)grid, FU_THREADS, 0, L.stream>>>(
-        w, edge, pad, c, in, map_out, ov_out, n, static_cast<float*>(S.partials), S.ticket, result);
+        w, edge, pad, c, in, map_out, ov_out, n, S.red_tagged, S.ticket, S.red_epoch, result);
   else
     fused_chain_kernel<R, MAPF, OP><<<(unsigned)grid, FU_THREADS, 0, L.stream>>>(
-        w, edge, pad, c, in, map_out, ov_out, n, static_cast<float*>(S.partials), S.ticket, result);
+        w, edge, pad, c, in, map_out, ov_out, n, S.red_tagged, S.ticket, S.red_epoch, result);
   ++*L.launches;
   return cudaGetLastError();
 }
