@@ -43,6 +43,9 @@ def instances(S):
     out.append(("overlap1d_cols_r8", I(skeleton=S.SK_OVERLAP1D_COL, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
     for r in (1, 2, 4):
         out.append((f"overlap2d_{2*r+1}x{2*r+1}", I(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.F32, r0=r, r1=r, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
+    # int32 containers (S:§8(f) f2): the same kernels on integer weights, IMAD instead of FFMA2
+    out.append(("overlap1d_r4_e1_i32", I(skeleton=S.SK_OVERLAP1D, fn=S.FN_WSTENCIL, dtype=S.I32, r0=4, edge=S.EDGE_DUPLICATE), 12, 26, 0))
+    out.append(("overlap2d_5x5_i32", I(skeleton=S.SK_OVERLAP2D, fn=S.FN_WSTENCIL, dtype=S.I32, r0=2, r1=2, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
     out.append(("reduce_rows_add_f32", I(skeleton=S.SK_REDUCE_ROWS, fn=S.FN_ADD, dtype=S.F32), 20, 26, 8192))
     out.append(("separable_r8", I(skeleton=S.SK_SEPARABLE, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, r1=8, edge=S.EDGE_DUPLICATE), 20, 26, 8192))
     out.append(("separable_r8_const", I(skeleton=S.SK_SEPARABLE, fn=S.FN_WSTENCIL, dtype=S.F32, r0=8, r1=8, edge=S.EDGE_CONSTANT), 20, 26, 8192))
