@@ -24,7 +24,11 @@
 // a block instead (its latency hides under the loads): the 8 blocks that STARTED last fold, each polling its eighth of
 // the slots for this launch's number, and the very last one folds their 8 sub-totals (fold_tagged); every block they
 // wait for is running or done or will start (8 waiting blocks never fill an SM), so the wait cannot deadlock. The fold
-// order depends on (n, variant) only, like the ticket fold: bitwise deterministic.
+// order depends on (n, variant) only, like the ticket fold: bitwise deterministic. Measured on B200 at n = 2^26, back to
+// back in one process: int32 max 46.3 -> 44.1 us, fp32 dot 88.5 -> 86.4 us (common.cuh holds fold_tagged: fused.cu
+// ends its chain kernels the same way).
+// `reverse` (chunk variants): block b takes chunk G - 1 - b, so the operand is walked from its end to its front; the
+// partial's slot is the chunk's, so the result has the same bits (api.cu: L2-aware direction, skel_ctx_set_l2_reuse).
 #include "common.cuh"
 #include "kernels.hpp"
 #include <string.h>
