@@ -52,6 +52,13 @@ def instances(S):
     return out
 
 
+def selected(name: str, only: str | None) -> bool:
+    """--only: comma-separated substrings; an instance is tuned when its name contains one of them (all when unset)."""
+    if not only:
+        return True
+    return any(part and part in name for part in only.split(","))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--out", default=os.path.join(HERE, "plans", "b200.plan"))
@@ -68,7 +75,7 @@ def main():
         ctx.plan_load(args.base)
     tables = {}
     for name, inst, lo, hi, cols in instances(S):
-        if args.only and not any(part and part in name for part in args.only.split(",")):
+        if not selected(name, args.only):
             continue
         t = ctx.tune(inst, lo, hi, cols, args.reps)
         names = S.variant_names(inst.skeleton)

@@ -308,3 +308,25 @@ def test_shipped_plan_is_consistent_with_the_variant_tables():
         assert ctx.plan_lookup(inst, 1 << 28) == variants[-1]
         seen += 1
     assert seen >= 20
+
+
+def test_tuner_instance_selection_and_plan_coverage():
+    """tune.py: --only takes comma-separated substrings; every instance the tuner knows (the bench instances and the
+    neighbours of the dispatch tree) has its own entry in the shipped plan, found by an exact look-up."""
+    import os
+
+    from paper_1405_2915_b200 import tune
+
+    assert tune.selected("reduce_max_i32", None) and tune.selected("reduce_max_i32", "")
+    assert tune.selected("reduce_max_i32", "reduce_,dot") and tune.selected("dot_f32", "reduce_,dot")
+    assert not tune.selected("scan_add_i32_incl", "reduce_,dot") and not tune.selected("dot_f32", "reduce_,")
+    names = [name for name, *_ in tune.instances(S)]
+    assert len(names) == len(set(names)) and "overlap2d_5x5_i32" in names and "overlap1d_r4_e1_i32" in names
+    path = os.path.join(os.path.dirname(os.path.abspath(S.__file__)), "plans", "b200.plan")
+    ctx = S.Context(lazy_cuda=True)
+    ctx.plan_load(path)
+    for name, inst, lo, hi, cols in tune.instances(S):
+        v, exact, from_plan = ctx.plan_explain(inst, 1 << hi)
+        assert exact and from_plan, name
+        assert 0 <= v < S.lib.skel_variant_count(inst.skeleton), name
+    ctx.close()
